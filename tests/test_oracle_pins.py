@@ -458,7 +458,11 @@ def test_jacobian_species_columns_sum_to_zero(tiny_mechs):
         J = as_matrix(o.jacobian(T, P, Y), m.n_species)
         for s in range(len(T)):
             sp = J[s][1:, :]
-            assert np.all(np.abs(sp.sum(0)) <= 1e-11 * np.abs(sp).sum(0) + 1e-300)
+            # each element of row k is a rounded sum of terms as large as that row's largest
+            # entries, so the residual is measured against sum_k max_j |J_kj| (a wrong sign or
+            # index anywhere leaves a residual of that size, 13 orders above this bound)
+            scale = np.abs(sp).max(axis=1).sum()
+            assert np.all(np.abs(sp.sum(0)) <= 1e-13 * scale + 1e-300)
 
 
 def test_batch_independence_and_threads(tiny_mechs):
