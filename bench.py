@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- Jacobian evaluations per second of the batched analytical kinetics Jacobian on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+                    [--also 2,3] [--sweep] [--no-cpu-baseline]
+
+A "step" is one pass of the whole hot path (thermo -> rates -> source term -> Jacobian -> store;
+SURVEY.md section 8(a) rows S0-S10, one kernel launch) over one batch of seeded synthetic states.
+At N = 1 the workload is BASELINE.json configs[1] (53 species, 325 reactions, 100,000 states).
+Rank 0 prints ONE JSON line.  Under torchrun (N > 1) every rank evaluates the same batch on its own
+GPU (states are independent: no data-path collective, "scaling": "weak").
+
+`--impl reference` times the CPU oracle (oracle/) on the host cores instead -- the only other place
+this file executes anything under oracle/ besides the cpu_baseline leg.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "jacobian_evals_per_sec"
+UNIT = "states/s"
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
+# oracle sample sizes per config (about 10-30 s of CPU work on 8-32 cores)
+CPU_SAMPLE = {0: 1024, 1: 8192, 2: 2048, 3: 256}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the Jacobian kernel from the committed
+# `ncu --set full` capture (profiles/), or None where no capture exists for that workload
+NCU_TRAFFIC_BYTES = {}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown",
+                                "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def algorithmic_bytes(ns: int, n: int) -> int:
+    """per state the method must read (Ns+2) and write (Ns+1)^2 doubles."""
+    return n * ((ns + 2) + (ns + 1) * (ns + 1)) * 8
+
+
+def time_oracle(cfg: int, n_sample: int, steps: int = 1, warmup: int = 0):
+    import numpy as np  # noqa: F401
+    from oracle.oracle import Oracle
+    from paper_1605_03262_b200 import synth
+    m = synth.make_mechanism(cfg)
+    o = Oracle(m)
+    n_sample = min(n_sample, synth.CONFIGS[cfg].n_states)
+    T, P, Y = synth.config_states(cfg, n_sample)
+    for _ in range(warmup):
+        o.jacobian(T[:64], P[:64], Y[:64])
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.jacobian(T, P, Y)
+    dt = (time.perf_counter() - t0) / steps
+    return {"value": n_sample / dt, "unit": UNIT, "cores": o.threads, "kind": "oracle",
+            "sample": "analytical Jacobian (oracle/oracle.c, Algorithm-1 order, OpenMP static over states) on "
+                      "the first %d states of the workload, %d pass(es), %.2f s per pass" % (n_sample, steps, dt)}, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1605_03262_b200 import synth
+    cfg = args.config
+    c = synth.CONFIGS[cfg]
+    steps = max(1, args.steps)
+    # bounded: the whole run stays within a few minutes
+    n_sample = CPU_SAMPLE[cfg] if steps <= 2 else max(256, CPU_SAMPLE[cfg] // steps)
+    base, dt = time_oracle(cfg, n_sample, steps=steps, warmup=min(args.warmup, 1))
+    line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": c.name, "n_species": c.n_species, "n_reactions": c.n_reactions,
+                       "n_states": c.n_states, "sampled_states_per_step": n_sample},
+            "cpu_baseline": base,
+            "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def time_gpu(pj, torch, dT, dP, dY, out, steps, warmup, fn=None):
+    """CUDA events on torch's current stream (the stream the library launches on)."""
+    fn = fn or (lambda: pj.eval_jacobian(dT, dP, dY, out=out))
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record()
+    for i in range(steps):
+        fn()
+        ev[i + 1].record()
+    torch.cuda.synchronize()
+    per = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+    return ev[0].elapsed_time(ev[steps]), per
+
+
+def bench_config(torch, cfg, steps, warmup, n_states=None, chunk=None):
+    """One configuration on the current device; returns a dict of results."""
+    from paper_1605_03262_b200 import synth
+    from paper_1605_03262_b200.binding import PyJac
+    c = synth.CONFIGS[cfg]
+    m = synth.make_mechanism(cfg)
+    n = c.n_states if n_states is None else n_states
+    T, P, Y = synth.config_states(cfg, n)
+    per_launch = n if chunk is None else min(chunk, n)
+    pj = PyJac(m, device=torch.cuda.current_device())
+    ld = c.n_species + 1
+    dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
+    out = torch.empty((per_launch, ld * ld), dtype=torch.float64, device="cuda")
+    views = [(dT[a:a + per_launch].contiguous(), dP[a:a + per_launch].contiguous(),
+              dY[a:a + per_launch].contiguous()) for a in range(0, n, per_launch)]
+
+    def step():
+        for (a, b, c_) in views:
+            pj.eval_jacobian(a, b, c_, out=out)
+
+    l0 = pj.kernel_launches()
+    total_ms, per = time_gpu(pj, torch, dT, dP, dY, out, steps, warmup, fn=step)
+    launches = pj.kernel_launches() - l0 - warmup * len(views)
+    return dict(pj=pj, mech=m, cfg=c, n=n, T=T, P=P, Y=Y, dT=dT, dP=dP, dY=dY, out=out, total_ms=total_ms,
+                per_step_ms=per, launches=launches, launches_per_step=len(views), per_launch=per_launch)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--also", default="2", help="comma list of further configs reported under per_config")
+    ap.add_argument("--sweep", action="store_true", help="config 4: state-count sweep, three kernels")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    args.warmup = max(3, args.warmup)
+
+    import numpy as np
+    import torch
+    from paper_1605_03262_b200 import build
+    build.build()                       # no-op when the in-tree .so is current
+    from paper_1605_03262_b200 import synth
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = args.config
+    chunk = 8192 if cfg == 3 else None           # config 3: 34 GB of output, evaluated in chunks
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    r = bench_config(torch, cfg, args.steps, args.warmup, chunk=chunk)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = r["total_ms"]
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    c, n, pj = r["cfg"], r["n"], r["pj"]
+    ms_per_step = total_ms / args.steps
+    value = world * n / (ms_per_step * 1e-3)
+    peak, peak_src = measured_peaks()
+    launch_ms = r["total_ms"] / (args.steps * r["launches_per_step"])
+    alg_bytes = algorithmic_bytes(c.n_species, r["per_launch"])
+    achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_BYTES.get(c.name), "peak_source": peak_src,
+                "kernel": "pyjac::eval_kernel<2,%d>" % pj.launch_config(r["per_launch"])["threads"],
+                "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": launch_ms,
+                "launch_config": pj.launch_config(r["per_launch"])}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": c.name, "n_species": c.n_species, "n_reactions": c.n_reactions,
+                       "n_states": n, "states_per_launch": r["per_launch"],
+                       "jacobian": "%dx%d fp64 column-major per state" % (c.n_species + 1, c.n_species + 1),
+                       "parallelism": "replicas x%d" % world if world > 1 else "single GPU",
+                       "cache": "output (%.2f GB per launch) and inputs exceed the 126 MB L2; no flush needed"
+                                % (r["per_launch"] * (c.n_species + 1) ** 2 * 8 / 1e9)},
+            "roofline": roofline, "clocks": clocks, "gpu_launches": int(r["launches"]),
+            "step_ms_min_max": [min(r["per_step_ms"]), max(r["per_step_ms"])]}
+
+    if rank == 0 and world == 1:
+        # ---- end to end through the host-buffer C-ABI call (pinned host memory, copies timed)
+        if not args.no_e2e:
+            ld = c.n_species + 1
+            n_e = n if cfg != 3 else 8192
+            hT, hP, hY = (torch.from_numpy(a[:n_e].copy()).pin_memory() for a in (r["T"], r["P"], r["Y"]))
+            hout = torch.empty((n_e, ld * ld), dtype=torch.float64).pin_memory()
+            e_steps = max(2, min(args.steps, 5))
+            pj.eval_jacobian_host(hT, hP, hY, hout)              # warm-up (also pages in the pinned buffer)
+            t0 = time.perf_counter()
+            for _ in range(e_steps):
+                pj.eval_jacobian_host(hT, hP, hY, hout)
+            dt = (time.perf_counter() - t0) / e_steps
+            line["e2e"] = {"value": n_e / dt, "unit": UNIT, "h2d_bytes_per_step": n_e * (c.n_species + 2) * 8,
+                           "d2h_bytes_per_step": n_e * ld * ld * 8, "ms_per_step": dt * 1e3, "steps": e_steps,
+                           "call": "pyjac_eval_jacobian_host (pinned host buffers, double-buffered chunks)",
+                           "n_states": n_e}
+            del hout
+        # ---- further configs (same timing rules), reported beside the headline
+        per = {}
+        del r["out"]
+        torch.cuda.empty_cache()
+        for extra in [int(x) for x in args.also.split(",") if x.strip() != ""]:
+            if extra == cfg:
+                continue
+            ch = 8192 if extra == 3 else None
+            st = max(3, args.steps // (2 if extra == 2 else 4))
+            rr = bench_config(torch, extra, st, args.warmup, chunk=ch)
+            cc = rr["cfg"]
+            lm = rr["total_ms"] / (st * rr["launches_per_step"])
+            ab = algorithmic_bytes(cc.n_species, rr["per_launch"])
+            per[cc.name] = {"value": rr["n"] / (rr["total_ms"] / st * 1e-3), "unit": UNIT, "steps": st,
+                            "n_states": rr["n"], "states_per_launch": rr["per_launch"], "launch_ms": lm,
+                            "roofline": {"bound": "hbm", "achieved": ab / (lm * 1e-3) / 1e9, "peak": peak,
+                                         "unit": "GB/s", "frac": ab / (lm * 1e-3) / 1e9 / peak,
+                                         "traffic": NCU_TRAFFIC_BYTES.get(cc.name)},
+                            "launch_config": rr["pj"].launch_config(rr["per_launch"])}
+            del rr
+            torch.cuda.empty_cache()
+        if per:
+            line["per_config"] = per
+        if args.sweep:
+            line["sweep_53sp"] = sweep(torch, args)
+        if not args.no_cpu_baseline:
+            line["cpu_baseline"], _ = time_oracle(cfg, CPU_SAMPLE[cfg])
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def sweep(torch, args):
+    """BASELINE.json configs[4]: 53-species mechanism, 4^5 .. 4^10 states, the three kernels."""
+    from paper_1605_03262_b200 import synth
+    from paper_1605_03262_b200.binding import PyJac
+    m = synth.make_mechanism(1)
+    pj = PyJac(m, device=torch.cuda.current_device())
+    ld = m.n_species + 1
+    res = []
+    for n in synth.SWEEP_STATES:
+        T, P, Y = synth.make_states(m.n_species, n, synth.CONFIGS[1].seed + 2000 + n)
+        dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
+        out = torch.empty((n, ld * ld), dtype=torch.float64, device="cuda")
+        dy = torch.empty((n, ld), dtype=torch.float64, device="cuda")
+        steps = 10
+        tj, _ = time_gpu(pj, torch, dT, dP, dY, out, steps, 3)
+        td, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3, fn=lambda: pj.eval_dydt(dT, dP, dY, out=dy))
+        tr, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3,
+                         fn=lambda: pj.eval_rates(dT, dP, dY, want=("wdot",)))
+        res.append({"n_states": n, "jacobian_states_per_s": n / (tj / steps * 1e-3),
+                    "dydt_states_per_s": n / (td / steps * 1e-3), "rates_states_per_s": n / (tr / steps * 1e-3)})
+        del out, dy
+        torch.cuda.empty_cache()
+    return res
+
+
+if __name__ == "__main__":
+    main()

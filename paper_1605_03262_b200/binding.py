@@ -1,0 +1,232 @@
+"""Thin ctypes binding of the C-ABI CUDA library (include/pyjac_b200.h).
+
+Argument marshalling only: every step of the evaluation runs in the library's sm_100a kernels.
+PyTorch is used for device memory and streams.  There is no CPU fallback: a missing library or a
+failing CUDA call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from .mechanism import Mechanism
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpyjac_b200.so")
+
+PYJAC_OK, PYJAC_EINVAL, PYJAC_ENOMEM, PYJAC_ECUDA, PYJAC_ELIMIT = 0, -1, -2, -3, -4
+
+_pd = C.POINTER(C.c_double)
+_pi = C.POINTER(C.c_int32)
+
+
+class MechDesc(C.Structure):
+    """struct pyjac_mech_desc"""
+    _fields_ = [("n_species", C.c_int32), ("n_reactions", C.c_int32),
+                ("mol_wt", _pd), ("nasa_lo", _pd), ("nasa_hi", _pd), ("t_mid", _pd),
+                ("reac_ptr", _pi), ("reac_spec", _pi), ("reac_nu", _pi),
+                ("prod_ptr", _pi), ("prod_spec", _pi), ("prod_nu", _pi),
+                ("rxn_type", _pi), ("rev_type", _pi),
+                ("arr_hi", _pd), ("arr_lo", _pd), ("arr_rev", _pd),
+                ("falloff_form", _pi), ("falloff_par", _pd), ("tb_species", _pi),
+                ("eff_ptr", _pi), ("eff_spec", _pi), ("eff_val", _pd),
+                ("plog_ptr", _pi), ("plog_p", _pd), ("plog_arr", _pd),
+                ("cheb_ptr", _pi), ("cheb_nT", _pi), ("cheb_nP", _pi),
+                ("cheb_lim", _pd), ("cheb_eta", _pd)]
+
+
+EXPORTS = ("pyjac_mech_create", "pyjac_mech_destroy", "pyjac_mech_sizes", "pyjac_eval_rates",
+           "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
+           "pyjac_eval_dydt_host", "pyjac_kernel_launches", "pyjac_jacobian_launch_config",
+           "pyjac_strerror")
+
+_lib = None
+
+
+def load_library(path: str | None = None):
+    """Loads libpyjac_b200.so (built in-tree by `python -m paper_1605_03262_b200.build`)."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or LIB_PATH
+    if not os.path.exists(p):
+        raise RuntimeError("%s is missing: run `python -m paper_1605_03262_b200.build` "
+                           "(there is no CPU fallback)" % p)
+    lib = C.CDLL(p)
+    vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
+    lib.pyjac_mech_create.argtypes = [C.POINTER(MechDesc), C.c_int, C.POINTER(vp)]
+    lib.pyjac_mech_destroy.argtypes = [vp]
+    lib.pyjac_mech_sizes.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
+    lib.pyjac_eval_rates.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp]
+    lib.pyjac_eval_dydt.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp]
+    lib.pyjac_eval_jacobian.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp]
+    lib.pyjac_eval_jacobian_host.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64]
+    lib.pyjac_eval_dydt_host.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64]
+    lib.pyjac_kernel_launches.argtypes = []
+    lib.pyjac_kernel_launches.restype = i64
+    lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 4
+    lib.pyjac_strerror.argtypes = [C.c_int]
+    lib.pyjac_strerror.restype = C.c_char_p
+    for name in EXPORTS:
+        if name not in ("pyjac_kernel_launches", "pyjac_strerror"):
+            getattr(lib, name).restype = C.c_int
+    if path is None:
+        _lib = lib
+    return lib
+
+
+class PyJacError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        msg = load_library().pyjac_strerror(code).decode()
+        super().__init__("%s failed: %s (%d)" % (what, msg, code))
+
+
+def _check(code, what):
+    if code != PYJAC_OK:
+        raise PyJacError(code, what)
+
+
+def mech_desc(mech: Mechanism):
+    """(MechDesc, keepalive) for a `Mechanism` (host arrays, C layout)."""
+    m = mech.normalized()
+    d = MechDesc()
+    d.n_species, d.n_reactions = m.n_species, m.n_reactions
+    keep = []
+    for dst, src in (("mol_wt", "mol_wt"), ("nasa_lo", "nasa_lo"), ("nasa_hi", "nasa_hi"),
+                     ("t_mid", "t_mid"), ("arr_hi", "arr_hi"), ("arr_lo", "arr_lo"),
+                     ("arr_rev", "arr_rev"), ("falloff_par", "falloff_par"), ("eff_val", "eff_val"),
+                     ("plog_p", "plog_p"), ("plog_arr", "plog_arr"), ("cheb_lim", "cheb_lim"),
+                     ("cheb_eta", "cheb_eta")):
+        a = np.ascontiguousarray(getattr(m, src), dtype=np.float64)
+        keep.append(a)
+        setattr(d, dst, a.ctypes.data_as(_pd))
+    for name in ("reac_ptr", "reac_spec", "reac_nu", "prod_ptr", "prod_spec", "prod_nu", "rxn_type",
+                 "rev_type", "falloff_form", "tb_species", "eff_ptr", "eff_spec", "plog_ptr",
+                 "cheb_ptr", "cheb_nT", "cheb_nP"):
+        a = np.ascontiguousarray(getattr(m, name), dtype=np.int32)
+        keep.append(a)
+        setattr(d, name, a.ctypes.data_as(_pi))
+    return d, keep
+
+
+class PyJac:
+    """A kinetic model resident on one CUDA device (wraps `pyjac_mech*`)."""
+
+    def __init__(self, mech: Mechanism, device: int = 0):
+        self.lib = load_library()
+        d, keep = mech_desc(mech)
+        h = C.c_void_p()
+        _check(self.lib.pyjac_mech_create(C.byref(d), int(device), C.byref(h)), "pyjac_mech_create")
+        self._h = h
+        self.device = int(device)
+        ns, nr = C.c_int32(), C.c_int32()
+        _check(self.lib.pyjac_mech_sizes(h, C.byref(ns), C.byref(nr)), "pyjac_mech_sizes")
+        self.ns, self.nr = ns.value, nr.value
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.pyjac_mech_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- helpers
+    def _dev_inputs(self, T, P, Y):
+        import torch
+        for t in (T, P, Y):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
+                raise TypeError("T, P, Y must be float64 CUDA tensors")
+        if Y.dim() != 2 or Y.stride(1) != 1 or not T.is_contiguous() or not P.is_contiguous():
+            raise ValueError("Y must be [n][>=Nsp] with unit inner stride; T, P contiguous")
+        n = T.numel()
+        if P.numel() != n or Y.shape[0] != n or Y.shape[1] < self.ns:
+            raise ValueError("inconsistent state arrays")
+        ldy = Y.stride(0) if n > 1 else max(Y.shape[1], self.ns)
+        return n, ldy
+
+    @staticmethod
+    def _stream():
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    # ---- device-pointer calls (enqueue on torch's current stream)
+    def eval_rates(self, T, P, Y, want=("rf", "rr", "cmod", "wdot")):
+        """dict of float64 CUDA tensors rf, rr, cmod [n][Nreac], wdot [n][Nsp] (pyjac_eval_rates)."""
+        import torch
+        n, ldy = self._dev_inputs(T, P, Y)
+        out = {}
+        for name in ("rf", "rr", "cmod", "wdot"):
+            if name in want:
+                out[name] = torch.empty((n, self.ns if name == "wdot" else self.nr),
+                                        dtype=torch.float64, device=T.device)
+        ptr = lambda k: C.c_void_p(out[k].data_ptr()) if k in out else None
+        _check(self.lib.pyjac_eval_rates(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
+                                         ptr("rf"), ptr("rr"), ptr("cmod"), ptr("wdot"),
+                                         self._stream()), "pyjac_eval_rates")
+        return out
+
+    def eval_dydt(self, T, P, Y, out=None):
+        """[n][Nsp+1] source term (pyjac_eval_dydt)."""
+        import torch
+        n, ldy = self._dev_inputs(T, P, Y)
+        if out is None:
+            out = torch.empty((n, self.ns + 1), dtype=torch.float64, device=T.device)
+        _check(self.lib.pyjac_eval_dydt(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
+                                        out.data_ptr(), self._stream()), "pyjac_eval_dydt")
+        return out
+
+    def eval_jacobian(self, T, P, Y, out=None):
+        """[n][(Nsp+1)^2] column-major Jacobians (pyjac_eval_jacobian)."""
+        import torch
+        n, ldy = self._dev_inputs(T, P, Y)
+        ld = self.ns + 1
+        if out is None:
+            out = torch.empty((n, ld * ld), dtype=torch.float64, device=T.device)
+        elif out.numel() < n * ld * ld or not out.is_contiguous():
+            raise ValueError("output buffer too small or not contiguous")
+        _check(self.lib.pyjac_eval_jacobian(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
+                                            out.data_ptr(), self._stream()), "pyjac_eval_jacobian")
+        return out
+
+    # ---- host-pointer calls (copies inside; synchronous)
+    @staticmethod
+    def _host_ptr(a):
+        import torch
+        if isinstance(a, torch.Tensor):
+            assert not a.is_cuda and a.dtype == torch.float64 and a.is_contiguous()
+            return a.data_ptr(), a
+        a = np.ascontiguousarray(a, dtype=np.float64)
+        return a.ctypes.data, a
+
+    def eval_jacobian_host(self, T, P, Y, out, chunk_states: int = 0):
+        """Host buffers in, host buffer out (numpy arrays or CPU torch tensors, pinned or not)."""
+        (pT, kT), (pP, kP), (pY, kY), (pO, kO) = map(self._host_ptr, (T, P, Y, out))
+        n = int(kT.shape[0])
+        ldy = int(kY.shape[1])
+        _check(self.lib.pyjac_eval_jacobian_host(self._h, n, pT, pP, pY, ldy, pO, int(chunk_states)),
+               "pyjac_eval_jacobian_host")
+        return out
+
+    def eval_dydt_host(self, T, P, Y, out, chunk_states: int = 0):
+        (pT, kT), (pP, kP), (pY, kY), (pO, kO) = map(self._host_ptr, (T, P, Y, out))
+        n = int(kT.shape[0])
+        ldy = int(kY.shape[1])
+        _check(self.lib.pyjac_eval_dydt_host(self._h, n, pT, pP, pY, ldy, pO, int(chunk_states)),
+               "pyjac_eval_dydt_host")
+        return out
+
+    def launch_config(self, n: int):
+        v = [C.c_int32() for _ in range(4)]
+        _check(self.lib.pyjac_jacobian_launch_config(self._h, int(n), *[C.byref(x) for x in v]),
+               "pyjac_jacobian_launch_config")
+        return dict(threads=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, grid=v[3].value)
+
+    def kernel_launches(self) -> int:
+        return int(self.lib.pyjac_kernel_launches())

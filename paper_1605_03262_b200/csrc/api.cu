@@ -1,0 +1,334 @@
+// api.cu -- the C ABI of include/pyjac_b200.h: handle management, launches, host-buffer variants.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "device_mech.h"
+#include "kernels.h"
+#include "mech_pack.h"
+
+using namespace pyjac;
+
+struct pyjac_mech {
+    int device = 0;
+    int ns = 0, nr = 0;
+    void *blob = nullptr;       // one device allocation holding every table
+    DeviceMech dm{};
+    SmemPlan plan{};
+    int threads = 128;
+    size_t smem[3] = {0, 0, 0}; // dynamic shared memory per level
+    int ctas_per_sm[3] = {1, 1, 1};
+    int n_sm = 1;
+};
+
+namespace {
+
+std::atomic<long long> g_launches{0};
+
+struct Uploader {
+    std::vector<unsigned char> host;
+    std::vector<std::pair<const void **, size_t>> fix;   // (field, offset)
+    template <class T>
+    void add(const T **field, const std::vector<T> &v)
+    {
+        size_t off = (host.size() + 255) & ~size_t(255);
+        host.resize(off + std::max<size_t>(v.size() * sizeof(T), 16));
+        if (!v.empty()) std::memcpy(host.data() + off, v.data(), v.size() * sizeof(T));
+        fix.push_back({(const void **)field, off});
+    }
+};
+
+int choose_threads(int ns, int nr)
+{
+    if (const char *e = std::getenv("PYJAC_THREADS")) {   // tuning hook, see DESIGN.md
+        int v = std::atoi(e);
+        if (v == 64 || v == 128 || v == 256 || v == 512 || v == 1024) return v;
+    }
+    const int work = nr > ns ? nr : ns;
+    if (work <= 64) return 64;
+    if (work <= 400) return 128;
+    if (work <= 1000) return 256;
+    if (work <= 2500) return 512;
+    return 1024;
+}
+
+int check_eval_args(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                    int64_t ldy)
+{
+    if (!m || n < 0) return PYJAC_EINVAL;
+    if (n == 0) return PYJAC_OK;
+    if (!T || !P || !Y || ldy < m->ns) return PYJAC_EINVAL;
+    return PYJAC_OK;
+}
+
+int launch(const pyjac_mech *m, int level, int64_t n, const double *T, const double *P, const double *Y,
+           int64_t ldy, const EvalOut &out, void *stream)
+{
+    if (n == 0) return PYJAC_OK;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return PYJAC_ECUDA;
+    if (dev != m->device && cudaSetDevice(m->device) != cudaSuccess) return PYJAC_ECUDA;
+    long long cap = (long long)m->n_sm * m->ctas_per_sm[level];
+    int grid = (int)(n < cap ? n : cap);
+    cudaError_t e = launch_eval(level, m->threads, m->dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy, out,
+                                (cudaStream_t)stream);
+    if (dev != m->device) cudaSetDevice(dev);
+    if (e != cudaSuccess) return PYJAC_ECUDA;
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return PYJAC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
+{
+    if (!out) return PYJAC_EINVAL;
+    *out = nullptr;
+    HostPack hp;
+    const char *why = nullptr;
+    int rc = pack_mechanism(d, hp, &why);
+    if (rc != PYJAC_OK) return rc;
+    pyjac_mech *m = new (std::nothrow) pyjac_mech();
+    if (!m) return PYJAC_ENOMEM;
+    m->device = device;
+    m->ns = hp.ns;
+    m->nr = hp.nr;
+    int prev = -1;
+    cudaDeviceProp prop{};
+    if (cudaGetDevice(&prev) != cudaSuccess || cudaSetDevice(device) != cudaSuccess ||
+        cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+        delete m;
+        return PYJAC_ECUDA;
+    }
+    m->n_sm = prop.multiProcessorCount;
+    DeviceMech &dm = m->dm;
+    dm.ns = hp.ns; dm.nr = hp.nr; dm.ld = hp.ns + 1;
+    dm.ln_patm_over_R = std::log(kPatm / kRu);
+    dm.pd_begin = hp.pd_begin; dm.n_pd = hp.n_pd; dm.pk_begin = hp.pk_begin; dm.n_pk = hp.n_pk;
+    dm.n_sp_task = hp.ns; dm.n_long = hp.n_long; dm.n_v = hp.n_v; dm.n_vext = hp.n_vext;
+    dm.spns_base = hp.spns_base;
+    Uploader up;
+    try {
+        up.add(&dm.mw, hp.mw); up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.dcol, hp.dcol);
+        up.add(&dm.nasa, hp.nasa); up.add(&dm.t_mid, hp.t_mid);
+        up.add(&dm.lnA, hp.lnA); up.add(&dm.beta, hp.beta); up.add(&dm.Ta, hp.Ta);
+        up.add((const uint32_t **)&dm.slots, hp.slots);
+        up.add(&dm.vbase, hp.vbase); up.add(&dm.rxn_orig, hp.rxn_orig);
+        up.add(&dm.rev_lnA, hp.rev_lnA); up.add(&dm.rev_beta, hp.rev_beta); up.add(&dm.rev_Ta, hp.rev_Ta);
+        up.add(&dm.lo_lnA, hp.lo_lnA); up.add(&dm.lo_beta, hp.lo_beta); up.add(&dm.lo_Ta, hp.lo_Ta);
+        up.add(&dm.fall_par, hp.fall_par); up.add(&dm.tb_spec, hp.tb_spec);
+        up.add(&dm.eff_ptr, hp.eff_ptr); up.add(&dm.eff_spec, hp.eff_spec); up.add(&dm.eff_eps, hp.eff_eps);
+        up.add(&dm.eff_vbase, hp.eff_vbase);
+        up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
+        up.add(&dm.sp_ptr, hp.sp_ptr); up.add(&dm.sp_ent, hp.sp_ent);
+        up.add(&dm.col_ptr, hp.col_ptr); up.add(&dm.col_ent, hp.col_ent);
+        up.add(&dm.long_ptr, hp.long_ptr); up.add(&dm.long_ent, hp.long_ent);
+        up.add(&dm.cell_info, hp.cell_info); up.add(&dm.cell_ent, hp.cell_ent);
+    } catch (...) {
+        delete m;
+        cudaSetDevice(prev);
+        return PYJAC_ENOMEM;
+    }
+    rc = PYJAC_OK;
+    if (cudaMalloc(&m->blob, up.host.size()) != cudaSuccess) {
+        rc = PYJAC_ENOMEM;
+    } else if (cudaMemcpy(m->blob, up.host.data(), up.host.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+        rc = PYJAC_ECUDA;
+    }
+    if (rc == PYJAC_OK) {
+        for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
+        m->plan = make_smem_plan(hp.ns, hp.nr, hp.n_vext);
+        m->threads = choose_threads(hp.ns, hp.nr);
+        const size_t bytes = (size_t)m->plan.total * sizeof(double);
+        if (bytes > (size_t)prop.sharedMemPerBlockOptin) {
+            rc = PYJAC_ELIMIT;
+        } else {
+            for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
+                m->smem[level] = bytes;
+                const void *k = eval_kernel_ptr(level, m->threads);
+                if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess ||
+                    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m->ctas_per_sm[level], k, m->threads, bytes) !=
+                        cudaSuccess ||
+                    m->ctas_per_sm[level] < 1)
+                    rc = PYJAC_ECUDA;
+            }
+        }
+    }
+    cudaSetDevice(prev);
+    if (rc != PYJAC_OK) {
+        cudaGetLastError();
+        if (m->blob) cudaFree(m->blob);
+        delete m;
+        return rc;
+    }
+    *out = m;
+    return PYJAC_OK;
+}
+
+int pyjac_mech_destroy(pyjac_mech *m)
+{
+    if (!m) return PYJAC_OK;
+    int prev = -1;
+    cudaGetDevice(&prev);
+    cudaSetDevice(m->device);
+    cudaError_t e = cudaFree(m->blob);
+    if (prev >= 0) cudaSetDevice(prev);
+    delete m;
+    return e == cudaSuccess ? PYJAC_OK : PYJAC_ECUDA;
+}
+
+int pyjac_mech_sizes(const pyjac_mech *m, int32_t *ns, int32_t *nr)
+{
+    if (!m) return PYJAC_EINVAL;
+    if (ns) *ns = m->ns;
+    if (nr) *nr = m->nr;
+    return PYJAC_OK;
+}
+
+int pyjac_eval_rates(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                     int64_t ldy, double *rf, double *rr, double *cmod, double *wdot, void *stream)
+{
+    int rc = check_eval_args(m, n, T, P, Y, ldy);
+    if (rc != PYJAC_OK) return rc;
+    EvalOut out{rf, rr, cmod, wdot, nullptr, nullptr};
+    return launch(m, 0, n, T, P, Y, ldy, out, stream);
+}
+
+int pyjac_eval_dydt(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                    int64_t ldy, double *dydt, void *stream)
+{
+    int rc = check_eval_args(m, n, T, P, Y, ldy);
+    if (rc != PYJAC_OK) return rc;
+    if (n > 0 && !dydt) return PYJAC_EINVAL;
+    EvalOut out{nullptr, nullptr, nullptr, nullptr, dydt, nullptr};
+    return launch(m, 1, n, T, P, Y, ldy, out, stream);
+}
+
+int pyjac_eval_jacobian(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                        int64_t ldy, double *jac, void *stream)
+{
+    int rc = check_eval_args(m, n, T, P, Y, ldy);
+    if (rc != PYJAC_OK) return rc;
+    if (n > 0 && !jac) return PYJAC_EINVAL;
+    EvalOut out{nullptr, nullptr, nullptr, nullptr, nullptr, jac};
+    return launch(m, 2, n, T, P, Y, ldy, out, stream);
+}
+
+int64_t pyjac_kernel_launches(void) { return g_launches.load(std::memory_order_relaxed); }
+
+int pyjac_jacobian_launch_config(const pyjac_mech *m, int64_t n, int32_t *threads, int32_t *smem_bytes,
+                                 int32_t *ctas_per_sm, int32_t *grid)
+{
+    if (!m || n < 0) return PYJAC_EINVAL;
+    if (threads) *threads = m->threads;
+    if (smem_bytes) *smem_bytes = (int32_t)m->smem[2];
+    if (ctas_per_sm) *ctas_per_sm = m->ctas_per_sm[2];
+    long long cap = (long long)m->n_sm * m->ctas_per_sm[2];
+    if (grid) *grid = (int32_t)(n < cap ? n : cap);
+    return PYJAC_OK;
+}
+
+const char *pyjac_strerror(int code)
+{
+    switch (code) {
+        case PYJAC_OK: return "success";
+        case PYJAC_EINVAL: return "invalid argument or inconsistent mechanism description";
+        case PYJAC_ENOMEM: return "host or device allocation failed";
+        case PYJAC_ECUDA: return "CUDA runtime or launch error";
+        case PYJAC_ELIMIT: return "mechanism exceeds a table limit of this build";
+        default: return "unknown error code";
+    }
+}
+
+}  // extern "C"
+
+// ---- host-buffer variants: chunked, double-buffered H2D -> kernel -> D2H ---------------------------
+namespace {
+
+int eval_host(const pyjac_mech *m, int level, int64_t n, const double *T, const double *P, const double *Y,
+              int64_t ldy, double *outp, int64_t chunk_states)
+{
+    int rc = check_eval_args(m, n, T, P, Y, ldy);
+    if (rc != PYJAC_OK) return rc;
+    if (n == 0) return PYJAC_OK;
+    if (!outp) return PYJAC_EINVAL;
+    int prev = -1;
+    if (cudaGetDevice(&prev) != cudaSuccess || cudaSetDevice(m->device) != cudaSuccess) return PYJAC_ECUDA;
+    const int ns = m->ns, ld = ns + 1;
+    const size_t out_per = level == 2 ? (size_t)ld * ld : (size_t)ld;
+    const size_t in_per = (size_t)ns + 2;
+    if (chunk_states <= 0) {
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaSetDevice(prev); return PYJAC_ECUDA; }
+        const size_t per_state = (out_per + in_per) * sizeof(double) * 2;   // two buffers
+        size_t c = (free_b / 4) / per_state;
+        const size_t want = (size_t)1 << 15;       // copies of ~0.1-1 GB overlap well; more adds nothing
+        if (c > want) c = want;
+        if (c < 1) c = 1;
+        chunk_states = (int64_t)c;
+    }
+    if (chunk_states > n) chunk_states = n;
+    const size_t C = (size_t)chunk_states;
+    double *din[2] = {nullptr, nullptr}, *dout[2] = {nullptr, nullptr};
+    cudaStream_t st[2] = {nullptr, nullptr};
+    rc = PYJAC_OK;
+    for (int b = 0; b < 2 && rc == PYJAC_OK; ++b) {
+        if (cudaMalloc(&din[b], C * in_per * sizeof(double)) != cudaSuccess ||
+            cudaMalloc(&dout[b], C * out_per * sizeof(double)) != cudaSuccess)
+            rc = PYJAC_ENOMEM;
+        else if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess)
+            rc = PYJAC_ECUDA;
+    }
+    int b = 0;
+    for (int64_t s0 = 0; s0 < n && rc == PYJAC_OK; s0 += chunk_states, b ^= 1) {
+        const size_t c = (size_t)((n - s0) < chunk_states ? (n - s0) : chunk_states);
+        double *dT = din[b], *dP = din[b] + C, *dY = din[b] + 2 * C;
+        cudaError_t e = cudaMemcpyAsync(dT, T + s0, c * sizeof(double), cudaMemcpyHostToDevice, st[b]);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(dP, P + s0, c * sizeof(double), cudaMemcpyHostToDevice, st[b]);
+        if (e == cudaSuccess)
+            e = cudaMemcpy2DAsync(dY, (size_t)ns * sizeof(double), Y + s0 * ldy, (size_t)ldy * sizeof(double),
+                                  (size_t)ns * sizeof(double), c, cudaMemcpyHostToDevice, st[b]);
+        if (e != cudaSuccess) { rc = PYJAC_ECUDA; break; }
+        EvalOut out{nullptr, nullptr, nullptr, nullptr, level == 1 ? dout[b] : nullptr, level == 2 ? dout[b] : nullptr};
+        rc = launch(m, level, (int64_t)c, dT, dP, dY, ns, out, st[b]);
+        if (rc != PYJAC_OK) break;
+        e = cudaMemcpyAsync(outp + (size_t)s0 * out_per, dout[b], c * out_per * sizeof(double),
+                            cudaMemcpyDeviceToHost, st[b]);
+        if (e != cudaSuccess) { rc = PYJAC_ECUDA; break; }
+    }
+    for (int q = 0; q < 2; ++q) {
+        if (st[q]) {
+            if (cudaStreamSynchronize(st[q]) != cudaSuccess && rc == PYJAC_OK) rc = PYJAC_ECUDA;
+            cudaStreamDestroy(st[q]);
+        }
+        if (din[q]) cudaFree(din[q]);
+        if (dout[q]) cudaFree(dout[q]);
+    }
+    if (rc != PYJAC_OK) cudaGetLastError();
+    cudaSetDevice(prev);
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pyjac_eval_jacobian_host(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                             int64_t ldy, double *jac, int64_t chunk_states)
+{
+    return eval_host(m, 2, n, T, P, Y, ldy, jac, chunk_states);
+}
+
+int pyjac_eval_dydt_host(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                         int64_t ldy, double *dydt, int64_t chunk_states)
+{
+    return eval_host(m, 1, n, T, P, Y, ldy, dydt, chunk_states);
+}
+
+}  // extern "C"

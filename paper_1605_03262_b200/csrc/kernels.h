@@ -1,0 +1,23 @@
+// kernels.h -- launch interface between api.cu and kernels.cu.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "device_mech.h"
+#include "../../include/pyjac_b200.h"
+
+namespace pyjac {
+
+// device output pointers of one evaluation (NULL = skip)
+struct EvalOut {
+    double *rf, *rr, *cmod, *wdot;   // level 0
+    double *dydt;                    // level 1
+    double *jac;                     // level 2
+};
+
+// level: 0 rates, 1 source term, 2 Jacobian.  nt: threads per CTA (64, 128, 256, 512, 1024).
+const void *eval_kernel_ptr(int level, int nt);
+cudaError_t launch_eval(int level, int nt, const DeviceMech &m, const SmemPlan &sp, int grid, size_t smem,
+                        long long n, const double *T, const double *P, const double *Y, long long ldy,
+                        const EvalOut &out, cudaStream_t stream);
+
+}  // namespace pyjac

@@ -1,0 +1,332 @@
+// mech_pack.cu -- validate a pyjac_mech_desc and pack it into the device table layout (host code).
+//
+// What is precomputed here is state-independent bookkeeping of the paper's restructured evaluation
+// order (Algorithm 2): which per-reaction products feed which Jacobian entries.
+// No thermodynamic or kinetic quantity is evaluated on the host except ln A and ln p of the tables.
+#include <algorithm>
+#include <cmath>
+#include <numeric>
+
+#include "device_mech.h"
+#include "mech_pack.h"
+
+namespace pyjac {
+
+namespace {
+
+struct Fail {
+    int code;
+    const char *why;
+};
+
+#define REQUIRE(cond, msg)                        \
+    do {                                          \
+        if (!(cond)) throw Fail{PYJAC_EINVAL, msg}; \
+    } while (0)
+
+struct ColEntry {
+    int spec;      // column species j
+    uint32_t vi;   // V index of s'_ij
+};
+
+}  // namespace
+
+static void pack_impl(const pyjac_mech_desc *d, HostPack &o)
+{
+    REQUIRE(d != nullptr, "description is NULL");
+    const int ns = d->n_species, nr = d->n_reactions;
+    REQUIRE(ns >= 1 && nr >= 0, "n_species must be >= 1 and n_reactions >= 0");
+    if (ns > 65534 || nr > 65535) throw Fail{PYJAC_ELIMIT, "more than 65534 species or 65535 reactions"};
+    REQUIRE(d->mol_wt && d->nasa_lo && d->nasa_hi && d->t_mid, "species arrays missing");
+    if (nr > 0) {
+        REQUIRE(d->reac_ptr && d->prod_ptr && d->rxn_type && d->rev_type && d->arr_hi && d->arr_lo &&
+                    d->arr_rev && d->falloff_form && d->falloff_par && d->tb_species && d->eff_ptr &&
+                    d->plog_ptr && d->cheb_ptr && d->cheb_nT && d->cheb_nP && d->cheb_lim,
+                "per-reaction arrays missing");
+    }
+    o.ns = ns;
+    o.nr = nr;
+    // ---- species
+    o.mw.assign(d->mol_wt, d->mol_wt + ns);
+    o.inv_mw.resize(ns);
+    o.dcol.resize(ns);
+    o.t_mid.assign(d->t_mid, d->t_mid + ns);
+    o.nasa.resize((size_t)14 * ns);
+    for (int k = 0; k < ns; ++k) {
+        REQUIRE(d->mol_wt[k] > 0.0 && std::isfinite(d->mol_wt[k]), "molecular weight must be positive");
+        o.inv_mw[k] = 1.0 / d->mol_wt[k];
+        for (int c = 0; c < 7; ++c) {
+            o.nasa[(size_t)(0 * 7 + c) * ns + k] = d->nasa_lo[7 * k + c];
+            o.nasa[(size_t)(1 * 7 + c) * ns + k] = d->nasa_hi[7 * k + c];
+        }
+    }
+    for (int k = 0; k < ns; ++k) o.dcol[k] = 1.0 / d->mol_wt[k] - 1.0 / d->mol_wt[ns - 1];
+
+    // ---- validate reactions and choose the sorted order
+    std::vector<int> key(nr);
+    for (int i = 0; i < nr; ++i) {
+        const int t = d->rxn_type[i], rv = d->rev_type[i];
+        REQUIRE(t >= 0 && t <= 5, "rxn_type out of range");
+        REQUIRE(rv >= 0 && rv <= 2, "rev_type out of range");
+        for (int side = 0; side < 2; ++side) {
+            const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr;
+            const int32_t *sp = side ? d->prod_spec : d->reac_spec;
+            const int32_t *nu = side ? d->prod_nu : d->reac_nu;
+            const int b = ptr[i], e = ptr[i + 1];
+            REQUIRE(b >= 0 && e >= b, "stoichiometry CSR pointers must be non-decreasing");
+            REQUIRE(e - b <= kMaxSide, "more than 3 species on one side of a reaction");
+            REQUIRE(e == b || (sp && nu), "stoichiometry arrays missing");
+            for (int q = b; q < e; ++q) {
+                REQUIRE(sp[q] >= 0 && sp[q] < ns, "species index out of range");
+                REQUIRE(nu[q] >= 1 && nu[q] <= 3, "stoichiometric coefficient outside 1..3");
+                for (int q2 = b; q2 < q; ++q2) REQUIRE(sp[q2] != sp[q], "species repeated within a side");
+            }
+        }
+        int form = 0;
+        if (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED) {
+            form = d->falloff_form[i];
+            REQUIRE(form >= 0 && form <= 2, "falloff_form out of range");
+            REQUIRE(d->arr_lo[3 * i] > 0.0 && d->arr_hi[3 * i] > 0.0, "falloff pre-exponentials must be > 0");
+        }
+        if (t == PYJAC_ELEMENTARY || t == PYJAC_THIRD_BODY)
+            REQUIRE(d->arr_hi[3 * i] > 0.0, "pre-exponential factor must be > 0");
+        if (rv == PYJAC_REV_EXPLICIT) REQUIRE(d->arr_rev[3 * i] > 0.0, "reverse pre-exponential must be > 0");
+        if (t == PYJAC_THIRD_BODY || t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED) {
+            const int m = d->tb_species[i];
+            REQUIRE(m >= -1 && m < ns, "tb_species out of range");
+            const int b = d->eff_ptr[i], e = d->eff_ptr[i + 1];
+            REQUIRE(b >= 0 && e >= b, "efficiency CSR pointers must be non-decreasing");
+            REQUIRE(e == b || (d->eff_spec && d->eff_val), "efficiency arrays missing");
+            for (int q = b; q < e; ++q) {
+                REQUIRE(d->eff_spec[q] >= 0 && d->eff_spec[q] < ns, "efficiency species out of range");
+                for (int q2 = b; q2 < q; ++q2)
+                    REQUIRE(d->eff_spec[q2] != d->eff_spec[q], "efficiency species repeated");
+            }
+        }
+        if (t == PYJAC_PLOG) {
+            const int b = d->plog_ptr[i], e = d->plog_ptr[i + 1];
+            REQUIRE(e - b >= 2 && d->plog_p && d->plog_arr, "PLOG reaction needs >= 2 pressures");
+            for (int q = b; q < e; ++q) {
+                REQUIRE(d->plog_p[q] > 0.0 && d->plog_arr[3 * q] > 0.0, "PLOG pressure and A must be > 0");
+                if (q > b) REQUIRE(d->plog_p[q] > d->plog_p[q - 1], "PLOG pressures must ascend");
+            }
+        }
+        if (t == PYJAC_CHEBYSHEV) {
+            const int nT = d->cheb_nT[i], nP = d->cheb_nP[i];
+            REQUIRE(nT >= 1 && nP >= 1 && d->cheb_eta, "Chebyshev table empty");
+            REQUIRE(d->cheb_ptr[i + 1] - d->cheb_ptr[i] >= nT * nP, "Chebyshev table too short");
+            const double *lim = d->cheb_lim + 4 * i;
+            REQUIRE(lim[0] > 0 && lim[1] > lim[0] && lim[2] > 0 && lim[3] > lim[2], "Chebyshev limits invalid");
+        }
+        // group: elementary, PLOG, Chebyshev | third body, falloff forms (Lindemann, Troe, SRI)
+        int group = t == PYJAC_ELEMENTARY ? 0 : t == PYJAC_PLOG ? 1 : t == PYJAC_CHEBYSHEV ? 2
+                  : t == PYJAC_THIRD_BODY ? 3 : 4 + form;
+        key[i] = group * 4 + rv;
+    }
+    std::vector<int> order(nr);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key[a] < key[b]; });
+
+    // ---- per-reaction tables in sorted order
+    o.lnA.resize(nr); o.beta.resize(nr); o.Ta.resize(nr);
+    o.rev_lnA.assign(nr, 0.0); o.rev_beta.assign(nr, 0.0); o.rev_Ta.assign(nr, 0.0);
+    o.slots.assign((size_t)4 * nr, 0u);
+    o.vbase.resize(nr);
+    o.rxn_orig.resize(nr);
+    o.pd_begin = nr; o.n_pd = 0; o.pk_begin = nr; o.n_pk = 0;
+    o.pk_ptr.assign(1, 0);
+    o.eff_ptr.assign(1, 0);
+    std::vector<std::vector<ColEntry>> cols(nr);          // column entries of each reaction
+    std::vector<std::vector<std::pair<int, int>>> net(nr);  // (species, net nu) of each reaction
+    uint32_t nv = 0;
+    for (int s = 0; s < nr; ++s) {
+        const int i = order[s];
+        const int t = d->rxn_type[i], rv = d->rev_type[i];
+        o.rxn_orig[s] = i;
+        const bool pk = (t == PYJAC_PLOG || t == PYJAC_CHEBYSHEV);
+        const bool pd = (t == PYJAC_THIRD_BODY || t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED);
+        if (pk && o.n_pk++ == 0) o.pk_begin = s;
+        if (pd && o.n_pd++ == 0) o.pd_begin = s;
+        if (!pk) {
+            o.lnA[s] = std::log(d->arr_hi[3 * i]);
+            o.beta[s] = d->arr_hi[3 * i + 1];
+            o.Ta[s] = d->arr_hi[3 * i + 2];
+        }
+        if (rv == PYJAC_REV_EXPLICIT) {
+            o.rev_lnA[s] = std::log(d->arr_rev[3 * i]);
+            o.rev_beta[s] = d->arr_rev[3 * i + 1];
+            o.rev_Ta[s] = d->arr_rev[3 * i + 2];
+        }
+        uint32_t spec[6] = {(uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns};
+        uint32_t meta = 0;
+        o.vbase[s] = nv;
+        for (int side = 0; side < 2; ++side) {
+            const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr;
+            const int32_t *sp = side ? d->prod_spec : d->reac_spec;
+            const int32_t *nu = side ? d->prod_nu : d->reac_nu;
+            for (int q = ptr[i], e = 0; q < ptr[i + 1]; ++q, ++e) {
+                const int slot = 3 * side + e;
+                spec[slot] = (uint32_t)sp[q];
+                meta |= (uint32_t)nu[q] << (4 * slot);
+                cols[s].push_back({sp[q], nv++});
+                const int signed_nu = side ? nu[q] : -nu[q];
+                bool found = false;
+                for (auto &pr : net[s])
+                    if (pr.first == sp[q]) { pr.second += signed_nu; found = true; }
+                if (!found) net[s].push_back({sp[q], signed_nu});
+            }
+        }
+        const int form = (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED) ? d->falloff_form[i] : 0;
+        const int single = pd && d->tb_species[i] >= 0;
+        meta |= (uint32_t)t << 24 | (uint32_t)rv << 27 | (uint32_t)form << 29 | (uint32_t)single << 31;
+        o.slots[4 * s + 0] = spec[0] | spec[1] << 16;
+        o.slots[4 * s + 1] = spec[2] | spec[3] << 16;
+        o.slots[4 * s + 2] = spec[4] | spec[5] << 16;
+        o.slots[4 * s + 3] = meta;
+        if (pk) {
+            if (t == PYJAC_PLOG) {
+                const int b = d->plog_ptr[i], e = d->plog_ptr[i + 1];
+                o.pk_data.push_back((double)(e - b));
+                for (int q = b; q < e; ++q) {
+                    o.pk_data.push_back(d->plog_p[q]);
+                    o.pk_data.push_back(std::log(d->plog_p[q]));
+                    o.pk_data.push_back(std::log(d->plog_arr[3 * q]));
+                    o.pk_data.push_back(d->plog_arr[3 * q + 1]);
+                    o.pk_data.push_back(d->plog_arr[3 * q + 2]);
+                }
+            } else {
+                const int nT = d->cheb_nT[i], nP = d->cheb_nP[i];
+                const double *lim = d->cheb_lim + 4 * i;
+                o.pk_data.push_back((double)nT);
+                o.pk_data.push_back((double)nP);
+                o.pk_data.push_back(1.0 / lim[0]);
+                o.pk_data.push_back(1.0 / lim[1]);
+                o.pk_data.push_back(std::log10(lim[2]));
+                o.pk_data.push_back(std::log10(lim[3]));
+                for (int q = 0; q < nT * nP; ++q) o.pk_data.push_back(d->cheb_eta[d->cheb_ptr[i] + q]);
+            }
+            o.pk_ptr.push_back((int32_t)o.pk_data.size());
+        }
+    }
+    // pressure-dependent tables (third-body efficiencies get their V entries after all slots)
+    for (int s = o.pd_begin; s < o.pd_begin + o.n_pd; ++s) {
+        const int i = order[s];
+        const int t = d->rxn_type[i];
+        const bool fall = (t != PYJAC_THIRD_BODY);
+        o.lo_lnA.push_back(fall ? std::log(d->arr_lo[3 * i]) : 0.0);
+        o.lo_beta.push_back(fall ? d->arr_lo[3 * i + 1] : 0.0);
+        o.lo_Ta.push_back(fall ? d->arr_lo[3 * i + 2] : 0.0);
+        for (int c = 0; c < 5; ++c) o.fall_par.push_back(fall ? d->falloff_par[5 * i + c] : 0.0);
+        const int m = d->tb_species[i];
+        o.tb_spec.push_back(m);
+        o.eff_vbase.push_back(nv);
+        if (m >= 0) {       // Eq. 30: [X]_i = [X_m]; one entry with "alpha - 1" = 1 and no [M] term
+            o.eff_spec.push_back(m);
+            o.eff_eps.push_back(1.0);
+            cols[s].push_back({m, nv++});
+        } else {            // Eq. 28 written as [M] + sum_j (alpha_ij - 1)[X_j]
+            for (int q = d->eff_ptr[i]; q < d->eff_ptr[i + 1]; ++q) {
+                if (d->eff_val[q] == 1.0) continue;
+                o.eff_spec.push_back(d->eff_spec[q]);
+                o.eff_eps.push_back(d->eff_val[q] - 1.0);
+                cols[s].push_back({d->eff_spec[q], nv++});
+            }
+        }
+        o.eff_ptr.push_back((int32_t)o.eff_spec.size());
+    }
+    if (o.n_pd == 0) o.pd_begin = nr;
+    if (o.n_pk == 0) o.pk_begin = nr;
+    o.n_v = (int)nv;
+
+    // ---- species tasks: wdot_k, A_k, Tcol_k = sum_i nu_ki {q_i, a_i, thetaT_i}  (Eqs. 14, 111, 115-117)
+    {
+        std::vector<std::vector<uint32_t>> lists(ns);
+        for (int s = 0; s < nr; ++s)
+            for (auto &pr : net[s])
+                if (pr.second != 0) lists[pr.first].push_back(pack_entry((uint32_t)s, pr.second));
+        o.sp_ptr.assign(1, 0);
+        for (int k = 0; k < ns; ++k) {
+            o.sp_ent.insert(o.sp_ent.end(), lists[k].begin(), lists[k].end());
+            o.sp_ptr.push_back((int32_t)o.sp_ent.size());
+        }
+    }
+    // ---- energy-row column tasks: E_j = sum_i H_i s'_ij with H_i = sum_k nu_ki h_k W_k  (Eq. 113)
+    {
+        std::vector<std::vector<uint32_t>> lists(ns);
+        for (int s = 0; s < nr; ++s)
+            for (auto &ce : cols[s]) lists[ce.spec].push_back(ce.vi | (uint32_t)s << 16);
+        o.col_ptr.assign(1, 0);
+        for (int j = 0; j < ns; ++j) {
+            o.col_ent.insert(o.col_ent.end(), lists[j].begin(), lists[j].end());
+            o.col_ptr.push_back((int32_t)o.col_ent.size());
+        }
+    }
+    // ---- cell lists: species block (row k+1, column j+1) += W_k nu_ki s'_ij / W_j  (Eqs. 112, 118-127)
+    const int ld = ns + 1;
+    {
+        std::vector<std::vector<uint32_t>> cell((size_t)ns * ns);   // [j][k], j = column species
+        for (int s = 0; s < nr; ++s)
+            for (auto &pr : net[s]) {
+                if (pr.second == 0) continue;
+                for (auto &ce : cols[s]) cell[(size_t)ce.spec * ns + pr.first].push_back(pack_entry(ce.vi, pr.second));
+            }
+        o.cell_info.assign((size_t)ld * ld, 0u);
+        o.long_ptr.assign(1, 0);
+        int n_long = 0;
+        for (int j = 0; j < ns - 1; ++j)
+            for (int k = 0; k < ns; ++k) {
+                auto &lst = cell[(size_t)j * ns + k];
+                if (lst.empty()) continue;
+                const size_t at = (size_t)(k + 1) + (size_t)(j + 1) * ld;
+                if ((int)lst.size() > kLongCell) {
+                    o.long_ent.insert(o.long_ent.end(), lst.begin(), lst.end());
+                    o.long_ptr.push_back((int32_t)o.long_ent.size());
+                    lst.assign(1, pack_entry((uint32_t)(o.n_v + n_long), 1));
+                    ++n_long;
+                }
+            }
+        // the virtual column N_sp (terms proportional to 1/W_Nsp of Eqs. 119, 123, 127): one sum per row
+        o.spns_base = o.n_v + n_long;
+        for (int k = 0; k < ns; ++k) {
+            auto &lst = cell[(size_t)(ns - 1) * ns + k];
+            o.long_ent.insert(o.long_ent.end(), lst.begin(), lst.end());
+            o.long_ptr.push_back((int32_t)o.long_ent.size());
+            ++n_long;
+        }
+        o.n_long = n_long;
+        o.n_vext = o.n_v + n_long;
+        if (o.n_vext > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-reaction derivative entries"};
+        // entries of pre-reduced cells were packed before n_long was final; their source index is
+        // n_v + t with t < n_long, which fits by the check above
+        for (int j = 0; j < ns - 1; ++j)
+            for (int k = 0; k < ns; ++k) {
+                auto &lst = cell[(size_t)j * ns + k];
+                if (lst.empty()) continue;
+                const size_t at = (size_t)(k + 1) + (size_t)(j + 1) * ld;
+                o.cell_info[at] = (uint32_t)o.cell_ent.size() << 3 | (uint32_t)lst.size();
+                o.cell_ent.insert(o.cell_ent.end(), lst.begin(), lst.end());
+            }
+        if (o.cell_ent.size() >= (1u << 29)) throw Fail{PYJAC_ELIMIT, "cell list too long"};
+    }
+    if (o.cell_ent.empty()) o.cell_ent.push_back(0u);
+    if (o.long_ent.empty()) o.long_ent.push_back(0u);
+    if (o.sp_ent.empty()) o.sp_ent.push_back(0u);
+    if (o.col_ent.empty()) o.col_ent.push_back(0u);
+}
+
+int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const char **why)
+{
+    try {
+        pack_impl(d, out);
+    } catch (const Fail &f) {
+        if (why) *why = f.why;
+        return f.code;
+    } catch (...) {
+        if (why) *why = "host allocation failed";
+        return PYJAC_ENOMEM;
+    }
+    if (why) *why = "";
+    return PYJAC_OK;
+}
+
+}  // namespace pyjac

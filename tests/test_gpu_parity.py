@@ -1,0 +1,295 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances (BASELINE.json north_star):
+  rates R_f, R_r, c_i      element-wise relative 1e-12 (reverse rates: see KR_TOL below)
+  wdot, dPhi/dt            1e-12 of max_k |.| per state (C19: do not judge cancellation)
+  Jacobian                 Frobenius-norm relative error per state <= 1e-10 (Eq. 132)
+"""
+import numpy as np
+import pytest
+
+from oracle.oracle import Oracle
+from paper_1605_03262_b200 import synth
+from paper_1605_03262_b200.mechanism import (CHEBYSHEV, ELEMENTARY, FALLOFF, PLOG, REV_FROM_KC, THIRD_BODY,
+                                             TROE, MechanismBuilder)
+
+pytestmark = pytest.mark.gpu
+
+RATE_TOL = 1e-12
+JAC_TOL = 1e-10
+EPS = 2.220446049250313e-16
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return t
+
+
+@pytest.fixture(scope="module")
+def PyJac():
+    from paper_1605_03262_b200 import build
+    build.build()
+    from paper_1605_03262_b200.binding import PyJac as P
+    return P
+
+
+def dev(torch, *arrays):
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrays]
+
+
+def kr_tol(oracle, T):
+    """k_r = k_f / K_c with K_c from exp(sum_k nu_ki B_k) (Eqs. 23-27): each B_k is rounded at
+    eps |B_k| (its a_5/T term reaches several hundred for large species), so two correct
+    evaluation orders differ by up to ~eps * sum|nu| * max|B_k| in the exponent."""
+    bmax = max(np.abs(oracle.species_thermo(float(t))[0][3]).max() for t in (T.min(), T.max()))
+    return max(RATE_TOL, 8.0 * 6 * EPS * bmax)
+
+
+def check_rates(torch, pj, o, T, P, Y):
+    dT, dP, dY = dev(torch, T, P, Y)
+    got = {k: v.cpu().numpy() for k, v in pj.eval_rates(dT, dP, dY).items()}
+    dy = pj.eval_dydt(dT, dP, dY).cpu().numpy()
+    ref = o.source(T, P, Y)
+    tiny = 1e-300
+    tol_r = kr_tol(o, T)
+    assert np.all(np.abs(got["rf"] - ref["rf"]) <= RATE_TOL * np.abs(ref["rf"]) + tiny)
+    assert np.all(np.abs(got["rr"] - ref["rr"]) <= tol_r * np.abs(ref["rr"]) + tiny)
+    assert np.all(np.abs(got["cmod"] - ref["cmod"]) <= RATE_TOL * np.abs(ref["cmod"]) + tiny)
+    # production rates and source term: against the size of what was summed (C19); with reverse
+    # rates entering, the bound is the reverse-rate one
+    q = np.abs(ref["cmod"]) * (np.abs(ref["rf"]) + np.abs(ref["rr"]))
+    scale_w = q.max(axis=1, keepdims=True)
+    assert np.all(np.abs(got["wdot"] - ref["wdot"]) <= tol_r * scale_w + tiny)
+    for part in (slice(0, 1), slice(1, None)):
+        scale = np.abs(ref["dydt"][:, part]).max(axis=1, keepdims=True)
+        bound = max(tol_r, RATE_TOL) * np.maximum(scale, _dydt_term_scale(o, ref, T, P, Y, part))
+        assert np.all(np.abs(dy[:, part] - ref["dydt"][:, part]) <= bound + tiny)
+    return got, dy
+
+
+def _dydt_term_scale(o, ref, T, P, Y, part):
+    """size of the terms summed into dT/dt (Eq. 7) or dY_k/dt (Eq. 8), per state"""
+    m = o.mech
+    W = 1.0 / (Y / m.mol_wt).sum(1)
+    rho = P * W / (8314.46261815324 * T)
+    q = (np.abs(ref["cmod"]) * (np.abs(ref["rf"]) + np.abs(ref["rr"]))).max(axis=1)
+    if part.start == 1:
+        return (m.mol_wt.max() * q / rho)[:, None]
+    out = np.empty(len(T))
+    for s in range(len(T)):
+        re, _ = o.species_thermo(float(T[s]))
+        cp = (Y[s] * 8314.46261815324 * re[0] / m.mol_wt).sum()
+        out[s] = np.abs(8314.46261815324 * re[1]).max() * q[s] / (rho[s] * cp)
+    return out[:, None]
+
+
+def check_jacobian(torch, pj, o, T, P, Y, tol=JAC_TOL):
+    dT, dP, dY = dev(torch, T, P, Y)
+    J = pj.eval_jacobian(dT, dP, dY).cpu().numpy()
+    Jr = o.jacobian(T, P, Y)
+    num = np.linalg.norm(J - Jr, axis=1)
+    den = np.linalg.norm(Jr, axis=1)
+    assert np.all(np.isfinite(J))
+    assert np.all(num <= tol * den), (num / den).max()
+    ld = o.ns + 1
+    assert np.all(J.reshape(-1, ld, ld)[:, ld - 1, :] == 0.0)      # column Nsp is zero (C1)
+    return J, (num / np.maximum(den, 1e-300)).max()
+
+
+# ---------------------------------------------------------------------------------- small cases
+def test_tiny_mechanisms_all_reaction_types(torch, PyJac, tiny_mechs):
+    """Every reaction type, falloff form, reverse treatment and third-body variant (C17)."""
+    for m in tiny_mechs:
+        o, pj = Oracle(m), PyJac(m)
+        T, P, Y = synth.make_states(m.n_species, 257, 5, t_range=(500.0, 2800.0), p_range_atm=(0.05, 80.0))
+        check_rates(torch, pj, o, T, P, Y)
+        check_jacobian(torch, pj, o, T, P, Y)
+
+
+def test_tiny_mechanism_last_species_inert(torch, PyJac):
+    m = synth.make_tiny_mechanism(3, n_species=8, last_reacts=False)
+    o, pj = Oracle(m), PyJac(m)
+    T, P, Y = synth.make_states(m.n_species, 64, 6)
+    check_rates(torch, pj, o, T, P, Y)
+    check_jacobian(torch, pj, o, T, P, Y)
+
+
+def test_config0_all_states(torch, PyJac):
+    m = synth.make_mechanism(0)
+    o, pj = Oracle(m), PyJac(m)
+    T, P, Y = synth.config_states(0)
+    assert len(T) == 1024
+    check_rates(torch, pj, o, T, P, Y)
+    check_jacobian(torch, pj, o, T, P, Y)
+
+
+@pytest.mark.parametrize("cfg,n", [(1, 1500), (2, 300), (3, 24)])
+def test_config_prefix(torch, PyJac, cfg, n):
+    """Sizes the oracle finishes in seconds, spanning several CTAs' worth of states and a ragged tail."""
+    m = synth.make_mechanism(cfg)
+    o, pj = Oracle(m), PyJac(m)
+    T, P, Y = synth.config_states(cfg, n)
+    check_rates(torch, pj, o, T, P, Y)
+    check_jacobian(torch, pj, o, T, P, Y)
+
+
+# ---------------------------------------------------------------------------------- full sizes
+@pytest.mark.parametrize("cfg,chunk,n_sample", [(1, 100_000, 96), (2, 100_000, 32), (3, 8192, 6)])
+def test_config_full_size_sampled(torch, PyJac, cfg, chunk, n_sample):
+    """BASELINE.json's full state counts in the launch configuration bench.py times (one launch per
+    chunk); sampled states against the oracle, invariants on every state."""
+    m = synth.make_mechanism(cfg)
+    o, pj = Oracle(m), PyJac(m)
+    T, P, Y = synth.config_states(cfg)
+    n, ns, ld = len(T), m.n_species, m.n_species + 1
+    rng = np.random.default_rng(100 + cfg)
+    mw = torch.from_numpy(m.mol_wt).cuda()
+    buf = torch.empty((min(chunk, n), ld * ld), dtype=torch.float64, device="cuda")
+    for s0 in range(0, n, chunk):
+        s1 = min(n, s0 + chunk)
+        dT, dP, dY = dev(torch, T[s0:s1], P[s0:s1], Y[s0:s1])
+        J = pj.eval_jacobian(dT, dP, dY, out=buf)[: s1 - s0].view(-1, ld, ld)   # [n][col][row]
+        assert bool(torch.isfinite(J).all())
+        assert bool((J[:, ld - 1, :] == 0).all())
+        # P12: species rows (incl. placeholder) of every column sum to zero; checked on all states
+        sp = J[:, :, 1:]
+        resid = sp.sum(dim=2).abs().amax(dim=1)
+        scale = sp.abs().amax(dim=1).sum(dim=1)
+        assert bool((resid <= 1e-12 * scale).all())
+        pick = np.sort(rng.choice(s1 - s0, size=min(n_sample, s1 - s0), replace=False))
+        Jr = o.jacobian(T[s0:s1][pick], P[s0:s1][pick], Y[s0:s1][pick])
+        Jg = J.reshape(-1, ld * ld)[torch.from_numpy(pick).cuda()].cpu().numpy()
+        err = np.linalg.norm(Jg - Jr, axis=1) / np.linalg.norm(Jr, axis=1)
+        assert err.max() <= JAC_TOL, err.max()
+    del buf
+
+
+def test_state_count_sweep_rates_and_dydt(torch, PyJac):
+    """Config 4: the 53-species mechanism at 4^5 .. 4^8 states (larger counts are bench-only);
+    the three kernels agree with the oracle on sampled states at each count."""
+    m = synth.make_mechanism(1)
+    o, pj = Oracle(m), PyJac(m)
+    for n in (4 ** 5, 4 ** 6, 4 ** 7, 4 ** 8):
+        T, P, Y = synth.make_states(m.n_species, n, synth.CONFIGS[1].seed + 2000 + n)
+        dT, dP, dY = dev(torch, T, P, Y)
+        dy = pj.eval_dydt(dT, dP, dY).cpu().numpy()
+        J = pj.eval_jacobian(dT, dP, dY)
+        pick = np.sort(np.random.default_rng(n).choice(n, size=48, replace=False))
+        ref = o.source(T[pick], P[pick], Y[pick])
+        scale = np.abs(ref["dydt"][:, 1:]).max(axis=1, keepdims=True)
+        tol = kr_tol(o, T[pick])
+        bound = tol * np.maximum(scale, _dydt_term_scale(o, ref, T[pick], P[pick], Y[pick], slice(1, None)))
+        assert np.all(np.abs(dy[pick][:, 1:] - ref["dydt"][:, 1:]) <= bound)
+        Jr = o.jacobian(T[pick], P[pick], Y[pick])
+        Jg = J[torch.from_numpy(pick).cuda()].cpu().numpy()
+        assert (np.linalg.norm(Jg - Jr, axis=1) <= JAC_TOL * np.linalg.norm(Jr, axis=1)).all()
+
+
+# ---------------------------------------------------------------------------------- edge cases
+def test_empty_and_single_state(torch, PyJac, tiny_mechs):
+    m = tiny_mechs[0]
+    o, pj = Oracle(m), PyJac(m)
+    T, P, Y = synth.make_states(m.n_species, 1, 8)
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    eY = torch.empty((0, m.n_species), dtype=torch.float64, device="cuda")
+    assert pj.eval_jacobian(e, e, eY).shape == (0, (m.n_species + 1) ** 2)
+    assert pj.eval_dydt(e, e, eY).shape == (0, m.n_species + 1)
+    check_jacobian(torch, pj, o, T, P, Y)
+
+
+def test_padded_leading_dimension_and_batch_split_bit_identical(torch, PyJac):
+    """ldy > Nsp; results do not depend on n, batch split or stream (header contract; App. D)."""
+    m = synth.make_mechanism(0)
+    pj = PyJac(m)
+    T, P, Y = synth.config_states(0, 777)
+    dT, dP, dY = dev(torch, T, P, Y)
+    J = pj.eval_jacobian(dT, dP, dY)
+    Ypad = torch.full((777, m.n_species + 5), 7.0, dtype=torch.float64, device="cuda")
+    Ypad[:, : m.n_species] = dY
+    assert torch.equal(pj.eval_jacobian(dT, dP, Ypad), J)
+    parts = [pj.eval_jacobian(dT[a:b].contiguous(), dP[a:b].contiguous(), dY[a:b].contiguous())
+             for a, b in ((0, 1), (1, 300), (300, 777))]
+    assert torch.equal(torch.cat(parts), J)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        J2 = pj.eval_jacobian(dT, dP, dY)
+    s.synchronize()
+    assert torch.equal(J2, J)
+    r1 = pj.eval_rates(dT, dP, dY)
+    r2 = pj.eval_rates(dT[:100].contiguous(), dP[:100].contiguous(), dY[:100].contiguous())
+    for k in r1:
+        assert torch.equal(r1[k][:100], r2[k])
+
+
+def test_zero_mass_fractions(torch, PyJac, tiny_mechs):
+    """Y_k = 0 exactly for several species (no division by a concentration)."""
+    m = tiny_mechs[1]
+    o, pj = Oracle(m), PyJac(m)
+    T, P, Y = synth.make_states(m.n_species, 40, 12)
+    rng = np.random.default_rng(4)
+    for s in range(len(T)):
+        z = rng.choice(m.n_species - 1, size=3, replace=False)
+        Y[s, z] = 0.0
+        Y[s] /= Y[s].sum()
+    # falloff reactions need a non-zero third-body concentration (header precondition): keep the
+    # single-species third bodies present
+    for i in range(m.n_reactions):
+        if m.tb_species[i] >= 0:
+            Y[:, m.tb_species[i]] = np.maximum(Y[:, m.tb_species[i]], 1e-6)
+    Y /= Y.sum(axis=1, keepdims=True)
+    check_rates(torch, pj, o, T, P, Y)
+    check_jacobian(torch, pj, o, T, P, Y)
+
+
+def test_branch_points(torch, PyJac, tiny_mechs):
+    """T exactly at a NASA midpoint, P exactly at and outside PLOG table pressures (C4, C6)."""
+    m = tiny_mechs[0]
+    o, pj = Oracle(m), PyJac(m)
+    T, P, Y = synth.make_states(m.n_species, 12, 13)
+    T[:3] = [900.0, 1000.0, 1300.0]
+    P[3:8] = np.array([0.1, 1.0, 10.0, 100.0, 1e-3]) * 101325.0
+    P[8] = 500.0 * 101325.0
+    check_rates(torch, pj, o, T, P, Y)
+    check_jacobian(torch, pj, o, T, P, Y)
+
+
+def test_degenerate_mechanisms(torch, PyJac):
+    """No reactions at all; a single species; a reaction whose net stoichiometry cancels."""
+    sp = synth._make_species(np.random.default_rng(1), ("H", "O"), 2, 4, n2_last=False)
+    names, comp, w, lo, hi, tm = sp
+    b = MechanismBuilder(names, ("H", "O"), comp, w, lo, hi, tm)
+    m0 = b.build()
+    o, pj = Oracle(m0), PyJac(m0)
+    T, P, Y = synth.make_states(4, 9, 1)
+    J, _ = check_jacobian(torch, pj, o, T, P, Y, tol=0.0)
+    assert np.all(J == 0.0)
+    b1 = MechanismBuilder(names[:1], ("H", "O"), comp[:1], w[:1], lo[:1], hi[:1], tm[:1])
+    m1 = b1.build()
+    o, pj = Oracle(m1), PyJac(m1)
+    T, P, Y = synth.make_states(1, 3, 1)
+    check_jacobian(torch, pj, o, T, P, Y, tol=0.0)
+
+
+def test_host_buffer_variant_matches_device_variant(torch, PyJac):
+    m = synth.make_mechanism(0)
+    pj = PyJac(m)
+    T, P, Y = synth.config_states(0, 1000)
+    dT, dP, dY = dev(torch, T, P, Y)
+    J = pj.eval_jacobian(dT, dP, dY).cpu()
+    ld = m.n_species + 1
+    out = torch.empty((1000, ld * ld), dtype=torch.float64).pin_memory()
+    hT, hP, hY = (torch.from_numpy(a).pin_memory() for a in (T, P, Y))
+    pj.eval_jacobian_host(hT, hP, hY, out, chunk_states=333)      # ragged chunks, both buffers reused
+    assert torch.equal(out, J)
+    out2 = np.empty((1000, ld * ld))
+    pj.eval_jacobian_host(T, P, Y, out2)                           # pageable numpy buffers
+    assert np.array_equal(out2, J.numpy())
+    dy = np.empty((1000, ld))
+    pj.eval_dydt_host(T, P, Y, dy, chunk_states=512)
+    assert np.array_equal(dy, pj.eval_dydt(dT, dP, dY).cpu().numpy())
+    before = pj.kernel_launches()
+    pj.eval_jacobian(dT, dP, dY)
+    assert pj.kernel_launches() == before + 1

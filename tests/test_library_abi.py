@@ -1,0 +1,126 @@
+"""Host-side checks of the C-ABI library that need no GPU: it loads, exports every symbol that
+include/pyjac_b200.h declares, validates descriptions before touching CUDA, and fails loudly
+(PYJAC_ECUDA, never a CPU fallback) when no device is usable."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1605_03262_b200 import binding, build, synth
+from paper_1605_03262_b200.mechanism import FALLOFF, PLOG, THIRD_BODY, MechanismBuilder
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load_library()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "pyjac_b200.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(pyjac_[a-z_]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(lib):
+    names = declared_symbols()
+    assert set(names) == set(binding.EXPORTS)
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_strerror(lib):
+    for code in (0, -1, -2, -3, -4, -99):
+        assert lib.pyjac_strerror(code)
+    assert b"success" in lib.pyjac_strerror(0)
+
+
+def _create(lib, mech):
+    d, keep = binding.mech_desc(mech)
+    h = C.c_void_p()
+    rc = lib.pyjac_mech_create(C.byref(d), 0, C.byref(h))
+    if rc == 0:
+        lib.pyjac_mech_destroy(h)
+    return rc
+
+
+def _has_gpu():
+    try:
+        import torch
+        return torch.cuda.is_available()
+    except Exception:
+        return False
+
+
+def test_create_fails_loudly_without_a_device(lib):
+    """No GPU here: a valid description must give PYJAC_ECUDA, not a silent fallback."""
+    rc = _create(lib, synth.make_mechanism(0))
+    assert rc == (binding.PYJAC_OK if _has_gpu() else binding.PYJAC_ECUDA)
+
+
+def test_null_and_degenerate_arguments(lib):
+    assert lib.pyjac_mech_create(None, 0, None) == binding.PYJAC_EINVAL
+    h = C.c_void_p()
+    assert lib.pyjac_mech_create(None, 0, C.byref(h)) == binding.PYJAC_EINVAL
+    assert lib.pyjac_mech_destroy(None) == binding.PYJAC_OK
+    assert lib.pyjac_mech_sizes(None, None, None) == binding.PYJAC_EINVAL
+    assert lib.pyjac_eval_jacobian(None, 1, None, None, None, 1, None, None) == binding.PYJAC_EINVAL
+    assert lib.pyjac_eval_jacobian_host(None, 1, None, None, None, 1, None, 0) == binding.PYJAC_EINVAL
+    assert lib.pyjac_kernel_launches() >= 0
+
+
+def _base():
+    m = synth.make_tiny_mechanism(0)
+    return m
+
+
+@pytest.mark.parametrize("what", ["spec_range", "nu_range", "four_species", "neg_A", "plog_order",
+                                  "cheb_lim", "eff_range", "rxn_type", "repeat_species", "tb_range"])
+def test_validation_rejects_bad_descriptions(lib, what):
+    """pyjac_mech_create validates on the host before any CUDA call (PYJAC_EINVAL)."""
+    m = _base()
+    if what == "spec_range":
+        m.reac_spec = m.reac_spec.copy(); m.reac_spec[0] = m.n_species
+    elif what == "nu_range":
+        m.prod_nu = m.prod_nu.copy(); m.prod_nu[0] = 4
+    elif what == "four_species":
+        b = MechanismBuilder(m.species_names, m.element_names, m.composition, m.mol_wt, m.nasa_lo,
+                             m.nasa_hi, m.t_mid)
+        b.add([(0, 1), (1, 1), (2, 1), (3, 1)], [(4, 1)], (1.0, 0.0, 0.0))
+        m = b.build()
+    elif what == "neg_A":
+        i = int(np.where(m.rxn_type == 0)[0][0])
+        m.arr_hi = m.arr_hi.copy(); m.arr_hi[i, 0] = -1.0
+    elif what == "plog_order":
+        i = int(np.where(m.rxn_type == PLOG)[0][0])
+        m.plog_p = m.plog_p.copy(); b = m.plog_ptr[i]; m.plog_p[b + 1] = m.plog_p[b]
+    elif what == "cheb_lim":
+        i = int(np.where(m.rxn_type == 5)[0][0])
+        m.cheb_lim = m.cheb_lim.copy(); m.cheb_lim[i, 1] = m.cheb_lim[i, 0]
+    elif what == "eff_range":
+        m.eff_spec = m.eff_spec.copy(); m.eff_spec[0] = -1
+    elif what == "rxn_type":
+        m.rxn_type = m.rxn_type.copy(); m.rxn_type[0] = 6
+    elif what == "repeat_species":
+        b = MechanismBuilder(m.species_names, m.element_names, m.composition, m.mol_wt, m.nasa_lo,
+                             m.nasa_hi, m.t_mid)
+        b.add([(0, 1), (0, 1)], [(4, 1)], (1.0, 0.0, 0.0))
+        m = b.build()
+    elif what == "tb_range":
+        i = int(np.where(m.rxn_type == THIRD_BODY)[0][0])
+        m.tb_species = m.tb_species.copy(); m.tb_species[i] = m.n_species
+    assert _create(lib, m) == binding.PYJAC_EINVAL
+
+
+def test_binding_refuses_cpu_tensors():
+    """The product path never computes on the CPU: the binding rejects non-CUDA tensors."""
+    import torch
+    pj = binding.PyJac.__new__(binding.PyJac)
+    pj.ns, pj.nr = 3, 1
+    with pytest.raises(TypeError):
+        pj._dev_inputs(torch.zeros(2, dtype=torch.float64), torch.zeros(2, dtype=torch.float64),
+                       torch.zeros(2, 3, dtype=torch.float64))
