@@ -92,7 +92,11 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     *out = nullptr;
     HostPack hp;
     const char *why = nullptr;
-    int rc = pack_mechanism(d, hp, &why);
+    // validate first (no CUDA call yet), with the architecture's shared-memory size; the real
+    // device's limit is checked below
+    int panels = 0;
+    if (const char *e = std::getenv("PYJAC_PANELS")) panels = std::atoi(e);   // tuning hook, see DESIGN.md
+    int rc = pack_mechanism(d, hp, (size_t)227 * 1024, panels, &why);
     if (rc != PYJAC_OK) return rc;
     pyjac_mech *m = new (std::nothrow) pyjac_mech();
     if (!m) return PYJAC_ENOMEM;
@@ -111,8 +115,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     dm.ns = hp.ns; dm.nr = hp.nr; dm.ld = hp.ns + 1;
     dm.ln_patm_over_R = std::log(kPatm / kRu);
     dm.pd_begin = hp.pd_begin; dm.n_pd = hp.n_pd; dm.pk_begin = hp.pk_begin; dm.n_pk = hp.n_pk;
-    dm.n_sp_task = hp.ns; dm.n_long = hp.n_long; dm.n_v = hp.n_v; dm.n_vext = hp.n_vext;
-    dm.spns_base = hp.spns_base;
+    dm.n_spchunk = hp.n_spchunk; dm.n_panel = hp.n_panel; dm.pw = hp.pw; dm.ldt = hp.ldt; dm.n_v = hp.n_v;
     Uploader up;
     try {
         up.add(&dm.mw, hp.mw); up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.dcol, hp.dcol);
@@ -126,10 +129,11 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         up.add(&dm.eff_ptr, hp.eff_ptr); up.add(&dm.eff_spec, hp.eff_spec); up.add(&dm.eff_eps, hp.eff_eps);
         up.add(&dm.eff_vbase, hp.eff_vbase);
         up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
-        up.add(&dm.sp_ptr, hp.sp_ptr); up.add(&dm.sp_ent, hp.sp_ent);
-        up.add(&dm.col_ptr, hp.col_ptr); up.add(&dm.col_ent, hp.col_ent);
-        up.add(&dm.long_ptr, hp.long_ptr); up.add(&dm.long_ent, hp.long_ent);
-        up.add(&dm.cell_info, hp.cell_info); up.add(&dm.cell_ent, hp.cell_ent);
+        up.add((const uint32_t **)&dm.spchunk, hp.spchunk); up.add(&dm.sptask_k, hp.sptask_k);
+        up.add((const uint32_t **)&dm.sp_ent, hp.sp_ent);
+        up.add((const int32_t **)&dm.panel_chunks, hp.panel_chunks);
+        up.add((const uint32_t **)&dm.cchunk, hp.cchunk); up.add(&dm.ctask_addr, hp.ctask_addr);
+        up.add(&dm.c_ent, hp.c_ent);
     } catch (...) {
         delete m;
         cudaSetDevice(prev);
@@ -143,7 +147,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     }
     if (rc == PYJAC_OK) {
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
-        m->plan = make_smem_plan(hp.ns, hp.nr, hp.n_vext);
+        m->plan = make_smem_plan(hp.ns, hp.nr, hp.n_v, hp.ldt, hp.pw);
         m->threads = choose_threads(hp.ns, hp.nr);
         const size_t bytes = (size_t)m->plan.total * sizeof(double);
         if (bytes > (size_t)prop.sharedMemPerBlockOptin) {
@@ -153,6 +157,8 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
                 m->smem[level] = bytes;
                 const void *k = eval_kernel_ptr(level, m->threads);
                 if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess ||
+                    cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                         cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
                     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m->ctas_per_sm[level], k, m->threads, bytes) !=
                         cudaSuccess ||
                     m->ctas_per_sm[level] < 1)

@@ -13,7 +13,7 @@ namespace pyjac {
 constexpr double kRu = 8314.46261815324;   // J kmol^-1 K^-1
 constexpr double kPatm = 101325.0;         // Pa
 constexpr int kMaxSide = 3;                // species per reaction side
-constexpr int kLongCell = 3;               // cells with more contributions are pre-reduced (phase 2)
+constexpr int kSpLanes = 4;                // lanes that share one species task
 
 // meta word of a reaction: bits 0..23 six 4-bit nu (slots 0-2 reactants, 3-5 products; 0 = empty
 // slot), 24..26 rxn_type, 27..28 rev_type, 29..30 falloff_form, 31 third body is a single species.
@@ -65,48 +65,51 @@ struct DeviceMech {
     const int32_t *pk_ptr;      // [n_pk+1] offsets into pk_data
     const double *pk_data;      // PLOG: n, then n x {p, ln p, ln A, beta, Ta};
                                 // Chebyshev: nT, nP, 1/Tmin, 1/Tmax, log10 pmin, log10 pmax, eta[nT*nP]
-    // ---- phase-2 gather tasks (fixed summation order)
-    int n_sp_task;              // = ns: species sums over reactions (wdot, A, Tcol)
-    const int32_t *sp_ptr;      // [ns+1]
-    const uint32_t *sp_ent;     // entries: reaction (sorted) | coef16 (net nu_ki)
-    const int32_t *col_ptr;     // [ns+1] energy-row column sums: entries (V index | reaction<<16)
-    const uint32_t *col_ent;
-    int n_long;                 // pre-reduced cells (incl. every cell of the virtual column Ns)
-    const int32_t *long_ptr;    // [n_long+1]
-    const uint32_t *long_ent;   // entries: V index | coef16
-    // ---- phase-4 cell lists: cell (r, c), r, c in 0..ns, at r + c*ld
-    const uint32_t *cell_info;  // [ld*ld] offset<<3 | count (count <= kLongCell)
-    const uint32_t *cell_ent;   // entries: V index | coef16
-    // ---- sizes of the per-state shared-memory arrays
-    int n_v;                    // per-reaction derivative entries s'_ij (phase 1 output)
-    int n_vext;                 // n_v + n_long + 1 (a zero slot)
-    int spns_base;              // V-ext index of the (k, Ns) sums, k = 0..ns-1
+    // ---- species tasks: wdot_k, A_k, Tcol_k and the diagonal cell (k, k) are sums over the
+    // reactions that contain k.  kSpLanes lanes share one species; a chunk is 32 / kSpLanes species.
+    int n_spchunk;
+    const uint2 *spchunk;       // [n_spchunk] {first entry, steps}; entries at [first + step*32 + lane]
+    const int32_t *sptask_k;    // [n_spchunk * 32 / kSpLanes] species or -1
+    const uint2 *sp_ent;        // {reaction (sorted) | coef16, V index | coef16}
+    // ---- cell tasks: the off-diagonal cells (k, j) of the species block that collect at least
+    // one reaction, per column panel, sorted by list length (descending); 32 tasks per chunk.
+    int n_panel, pw, ldt;       // panels of pw columns; tile leading dimension (odd)
+    const int2 *panel_chunks;   // [n_panel] {first chunk, one past last}
+    const uint2 *cchunk;        // {first entry, steps}; entries at [first + step*32 + lane]
+    const uint32_t *ctask_addr; // [n_chunk*32] tile offset k + (j - j0)*ldt (pad: ldt*pw)
+    const uint32_t *c_ent;      // V index | coef16 (pad: zero slot n_v, coefficient 0)
+    int n_v;                    // per-reaction derivative entries s'_ij; V[n_v] is a zero slot
 };
 
-// Shared-memory plan of one CTA (doubles).  Every array is per state.
+// Shared-memory plan of one CTA (offsets in doubles).  Every array is per state.
 struct SmemPlan {
-    int X, B, dB, HW, Cp, dCp;          // [ns+1] species arrays (slot ns is the empty-slot dummy)
-    int Wdot, A, Tc, E, WA, Row0, Col0; // [ns+1]
-    int Q, Ar, Th, H;                   // [nr]
-    int V;                              // [n_vext]
+    int X, B, dB, HW, Cp;               // [ns+1] species arrays (slot ns is the empty-slot dummy)
+    int Wdot, A, Tc, Diag, WA, WC;      // [ns+1]
+    int Ep;                             // [kEParts][ns+1] partial energy-row column sums
+    int Row0, Col0;                     // [ns+1]
+    int Q, Ar, Th;                      // [nr+1] (slot nr stays zero: padding of the gather lists)
+    int V;                              // [n_v+1]
+    int Tile;                           // [ldt*pw + 2]
     int Red;                            // [8][32] reduction scratch
-    int Scal;                           // [16] per-state scalars
     int total;                          // doubles
 };
 
-inline SmemPlan make_smem_plan(int ns, int nr, int n_vext)
+constexpr int kEParts = 4;
+
+inline SmemPlan make_smem_plan(int ns, int nr, int n_v, int ldt, int pw)
 {
     SmemPlan p{};
     int o = 0;
     auto take = [&](int n) { int r = o; o += (n + 1) & ~1; return r; };
     const int s1 = ns + 1;
-    p.X = take(s1); p.B = take(s1); p.dB = take(s1); p.HW = take(s1); p.Cp = take(s1); p.dCp = take(s1);
-    p.Wdot = take(s1); p.A = take(s1); p.Tc = take(s1); p.E = take(s1); p.WA = take(s1);
+    p.X = take(s1); p.B = take(s1); p.dB = take(s1); p.HW = take(s1); p.Cp = take(s1);
+    p.Wdot = take(s1); p.A = take(s1); p.Tc = take(s1); p.Diag = take(s1); p.WA = take(s1); p.WC = take(s1);
+    p.Ep = take(kEParts * s1);
     p.Row0 = take(s1); p.Col0 = take(s1);
-    p.Q = take(nr); p.Ar = take(nr); p.Th = take(nr); p.H = take(nr);
-    p.V = take(n_vext);
+    p.Q = take(nr + 1); p.Ar = take(nr + 1); p.Th = take(nr + 1);
+    p.V = take(n_v + 1);
+    p.Tile = take(ldt * pw + 2);
     p.Red = take(8 * 32);
-    p.Scal = take(16);
     p.total = o;
     return p;
 }

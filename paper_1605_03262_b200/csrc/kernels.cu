@@ -240,11 +240,6 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         const double base = -st.W * (Rf * (double)snu_f - Rr * (double)snu_r);
         const double mix = (pdep && !meta_single(meta)) ? st.rho : 0.0;
         sm[sp.Ar + s] = c * base + b * (mix - st.W * Xi);
-        // H_i = sum_k nu_ki h_k W_k (weights of the energy row, Eq. 113)
-        double H = 0.0;
-#pragma unroll
-        for (int e = 0; e < 6; ++e) H += (e < 3 ? -(double)nu[e] : (double)nu[e]) * sm[sp.HW + spec[e]];
-        sm[sp.H + s] = H;
         // sparse terms s'_ij = c (k_f S'_j - k_r S''_j) per slot, b (alpha_ij - 1) per efficiency
         const double ckf = c * kf, ckr = -c * kr;
         double *V = sm + sp.V + m.vbase[s];
@@ -271,10 +266,14 @@ __global__ void __launch_bounds__(NT) eval_kernel(const DeviceMech m, const Smem
     extern __shared__ double sm[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
-    const int ns = m.ns, nr = m.nr, ld = m.ld;
-    if (tid == 0) {   // the empty-slot dummy species: [X] = 1, B = dB = hW = 0
+    const int ns = m.ns, nr = m.nr, ld = m.ld, ldt = m.ldt;
+    double *tile = sm + sp.Tile;
+    if (tid == 0) {   // the empty-slot dummy species ([X] = 1, B = dB = hW = 0) and the zero slots
         sm[sp.X + ns] = 1.0; sm[sp.B + ns] = 0.0; sm[sp.dB + ns] = 0.0; sm[sp.HW + ns] = 0.0;
+        sm[sp.Q + nr] = 0.0; sm[sp.Ar + nr] = 0.0; sm[sp.Th + nr] = 0.0; sm[sp.V + m.n_v] = 0.0;
     }
+    if (LEVEL == 2)   // cells that collect no reaction stay zero for the whole launch (single panel)
+        for (int i = tid; i < ldt * m.pw + 2; i += NT) tile[i] = 0.0;
     double *red = sm + sp.Red;
     for (long long state = blockIdx.x; state < n; state += gridDim.x) {
         StateScalars st;
@@ -317,114 +316,147 @@ __global__ void __launch_bounds__(NT) eval_kernel(const DeviceMech m, const Smem
         // ---- phase 1: reactions
         for (int s = tid; s < nr; s += NT) reaction<LEVEL>(m, sp, sm, s, st, out, state);
         __syncthreads();
-        // ---- phase 2: fixed-order gathers
-        {
-            const int ntask = LEVEL == 2 ? 2 * ns + m.n_long : ns;
-            for (int t = tid; t < ntask; t += NT) {
-                if (t < ns) {
-                    double wd = 0.0, A = 0.0, Tc = 0.0;
-                    for (int e = m.sp_ptr[t], e1 = m.sp_ptr[t + 1]; e < e1; ++e) {
-                        const uint32_t ent = m.sp_ent[e];
-                        const int s = ent & 0xFFFF;
-                        const double cf = entry_coef(ent);
-                        wd += cf * sm[sp.Q + s];
-                        if (LEVEL == 2) { A += cf * sm[sp.Ar + s]; Tc += cf * sm[sp.Th + s]; }
-                    }
-                    sm[sp.Wdot + t] = wd;
-                    if (LEVEL == 2) { sm[sp.A + t] = A; sm[sp.Tc + t] = Tc; }
-                } else if (t < 2 * ns) {
-                    const int j = t - ns;
-                    double E = 0.0;
-                    for (int e = m.col_ptr[j], e1 = m.col_ptr[j + 1]; e < e1; ++e) {
-                        const uint32_t ent = m.col_ent[e];
-                        E += sm[sp.H + (ent >> 16)] * sm[sp.V + (ent & 0xFFFF)];
-                    }
-                    sm[sp.E + j] = E;
-                } else {
-                    const int l = t - 2 * ns;
-                    double acc = 0.0;
-                    for (int e = m.long_ptr[l], e1 = m.long_ptr[l + 1]; e < e1; ++e) {
-                        const uint32_t ent = m.long_ent[e];
-                        acc += entry_coef(ent) * sm[sp.V + (ent & 0xFFFF)];
-                    }
-                    sm[sp.V + m.n_v + l] = acc;
+        // ---- phase 2a: species sums over reactions, kSpLanes lanes per species (fixed order)
+        for (int c = warp; c < m.n_spchunk; c += NW) {
+            const uint2 ch = m.spchunk[c];
+            const uint2 *ent = m.sp_ent + ch.x + lane;
+            double wd = 0.0, A = 0.0, Tc = 0.0, Dg = 0.0;
+            for (uint32_t t = 0; t < ch.y; ++t) {
+                const uint2 e = ent[t * 32];
+                const int s = e.x & 0xFFFF;
+                const double cf = entry_coef(e.x);
+                wd += cf * sm[sp.Q + s];
+                if (LEVEL == 2) {
+                    A += cf * sm[sp.Ar + s];
+                    Tc += cf * sm[sp.Th + s];
+                    Dg += entry_coef(e.y) * sm[sp.V + (e.y & 0xFFFF)];
+                }
+            }
+#pragma unroll
+            for (int o = kSpLanes / 2; o > 0; o >>= 1) {
+                wd += __shfl_xor_sync(0xFFFFFFFFu, wd, o);
+                if (LEVEL == 2) {
+                    A += __shfl_xor_sync(0xFFFFFFFFu, A, o);
+                    Tc += __shfl_xor_sync(0xFFFFFFFFu, Tc, o);
+                    Dg += __shfl_xor_sync(0xFFFFFFFFu, Dg, o);
+                }
+            }
+            const int k = m.sptask_k[c * (32 / kSpLanes) + lane / kSpLanes];
+            if ((lane % kSpLanes) == 0 && k >= 0) {
+                sm[sp.Wdot + k] = wd;
+                if (LEVEL == 2) {
+                    sm[sp.A + k] = A; sm[sp.Tc + k] = Tc;
+                    if (m.n_panel == 1) tile[k + k * ldt] = Dg; else sm[sp.Diag + k] = Dg;
                 }
             }
         }
+        // ---- phase 2b: off-diagonal cells of the species block, longest lists first (single panel)
+        auto gather_cells = [&](int p) {
+            const int2 pc = m.panel_chunks[p];
+            for (int c = pc.x + warp; c < pc.y; c += NW) {
+                const uint2 ch = m.cchunk[c];
+                const uint32_t *ent = m.c_ent + ch.x + lane;
+                double acc = 0.0;
+                for (uint32_t t = 0; t < ch.y; ++t) {
+                    const uint32_t e = ent[t * 32];
+                    acc += entry_coef(e) * sm[sp.V + (e & 0xFFFF)];
+                }
+                tile[m.ctask_addr[c * 32 + lane]] = acc;
+            }
+        };
+        if (LEVEL == 2 && m.n_panel == 1) gather_cells(0);
         __syncthreads();
         // ---- phase 3: species finalisation (Eqs. 7-8, 111, 113)
-        {
-            const double irho = 1.0 / st.rho;
-            double part[4] = {0.0, 0.0, 0.0, 0.0};
-            for (int k = tid; k < ns; k += NT) {
-                const double wd = sm[sp.Wdot + k];
-                const double Wk = m.mw[k];
-                const double hw = sm[sp.HW + k];
-                if (LEVEL == 0) { if (out.wdot) out.wdot[state * ns + k] = wd; }
-                if (LEVEL == 1) { out.dydt[state * ld + k + 1] = Wk * wd * irho; }
-                part[0] += hw * wd;
-                if (LEVEL == 2) {
-                    const double Ap = wd * st.W + sm[sp.A + k];
-                    const double Tc = sm[sp.Tc + k];
-                    sm[sp.WA + k] = Wk * Ap * irho;
-                    sm[sp.Col0 + k + 1] = Wk * irho * Tc;
-                    part[1] += hw * Ap;
-                    part[2] += sm[sp.Cp + k] * Wk * wd;
-                    part[3] += hw * Tc;
-                }
-            }
-            if (LEVEL >= 1) {
-                block_reduce<4>(part, red + 3 * 32, lane, warp, NW);
-                if (LEVEL == 1 && tid == 0) out.dydt[state * ld] = -part[0] * irho / st.cp;
-            }
+        const double irho = 1.0 / st.rho;
+        double part[4] = {0.0, 0.0, 0.0, 0.0};
+        for (int k = tid; k < ns; k += NT) {
+            const double wd = sm[sp.Wdot + k];
+            const double Wk = m.mw[k];
+            const double hw = sm[sp.HW + k];
+            if (LEVEL == 0) { if (out.wdot) out.wdot[state * ns + k] = wd; }
+            if (LEVEL == 1) { out.dydt[state * ld + k + 1] = Wk * wd * irho; }
+            part[0] += hw * wd;
             if (LEVEL == 2) {
-                const double icp = 1.0 / st.cp;
-                if (tid == 0)
-                    sm[sp.Col0] = -icp * irho * (part[2] - st.dcpdT * icp * part[0] + part[3]);
-                const double shg = part[0] * irho, shA = part[1] * irho;
-                const double cpl = sm[sp.Cp + ns - 1];
-                const double El = m.inv_mw[ns - 1] * sm[sp.E + ns - 1];
-                for (int j = tid; j < ns - 1; j += NT)
-                    sm[sp.Row0 + j + 1] = -icp * (-(sm[sp.Cp + j] - cpl) * icp * shg + m.dcol[j] * shA
-                                                  + m.inv_mw[j] * sm[sp.E + j] - El);
+                const double Ap = wd * st.W + sm[sp.A + k];
+                const double Tc = sm[sp.Tc + k];
+                sm[sp.WA + k] = Wk * Ap * irho;
+                sm[sp.Col0 + k + 1] = Wk * irho * Tc;
+                part[1] += hw * Ap;
+                part[2] += sm[sp.Cp + k] * Wk * wd;
+                part[3] += hw * Tc;
             }
         }
+        if (LEVEL >= 1) {
+            block_reduce<4>(part, red + 3 * 32, lane, warp, NW);
+            if (LEVEL == 1 && tid == 0) out.dydt[state * ld] = -part[0] * irho / st.cp;
+        }
         if (LEVEL == 2) {
-            __syncthreads();
-            // ---- phase 4: dense write-out (column-major, LD = ns + 1)
+            const double icp = 1.0 / st.cp;
+            if (tid == 0) sm[sp.Col0] = -icp * irho * (part[2] - st.dcpdT * icp * part[0] + part[3]);
+            const double shg = part[0] * irho, shA = part[1] * irho;
+            const double cpl = sm[sp.Cp + ns - 1];
+            const double iwl = m.inv_mw[ns - 1];
             double *J = out.jac + state * (long long)ld * ld;
             const int nrb = (ld + 31) >> 5;
             int g = NW, h = nrb;            // g = gcd(NW, nrb)
             while (h) { const int t = g % h; g = h; h = t; }
-            const double iwl = m.inv_mw[ns - 1];
-            for (int rb = warp % g; rb < nrb; rb += g) {
-                const int r = rb * 32 + lane;
-                const bool row_ok = r < ld;
-                const int k = r - 1;
-                double wa = 0.0, wk = 0.0, wc = 0.0;
-                if (row_ok && r >= 1) {
-                    wa = sm[sp.WA + k];
-                    wk = m.mw[k];
-                    wc = wk * iwl * sm[sp.V + m.spns_base + k];
+            double El = 0.0;                // energy-row sum of the virtual column Nsp
+            // panels of columns; the one holding the virtual column Nsp goes first (its sums enter
+            // every other column, Eqs. 119, 123, 127)
+            for (int pi = 0; pi < m.n_panel; ++pi) {
+                const int p = pi == 0 ? m.n_panel - 1 : pi - 1;
+                const int j0 = p * m.pw, j1 = min(ns, j0 + m.pw), pwc = j1 - j0;
+                if (m.n_panel > 1) {
+                    if (pi > 0) __syncthreads();                  // previous panel's write-out done
+                    for (int i = tid; i < ldt * m.pw; i += NT) tile[i] = 0.0;
+                    __syncthreads();
+                    gather_cells(p);
+                    for (int j = j0 + tid; j < j1; j += NT) tile[j + (j - j0) * ldt] = sm[sp.Diag + j];
+                    __syncthreads();
                 }
-                for (int c = 1 + warp / g; c < ns; c += NW / g) {
-                    const double dj = m.dcol[c - 1], iwj = m.inv_mw[c - 1];
-                    if (row_ok) {
-                        double val;
-                        if (r == 0) {
-                            val = sm[sp.Row0 + c];
-                        } else {
-                            const uint32_t info = m.cell_info[r + c * ld];
-                            const uint32_t *ent = m.cell_ent + (info >> 3);
-                            const int cnt = info & 7;
-                            double acc = 0.0;
-                            for (int t = 0; t < cnt; ++t) {
-                                const uint32_t en = ent[t];
-                                acc += entry_coef(en) * sm[sp.V + (en & 0xFFFF)];
-                            }
-                            val = wa * dj + (wk * iwj * acc - wc);
+                // energy-row partial sums E_j = sum_k h_k W_k cell(k, j), kEParts row ranges per column
+                const int rows = (ns + kEParts - 1) / kEParts;
+                for (int t = tid; t < pwc * kEParts; t += NT) {
+                    const int jl = t % pwc, pt = t / pwc;
+                    const int k1 = min(ns, (pt + 1) * rows);
+                    double e = 0.0;
+                    for (int k = pt * rows; k < k1; ++k) e += sm[sp.HW + k] * tile[k + jl * ldt];
+                    sm[sp.Ep + pt * (ns + 1) + jl] = e;
+                }
+                if (pi == 0)
+                    for (int k = tid; k < ns; k += NT) sm[sp.WC + k] = m.mw[k] * iwl * tile[k + (ns - 1 - j0) * ldt];
+                __syncthreads();
+                if (pi == 0) {
+                    const int jl = ns - 1 - j0;
+                    for (int pt = 0; pt < kEParts; ++pt) El += sm[sp.Ep + pt * (ns + 1) + jl];
+                    El *= iwl;
+                }
+                for (int jl = tid; jl < pwc; jl += NT) {
+                    const int j = j0 + jl;
+                    if (j >= ns - 1) continue;
+                    double E = 0.0;
+                    for (int pt = 0; pt < kEParts; ++pt) E += sm[sp.Ep + pt * (ns + 1) + jl];
+                    sm[sp.Row0 + j + 1] = -icp * (-(sm[sp.Cp + j] - cpl) * icp * shg + m.dcol[j] * shA
+                                                  + m.inv_mw[j] * E - El);
+                }
+                __syncthreads();
+                // ---- phase 4: dense write-out (column-major, LD = ns + 1), one column segment per warp
+                const int pwo = min(j1, ns - 1) - j0;
+                for (int rb = warp % g; rb < nrb; rb += g) {
+                    const int r = rb * 32 + lane;
+                    const bool row_ok = r < ld;
+                    const int k = r - 1;
+                    double wa = 0.0, wk = 0.0, wc = 0.0;
+                    if (row_ok && r >= 1) { wa = sm[sp.WA + k]; wk = m.mw[k]; wc = sm[sp.WC + k]; }
+                    for (int jl = warp / g; jl < pwo; jl += NW / g) {
+                        const int j = j0 + jl;
+                        const double dj = m.dcol[j], iwj = m.inv_mw[j];
+                        if (row_ok) {
+                            double val;
+                            if (r == 0) val = sm[sp.Row0 + j + 1];
+                            else val = wa * dj + (wk * iwj * tile[k + jl * ldt] - wc);
+                            __stcs(J + r + (long long)(j + 1) * ld, val);
                         }
-                        __stcs(J + r + (long long)c * ld, val);
                     }
                 }
             }
@@ -433,8 +465,8 @@ __global__ void __launch_bounds__(NT) eval_kernel(const DeviceMech m, const Smem
                 __stcs(J + r + (long long)ns * ld, 0.0);
             }
         }
-        // the next state's phase 0 writes only arrays that phase 4 does not read; its first
-        // __syncthreads orders everything else
+        // the next state's phase 0 writes only arrays that phase 4 does not read; its
+        // __syncthreads (two before the tile is written again) order everything else
     }
 }
 

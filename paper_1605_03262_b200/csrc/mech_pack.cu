@@ -31,12 +31,12 @@ struct ColEntry {
 
 }  // namespace
 
-static void pack_impl(const pyjac_mech_desc *d, HostPack &o)
+static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget, int panel_override)
 {
     REQUIRE(d != nullptr, "description is NULL");
     const int ns = d->n_species, nr = d->n_reactions;
     REQUIRE(ns >= 1 && nr >= 0, "n_species must be >= 1 and n_reactions >= 0");
-    if (ns > 65534 || nr > 65535) throw Fail{PYJAC_ELIMIT, "more than 65534 species or 65535 reactions"};
+    if (ns > 65534 || nr > 65534) throw Fail{PYJAC_ELIMIT, "more than 65534 species or reactions"};
     REQUIRE(d->mol_wt && d->nasa_lo && d->nasa_hi && d->t_mid, "species arrays missing");
     if (nr > 0) {
         REQUIRE(d->reac_ptr && d->prod_ptr && d->rxn_type && d->rev_type && d->arr_hi && d->arr_lo &&
@@ -238,86 +238,120 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o)
     if (o.n_pk == 0) o.pk_begin = nr;
     o.n_v = (int)nv;
 
-    // ---- species tasks: wdot_k, A_k, Tcol_k = sum_i nu_ki {q_i, a_i, thetaT_i}  (Eqs. 14, 111, 115-117)
-    {
-        std::vector<std::vector<uint32_t>> lists(ns);
-        for (int s = 0; s < nr; ++s)
-            for (auto &pr : net[s])
-                if (pr.second != 0) lists[pr.first].push_back(pack_entry((uint32_t)s, pr.second));
-        o.sp_ptr.assign(1, 0);
-        for (int k = 0; k < ns; ++k) {
-            o.sp_ent.insert(o.sp_ent.end(), lists[k].begin(), lists[k].end());
-            o.sp_ptr.push_back((int32_t)o.sp_ent.size());
+    if (o.n_v + 1 > 65535) throw Fail{PYJAC_ELIMIT, "more than 65534 per-reaction derivative entries"};
+    const uint32_t zero_slot = (uint32_t)o.n_v;
+
+    // ---- cells of the species block: (k, j) += nu_ki s'_ij  (Eqs. 112, 118-127); j = ns-1 is the
+    // virtual column of the terms proportional to 1/W_Nsp
+    std::vector<std::vector<uint32_t>> cell((size_t)ns * ns);   // [j][k]
+    for (int s = 0; s < nr; ++s)
+        for (auto &pr : net[s]) {
+            if (pr.second == 0) continue;
+            for (auto &ce : cols[s]) cell[(size_t)ce.spec * ns + pr.first].push_back(pack_entry(ce.vi, pr.second));
         }
-    }
-    // ---- energy-row column tasks: E_j = sum_i H_i s'_ij with H_i = sum_k nu_ki h_k W_k  (Eq. 113)
+
+    // ---- species tasks: wdot_k, A_k, Tcol_k = sum_i nu_ki {q_i, a_i, thetaT_i} (Eqs. 14, 111,
+    // 115-117) and the diagonal cell (k, k); kSpLanes lanes per species, longest lists first
     {
-        std::vector<std::vector<uint32_t>> lists(ns);
-        for (int s = 0; s < nr; ++s)
-            for (auto &ce : cols[s]) lists[ce.spec].push_back(ce.vi | (uint32_t)s << 16);
-        o.col_ptr.assign(1, 0);
-        for (int j = 0; j < ns; ++j) {
-            o.col_ent.insert(o.col_ent.end(), lists[j].begin(), lists[j].end());
-            o.col_ptr.push_back((int32_t)o.col_ent.size());
-        }
-    }
-    // ---- cell lists: species block (row k+1, column j+1) += W_k nu_ki s'_ij / W_j  (Eqs. 112, 118-127)
-    const int ld = ns + 1;
-    {
-        std::vector<std::vector<uint32_t>> cell((size_t)ns * ns);   // [j][k], j = column species
+        std::vector<std::vector<std::pair<uint32_t, uint32_t>>> lists(ns);
         for (int s = 0; s < nr; ++s)
             for (auto &pr : net[s]) {
                 if (pr.second == 0) continue;
-                for (auto &ce : cols[s]) cell[(size_t)ce.spec * ns + pr.first].push_back(pack_entry(ce.vi, pr.second));
-            }
-        o.cell_info.assign((size_t)ld * ld, 0u);
-        o.long_ptr.assign(1, 0);
-        int n_long = 0;
-        for (int j = 0; j < ns - 1; ++j)
-            for (int k = 0; k < ns; ++k) {
-                auto &lst = cell[(size_t)j * ns + k];
-                if (lst.empty()) continue;
-                const size_t at = (size_t)(k + 1) + (size_t)(j + 1) * ld;
-                if ((int)lst.size() > kLongCell) {
-                    o.long_ent.insert(o.long_ent.end(), lst.begin(), lst.end());
-                    o.long_ptr.push_back((int32_t)o.long_ent.size());
-                    lst.assign(1, pack_entry((uint32_t)(o.n_v + n_long), 1));
-                    ++n_long;
+                const int k = pr.first;
+                bool first = true;
+                for (auto &ce : cols[s]) {
+                    if (ce.spec != k) continue;
+                    lists[k].push_back({first ? pack_entry((uint32_t)s, pr.second) : (uint32_t)nr,
+                                        pack_entry(ce.vi, pr.second)});
+                    first = false;
                 }
+                if (first) lists[k].push_back({pack_entry((uint32_t)s, pr.second), zero_slot});
             }
-        // the virtual column N_sp (terms proportional to 1/W_Nsp of Eqs. 119, 123, 127): one sum per row
-        o.spns_base = o.n_v + n_long;
-        for (int k = 0; k < ns; ++k) {
-            auto &lst = cell[(size_t)(ns - 1) * ns + k];
-            o.long_ent.insert(o.long_ent.end(), lst.begin(), lst.end());
-            o.long_ptr.push_back((int32_t)o.long_ent.size());
-            ++n_long;
+        std::vector<int> ord(ns);
+        std::iota(ord.begin(), ord.end(), 0);
+        std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return lists[a].size() > lists[b].size(); });
+        const int per = 32 / kSpLanes;
+        const int nchunk = (ns + per - 1) / per;
+        o.sptask_k.assign((size_t)nchunk * per, -1);
+        for (int c = 0; c < nchunk; ++c) {
+            int steps = 0;
+            for (int i = 0; i < per && c * per + i < ns; ++i) {
+                const int k = ord[c * per + i];
+                o.sptask_k[(size_t)c * per + i] = k;
+                steps = std::max(steps, (int)((lists[k].size() + kSpLanes - 1) / kSpLanes));
+            }
+            const uint32_t base = (uint32_t)(o.sp_ent.size() / 2);
+            o.spchunk.push_back(base);
+            o.spchunk.push_back((uint32_t)steps);
+            o.sp_ent.resize(o.sp_ent.size() + (size_t)2 * steps * 32, 0u);
+            for (int st = 0; st < steps; ++st)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const int i = lane / kSpLanes, sub = lane % kSpLanes;
+                    uint32_t w0 = (uint32_t)nr, w1 = zero_slot;   // coefficient 0 on the zero slots
+                    if (c * per + i < ns) {
+                        const auto &lst = lists[ord[c * per + i]];
+                        const size_t e = (size_t)st * kSpLanes + sub;
+                        if (e < lst.size()) { w0 = lst[e].first; w1 = lst[e].second; }
+                    }
+                    o.sp_ent[2 * ((size_t)base + (size_t)st * 32 + lane) + 0] = w0;
+                    o.sp_ent[2 * ((size_t)base + (size_t)st * 32 + lane) + 1] = w1;
+                }
         }
-        o.n_long = n_long;
-        o.n_vext = o.n_v + n_long;
-        if (o.n_vext > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-reaction derivative entries"};
-        // entries of pre-reduced cells were packed before n_long was final; their source index is
-        // n_v + t with t < n_long, which fits by the check above
-        for (int j = 0; j < ns - 1; ++j)
-            for (int k = 0; k < ns; ++k) {
-                auto &lst = cell[(size_t)j * ns + k];
-                if (lst.empty()) continue;
-                const size_t at = (size_t)(k + 1) + (size_t)(j + 1) * ld;
-                o.cell_info[at] = (uint32_t)o.cell_ent.size() << 3 | (uint32_t)lst.size();
-                o.cell_ent.insert(o.cell_ent.end(), lst.begin(), lst.end());
-            }
-        if (o.cell_ent.size() >= (1u << 29)) throw Fail{PYJAC_ELIMIT, "cell list too long"};
+        o.n_spchunk = nchunk;
     }
-    if (o.cell_ent.empty()) o.cell_ent.push_back(0u);
-    if (o.long_ent.empty()) o.long_ent.push_back(0u);
-    if (o.sp_ent.empty()) o.sp_ent.push_back(0u);
-    if (o.col_ent.empty()) o.col_ent.push_back(0u);
+
+    // ---- cell tasks per column panel
+    o.ldt = (ns & 1) ? ns : ns + 1;
+    {
+        // shared memory that does not depend on the panel width (doubles), see make_smem_plan
+        const SmemPlan fixed = make_smem_plan(ns, nr, o.n_v, o.ldt, 0);
+        long long room = (long long)smem_budget / 8 - fixed.total;
+        int pw = ns;
+        if ((long long)o.ldt * ns > room) pw = (int)(room / o.ldt);
+        if (panel_override > 0) pw = std::min(ns, (ns + panel_override - 1) / panel_override);
+        if (pw < 1) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
+        if (pw < ns && pw > 8) pw &= ~3;
+        o.pw = pw;
+        o.n_panel = (ns + pw - 1) / pw;
+    }
+    const uint32_t pad_addr = (uint32_t)(o.ldt * o.pw);
+    for (int p = 0; p < o.n_panel; ++p) {
+        const int j0 = p * o.pw, j1 = std::min(ns, j0 + o.pw);
+        std::vector<std::pair<int, int>> tasks;   // (j, k) with a non-empty list, off the diagonal
+        for (int j = j0; j < j1; ++j)
+            for (int k = 0; k < ns; ++k)
+                if (k != j && !cell[(size_t)j * ns + k].empty()) tasks.push_back({j, k});
+        std::stable_sort(tasks.begin(), tasks.end(), [&](const std::pair<int, int> &a, const std::pair<int, int> &b) {
+            return cell[(size_t)a.first * ns + a.second].size() > cell[(size_t)b.first * ns + b.second].size();
+        });
+        o.panel_chunks.push_back((int32_t)(o.cchunk.size() / 2));
+        for (size_t t0 = 0; t0 < tasks.size(); t0 += 32) {
+            const int steps = (int)cell[(size_t)tasks[t0].first * ns + tasks[t0].second].size();
+            const uint32_t base = (uint32_t)o.c_ent.size();
+            o.cchunk.push_back(base);
+            o.cchunk.push_back((uint32_t)steps);
+            o.c_ent.resize(o.c_ent.size() + (size_t)steps * 32, zero_slot);
+            for (int lane = 0; lane < 32; ++lane) {
+                if (t0 + lane >= tasks.size()) { o.ctask_addr.push_back(pad_addr); continue; }
+                const int j = tasks[t0 + lane].first, k = tasks[t0 + lane].second;
+                o.ctask_addr.push_back((uint32_t)(k + (j - j0) * o.ldt));
+                const auto &lst = cell[(size_t)j * ns + k];
+                for (size_t e = 0; e < lst.size(); ++e) o.c_ent[(size_t)base + e * 32 + lane] = lst[e];
+            }
+        }
+        o.panel_chunks.push_back((int32_t)(o.cchunk.size() / 2));
+    }
+    if (o.c_ent.empty()) o.c_ent.push_back(zero_slot);
+    if (o.cchunk.empty()) { o.cchunk.push_back(0u); o.cchunk.push_back(0u); }
+    if (o.ctask_addr.empty()) o.ctask_addr.push_back(pad_addr);
+    if (o.sp_ent.empty()) { o.sp_ent.push_back((uint32_t)nr); o.sp_ent.push_back(zero_slot); }
 }
 
-int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const char **why)
+int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, size_t smem_budget, int panel_override,
+                   const char **why)
 {
     try {
-        pack_impl(d, out);
+        pack_impl(d, out, smem_budget, panel_override);
     } catch (const Fail &f) {
         if (why) *why = f.why;
         return f.code;

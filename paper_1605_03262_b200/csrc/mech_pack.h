@@ -22,12 +22,19 @@ struct HostPack {
     int pk_begin = 0, n_pk = 0;
     std::vector<int32_t> pk_ptr;
     std::vector<double> pk_data;
-    std::vector<int32_t> sp_ptr, col_ptr, long_ptr;
-    std::vector<uint32_t> sp_ent, col_ent, long_ent, cell_info, cell_ent;
-    int n_long = 0, n_v = 0, n_vext = 0, spns_base = 0;
+    int n_spchunk = 0;
+    std::vector<uint32_t> spchunk, sp_ent;      // uint2 pairs flattened
+    std::vector<int32_t> sptask_k;
+    int n_panel = 1, pw = 0, ldt = 0;
+    std::vector<int32_t> panel_chunks;          // int2 pairs flattened
+    std::vector<uint32_t> cchunk, ctask_addr, c_ent;
+    int n_v = 0;
 };
 
 // Returns PYJAC_OK, PYJAC_EINVAL or PYJAC_ELIMIT.  `why` (optional) receives a static message.
-int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const char **why);
+// smem_budget: bytes of shared memory one CTA may use (decides the column-panel width);
+// panel_override > 0 forces that many column panels (tuning).
+int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, size_t smem_budget, int panel_override,
+                   const char **why);
 
 }  // namespace pyjac
