@@ -20,6 +20,7 @@ struct pyjac_mech {
     DeviceMech dm{};
     SmemPlan plan{};
     int threads = 128;
+    int S = 1;                  // states per CTA iteration
     size_t smem[3] = {0, 0, 0}; // dynamic shared memory per level
     int ctas_per_sm[3] = {1, 1, 1};
     int n_sm = 1;
@@ -42,18 +43,22 @@ struct Uploader {
     }
 };
 
-int choose_threads(int ns, int nr)
+// Launch shape: S states per CTA iteration (as many as fit the shared memory, at most 4) and the
+// CTA size by the amount of per-state work.  PYJAC_THREADS / PYJAC_S override it (tuning hooks,
+// see DESIGN.md); a pair that is not instantiated or does not fit falls back to the default.
+void choose_shape(const SmemPlan &plan, int ns, int nr, size_t smem_max, int *threads, int *S)
 {
-    if (const char *e = std::getenv("PYJAC_THREADS")) {   // tuning hook, see DESIGN.md
-        int v = std::atoi(e);
-        if (v == 64 || v == 128 || v == 256 || v == 512 || v == 1024) return v;
-    }
+    auto fits = [&](int s) { return eval_smem_bytes(plan, s) <= smem_max; };
+    int s = fits(4) ? 4 : fits(2) ? 2 : 1;
     const int work = nr > ns ? nr : ns;
-    if (work <= 64) return 64;
-    if (work <= 400) return 128;
-    if (work <= 1000) return 256;
-    if (work <= 2500) return 512;
-    return 1024;
+    int nt = work <= 64 ? 128 : work <= 200 ? 256 : 512;
+    int es = 0, et = 0;
+    if (const char *e = std::getenv("PYJAC_S")) es = std::atoi(e);
+    if (const char *e = std::getenv("PYJAC_THREADS")) et = std::atoi(e);
+    if (es > 0 && fits(es) && eval_kernel_ptr(2, et > 0 ? et : nt, es)) s = es;
+    if (et > 0 && eval_kernel_ptr(2, et, s)) nt = et;
+    *threads = nt;
+    *S = s;
 }
 
 int check_eval_args(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
@@ -73,9 +78,10 @@ int launch(const pyjac_mech *m, int level, int64_t n, const double *T, const dou
     if (cudaGetDevice(&dev) != cudaSuccess) return PYJAC_ECUDA;
     if (dev != m->device && cudaSetDevice(m->device) != cudaSuccess) return PYJAC_ECUDA;
     long long cap = (long long)m->n_sm * m->ctas_per_sm[level];
-    int grid = (int)(n < cap ? n : cap);
-    cudaError_t e = launch_eval(level, m->threads, m->dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy, out,
-                                (cudaStream_t)stream);
+    const long long blocks = (n + m->S - 1) / m->S;
+    int grid = (int)(blocks < cap ? blocks : cap);
+    cudaError_t e = launch_eval(level, m->threads, m->S, m->dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy,
+                                out, (cudaStream_t)stream);
     if (dev != m->device) cudaSetDevice(dev);
     if (e != cudaSuccess) return PYJAC_ECUDA;
     g_launches.fetch_add(1, std::memory_order_relaxed);
@@ -96,7 +102,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     // device's limit is checked below
     int panels = 0;
     if (const char *e = std::getenv("PYJAC_PANELS")) panels = std::atoi(e);   // tuning hook, see DESIGN.md
-    int rc = pack_mechanism(d, hp, (size_t)227 * 1024, panels, &why);
+    int rc = pack_mechanism(d, hp, (size_t)227 * 1024 - eval_smem_bytes(SmemPlan{}, 0), panels, &why);
     if (rc != PYJAC_OK) return rc;
     pyjac_mech *m = new (std::nothrow) pyjac_mech();
     if (!m) return PYJAC_ENOMEM;
@@ -119,6 +125,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     Uploader up;
     try {
         up.add(&dm.mw, hp.mw); up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.dcol, hp.dcol);
+        up.add((const double **)&dm.colc, hp.colc); up.add(&dm.wrow, hp.wrow);
         up.add(&dm.nasa, hp.nasa); up.add(&dm.t_mid, hp.t_mid);
         up.add(&dm.lnA, hp.lnA); up.add(&dm.beta, hp.beta); up.add(&dm.Ta, hp.Ta);
         up.add((const uint32_t **)&dm.slots, hp.slots);
@@ -148,14 +155,14 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     if (rc == PYJAC_OK) {
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
         m->plan = make_smem_plan(hp.ns, hp.nr, hp.n_v, hp.ldt, hp.pw);
-        m->threads = choose_threads(hp.ns, hp.nr);
-        const size_t bytes = (size_t)m->plan.total * sizeof(double);
+        choose_shape(m->plan, hp.ns, hp.nr, (size_t)prop.sharedMemPerBlockOptin, &m->threads, &m->S);
+        const size_t bytes = eval_smem_bytes(m->plan, m->S);
         if (bytes > (size_t)prop.sharedMemPerBlockOptin) {
             rc = PYJAC_ELIMIT;
         } else {
             for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
                 m->smem[level] = bytes;
-                const void *k = eval_kernel_ptr(level, m->threads);
+                const void *k = eval_kernel_ptr(level, m->threads, m->S);
                 if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess ||
                     cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout,
                                          cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
@@ -236,7 +243,8 @@ int pyjac_jacobian_launch_config(const pyjac_mech *m, int64_t n, int32_t *thread
     if (smem_bytes) *smem_bytes = (int32_t)m->smem[2];
     if (ctas_per_sm) *ctas_per_sm = m->ctas_per_sm[2];
     long long cap = (long long)m->n_sm * m->ctas_per_sm[2];
-    if (grid) *grid = (int32_t)(n < cap ? n : cap);
+    const long long blocks = (n + m->S - 1) / m->S;
+    if (grid) *grid = (int32_t)(blocks < cap ? blocks : cap);
     return PYJAC_OK;
 }
 

@@ -43,6 +43,8 @@ struct DeviceMech {
     const double *mw;           // [ns]
     const double *inv_mw;       // [ns]
     const double *dcol;         // [ns] d_j = 1/W_j - 1/W_Ns  (the d rho / d Y_j factor, Eq. 51)
+    const double2 *colc;        // [ns] {d_j, 1/W_j}: the two column constants of phase 4
+    const double *wrow;         // [ns+2] row factors of phase 4: {1, W_0 .. W_{ns-1}, 1}
     const double *nasa;         // [2][7][ns]  range-major, coefficient-major (coalesced over k)
     const double *t_mid;        // [ns]
     // ---- reaction tables, sorted order
@@ -73,25 +75,28 @@ struct DeviceMech {
     const uint2 *sp_ent;        // {reaction (sorted) | coef16, V index | coef16}
     // ---- cell tasks: the off-diagonal cells (k, j) of the species block that collect at least
     // one reaction, per column panel, sorted by list length (descending); 32 tasks per chunk.
-    int n_panel, pw, ldt;       // panels of pw columns; tile leading dimension (odd)
+    int n_panel, pw, ldt;       // panels of pw columns; tile leading dimension (even, rows r = k + 1)
     const int2 *panel_chunks;   // [n_panel] {first chunk, one past last}
     const uint2 *cchunk;        // {first entry, steps}; entries at [first + step*32 + lane]
-    const uint32_t *ctask_addr; // [n_chunk*32] tile offset k + (j - j0)*ldt (pad: ldt*pw)
+    const uint32_t *ctask_addr; // [n_chunk*32] tile offset (k + 1) + (j - j0)*ldt (pad: ldt*pw)
     const uint32_t *c_ent;      // V index | coef16 (pad: zero slot n_v, coefficient 0)
     int n_v;                    // per-reaction derivative entries s'_ij; V[n_v] is a zero slot
 };
 
-// Shared-memory plan of one CTA (offsets in doubles).  Every array is per state.
+// Shared-memory plan of ONE state (offsets in doubles).  A CTA that evaluates S states at a time
+// holds S such blocks back to back (stride `total`).
 struct SmemPlan {
-    int X, B, dB, HW, Cp;               // [ns+1] species arrays (slot ns is the empty-slot dummy)
-    int Wdot, A, Tc, Diag, WA, WC;      // [ns+1]
+    int Sp4;                            // [ns+1][4] {[X_k], B_k, dB_k/dT, h_k W_k}; slot ns = {1, 0, 0, 0}
+    int Cp;                             // [ns+1] c_pk
+    int Wdot, A, Tc, Diag;              // [ns+1] indexed by species k
+    int WA, WC;                         // [ns+2] indexed by row r = k + 1; slot 0 is zero (energy row)
     int Ep;                             // [kEParts][ns+1] partial energy-row column sums
-    int Row0, Col0;                     // [ns+1]
+    int Col0;                           // [ns+1] column 0 (d/dT) by row
     int Q, Ar, Th;                      // [nr+1] (slot nr stays zero: padding of the gather lists)
     int V;                              // [n_v+1]
     int Tile;                           // [ldt*pw + 2]
-    int Red;                            // [8][32] reduction scratch
-    int total;                          // doubles
+    int Scal;                           // [16] per-state scalars, see kernels.cu
+    int total;                          // doubles per state
 };
 
 constexpr int kEParts = 4;
@@ -102,14 +107,14 @@ inline SmemPlan make_smem_plan(int ns, int nr, int n_v, int ldt, int pw)
     int o = 0;
     auto take = [&](int n) { int r = o; o += (n + 1) & ~1; return r; };
     const int s1 = ns + 1;
-    p.X = take(s1); p.B = take(s1); p.dB = take(s1); p.HW = take(s1); p.Cp = take(s1);
-    p.Wdot = take(s1); p.A = take(s1); p.Tc = take(s1); p.Diag = take(s1); p.WA = take(s1); p.WC = take(s1);
+    p.Sp4 = take(4 * s1); p.Cp = take(s1);
+    p.Wdot = take(s1); p.A = take(s1); p.Tc = take(s1); p.Diag = take(s1); p.WA = take(s1 + 1); p.WC = take(s1 + 1);
     p.Ep = take(kEParts * s1);
-    p.Row0 = take(s1); p.Col0 = take(s1);
+    p.Col0 = take(s1);
     p.Q = take(nr + 1); p.Ar = take(nr + 1); p.Th = take(nr + 1);
     p.V = take(n_v + 1);
     p.Tile = take(ldt * pw + 2);
-    p.Red = take(8 * 32);
+    p.Scal = take(16);
     p.total = o;
     return p;
 }

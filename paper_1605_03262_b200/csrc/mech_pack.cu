@@ -61,6 +61,10 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
         }
     }
     for (int k = 0; k < ns; ++k) o.dcol[k] = 1.0 / d->mol_wt[k] - 1.0 / d->mol_wt[ns - 1];
+    o.wrow.assign((size_t)ns + 2, 1.0);
+    for (int k = 0; k < ns; ++k) o.wrow[k + 1] = d->mol_wt[k];
+    o.colc.resize((size_t)2 * ns);
+    for (int k = 0; k < ns; ++k) { o.colc[2 * k] = o.dcol[k]; o.colc[2 * k + 1] = o.inv_mw[k]; }
 
     // ---- validate reactions and choose the sorted order
     std::vector<int> key(nr);
@@ -121,7 +125,13 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
         // group: elementary, PLOG, Chebyshev | third body, falloff forms (Lindemann, Troe, SRI)
         int group = t == PYJAC_ELEMENTARY ? 0 : t == PYJAC_PLOG ? 1 : t == PYJAC_CHEBYSHEV ? 2
                   : t == PYJAC_THIRD_BODY ? 3 : 4 + form;
-        key[i] = group * 4 + rv;
+        bool unit = true;
+        for (int q = d->reac_ptr[i]; q < d->reac_ptr[i + 1]; ++q) unit = unit && d->reac_nu[q] == 1;
+        for (int q = d->prod_ptr[i]; q < d->prod_ptr[i + 1]; ++q) unit = unit && d->prod_nu[q] == 1;
+        int neff = 0;
+        if (group >= 3) neff = d->tb_species[i] >= 0 ? 1 : d->eff_ptr[i + 1] - d->eff_ptr[i];
+        // warps evaluate one rate form, one stoichiometry path and equally long efficiency lists
+        key[i] = ((group * 2 + (unit ? 0 : 1)) * 4 + rv) * 64 + std::min(neff, 63);
     }
     std::vector<int> order(nr);
     std::iota(order.begin(), order.end(), 0);
@@ -301,7 +311,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
     }
 
     // ---- cell tasks per column panel
-    o.ldt = (ns & 1) ? ns : ns + 1;
+    o.ldt = (ns + 1 + 1) & ~1;                 // rows r = 0..ns (r = k + 1), even
+    if ((o.ldt & 3) == 0) o.ldt += 2;            // 2 (mod 4): 2-way instead of 4-way bank conflicts across columns
     {
         // shared memory that does not depend on the panel width (doubles), see make_smem_plan
         const SmemPlan fixed = make_smem_plan(ns, nr, o.n_v, o.ldt, 0);
@@ -334,7 +345,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
             for (int lane = 0; lane < 32; ++lane) {
                 if (t0 + lane >= tasks.size()) { o.ctask_addr.push_back(pad_addr); continue; }
                 const int j = tasks[t0 + lane].first, k = tasks[t0 + lane].second;
-                o.ctask_addr.push_back((uint32_t)(k + (j - j0) * o.ldt));
+                o.ctask_addr.push_back((uint32_t)(k + 1 + (j - j0) * o.ldt));
                 const auto &lst = cell[(size_t)j * ns + k];
                 for (size_t e = 0; e < lst.size(); ++e) o.c_ent[(size_t)base + e * 32 + lane] = lst[e];
             }

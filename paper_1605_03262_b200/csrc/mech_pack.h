@@ -9,7 +9,7 @@ namespace pyjac {
 
 struct HostPack {
     int ns = 0, nr = 0;
-    std::vector<double> mw, inv_mw, dcol, nasa, t_mid;
+    std::vector<double> mw, inv_mw, dcol, colc, wrow, nasa, t_mid;
     std::vector<double> lnA, beta, Ta, rev_lnA, rev_beta, rev_Ta;
     std::vector<uint32_t> slots;          // 4 words per reaction
     std::vector<uint32_t> vbase;
