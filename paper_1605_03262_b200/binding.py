@@ -40,7 +40,7 @@ class MechDesc(C.Structure):
 EXPORTS = ("pyjac_mech_create", "pyjac_mech_destroy", "pyjac_mech_sizes", "pyjac_eval_rates",
            "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
            "pyjac_eval_dydt_host", "pyjac_kernel_launches", "pyjac_jacobian_launch_config",
-           "pyjac_strerror")
+           "pyjac_pack_stats", "pyjac_strerror")
 
 _lib = None
 
@@ -67,6 +67,7 @@ def load_library(path: str | None = None):
     lib.pyjac_kernel_launches.argtypes = []
     lib.pyjac_kernel_launches.restype = i64
     lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 4
+    lib.pyjac_pack_stats.argtypes = [C.POINTER(MechDesc), C.POINTER(i64)]
     lib.pyjac_strerror.argtypes = [C.c_int]
     lib.pyjac_strerror.restype = C.c_char_p
     for name in EXPORTS:
@@ -110,6 +111,19 @@ def mech_desc(mech: Mechanism):
         keep.append(a)
         setattr(d, name, a.ctypes.data_as(_pi))
     return d, keep
+
+
+PACK_STAT_NAMES = ("e_doubles", "list_entries", "main_entry_slots", "aux_entry_slots", "main_tasks", "aux_chunks",
+                   "smem_bytes_one_state", "reaction_chunks")
+
+
+def pack_stats(mech: Mechanism) -> dict:
+    """Host-only: sizes of the evaluation tables `pyjac_mech_create` would build (no CUDA call)."""
+    lib = load_library()
+    d, keep = mech_desc(mech)
+    out = (C.c_int64 * 8)()
+    _check(lib.pyjac_pack_stats(C.byref(d), out), "pyjac_pack_stats")
+    return dict(zip(PACK_STAT_NAMES, [int(v) for v in out]))
 
 
 class PyJac:

@@ -24,6 +24,7 @@ struct pyjac_mech {
     size_t smem[3] = {0, 0, 0}; // dynamic shared memory per level
     int ctas_per_sm[3] = {1, 1, 1};
     int n_sm = 1;
+    long long stats[6] = {0, 0, 0, 0, 0, 0};
 };
 
 namespace {
@@ -43,15 +44,16 @@ struct Uploader {
     }
 };
 
-// Launch shape: S states per CTA iteration (as many as fit the shared memory, at most 4) and the
-// CTA size by the amount of per-state work.  PYJAC_THREADS / PYJAC_S override it (tuning hooks,
-// see DESIGN.md); a pair that is not instantiated or does not fit falls back to the default.
-void choose_shape(const SmemPlan &plan, int ns, int nr, size_t smem_max, int *threads, int *S)
+// Launch shape: S states per CTA iteration and the CTA size, by the shared memory one state needs
+// (several small CTAs per SM overlap each other's phases; large mechanisms get one large CTA).
+// PYJAC_THREADS / PYJAC_S override it (tuning hooks); a pair that is not
+// instantiated or does not fit falls back to the default.
+void choose_shape(const SmemPlan &plan, size_t smem_max, int *threads, int *S)
 {
     auto fits = [&](int s) { return eval_smem_bytes(plan, s) <= smem_max; };
-    int s = fits(4) ? 4 : fits(2) ? 2 : 1;
-    const int work = nr > ns ? nr : ns;
-    int nt = work <= 64 ? 128 : work <= 200 ? 256 : 512;
+    const size_t one = eval_smem_bytes(plan, 1);
+    int s = (fits(2) && 2 * one <= smem_max / 2) ? 2 : 1;
+    int nt = one <= 48 * 1024 ? 128 : one <= 110 * 1024 ? 256 : 512;
     int es = 0, et = 0;
     if (const char *e = std::getenv("PYJAC_S")) es = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_THREADS")) et = std::atoi(e);
@@ -98,11 +100,10 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     *out = nullptr;
     HostPack hp;
     const char *why = nullptr;
-    // validate first (no CUDA call yet), with the architecture's shared-memory size; the real
-    // device's limit is checked below
-    int panels = 0;
-    if (const char *e = std::getenv("PYJAC_PANELS")) panels = std::atoi(e);   // tuning hook, see DESIGN.md
-    int rc = pack_mechanism(d, hp, (size_t)227 * 1024 - eval_smem_bytes(SmemPlan{}, 0), panels, &why);
+    // validate and pack first (no CUDA call yet), with the architecture's shared-memory size; the
+    // real device's limit is checked below
+    const long long e_doubles = (long long)((size_t)227 * 1024 - 64 - eval_smem_bytes(make_smem_plan(d ? d->n_species : 1, 0), 1)) / 8;
+    int rc = pack_mechanism(d, hp, e_doubles, &why);
     if (rc != PYJAC_OK) return rc;
     pyjac_mech *m = new (std::nothrow) pyjac_mech();
     if (!m) return PYJAC_ENOMEM;
@@ -119,28 +120,28 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     m->n_sm = prop.multiProcessorCount;
     DeviceMech &dm = m->dm;
     dm.ns = hp.ns; dm.nr = hp.nr; dm.ld = hp.ns + 1;
-    dm.ln_patm_over_R = std::log(kPatm / kRu);
-    dm.pd_begin = hp.pd_begin; dm.n_pd = hp.n_pd; dm.pk_begin = hp.pk_begin; dm.n_pk = hp.n_pk;
-    dm.n_spchunk = hp.n_spchunk; dm.n_panel = hp.n_panel; dm.pw = hp.pw; dm.ldt = hp.ldt; dm.n_v = hp.n_v;
+    dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk;
+    dm.n_achunk = hp.n_achunk; dm.n_achunk01 = hp.n_achunk01; dm.n_mtask = hp.n_mtask;
+    dm.eQ = hp.eQ; dm.eAr = hp.eAr; dm.eTh = hp.eTh; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;
+    dm.eWdot = hp.eWdot; dm.eS1 = hp.eS1; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.n_e = hp.n_e;
     Uploader up;
     try {
-        up.add(&dm.mw, hp.mw); up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.dcol, hp.dcol);
+        up.add(&dm.inv_mw, hp.inv_mw);
         up.add((const double **)&dm.colc, hp.colc); up.add(&dm.wrow, hp.wrow);
         up.add(&dm.nasa, hp.nasa); up.add(&dm.t_mid, hp.t_mid);
-        up.add(&dm.lnA, hp.lnA); up.add(&dm.beta, hp.beta); up.add(&dm.Ta, hp.Ta);
         up.add((const uint32_t **)&dm.slots, hp.slots);
+        up.add(&dm.lnA, hp.lnA); up.add(&dm.beta, hp.beta); up.add(&dm.Ta, hp.Ta);
         up.add(&dm.vbase, hp.vbase); up.add(&dm.rxn_orig, hp.rxn_orig);
         up.add(&dm.rev_lnA, hp.rev_lnA); up.add(&dm.rev_beta, hp.rev_beta); up.add(&dm.rev_Ta, hp.rev_Ta);
+        up.add(&dm.th_off, hp.th_off); up.add(&dm.th_data, hp.th_data);
         up.add(&dm.lo_lnA, hp.lo_lnA); up.add(&dm.lo_beta, hp.lo_beta); up.add(&dm.lo_Ta, hp.lo_Ta);
-        up.add(&dm.fall_par, hp.fall_par); up.add(&dm.tb_spec, hp.tb_spec);
+        up.add(&dm.fall_par, hp.fall_par);
         up.add(&dm.eff_ptr, hp.eff_ptr); up.add(&dm.eff_spec, hp.eff_spec); up.add(&dm.eff_eps, hp.eff_eps);
         up.add(&dm.eff_vbase, hp.eff_vbase);
         up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
-        up.add((const uint32_t **)&dm.spchunk, hp.spchunk); up.add(&dm.sptask_k, hp.sptask_k);
-        up.add((const uint32_t **)&dm.sp_ent, hp.sp_ent);
-        up.add((const int32_t **)&dm.panel_chunks, hp.panel_chunks);
-        up.add((const uint32_t **)&dm.cchunk, hp.cchunk); up.add(&dm.ctask_addr, hp.ctask_addr);
-        up.add(&dm.c_ent, hp.c_ent);
+        up.add((const uint32_t **)&dm.achunk, hp.achunk); up.add(&dm.a_ent, hp.a_ent);
+        up.add(&dm.a_out, hp.a_out); up.add(&dm.a_const, hp.a_const);
+        up.add((const uint32_t **)&dm.mtask, hp.mtask); up.add(&dm.m_ent, hp.m_ent);
     } catch (...) {
         delete m;
         cudaSetDevice(prev);
@@ -154,10 +155,12 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     }
     if (rc == PYJAC_OK) {
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
-        m->plan = make_smem_plan(hp.ns, hp.nr, hp.n_v, hp.ldt, hp.pw);
-        choose_shape(m->plan, hp.ns, hp.nr, (size_t)prop.sharedMemPerBlockOptin, &m->threads, &m->S);
+        m->plan = make_smem_plan(hp.ns, hp.n_e);
+        choose_shape(m->plan, (size_t)prop.sharedMemPerBlockOptin - 64, &m->threads, &m->S);
+        m->stats[0] = hp.n_e; m->stats[1] = hp.n_list_entries; m->stats[2] = hp.n_main_entries;
+        m->stats[3] = hp.n_aux_entries; m->stats[4] = hp.n_mtask; m->stats[5] = hp.n_achunk;
         const size_t bytes = eval_smem_bytes(m->plan, m->S);
-        if (bytes > (size_t)prop.sharedMemPerBlockOptin) {
+        if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin) {
             rc = PYJAC_ELIMIT;
         } else {
             for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
@@ -245,6 +248,19 @@ int pyjac_jacobian_launch_config(const pyjac_mech *m, int64_t n, int32_t *thread
     long long cap = (long long)m->n_sm * m->ctas_per_sm[2];
     const long long blocks = (n + m->S - 1) / m->S;
     if (grid) *grid = (int32_t)(blocks < cap ? blocks : cap);
+    return PYJAC_OK;
+}
+
+int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
+{
+    if (!stats) return PYJAC_EINVAL;
+    HostPack hp;
+    const long long e_doubles = (long long)((size_t)227 * 1024 - 64 - eval_smem_bytes(make_smem_plan(d ? d->n_species : 1, 0), 1)) / 8;
+    const int rc = pack_mechanism(d, hp, e_doubles, nullptr);
+    if (rc != PYJAC_OK) return rc;
+    const SmemPlan plan = make_smem_plan(hp.ns, hp.n_e);
+    stats[0] = hp.n_e; stats[1] = hp.n_list_entries; stats[2] = hp.n_main_entries; stats[3] = hp.n_aux_entries;
+    stats[4] = hp.n_mtask; stats[5] = hp.n_achunk; stats[6] = (int64_t)eval_smem_bytes(plan, 1); stats[7] = hp.n_rchunk;
     return PYJAC_OK;
 }
 

@@ -1,10 +1,19 @@
-// device_mech.h -- device-resident SoA tables of one kinetic model and the shared-memory plan of
-// the evaluation kernels.  Built by mech_pack.cpp (host), consumed by kernels.cu (device).
+// device_mech.h -- device-resident tables of one kinetic model and the shared-memory plan of the
+// evaluation kernels.  Built by mech_pack.cu (host), consumed by kernels.cu (device).
 //
 // Notation follows the paper (PAPER.md Sections 2-4): species k, reaction i, nu' / nu'' the
 // reactant / product coefficients (Eq. 15), [X_k] concentrations (Eq. 5), c_i the pressure
-// modification (Eq. 20).  Reactions are stored in a SORTED order (grouped by type so that a warp
-// evaluates one rate form); `rxn_orig` maps back to the caller's order.
+// modification (Eq. 20).  Reactions are stored in a SORTED order (most expensive rate form first,
+// one form per group of 32); `rxn_orig` maps back to the caller's order.
+//
+// The evaluation is a chain of gathers over one per-state array `E` in shared memory:
+//   phase 1 writes, per reaction, the reusable products of Section 4.1:
+//           the sparse derivative terms s'_ij (region V), q_i, a_i, Theta_dT,i and the reaction
+//           enthalpy H_i (regions Q, Ar, Th, H);
+//   the AUX gathers sum them into per-species / per-column quantities (regions Alpha, Gamma, Wdot,
+//           the scalars S1, S4 and the sums of the long cell lists, region Ovf);
+//   the MAIN pass owns the Jacobian as a flat array: lane <-> one output element, which gathers
+//           its (short) list from E, applies Eq. 112 / 113 and stores -- there is no Jacobian tile.
 #pragma once
 #include <cstdint>
 
@@ -13,7 +22,7 @@ namespace pyjac {
 constexpr double kRu = 8314.46261815324;   // J kmol^-1 K^-1
 constexpr double kPatm = 101325.0;         // Pa
 constexpr int kMaxSide = 3;                // species per reaction side
-constexpr int kSpLanes = 4;                // lanes that share one species task
+constexpr int kVStride = 32;               // V entries of one reaction are 32 apart (lane-contiguous stores)
 
 // meta word of a reaction: bits 0..23 six 4-bit nu (slots 0-2 reactants, 3-5 products; 0 = empty
 // slot), 24..26 rxn_type, 27..28 rev_type, 29..30 falloff_form, 31 third body is a single species.
@@ -23,11 +32,10 @@ __host__ __device__ inline int meta_rev(uint32_t m) { return (m >> 27) & 3; }
 __host__ __device__ inline int meta_form(uint32_t m) { return (m >> 29) & 3; }
 __host__ __device__ inline int meta_single(uint32_t m) { return (m >> 31) & 1; }
 
-// A gather entry: low 16 bits = source index, high 16 bits = the top 16 bits of the fp64
-// coefficient (exact for +-1, +-2, +-3: the only stoichiometric factors that occur).
+// A gather entry: low 16 bits = index into E, high 16 bits = the top 16 bits of the fp64
+// coefficient (exact for the small integers that occur as stoichiometric factors).
 __host__ __device__ inline uint32_t pack_entry(uint32_t src, int coef)
 {
-    // 1.0 = 0x3FF0.., 2.0 = 0x4000.., 3.0 = 0x4008..; sign in bit 15
     uint32_t a = coef < 0 ? uint32_t(-coef) : uint32_t(coef);
     uint32_t hi = a == 1 ? 0x3FF0u : a == 2 ? 0x4000u : a == 3 ? 0x4008u
                 : a == 4 ? 0x4010u : a == 5 ? 0x4014u : a == 6 ? 0x4018u : 0u;
@@ -35,88 +43,95 @@ __host__ __device__ inline uint32_t pack_entry(uint32_t src, int coef)
     return (hi << 16) | (src & 0xFFFFu);
 }
 
+// aux chunk flags (AuxChunk.z)
+enum : uint32_t {
+    kAuxTwoIndex = 1u,   // entries are {index a | index b << 16}: sum of E[a] * E[b]
+    kAuxReduce = 2u,     // the 32 lanes hold parts of ONE sum: butterfly, lane 0 stores to slot w
+    kAuxScaled = 4u,     // result *= task constant * per-state scalar (index in bits 8..15)
+};
+
 struct DeviceMech {
     int ns, nr;                 // N_sp, N_reac
     int ld;                     // N_sp + 1
-    double ln_patm_over_R;      // ln(p_atm / R) of Eq. 26
     // ---- species tables
-    const double *mw;           // [ns]
     const double *inv_mw;       // [ns]
-    const double *dcol;         // [ns] d_j = 1/W_j - 1/W_Ns  (the d rho / d Y_j factor, Eq. 51)
-    const double2 *colc;        // [ns] {d_j, 1/W_j}: the two column constants of phase 4
-    const double *wrow;         // [ns+2] row factors of phase 4: {1, W_0 .. W_{ns-1}, 1}
-    const double *nasa;         // [2][7][ns]  range-major, coefficient-major (coalesced over k)
+    const double2 *colc;        // [ns+1] column constants by Jacobian column c: {d_j, 1/W_j}, j = c - 1;
+                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51); c = 0: {0, 1}
+    const double *wrow;         // [ns+1] row factors by Jacobian row r: {1, W_0 .. W_{ns-1}}
+    const double *nasa;         // [2][5][ns] a_0..a_4, range-major, coefficient-major (coalesced over k)
     const double *t_mid;        // [ns]
     // ---- reaction tables, sorted order
-    const double *lnA, *beta, *Ta;        // [nr] forward Arrhenius (k_inf for falloff forms)
-    const uint4 *slots;                   // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
-    const uint32_t *vbase;                // [nr] first V entry (reactant slots, then product slots)
-    const int32_t *rxn_orig;              // [nr] caller's reaction index
+    int n_pd;                   // pressure-dependent reactions (third body, falloff, chem. activated): [0, n_pd)
+    int n_pk;                   // PLOG / Chebyshev reactions: [n_pd, n_pd + n_pk)
+    const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
+    const double *lnA, *beta, *Ta;               // [nr] forward Arrhenius (k_inf for falloff forms)
+    const uint32_t *vbase;      // [nr] E index of the first used slot's s'_ij; the n-th used slot is n*kVStride further
+    const int32_t *rxn_orig;    // [nr] caller's reaction index
     const double *rev_lnA, *rev_beta, *rev_Ta;   // [nr] explicit reverse parameters
-    // pressure-dependent reactions occupy sorted indices [pd_begin, nr); tables indexed by s - pd_begin
-    int pd_begin, n_pd;
+    const uint32_t *th_off;     // [nr] offset into th_data
+    const double *th_data;      // per reaction: n_int, (n_int - 1) ascending breakpoints, n_int x {g_0..g_6}:
+                                // sum_k nu_ki B_k(T) = g0 + g1 ln T + T (g2 + T (g3 + T (g4 + T g5))) + g6 / T
+                                // (Eq. 27 summed over the reaction, one set per interval between the t_mid of
+                                // its species; g0 includes (sum nu) ln(p_atm / R) of Eq. 26)
     const double *lo_lnA, *lo_beta, *lo_Ta;      // [n_pd] k_0
     const double *fall_par;                      // [n_pd][5]
-    const int32_t *tb_spec;                      // [n_pd] single species or -1
     const int32_t *eff_ptr;                      // [n_pd+1]
     const int32_t *eff_spec;                     // species of alpha_ij != 1 (or the single species)
     const double *eff_eps;                       // alpha_ij - 1      (1 for the single species)
-    const uint32_t *eff_vbase;                   // [n_pd] first V entry of the efficiency terms
-    // PLOG / Chebyshev reactions occupy sorted indices [pk_begin, pk_begin + n_pk)
-    int pk_begin, n_pk;
+    const uint32_t *eff_vbase;                   // [n_pd] E index of the first efficiency term (stride kVStride)
     const int32_t *pk_ptr;      // [n_pk+1] offsets into pk_data
     const double *pk_data;      // PLOG: n, then n x {p, ln p, ln A, beta, Ta};
                                 // Chebyshev: nT, nP, 1/Tmin, 1/Tmax, log10 pmin, log10 pmax, eta[nT*nP]
-    // ---- species tasks: wdot_k, A_k, Tcol_k and the diagonal cell (k, k) are sums over the
-    // reactions that contain k.  kSpLanes lanes share one species; a chunk is 32 / kSpLanes species.
-    int n_spchunk;
-    const uint2 *spchunk;       // [n_spchunk] {first entry, steps}; entries at [first + step*32 + lane]
-    const int32_t *sptask_k;    // [n_spchunk * 32 / kSpLanes] species or -1
-    const uint2 *sp_ent;        // {reaction (sorted) | coef16, V index | coef16}
-    // ---- cell tasks: the off-diagonal cells (k, j) of the species block that collect at least
-    // one reaction, per column panel, sorted by list length (descending); 32 tasks per chunk.
-    int n_panel, pw, ldt;       // panels of pw columns; tile leading dimension (even, rows r = k + 1)
-    const int2 *panel_chunks;   // [n_panel] {first chunk, one past last}
-    const uint2 *cchunk;        // {first entry, steps}; entries at [first + step*32 + lane]
-    const uint32_t *ctask_addr; // [n_chunk*32] tile offset (k + 1) + (j - j0)*ldt (pad: ldt*pw)
-    const uint32_t *c_ent;      // V index | coef16 (pad: zero slot n_v, coefficient 0)
-    int n_v;                    // per-reaction derivative entries s'_ij; V[n_v] is a zero slot
+    int n_rchunk;               // groups of 32 reactions
+    // ---- AUX gathers: chunks of 32 tasks with equally long lists (sorted at create time)
+    int n_achunk;               // all chunks (Jacobian); the first n_achunk01 serve rates / dydt too
+    int n_achunk01;
+    const uint4 *achunk;        // {first entry, steps, flags | scalar << 8, REDUCE: E slot; else first task}
+    const uint32_t *a_ent;      // entries at [first + step*32 + lane]
+    const uint32_t *a_out;      // [task] E slot of the result
+    const double *a_const;      // [task] constant factor of scaled tasks
+    // ---- MAIN pass: the Jacobian as a flat column-major array, 32 consecutive elements per task
+    int n_mtask;
+    const uint4 *mtask;         // {first entry, steps, row of lane 0, column of lane 0}
+    const uint32_t *m_ent;      // entries at [first + step*32 + lane]
+    // ---- regions of E (indices in doubles per state)
+    int eQ, eAr, eTh, eH;       // [nr] each
+    int eAlpha, eGamma;         // [ns+1] by Jacobian row
+    int eWdot;                  // [ns]
+    int eS1, eS4;               // scalars: sum_i H_i q_i, sum_i H_i Theta_i
+    int eZero;                  // a slot that stays 0 (padding of the lists)
+    int n_e;                    // size of E
 };
 
-// Shared-memory plan of ONE state (offsets in doubles).  A CTA that evaluates S states at a time
-// holds S such blocks back to back (stride `total`).
+// per-state scalars (region Scal of the shared-memory plan)
+enum {
+    kOne = 0, kIrho, kNegIcp, kNegIrhoIcp,          // factors of the scaled AUX tasks (kOne stays 1)
+    kT, kLnT, kInvT, kP, kRho, kW, kM, kCpMix, kDcpDT, kNScal = 16
+};
+
+// Shared-memory plan (offsets in doubles PER STATE).  A CTA evaluates S states at a time and
+// interleaves them: element i of region R of state q lives at (R + i) * S + q.
 struct SmemPlan {
-    int Sp4;                            // [ns+1][4] {[X_k], B_k, dB_k/dT, h_k W_k}; slot ns = {1, 0, 0, 0}
-    int Cp;                             // [ns+1] c_pk
-    int Wdot, A, Tc, Diag;              // [ns+1] indexed by species k
-    int WA, WC;                         // [ns+2] indexed by row r = k + 1; slot 0 is zero (energy row)
-    int Ep;                             // [kEParts][ns+1] partial energy-row column sums
-    int Col0;                           // [ns+1] column 0 (d/dT) by row
-    int Q, Ar, Th;                      // [nr+1] (slot nr stays zero: padding of the gather lists)
-    int V;                              // [n_v+1]
-    int Tile;                           // [ldt*pw + 2]
-    int Scal;                           // [16] per-state scalars, see kernels.cu
+    int E;                              // [n_e]
+    int X;                              // [ns+1] concentrations; slot ns = 1 (empty reaction slots)
+    int Cp;                             // [ns] c_pk (mass based)
+    int Scal;                           // [2][kNScal], double-buffered by iteration parity
     int total;                          // doubles per state
 };
 
-constexpr int kEParts = 4;
-
-inline SmemPlan make_smem_plan(int ns, int nr, int n_v, int ldt, int pw)
+inline SmemPlan make_smem_plan(int ns, int n_e)
 {
     SmemPlan p{};
     int o = 0;
     auto take = [&](int n) { int r = o; o += (n + 1) & ~1; return r; };
-    const int s1 = ns + 1;
-    p.Sp4 = take(4 * s1); p.Cp = take(s1);
-    p.Wdot = take(s1); p.A = take(s1); p.Tc = take(s1); p.Diag = take(s1); p.WA = take(s1 + 1); p.WC = take(s1 + 1);
-    p.Ep = take(kEParts * s1);
-    p.Col0 = take(s1);
-    p.Q = take(nr + 1); p.Ar = take(nr + 1); p.Th = take(nr + 1);
-    p.V = take(n_v + 1);
-    p.Tile = take(ldt * pw + 2);
-    p.Scal = take(16);
+    p.E = take(n_e);
+    p.X = take(ns + 1);
+    p.Cp = take(ns);
+    p.Scal = take(2 * kNScal);
     p.total = o;
     return p;
 }
+
+constexpr int kRedRows = 4;             // block-reduction scratch: kRedRows x 32 doubles per state
 
 }  // namespace pyjac

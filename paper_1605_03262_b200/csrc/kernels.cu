@@ -1,22 +1,23 @@
 // kernels.cu -- sm_100a kernels for the batched source term and analytical Jacobian.
 //
-// One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop, each
-// state in its own block of shared memory.  Whatever does not depend on the state -- decoding a
-// reaction, a gather-list entry, a column constant -- is done once and applied to the S states.
-// Per iteration:
-//   phase 0  species: [X_k] (Eq. 5), NASA-7 c_pk, h_k W_k, B_k, dB_k/dT (Eqs. 9-12, 27, 74)
-//   phase 1  reactions (one thread per reaction, sorted by type): k_f, k_r, R_f, R_r, c_i and the
-//            reusable per-reaction products of Section 4.1: q_i, Theta_dT,i,
-//            the d_j-proportional coefficient a_i and the sparse terms s'_ij
-//   phase 2  fixed-order gathers: wdot_k, A_k, T-column sums and diagonal cells (kSpLanes lanes per
-//            species); off-diagonal cells of the species block into a shared-memory tile, lists
-//            sorted by length so that the 32 lanes of a warp run the same number of steps
-//   phase 3  species finalisation + block reductions (dT/dt, energy row of Eq. 113)
-//   phase 4  dense write-out, one coalesced column segment per warp: each element is
-//            W_k ( A_k/rho d_j + sum_i nu_ki s'_ij / W_j - sum_i nu_ki s'_iNs / W_Ns )
+// One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop; the S
+// states are interleaved in shared memory (element i of a region for state q at (R + i) * S + q), so
+// whatever does not depend on the state -- decoding a reaction, a gather entry, a column constant --
+// is done once and applied to the S states with one vector load.  Per iteration:
+//   phase 0  mixture (Eqs. 3-5) and species: [X_k], c_pk, mixture c_p and d c_p / dT (Eqs. 9-13, 54-55)
+//   phase 1  reactions, one thread per reaction, groups of 32 of one rate form taken from a queue:
+//            k_f, k_r (K_c from the per-reaction polynomial of device_mech.h `th_data`), R_f, R_r, c_i
+//            and the reusable per-reaction products of Section 4.1 into E:
+//            q_i, Theta_dT,i, a_i (the coefficient of d_j), the sparse terms s'_ij, the enthalpy H_i
+//   AUX      fixed-order gathers over E, 32 equally long lists per warp: wdot_k (Eq. 14), the row
+//            vectors alpha_r, gamma_r of Eq. 112, the column sums of the energy row (Eq. 113) and the
+//            sums of the long Jacobian cell lists
+//   MAIN     the Jacobian as a flat column-major array: lane <-> output element.  Each element
+//            gathers its short list from E and is stored straight from the register:
+//              J(r, c) = alpha_r d_j + (W_k / W_j) sum_i nu_ki s'_ij - gamma_r        (r = k+1, c = j+1)
 //            which is Eq. 112 with the per-reaction terms of Eqs. 118-127 regrouped by what they
-//            multiply.
-// There are no atomics: every sum has an order fixed at pyjac_mech_create.
+//            multiply.  A warp stores 256 contiguous bytes.
+// There are no atomics on data and no Jacobian tile: every sum has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
 
 #include "device_mech.h"
@@ -28,9 +29,6 @@ namespace {
 
 constexpr double kLn10 = 2.302585092994045684;
 constexpr double kInvLn10 = 0.434294481903251828;
-
-// indices into the per-state scalar block
-enum { kT = 0, kLnT, kInvT, kP, kRho, kW, kM, kCpMix, kDcpDT, kIrho };
 
 __device__ __forceinline__ double entry_coef(uint32_t e) { return __hiloint2double((int)(e & 0xFFFF0000u), 0); }
 
@@ -79,42 +77,64 @@ __device__ __forceinline__ void int_pow(double x, int nu, double &p, double &pm)
     pm = nu == 0 ? 0.0 : nu == 1 ? 1.0 : nu == 2 ? 2.0 * x : 3.0 * x2;
 }
 
-// deterministic block reduction of NV values over the first `nwa` warps (the others hold zeros):
-// xor-butterfly inside the warp, one partial per warp into `red` (NV rows of 32 doubles); after a
-// __syncthreads, red_sum adds the partials of one row in warp order -- only the threads that need a
-// sum pay for it.
-template <int NV>
-__device__ __forceinline__ void block_partials(double (&v)[NV], double *red, int lane, int warp, int nwa)
+__device__ __forceinline__ double warp_sum(double v)
 {
-    if (warp < nwa) {
 #pragma unroll
-        for (int q = 0; q < NV; ++q) {
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    return v;
+}
+
+// the S interleaved values of one element: one vector load / store
+template <int S>
+__device__ __forceinline__ void ldv(const double *p, double (&v)[S])
+{
+    if (S == 2) {
+        const double2 t = *reinterpret_cast<const double2 *>(p);
+        v[0] = t.x; v[1] = t.y;
+    } else if (S == 4) {
+        const double2 t = *reinterpret_cast<const double2 *>(p), u = *reinterpret_cast<const double2 *>(p + 2);
+        v[0] = t.x; v[1] = t.y; v[2] = u.x; v[3] = u.y;
+    } else {
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xFFFFFFFFu, v[q], o);
-            if (lane == 0) red[q * 32 + warp] = v[q];
-        }
+        for (int q = 0; q < S; ++q) v[q] = p[q];
     }
 }
-__device__ __forceinline__ double red_sum(const double *red, int row, int nwa)
+template <int S>
+__device__ __forceinline__ void stv(double *p, const double (&v)[S])
 {
-    double s = red[row * 32];
-    for (int w = 1; w < nwa; ++w) s += red[row * 32 + w];
-    return s;
+    if (S == 2) {
+        *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]);
+    } else if (S == 4) {
+        *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]);
+        *reinterpret_cast<double2 *>(p + 2) = make_double2(v[2], v[3]);
+    } else {
+#pragma unroll
+        for (int q = 0; q < S; ++q) p[q] = v[q];
+    }
+}
+
+// next item of a phase's work queue (one shared counter per phase)
+__device__ __forceinline__ int grab(int *ctr, int lane)
+{
+    int t = 0;
+    if (lane == 0) t = atomicAdd(ctr, 1);
+    return __shfl_sync(0xFFFFFFFFu, t, 0);
 }
 
 // ---- phase 1: one reaction, S states --------------------------------------------------------------
 // Everything that does not depend on the state (slot decoding, Arrhenius parameters, table
-// pointers) is read once; the loop over the S states of the CTA is inside.
+// pointers) is read once; the loop over the S states of the CTA is inside.  `sm` is the CTA's
+// shared memory, `sc` the scalar block of this iteration.
 template <int LEVEL, int S>
-__device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *sm0, int SS, int s,
-                                         const EvalOut &out, long long state0, long long n)
+__device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *sm, const double *sc,
+                                         int s, const EvalOut &out, long long state0, long long n)
 {
     const uint4 sl = m.slots[s];
     const uint32_t meta = sl.w;
     const int type = meta_type(meta), rev = meta_rev(meta);
-    // offsets of the species blocks {X, B, dB, hW}
-    const int sp0 = (sl.x & 0xFFFF) * 4, sp1 = (sl.x >> 16) * 4, sp2 = (sl.y & 0xFFFF) * 4,
-              sp3 = (sl.y >> 16) * 4, sp4 = (sl.z & 0xFFFF) * 4, sp5 = (sl.z >> 16) * 4;
+    const double *X = sm + sp.X * S;
+    const int x0 = (sl.x & 0xFFFF) * S, x1 = (sl.x >> 16) * S, x2 = (sl.y & 0xFFFF) * S,
+              x3 = (sl.y >> 16) * S, x4 = (sl.z & 0xFFFF) * S, x5 = (sl.z >> 16) * S;
     const bool unit_nu = (meta & 0x00EEEEEEu) == 0;          // every nu is 0 or 1
     const int snu_f = meta_nu(meta, 0) + meta_nu(meta, 1) + meta_nu(meta, 2);
     const int snu_r = meta_nu(meta, 3) + meta_nu(meta, 4) + meta_nu(meta, 5);
@@ -122,14 +142,14 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     const bool arrh = type != PYJAC_PLOG && type != PYJAC_CHEBYSHEV;
     double lnA = 0.0, beta = 0.0, Ta = 0.0;
     if (arrh) { lnA = m.lnA[s]; beta = m.beta[s]; Ta = m.Ta[s]; }
-    const double dnu_lnc = (double)(snu_r - snu_f) * m.ln_patm_over_R;
-    const uint32_t vb = LEVEL == 2 ? m.vbase[s] : 0u;
+    const double dnu = (double)(snu_r - snu_f);
+    const double *th = m.th_data + m.th_off[s];
+    const int nint = (int)th[0];
+    double *E = sm + sp.E * S;
 
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
-        double *sm = sm0 + q * SS;
-        const double *S4 = sm + sp.Sp4;
-        const double T = sm[sp.Scal + kT], lnT = sm[sp.Scal + kLnT], invT = sm[sp.Scal + kInvT];
+        const double T = sc[kT * S + q], lnT = sc[kLnT * S + q], invT = sc[kInvT * S + q];
 
         // ---- forward rate coefficient: ln k_f and L = d ln k_f / dT
         double lnkf, L;
@@ -139,15 +159,14 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             lnkf = lnkinf;
             L = (beta + Ta * invT) * invT;                          // Eq. 65
             if (type == PYJAC_FALLOFF || type == PYJAC_CHEM_ACTIVATED) {
-                const int pd = s - m.pd_begin;
-                const double b0 = m.lo_beta[pd], Ta0 = m.lo_Ta[pd];
-                lnk0 = m.lo_lnA[pd] + b0 * lnT - Ta0 * invT;
+                const double b0 = m.lo_beta[s], Ta0 = m.lo_Ta[s];
+                lnk0 = m.lo_lnA[s] + b0 * lnT - Ta0 * invT;
                 lPrT = invT * (b0 - beta + (Ta0 - Ta) * invT - 1.0);   // Eq. 84 / P_r
                 if (type == PYJAC_CHEM_ACTIVATED) { lnkf = lnk0; L = (b0 + Ta0 * invT) * invT; }
             }
         } else if (type == PYJAC_PLOG) {                            // Eqs. 37-39, 105
-            const double P = sm[sp.Scal + kP];
-            const double *pk = m.pk_data + m.pk_ptr[s - m.pk_begin];
+            const double P = sc[kP * S + q];
+            const double *pk = m.pk_data + m.pk_ptr[s - m.n_pd];
             const int np = (int)pk[0];
             const double *row = pk + 1;                              // {p, ln p, ln A, beta, Ta}
             int lo = 0, hi = 0;
@@ -168,8 +187,8 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             lnkf = lnk1 + (lnk2 - lnk1) * wt;
             L = (a1[3] + a1[4] * invT + (a2[3] - a1[3] + (a2[4] - a1[4]) * invT) * wt) * invT;
         } else {                                                    // Chebyshev, Eqs. 40-43, 110
-            const double P = sm[sp.Scal + kP];
-            const double *pk = m.pk_data + m.pk_ptr[s - m.pk_begin];
+            const double P = sc[kP * S + q];
+            const double *pk = m.pk_data + m.pk_ptr[s - m.n_pd];
             const int nT = (int)pk[0], nP = (int)pk[1];
             const double iTmin = pk[2], iTmax = pk[3], lpmin = pk[4], lpmax = pk[5];
             const double *eta = pk + 6;
@@ -201,44 +220,41 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         }
         const double kf = exp_rate(lnkf);
 
-        // ---- species data of the six slots (empty slots point at the dummy species {1, 0, 0, 0})
-        const double2 xb0 = *reinterpret_cast<const double2 *>(S4 + sp0);
-        const double2 xb1 = *reinterpret_cast<const double2 *>(S4 + sp1);
-        const double2 xb2 = *reinterpret_cast<const double2 *>(S4 + sp2);
-        const double2 xb3 = *reinterpret_cast<const double2 *>(S4 + sp3);
-        const double2 xb4 = *reinterpret_cast<const double2 *>(S4 + sp4);
-        const double2 xb5 = *reinterpret_cast<const double2 *>(S4 + sp5);
+        // ---- sum_k nu_ki B_k (Eq. 27 over the reaction), its T derivative (Eq. 74) and the reaction
+        //      enthalpy H_i = sum_k nu_ki h_k W_k = R T (T d(sum nu B)/dT + sum nu)
+        int iv = 0;
+        for (int b = 1; b < nint; ++b) iv += T > th[b] ? 1 : 0;
+        const double *g = th + nint + 7 * iv;
+        const double g1 = g[1], g2 = g[2], g3 = g[3], g4 = g[4], g5 = g[5], g6 = g[6];
+        const double sB = g[0] + g1 * lnT + T * (g2 + T * (g3 + T * (g4 + T * g5))) + g6 * invT;
+        const double sdB = (g1 - g6 * invT) * invT + g2 + T * (2.0 * g3 + T * (3.0 * g4 + 4.0 * g5 * T));
+        const double H = kRu * T * (T * sdB + dnu);
+
+        // ---- concentrations of the six slots (empty slots point at the dummy species [X] = 1)
+        const double c0 = X[x0 + q], c1 = X[x1 + q], c2 = X[x2 + q], c3 = X[x3 + q], c4 = X[x4 + q], c5 = X[x5 + q];
 
         // ---- rates of progress (Eqs. 18-19) and the products that skip one factor (Eqs. 120-121)
-        double Pf, Pr_, sk0, sk1, sk2, sk3, sk4, sk5, sB, sdB = 0.0;
+        double Pf, Pr_, sk0, sk1, sk2, sk3, sk4, sk5;
         if (unit_nu) {
-            const double p01 = xb0.x * xb1.x, p34 = xb3.x * xb4.x;
-            Pf = p01 * xb2.x; Pr_ = p34 * xb5.x;
-            sk0 = xb1.x * xb2.x; sk1 = xb0.x * xb2.x; sk2 = p01;
-            sk3 = xb4.x * xb5.x; sk4 = xb3.x * xb5.x; sk5 = p34;
-            sB = (xb3.y + xb4.y + xb5.y) - (xb0.y + xb1.y + xb2.y);
-            if (LEVEL == 2)
-                sdB = (S4[sp3 + 2] + S4[sp4 + 2] + S4[sp5 + 2]) - (S4[sp0 + 2] + S4[sp1 + 2] + S4[sp2 + 2]);
+            const double p01 = c0 * c1, p34 = c3 * c4;
+            Pf = p01 * c2; Pr_ = p34 * c5;
+            sk0 = c1 * c2; sk1 = c0 * c2; sk2 = p01;
+            sk3 = c4 * c5; sk4 = c3 * c5; sk5 = p34;
         } else {
             const int n0 = meta_nu(meta, 0), n1 = meta_nu(meta, 1), n2 = meta_nu(meta, 2),
                       n3 = meta_nu(meta, 3), n4 = meta_nu(meta, 4), n5 = meta_nu(meta, 5);
             double p0, p1, p2, p3, p4, p5, m0, m1, m2, m3, m4, m5;
-            int_pow(xb0.x, n0, p0, m0); int_pow(xb1.x, n1, p1, m1); int_pow(xb2.x, n2, p2, m2);
-            int_pow(xb3.x, n3, p3, m3); int_pow(xb4.x, n4, p4, m4); int_pow(xb5.x, n5, p5, m5);
+            int_pow(c0, n0, p0, m0); int_pow(c1, n1, p1, m1); int_pow(c2, n2, p2, m2);
+            int_pow(c3, n3, p3, m3); int_pow(c4, n4, p4, m4); int_pow(c5, n5, p5, m5);
             Pf = p0 * p1 * p2; Pr_ = p3 * p4 * p5;
             sk0 = m0 * p1 * p2; sk1 = p0 * m1 * p2; sk2 = p0 * p1 * m2;
             sk3 = m3 * p4 * p5; sk4 = p3 * m4 * p5; sk5 = p3 * p4 * m5;
-            sB = ((double)n3 * xb3.y + (double)n4 * xb4.y + (double)n5 * xb5.y)
-                 - ((double)n0 * xb0.y + (double)n1 * xb1.y + (double)n2 * xb2.y);
-            if (LEVEL == 2)
-                sdB = ((double)n3 * S4[sp3 + 2] + (double)n4 * S4[sp4 + 2] + (double)n5 * S4[sp5 + 2])
-                      - ((double)n0 * S4[sp0 + 2] + (double)n1 * S4[sp1 + 2] + (double)n2 * S4[sp2 + 2]);
         }
 
         // ---- reverse rate coefficient (Eqs. 23-27, 69, 75)
         double kr = 0.0, Lr = 0.0;
         if (rev == PYJAC_REV_FROM_KC) {
-            kr = exp_rate(lnkf - sB - dnu_lnc);
+            kr = exp_rate(lnkf - sB);
             Lr = L - sdB;
         } else if (rev == PYJAC_REV_EXPLICIT) {
             const double rb = m.rev_beta[s], rTa = m.rev_Ta[s];
@@ -253,15 +269,14 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         double c = 1.0, G = 0.0, fT = 0.0, b = 0.0, Xi = 0.0;
         int eb = 0, ee = 0;
         if (pdep) {
-            const int pd = s - m.pd_begin;
-            eb = m.eff_ptr[pd]; ee = m.eff_ptr[pd + 1];
-            Xi = meta_single(meta) ? 0.0 : sm[sp.Scal + kM];             // Eqs. 28-30
-            for (int e = eb; e < ee; ++e) Xi += m.eff_eps[e] * S4[4 * m.eff_spec[e]];
+            eb = m.eff_ptr[s]; ee = m.eff_ptr[s + 1];
+            Xi = meta_single(meta) ? 0.0 : sc[kM * S + q];               // Eqs. 28-30
+            for (int e = eb; e < ee; ++e) Xi += m.eff_eps[e] * X[m.eff_spec[e] * S + q];
             if (type == PYJAC_THIRD_BODY) {
                 c = Xi; G = Xi; lPrT = -invT; b = R;                     // Eqs. 79-80
             } else {
                 const double Pr = exp_rate(lnk0 - lnkinf) * Xi;          // Eq. 31
-                const double *fp = m.fall_par + 5 * pd;
+                const double *fp = m.fall_par + 5 * s;
                 const int form = meta_form(meta);
                 double F = 1.0, gF = 0.0;                                // gF = (P_r/F) dF/dP_r
                 if (form == PYJAC_TROE) {                                // Eqs. 33-35, 90-96
@@ -295,7 +310,9 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
                 b = R * G / Xi;
             }
         }
-        sm[sp.Q + s] = c * R;
+        const double qi = c * R;
+        E[(m.eQ + s) * S + q] = qi;
+        E[(m.eH + s) * S + q] = H;
         if (LEVEL == 0) {
             const long long st = state0 + q;
             if (st < n) {
@@ -310,398 +327,242 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             const double dcdT = pdep ? G * lPrT + c * fT : 0.0;
             const double dRfdT = Rf * (L - (double)snu_f * invT);                 // Eq. 66
             const double dRrdT = Rr * (Lr - (double)snu_r * invT);                // Eqs. 69, 75
-            sm[sp.Th + s] = dcdT * R + c * (dRfdT - dRrdT + R * invT);
-            // coefficient of d_j (Eqs. 119, 123, 127 regrouped)
-            const double W = sm[sp.Scal + kW];
+            E[(m.eTh + s) * S + q] = dcdT * R + c * (dRfdT - dRrdT + R * invT);
+            // coefficient of d_j (Eqs. 119, 123, 127 regrouped), plus W q_i: the omega_k W d_j term of
+            // Eq. 112 summed per reaction
+            const double W = sc[kW * S + q];
             const double base = -W * (Rf * (double)snu_f - Rr * (double)snu_r);
-            const double mix = (pdep && !meta_single(meta)) ? sm[sp.Scal + kRho] : 0.0;
-            sm[sp.Ar + s] = c * base + b * (mix - W * Xi);
+            const double mix = (pdep && !meta_single(meta)) ? sc[kRho * S + q] : 0.0;
+            E[(m.eAr + s) * S + q] = c * base + b * (mix - W * Xi) + W * qi;
             // sparse terms s'_ij = c (k_f S'_j - k_r S''_j) per slot, b (alpha_ij - 1) per efficiency
             const double ckf = c * kf, ckr = -c * kr;
-            double *V = sm + sp.V + vb;
-            if (meta & 0x00000Fu) *V++ = ckf * sk0;
-            if (meta & 0x0000F0u) *V++ = ckf * sk1;
-            if (meta & 0x000F00u) *V++ = ckf * sk2;
-            if (meta & 0x00F000u) *V++ = ckr * sk3;
-            if (meta & 0x0F0000u) *V++ = ckr * sk4;
-            if (meta & 0xF00000u) *V++ = ckr * sk5;
+            double *V = E + m.vbase[s] * S + q;
+            if (meta & 0x00000Fu) { *V = ckf * sk0; V += kVStride * S; }
+            if (meta & 0x0000F0u) { *V = ckf * sk1; V += kVStride * S; }
+            if (meta & 0x000F00u) { *V = ckf * sk2; V += kVStride * S; }
+            if (meta & 0x00F000u) { *V = ckr * sk3; V += kVStride * S; }
+            if (meta & 0x0F0000u) { *V = ckr * sk4; V += kVStride * S; }
+            if (meta & 0xF00000u) { *V = ckr * sk5; V += kVStride * S; }
             if (pdep) {
-                double *Ve = sm + sp.V + m.eff_vbase[s - m.pd_begin] - eb;
-                for (int e = eb; e < ee; ++e) Ve[e] = b * m.eff_eps[e];
+                double *Ve = E + m.eff_vbase[s] * S + q;
+                for (int e = eb; e < ee; ++e, Ve += kVStride * S) *Ve = b * m.eff_eps[e];
             }
         }
     }
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------
-// Shared memory: S state blocks of sp.total doubles, then 7*S rows of 32 doubles of reduction scratch
-// (3S rows for phase 0, 4S for phase 3).  The Jacobian tile of a state holds rows r = 0..ns of a
-// panel of columns: r = 0 is the energy row (stored times W_j), r = k + 1 the raw species sums.
+// Shared memory: S interleaved state blocks of sp.total doubles, then kRedRows * S rows of 32 doubles
+// of reduction scratch.  The scalar block is double-buffered by iteration parity: the mixture of the
+// next batch is written while other warps still finish this batch's MAIN pass.
 template <int LEVEL, int NT, int S>
 __global__ void __launch_bounds__(NT, (NT <= 128 ? 4 : NT <= 256 ? 2 : 1))
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
                 const double *__restrict__ Pg, const double *__restrict__ Yg, long long ldy, const EvalOut out)
 {
-    extern __shared__ double sm_all[];
+    extern __shared__ __align__(16) double sm[];
+    __shared__ int ctr[4];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
-    const int ns = m.ns, nr = m.nr, ld = m.ld, ldt = m.ldt;
-    const int SS = sp.total;
-    double *red0 = sm_all + S * SS, *red3 = red0 + 3 * S * 32;
-    const int nwa = min(NW, (ns + 31) >> 5);     // warps that own species
-#pragma unroll
-    for (int q = 0; q < S; ++q) {
-        double *sm = sm_all + q * SS;
-        if (tid == 0) {   // the empty-slot dummy species {[X] = 1, B = dB = hW = 0} and the zero slots
-            sm[sp.Sp4 + 4 * ns] = 1.0; sm[sp.Sp4 + 4 * ns + 1] = 0.0;
-            sm[sp.Sp4 + 4 * ns + 2] = 0.0; sm[sp.Sp4 + 4 * ns + 3] = 0.0;
-            sm[sp.Q + nr] = 0.0; sm[sp.Ar + nr] = 0.0; sm[sp.Th + nr] = 0.0; sm[sp.V + m.n_v] = 0.0;
-            sm[sp.WA] = 0.0; sm[sp.WC] = 0.0; sm[sp.WA + ns + 1] = 0.0; sm[sp.WC + ns + 1] = 0.0;
-        }
-        if (LEVEL == 2)   // cells that collect no reaction stay zero for the whole launch (single panel)
-            for (int i = tid; i < ldt * m.pw + 2; i += NT) sm[sp.Tile + i] = 0.0;
+    const int ns = m.ns, ld = m.ld;
+    double *red = sm + (size_t)sp.total * S;
+    double *E = sm + sp.E * S;
+    double *X = sm + sp.X * S;
+    double *Cp = sm + sp.Cp * S;
+    if (tid < S) {   // the empty-slot dummy species, the zero slot and the constant scalar 1
+        X[ns * S + tid] = 1.0;
+        E[m.eZero * S + tid] = 0.0;
+        sm[(sp.Scal + kOne) * S + tid] = 1.0;
+        sm[(sp.Scal + kNScal + kOne) * S + tid] = 1.0;
     }
     const long long nblk = (n + S - 1) / S;
-    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
+    int par = 0;
+    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x, par ^= 1) {
         const long long state0 = blk * S;
-        // ---- per-state scalars (one thread per state)
-        if (tid < S) {
-            const long long st = min(state0 + tid, n - 1);
-            double *sc = sm_all + tid * SS + sp.Scal;
-            const double T = Tg[st], P = Pg[st];
-            sc[kT] = T; sc[kLnT] = log(T); sc[kInvT] = 1.0 / T; sc[kP] = P; sc[kM] = P / (kRu * T);
+        double *sc = sm + (sp.Scal + par * kNScal) * S;
+        // ---- phase 0a: mixture molecular weight, density (Eqs. 3-5); warp q <-> state q
+        for (int q = warp; q < S; q += NW) {
+            const long long st = min(state0 + q, n - 1);
+            double s = 0.0;
+            for (int k = lane; k < ns; k += 32) s += Yg[st * ldy + k] * m.inv_mw[k];
+            s = warp_sum(s);
+            if (lane == 0) {
+                const double T = Tg[st], P = Pg[st];
+                const double W = 1.0 / s, M = P / (kRu * T), rho = M * W;
+                sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P;
+                sc[kM * S + q] = M; sc[kW * S + q] = W; sc[kRho * S + q] = rho; sc[kIrho * S + q] = 1.0 / rho;
+            }
         }
-        __syncthreads();
-        // ---- phase 0: species (Eqs. 3-5, 9-13, 27, 54-55, 74)
+        __syncthreads();      // every warp has also left the previous iteration's last phase
+        if (tid == 0) { ctr[0] = 0; ctr[1] = 0; ctr[2] = 0; }
+        // ---- phase 0b: species (Eqs. 5, 9, 12-13, 54-55)
         {
-            double part[3 * S];
+            double part[2 * S];
 #pragma unroll
-            for (int i = 0; i < 3 * S; ++i) part[i] = 0.0;
+            for (int i = 0; i < 2 * S; ++i) part[i] = 0.0;
+            for (int k = tid; k < ns; k += NT) {
+                const double iw = m.inv_mw[k], tm = m.t_mid[k];
 #pragma unroll
-            for (int q = 0; q < S; ++q) {
-                double *sm = sm_all + q * SS;
-                const long long st = min(state0 + q, n - 1);
-                const double T = sm[sp.Scal + kT], lnT = sm[sp.Scal + kLnT], invT = sm[sp.Scal + kInvT];
-                for (int k = tid; k < ns; k += NT) {
+                for (int q = 0; q < S; ++q) {
+                    const long long st = min(state0 + q, n - 1);
+                    const double T = sc[kT * S + q];
                     const double y = Yg[st * ldy + k];
-                    const double iw = m.inv_mw[k];
-                    const double *a = m.nasa + (T <= m.t_mid[k] ? 0 : (size_t)7 * ns) + k;
+                    const double *a = m.nasa + (T <= tm ? 0 : (size_t)5 * ns) + k;
                     const double a0 = a[0], a1 = a[ns], a2 = a[2 * (size_t)ns], a3 = a[3 * (size_t)ns],
-                                 a4 = a[4 * (size_t)ns], a5 = a[5 * (size_t)ns], a6 = a[6 * (size_t)ns];
-                    const double cpR = a0 + T * (a1 + T * (a2 + T * (a3 + a4 * T)));
-                    const double hR = T * (a0 + T * (a1 * 0.5 + T * (a2 * (1.0 / 3.0) + T * (a3 * 0.25 + a4 * 0.2 * T)))) + a5;
-                    const double cpk = kRu * cpR * iw;
-                    double4 v;
-                    v.x = y * iw;
-                    v.y = a6 - a0 + (a0 - 1.0) * lnT
-                          + T * (a1 * 0.5 + T * (a2 * (1.0 / 6.0) + T * (a3 * (1.0 / 12.0) + a4 * 0.05 * T))) - a5 * invT;
-                    v.z = (a0 - 1.0 + a5 * invT) * invT + a1 * 0.5 + T * (a2 * (1.0 / 3.0) + T * (a3 * 0.25 + a4 * 0.2 * T));
-                    v.w = kRu * hR;
-                    *reinterpret_cast<double4 *>(sm + sp.Sp4 + 4 * k) = v;
-                    part[3 * q] += y * iw;
-                    if (LEVEL >= 1) { sm[sp.Cp + k] = cpk; part[3 * q + 1] += y * cpk; }
-                    if (LEVEL == 2)
-                        part[3 * q + 2] += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
-                }
-            }
-            block_partials<3 * S>(part, red0, lane, warp, nwa);
-            __syncthreads();
-            if (tid < ns) {
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    double *sm = sm_all + q * SS;
-                    const double W = 1.0 / red_sum(red0, 3 * q, nwa);
-                    const double rho = sm[sp.Scal + kM] * W;
-                    if (tid == 0) {
-                        sm[sp.Scal + kW] = W; sm[sp.Scal + kRho] = rho; sm[sp.Scal + kIrho] = 1.0 / rho;
-                        if (LEVEL >= 1) sm[sp.Scal + kCpMix] = red_sum(red0, 3 * q + 1, nwa);
-                        if (LEVEL == 2) sm[sp.Scal + kDcpDT] = red_sum(red0, 3 * q + 2, nwa);
-                    }
-                    for (int k = tid; k < ns; k += NT) sm[sp.Sp4 + 4 * k] *= rho;
-                }
-            }
-        }
-        __syncthreads();
-        // ---- phase 1: reactions
-        for (int s = tid; s < nr; s += NT) reaction<LEVEL, S>(m, sp, sm_all, SS, s, out, state0, n);
-        __syncthreads();
-        // ---- phase 2a: species sums over reactions, kSpLanes lanes per species (fixed order)
-        for (int c = warp; c < m.n_spchunk; c += NW) {
-            const uint2 ch = m.spchunk[c];
-            const uint2 *ent = m.sp_ent + ch.x + lane;
-            double wd[S], A[S], Tc[S], Dg[S];
-#pragma unroll
-            for (int q = 0; q < S; ++q) { wd[q] = 0.0; A[q] = 0.0; Tc[q] = 0.0; Dg[q] = 0.0; }
-#pragma unroll 2
-            for (uint32_t t = 0; t < ch.y; ++t) {
-                const uint2 e = ent[t * 32];
-                const int s = e.x & 0xFFFF, v = e.y & 0xFFFF;
-                const double cf = entry_coef(e.x), cv = entry_coef(e.y);
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    const double *sm = sm_all + q * SS;
-                    wd[q] += cf * sm[sp.Q + s];
-                    if (LEVEL == 2) {
-                        A[q] += cf * sm[sp.Ar + s];
-                        Tc[q] += cf * sm[sp.Th + s];
-                        Dg[q] += cv * sm[sp.V + v];
-                    }
-                }
-            }
-#pragma unroll
-            for (int o = kSpLanes / 2; o > 0; o >>= 1) {
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    wd[q] += __shfl_xor_sync(0xFFFFFFFFu, wd[q], o);
-                    if (LEVEL == 2) {
-                        A[q] += __shfl_xor_sync(0xFFFFFFFFu, A[q], o);
-                        Tc[q] += __shfl_xor_sync(0xFFFFFFFFu, Tc[q], o);
-                        Dg[q] += __shfl_xor_sync(0xFFFFFFFFu, Dg[q], o);
-                    }
-                }
-            }
-            const int k = m.sptask_k[c * (32 / kSpLanes) + lane / kSpLanes];
-            if ((lane % kSpLanes) == 0 && k >= 0) {
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    double *sm = sm_all + q * SS;
-                    sm[sp.Wdot + k] = wd[q];
-                    if (LEVEL == 2) {
-                        sm[sp.A + k] = A[q]; sm[sp.Tc + k] = Tc[q];
-                        if (m.n_panel == 1) sm[sp.Tile + k + 1 + k * ldt] = Dg[q]; else sm[sp.Diag + k] = Dg[q];
-                    }
-                }
-            }
-        }
-        // ---- phase 2b: off-diagonal cells of the species block, longest lists first
-        auto gather_cells = [&](int p) {
-            const int2 pc = m.panel_chunks[p];
-            for (int c = pc.x + warp; c < pc.y; c += NW) {
-                const uint2 ch = m.cchunk[c];
-                const uint32_t *ent = m.c_ent + ch.x + lane;
-                const uint32_t addr = m.ctask_addr[c * 32 + lane];
-                double acc[S];
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] = 0.0;
-#pragma unroll 2
-                for (uint32_t t = 0; t < ch.y; ++t) {
-                    const uint32_t e = ent[t * 32];
-                    const double cf = entry_coef(e);
-                    const double *v = sm_all + sp.V + (e & 0xFFFF);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[q] += cf * v[q * SS];
-                }
-#pragma unroll
-                for (int q = 0; q < S; ++q) sm_all[q * SS + sp.Tile + addr] = acc[q];
-            }
-        };
-        if (LEVEL == 2 && m.n_panel == 1) gather_cells(0);
-        __syncthreads();
-        // ---- phase 3: species finalisation (Eqs. 7-8, 111, 113)
-        {
-            double part[4 * S];
-#pragma unroll
-            for (int i = 0; i < 4 * S; ++i) part[i] = 0.0;
-#pragma unroll
-            for (int q = 0; q < S; ++q) {
-                double *sm = sm_all + q * SS;
-                const bool live = state0 + q < n;
-                const long long st = state0 + q;
-                const double irho = sm[sp.Scal + kIrho], W = sm[sp.Scal + kW];
-                for (int k = tid; k < ns; k += NT) {
-                    const double wd = sm[sp.Wdot + k];
-                    const double Wk = m.mw[k];
-                    const double hw = sm[sp.Sp4 + 4 * k + 3];
-                    if (LEVEL == 0) { if (out.wdot && live) out.wdot[st * ns + k] = wd; }
-                    if (LEVEL == 1) { if (live) out.dydt[st * ld + k + 1] = Wk * wd * irho; }
-                    part[4 * q] += hw * wd;
-                    if (LEVEL == 2) {
-                        const double Ap = wd * W + sm[sp.A + k];
-                        const double Tc = sm[sp.Tc + k];
-                        sm[sp.WA + k + 1] = Wk * Ap * irho;
-                        sm[sp.Col0 + k + 1] = Wk * irho * Tc;
-                        part[4 * q + 1] += hw * Ap;
-                        part[4 * q + 2] += sm[sp.Cp + k] * Wk * wd;
-                        part[4 * q + 3] += hw * Tc;
+                                 a4 = a[4 * (size_t)ns];
+                    X[k * S + q] = sc[kRho * S + q] * (y * iw);
+                    if (LEVEL >= 1) {
+                        const double cpk = kRu * (a0 + T * (a1 + T * (a2 + T * (a3 + a4 * T)))) * iw;
+                        Cp[k * S + q] = cpk;
+                        part[2 * q] += y * cpk;
+                        if (LEVEL == 2) part[2 * q + 1] += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
                     }
                 }
             }
             if (LEVEL >= 1) {
-                block_partials<4 * S>(part, red3, lane, warp, nwa);
-                __syncthreads();
-            }
-        }
-        if (LEVEL == 1 && tid < S && state0 + tid < n) {
-            const double *sm = sm_all + tid * SS;
-            out.dydt[(state0 + tid) * ld] = -red_sum(red3, 4 * tid, nwa) * sm[sp.Scal + kIrho] / sm[sp.Scal + kCpMix];
-        }
-        if (LEVEL == 2) {
-            // sums needed by the energy row: only the threads that own a column (tid < ns) use them
-            double shg[S], shA[S], icp[S], cpl[S], El[S];
 #pragma unroll
-            for (int q = 0; q < S; ++q) { shg[q] = 0.0; shA[q] = 0.0; icp[q] = 0.0; cpl[q] = 0.0; El[q] = 0.0; }
-            const double iwl = m.inv_mw[ns - 1];
-            const long long Jstate = (long long)ld * ld;
-            if (tid < ns) {
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    double *sm = sm_all + q * SS;
-                    const double irho = sm[sp.Scal + kIrho];
-                    const double p0 = red_sum(red3, 4 * q, nwa);
-                    icp[q] = 1.0 / sm[sp.Scal + kCpMix];
-                    if (tid == 0)
-                        sm[sp.Col0] = -icp[q] * irho * (red_sum(red3, 4 * q + 2, nwa) - sm[sp.Scal + kDcpDT] * icp[q] * p0
-                                                        + red_sum(red3, 4 * q + 3, nwa));
-                    shg[q] = p0 * irho; shA[q] = red_sum(red3, 4 * q + 1, nwa) * irho;
-                    cpl[q] = sm[sp.Cp + ns - 1];
-                    El[q] = 0.0;                      // energy-row sum of the virtual column Nsp
+                for (int i = 0; i < 2 * S; ++i) {
+                    const double v = warp_sum(part[i]);
+                    if (lane == 0) red[i * 32 + warp] = v;
                 }
             }
-            // panels of columns; the one holding the virtual column Nsp goes first (its sums enter
-            // every other column, Eqs. 119, 123, 127)
-            for (int pi = 0; pi < m.n_panel; ++pi) {
-                const int p = pi == 0 ? m.n_panel - 1 : pi - 1;
-                const int j0 = p * m.pw, j1 = min(ns, j0 + m.pw), pwc = j1 - j0;
-                if (m.n_panel > 1) {
-                    if (pi > 0) __syncthreads();                  // previous panel's write-out done
+        }
+        __syncthreads();
+        // ---- phase 1: reactions (the mixture heat capacity is finished on the side)
+        if (LEVEL >= 1 && tid < S) {
+            double cp = 0.0, dcp = 0.0;
+            for (int w = 0; w < NW; ++w) { cp += red[(2 * tid) * 32 + w]; dcp += red[(2 * tid + 1) * 32 + w]; }
+            const double icp = 1.0 / cp;
+            sc[kCpMix * S + tid] = cp; sc[kDcpDT * S + tid] = dcp;
+            sc[kNegIcp * S + tid] = -icp; sc[kNegIrhoIcp * S + tid] = -icp * sc[kIrho * S + tid];
+        }
+        for (int c = grab(&ctr[0], lane); c < m.n_rchunk; c = grab(&ctr[0], lane)) {
+            const int s = c * 32 + lane;
+            if (s < m.nr) reaction<LEVEL, S>(m, sp, sm, sc, s, out, state0, n);
+        }
+        __syncthreads();
+        // ---- AUX gathers
+        {
+            const int nch = LEVEL == 2 ? m.n_achunk : m.n_achunk01;
+            for (int c = grab(&ctr[1], lane); c < nch; c = grab(&ctr[1], lane)) {
+                const uint4 ch = m.achunk[c];
+                const uint32_t *ent = m.a_ent + ch.x + lane;
+                double acc[S];
 #pragma unroll
-                    for (int q = 0; q < S; ++q)
-                        for (int i = tid; i < ldt * m.pw; i += NT) sm_all[q * SS + sp.Tile + i] = 0.0;
-                    __syncthreads();
-                    gather_cells(p);
+                for (int q = 0; q < S; ++q) acc[q] = 0.0;
+                if (ch.z & kAuxTwoIndex) {
+#pragma unroll 2
+                    for (uint32_t t = 0; t < ch.y; ++t) {
+                        const uint32_t e = ent[t * 32];
+                        double a[S], b[S];
+                        ldv<S>(E + (e & 0xFFFF) * S, a);
+                        ldv<S>(E + (e >> 16) * S, b);
 #pragma unroll
-                    for (int q = 0; q < S; ++q)
-                        for (int j = j0 + tid; j < j1; j += NT)
-                            sm_all[q * SS + sp.Tile + j + 1 + (j - j0) * ldt] = sm_all[q * SS + sp.Diag + j];
-                    __syncthreads();
-                }
-                // energy-row partial sums E_j = sum_k h_k W_k cell(k, j), kEParts row ranges per column
-                const int rows = (ns + kEParts - 1) / kEParts;
-                for (int t = tid; t < pwc * kEParts; t += NT) {
-                    const int pt = t / pwc, jl = t - pt * pwc;
-                    const int k1 = min(ns, (pt + 1) * rows);
-                    double e[S];
-#pragma unroll
-                    for (int q = 0; q < S; ++q) e[q] = 0.0;
-                    const double *hw = sm_all + sp.Sp4 + 3, *tl = sm_all + sp.Tile + 1 + jl * ldt;
-                    for (int k = pt * rows; k < k1; ++k) {
-#pragma unroll
-                        for (int q = 0; q < S; ++q) e[q] += hw[q * SS + 4 * k] * tl[q * SS + k];
-                    }
-#pragma unroll
-                    for (int q = 0; q < S; ++q) sm_all[q * SS + sp.Ep + pt * (ns + 1) + jl] = e[q];
-                }
-                if (pi == 0) {
-#pragma unroll
-                    for (int q = 0; q < S; ++q)
-                        for (int k = tid; k < ns; k += NT)
-                            sm_all[q * SS + sp.WC + k + 1] = m.mw[k] * iwl * sm_all[q * SS + sp.Tile + k + 1 + (ns - 1 - j0) * ldt];
-                }
-                __syncthreads();
-                if (tid < ns) {
-                    if (pi == 0) {
-                        const int jl = ns - 1 - j0;
-#pragma unroll
-                        for (int q = 0; q < S; ++q) {
-                            for (int pt = 0; pt < kEParts; ++pt) El[q] += sm_all[q * SS + sp.Ep + pt * (ns + 1) + jl];
-                            El[q] *= iwl;
-                        }
-                    }
-                    // row 0 of the panel's columns, stored times W_j (phase 4 multiplies by 1/W_j)
-                    for (int jl = tid; jl < pwc; jl += NT) {
-                        const int j = j0 + jl;
-                        if (j >= ns - 1) continue;
-                        const double2 cc = m.colc[j];
-                        const double Wj = m.mw[j];
-#pragma unroll
-                        for (int q = 0; q < S; ++q) {
-                            double *sm = sm_all + q * SS;
-                            double E = 0.0;
-                            for (int pt = 0; pt < kEParts; ++pt) E += sm[sp.Ep + pt * (ns + 1) + jl];
-                            sm[sp.Tile + jl * ldt] = -icp[q] * Wj * (-(sm[sp.Cp + j] - cpl[q]) * icp[q] * shg[q]
-                                                                      + cc.x * shA[q] + cc.y * E - El[q]);
-                        }
-                    }
-                }
-                __syncthreads();
-                // ---- phase 4: dense write-out (column-major, LD = ns + 1): element (r, j + 1) =
-                //      WA[r] d_j + (wrow[r] / W_j) tile(r, j) - WC[r]; a warp writes one column segment
-                const int pwo = min(j1, ns - 1) - j0;
-                if ((ld & 1) == 0) {
-                    // even LD: two rows per lane, 16-byte loads and stores
-                    const int nrb = (ld + 63) >> 6;
-                    int g = NW, h = nrb;                  // g = gcd(NW, nrb)
-                    while (h) { const int t = g % h; g = h; h = t; }
-                    const int cstep = NW / g, jl0 = warp / g;
-                    for (int rb = warp % g; rb < nrb; rb += g) {
-                        const int r0 = rb * 64 + 2 * lane;
-                        const bool ok = r0 < ld;
-                        const int rc = ok ? r0 : 0;
-                        const double2 wk2 = *reinterpret_cast<const double2 *>(m.wrow + rc);
-                        double2 wa2[S], wc2[S];
-#pragma unroll
-                        for (int q = 0; q < S; ++q) {
-                            wa2[q] = *reinterpret_cast<const double2 *>(sm_all + q * SS + sp.WA + rc);
-                            wc2[q] = *reinterpret_cast<const double2 *>(sm_all + q * SS + sp.WC + rc);
-                        }
-                        const double *src = sm_all + sp.Tile + rc + jl0 * ldt;
-                        double *Jp = out.jac + state0 * Jstate + r0 + (long long)(j0 + 1 + jl0) * ld;
-                        const double2 *cc = m.colc + j0 + jl0;
-                        for (int jl = jl0; jl < pwo; jl += cstep) {
-                            const double2 c2 = *cc;
-                            const double wa_ = wk2.x * c2.y, wb_ = wk2.y * c2.y;
-#pragma unroll
-                            for (int q = 0; q < S; ++q) {
-                                const double2 x = *reinterpret_cast<const double2 *>(src + q * SS);
-                                double2 v;
-                                v.x = fma(wa2[q].x, c2.x, fma(wa_, x.x, -wc2[q].x));
-                                v.y = fma(wa2[q].y, c2.x, fma(wb_, x.y, -wc2[q].y));
-                                if (ok && state0 + q < n) __stcs(reinterpret_cast<double2 *>(Jp + q * Jstate), v);
-                            }
-                            src += cstep * ldt; Jp += (long long)cstep * ld; cc += cstep;
-                        }
+                        for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
                     }
                 } else {
-                    const int nrb = (ld + 31) >> 5;
-                    int g = NW, h = nrb;
-                    while (h) { const int t = g % h; g = h; h = t; }
-                    const int cstep = NW / g, jl0 = warp / g;
-                    for (int rb = warp % g; rb < nrb; rb += g) {
-                        const int r = rb * 32 + lane;
-                        const bool ok = r < ld;
-                        const int rc = ok ? r : 0;
-                        const double wk = m.wrow[rc];
-                        double wa[S], wc[S];
+#pragma unroll 2
+                    for (uint32_t t = 0; t < ch.y; ++t) {
+                        const uint32_t e = ent[t * 32];
+                        const double cf = entry_coef(e);
+                        double a[S];
+                        ldv<S>(E + (e & 0xFFFF) * S, a);
 #pragma unroll
-                        for (int q = 0; q < S; ++q) { wa[q] = sm_all[q * SS + sp.WA + rc]; wc[q] = sm_all[q * SS + sp.WC + rc]; }
-                        const double *src = sm_all + sp.Tile + rc + jl0 * ldt;
-                        double *Jp = out.jac + state0 * Jstate + r + (long long)(j0 + 1 + jl0) * ld;
-                        const double2 *cc = m.colc + j0 + jl0;
-                        for (int jl = jl0; jl < pwo; jl += cstep) {
-                            const double2 c2 = *cc;
-                            const double wkiw = wk * c2.y;
-#pragma unroll
-                            for (int q = 0; q < S; ++q) {
-                                const double val = fma(wa[q], c2.x, fma(wkiw, src[q * SS], -wc[q]));
-                                if (ok && state0 + q < n) __stcs(Jp + q * Jstate, val);
-                            }
-                            src += cstep * ldt; Jp += (long long)cstep * ld; cc += cstep;
-                        }
+                        for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
                     }
                 }
+                if (ch.z & kAuxReduce) {
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[q] = warp_sum(acc[q]);
+                }
+                const uint32_t task = ch.w + ((ch.z & kAuxReduce) ? 0 : lane);
+                const uint32_t slot = m.a_out[task];
+                if (ch.z & kAuxScaled) {
+                    const double cst = m.a_const[task];
+                    const double *f = sc + ((ch.z >> 8) & 0xFF) * S;
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[q] *= cst * f[q];
+                }
+                if (slot != 0xFFFFFFFFu && (!(ch.z & kAuxReduce) || lane == 0)) stv<S>(E + slot * S, acc);
             }
+        }
+        __syncthreads();
+        // ---- outputs of the rates / source-term kernels (Eqs. 7-8, 14)
+        if (LEVEL == 0 && out.wdot) {
+            for (int k = tid; k < ns; k += NT)
+#pragma unroll
+                for (int q = 0; q < S; ++q)
+                    if (state0 + q < n) out.wdot[(state0 + q) * ns + k] = E[(m.eWdot + k) * S + q];
+        }
+        if (LEVEL == 1) {
+            for (int r = tid; r < ld; r += NT)
+#pragma unroll
+                for (int q = 0; q < S; ++q) {
+                    if (state0 + q >= n) continue;
+                    const double irho = sc[kIrho * S + q];
+                    const double v = r == 0 ? -E[m.eS1 * S + q] * irho / sc[kCpMix * S + q]
+                                            : m.wrow[r] * E[(m.eWdot + r - 1) * S + q] * irho;
+                    out.dydt[(state0 + q) * ld + r] = v;
+                }
+        }
+        // ---- MAIN pass: lane <-> Jacobian element f = r + c * ld (column-major), gather + Eq. 112 / 113 + store
+        if (LEVEL == 2) {
+            const long long Jstate = (long long)ld * ld;
+            double a1[S], irho[S];
 #pragma unroll
             for (int q = 0; q < S; ++q) {
-                if (state0 + q >= n) break;
-                double *J = out.jac + (state0 + q) * Jstate;
-                for (int r = tid; r < ld; r += NT) {
-                    __stcs(J + r, sm_all[q * SS + sp.Col0 + r]);
-                    __stcs(J + r + (long long)ns * ld, 0.0);
+                const double icp = -sc[kNegIcp * S + q];
+                irho[q] = sc[kIrho * S + q];
+                a1[q] = irho[q] * E[m.eS1 * S + q] * icp * icp;    // energy row: coefficient of c_pj - c_pNs
+            }
+            for (int t = grab(&ctr[2], lane); t < m.n_mtask; t = grab(&ctr[2], lane)) {
+                const uint4 mt = m.mtask[t];
+                int r = (int)mt.z + lane, c = (int)mt.w;
+                while (r >= ld) { r -= ld; ++c; }
+                const bool live = c <= ns;
+                const uint32_t *ent = m.m_ent + mt.x + lane;
+                double acc[S];
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[q] = 0.0;
+#pragma unroll 2
+                for (uint32_t st = 0; st < mt.y; ++st) {
+                    const uint32_t e = ent[st * 32];
+                    const double cf = entry_coef(e);
+                    double a[S];
+                    ldv<S>(E + (e & 0xFFFF) * S, a);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
+                }
+                double j00[S];
+                if (t == 0) {
+                    // J(0,0) of Eq. 113: -(1/(rho c_p)) [sum_k c_pk W_k wdot_k - (dc_p/dT / c_p) S1 + S4]
+#pragma unroll
+                    for (int q = 0; q < S; ++q) {
+                        double s3 = 0.0;
+                        for (int k = lane; k < ns; k += 32) s3 += Cp[k * S + q] * m.wrow[k + 1] * E[(m.eWdot + k) * S + q];
+                        s3 = warp_sum(s3);
+                        const double nicp = sc[kNegIcp * S + q];
+                        j00[q] = nicp * irho[q] * (s3 + sc[kDcpDT * S + q] * nicp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
+                    }
+                }
+                const int cc_i = live ? c : 0;
+                const double2 cc = m.colc[cc_i];
+                const double wr = m.wrow[r];
+                const double wj = wr * cc.y;
+                double *Jp = out.jac + state0 * Jstate + (long long)t * 32 + lane;
+                double alpha[S], gamma[S];
+                ldv<S>(E + (m.eAlpha + r) * S, alpha);
+                ldv<S>(E + (m.eGamma + r) * S, gamma);
+#pragma unroll
+                for (int q = 0; q < S; ++q) {
+                    double v = fma(alpha[q], cc.x, fma(wj, acc[q], -gamma[q]));
+                    if (r == 0 && c > 0) v = fma(a1[q], Cp[(cc_i - 1) * S + q] - Cp[(ns - 1) * S + q], v);
+                    if (c == 0) v = r == 0 ? (t == 0 ? j00[q] : 0.0) : wr * irho[q] * acc[q];
+                    if (c == ns) v = 0.0;
+                    if (live && state0 + q < n) __stcs(Jp + q * Jstate, v);
                 }
             }
         }
-        // the next iteration writes the scalars and the species arrays first: phase 4 reads neither,
-        // and the three __syncthreads before phase 1 order everything else
     }
 }
 
@@ -716,10 +577,10 @@ cudaError_t launch_t(const DeviceMech &m, const SmemPlan &sp, int grid, size_t s
 
 }  // namespace
 
-size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + 7 * S * 32) * sizeof(double); }
+size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + (size_t)kRedRows * S * 32) * sizeof(double); }
 
 #define PYJAC_FOR_ALL(X) \
-    X(128, 1) X(128, 2) X(128, 4) X(256, 1) X(256, 2) X(256, 4) X(512, 1) X(512, 2) X(512, 4) X(1024, 1) X(1024, 2)
+    X(128, 1) X(128, 2) X(128, 4) X(256, 1) X(256, 2) X(256, 4) X(512, 1) X(512, 2) X(512, 4)
 
 const void *eval_kernel_ptr(int level, int nt, int S)
 {

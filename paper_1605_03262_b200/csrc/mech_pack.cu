@@ -1,8 +1,10 @@
 // mech_pack.cu -- validate a pyjac_mech_desc and pack it into the device table layout (host code).
 //
 // What is precomputed here is state-independent bookkeeping of the paper's restructured evaluation
-// order (Algorithm 2): which per-reaction products feed which Jacobian entries.
-// No thermodynamic or kinetic quantity is evaluated on the host except ln A and ln p of the tables.
+// order (Algorithm 2): which per-reaction products feed which Jacobian entries,
+// and in which fixed order they are summed.  No kinetic quantity is evaluated on the host except
+// ln A, ln p of the tables and the per-reaction sums of NASA coefficients (Eq. 27 summed over a
+// reaction, see device_mech.h `th_data`).
 #include <algorithm>
 #include <cmath>
 #include <numeric>
@@ -26,12 +28,20 @@ struct Fail {
 
 struct ColEntry {
     int spec;      // column species j
-    uint32_t vi;   // V index of s'_ij
+    uint32_t vi;   // E index of s'_ij
 };
 
-}  // namespace
+// one gathered sum of the AUX phase
+struct Task {
+    std::vector<uint32_t> ent;
+    uint32_t flags = 0;     // kAuxTwoIndex | kAuxScaled | scalar << 8
+    uint32_t out = 0;       // E slot
+    double cst = 0.0;
+    bool reduce = false;    // spread over the 32 lanes of its own chunk
+    bool lvl01 = false;     // needed by the rates / dydt kernels too
+};
 
-static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget, int panel_override)
+void validate(const pyjac_mech_desc *d)
 {
     REQUIRE(d != nullptr, "description is NULL");
     const int ns = d->n_species, nr = d->n_reactions;
@@ -44,30 +54,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
                     d->plog_ptr && d->cheb_ptr && d->cheb_nT && d->cheb_nP && d->cheb_lim,
                 "per-reaction arrays missing");
     }
-    o.ns = ns;
-    o.nr = nr;
-    // ---- species
-    o.mw.assign(d->mol_wt, d->mol_wt + ns);
-    o.inv_mw.resize(ns);
-    o.dcol.resize(ns);
-    o.t_mid.assign(d->t_mid, d->t_mid + ns);
-    o.nasa.resize((size_t)14 * ns);
-    for (int k = 0; k < ns; ++k) {
+    for (int k = 0; k < ns; ++k)
         REQUIRE(d->mol_wt[k] > 0.0 && std::isfinite(d->mol_wt[k]), "molecular weight must be positive");
-        o.inv_mw[k] = 1.0 / d->mol_wt[k];
-        for (int c = 0; c < 7; ++c) {
-            o.nasa[(size_t)(0 * 7 + c) * ns + k] = d->nasa_lo[7 * k + c];
-            o.nasa[(size_t)(1 * 7 + c) * ns + k] = d->nasa_hi[7 * k + c];
-        }
-    }
-    for (int k = 0; k < ns; ++k) o.dcol[k] = 1.0 / d->mol_wt[k] - 1.0 / d->mol_wt[ns - 1];
-    o.wrow.assign((size_t)ns + 2, 1.0);
-    for (int k = 0; k < ns; ++k) o.wrow[k + 1] = d->mol_wt[k];
-    o.colc.resize((size_t)2 * ns);
-    for (int k = 0; k < ns; ++k) { o.colc[2 * k] = o.dcol[k]; o.colc[2 * k + 1] = o.inv_mw[k]; }
-
-    // ---- validate reactions and choose the sorted order
-    std::vector<int> key(nr);
     for (int i = 0; i < nr; ++i) {
         const int t = d->rxn_type[i], rv = d->rev_type[i];
         REQUIRE(t >= 0 && t <= 5, "rxn_type out of range");
@@ -86,9 +74,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
                 for (int q2 = b; q2 < q; ++q2) REQUIRE(sp[q2] != sp[q], "species repeated within a side");
             }
         }
-        int form = 0;
         if (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED) {
-            form = d->falloff_form[i];
+            const int form = d->falloff_form[i];
             REQUIRE(form >= 0 && form <= 2, "falloff_form out of range");
             REQUIRE(d->arr_lo[3 * i] > 0.0 && d->arr_hi[3 * i] > 0.0, "falloff pre-exponentials must be > 0");
         }
@@ -122,42 +109,117 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
             const double *lim = d->cheb_lim + 4 * i;
             REQUIRE(lim[0] > 0 && lim[1] > lim[0] && lim[2] > 0 && lim[3] > lim[2], "Chebyshev limits invalid");
         }
-        // group: elementary, PLOG, Chebyshev | third body, falloff forms (Lindemann, Troe, SRI)
-        int group = t == PYJAC_ELEMENTARY ? 0 : t == PYJAC_PLOG ? 1 : t == PYJAC_CHEBYSHEV ? 2
-                  : t == PYJAC_THIRD_BODY ? 3 : 4 + form;
+    }
+}
+
+bool is_pd(int t) { return t == PYJAC_THIRD_BODY || t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED; }
+bool is_pk(int t) { return t == PYJAC_PLOG || t == PYJAC_CHEBYSHEV; }
+
+// number of efficiency terms the kernel sums for reaction i (Eq. 28 written as [M] + sum (alpha - 1)[X_j])
+int n_eff_terms(const pyjac_mech_desc *d, int i)
+{
+    if (!is_pd(d->rxn_type[i])) return 0;
+    if (d->tb_species[i] >= 0) return 1;
+    int n = 0;
+    for (int q = d->eff_ptr[i]; q < d->eff_ptr[i + 1]; ++q) n += d->eff_val[q] != 1.0;
+    return n;
+}
+
+}  // namespace
+
+static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doubles)
+{
+    validate(d);
+    const int ns = d->n_species, nr = d->n_reactions, ld = ns + 1;
+    o.ns = ns;
+    o.nr = nr;
+    // ---- species
+    o.inv_mw.resize(ns);
+    o.t_mid.assign(d->t_mid, d->t_mid + ns);
+    o.nasa.resize((size_t)10 * ns);
+    for (int k = 0; k < ns; ++k) {
+        o.inv_mw[k] = 1.0 / d->mol_wt[k];
+        for (int c = 0; c < 5; ++c) {
+            o.nasa[(size_t)(0 * 5 + c) * ns + k] = d->nasa_lo[7 * k + c];
+            o.nasa[(size_t)(1 * 5 + c) * ns + k] = d->nasa_hi[7 * k + c];
+        }
+    }
+    const double iw_last = 1.0 / d->mol_wt[ns - 1];
+    o.wrow.assign((size_t)ld, 1.0);
+    for (int k = 0; k < ns; ++k) o.wrow[k + 1] = d->mol_wt[k];
+    o.colc.assign((size_t)2 * ld, 0.0);
+    o.colc[1] = 1.0;
+    for (int k = 0; k < ns; ++k) {
+        o.colc[2 * (k + 1)] = 1.0 / d->mol_wt[k] - iw_last;
+        o.colc[2 * (k + 1) + 1] = 1.0 / d->mol_wt[k];
+    }
+
+    // ---- sorted order: most expensive rate form first; one form, one stoichiometry path and
+    // equally many V entries per group of 32
+    std::vector<int> key(nr);
+    for (int i = 0; i < nr; ++i) {
+        const int t = d->rxn_type[i], rv = d->rev_type[i];
+        const int form = (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED) ? d->falloff_form[i] : 0;
+        int rank;
+        if (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED)
+            rank = form == PYJAC_TROE ? 0 : form == PYJAC_SRI ? 1 : 2;
+        else
+            rank = t == PYJAC_THIRD_BODY ? 3 : t == PYJAC_CHEBYSHEV ? 4 : t == PYJAC_PLOG ? 5 : 6;
         bool unit = true;
         for (int q = d->reac_ptr[i]; q < d->reac_ptr[i + 1]; ++q) unit = unit && d->reac_nu[q] == 1;
         for (int q = d->prod_ptr[i]; q < d->prod_ptr[i + 1]; ++q) unit = unit && d->prod_nu[q] == 1;
-        int neff = 0;
-        if (group >= 3) neff = d->tb_species[i] >= 0 ? 1 : d->eff_ptr[i + 1] - d->eff_ptr[i];
-        // warps evaluate one rate form, one stoichiometry path and equally long efficiency lists
-        key[i] = ((group * 2 + (unit ? 0 : 1)) * 4 + rv) * 64 + std::min(neff, 63);
+        const int nslot = (d->reac_ptr[i + 1] - d->reac_ptr[i]) + (d->prod_ptr[i + 1] - d->prod_ptr[i]);
+        const int neff = std::min(n_eff_terms(d, i), 63);
+        key[i] = ((((rank * 2 + (unit ? 0 : 1)) * 4 + rv) * 8 + nslot) * 64) + neff;
     }
     std::vector<int> order(nr);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key[a] < key[b]; });
+    o.n_rchunk = (nr + 31) / 32;
+
+    // ---- E indices of the V entries: per group of 32 reactions, slot-major (lane-contiguous)
+    o.vbase.assign(nr, 0u);
+    std::vector<uint32_t> eff_vb(nr, 0u);
+    uint32_t nv = 0;
+    for (int c = 0; c < o.n_rchunk; ++c) {
+        int maxslot = 0, maxeff = 0;
+        for (int s = 32 * c; s < std::min(nr, 32 * c + 32); ++s) {
+            const int i = order[s];
+            maxslot = std::max(maxslot, (d->reac_ptr[i + 1] - d->reac_ptr[i]) + (d->prod_ptr[i + 1] - d->prod_ptr[i]));
+            maxeff = std::max(maxeff, n_eff_terms(d, i));
+        }
+        for (int s = 32 * c; s < std::min(nr, 32 * c + 32); ++s) {
+            o.vbase[s] = nv + (uint32_t)(s - 32 * c);
+            eff_vb[s] = nv + (uint32_t)(kVStride * maxslot + (s - 32 * c));
+        }
+        nv += (uint32_t)(kVStride * (maxslot + maxeff));
+    }
+    const int eQ = (int)nv, eAr = eQ + nr, eTh = eAr + nr, eH = eTh + nr;
+    const int eAlpha = eH + nr, eGamma = eAlpha + ld, eWdot = eGamma + ld;
+    const int eS1 = eWdot + ns, eS4 = eS1 + 1;
+    int next_slot = eS4 + 1;          // further AUX results
+    o.eQ = eQ; o.eAr = eAr; o.eTh = eTh; o.eH = eH; o.eAlpha = eAlpha; o.eGamma = eGamma; o.eWdot = eWdot;
+    o.eS1 = eS1; o.eS4 = eS4;
 
     // ---- per-reaction tables in sorted order
-    o.lnA.resize(nr); o.beta.resize(nr); o.Ta.resize(nr);
+    o.lnA.assign(nr, 0.0); o.beta.assign(nr, 0.0); o.Ta.assign(nr, 0.0);
     o.rev_lnA.assign(nr, 0.0); o.rev_beta.assign(nr, 0.0); o.rev_Ta.assign(nr, 0.0);
     o.slots.assign((size_t)4 * nr, 0u);
-    o.vbase.resize(nr);
     o.rxn_orig.resize(nr);
-    o.pd_begin = nr; o.n_pd = 0; o.pk_begin = nr; o.n_pk = 0;
+    o.th_off.resize(nr);
+    o.n_pd = 0; o.n_pk = 0;
     o.pk_ptr.assign(1, 0);
     o.eff_ptr.assign(1, 0);
-    std::vector<std::vector<ColEntry>> cols(nr);          // column entries of each reaction
+    std::vector<std::vector<ColEntry>> cols(nr);            // column entries of each reaction
     std::vector<std::vector<std::pair<int, int>>> net(nr);  // (species, net nu) of each reaction
-    uint32_t nv = 0;
+    const double ln_patm_R = std::log(kPatm / kRu);
     for (int s = 0; s < nr; ++s) {
         const int i = order[s];
         const int t = d->rxn_type[i], rv = d->rev_type[i];
         o.rxn_orig[s] = i;
-        const bool pk = (t == PYJAC_PLOG || t == PYJAC_CHEBYSHEV);
-        const bool pd = (t == PYJAC_THIRD_BODY || t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED);
-        if (pk && o.n_pk++ == 0) o.pk_begin = s;
-        if (pd && o.n_pd++ == 0) o.pd_begin = s;
-        if (!pk) {
+        if (is_pd(t)) { REQUIRE(s == o.n_pd, "internal: sort order"); ++o.n_pd; }
+        if (is_pk(t)) { REQUIRE(s == o.n_pd + o.n_pk, "internal: sort order"); ++o.n_pk; }
+        if (!is_pk(t)) {
             o.lnA[s] = std::log(d->arr_hi[3 * i]);
             o.beta[s] = d->arr_hi[3 * i + 1];
             o.Ta[s] = d->arr_hi[3 * i + 2];
@@ -169,7 +231,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
         }
         uint32_t spec[6] = {(uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns};
         uint32_t meta = 0;
-        o.vbase[s] = nv;
+        uint32_t vi = o.vbase[s];
+        int dnu = 0;
         for (int side = 0; side < 2; ++side) {
             const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr;
             const int32_t *sp = side ? d->prod_spec : d->reac_spec;
@@ -178,8 +241,10 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
                 const int slot = 3 * side + e;
                 spec[slot] = (uint32_t)sp[q];
                 meta |= (uint32_t)nu[q] << (4 * slot);
-                cols[s].push_back({sp[q], nv++});
+                cols[s].push_back({sp[q], vi});
+                vi += kVStride;
                 const int signed_nu = side ? nu[q] : -nu[q];
+                dnu += signed_nu;
                 bool found = false;
                 for (auto &pr : net[s])
                     if (pr.first == sp[q]) { pr.second += signed_nu; found = true; }
@@ -187,13 +252,67 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
             }
         }
         const int form = (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED) ? d->falloff_form[i] : 0;
-        const int single = pd && d->tb_species[i] >= 0;
+        const int single = is_pd(t) && d->tb_species[i] >= 0;
         meta |= (uint32_t)t << 24 | (uint32_t)rv << 27 | (uint32_t)form << 29 | (uint32_t)single << 31;
         o.slots[4 * s + 0] = spec[0] | spec[1] << 16;
         o.slots[4 * s + 1] = spec[2] | spec[3] << 16;
         o.slots[4 * s + 2] = spec[4] | spec[5] << 16;
         o.slots[4 * s + 3] = meta;
-        if (pk) {
+
+        // sum_k nu_ki B_k(T) as one polynomial per interval between the t_mid of the species
+        {
+            std::vector<double> brk;
+            for (auto &pr : net[s]) brk.push_back(d->t_mid[pr.first]);
+            std::sort(brk.begin(), brk.end());
+            brk.erase(std::unique(brk.begin(), brk.end()), brk.end());
+            const int nint = (int)brk.size() + 1;
+            o.th_off[s] = (uint32_t)o.th_data.size();
+            o.th_data.push_back((double)nint);
+            for (double b : brk) o.th_data.push_back(b);
+            for (int iv = 0; iv < nint; ++iv) {
+                // interval iv: brk[iv-1] < T <= brk[iv]; species k is in its low range iff T <= t_mid[k]
+                double da[7] = {0, 0, 0, 0, 0, 0, 0};
+                for (auto &pr : net[s]) {
+                    const int k = pr.first;
+                    const int m = (int)(std::lower_bound(brk.begin(), brk.end(), d->t_mid[k]) - brk.begin());  // 0-based
+                    const bool low = m >= iv;
+                    const double *a = (low ? d->nasa_lo : d->nasa_hi) + 7 * k;
+                    for (int c = 0; c < 7; ++c) da[c] += (double)pr.second * a[c];
+                }
+                o.th_data.push_back(da[6] - da[0] + (double)dnu * ln_patm_R);   // g0
+                o.th_data.push_back(da[0] - (double)dnu);                        // g1
+                o.th_data.push_back(da[1] * 0.5);                                // g2
+                o.th_data.push_back(da[2] * (1.0 / 6.0));                        // g3
+                o.th_data.push_back(da[3] * (1.0 / 12.0));                       // g4
+                o.th_data.push_back(da[4] * 0.05);                               // g5
+                o.th_data.push_back(-da[5]);                                     // g6
+            }
+        }
+        if (is_pd(t)) {
+            const bool fall = (t != PYJAC_THIRD_BODY);
+            o.lo_lnA.push_back(fall ? std::log(d->arr_lo[3 * i]) : 0.0);
+            o.lo_beta.push_back(fall ? d->arr_lo[3 * i + 1] : 0.0);
+            o.lo_Ta.push_back(fall ? d->arr_lo[3 * i + 2] : 0.0);
+            for (int c = 0; c < 5; ++c) o.fall_par.push_back(fall ? d->falloff_par[5 * i + c] : 0.0);
+            o.eff_vbase.push_back(eff_vb[s]);
+            uint32_t ve = eff_vb[s];
+            const int m = d->tb_species[i];
+            if (m >= 0) {       // Eq. 30: [X]_i = [X_m]; one entry with "alpha - 1" = 1 and no [M] term
+                o.eff_spec.push_back(m);
+                o.eff_eps.push_back(1.0);
+                cols[s].push_back({m, ve});
+            } else {            // Eq. 28 written as [M] + sum_j (alpha_ij - 1)[X_j]
+                for (int q = d->eff_ptr[i]; q < d->eff_ptr[i + 1]; ++q) {
+                    if (d->eff_val[q] == 1.0) continue;
+                    o.eff_spec.push_back(d->eff_spec[q]);
+                    o.eff_eps.push_back(d->eff_val[q] - 1.0);
+                    cols[s].push_back({d->eff_spec[q], ve});
+                    ve += kVStride;
+                }
+            }
+            o.eff_ptr.push_back((int32_t)o.eff_spec.size());
+        }
+        if (is_pk(t)) {
             if (t == PYJAC_PLOG) {
                 const int b = d->plog_ptr[i], e = d->plog_ptr[i + 1];
                 o.pk_data.push_back((double)(e - b));
@@ -218,151 +337,219 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, size_t smem_budget,
             o.pk_ptr.push_back((int32_t)o.pk_data.size());
         }
     }
-    // pressure-dependent tables (third-body efficiencies get their V entries after all slots)
-    for (int s = o.pd_begin; s < o.pd_begin + o.n_pd; ++s) {
-        const int i = order[s];
-        const int t = d->rxn_type[i];
-        const bool fall = (t != PYJAC_THIRD_BODY);
-        o.lo_lnA.push_back(fall ? std::log(d->arr_lo[3 * i]) : 0.0);
-        o.lo_beta.push_back(fall ? d->arr_lo[3 * i + 1] : 0.0);
-        o.lo_Ta.push_back(fall ? d->arr_lo[3 * i + 2] : 0.0);
-        for (int c = 0; c < 5; ++c) o.fall_par.push_back(fall ? d->falloff_par[5 * i + c] : 0.0);
-        const int m = d->tb_species[i];
-        o.tb_spec.push_back(m);
-        o.eff_vbase.push_back(nv);
-        if (m >= 0) {       // Eq. 30: [X]_i = [X_m]; one entry with "alpha - 1" = 1 and no [M] term
-            o.eff_spec.push_back(m);
-            o.eff_eps.push_back(1.0);
-            cols[s].push_back({m, nv++});
-        } else {            // Eq. 28 written as [M] + sum_j (alpha_ij - 1)[X_j]
-            for (int q = d->eff_ptr[i]; q < d->eff_ptr[i + 1]; ++q) {
-                if (d->eff_val[q] == 1.0) continue;
-                o.eff_spec.push_back(d->eff_spec[q]);
-                o.eff_eps.push_back(d->eff_val[q] - 1.0);
-                cols[s].push_back({d->eff_spec[q], nv++});
-            }
-        }
-        o.eff_ptr.push_back((int32_t)o.eff_spec.size());
+
+    // ---- AUX tasks that always exist
+    std::vector<Task> tasks;
+    auto scaled = [](uint32_t scalar) { return (uint32_t)kAuxScaled | scalar << 8; };
+    // (a) wdot_k = sum_i nu_ki q_i (Eq. 14) and S1 = sum_i H_i q_i: the rates / dydt kernels need them too
+    for (int k = 0; k < ns; ++k) {
+        Task t;
+        t.out = (uint32_t)(eWdot + k);
+        t.lvl01 = true;
+        tasks.push_back(t);
     }
-    if (o.n_pd == 0) o.pd_begin = nr;
-    if (o.n_pk == 0) o.pk_begin = nr;
-    o.n_v = (int)nv;
+    const size_t tS1 = tasks.size();
+    { Task t; t.flags = kAuxTwoIndex; t.out = (uint32_t)eS1; t.reduce = true; t.lvl01 = true; tasks.push_back(t); }
+    // (b) alpha_r = (W_k / rho) sum_i nu_ki (a_i + W q_i), the coefficient of d_j in row r = k + 1
+    //     (Eqs. 112, 119, 123, 127 regrouped); gamma_r = (W_k / W_Ns) sum_i nu_ki s'_iNs
+    const size_t tAlpha = tasks.size();
+    for (int k = 0; k < ns; ++k) {
+        Task t;
+        t.out = (uint32_t)(eAlpha + k + 1); t.flags = scaled(kIrho); t.cst = d->mol_wt[k];
+        tasks.push_back(t);
+    }
+    const size_t tGamma = tasks.size();
+    for (int k = 0; k < ns; ++k) {
+        Task t;
+        t.out = (uint32_t)(eGamma + k + 1); t.flags = scaled(kOne); t.cst = d->mol_wt[k] * iw_last;
+        tasks.push_back(t);
+    }
+    // (c) energy row (Eq. 113): G0_j = sum_i H_i s'_ij per column, scaled by -1/c_p
+    const size_t tG0 = tasks.size();
+    std::vector<uint32_t> g0_slot(ns, 0u);
+    for (int j = 0; j < ns; ++j) {
+        Task t;
+        t.flags = kAuxTwoIndex | scaled(kNegIcp);
+        if (j == ns - 1) { t.out = (uint32_t)eGamma; t.cst = iw_last; }
+        else { t.out = (uint32_t)next_slot++; t.cst = 1.0; g0_slot[j] = t.out; }
+        tasks.push_back(t);
+    }
+    //     alpha_0 = -(1 / (rho c_p)) sum_i H_i (a_i + W q_i);  S4 = sum_i H_i Theta_i
+    const size_t tA0 = tasks.size();
+    { Task t; t.flags = kAuxTwoIndex | scaled(kNegIrhoIcp); t.out = (uint32_t)eAlpha; t.cst = 1.0; t.reduce = true; tasks.push_back(t); }
+    const size_t tS4 = tasks.size();
+    { Task t; t.flags = kAuxTwoIndex; t.out = (uint32_t)eS4; t.reduce = true; tasks.push_back(t); }
 
-    if (o.n_v + 1 > 65535) throw Fail{PYJAC_ELIMIT, "more than 65534 per-reaction derivative entries"};
-    const uint32_t zero_slot = (uint32_t)o.n_v;
-
-    // ---- cells of the species block: (k, j) += nu_ki s'_ij  (Eqs. 112, 118-127); j = ns-1 is the
-    // virtual column of the terms proportional to 1/W_Nsp
-    std::vector<std::vector<uint32_t>> cell((size_t)ns * ns);   // [j][k]
-    for (int s = 0; s < nr; ++s)
+    // ---- lists of the Jacobian cells, flat column-major index f = r + c * ld
+    std::vector<std::vector<uint32_t>> cell((size_t)ld * ld);
+    for (int s = 0; s < nr; ++s) {
+        const uint32_t hs = (uint32_t)(eH + s);
+        tasks[tS1].ent.push_back((uint32_t)(eQ + s) | hs << 16);
+        tasks[tA0].ent.push_back((uint32_t)(eAr + s) | hs << 16);
+        tasks[tS4].ent.push_back((uint32_t)(eTh + s) | hs << 16);
+        for (auto &ce : cols[s]) tasks[tG0 + ce.spec].ent.push_back(ce.vi | hs << 16);
         for (auto &pr : net[s]) {
             if (pr.second == 0) continue;
-            for (auto &ce : cols[s]) cell[(size_t)ce.spec * ns + pr.first].push_back(pack_entry(ce.vi, pr.second));
-        }
-
-    // ---- species tasks: wdot_k, A_k, Tcol_k = sum_i nu_ki {q_i, a_i, thetaT_i} (Eqs. 14, 111,
-    // 115-117) and the diagonal cell (k, k); kSpLanes lanes per species, longest lists first
-    {
-        std::vector<std::vector<std::pair<uint32_t, uint32_t>>> lists(ns);
-        for (int s = 0; s < nr; ++s)
-            for (auto &pr : net[s]) {
-                if (pr.second == 0) continue;
-                const int k = pr.first;
-                bool first = true;
-                for (auto &ce : cols[s]) {
-                    if (ce.spec != k) continue;
-                    lists[k].push_back({first ? pack_entry((uint32_t)s, pr.second) : (uint32_t)nr,
-                                        pack_entry(ce.vi, pr.second)});
-                    first = false;
-                }
-                if (first) lists[k].push_back({pack_entry((uint32_t)s, pr.second), zero_slot});
+            const int k = pr.first;
+            tasks[k].ent.push_back(pack_entry((uint32_t)(eQ + s), pr.second));
+            tasks[tAlpha + k].ent.push_back(pack_entry((uint32_t)(eAr + s), pr.second));
+            cell[(size_t)(k + 1)].push_back(pack_entry((uint32_t)(eTh + s), pr.second));        // column 0 (d/dT)
+            for (auto &ce : cols[s]) {
+                if (ce.spec == ns - 1) tasks[tGamma + k].ent.push_back(pack_entry(ce.vi, pr.second));
+                else cell[(size_t)(k + 1) + (size_t)(ce.spec + 1) * ld].push_back(pack_entry(ce.vi, pr.second));
             }
-        std::vector<int> ord(ns);
-        std::iota(ord.begin(), ord.end(), 0);
-        std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) { return lists[a].size() > lists[b].size(); });
-        const int per = 32 / kSpLanes;
-        const int nchunk = (ns + per - 1) / per;
-        o.sptask_k.assign((size_t)nchunk * per, -1);
-        for (int c = 0; c < nchunk; ++c) {
-            int steps = 0;
-            for (int i = 0; i < per && c * per + i < ns; ++i) {
-                const int k = ord[c * per + i];
-                o.sptask_k[(size_t)c * per + i] = k;
-                steps = std::max(steps, (int)((lists[k].size() + kSpLanes - 1) / kSpLanes));
-            }
-            const uint32_t base = (uint32_t)(o.sp_ent.size() / 2);
-            o.spchunk.push_back(base);
-            o.spchunk.push_back((uint32_t)steps);
-            o.sp_ent.resize(o.sp_ent.size() + (size_t)2 * steps * 32, 0u);
-            for (int st = 0; st < steps; ++st)
-                for (int lane = 0; lane < 32; ++lane) {
-                    const int i = lane / kSpLanes, sub = lane % kSpLanes;
-                    uint32_t w0 = (uint32_t)nr, w1 = zero_slot;   // coefficient 0 on the zero slots
-                    if (c * per + i < ns) {
-                        const auto &lst = lists[ord[c * per + i]];
-                        const size_t e = (size_t)st * kSpLanes + sub;
-                        if (e < lst.size()) { w0 = lst[e].first; w1 = lst[e].second; }
-                    }
-                    o.sp_ent[2 * ((size_t)base + (size_t)st * 32 + lane) + 0] = w0;
-                    o.sp_ent[2 * ((size_t)base + (size_t)st * 32 + lane) + 1] = w1;
-                }
         }
-        o.n_spchunk = nchunk;
     }
+    for (int j = 0; j < ns - 1; ++j) cell[(size_t)(j + 1) * ld].push_back(pack_entry(g0_slot[j], 1));   // row 0
+    for (auto &c : cell) o.n_list_entries += (long long)c.size();
 
-    // ---- cell tasks per column panel
-    o.ldt = (ns + 1 + 1) & ~1;                 // rows r = 0..ns (r = k + 1), even
-    if ((o.ldt & 3) == 0) o.ldt += 2;            // 2 (mod 4): 2-way instead of 4-way bank conflicts across columns
-    {
-        // shared memory that does not depend on the panel width (doubles), see make_smem_plan
-        const SmemPlan fixed = make_smem_plan(ns, nr, o.n_v, o.ldt, 0);
-        long long room = (long long)smem_budget / 8 - fixed.total;
-        int pw = ns;
-        if ((long long)o.ldt * ns > room) pw = (int)(room / o.ldt);
-        if (panel_override > 0) pw = std::min(ns, (ns + panel_override - 1) / panel_override);
-        if (pw < 1) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
-        if (pw < ns && pw > 8) pw &= ~3;
-        o.pw = pw;
-        o.n_panel = (ns + pw - 1) / pw;
+    // ---- MAIN tasks: 32 consecutive cells; lists longer than the task's cap are summed by an AUX
+    // task and enter as one entry.  The cap minimises (steps of the task) + (steps of the AUX
+    // chunks it causes); `lambda` prices the extra E slots and grows until E fits the shared memory.
+    const size_t ncell = (size_t)ld * ld;
+    o.n_mtask = (int)((ncell + 31) / 32);
+    const size_t fixed_tasks = tasks.size();
+    std::vector<int> cap(o.n_mtask, 0);
+    for (double lambda = 0.15;; lambda *= 2.0) {
+        tasks.resize(fixed_tasks);
+        int slots = next_slot;
+        bool any_overflow = false;
+        for (int t = 0; t < o.n_mtask; ++t) {
+            int len[32], mx = 0;
+            for (int l = 0; l < 32; ++l) {
+                const size_t f = (size_t)t * 32 + l;
+                len[l] = f < ncell ? (int)cell[f].size() : 0;
+                mx = std::max(mx, len[l]);
+            }
+            double best = 1e300;
+            int bestc = mx;
+            for (int c = (mx > 0 ? 1 : 0); c <= mx; ++c) {
+                double cost = (double)c;
+                for (int l = 0; l < 32; ++l)
+                    if (len[l] > c) cost += 1.25 * len[l] / 32.0 + lambda;
+                if (cost < best) { best = cost; bestc = c; }
+            }
+            cap[t] = bestc;
+            for (int l = 0; l < 32; ++l)
+                if (len[l] > bestc) { ++slots; any_overflow = true; }
+        }
+        if (slots + 1 <= std::min<long long>(smem_doubles, 65535)) break;
+        if (!any_overflow) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
+        if (lambda > 1e6) {   // no overflow at all: every list inline
+            for (int t = 0; t < o.n_mtask; ++t) {
+                int mx = 0;
+                for (int l = 0; l < 32; ++l) {
+                    const size_t f = (size_t)t * 32 + l;
+                    if (f < ncell) mx = std::max(mx, (int)cell[f].size());
+                }
+                cap[t] = mx;
+            }
+            if (next_slot + 1 > std::min<long long>(smem_doubles, 65535))
+                throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
+            break;
+        }
     }
-    const uint32_t pad_addr = (uint32_t)(o.ldt * o.pw);
-    for (int p = 0; p < o.n_panel; ++p) {
-        const int j0 = p * o.pw, j1 = std::min(ns, j0 + o.pw);
-        std::vector<std::pair<int, int>> tasks;   // (j, k) with a non-empty list, off the diagonal
-        for (int j = j0; j < j1; ++j)
-            for (int k = 0; k < ns; ++k)
-                if (k != j && !cell[(size_t)j * ns + k].empty()) tasks.push_back({j, k});
-        std::stable_sort(tasks.begin(), tasks.end(), [&](const std::pair<int, int> &a, const std::pair<int, int> &b) {
-            return cell[(size_t)a.first * ns + a.second].size() > cell[(size_t)b.first * ns + b.second].size();
+    for (int t = 0; t < o.n_mtask; ++t)
+        for (int l = 0; l < 32; ++l) {
+            const size_t f = (size_t)t * 32 + l;
+            if (f >= ncell || (int)cell[f].size() <= cap[t]) continue;
+            Task a;
+            a.out = (uint32_t)next_slot++;
+            a.ent.swap(cell[f]);
+            tasks.push_back(a);
+            cell[f].push_back(pack_entry(tasks.back().out, 1));
+        }
+    const int eZero = next_slot++;
+    o.eZero = eZero;
+    o.n_e = next_slot;
+    if (o.n_e > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-state table entries"};
+    const uint32_t pad1 = pack_entry((uint32_t)eZero, 0);
+    const uint32_t pad2 = (uint32_t)eZero | (uint32_t)eZero << 16;
+
+    // ---- MAIN entries
+    o.mtask.assign((size_t)4 * o.n_mtask, 0u);
+    for (int t = 0; t < o.n_mtask; ++t) {
+        const uint32_t base = (uint32_t)o.m_ent.size();
+        o.mtask[4 * t + 0] = base;
+        o.mtask[4 * t + 1] = (uint32_t)cap[t];
+        o.mtask[4 * t + 2] = (uint32_t)(((size_t)t * 32) % ld);
+        o.mtask[4 * t + 3] = (uint32_t)(((size_t)t * 32) / ld);
+        o.m_ent.resize(o.m_ent.size() + (size_t)cap[t] * 32, pad1);
+        for (int l = 0; l < 32; ++l) {
+            const size_t f = (size_t)t * 32 + l;
+            if (f >= ncell) continue;
+            for (size_t e = 0; e < cell[f].size(); ++e) o.m_ent[(size_t)base + e * 32 + l] = cell[f][e];
+        }
+        o.n_main_entries += (long long)cap[t] * 32;
+    }
+    if (o.m_ent.empty()) o.m_ent.push_back(pad1);
+
+    // ---- AUX chunks: tasks with equal flags and similar length share a chunk of 32 lanes
+    struct Chunk { std::vector<size_t> t; int steps; bool lvl01; bool reduce; };
+    std::vector<Chunk> chunks;
+    {
+        std::vector<size_t> idx;
+        for (size_t t = 0; t < tasks.size(); ++t) {
+            if (tasks[t].reduce) chunks.push_back({{t}, (int)((tasks[t].ent.size() + 31) / 32), tasks[t].lvl01, true});
+            else idx.push_back(t);
+        }
+        std::stable_sort(idx.begin(), idx.end(), [&](size_t a, size_t b) {
+            if (tasks[a].lvl01 != tasks[b].lvl01) return tasks[a].lvl01;
+            if (tasks[a].flags != tasks[b].flags) return tasks[a].flags < tasks[b].flags;
+            return tasks[a].ent.size() > tasks[b].ent.size();
         });
-        o.panel_chunks.push_back((int32_t)(o.cchunk.size() / 2));
-        for (size_t t0 = 0; t0 < tasks.size(); t0 += 32) {
-            const int steps = (int)cell[(size_t)tasks[t0].first * ns + tasks[t0].second].size();
-            const uint32_t base = (uint32_t)o.c_ent.size();
-            o.cchunk.push_back(base);
-            o.cchunk.push_back((uint32_t)steps);
-            o.c_ent.resize(o.c_ent.size() + (size_t)steps * 32, zero_slot);
-            for (int lane = 0; lane < 32; ++lane) {
-                if (t0 + lane >= tasks.size()) { o.ctask_addr.push_back(pad_addr); continue; }
-                const int j = tasks[t0 + lane].first, k = tasks[t0 + lane].second;
-                o.ctask_addr.push_back((uint32_t)(k + 1 + (j - j0) * o.ldt));
-                const auto &lst = cell[(size_t)j * ns + k];
-                for (size_t e = 0; e < lst.size(); ++e) o.c_ent[(size_t)base + e * 32 + lane] = lst[e];
+        for (size_t p = 0; p < idx.size();) {
+            Chunk c{{}, 0, tasks[idx[p]].lvl01, false};
+            const uint32_t fl = tasks[idx[p]].flags;
+            while (p < idx.size() && c.t.size() < 32 && tasks[idx[p]].lvl01 == c.lvl01 && tasks[idx[p]].flags == fl) {
+                c.steps = std::max(c.steps, (int)tasks[idx[p]].ent.size());
+                c.t.push_back(idx[p++]);
+            }
+            chunks.push_back(c);
+        }
+        // longest first (the warps take chunks from a queue); the rates / dydt subset in front
+        std::stable_sort(chunks.begin(), chunks.end(), [&](const Chunk &a, const Chunk &b) {
+            if (a.lvl01 != b.lvl01) return a.lvl01;
+            return a.steps > b.steps;
+        });
+    }
+    o.n_achunk = (int)chunks.size();
+    o.n_achunk01 = 0;
+    for (auto &c : chunks) o.n_achunk01 += c.lvl01 ? 1 : 0;
+    for (auto &c : chunks) {
+        const Task &t0 = tasks[c.t[0]];
+        const uint32_t base = (uint32_t)o.a_ent.size();
+        const bool two = (t0.flags & kAuxTwoIndex) != 0;
+        o.a_ent.resize(o.a_ent.size() + (size_t)c.steps * 32, two ? pad2 : pad1);
+        o.achunk.push_back(base);
+        o.achunk.push_back((uint32_t)c.steps);
+        o.achunk.push_back(t0.flags | (c.reduce ? (uint32_t)kAuxReduce : 0u));
+        o.achunk.push_back((uint32_t)o.a_out.size());
+        if (c.reduce) {
+            for (size_t e = 0; e < t0.ent.size(); ++e) o.a_ent[(size_t)base + (e / 32) * 32 + (e % 32)] = t0.ent[e];
+            o.a_out.push_back(t0.out);
+            o.a_const.push_back(t0.cst);
+            for (int l = 1; l < 32; ++l) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); }
+        } else {
+            for (int l = 0; l < 32; ++l) {
+                if (l >= (int)c.t.size()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); continue; }
+                const Task &t = tasks[c.t[l]];
+                o.a_out.push_back(t.out);
+                o.a_const.push_back(t.cst);
+                for (size_t e = 0; e < t.ent.size(); ++e) o.a_ent[(size_t)base + e * 32 + l] = t.ent[e];
             }
         }
-        o.panel_chunks.push_back((int32_t)(o.cchunk.size() / 2));
+        o.n_aux_entries += (long long)c.steps * 32;
     }
-    if (o.c_ent.empty()) o.c_ent.push_back(zero_slot);
-    if (o.cchunk.empty()) { o.cchunk.push_back(0u); o.cchunk.push_back(0u); }
-    if (o.ctask_addr.empty()) o.ctask_addr.push_back(pad_addr);
-    if (o.sp_ent.empty()) { o.sp_ent.push_back((uint32_t)nr); o.sp_ent.push_back(zero_slot); }
+    if (o.a_ent.empty()) o.a_ent.push_back(pad1);
+    if (o.achunk.empty()) { o.achunk.assign(4, 0u); }
+    if (o.a_out.empty()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); }
 }
 
-int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, size_t smem_budget, int panel_override,
-                   const char **why)
+int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, long long smem_doubles, const char **why)
 {
     try {
-        pack_impl(d, out, smem_budget, panel_override);
+        pack_impl(d, out, smem_doubles);
     } catch (const Fail &f) {
         if (why) *why = f.why;
         return f.code;
