@@ -123,21 +123,22 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk;
     dm.n_achunk = hp.n_achunk; dm.n_achunk01 = hp.n_achunk01; dm.n_mtask = hp.n_mtask;
     dm.eQ = hp.eQ; dm.eAr = hp.eAr; dm.eTh = hp.eTh; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;
-    dm.eWdot = hp.eWdot; dm.eS1 = hp.eS1; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.n_e = hp.n_e;
+    dm.eWdot = hp.eWdot; dm.eTcol = hp.eTcol; dm.eG0 = hp.eG0; dm.eZ = hp.eZ;
+    dm.eS1 = hp.eS1; dm.eA0 = hp.eA0; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.eDump = hp.eDump; dm.n_e = hp.n_e;
     Uploader up;
     try {
-        up.add(&dm.inv_mw, hp.inv_mw);
+        up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.mw, hp.mw);
         up.add((const double **)&dm.colc, hp.colc); up.add(&dm.wrow, hp.wrow);
         up.add(&dm.nasa, hp.nasa); up.add(&dm.t_mid, hp.t_mid);
-        up.add((const uint32_t **)&dm.slots, hp.slots);
+        up.add(&dm.rchunk, hp.rchunk);
+        up.add((const uint32_t **)&dm.slots, hp.slots); up.add((const uint32_t **)&dm.vidx, hp.vidx);
         up.add(&dm.lnA, hp.lnA); up.add(&dm.beta, hp.beta); up.add(&dm.Ta, hp.Ta);
-        up.add(&dm.vbase, hp.vbase); up.add(&dm.rxn_orig, hp.rxn_orig);
+        up.add(&dm.rxn_orig, hp.rxn_orig);
         up.add(&dm.rev_lnA, hp.rev_lnA); up.add(&dm.rev_beta, hp.rev_beta); up.add(&dm.rev_Ta, hp.rev_Ta);
-        up.add(&dm.th_off, hp.th_off); up.add(&dm.th_data, hp.th_data);
+        up.add(&dm.th_off, hp.th_off); up.add(&dm.th_data, hp.th_data); up.add(&dm.th_soa, hp.th_soa);
         up.add(&dm.lo_lnA, hp.lo_lnA); up.add(&dm.lo_beta, hp.lo_beta); up.add(&dm.lo_Ta, hp.lo_Ta);
         up.add(&dm.fall_par, hp.fall_par);
         up.add(&dm.eff_ptr, hp.eff_ptr); up.add(&dm.eff_spec, hp.eff_spec); up.add(&dm.eff_eps, hp.eff_eps);
-        up.add(&dm.eff_vbase, hp.eff_vbase);
         up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
         up.add((const uint32_t **)&dm.achunk, hp.achunk); up.add(&dm.a_ent, hp.a_ent);
         up.add(&dm.a_out, hp.a_out); up.add(&dm.a_const, hp.a_const);

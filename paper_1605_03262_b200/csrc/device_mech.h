@@ -4,16 +4,17 @@
 // Notation follows the paper (PAPER.md Sections 2-4): species k, reaction i, nu' / nu'' the
 // reactant / product coefficients (Eq. 15), [X_k] concentrations (Eq. 5), c_i the pressure
 // modification (Eq. 20).  Reactions are stored in a SORTED order (most expensive rate form first,
-// one form per group of 32); `rxn_orig` maps back to the caller's order.
+// the plain elementary ones last); `rxn_orig` maps back to the caller's order.
 //
-// The evaluation is a chain of gathers over one per-state array `E` in shared memory:
+// The evaluation is a chain of fixed-order gathers over one per-state array `E` in shared memory:
 //   phase 1 writes, per reaction, the reusable products of Section 4.1:
 //           the sparse derivative terms s'_ij (region V), q_i, a_i, Theta_dT,i and the reaction
 //           enthalpy H_i (regions Q, Ar, Th, H);
-//   the AUX gathers sum them into per-species / per-column quantities (regions Alpha, Gamma, Wdot,
-//           the scalars S1, S4 and the sums of the long cell lists, region Ovf);
+//   the AUX gathers sum them into per-species / per-column quantities (wdot_k, alpha_r, gamma_r,
+//           the T column, the column sums of the energy row, the sums of the long cell lists);
+//   a short FIX phase finishes the energy row (Eq. 113) into region Z;
 //   the MAIN pass owns the Jacobian as a flat array: lane <-> one output element, which gathers
-//           its (short) list from E, applies Eq. 112 / 113 and stores -- there is no Jacobian tile.
+//           its (short) list from E, applies Eq. 112 and stores -- there is no Jacobian tile.
 #pragma once
 #include <cstdint>
 
@@ -22,10 +23,12 @@ namespace pyjac {
 constexpr double kRu = 8314.46261815324;   // J kmol^-1 K^-1
 constexpr double kPatm = 101325.0;         // Pa
 constexpr int kMaxSide = 3;                // species per reaction side
-constexpr int kVStride = 32;               // V entries of one reaction are 32 apart (lane-contiguous stores)
 
 // meta word of a reaction: bits 0..23 six 4-bit nu (slots 0-2 reactants, 3-5 products; 0 = empty
 // slot), 24..26 rxn_type, 27..28 rev_type, 29..30 falloff_form, 31 third body is a single species.
+// A reaction with at most three molecules per side is stored with one slot per MOLECULE (nu = 1,
+// a species may repeat): then R_f = k_f [X_a][X_b][X_c] and every S'_j of Eq. 120 is a product of
+// the other slots -- no powers, and the repeated slots' list entries add up to nu [X]^(nu-1).
 __host__ __device__ inline int meta_nu(uint32_t m, int slot) { return (m >> (4 * slot)) & 0xF; }
 __host__ __device__ inline int meta_type(uint32_t m) { return (m >> 24) & 7; }
 __host__ __device__ inline int meta_rev(uint32_t m) { return (m >> 27) & 3; }
@@ -38,16 +41,18 @@ __host__ __device__ inline uint32_t pack_entry(uint32_t src, int coef)
 {
     uint32_t a = coef < 0 ? uint32_t(-coef) : uint32_t(coef);
     uint32_t hi = a == 1 ? 0x3FF0u : a == 2 ? 0x4000u : a == 3 ? 0x4008u
-                : a == 4 ? 0x4010u : a == 5 ? 0x4014u : a == 6 ? 0x4018u : 0u;
+                : a == 4 ? 0x4010u : a == 5 ? 0x4014u : a == 6 ? 0x4018u
+                : a == 7 ? 0x401Cu : a == 8 ? 0x4020u : a == 9 ? 0x4022u : 0u;
     if (coef < 0) hi |= 0x8000u;
     return (hi << 16) | (src & 0xFFFFu);
 }
 
-// aux chunk flags (AuxChunk.z)
+// kinds of AUX chunks (AuxChunk.z bits 0..7; bits 8..15 = log2 of the lanes that share one sum)
 enum : uint32_t {
-    kAuxTwoIndex = 1u,   // entries are {index a | index b << 16}: sum of E[a] * E[b]
-    kAuxReduce = 2u,     // the 32 lanes hold parts of ONE sum: butterfly, lane 0 stores to slot w
-    kAuxScaled = 4u,     // result *= task constant * per-state scalar (index in bits 8..15)
+    kAuxT3 = 0,    // entries {E index of q_i, nu_ki}: sums of nu q_i, nu a_i, nu Theta_i -> wdot_k, alpha_{k+1}, T column
+    kAuxS1 = 1,    // entries {E index, coef}: one sum, times a task constant -> E slot
+    kAuxH2 = 2,    // entries {index a | index b << 16}: sum of E[a] * E[b] -> E slot
+    kAuxR3 = 3,    // no entries: sums over all reactions of H_i {q_i, a_i, Theta_i} -> S1, A0, S4
 };
 
 struct DeviceMech {
@@ -55,17 +60,22 @@ struct DeviceMech {
     int ld;                     // N_sp + 1
     // ---- species tables
     const double *inv_mw;       // [ns]
+    const double *mw;           // [ns]
     const double2 *colc;        // [ns+1] column constants by Jacobian column c: {d_j, 1/W_j}, j = c - 1;
-                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51); c = 0: {0, 1}
+                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51);
+                                //        c = 0: {0, 1}; c = ns (the zero column): {0, 0}
     const double *wrow;         // [ns+1] row factors by Jacobian row r: {1, W_0 .. W_{ns-1}}
     const double *nasa;         // [2][5][ns] a_0..a_4, range-major, coefficient-major (coalesced over k)
     const double *t_mid;        // [ns]
     // ---- reaction tables, sorted order
     int n_pd;                   // pressure-dependent reactions (third body, falloff, chem. activated): [0, n_pd)
     int n_pk;                   // PLOG / Chebyshev reactions: [n_pd, n_pd + n_pk)
+    int n_rchunk;               // groups of 32 reactions
+    const uint32_t *rchunk;     // [n_rchunk] 1 = every reaction of the group takes the plain path
     const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
+    const uint4 *vidx;          // [nr] E indices of the slots' s'_ij: {v0|v1<<16, v2|v3<<16, v4|v5<<16, 0}
+                                //      (empty slots point at the dump slot)
     const double *lnA, *beta, *Ta;               // [nr] forward Arrhenius (k_inf for falloff forms)
-    const uint32_t *vbase;      // [nr] E index of the first used slot's s'_ij; the n-th used slot is n*kVStride further
     const int32_t *rxn_orig;    // [nr] caller's reaction index
     const double *rev_lnA, *rev_beta, *rev_Ta;   // [nr] explicit reverse parameters
     const uint32_t *th_off;     // [nr] offset into th_data
@@ -73,50 +83,58 @@ struct DeviceMech {
                                 // sum_k nu_ki B_k(T) = g0 + g1 ln T + T (g2 + T (g3 + T (g4 + T g5))) + g6 / T
                                 // (Eq. 27 summed over the reaction, one set per interval between the t_mid of
                                 // its species; g0 includes (sum nu) ln(p_atm / R) of Eq. 26)
+    const double *th_soa;       // [15][nr] the same for reactions with n_int <= 2, coalesced over reactions:
+                                // row 0 the breakpoint (+inf if n_int = 1), rows 1..7 g of the lower interval,
+                                // rows 8..14 g of the upper one
     const double *lo_lnA, *lo_beta, *lo_Ta;      // [n_pd] k_0
     const double *fall_par;                      // [n_pd][5]
     const int32_t *eff_ptr;                      // [n_pd+1]
-    const int32_t *eff_spec;                     // species of alpha_ij != 1 (or the single species)
+    const uint32_t *eff_spec;                    // species of alpha_ij != 1 (or the single species) | E index of its term << 16
     const double *eff_eps;                       // alpha_ij - 1      (1 for the single species)
-    const uint32_t *eff_vbase;                   // [n_pd] E index of the first efficiency term (stride kVStride)
     const int32_t *pk_ptr;      // [n_pk+1] offsets into pk_data
     const double *pk_data;      // PLOG: n, then n x {p, ln p, ln A, beta, Ta};
                                 // Chebyshev: nT, nP, 1/Tmin, 1/Tmax, log10 pmin, log10 pmax, eta[nT*nP]
-    int n_rchunk;               // groups of 32 reactions
-    // ---- AUX gathers: chunks of 32 tasks with equally long lists (sorted at create time)
+    // ---- AUX gathers: chunks of 32 lanes, 32 >> rshift sums each, sorted by length at create time
     int n_achunk;               // all chunks (Jacobian); the first n_achunk01 serve rates / dydt too
     int n_achunk01;
-    const uint4 *achunk;        // {first entry, steps, flags | scalar << 8, REDUCE: E slot; else first task}
+    const uint4 *achunk;        // {first entry, steps, kind | rshift << 8, first task}
     const uint32_t *a_ent;      // entries at [first + step*32 + lane]
-    const uint32_t *a_out;      // [task] E slot of the result
-    const double *a_const;      // [task] constant factor of scaled tasks
+    const uint32_t *a_out;      // [task] E slot of the result (kAuxT3: the species k)
+    const double *a_const;      // [task] constant factor (kAuxS1)
     // ---- MAIN pass: the Jacobian as a flat column-major array, 32 consecutive elements per task
     int n_mtask;
-    const uint4 *mtask;         // {first entry, steps, row of lane 0, column of lane 0}
+    const uint4 *mtask;         // {first entry, steps | edge << 16, row of lane 0, column of lane 0}
     const uint32_t *m_ent;      // entries at [first + step*32 + lane]
     // ---- regions of E (indices in doubles per state)
-    int eQ, eAr, eTh, eH;       // [nr] each
-    int eAlpha, eGamma;         // [ns+1] by Jacobian row
+    int eQ, eAr, eTh, eH;       // [nr] each, consecutive (eAr = eQ + nr, eTh = eQ + 2 nr, eH = eQ + 3 nr)
+    int eAlpha, eGamma;         // [ns+1] by Jacobian row; row 0 stays 0
     int eWdot;                  // [ns]
-    int eS1, eS4;               // scalars: sum_i H_i q_i, sum_i H_i Theta_i
+    int eTcol;                  // [ns]   (1/rho) sum_i nu_ki Theta_i
+    int eG0;                    // [ns]   sum_i H_i s'_ij per column species j
+    int eZ;                     // [ns+1] finished energy row: Z_c = J(0,c) W_j (c >= 1), Z_0 = J(0,0)
+    int eS1, eA0, eS4;          // scalars: sum_i H_i q_i, sum_i H_i a_i, sum_i H_i Theta_i
     int eZero;                  // a slot that stays 0 (padding of the lists)
+    int eDump;                  // a slot nobody reads (stores of empty reaction slots)
     int n_e;                    // size of E
 };
 
 // per-state scalars (region Scal of the shared-memory plan)
 enum {
-    kOne = 0, kIrho, kNegIcp, kNegIrhoIcp,          // factors of the scaled AUX tasks (kOne stays 1)
-    kT, kLnT, kInvT, kP, kRho, kW, kM, kCpMix, kDcpDT, kNScal = 16
+    kT = 0, kLnT, kInvT, kP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kNScal = 12
 };
 
 // Shared-memory plan (offsets in doubles PER STATE).  A CTA evaluates S states at a time and
-// interleaves them: element i of region R of state q lives at (R + i) * S + q.
+// interleaves them: element i of region R of state q lives at (R + i) * S + q.  After the S
+// interleaved state blocks come the state-independent tables (colc, wrow), loaded once per CTA.
 struct SmemPlan {
     int E;                              // [n_e]
     int X;                              // [ns+1] concentrations; slot ns = 1 (empty reaction slots)
     int Cp;                             // [ns] c_pk (mass based)
     int Scal;                           // [2][kNScal], double-buffered by iteration parity
     int total;                          // doubles per state
+    int colc;                           // [ld] double2, offset in doubles from the end of the state blocks
+    int wrow;                           // [ld]
+    int shared_total;                   // doubles of the state-independent part
 };
 
 inline SmemPlan make_smem_plan(int ns, int n_e)
@@ -129,9 +147,11 @@ inline SmemPlan make_smem_plan(int ns, int n_e)
     p.Cp = take(ns);
     p.Scal = take(2 * kNScal);
     p.total = o;
+    o = 0;
+    p.colc = take(2 * (ns + 1));
+    p.wrow = take(ns + 1);
+    p.shared_total = o;
     return p;
 }
-
-constexpr int kRedRows = 4;             // block-reduction scratch: kRedRows x 32 doubles per state
 
 }  // namespace pyjac

@@ -3,21 +3,27 @@
 // One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop; the S
 // states are interleaved in shared memory (element i of a region for state q at (R + i) * S + q), so
 // whatever does not depend on the state -- decoding a reaction, a gather entry, a column constant --
-// is done once and applied to the S states with one vector load.  Per iteration:
-//   phase 0  mixture (Eqs. 3-5) and species: [X_k], c_pk, mixture c_p and d c_p / dT (Eqs. 9-13, 54-55)
-//   phase 1  reactions, one thread per reaction, groups of 32 of one rate form taken from a queue:
-//            k_f, k_r (K_c from the per-reaction polynomial of device_mech.h `th_data`), R_f, R_r, c_i
-//            and the reusable per-reaction products of Section 4.1 into E:
-//            q_i, Theta_dT,i, a_i (the coefficient of d_j), the sparse terms s'_ij, the enthalpy H_i
-//   AUX      fixed-order gathers over E, 32 equally long lists per warp: wdot_k (Eq. 14), the row
-//            vectors alpha_r, gamma_r of Eq. 112, the column sums of the energy row (Eq. 113) and the
-//            sums of the long Jacobian cell lists
-//   MAIN     the Jacobian as a flat column-major array: lane <-> output element.  Each element
-//            gathers its short list from E and is stored straight from the register:
-//              J(r, c) = alpha_r d_j + (W_k / W_j) sum_i nu_ki s'_ij - gamma_r        (r = k+1, c = j+1)
-//            which is Eq. 112 with the per-reaction terms of Eqs. 118-127 regrouped by what they
-//            multiply.  A warp stores 256 contiguous bytes.
-// There are no atomics on data and no Jacobian tile: every sum has an order fixed at pyjac_mech_create.
+// is done once and applied to the S states with one vector load.  All work is assigned to the warps
+// statically (item i of a phase goes to warp i mod NW; the items were sorted by cost at create
+// time).  Per iteration:
+//   P0    mixture (Eqs. 3-5) and species, warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT
+//         (Eqs. 9-13, 54-55)
+//   P1    reactions, lane <-> reaction, groups of 32: k_f, k_r (K_c from the per-reaction polynomial
+//         of device_mech.h `th_data`), R_f, R_r, c_i and the reusable per-reaction products of
+//         Section 4.1 into E: q_i, Theta_dT,i, a_i (the coefficient of d_j), the
+//         sparse terms s'_ij, the enthalpy H_i.  Groups made only of plain elementary reactions take
+//         a branch-free path that evaluates two states at a time.
+//   AUX   fixed-order gathers over E: wdot_k (Eq. 14), alpha_r, gamma_r of Eq. 112, the T column
+//         (Eq. 111), the column sums of the energy row (Eq. 113), the sums of long cell lists.
+//         2^rshift neighbouring lanes share one sum (butterfly at the end).
+//   FIX   the energy row, Eq. 113, per column into region Z
+//   MAIN  the Jacobian as a flat column-major array: lane <-> output element.  Each element
+//         gathers its short list from E and is stored straight from the register:
+//           J(r, c) = alpha_r d_j + (W_k / W_j) sum_i nu_ki s'_ij - gamma_r        (r = k+1, c = j+1)
+//         which is Eq. 112 with the per-reaction terms of Eqs. 118-127 regrouped by what they
+//         multiply.  Row 0 and column 0 are lists of one finished entry
+//         (Z_c, the T column), so the pass has no special cases.  A warp stores 256 contiguous bytes.
+// There are no atomics and no Jacobian tile: every sum has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
 
 #include "device_mech.h"
@@ -113,18 +119,93 @@ __device__ __forceinline__ void stv(double *p, const double (&v)[S])
     }
 }
 
-// next item of a phase's work queue (one shared counter per phase)
-__device__ __forceinline__ int grab(int *ctr, int lane)
+// ---- P1, plain path: 32 elementary reactions with at most three molecules per side (one slot per
+// molecule), k_r from K_c or irreversible, one NASA breakpoint.  Two states at a time, no branches.
+template <int LEVEL, int S>
+__device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemPlan &sp, double *sm, const double *sc,
+                                                int s, const EvalOut &out, long long state0, long long n)
 {
-    int t = 0;
-    if (lane == 0) t = atomicAdd(ctr, 1);
-    return __shfl_sync(0xFFFFFFFFu, t, 0);
+    constexpr int SP = S >= 2 ? 2 : 1;
+    const int nr = m.nr;
+    const uint4 sl = m.slots[s];
+    const uint32_t meta = sl.w;
+    const double *X = sm + sp.X * S;
+    double *E = sm + sp.E * S;
+    const int x0 = (sl.x & 0xFFFF) * S, x1 = (sl.x >> 16) * S, x2 = (sl.y & 0xFFFF) * S,
+              x3 = (sl.y >> 16) * S, x4 = (sl.z & 0xFFFF) * S, x5 = (sl.z >> 16) * S;
+    const int nf = (meta & 0xF) + ((meta >> 4) & 0xF) + ((meta >> 8) & 0xF);
+    const int nb = ((meta >> 12) & 0xF) + ((meta >> 16) & 0xF) + ((meta >> 20) & 0xF);
+    const double snf = (double)nf, snr = (double)nb, dnu = (double)(nb - nf);
+    const bool rev = meta_rev(meta) != PYJAC_IRREVERSIBLE;
+    const double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
+    const double *th = m.th_soa + s;
+    const double brk = th[0];
+    int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
+    if (LEVEL == 2) {
+        const uint4 vi = m.vidx[s];
+        v0 = (vi.x & 0xFFFF) * S; v1 = (vi.x >> 16) * S; v2 = (vi.y & 0xFFFF) * S;
+        v3 = (vi.y >> 16) * S; v4 = (vi.z & 0xFFFF) * S; v5 = (vi.z >> 16) * S;
+    }
+    const int orig = LEVEL == 0 ? m.rxn_orig[s] : 0;
+
+#pragma unroll 1
+    for (int q0 = 0; q0 < S; q0 += SP) {
+        double T[SP], lnT[SP], invT[SP], lnkf[SP], L[SP], sB[SP], sdB[SP], kf[SP], kr[SP];
+#pragma unroll
+        for (int u = 0; u < SP; ++u) {
+            T[u] = sc[kT * S + q0 + u]; lnT[u] = sc[kLnT * S + q0 + u]; invT[u] = sc[kInvT * S + q0 + u];
+            lnkf[u] = fma(beta, lnT[u], fma(-Ta, invT[u], lnA));                 // Eq. 21
+            L[u] = fma(Ta, invT[u], beta) * invT[u];                             // Eq. 65
+        }
+        // sum_k nu_ki B_k (Eq. 27 over the reaction) and its T derivative (Eq. 74)
+#pragma unroll
+        for (int u = 0; u < SP; ++u) {
+            const double *g = th + (size_t)(T[u] > brk ? 8 : 1) * nr;
+            const double g0 = g[0], g1 = g[nr], g2 = g[2 * (size_t)nr], g3 = g[3 * (size_t)nr], g4 = g[4 * (size_t)nr],
+                         g5 = g[5 * (size_t)nr], g6 = g[6 * (size_t)nr];
+            const double t = T[u];
+            sB[u] = fma(g1, lnT[u], g0) + fma(t, fma(t, fma(t, fma(t, g5, g4), g3), g2), g6 * invT[u]);
+            sdB[u] = fma(fma(-g6, invT[u], g1), invT[u], g2) + t * fma(t, fma(4.0 * g5, t, 3.0 * g4), 2.0 * g3);
+        }
+#pragma unroll
+        for (int u = 0; u < SP; ++u) kf[u] = exp_rate(lnkf[u]);
+#pragma unroll
+        for (int u = 0; u < SP; ++u) { kr[u] = exp_rate(lnkf[u] - sB[u]); kr[u] = rev ? kr[u] : 0.0; }   // Eqs. 23-27
+#pragma unroll
+        for (int u = 0; u < SP; ++u) {
+            const int q = q0 + u;
+            const double c0 = X[x0 + q], c1 = X[x1 + q], c2 = X[x2 + q], c3 = X[x3 + q], c4 = X[x4 + q], c5 = X[x5 + q];
+            const double p01 = c0 * c1, p34 = c3 * c4;
+            const double Rf = kf[u] * (p01 * c2), Rr = kr[u] * (p34 * c5);       // Eqs. 18-19
+            const double R = Rf - Rr;
+            E[(m.eQ + s) * S + q] = R;
+            if (LEVEL >= 1) E[(m.eH + s) * S + q] = kRu * T[u] * fma(T[u], sdB[u], dnu);
+            if (LEVEL == 0) {
+                const long long st = state0 + q;
+                if (st < n) {
+                    const long long o = st * nr + orig;
+                    if (out.rf) out.rf[o] = Rf;
+                    if (out.rr) out.rr[o] = Rr;
+                    if (out.cmod) out.cmod[o] = 1.0;
+                }
+            }
+            if (LEVEL == 2) {
+                const double W = sc[kW * S + q];
+                const double iT = invT[u];
+                // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
+                const double dRf = Rf * fma(-snf, iT, L[u]);
+                const double dRr = Rr * (fma(-snr, iT, L[u]) - sdB[u]);
+                E[(m.eTh + s) * S + q] = fma(R, iT, dRf - dRr);
+                E[(m.eAr + s) * S + q] = W * (R - fma(Rf, snf, -Rr * snr));
+                const double nkr = -kr[u];
+                E[v0 + q] = kf[u] * (c1 * c2); E[v1 + q] = kf[u] * (c0 * c2); E[v2 + q] = kf[u] * p01;   // Eq. 120
+                E[v3 + q] = nkr * (c4 * c5); E[v4 + q] = nkr * (c3 * c5); E[v5 + q] = nkr * p34;         // Eq. 121
+            }
+        }
+    }
 }
 
-// ---- phase 1: one reaction, S states --------------------------------------------------------------
-// Everything that does not depend on the state (slot decoding, Arrhenius parameters, table
-// pointers) is read once; the loop over the S states of the CTA is inside.  `sm` is the CTA's
-// shared memory, `sc` the scalar block of this iteration.
+// ---- P1, general path: one reaction of any type, the S states one after the other --------------------
 template <int LEVEL, int S>
 __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *sm, const double *sc,
                                          int s, const EvalOut &out, long long state0, long long n)
@@ -146,6 +227,14 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     const double *th = m.th_data + m.th_off[s];
     const int nint = (int)th[0];
     double *E = sm + sp.E * S;
+    int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
+    if (LEVEL == 2) {
+        const uint4 vi = m.vidx[s];
+        v0 = (vi.x & 0xFFFF) * S; v1 = (vi.x >> 16) * S; v2 = (vi.y & 0xFFFF) * S;
+        v3 = (vi.y >> 16) * S; v4 = (vi.z & 0xFFFF) * S; v5 = (vi.z >> 16) * S;
+    }
+    int eb = 0, ee = 0;
+    if (pdep) { eb = m.eff_ptr[s]; ee = m.eff_ptr[s + 1]; }
 
 #pragma unroll 1
     for (int q = 0; q < S; ++q) {
@@ -226,9 +315,9 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         for (int b = 1; b < nint; ++b) iv += T > th[b] ? 1 : 0;
         const double *g = th + nint + 7 * iv;
         const double g1 = g[1], g2 = g[2], g3 = g[3], g4 = g[4], g5 = g[5], g6 = g[6];
-        const double sB = g[0] + g1 * lnT + T * (g2 + T * (g3 + T * (g4 + T * g5))) + g6 * invT;
-        const double sdB = (g1 - g6 * invT) * invT + g2 + T * (2.0 * g3 + T * (3.0 * g4 + 4.0 * g5 * T));
-        const double H = kRu * T * (T * sdB + dnu);
+        const double sB = fma(g1, lnT, g[0]) + fma(T, fma(T, fma(T, fma(T, g5, g4), g3), g2), g6 * invT);
+        const double sdB = fma(fma(-g6, invT, g1), invT, g2) + T * fma(T, fma(4.0 * g5, T, 3.0 * g4), 2.0 * g3);
+        const double H = kRu * T * fma(T, sdB, dnu);
 
         // ---- concentrations of the six slots (empty slots point at the dummy species [X] = 1)
         const double c0 = X[x0 + q], c1 = X[x1 + q], c2 = X[x2 + q], c3 = X[x3 + q], c4 = X[x4 + q], c5 = X[x5 + q];
@@ -267,11 +356,9 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
 
         // ---- pressure modification c_i (Eq. 20) and its derivatives (Eqs. 77-100)
         double c = 1.0, G = 0.0, fT = 0.0, b = 0.0, Xi = 0.0;
-        int eb = 0, ee = 0;
         if (pdep) {
-            eb = m.eff_ptr[s]; ee = m.eff_ptr[s + 1];
             Xi = meta_single(meta) ? 0.0 : sc[kM * S + q];               // Eqs. 28-30
-            for (int e = eb; e < ee; ++e) Xi += m.eff_eps[e] * X[m.eff_spec[e] * S + q];
+            for (int e = eb; e < ee; ++e) Xi += m.eff_eps[e] * X[(m.eff_spec[e] & 0xFFFF) * S + q];
             if (type == PYJAC_THIRD_BODY) {
                 c = Xi; G = Xi; lPrT = -invT; b = R;                     // Eqs. 79-80
             } else {
@@ -312,7 +399,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         }
         const double qi = c * R;
         E[(m.eQ + s) * S + q] = qi;
-        E[(m.eH + s) * S + q] = H;
+        if (LEVEL >= 1) E[(m.eH + s) * S + q] = H;
         if (LEVEL == 0) {
             const long long st = state0 + q;
             if (st < n) {
@@ -336,154 +423,191 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             E[(m.eAr + s) * S + q] = c * base + b * (mix - W * Xi) + W * qi;
             // sparse terms s'_ij = c (k_f S'_j - k_r S''_j) per slot, b (alpha_ij - 1) per efficiency
             const double ckf = c * kf, ckr = -c * kr;
-            double *V = E + m.vbase[s] * S + q;
-            if (meta & 0x00000Fu) { *V = ckf * sk0; V += kVStride * S; }
-            if (meta & 0x0000F0u) { *V = ckf * sk1; V += kVStride * S; }
-            if (meta & 0x000F00u) { *V = ckf * sk2; V += kVStride * S; }
-            if (meta & 0x00F000u) { *V = ckr * sk3; V += kVStride * S; }
-            if (meta & 0x0F0000u) { *V = ckr * sk4; V += kVStride * S; }
-            if (meta & 0xF00000u) { *V = ckr * sk5; V += kVStride * S; }
-            if (pdep) {
-                double *Ve = E + m.eff_vbase[s] * S + q;
-                for (int e = eb; e < ee; ++e, Ve += kVStride * S) *Ve = b * m.eff_eps[e];
-            }
+            E[v0 + q] = ckf * sk0; E[v1 + q] = ckf * sk1; E[v2 + q] = ckf * sk2;
+            E[v3 + q] = ckr * sk3; E[v4 + q] = ckr * sk4; E[v5 + q] = ckr * sk5;
+            for (int e = eb; e < ee; ++e) E[(m.eff_spec[e] >> 16) * S + q] = b * m.eff_eps[e];
         }
     }
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------
-// Shared memory: S interleaved state blocks of sp.total doubles, then kRedRows * S rows of 32 doubles
-// of reduction scratch.  The scalar block is double-buffered by iteration parity: the mixture of the
-// next batch is written while other warps still finish this batch's MAIN pass.
-template <int LEVEL, int NT, int S>
-__global__ void __launch_bounds__(NT, (NT <= 128 ? 4 : NT <= 256 ? 2 : 1))
+// Shared memory: S interleaved state blocks of sp.total doubles, then the state-independent column
+// and row constants.
+template <int LEVEL, int NT, int S, int MB>
+__global__ void __launch_bounds__(NT, MB)
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
                 const double *__restrict__ Pg, const double *__restrict__ Yg, long long ldy, const EvalOut out)
 {
     extern __shared__ __align__(16) double sm[];
-    __shared__ int ctr[4];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
-    const int ns = m.ns, ld = m.ld;
-    double *red = sm + (size_t)sp.total * S;
+    const int ns = m.ns, ld = m.ld, nr = m.nr;
     double *E = sm + sp.E * S;
     double *X = sm + sp.X * S;
     double *Cp = sm + sp.Cp * S;
-    if (tid < S) {   // the empty-slot dummy species, the zero slot and the constant scalar 1
+    double *sc = sm + sp.Scal * S;
+    double2 *colc = reinterpret_cast<double2 *>(sm + (size_t)sp.total * S + sp.colc);
+    double *wrow = sm + (size_t)sp.total * S + sp.wrow;
+    for (int i = tid; i < ld; i += NT) { colc[i] = m.colc[i]; wrow[i] = m.wrow[i]; }
+    if (tid < S) {   // the empty-slot dummy species, the zero slot, row 0 of alpha / gamma
         X[ns * S + tid] = 1.0;
         E[m.eZero * S + tid] = 0.0;
-        sm[(sp.Scal + kOne) * S + tid] = 1.0;
-        sm[(sp.Scal + kNScal + kOne) * S + tid] = 1.0;
+        E[m.eAlpha * S + tid] = 0.0;
+        E[m.eGamma * S + tid] = 0.0;
+        if (nr == 0) { E[m.eS1 * S + tid] = 0.0; E[m.eA0 * S + tid] = 0.0; E[m.eS4 * S + tid] = 0.0; }
     }
     const long long nblk = (n + S - 1) / S;
-    int par = 0;
-    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x, par ^= 1) {
+    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
         const long long state0 = blk * S;
-        double *sc = sm + (sp.Scal + par * kNScal) * S;
-        // ---- phase 0a: mixture molecular weight, density (Eqs. 3-5); warp q <-> state q
+        // ---- P0: mixture (Eqs. 3-5) and species (Eqs. 5, 9, 12-13, 54-55); warp q <-> state q
         for (int q = warp; q < S; q += NW) {
             const long long st = min(state0 + q, n - 1);
+            const double *Ys = Yg + st * ldy;
+            const double T = Tg[st], P = Pg[st];
             double s = 0.0;
-            for (int k = lane; k < ns; k += 32) s += Yg[st * ldy + k] * m.inv_mw[k];
+            for (int k = lane; k < ns; k += 32) s += Ys[k] * m.inv_mw[k];
             s = warp_sum(s);
-            if (lane == 0) {
-                const double T = Tg[st], P = Pg[st];
-                const double W = 1.0 / s, M = P / (kRu * T), rho = M * W;
-                sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P;
-                sc[kM * S + q] = M; sc[kW * S + q] = W; sc[kRho * S + q] = rho; sc[kIrho * S + q] = 1.0 / rho;
-            }
-        }
-        __syncthreads();      // every warp has also left the previous iteration's last phase
-        if (tid == 0) { ctr[0] = 0; ctr[1] = 0; ctr[2] = 0; }
-        // ---- phase 0b: species (Eqs. 5, 9, 12-13, 54-55)
-        {
-            double part[2 * S];
-#pragma unroll
-            for (int i = 0; i < 2 * S; ++i) part[i] = 0.0;
-            for (int k = tid; k < ns; k += NT) {
-                const double iw = m.inv_mw[k], tm = m.t_mid[k];
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    const long long st = min(state0 + q, n - 1);
-                    const double T = sc[kT * S + q];
-                    const double y = Yg[st * ldy + k];
-                    const double *a = m.nasa + (T <= tm ? 0 : (size_t)5 * ns) + k;
+            const double W = 1.0 / s, M = P / (kRu * T), rho = M * W;
+            double cp = 0.0, dcp = 0.0;
+            for (int k = lane; k < ns; k += 32) {
+                const double iw = m.inv_mw[k], y = Ys[k];
+                X[k * S + q] = rho * (y * iw);
+                if (LEVEL >= 1) {
+                    const double *a = m.nasa + (T <= m.t_mid[k] ? 0 : (size_t)5 * ns) + k;
                     const double a0 = a[0], a1 = a[ns], a2 = a[2 * (size_t)ns], a3 = a[3 * (size_t)ns],
                                  a4 = a[4 * (size_t)ns];
-                    X[k * S + q] = sc[kRho * S + q] * (y * iw);
-                    if (LEVEL >= 1) {
-                        const double cpk = kRu * (a0 + T * (a1 + T * (a2 + T * (a3 + a4 * T)))) * iw;
-                        Cp[k * S + q] = cpk;
-                        part[2 * q] += y * cpk;
-                        if (LEVEL == 2) part[2 * q + 1] += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
-                    }
+                    const double cpk = kRu * (a0 + T * (a1 + T * (a2 + T * (a3 + a4 * T)))) * iw;
+                    Cp[k * S + q] = cpk;
+                    cp += y * cpk;
+                    if (LEVEL == 2) dcp += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
                 }
             }
-            if (LEVEL >= 1) {
-#pragma unroll
-                for (int i = 0; i < 2 * S; ++i) {
-                    const double v = warp_sum(part[i]);
-                    if (lane == 0) red[i * 32 + warp] = v;
-                }
+            if (LEVEL >= 1) { cp = warp_sum(cp); dcp = warp_sum(dcp); }
+            if (lane == 0) {
+                sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P;
+                sc[kM * S + q] = M; sc[kW * S + q] = W; sc[kRho * S + q] = rho; sc[kIrho * S + q] = 1.0 / rho;
+                sc[kCpMix * S + q] = cp; sc[kDcpDT * S + q] = dcp;
             }
         }
-        __syncthreads();
-        // ---- phase 1: reactions (the mixture heat capacity is finished on the side)
-        if (LEVEL >= 1 && tid < S) {
-            double cp = 0.0, dcp = 0.0;
-            for (int w = 0; w < NW; ++w) { cp += red[(2 * tid) * 32 + w]; dcp += red[(2 * tid + 1) * 32 + w]; }
-            const double icp = 1.0 / cp;
-            sc[kCpMix * S + tid] = cp; sc[kDcpDT * S + tid] = dcp;
-            sc[kNegIcp * S + tid] = -icp; sc[kNegIrhoIcp * S + tid] = -icp * sc[kIrho * S + tid];
-        }
-        for (int c = grab(&ctr[0], lane); c < m.n_rchunk; c = grab(&ctr[0], lane)) {
-            const int s = c * 32 + lane;
-            if (s < m.nr) reaction<LEVEL, S>(m, sp, sm, sc, s, out, state0, n);
+        __syncthreads();      // every warp has also left the previous iteration's MAIN pass
+        // ---- P1: reactions
+        for (int c = warp; c < m.n_rchunk; c += NW) {
+            const int s = min(c * 32 + lane, nr - 1);      // the last group repeats its last reaction
+            if (m.rchunk[c]) plain_reactions<LEVEL, S>(m, sp, sm, sc, s, out, state0, n);
+            else reaction<LEVEL, S>(m, sp, sm, sc, s, out, state0, n);
         }
         __syncthreads();
         // ---- AUX gathers
         {
             const int nch = LEVEL == 2 ? m.n_achunk : m.n_achunk01;
-            for (int c = grab(&ctr[1], lane); c < nch; c = grab(&ctr[1], lane)) {
+            for (int c = warp; c < nch; c += NW) {
                 const uint4 ch = m.achunk[c];
+                const uint32_t kind = ch.z & 0xFF;
+                const int rshift = (ch.z >> 8) & 0xFF, width = 1 << rshift;
                 const uint32_t *ent = m.a_ent + ch.x + lane;
-                double acc[S];
+                const bool head = (lane & (width - 1)) == 0;
+                const uint32_t task = ch.w + (lane >> rshift);
+                if (kind == kAuxT3 || kind == kAuxR3) {
+                    constexpr int NA = LEVEL == 2 ? 3 : 1;
+                    constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
+                    double acc[NA][S];
 #pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] = 0.0;
-                if (ch.z & kAuxTwoIndex) {
+                    for (int w = 0; w < NA; ++w)
+#pragma unroll
+                        for (int q = 0; q < S; ++q) acc[w][q] = 0.0;
+                    if (kind == kAuxT3) {
 #pragma unroll 2
-                    for (uint32_t t = 0; t < ch.y; ++t) {
-                        const uint32_t e = ent[t * 32];
-                        double a[S], b[S];
-                        ldv<S>(E + (e & 0xFFFF) * S, a);
-                        ldv<S>(E + (e >> 16) * S, b);
+                        for (uint32_t t = 0; t < ch.y; ++t) {
+                            const uint32_t e = ent[t * 32];
+                            const double cf = entry_coef(e);
+                            const double *p = E + (e & 0xFFFF) * S;
 #pragma unroll
-                        for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
+                            for (int w = 0; w < NA; ++w) {
+                                double a[S];
+                                ldv<S>(p + (size_t)w * nr * S, a);
+#pragma unroll
+                                for (int q = 0; q < S; ++q) acc[w][q] = fma(cf, a[q], acc[w][q]);
+                            }
+                        }
+                    } else {
+                        for (int i = lane; i < nr; i += 32) {
+                            double h[S];
+                            ldv<S>(E + (m.eH + i) * S, h);
+#pragma unroll
+                            for (int w = 0; w < NA; ++w) {
+                                double a[S];
+                                ldv<S>(E + (m.eQ + w * nr + i) * S, a);
+#pragma unroll
+                                for (int q = 0; q < S; ++q) acc[w][q] = fma(h[q], a[q], acc[w][q]);
+                            }
+                        }
                     }
-                } else {
+                    for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+                        for (int w = 0; w < NA; ++w)
+#pragma unroll
+                            for (int q = 0; q < S; ++q) acc[w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[w][q], o);
+                    if (head) {
+                        if (kind == kAuxR3) {
+                            stv<S>(E + m.eS1 * S, acc[0]);
+                            if (LEVEL == 2) { stv<S>(E + m.eA0 * S, acc[iA]); stv<S>(E + m.eS4 * S, acc[iT]); }
+                        } else {
+                            const uint32_t k = m.a_out[task];
+                            if (k != 0xFFFFFFFFu) {
+                                stv<S>(E + (m.eWdot + k) * S, acc[0]);
+                                if (LEVEL == 2) {
+                                    const double wk = m.mw[k];
+                                    double al[S], tc[S];
+#pragma unroll
+                                    for (int q = 0; q < S; ++q) {
+                                        const double ir = sc[kIrho * S + q];
+                                        al[q] = wk * ir * acc[iA][q];
+                                        tc[q] = ir * acc[iT][q];
+                                    }
+                                    stv<S>(E + (m.eAlpha + k + 1) * S, al);
+                                    stv<S>(E + (m.eTcol + k) * S, tc);
+                                }
+                            }
+                        }
+                    }
+                } else if (LEVEL == 2) {
+                    double acc[S];
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[q] = 0.0;
+                    if (kind == kAuxH2) {
 #pragma unroll 2
-                    for (uint32_t t = 0; t < ch.y; ++t) {
-                        const uint32_t e = ent[t * 32];
-                        const double cf = entry_coef(e);
-                        double a[S];
-                        ldv<S>(E + (e & 0xFFFF) * S, a);
+                        for (uint32_t t = 0; t < ch.y; ++t) {
+                            const uint32_t e = ent[t * 32];
+                            double a[S], b[S];
+                            ldv<S>(E + (e & 0xFFFF) * S, a);
+                            ldv<S>(E + (e >> 16) * S, b);
 #pragma unroll
-                        for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
+                            for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
+                        }
+                    } else {
+#pragma unroll 2
+                        for (uint32_t t = 0; t < ch.y; ++t) {
+                            const uint32_t e = ent[t * 32];
+                            const double cf = entry_coef(e);
+                            double a[S];
+                            ldv<S>(E + (e & 0xFFFF) * S, a);
+#pragma unroll
+                            for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
+                        }
+                    }
+                    for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+                        for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
+                    const uint32_t slot = m.a_out[task];
+                    if (head && slot != 0xFFFFFFFFu) {
+                        if (kind == kAuxS1) {
+                            const double cst = m.a_const[task];
+#pragma unroll
+                            for (int q = 0; q < S; ++q) acc[q] *= cst;
+                        }
+                        stv<S>(E + slot * S, acc);
                     }
                 }
-                if (ch.z & kAuxReduce) {
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[q] = warp_sum(acc[q]);
-                }
-                const uint32_t task = ch.w + ((ch.z & kAuxReduce) ? 0 : lane);
-                const uint32_t slot = m.a_out[task];
-                if (ch.z & kAuxScaled) {
-                    const double cst = m.a_const[task];
-                    const double *f = sc + ((ch.z >> 8) & 0xFF) * S;
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[q] *= cst * f[q];
-                }
-                if (slot != 0xFFFFFFFFu && (!(ch.z & kAuxReduce) || lane == 0)) stv<S>(E + slot * S, acc);
             }
         }
         __syncthreads();
@@ -501,22 +625,51 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 4 : NT <= 256 ? 2 : 1))
                     if (state0 + q >= n) continue;
                     const double irho = sc[kIrho * S + q];
                     const double v = r == 0 ? -E[m.eS1 * S + q] * irho / sc[kCpMix * S + q]
-                                            : m.wrow[r] * E[(m.eWdot + r - 1) * S + q] * irho;
+                                            : wrow[r] * E[(m.eWdot + r - 1) * S + q] * irho;
                     out.dydt[(state0 + q) * ld + r] = v;
                 }
         }
-        // ---- MAIN pass: lane <-> Jacobian element f = r + c * ld (column-major), gather + Eq. 112 / 113 + store
         if (LEVEL == 2) {
-            const long long Jstate = (long long)ld * ld;
-            double a1[S], irho[S];
+            // ---- FIX: the energy row (Eq. 113).  Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 ..
+            const int nfix = 1 + (ns - 1 + 31) / 32;
+            for (int it = warp; it < nfix; it += NW) {
+                if (it == 0) {
 #pragma unroll
-            for (int q = 0; q < S; ++q) {
-                const double icp = -sc[kNegIcp * S + q];
-                irho[q] = sc[kIrho * S + q];
-                a1[q] = irho[q] * E[m.eS1 * S + q] * icp * icp;    // energy row: coefficient of c_pj - c_pNs
+                    for (int q = 0; q < S; ++q) {
+                        double s3 = 0.0;       // sum_k c_pk W_k wdot_k
+                        for (int k = lane; k < ns; k += 32) s3 += Cp[k * S + q] * wrow[k + 1] * E[(m.eWdot + k) * S + q];
+                        s3 = warp_sum(s3);
+                        if (lane == 0) {
+                            const double icp = 1.0 / sc[kCpMix * S + q];
+                            E[m.eZ * S + q] = -icp * sc[kIrho * S + q] *
+                                              (s3 - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
+                        }
+                    }
+                } else {
+                    const int c = (it - 1) * 32 + lane + 1;
+                    if (c < ns) {
+                        const double2 cc = colc[c];
+                        const double wj = wrow[c], iwl = m.inv_mw[ns - 1];
+#pragma unroll
+                        for (int q = 0; q < S; ++q) {
+                            const double icp = 1.0 / sc[kCpMix * S + q], irho = sc[kIrho * S + q];
+                            const double a1 = irho * E[m.eS1 * S + q] * icp * icp;     // coefficient of c_pj - c_pNs
+                            const double alpha0 = -(irho * icp) * E[m.eA0 * S + q];
+                            const double gamma0 = -(iwl * icp) * E[(m.eG0 + ns - 1) * S + q];
+                            const double dcp = Cp[(c - 1) * S + q] - Cp[(ns - 1) * S + q];
+                            E[(m.eZ + c) * S + q] =
+                                wj * (alpha0 * cc.x - gamma0 + a1 * dcp) - icp * E[(m.eG0 + c - 1) * S + q];
+                        }
+                    }
+                }
             }
-            for (int t = grab(&ctr[2], lane); t < m.n_mtask; t = grab(&ctr[2], lane)) {
+            __syncthreads();
+            // ---- MAIN pass: lane <-> Jacobian element f = r + c * ld (column-major): gather, Eq. 112, store
+            const long long Jstate = (long long)ld * ld;
+            double *Jbase = out.jac + state0 * Jstate + lane;
+            for (int t = warp; t < m.n_mtask; t += NW) {
                 const uint4 mt = m.mtask[t];
+                const uint32_t steps = mt.y & 0xFFFF;
                 int r = (int)mt.z + lane, c = (int)mt.w;
                 while (r >= ld) { r -= ld; ++c; }
                 const bool live = c <= ns;
@@ -525,7 +678,7 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 4 : NT <= 256 ? 2 : 1))
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] = 0.0;
 #pragma unroll 2
-                for (uint32_t st = 0; st < mt.y; ++st) {
+                for (uint32_t st = 0; st < steps; ++st) {
                     const uint32_t e = ent[st * 32];
                     const double cf = entry_coef(e);
                     double a[S];
@@ -533,32 +686,21 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 4 : NT <= 256 ? 2 : 1))
 #pragma unroll
                     for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
                 }
-                double j00[S];
-                if (t == 0) {
-                    // J(0,0) of Eq. 113: -(1/(rho c_p)) [sum_k c_pk W_k wdot_k - (dc_p/dT / c_p) S1 + S4]
-#pragma unroll
-                    for (int q = 0; q < S; ++q) {
-                        double s3 = 0.0;
-                        for (int k = lane; k < ns; k += 32) s3 += Cp[k * S + q] * m.wrow[k + 1] * E[(m.eWdot + k) * S + q];
-                        s3 = warp_sum(s3);
-                        const double nicp = sc[kNegIcp * S + q];
-                        j00[q] = nicp * irho[q] * (s3 + sc[kDcpDT * S + q] * nicp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
-                    }
-                }
-                const int cc_i = live ? c : 0;
-                const double2 cc = m.colc[cc_i];
-                const double wr = m.wrow[r];
-                const double wj = wr * cc.y;
-                double *Jp = out.jac + state0 * Jstate + (long long)t * 32 + lane;
+                const double2 cc = colc[live ? c : 0];
+                const double wj = wrow[r] * cc.y;
                 double alpha[S], gamma[S];
                 ldv<S>(E + (m.eAlpha + r) * S, alpha);
                 ldv<S>(E + (m.eGamma + r) * S, gamma);
+                if (mt.y >> 16) {          // the task touches column 0 or the zero column: no gamma there
+                    if (c == 0 || c >= ns) {
+#pragma unroll
+                        for (int q = 0; q < S; ++q) gamma[q] = 0.0;
+                    }
+                }
+                double *Jp = Jbase + (long long)t * 32;
 #pragma unroll
                 for (int q = 0; q < S; ++q) {
-                    double v = fma(alpha[q], cc.x, fma(wj, acc[q], -gamma[q]));
-                    if (r == 0 && c > 0) v = fma(a1[q], Cp[(cc_i - 1) * S + q] - Cp[(ns - 1) * S + q], v);
-                    if (c == 0) v = r == 0 ? (t == 0 ? j00[q] : 0.0) : wr * irho[q] * acc[q];
-                    if (c == ns) v = 0.0;
+                    const double v = fma(wj, acc[q], fma(alpha[q], cc.x, -gamma[q]));
                     if (live && state0 + q < n) __stcs(Jp + q * Jstate, v);
                 }
             }
@@ -566,28 +708,30 @@ __global__ void __launch_bounds__(NT, (NT <= 128 ? 4 : NT <= 256 ? 2 : 1))
     }
 }
 
-template <int LEVEL, int NT, int S>
+template <int LEVEL, int NT, int S, int MB>
 cudaError_t launch_t(const DeviceMech &m, const SmemPlan &sp, int grid, size_t smem, long long n,
                      const double *T, const double *P, const double *Y, long long ldy, const EvalOut &out,
                      cudaStream_t stream)
 {
-    eval_kernel<LEVEL, NT, S><<<grid, NT, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+    eval_kernel<LEVEL, NT, S, MB><<<grid, NT, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
     return cudaGetLastError();
 }
 
 }  // namespace
 
-size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + (size_t)kRedRows * S * 32) * sizeof(double); }
+size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + (size_t)sp.shared_total) * sizeof(double); }
 
+// (threads, S, CTAs per SM the register budget is set for)
 #define PYJAC_FOR_ALL(X) \
-    X(128, 1) X(128, 2) X(128, 4) X(256, 1) X(256, 2) X(256, 4) X(512, 1) X(512, 2) X(512, 4)
+    X(128, 1, 4) X(128, 2, 4) X(128, 4, 4) X(256, 1, 2) X(256, 2, 2) X(256, 4, 2) X(512, 1, 1) X(512, 2, 1) X(512, 4, 1) \
+    X(1024, 1, 1) X(1024, 2, 1) X(1024, 4, 1)
 
 const void *eval_kernel_ptr(int level, int nt, int S)
 {
-#define PYJAC_PTR(N, SV)                                                      \
-    if (nt == N && S == SV)                                                   \
-        return level == 0 ? (const void *)eval_kernel<0, N, SV>               \
-             : level == 1 ? (const void *)eval_kernel<1, N, SV> : (const void *)eval_kernel<2, N, SV>;
+#define PYJAC_PTR(N, SV, MB)                                                      \
+    if (nt == N && S == SV)                                                       \
+        return level == 0 ? (const void *)eval_kernel<0, N, SV, MB>               \
+             : level == 1 ? (const void *)eval_kernel<1, N, SV, MB> : (const void *)eval_kernel<2, N, SV, MB>;
     PYJAC_FOR_ALL(PYJAC_PTR)
 #undef PYJAC_PTR
     return nullptr;
@@ -597,11 +741,11 @@ cudaError_t launch_eval(int level, int nt, int S, const DeviceMech &m, const Sme
                         long long n, const double *T, const double *P, const double *Y, long long ldy,
                         const EvalOut &out, cudaStream_t stream)
 {
-#define PYJAC_CASE(N, SV)                                                                                   \
-    if (nt == N && S == SV) {                                                                               \
-        if (level == 0) return launch_t<0, N, SV>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);         \
-        if (level == 1) return launch_t<1, N, SV>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);         \
-        return launch_t<2, N, SV>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);                         \
+#define PYJAC_CASE(N, SV, MB)                                                                                   \
+    if (nt == N && S == SV) {                                                                                   \
+        if (level == 0) return launch_t<0, N, SV, MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);         \
+        if (level == 1) return launch_t<1, N, SV, MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);         \
+        return launch_t<2, N, SV, MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);                         \
     }
     PYJAC_FOR_ALL(PYJAC_CASE)
 #undef PYJAC_CASE

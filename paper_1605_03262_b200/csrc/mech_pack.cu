@@ -6,6 +6,7 @@
 // ln A, ln p of the tables and the per-reaction sums of NASA coefficients (Eq. 27 summed over a
 // reaction, see device_mech.h `th_data`).
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <numeric>
 
@@ -34,12 +35,22 @@ struct ColEntry {
 // one gathered sum of the AUX phase
 struct Task {
     std::vector<uint32_t> ent;
-    uint32_t flags = 0;     // kAuxTwoIndex | kAuxScaled | scalar << 8
-    uint32_t out = 0;       // E slot
-    double cst = 0.0;
-    bool reduce = false;    // spread over the 32 lanes of its own chunk
+    uint32_t kind = kAuxS1;
+    uint32_t out = 0;       // E slot (kAuxT3: species k)
+    double cst = 1.0;
+    int rshift = 0;         // 2^rshift lanes share the sum
     bool lvl01 = false;     // needed by the rates / dydt kernels too
+    int steps() const { return (int)((ent.size() + (size_t(1) << rshift) - 1) >> rshift); }
 };
+
+// lanes that share one sum: enough that no lane walks more than about 12 entries
+int pick_rshift(size_t len)
+{
+    if (len <= 12) return 0;
+    for (int r = 2; r < 5; ++r)
+        if (((len + (size_t(1) << r) - 1) >> r) <= 12) return r;
+    return 5;
+}
 
 void validate(const pyjac_mech_desc *d)
 {
@@ -135,6 +146,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     o.nr = nr;
     // ---- species
     o.inv_mw.resize(ns);
+    o.mw.assign(d->mol_wt, d->mol_wt + ns);
     o.t_mid.assign(d->t_mid, d->t_mid + ns);
     o.nasa.resize((size_t)10 * ns);
     for (int k = 0; k < ns; ++k) {
@@ -149,13 +161,29 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     for (int k = 0; k < ns; ++k) o.wrow[k + 1] = d->mol_wt[k];
     o.colc.assign((size_t)2 * ld, 0.0);
     o.colc[1] = 1.0;
-    for (int k = 0; k < ns; ++k) {
+    for (int k = 0; k + 1 < ns; ++k) {
         o.colc[2 * (k + 1)] = 1.0 / d->mol_wt[k] - iw_last;
         o.colc[2 * (k + 1) + 1] = 1.0 / d->mol_wt[k];
     }
 
-    // ---- sorted order: most expensive rate form first; one form, one stoichiometry path and
-    // equally many V entries per group of 32
+    // ---- per reaction: molecules per side, breakpoints of its species' NASA ranges
+    std::vector<int> mol_f(nr, 0), mol_r(nr, 0), n_brk(nr, 0);
+    for (int i = 0; i < nr; ++i) {
+        for (int q = d->reac_ptr[i]; q < d->reac_ptr[i + 1]; ++q) mol_f[i] += d->reac_nu[q];
+        for (int q = d->prod_ptr[i]; q < d->prod_ptr[i + 1]; ++q) mol_r[i] += d->prod_nu[q];
+        std::vector<double> brk;
+        for (int q = d->reac_ptr[i]; q < d->reac_ptr[i + 1]; ++q) brk.push_back(d->t_mid[d->reac_spec[q]]);
+        for (int q = d->prod_ptr[i]; q < d->prod_ptr[i + 1]; ++q) brk.push_back(d->t_mid[d->prod_spec[q]]);
+        std::sort(brk.begin(), brk.end());
+        n_brk[i] = (int)(std::unique(brk.begin(), brk.end()) - brk.begin());
+    }
+    auto expandable = [&](int i) { return mol_f[i] <= kMaxSide && mol_r[i] <= kMaxSide; };
+    auto plain = [&](int i) {
+        return d->rxn_type[i] == PYJAC_ELEMENTARY && d->rev_type[i] != PYJAC_REV_EXPLICIT && expandable(i) &&
+               n_brk[i] <= 1;
+    };
+
+    // ---- sorted order: most expensive rate form first, the plain elementary reactions last
     std::vector<int> key(nr);
     for (int i = 0; i < nr; ++i) {
         const int t = d->rxn_type[i], rv = d->rev_type[i];
@@ -164,49 +192,78 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
         if (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED)
             rank = form == PYJAC_TROE ? 0 : form == PYJAC_SRI ? 1 : 2;
         else
-            rank = t == PYJAC_THIRD_BODY ? 3 : t == PYJAC_CHEBYSHEV ? 4 : t == PYJAC_PLOG ? 5 : 6;
-        bool unit = true;
-        for (int q = d->reac_ptr[i]; q < d->reac_ptr[i + 1]; ++q) unit = unit && d->reac_nu[q] == 1;
-        for (int q = d->prod_ptr[i]; q < d->prod_ptr[i + 1]; ++q) unit = unit && d->prod_nu[q] == 1;
-        const int nslot = (d->reac_ptr[i + 1] - d->reac_ptr[i]) + (d->prod_ptr[i + 1] - d->prod_ptr[i]);
+            rank = t == PYJAC_THIRD_BODY ? 3 : t == PYJAC_CHEBYSHEV ? 4 : t == PYJAC_PLOG ? 5 : plain(i) ? 7 : 6;
+        const int nslot = expandable(i) ? mol_f[i] + mol_r[i]
+                                        : (d->reac_ptr[i + 1] - d->reac_ptr[i]) + (d->prod_ptr[i + 1] - d->prod_ptr[i]);
         const int neff = std::min(n_eff_terms(d, i), 63);
-        key[i] = ((((rank * 2 + (unit ? 0 : 1)) * 4 + rv) * 8 + nslot) * 64) + neff;
+        key[i] = (((rank * 4 + rv) * 8 + nslot) * 64) + neff;
     }
     std::vector<int> order(nr);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key[a] < key[b]; });
     o.n_rchunk = (nr + 31) / 32;
+    o.rchunk.assign(std::max(o.n_rchunk, 1), 0u);
+    for (int c = 0; c < o.n_rchunk; ++c) {
+        bool all = true;
+        for (int s = 32 * c; s < std::min(nr, 32 * c + 32); ++s) all = all && plain(order[s]);
+        o.rchunk[c] = all ? 1u : 0u;
+        o.n_plain_chunks += all ? 1 : 0;
+    }
 
-    // ---- E indices of the V entries: per group of 32 reactions, slot-major (lane-contiguous)
-    o.vbase.assign(nr, 0u);
-    std::vector<uint32_t> eff_vb(nr, 0u);
+    // ---- slots of every reaction (sorted order): species and nu per slot
+    struct Slots { int spec[6]; int nu[6]; };
+    std::vector<Slots> sl(nr);
+    for (int s = 0; s < nr; ++s) {
+        const int i = order[s];
+        for (int p = 0; p < 6; ++p) { sl[s].spec[p] = ns; sl[s].nu[p] = 0; }
+        for (int side = 0; side < 2; ++side) {
+            const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr;
+            const int32_t *sp = side ? d->prod_spec : d->reac_spec;
+            const int32_t *nu = side ? d->prod_nu : d->reac_nu;
+            int p = 3 * side;
+            for (int q = ptr[i]; q < ptr[i + 1]; ++q) {
+                if (expandable(i)) {
+                    for (int r = 0; r < nu[q]; ++r, ++p) { sl[s].spec[p] = sp[q]; sl[s].nu[p] = 1; }
+                } else {
+                    sl[s].spec[p] = sp[q]; sl[s].nu[p] = nu[q]; ++p;
+                }
+            }
+        }
+    }
+
+    // ---- E indices of the V entries, compact: per group of 32 reactions, slot position by slot
+    // position, the lanes that use the position in lane order (neighbouring lanes, neighbouring words)
+    std::vector<std::array<uint32_t, 6>> vslot(nr);
+    std::vector<std::vector<uint32_t>> veff(nr);
     uint32_t nv = 0;
     for (int c = 0; c < o.n_rchunk; ++c) {
-        int maxslot = 0, maxeff = 0;
-        for (int s = 32 * c; s < std::min(nr, 32 * c + 32); ++s) {
-            const int i = order[s];
-            maxslot = std::max(maxslot, (d->reac_ptr[i + 1] - d->reac_ptr[i]) + (d->prod_ptr[i + 1] - d->prod_ptr[i]));
-            maxeff = std::max(maxeff, n_eff_terms(d, i));
-        }
-        for (int s = 32 * c; s < std::min(nr, 32 * c + 32); ++s) {
-            o.vbase[s] = nv + (uint32_t)(s - 32 * c);
-            eff_vb[s] = nv + (uint32_t)(kVStride * maxslot + (s - 32 * c));
-        }
-        nv += (uint32_t)(kVStride * (maxslot + maxeff));
+        const int s0 = 32 * c, s1 = std::min(nr, 32 * c + 32);
+        for (int p = 0; p < 6; ++p)
+            for (int s = s0; s < s1; ++s) vslot[s][p] = sl[s].nu[p] ? nv++ : 0xFFFFFFFFu;
+        int maxeff = 0;
+        for (int s = s0; s < s1; ++s) maxeff = std::max(maxeff, n_eff_terms(d, order[s]));
+        for (int s = s0; s < s1; ++s) veff[s].clear();
+        for (int e = 0; e < maxeff; ++e)
+            for (int s = s0; s < s1; ++s)
+                if (n_eff_terms(d, order[s]) > e) veff[s].push_back(nv++);
     }
-    const int eQ = (int)nv, eAr = eQ + nr, eTh = eAr + nr, eH = eTh + nr;
-    const int eAlpha = eH + nr, eGamma = eAlpha + ld, eWdot = eGamma + ld;
-    const int eS1 = eWdot + ns, eS4 = eS1 + 1;
-    int next_slot = eS4 + 1;          // further AUX results
+    int next_slot = (int)nv;
+    auto take = [&](int n) { int r = next_slot; next_slot += n; return r; };
+    const int eQ = take(nr), eAr = take(nr), eTh = take(nr), eH = take(nr);
+    const int eAlpha = take(ld), eGamma = take(ld), eWdot = take(ns), eTcol = take(ns), eG0 = take(ns), eZ = take(ld);
+    const int eS1 = take(1), eA0 = take(1), eS4 = take(1), eZero = take(1), eDump = take(1);
     o.eQ = eQ; o.eAr = eAr; o.eTh = eTh; o.eH = eH; o.eAlpha = eAlpha; o.eGamma = eGamma; o.eWdot = eWdot;
-    o.eS1 = eS1; o.eS4 = eS4;
+    o.eTcol = eTcol; o.eG0 = eG0; o.eZ = eZ; o.eS1 = eS1; o.eA0 = eA0; o.eS4 = eS4; o.eZero = eZero; o.eDump = eDump;
+    if (next_slot > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-state table entries"};
 
     // ---- per-reaction tables in sorted order
     o.lnA.assign(nr, 0.0); o.beta.assign(nr, 0.0); o.Ta.assign(nr, 0.0);
     o.rev_lnA.assign(nr, 0.0); o.rev_beta.assign(nr, 0.0); o.rev_Ta.assign(nr, 0.0);
-    o.slots.assign((size_t)4 * nr, 0u);
+    o.slots.assign((size_t)4 * std::max(nr, 1), 0u);
+    o.vidx.assign((size_t)4 * std::max(nr, 1), 0u);
     o.rxn_orig.resize(nr);
     o.th_off.resize(nr);
+    o.th_soa.assign((size_t)15 * std::max(nr, 1), 0.0);
     o.n_pd = 0; o.n_pk = 0;
     o.pk_ptr.assign(1, 0);
     o.eff_ptr.assign(1, 0);
@@ -229,35 +286,32 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
             o.rev_beta[s] = d->arr_rev[3 * i + 1];
             o.rev_Ta[s] = d->arr_rev[3 * i + 2];
         }
-        uint32_t spec[6] = {(uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns, (uint32_t)ns};
-        uint32_t meta = 0;
-        uint32_t vi = o.vbase[s];
+        uint32_t meta = 0, vi[6];
         int dnu = 0;
-        for (int side = 0; side < 2; ++side) {
-            const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr;
-            const int32_t *sp = side ? d->prod_spec : d->reac_spec;
-            const int32_t *nu = side ? d->prod_nu : d->reac_nu;
-            for (int q = ptr[i], e = 0; q < ptr[i + 1]; ++q, ++e) {
-                const int slot = 3 * side + e;
-                spec[slot] = (uint32_t)sp[q];
-                meta |= (uint32_t)nu[q] << (4 * slot);
-                cols[s].push_back({sp[q], vi});
-                vi += kVStride;
-                const int signed_nu = side ? nu[q] : -nu[q];
-                dnu += signed_nu;
-                bool found = false;
-                for (auto &pr : net[s])
-                    if (pr.first == sp[q]) { pr.second += signed_nu; found = true; }
-                if (!found) net[s].push_back({sp[q], signed_nu});
-            }
+        for (int p = 0; p < 6; ++p) {
+            vi[p] = (uint32_t)eDump;
+            if (!sl[s].nu[p]) continue;
+            const int k = sl[s].spec[p];
+            meta |= (uint32_t)sl[s].nu[p] << (4 * p);
+            vi[p] = vslot[s][p];
+            cols[s].push_back({k, vi[p]});
+            const int signed_nu = p >= 3 ? sl[s].nu[p] : -sl[s].nu[p];
+            dnu += signed_nu;
+            bool found = false;
+            for (auto &pr : net[s])
+                if (pr.first == k) { pr.second += signed_nu; found = true; }
+            if (!found) net[s].push_back({k, signed_nu});
         }
         const int form = (t == PYJAC_FALLOFF || t == PYJAC_CHEM_ACTIVATED) ? d->falloff_form[i] : 0;
         const int single = is_pd(t) && d->tb_species[i] >= 0;
         meta |= (uint32_t)t << 24 | (uint32_t)rv << 27 | (uint32_t)form << 29 | (uint32_t)single << 31;
-        o.slots[4 * s + 0] = spec[0] | spec[1] << 16;
-        o.slots[4 * s + 1] = spec[2] | spec[3] << 16;
-        o.slots[4 * s + 2] = spec[4] | spec[5] << 16;
+        o.slots[4 * s + 0] = (uint32_t)sl[s].spec[0] | (uint32_t)sl[s].spec[1] << 16;
+        o.slots[4 * s + 1] = (uint32_t)sl[s].spec[2] | (uint32_t)sl[s].spec[3] << 16;
+        o.slots[4 * s + 2] = (uint32_t)sl[s].spec[4] | (uint32_t)sl[s].spec[5] << 16;
         o.slots[4 * s + 3] = meta;
+        o.vidx[4 * s + 0] = vi[0] | vi[1] << 16;
+        o.vidx[4 * s + 1] = vi[2] | vi[3] << 16;
+        o.vidx[4 * s + 2] = vi[4] | vi[5] << 16;
 
         // sum_k nu_ki B_k(T) as one polynomial per interval between the t_mid of the species
         {
@@ -269,6 +323,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
             o.th_off[s] = (uint32_t)o.th_data.size();
             o.th_data.push_back((double)nint);
             for (double b : brk) o.th_data.push_back(b);
+            if (nint <= 2) o.th_soa[s] = nint == 2 ? brk[0] : HUGE_VAL;
             for (int iv = 0; iv < nint; ++iv) {
                 // interval iv: brk[iv-1] < T <= brk[iv]; species k is in its low range iff T <= t_mid[k]
                 double da[7] = {0, 0, 0, 0, 0, 0, 0};
@@ -279,13 +334,14 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
                     const double *a = (low ? d->nasa_lo : d->nasa_hi) + 7 * k;
                     for (int c = 0; c < 7; ++c) da[c] += (double)pr.second * a[c];
                 }
-                o.th_data.push_back(da[6] - da[0] + (double)dnu * ln_patm_R);   // g0
-                o.th_data.push_back(da[0] - (double)dnu);                        // g1
-                o.th_data.push_back(da[1] * 0.5);                                // g2
-                o.th_data.push_back(da[2] * (1.0 / 6.0));                        // g3
-                o.th_data.push_back(da[3] * (1.0 / 12.0));                       // g4
-                o.th_data.push_back(da[4] * 0.05);                               // g5
-                o.th_data.push_back(-da[5]);                                     // g6
+                const double g[7] = {da[6] - da[0] + (double)dnu * ln_patm_R, da[0] - (double)dnu, da[1] * 0.5,
+                                     da[2] * (1.0 / 6.0), da[3] * (1.0 / 12.0), da[4] * 0.05, -da[5]};
+                for (int c = 0; c < 7; ++c) o.th_data.push_back(g[c]);
+                if (nint <= 2)
+                    for (int c = 0; c < 7; ++c) {
+                        o.th_soa[(size_t)(1 + 7 * iv + c) * nr + s] = g[c];
+                        if (nint == 1) o.th_soa[(size_t)(8 + c) * nr + s] = g[c];
+                    }
             }
         }
         if (is_pd(t)) {
@@ -294,20 +350,19 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
             o.lo_beta.push_back(fall ? d->arr_lo[3 * i + 1] : 0.0);
             o.lo_Ta.push_back(fall ? d->arr_lo[3 * i + 2] : 0.0);
             for (int c = 0; c < 5; ++c) o.fall_par.push_back(fall ? d->falloff_par[5 * i + c] : 0.0);
-            o.eff_vbase.push_back(eff_vb[s]);
-            uint32_t ve = eff_vb[s];
+            size_t e = 0;
             const int m = d->tb_species[i];
             if (m >= 0) {       // Eq. 30: [X]_i = [X_m]; one entry with "alpha - 1" = 1 and no [M] term
-                o.eff_spec.push_back(m);
+                o.eff_spec.push_back((uint32_t)m | veff[s][0] << 16);
                 o.eff_eps.push_back(1.0);
-                cols[s].push_back({m, ve});
+                cols[s].push_back({m, veff[s][0]});
             } else {            // Eq. 28 written as [M] + sum_j (alpha_ij - 1)[X_j]
                 for (int q = d->eff_ptr[i]; q < d->eff_ptr[i + 1]; ++q) {
                     if (d->eff_val[q] == 1.0) continue;
-                    o.eff_spec.push_back(d->eff_spec[q]);
+                    o.eff_spec.push_back((uint32_t)d->eff_spec[q] | veff[s][e] << 16);
                     o.eff_eps.push_back(d->eff_val[q] - 1.0);
-                    cols[s].push_back({d->eff_spec[q], ve});
-                    ve += kVStride;
+                    cols[s].push_back({d->eff_spec[q], veff[s][e]});
+                    ++e;
                 }
             }
             o.eff_ptr.push_back((int32_t)o.eff_spec.size());
@@ -338,69 +393,39 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
         }
     }
 
-    // ---- AUX tasks that always exist
+    // ---- AUX sums that always exist
     std::vector<Task> tasks;
-    auto scaled = [](uint32_t scalar) { return (uint32_t)kAuxScaled | scalar << 8; };
-    // (a) wdot_k = sum_i nu_ki q_i (Eq. 14) and S1 = sum_i H_i q_i: the rates / dydt kernels need them too
-    for (int k = 0; k < ns; ++k) {
-        Task t;
-        t.out = (uint32_t)(eWdot + k);
-        t.lvl01 = true;
-        tasks.push_back(t);
-    }
-    const size_t tS1 = tasks.size();
-    { Task t; t.flags = kAuxTwoIndex; t.out = (uint32_t)eS1; t.reduce = true; t.lvl01 = true; tasks.push_back(t); }
-    // (b) alpha_r = (W_k / rho) sum_i nu_ki (a_i + W q_i), the coefficient of d_j in row r = k + 1
-    //     (Eqs. 112, 119, 123, 127 regrouped); gamma_r = (W_k / W_Ns) sum_i nu_ki s'_iNs
-    const size_t tAlpha = tasks.size();
-    for (int k = 0; k < ns; ++k) {
-        Task t;
-        t.out = (uint32_t)(eAlpha + k + 1); t.flags = scaled(kIrho); t.cst = d->mol_wt[k];
-        tasks.push_back(t);
-    }
+    // (a) per species k: sums of nu_ki {q_i, a_i, Theta_i} (Eq. 14; the d_j coefficient of Eqs. 112, 119,
+    //     123, 127 regrouped; the T column, Eq. 111).  The rates / dydt kernels need wdot too.
+    const size_t tT3 = tasks.size();
+    for (int k = 0; k < ns; ++k) { Task t; t.kind = kAuxT3; t.out = (uint32_t)k; t.lvl01 = true; tasks.push_back(t); }
+    // (b) gamma_r = (W_k / W_Ns) sum_i nu_ki s'_iNs
     const size_t tGamma = tasks.size();
     for (int k = 0; k < ns; ++k) {
-        Task t;
-        t.out = (uint32_t)(eGamma + k + 1); t.flags = scaled(kOne); t.cst = d->mol_wt[k] * iw_last;
+        Task t; t.kind = kAuxS1; t.out = (uint32_t)(eGamma + k + 1); t.cst = d->mol_wt[k] * iw_last;
         tasks.push_back(t);
     }
-    // (c) energy row (Eq. 113): G0_j = sum_i H_i s'_ij per column, scaled by -1/c_p
+    // (c) energy row (Eq. 113): G0_j = sum_i H_i s'_ij per column species
     const size_t tG0 = tasks.size();
-    std::vector<uint32_t> g0_slot(ns, 0u);
-    for (int j = 0; j < ns; ++j) {
-        Task t;
-        t.flags = kAuxTwoIndex | scaled(kNegIcp);
-        if (j == ns - 1) { t.out = (uint32_t)eGamma; t.cst = iw_last; }
-        else { t.out = (uint32_t)next_slot++; t.cst = 1.0; g0_slot[j] = t.out; }
-        tasks.push_back(t);
-    }
-    //     alpha_0 = -(1 / (rho c_p)) sum_i H_i (a_i + W q_i);  S4 = sum_i H_i Theta_i
-    const size_t tA0 = tasks.size();
-    { Task t; t.flags = kAuxTwoIndex | scaled(kNegIrhoIcp); t.out = (uint32_t)eAlpha; t.cst = 1.0; t.reduce = true; tasks.push_back(t); }
-    const size_t tS4 = tasks.size();
-    { Task t; t.flags = kAuxTwoIndex; t.out = (uint32_t)eS4; t.reduce = true; tasks.push_back(t); }
+    for (int j = 0; j < ns; ++j) { Task t; t.kind = kAuxH2; t.out = (uint32_t)(eG0 + j); tasks.push_back(t); }
 
     // ---- lists of the Jacobian cells, flat column-major index f = r + c * ld
     std::vector<std::vector<uint32_t>> cell((size_t)ld * ld);
     for (int s = 0; s < nr; ++s) {
         const uint32_t hs = (uint32_t)(eH + s);
-        tasks[tS1].ent.push_back((uint32_t)(eQ + s) | hs << 16);
-        tasks[tA0].ent.push_back((uint32_t)(eAr + s) | hs << 16);
-        tasks[tS4].ent.push_back((uint32_t)(eTh + s) | hs << 16);
         for (auto &ce : cols[s]) tasks[tG0 + ce.spec].ent.push_back(ce.vi | hs << 16);
         for (auto &pr : net[s]) {
             if (pr.second == 0) continue;
             const int k = pr.first;
-            tasks[k].ent.push_back(pack_entry((uint32_t)(eQ + s), pr.second));
-            tasks[tAlpha + k].ent.push_back(pack_entry((uint32_t)(eAr + s), pr.second));
-            cell[(size_t)(k + 1)].push_back(pack_entry((uint32_t)(eTh + s), pr.second));        // column 0 (d/dT)
+            tasks[tT3 + k].ent.push_back(pack_entry((uint32_t)(eQ + s), pr.second));
             for (auto &ce : cols[s]) {
                 if (ce.spec == ns - 1) tasks[tGamma + k].ent.push_back(pack_entry(ce.vi, pr.second));
                 else cell[(size_t)(k + 1) + (size_t)(ce.spec + 1) * ld].push_back(pack_entry(ce.vi, pr.second));
             }
         }
     }
-    for (int j = 0; j < ns - 1; ++j) cell[(size_t)(j + 1) * ld].push_back(pack_entry(g0_slot[j], 1));   // row 0
+    for (int k = 0; k < ns; ++k) cell[(size_t)(k + 1)].push_back(pack_entry((uint32_t)(eTcol + k), 1));   // column 0
+    for (int c = 0; c < ns; ++c) cell[(size_t)c * ld].push_back(pack_entry((uint32_t)(eZ + c), 1));        // row 0
     for (auto &c : cell) o.n_list_entries += (long long)c.size();
 
     // ---- MAIN tasks: 32 consecutive cells; lists longer than the task's cap are summed by an AUX
@@ -410,8 +435,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     o.n_mtask = (int)((ncell + 31) / 32);
     const size_t fixed_tasks = tasks.size();
     std::vector<int> cap(o.n_mtask, 0);
+    const long long e_limit = std::min<long long>(smem_doubles, 65535);
     for (double lambda = 0.15;; lambda *= 2.0) {
-        tasks.resize(fixed_tasks);
         int slots = next_slot;
         bool any_overflow = false;
         for (int t = 0; t < o.n_mtask; ++t) {
@@ -433,36 +458,23 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
             for (int l = 0; l < 32; ++l)
                 if (len[l] > bestc) { ++slots; any_overflow = true; }
         }
-        if (slots + 1 <= std::min<long long>(smem_doubles, 65535)) break;
-        if (!any_overflow) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
-        if (lambda > 1e6) {   // no overflow at all: every list inline
-            for (int t = 0; t < o.n_mtask; ++t) {
-                int mx = 0;
-                for (int l = 0; l < 32; ++l) {
-                    const size_t f = (size_t)t * 32 + l;
-                    if (f < ncell) mx = std::max(mx, (int)cell[f].size());
-                }
-                cap[t] = mx;
-            }
-            if (next_slot + 1 > std::min<long long>(smem_doubles, 65535))
-                throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
-            break;
-        }
+        if (slots <= e_limit) break;
+        if (!any_overflow || lambda > 1e6) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
     }
+    (void)fixed_tasks;
     for (int t = 0; t < o.n_mtask; ++t)
         for (int l = 0; l < 32; ++l) {
             const size_t f = (size_t)t * 32 + l;
             if (f >= ncell || (int)cell[f].size() <= cap[t]) continue;
             Task a;
+            a.kind = kAuxS1;
             a.out = (uint32_t)next_slot++;
             a.ent.swap(cell[f]);
             tasks.push_back(a);
             cell[f].push_back(pack_entry(tasks.back().out, 1));
         }
-    const int eZero = next_slot++;
-    o.eZero = eZero;
     o.n_e = next_slot;
-    if (o.n_e > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-state table entries"};
+    if (o.n_e > e_limit) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
     const uint32_t pad1 = pack_entry((uint32_t)eZero, 0);
     const uint32_t pad2 = (uint32_t)eZero | (uint32_t)eZero << 16;
 
@@ -470,13 +482,15 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     o.mtask.assign((size_t)4 * o.n_mtask, 0u);
     for (int t = 0; t < o.n_mtask; ++t) {
         const uint32_t base = (uint32_t)o.m_ent.size();
+        const size_t f0 = (size_t)t * 32, f1 = std::min(ncell, f0 + 32) - 1;
+        const bool edge = f0 / ld == 0 || f1 / ld == (size_t)ns;       // touches column 0 or the zero column
         o.mtask[4 * t + 0] = base;
-        o.mtask[4 * t + 1] = (uint32_t)cap[t];
-        o.mtask[4 * t + 2] = (uint32_t)(((size_t)t * 32) % ld);
-        o.mtask[4 * t + 3] = (uint32_t)(((size_t)t * 32) / ld);
+        o.mtask[4 * t + 1] = (uint32_t)cap[t] | (edge ? 1u << 16 : 0u);
+        o.mtask[4 * t + 2] = (uint32_t)(f0 % ld);
+        o.mtask[4 * t + 3] = (uint32_t)(f0 / ld);
         o.m_ent.resize(o.m_ent.size() + (size_t)cap[t] * 32, pad1);
         for (int l = 0; l < 32; ++l) {
-            const size_t f = (size_t)t * 32 + l;
+            const size_t f = f0 + l;
             if (f >= ncell) continue;
             for (size_t e = 0; e < cell[f].size(); ++e) o.m_ent[(size_t)base + e * 32 + l] = cell[f][e];
         }
@@ -484,60 +498,63 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     }
     if (o.m_ent.empty()) o.m_ent.push_back(pad1);
 
-    // ---- AUX chunks: tasks with equal flags and similar length share a chunk of 32 lanes
-    struct Chunk { std::vector<size_t> t; int steps; bool lvl01; bool reduce; };
+    // ---- AUX chunks: sums of one kind, shared by equally many lanes and of similar length, fill the
+    // 32 lanes of a chunk; the warps take the chunks in a fixed round-robin order, longest first
+    for (auto &t : tasks) t.rshift = pick_rshift(t.ent.size());
+    struct Chunk { std::vector<size_t> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; };
     std::vector<Chunk> chunks;
+    if (nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0});
     {
-        std::vector<size_t> idx;
-        for (size_t t = 0; t < tasks.size(); ++t) {
-            if (tasks[t].reduce) chunks.push_back({{t}, (int)((tasks[t].ent.size() + 31) / 32), tasks[t].lvl01, true});
-            else idx.push_back(t);
-        }
+        std::vector<size_t> idx(tasks.size());
+        std::iota(idx.begin(), idx.end(), 0);
         std::stable_sort(idx.begin(), idx.end(), [&](size_t a, size_t b) {
-            if (tasks[a].lvl01 != tasks[b].lvl01) return tasks[a].lvl01;
-            if (tasks[a].flags != tasks[b].flags) return tasks[a].flags < tasks[b].flags;
-            return tasks[a].ent.size() > tasks[b].ent.size();
+            if (tasks[a].kind != tasks[b].kind) return tasks[a].kind < tasks[b].kind;
+            if (tasks[a].rshift != tasks[b].rshift) return tasks[a].rshift > tasks[b].rshift;
+            return tasks[a].steps() > tasks[b].steps();
         });
         for (size_t p = 0; p < idx.size();) {
-            Chunk c{{}, 0, tasks[idx[p]].lvl01, false};
-            const uint32_t fl = tasks[idx[p]].flags;
-            while (p < idx.size() && c.t.size() < 32 && tasks[idx[p]].lvl01 == c.lvl01 && tasks[idx[p]].flags == fl) {
-                c.steps = std::max(c.steps, (int)tasks[idx[p]].ent.size());
+            const Task &t0 = tasks[idx[p]];
+            Chunk c{{}, t0.kind, t0.rshift, 0, t0.lvl01, 0.0};
+            const size_t per = (size_t)32 >> t0.rshift;
+            while (p < idx.size() && c.t.size() < per && tasks[idx[p]].kind == c.kind && tasks[idx[p]].rshift == c.rshift) {
+                c.steps = std::max(c.steps, tasks[idx[p]].steps());
                 c.t.push_back(idx[p++]);
             }
             chunks.push_back(c);
         }
-        // longest first (the warps take chunks from a queue); the rates / dydt subset in front
+        for (auto &c : chunks) {
+            const double per_step = c.kind == kAuxT3 ? 3.0 : c.kind == kAuxR3 ? 4.0 : c.kind == kAuxH2 ? 1.5 : 1.0;
+            const double sums = (c.kind == kAuxT3 || c.kind == kAuxR3) ? 3.0 : 1.0;
+            c.cost = per_step * c.steps + 1.0 * sums * c.rshift + 3.0;
+        }
         std::stable_sort(chunks.begin(), chunks.end(), [&](const Chunk &a, const Chunk &b) {
             if (a.lvl01 != b.lvl01) return a.lvl01;
-            return a.steps > b.steps;
+            return a.cost > b.cost;
         });
     }
     o.n_achunk = (int)chunks.size();
     o.n_achunk01 = 0;
     for (auto &c : chunks) o.n_achunk01 += c.lvl01 ? 1 : 0;
     for (auto &c : chunks) {
-        const Task &t0 = tasks[c.t[0]];
         const uint32_t base = (uint32_t)o.a_ent.size();
-        const bool two = (t0.flags & kAuxTwoIndex) != 0;
-        o.a_ent.resize(o.a_ent.size() + (size_t)c.steps * 32, two ? pad2 : pad1);
+        const int per = 32 >> c.rshift, width = 1 << c.rshift;
         o.achunk.push_back(base);
         o.achunk.push_back((uint32_t)c.steps);
-        o.achunk.push_back(t0.flags | (c.reduce ? (uint32_t)kAuxReduce : 0u));
+        o.achunk.push_back(c.kind | (uint32_t)c.rshift << 8);
         o.achunk.push_back((uint32_t)o.a_out.size());
-        if (c.reduce) {
-            for (size_t e = 0; e < t0.ent.size(); ++e) o.a_ent[(size_t)base + (e / 32) * 32 + (e % 32)] = t0.ent[e];
-            o.a_out.push_back(t0.out);
-            o.a_const.push_back(t0.cst);
-            for (int l = 1; l < 32; ++l) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); }
-        } else {
-            for (int l = 0; l < 32; ++l) {
-                if (l >= (int)c.t.size()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); continue; }
-                const Task &t = tasks[c.t[l]];
-                o.a_out.push_back(t.out);
-                o.a_const.push_back(t.cst);
-                for (size_t e = 0; e < t.ent.size(); ++e) o.a_ent[(size_t)base + e * 32 + l] = t.ent[e];
-            }
+        if (c.kind == kAuxR3) {
+            o.a_out.push_back(0u);
+            o.a_const.push_back(0.0);
+            continue;
+        }
+        o.a_ent.resize(o.a_ent.size() + (size_t)c.steps * 32, c.kind == kAuxH2 ? pad2 : pad1);
+        for (int l = 0; l < per; ++l) {
+            if (l >= (int)c.t.size()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); continue; }
+            const Task &t = tasks[c.t[l]];
+            o.a_out.push_back(t.out);
+            o.a_const.push_back(t.cst);
+            for (size_t e = 0; e < t.ent.size(); ++e)
+                o.a_ent[(size_t)base + (e / width) * 32 + (size_t)l * width + (e % width)] = t.ent[e];
         }
         o.n_aux_entries += (long long)c.steps * 32;
     }

@@ -9,18 +9,19 @@ namespace pyjac {
 
 struct HostPack {
     int ns = 0, nr = 0;
-    std::vector<double> inv_mw, colc, wrow, nasa, t_mid;
+    std::vector<double> inv_mw, mw, colc, wrow, nasa, t_mid;
     int n_pd = 0, n_pk = 0;
+    std::vector<uint32_t> rchunk;
     std::vector<uint32_t> slots;          // 4 words per reaction
+    std::vector<uint32_t> vidx;           // 4 words per reaction
     std::vector<double> lnA, beta, Ta, rev_lnA, rev_beta, rev_Ta;
-    std::vector<uint32_t> vbase;
     std::vector<int32_t> rxn_orig;
     std::vector<uint32_t> th_off;
-    std::vector<double> th_data;
+    std::vector<double> th_data, th_soa;
     std::vector<double> lo_lnA, lo_beta, lo_Ta, fall_par;
-    std::vector<int32_t> eff_ptr, eff_spec;
+    std::vector<int32_t> eff_ptr;
+    std::vector<uint32_t> eff_spec;
     std::vector<double> eff_eps;
-    std::vector<uint32_t> eff_vbase;
     std::vector<int32_t> pk_ptr;
     std::vector<double> pk_data;
     int n_rchunk = 0;
@@ -31,9 +32,10 @@ struct HostPack {
     int n_mtask = 0;
     std::vector<uint32_t> mtask;          // uint4 flattened
     std::vector<uint32_t> m_ent;
-    int eQ = 0, eAr = 0, eTh = 0, eH = 0, eAlpha = 0, eGamma = 0, eWdot = 0, eS1 = 0, eS4 = 0, eZero = 0, n_e = 0;
-    // statistics (reported through pyjac_mech_stats for DESIGN.md / bench.py)
-    long long n_main_entries = 0, n_aux_entries = 0, n_list_entries = 0;
+    int eQ = 0, eAr = 0, eTh = 0, eH = 0, eAlpha = 0, eGamma = 0, eWdot = 0, eTcol = 0, eG0 = 0, eZ = 0;
+    int eS1 = 0, eA0 = 0, eS4 = 0, eZero = 0, eDump = 0, n_e = 0;
+    // statistics (pyjac_pack_stats)
+    long long n_main_entries = 0, n_aux_entries = 0, n_list_entries = 0, n_plain_chunks = 0;
 };
 
 // Returns PYJAC_OK, PYJAC_EINVAL or PYJAC_ELIMIT.  `why` (optional) receives a static message.
