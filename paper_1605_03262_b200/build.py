@@ -38,6 +38,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return SO
     cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
+    cmd += os.environ.get("PYJAC_NVCC_FLAGS", "").split()      # e.g. -DPYJAC_PROF (per-phase cycle print)
     cmd += [os.path.join(CSRC, f) for f in SOURCES] + ["-o", SO]
     res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
     if verbose or res.returncode != 0:

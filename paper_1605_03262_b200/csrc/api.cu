@@ -120,15 +120,15 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     m->n_sm = prop.multiProcessorCount;
     DeviceMech &dm = m->dm;
     dm.ns = hp.ns; dm.nr = hp.nr; dm.ld = hp.ns + 1;
-    dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk;
-    dm.n_achunk = hp.n_achunk; dm.n_achunk01 = hp.n_achunk01; dm.n_mtask = hp.n_mtask;
+    dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk; dm.n_plain = (int)hp.n_plain_chunks;
+    dm.n_achunk = hp.n_achunk; dm.n_achunk01 = hp.n_achunk01; dm.n_slab = hp.n_slab; dm.m_seg = 8;
     dm.eQ = hp.eQ; dm.eAr = hp.eAr; dm.eTh = hp.eTh; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;
     dm.eWdot = hp.eWdot; dm.eTcol = hp.eTcol; dm.eG0 = hp.eG0; dm.eZ = hp.eZ;
     dm.eS1 = hp.eS1; dm.eA0 = hp.eA0; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.eDump = hp.eDump; dm.n_e = hp.n_e;
     Uploader up;
     try {
         up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.mw, hp.mw);
-        up.add((const double **)&dm.colc, hp.colc); up.add(&dm.wrow, hp.wrow);
+        up.add(&dm.colc, hp.colc); up.add(&dm.wrow, hp.wrow);
         up.add(&dm.nasa, hp.nasa); up.add(&dm.t_mid, hp.t_mid);
         up.add(&dm.rchunk, hp.rchunk);
         up.add((const uint32_t **)&dm.slots, hp.slots); up.add((const uint32_t **)&dm.vidx, hp.vidx);
@@ -142,7 +142,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
         up.add((const uint32_t **)&dm.achunk, hp.achunk); up.add(&dm.a_ent, hp.a_ent);
         up.add(&dm.a_out, hp.a_out); up.add(&dm.a_const, hp.a_const);
-        up.add((const uint32_t **)&dm.mtask, hp.mtask); up.add(&dm.m_ent, hp.m_ent);
+        up.add(&dm.m_hdr, hp.m_hdr); up.add((const uint32_t **)&dm.m_ent, hp.m_ent);
     } catch (...) {
         delete m;
         cudaSetDevice(prev);
@@ -158,8 +158,15 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
         m->plan = make_smem_plan(hp.ns, hp.n_e);
         choose_shape(m->plan, (size_t)prop.sharedMemPerBlockOptin - 64, &m->threads, &m->S);
+        {   // MAIN work items: about three per warp, 4..32 columns each
+            const int nw = m->threads / 32, cols = hp.ns + 1;
+            int seg = (hp.n_slab * cols + 3 * nw - 1) / (3 * nw);
+            seg = seg < 4 ? 4 : seg > 32 ? 32 : seg;
+            if (const char *e = std::getenv("PYJAC_SEG")) { const int v = std::atoi(e); if (v >= 1 && v <= 32) seg = v; }
+            dm.m_seg = seg;
+        }
         m->stats[0] = hp.n_e; m->stats[1] = hp.n_list_entries; m->stats[2] = hp.n_main_entries;
-        m->stats[3] = hp.n_aux_entries; m->stats[4] = hp.n_mtask; m->stats[5] = hp.n_achunk;
+        m->stats[3] = hp.n_aux_entries; m->stats[4] = (long long)hp.n_slab * (hp.ns + 1); m->stats[5] = hp.n_achunk;
         const size_t bytes = eval_smem_bytes(m->plan, m->S);
         if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin) {
             rc = PYJAC_ELIMIT;
@@ -261,7 +268,7 @@ int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
     if (rc != PYJAC_OK) return rc;
     const SmemPlan plan = make_smem_plan(hp.ns, hp.n_e);
     stats[0] = hp.n_e; stats[1] = hp.n_list_entries; stats[2] = hp.n_main_entries; stats[3] = hp.n_aux_entries;
-    stats[4] = hp.n_mtask; stats[5] = hp.n_achunk; stats[6] = (int64_t)eval_smem_bytes(plan, 1); stats[7] = hp.n_rchunk;
+    stats[4] = (int64_t)hp.n_slab * (hp.ns + 1); stats[5] = hp.n_achunk; stats[6] = (int64_t)eval_smem_bytes(plan, 1); stats[7] = hp.n_rchunk;
     return PYJAC_OK;
 }
 

@@ -61,9 +61,9 @@ struct DeviceMech {
     // ---- species tables
     const double *inv_mw;       // [ns]
     const double *mw;           // [ns]
-    const double2 *colc;        // [ns+1] column constants by Jacobian column c: {d_j, 1/W_j}, j = c - 1;
-                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51);
-                                //        c = 0: {0, 1}; c = ns (the zero column): {0, 0}
+    const double *colc;         // [ns+1][4] column constants by Jacobian column c: {d_j, 1/W_j, 1, 0}, j = c - 1;
+                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51); the third
+                                //        entry switches gamma_r on; c = 0: {0, 1, 0, 0}; c = ns (zero column): zeros
     const double *wrow;         // [ns+1] row factors by Jacobian row r: {1, W_0 .. W_{ns-1}}
     const double *nasa;         // [2][5][ns] a_0..a_4, range-major, coefficient-major (coalesced over k)
     const double *t_mid;        // [ns]
@@ -71,6 +71,7 @@ struct DeviceMech {
     int n_pd;                   // pressure-dependent reactions (third body, falloff, chem. activated): [0, n_pd)
     int n_pk;                   // PLOG / Chebyshev reactions: [n_pd, n_pd + n_pk)
     int n_rchunk;               // groups of 32 reactions
+    int n_plain;                // the last n_plain groups hold only plain reactions
     const uint32_t *rchunk;     // [n_rchunk] 1 = every reaction of the group takes the plain path
     const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
     const uint4 *vidx;          // [nr] E indices of the slots' s'_ij: {v0|v1<<16, v2|v3<<16, v4|v5<<16, 0}
@@ -101,10 +102,11 @@ struct DeviceMech {
     const uint32_t *a_ent;      // entries at [first + step*32 + lane]
     const uint32_t *a_out;      // [task] E slot of the result (kAuxT3: the species k)
     const double *a_const;      // [task] constant factor (kAuxS1)
-    // ---- MAIN pass: the Jacobian as a flat column-major array, 32 consecutive elements per task
-    int n_mtask;
-    const uint4 *mtask;         // {first entry, steps | edge << 16, row of lane 0, column of lane 0}
-    const uint32_t *m_ent;      // entries at [first + step*32 + lane]
+    // ---- MAIN pass: the Jacobian in slabs of 32 rows, walked column by column
+    int n_slab;
+    int m_seg;                  // columns per work item (<= 32), chosen with the launch shape
+    const uint32_t *m_hdr;      // [n_slab][ns+1] (entry block << 3) | steps, steps <= 4
+    const uint4 *m_ent;         // blocks of 32 lanes x 4 entries: lane l of block b at [b*32 + l]
     // ---- regions of E (indices in doubles per state)
     int eQ, eAr, eTh, eH;       // [nr] each, consecutive (eAr = eQ + nr, eTh = eQ + 2 nr, eH = eQ + 3 nr)
     int eAlpha, eGamma;         // [ns+1] by Jacobian row; row 0 stays 0
@@ -120,19 +122,22 @@ struct DeviceMech {
 
 // per-state scalars (region Scal of the shared-memory plan)
 enum {
-    kT = 0, kLnT, kInvT, kP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kNScal = 12
+    kT = 0, kLnT, kInvT, kP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kNScal = 10
 };
 
 // Shared-memory plan (offsets in doubles PER STATE).  A CTA evaluates S states at a time and
-// interleaves them: element i of region R of state q lives at (R + i) * S + q.  After the S
-// interleaved state blocks come the state-independent tables (colc, wrow), loaded once per CTA.
+// interleaves them: element i of region R of state q lives at (R + i) * S + q.  The mixture block
+// (X, Cp, Scal) exists twice: the block of the next batch is filled while this one is in use.  After
+// the S interleaved state blocks come the state-independent tables (colc, wrow), loaded once per CTA.
 struct SmemPlan {
     int E;                              // [n_e]
-    int X;                              // [ns+1] concentrations; slot ns = 1 (empty reaction slots)
-    int Cp;                             // [ns] c_pk (mass based)
-    int Scal;                           // [2][kNScal], double-buffered by iteration parity
+    int P0;                             // two mixture blocks of p0size doubles
+    int p0size;
+    int oX;                             // within a mixture block: [ns+1] concentrations; slot ns = 1 (empty reaction slots)
+    int oCp;                            // [ns] c_pk (mass based)
+    int oScal;                          // [kNScal]
     int total;                          // doubles per state
-    int colc;                           // [ld] double2, offset in doubles from the end of the state blocks
+    int colc;                           // [ld][4], offset in doubles from the end of the state blocks
     int wrow;                           // [ld]
     int shared_total;                   // doubles of the state-independent part
 };
@@ -143,12 +148,18 @@ inline SmemPlan make_smem_plan(int ns, int n_e)
     int o = 0;
     auto take = [&](int n) { int r = o; o += (n + 1) & ~1; return r; };
     p.E = take(n_e);
-    p.X = take(ns + 1);
-    p.Cp = take(ns);
-    p.Scal = take(2 * kNScal);
+    p.P0 = o;
+    {
+        const int base = o;
+        p.oX = take(ns + 1) - base;
+        p.oCp = take(ns) - base;
+        p.oScal = take(kNScal) - base;
+        p.p0size = o - base;
+        o += p.p0size;
+    }
     p.total = o;
     o = 0;
-    p.colc = take(2 * (ns + 1));
+    p.colc = take(4 * (ns + 1));
     p.wrow = take(ns + 1);
     p.shared_total = o;
     return p;

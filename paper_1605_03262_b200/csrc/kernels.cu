@@ -26,12 +26,21 @@
 // There are no atomics and no Jacobian tile: every sum has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
 
+#include <cstdio>
+
 #include "device_mech.h"
 #include "kernels.h"
 
 namespace pyjac {
 
 namespace {
+
+// -DPYJAC_PROF: CTA 0 prints the cycles warp 0 spends in each phase of its fourth iteration
+#ifdef PYJAC_PROF
+#define PROF_MARK(i) do { if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x) prof_t[i] = clock64(); } while (0)
+#else
+#define PROF_MARK(i) do { } while (0)
+#endif
 
 constexpr double kLn10 = 2.302585092994045684;
 constexpr double kInvLn10 = 0.434294481903251828;
@@ -120,17 +129,16 @@ __device__ __forceinline__ void stv(double *p, const double (&v)[S])
 }
 
 // ---- P1, plain path: 32 elementary reactions with at most three molecules per side (one slot per
-// molecule), k_r from K_c or irreversible, one NASA breakpoint.  Two states at a time, no branches.
+// molecule), k_r from K_c or irreversible, one NASA breakpoint.  Two states at a time (q0, q0 + 1), no branches.
 template <int LEVEL, int S>
-__device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemPlan &sp, double *sm, const double *sc,
-                                                int s, const EvalOut &out, long long state0, long long n)
+__device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemPlan &sp, double *E, const double *X,
+                                                const double *sc, int s, int q0, const EvalOut &out, long long state0,
+                                                long long n)
 {
     constexpr int SP = S >= 2 ? 2 : 1;
     const int nr = m.nr;
     const uint4 sl = m.slots[s];
     const uint32_t meta = sl.w;
-    const double *X = sm + sp.X * S;
-    double *E = sm + sp.E * S;
     const int x0 = (sl.x & 0xFFFF) * S, x1 = (sl.x >> 16) * S, x2 = (sl.y & 0xFFFF) * S,
               x3 = (sl.y >> 16) * S, x4 = (sl.z & 0xFFFF) * S, x5 = (sl.z >> 16) * S;
     const int nf = (meta & 0xF) + ((meta >> 4) & 0xF) + ((meta >> 8) & 0xF);
@@ -148,8 +156,7 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
     }
     const int orig = LEVEL == 0 ? m.rxn_orig[s] : 0;
 
-#pragma unroll 1
-    for (int q0 = 0; q0 < S; q0 += SP) {
+    {
         double T[SP], lnT[SP], invT[SP], lnkf[SP], L[SP], sB[SP], sdB[SP], kf[SP], kr[SP];
 #pragma unroll
         for (int u = 0; u < SP; ++u) {
@@ -205,15 +212,14 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
     }
 }
 
-// ---- P1, general path: one reaction of any type, the S states one after the other --------------------
+// ---- P1, general path: one reaction of any type, one state (q) ----------------------------------------
 template <int LEVEL, int S>
-__device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *sm, const double *sc,
-                                         int s, const EvalOut &out, long long state0, long long n)
+__device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *E, const double *X,
+                                         const double *sc, int s, int q, const EvalOut &out, long long state0, long long n)
 {
     const uint4 sl = m.slots[s];
     const uint32_t meta = sl.w;
     const int type = meta_type(meta), rev = meta_rev(meta);
-    const double *X = sm + sp.X * S;
     const int x0 = (sl.x & 0xFFFF) * S, x1 = (sl.x >> 16) * S, x2 = (sl.y & 0xFFFF) * S,
               x3 = (sl.y >> 16) * S, x4 = (sl.z & 0xFFFF) * S, x5 = (sl.z >> 16) * S;
     const bool unit_nu = (meta & 0x00EEEEEEu) == 0;          // every nu is 0 or 1
@@ -226,7 +232,6 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     const double dnu = (double)(snu_r - snu_f);
     const double *th = m.th_data + m.th_off[s];
     const int nint = (int)th[0];
-    double *E = sm + sp.E * S;
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
     if (LEVEL == 2) {
         const uint4 vi = m.vidx[s];
@@ -236,8 +241,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     int eb = 0, ee = 0;
     if (pdep) { eb = m.eff_ptr[s]; ee = m.eff_ptr[s + 1]; }
 
-#pragma unroll 1
-    for (int q = 0; q < S; ++q) {
+    {
         const double T = sc[kT * S + q], lnT = sc[kLnT * S + q], invT = sc[kInvT * S + q];
 
         // ---- forward rate coefficient: ln k_f and L = d ln k_f / dT
@@ -430,83 +434,147 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     }
 }
 
+// next item of a phase's work queue (one shared counter per phase); plain ATOMS by lane 0
+__device__ __forceinline__ int grab(int *ctr, int lane)
+{
+    int t = 0;
+    if (lane == 0) {
+        const unsigned a = (unsigned)__cvta_generic_to_shared(ctr);
+        asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(t) : "r"(a) : "memory");
+    }
+    return __shfl_sync(0xFFFFFFFFu, t, 0);
+}
+
+// ---- P0: mixture (Eqs. 3-5) and species (Eqs. 5, 9, 12-13, 54-55) of one state, by one warp ----------
+template <int LEVEL, int S>
+__device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double *X, double *Cp, double *sc, int q,
+                                                    long long st, const double *__restrict__ Tg,
+                                                    const double *__restrict__ Pg, const double *__restrict__ Yg,
+                                                    long long ldy, int lane)
+{
+    const int ns = m.ns;
+    const double *Ys = Yg + st * ldy;
+    const double T = Tg[st], P = Pg[st];
+    double s = 0.0;
+    for (int k = lane; k < ns; k += 32) s += Ys[k] * m.inv_mw[k];
+    s = warp_sum(s);
+    const double W = 1.0 / s, M = P / (kRu * T), rho = M * W;
+    double cp = 0.0, dcp = 0.0;
+    for (int k = lane; k < ns; k += 32) {
+        const double iw = m.inv_mw[k], y = Ys[k];
+        X[k * S + q] = rho * (y * iw);
+        if (LEVEL >= 1) {
+            const double *a = m.nasa + (T <= m.t_mid[k] ? 0 : (size_t)5 * ns) + k;
+            const double a0 = a[0], a1 = a[ns], a2 = a[2 * (size_t)ns], a3 = a[3 * (size_t)ns], a4 = a[4 * (size_t)ns];
+            const double cpk = kRu * (a0 + T * (a1 + T * (a2 + T * (a3 + a4 * T)))) * iw;
+            Cp[k * S + q] = cpk;
+            cp += y * cpk;
+            if (LEVEL == 2) dcp += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
+        }
+    }
+    if (LEVEL >= 1) { cp = warp_sum(cp); dcp = warp_sum(dcp); }
+    if (lane == 0) {
+        sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P;
+        sc[kM * S + q] = M; sc[kW * S + q] = W; sc[kRho * S + q] = rho; sc[kIrho * S + q] = 1.0 / rho;
+        sc[kCpMix * S + q] = cp; sc[kDcpDT * S + q] = dcp;
+    }
+}
+
 // ---- the kernel ------------------------------------------------------------------------------------
 // Shared memory: S interleaved state blocks of sp.total doubles, then the state-independent column
-// and row constants.
+// and row constants.  The mixture block (X, Cp, scalars) is double-buffered: P0 of the NEXT batch is
+// an item of this batch's P1 queue.
 template <int LEVEL, int NT, int S, int MB>
 __global__ void __launch_bounds__(NT, MB)
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
                 const double *__restrict__ Pg, const double *__restrict__ Yg, long long ldy, const EvalOut out)
 {
     extern __shared__ __align__(16) double sm[];
+    __shared__ int ctr[2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
+    constexpr int SP = S >= 2 ? 2 : 1;
     const int ns = m.ns, ld = m.ld, nr = m.nr;
     double *E = sm + sp.E * S;
-    double *X = sm + sp.X * S;
-    double *Cp = sm + sp.Cp * S;
-    double *sc = sm + sp.Scal * S;
-    double2 *colc = reinterpret_cast<double2 *>(sm + (size_t)sp.total * S + sp.colc);
+    const double *colc = sm + (size_t)sp.total * S + sp.colc;
     double *wrow = sm + (size_t)sp.total * S + sp.wrow;
-    for (int i = tid; i < ld; i += NT) { colc[i] = m.colc[i]; wrow[i] = m.wrow[i]; }
+    {
+        double *cw = sm + (size_t)sp.total * S + sp.colc;
+        for (int i = tid; i < 4 * ld; i += NT) cw[i] = m.colc[i];
+        for (int i = tid; i < ld; i += NT) wrow[i] = m.wrow[i];
+    }
     if (tid < S) {   // the empty-slot dummy species, the zero slot, row 0 of alpha / gamma
-        X[ns * S + tid] = 1.0;
+        sm[(sp.P0 + sp.oX + ns) * S + tid] = 1.0;
+        sm[(sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
         E[m.eZero * S + tid] = 0.0;
         E[m.eAlpha * S + tid] = 0.0;
         E[m.eGamma * S + tid] = 0.0;
         if (nr == 0) { E[m.eS1 * S + tid] = 0.0; E[m.eA0 * S + tid] = 0.0; E[m.eS4 * S + tid] = 0.0; }
     }
+    if (tid == 0) ctr[0] = 0;
     const long long nblk = (n + S - 1) / S;
-    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x) {
+    // work items of P1: the general groups one state at a time (most expensive first), P0 of the next
+    // batch (one state each), then the plain groups SP states at a time
+    const int n_gen = m.n_rchunk - m.n_plain;
+    const int i_p0 = n_gen * S, i_plain = i_p0 + S;
+    const int n_p1 = i_plain + m.n_plain * (S / SP);
+    if (warp < S && (long long)blockIdx.x < nblk) {
+        double *P0 = sm + sp.P0 * S;
+        mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oScal * S, warp,
+                                      min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
+    }
+    int par = 0;
+    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x, par ^= 1) {
         const long long state0 = blk * S;
-        // ---- P0: mixture (Eqs. 3-5) and species (Eqs. 5, 9, 12-13, 54-55); warp q <-> state q
-        for (int q = warp; q < S; q += NW) {
-            const long long st = min(state0 + q, n - 1);
-            const double *Ys = Yg + st * ldy;
-            const double T = Tg[st], P = Pg[st];
-            double s = 0.0;
-            for (int k = lane; k < ns; k += 32) s += Ys[k] * m.inv_mw[k];
-            s = warp_sum(s);
-            const double W = 1.0 / s, M = P / (kRu * T), rho = M * W;
-            double cp = 0.0, dcp = 0.0;
-            for (int k = lane; k < ns; k += 32) {
-                const double iw = m.inv_mw[k], y = Ys[k];
-                X[k * S + q] = rho * (y * iw);
-                if (LEVEL >= 1) {
-                    const double *a = m.nasa + (T <= m.t_mid[k] ? 0 : (size_t)5 * ns) + k;
-                    const double a0 = a[0], a1 = a[ns], a2 = a[2 * (size_t)ns], a3 = a[3 * (size_t)ns],
-                                 a4 = a[4 * (size_t)ns];
-                    const double cpk = kRu * (a0 + T * (a1 + T * (a2 + T * (a3 + a4 * T)))) * iw;
-                    Cp[k * S + q] = cpk;
-                    cp += y * cpk;
-                    if (LEVEL == 2) dcp += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
-                }
-            }
-            if (LEVEL >= 1) { cp = warp_sum(cp); dcp = warp_sum(dcp); }
-            if (lane == 0) {
-                sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P;
-                sc[kM * S + q] = M; sc[kW * S + q] = W; sc[kRho * S + q] = rho; sc[kIrho * S + q] = 1.0 / rho;
-                sc[kCpMix * S + q] = cp; sc[kDcpDT * S + q] = dcp;
+        double *P0 = sm + (sp.P0 + par * sp.p0size) * S, *P0n = sm + (sp.P0 + (par ^ 1) * sp.p0size) * S;
+        const double *X = P0 + sp.oX * S, *Cp = P0 + sp.oCp * S, *sc = P0 + sp.oScal * S;
+#ifdef PYJAC_PROF
+        long long prof_t[12];
+#endif
+        PROF_MARK(0);
+        __syncthreads();      // every warp has left the previous MAIN pass (and the first P0 is done)
+        PROF_MARK(1);
+        // ---- P1: reactions (+ the mixture of the next batch)
+        for (int it = grab(&ctr[0], lane); it < n_p1; it = grab(&ctr[0], lane)) {
+            if (it < i_p0) {
+                const int c = it / S, q = it - c * S;
+                reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q, out, state0, n);
+            } else if (it < i_plain) {
+                const int q = it - i_p0;
+                if (blk + gridDim.x < nblk)
+                    mixture_and_species<LEVEL, S>(m, P0n + sp.oX * S, P0n + sp.oCp * S, P0n + sp.oScal * S, q,
+                                                  min((blk + gridDim.x) * S + q, n - 1), Tg, Pg, Yg, ldy, lane);
+            } else {
+                const int j = it - i_plain;
+                const int c = n_gen + j / (S / SP), q0 = (j % (S / SP)) * SP;
+                plain_reactions<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q0, out, state0, n);
             }
         }
-        __syncthreads();      // every warp has also left the previous iteration's MAIN pass
-        // ---- P1: reactions
-        for (int c = warp; c < m.n_rchunk; c += NW) {
-            const int s = min(c * 32 + lane, nr - 1);      // the last group repeats its last reaction
-            if (m.rchunk[c]) plain_reactions<LEVEL, S>(m, sp, sm, sc, s, out, state0, n);
-            else reaction<LEVEL, S>(m, sp, sm, sc, s, out, state0, n);
-        }
+        PROF_MARK(2);
         __syncthreads();
-        // ---- AUX gathers
+        if (tid == 0) ctr[0] = 0;
+        PROF_MARK(3);
+        // ---- AUX gathers: chunk i of the list goes to warp i mod NW; the entries of a warp's next
+        // chunk are fetched before the current one is summed
         {
             const int nch = LEVEL == 2 ? m.n_achunk : m.n_achunk01;
-            for (int c = warp; c < nch; c += NW) {
-                const uint4 ch = m.achunk[c];
+            const uint4 hz = make_uint4(0u, 0u, 0u, 0u);
+            int t0 = warp;
+            uint4 h0 = t0 < nch ? m.achunk[t0] : hz, h1 = t0 + NW < nch ? m.achunk[t0 + NW] : hz;
+            const uint4 *ap = reinterpret_cast<const uint4 *>(m.a_ent);
+            uint4 ea = hz, eb = hz;
+            if (h0.y > 0 && (h0.z & 0xFF) != kAuxR3) { ea = ap[h0.x / 4 + lane * 2]; if (h0.y > 4) eb = ap[h0.x / 4 + lane * 2 + 1]; }
+            for (; t0 < nch; t0 += NW) {
+                const uint4 h2 = t0 + 2 * NW < nch ? m.achunk[t0 + 2 * NW] : hz;
+                uint4 na = hz, nb = hz;
+                if (h1.y > 0 && (h1.z & 0xFF) != kAuxR3) { na = ap[h1.x / 4 + lane * 2]; if (h1.y > 4) nb = ap[h1.x / 4 + lane * 2 + 1]; }
+                // ---- chunk t0
+                const uint4 ch = h0;
                 const uint32_t kind = ch.z & 0xFF;
                 const int rshift = (ch.z >> 8) & 0xFF, width = 1 << rshift;
-                const uint32_t *ent = m.a_ent + ch.x + lane;
                 const bool head = (lane & (width - 1)) == 0;
                 const uint32_t task = ch.w + (lane >> rshift);
+                const uint32_t e0[8] = {ea.x, ea.y, ea.z, ea.w, eb.x, eb.y, eb.z, eb.w};
                 if (kind == kAuxT3 || kind == kAuxR3) {
                     constexpr int NA = LEVEL == 2 ? 3 : 1;
                     constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
@@ -516,9 +584,7 @@ __global__ void __launch_bounds__(NT, MB)
 #pragma unroll
                         for (int q = 0; q < S; ++q) acc[w][q] = 0.0;
                     if (kind == kAuxT3) {
-#pragma unroll 2
-                        for (uint32_t t = 0; t < ch.y; ++t) {
-                            const uint32_t e = ent[t * 32];
+                        auto step = [&](uint32_t e) {
                             const double cf = entry_coef(e);
                             const double *p = E + (e & 0xFFFF) * S;
 #pragma unroll
@@ -528,7 +594,11 @@ __global__ void __launch_bounds__(NT, MB)
 #pragma unroll
                                 for (int q = 0; q < S; ++q) acc[w][q] = fma(cf, a[q], acc[w][q]);
                             }
-                        }
+                        };
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if ((uint32_t)j < ch.y) step(e0[j]);
+                        for (uint32_t t = 8; t < ch.y; ++t) step(m.a_ent[ch.x + (t >> 3) * 256 + lane * 8 + (t & 7)]);
                     } else {
                         for (int i = lane; i < nr; i += 32) {
                             double h[S];
@@ -575,25 +645,29 @@ __global__ void __launch_bounds__(NT, MB)
 #pragma unroll
                     for (int q = 0; q < S; ++q) acc[q] = 0.0;
                     if (kind == kAuxH2) {
-#pragma unroll 2
-                        for (uint32_t t = 0; t < ch.y; ++t) {
-                            const uint32_t e = ent[t * 32];
+                        auto step = [&](uint32_t e) {
                             double a[S], b[S];
                             ldv<S>(E + (e & 0xFFFF) * S, a);
                             ldv<S>(E + (e >> 16) * S, b);
 #pragma unroll
                             for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
-                        }
+                        };
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if ((uint32_t)j < ch.y) step(e0[j]);
+                        for (uint32_t t = 8; t < ch.y; ++t) step(m.a_ent[ch.x + (t >> 3) * 256 + lane * 8 + (t & 7)]);
                     } else {
-#pragma unroll 2
-                        for (uint32_t t = 0; t < ch.y; ++t) {
-                            const uint32_t e = ent[t * 32];
+                        auto step = [&](uint32_t e) {
                             const double cf = entry_coef(e);
                             double a[S];
                             ldv<S>(E + (e & 0xFFFF) * S, a);
 #pragma unroll
                             for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
-                        }
+                        };
+#pragma unroll
+                        for (int j = 0; j < 8; ++j)
+                            if ((uint32_t)j < ch.y) step(e0[j]);
+                        for (uint32_t t = 8; t < ch.y; ++t) step(m.a_ent[ch.x + (t >> 3) * 256 + lane * 8 + (t & 7)]);
                     }
                     for (int o = 1; o < width; o <<= 1)
 #pragma unroll
@@ -608,9 +682,12 @@ __global__ void __launch_bounds__(NT, MB)
                         stv<S>(E + slot * S, acc);
                     }
                 }
+                h0 = h1; h1 = h2; ea = na; eb = nb;
             }
         }
+        PROF_MARK(4);
         __syncthreads();
+        PROF_MARK(5);
         // ---- outputs of the rates / source-term kernels (Eqs. 7-8, 14)
         if (LEVEL == 0 && out.wdot) {
             for (int k = tid; k < ns; k += NT)
@@ -634,21 +711,34 @@ __global__ void __launch_bounds__(NT, MB)
             const int nfix = 1 + (ns - 1 + 31) / 32;
             for (int it = warp; it < nfix; it += NW) {
                 if (it == 0) {
+                    double s3[S];       // sum_k c_pk W_k wdot_k
 #pragma unroll
-                    for (int q = 0; q < S; ++q) {
-                        double s3 = 0.0;       // sum_k c_pk W_k wdot_k
-                        for (int k = lane; k < ns; k += 32) s3 += Cp[k * S + q] * wrow[k + 1] * E[(m.eWdot + k) * S + q];
-                        s3 = warp_sum(s3);
-                        if (lane == 0) {
-                            const double icp = 1.0 / sc[kCpMix * S + q];
-                            E[m.eZ * S + q] = -icp * sc[kIrho * S + q] *
-                                              (s3 - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
-                        }
+                    for (int q = 0; q < S; ++q) s3[q] = 0.0;
+                    for (int k = lane; k < ns; k += 32) {
+                        const double wk = wrow[k + 1];
+                        double cp[S], wd[S];
+                        ldv<S>(Cp + k * S, cp);
+                        ldv<S>(E + (m.eWdot + k) * S, wd);
+#pragma unroll
+                        for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
+                    }
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                        for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
+                    if (lane < S) {
+                        const int q = lane;
+                        double s = s3[0];
+#pragma unroll
+                        for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
+                        const double icp = 1.0 / sc[kCpMix * S + q];
+                        E[m.eZ * S + q] = -icp * sc[kIrho * S + q] *
+                                          (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
                     }
                 } else {
                     const int c = (it - 1) * 32 + lane + 1;
                     if (c < ns) {
-                        const double2 cc = colc[c];
+                        const double dx = colc[4 * c];
                         const double wj = wrow[c], iwl = m.inv_mw[ns - 1];
 #pragma unroll
                         for (int q = 0; q < S; ++q) {
@@ -658,52 +748,73 @@ __global__ void __launch_bounds__(NT, MB)
                             const double gamma0 = -(iwl * icp) * E[(m.eG0 + ns - 1) * S + q];
                             const double dcp = Cp[(c - 1) * S + q] - Cp[(ns - 1) * S + q];
                             E[(m.eZ + c) * S + q] =
-                                wj * (alpha0 * cc.x - gamma0 + a1 * dcp) - icp * E[(m.eG0 + c - 1) * S + q];
+                                wj * (alpha0 * dx - gamma0 + a1 * dcp) - icp * E[(m.eG0 + c - 1) * S + q];
                         }
                     }
                 }
             }
+            PROF_MARK(6);
             __syncthreads();
-            // ---- MAIN pass: lane <-> Jacobian element f = r + c * ld (column-major): gather, Eq. 112, store
+            PROF_MARK(7);
+            // ---- MAIN pass: warp <-> (slab of 32 rows, segment of columns); lane <-> row.  alpha_r,
+            // gamma_r, W_r stay in registers; per column: one 16-byte load of the lane's entries (the
+            // next column's is in flight), gather, Eq. 112, store (32 consecutive rows = 256 bytes).
             const long long Jstate = (long long)ld * ld;
-            double *Jbase = out.jac + state0 * Jstate + lane;
-            for (int t = warp; t < m.n_mtask; t += NW) {
-                const uint4 mt = m.mtask[t];
-                const uint32_t steps = mt.y & 0xFFFF;
-                int r = (int)mt.z + lane, c = (int)mt.w;
-                while (r >= ld) { r -= ld; ++c; }
-                const bool live = c <= ns;
-                const uint32_t *ent = m.m_ent + mt.x + lane;
-                double acc[S];
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] = 0.0;
-#pragma unroll 2
-                for (uint32_t st = 0; st < steps; ++st) {
-                    const uint32_t e = ent[st * 32];
-                    const double cf = entry_coef(e);
-                    double a[S];
-                    ldv<S>(E + (e & 0xFFFF) * S, a);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
-                }
-                const double2 cc = colc[live ? c : 0];
-                const double wj = wrow[r] * cc.y;
+            const int seg = m.m_seg, nseg = (ld + seg - 1) / seg;
+            const int n_items = m.n_slab * nseg;
+            const uint4 ez = make_uint4(0u, 0u, 0u, 0u);
+            for (int it = warp; it < n_items; it += NW) {
+                const int slab = it % m.n_slab, sg = it / m.n_slab;
+                const int c0 = sg * seg, c1 = min(ld, c0 + seg);
+                const int r = slab * 32 + lane;
+                const bool rlive = r < ld;
+                const int rr = rlive ? r : 0;
+                const double wr = wrow[rr];
                 double alpha[S], gamma[S];
-                ldv<S>(E + (m.eAlpha + r) * S, alpha);
-                ldv<S>(E + (m.eGamma + r) * S, gamma);
-                if (mt.y >> 16) {          // the task touches column 0 or the zero column: no gamma there
-                    if (c == 0 || c >= ns) {
+                ldv<S>(E + (m.eAlpha + rr) * S, alpha);
+                ldv<S>(E + (m.eGamma + rr) * S, gamma);
+                const uint32_t hdrs = c0 + lane < c1 ? m.m_hdr[slab * ld + c0 + lane] : 0u;
+                double *Jp = out.jac + state0 * Jstate + (long long)c0 * ld + rr;
+                uint32_t h = __shfl_sync(0xFFFFFFFFu, hdrs, 0);
+                uint4 e = (h & 7) ? m.m_ent[(h >> 3) * 32 + lane] : ez;
+                for (int c = c0; c < c1; ++c, Jp += ld) {
+                    const uint32_t hn = __shfl_sync(0xFFFFFFFFu, hdrs, (c + 1 - c0) & 31);
+                    const uint4 en = (c + 1 < c1 && (hn & 7)) ? m.m_ent[(hn >> 3) * 32 + lane] : ez;
+                    const uint32_t steps = h & 7;
+                    double acc[S];
 #pragma unroll
-                        for (int q = 0; q < S; ++q) gamma[q] = 0.0;
+                    for (int q = 0; q < S; ++q) acc[q] = 0.0;
+                    auto step = [&](uint32_t w) {
+                        const double cf = entry_coef(w);
+                        double a[S];
+                        ldv<S>(E + (w & 0xFFFF) * S, a);
+#pragma unroll
+                        for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
+                    };
+                    if (steps > 0) step(e.x);
+                    if (steps > 1) step(e.y);
+                    if (steps > 2) step(e.z);
+                    if (steps > 3) step(e.w);
+                    const double2 c01 = *reinterpret_cast<const double2 *>(colc + 4 * c);
+                    const double gz = colc[4 * c + 2];
+                    const double wj = wr * c01.y;
+#pragma unroll
+                    for (int q = 0; q < S; ++q) {
+                        const double v = fma(wj, acc[q], fma(alpha[q], c01.x, -(gamma[q] * gz)));
+                        if (rlive && state0 + q < n) __stcs(Jp + q * Jstate, v);
                     }
-                }
-                double *Jp = Jbase + (long long)t * 32;
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    const double v = fma(wj, acc[q], fma(alpha[q], cc.x, -gamma[q]));
-                    if (live && state0 + q < n) __stcs(Jp + q * Jstate, v);
+                    h = hn; e = en;
                 }
             }
+            PROF_MARK(8);
+#ifdef PYJAC_PROF
+            if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x)
+                printf("PROF w%d wait %lld | P1 %lld wait %lld | AUX %lld wait %lld | FIX %lld wait %lld | MAIN %lld\n",
+                       warp, prof_t[1] - prof_t[0], prof_t[2] - prof_t[1], prof_t[3] - prof_t[2], prof_t[4] - prof_t[3],
+                       prof_t[5] - prof_t[4], prof_t[6] - prof_t[5], prof_t[7] - prof_t[6], prof_t[8] - prof_t[7]);
+#endif
+        } else {
+            __syncthreads();      // the outputs above read E and the scalars
         }
     }
 }

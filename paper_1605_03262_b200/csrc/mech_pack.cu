@@ -43,12 +43,12 @@ struct Task {
     int steps() const { return (int)((ent.size() + (size_t(1) << rshift) - 1) >> rshift); }
 };
 
-// lanes that share one sum: enough that no lane walks more than about 12 entries
+// lanes that share one sum: enough that no lane walks more than 8 entries (kAuxPre of kernels.cu)
 int pick_rshift(size_t len)
 {
-    if (len <= 12) return 0;
+    if (len <= 8) return 0;
     for (int r = 2; r < 5; ++r)
-        if (((len + (size_t(1) << r) - 1) >> r) <= 12) return r;
+        if (((len + (size_t(1) << r) - 1) >> r) <= 8) return r;
     return 5;
 }
 
@@ -159,11 +159,12 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     const double iw_last = 1.0 / d->mol_wt[ns - 1];
     o.wrow.assign((size_t)ld, 1.0);
     for (int k = 0; k < ns; ++k) o.wrow[k + 1] = d->mol_wt[k];
-    o.colc.assign((size_t)2 * ld, 0.0);
+    o.colc.assign((size_t)4 * ld, 0.0);       // {d_j, 1/W_j, 1 (gamma_r applies), 0}; column 0: {0, 1, 0, 0}; column ns: zeros
     o.colc[1] = 1.0;
     for (int k = 0; k + 1 < ns; ++k) {
-        o.colc[2 * (k + 1)] = 1.0 / d->mol_wt[k] - iw_last;
-        o.colc[2 * (k + 1) + 1] = 1.0 / d->mol_wt[k];
+        o.colc[4 * (k + 1)] = 1.0 / d->mol_wt[k] - iw_last;
+        o.colc[4 * (k + 1) + 1] = 1.0 / d->mol_wt[k];
+        o.colc[4 * (k + 1) + 2] = 1.0;
     }
 
     // ---- per reaction: molecules per side, breakpoints of its species' NASA ranges
@@ -428,78 +429,88 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     for (int c = 0; c < ns; ++c) cell[(size_t)c * ld].push_back(pack_entry((uint32_t)(eZ + c), 1));        // row 0
     for (auto &c : cell) o.n_list_entries += (long long)c.size();
 
-    // ---- MAIN tasks: 32 consecutive cells; lists longer than the task's cap are summed by an AUX
-    // task and enter as one entry.  The cap minimises (steps of the task) + (steps of the AUX
-    // chunks it causes); `lambda` prices the extra E slots and grows until E fits the shared memory.
-    const size_t ncell = (size_t)ld * ld;
-    o.n_mtask = (int)((ncell + 31) / 32);
-    const size_t fixed_tasks = tasks.size();
-    std::vector<int> cap(o.n_mtask, 0);
+    // ---- MAIN pass: the Jacobian in slabs of 32 rows; a warp walks a slab column by column.  Per
+    // (slab, column) every lane (row) gathers at most `cap` <= 4 entries (one 16-byte load); longer
+    // lists are summed by an AUX task and enter as one entry.  The cap minimises (steps of the slab
+    // column) + (steps of the AUX chunks it causes); `lambda` prices the extra E slots and grows until
+    // E fits the shared memory.
+    const int n_slab = (ld + 31) / 32;
+    o.n_slab = n_slab;
+    auto cell_at = [&](int slab, int c, int l) -> std::vector<uint32_t> * {
+        const int r = 32 * slab + l;
+        return r < ld ? &cell[(size_t)r + (size_t)c * ld] : nullptr;
+    };
+    std::vector<int> cap((size_t)n_slab * ld, 0);
     const long long e_limit = std::min<long long>(smem_doubles, 65535);
     for (double lambda = 0.15;; lambda *= 2.0) {
         int slots = next_slot;
         bool any_overflow = false;
-        for (int t = 0; t < o.n_mtask; ++t) {
-            int len[32], mx = 0;
-            for (int l = 0; l < 32; ++l) {
-                const size_t f = (size_t)t * 32 + l;
-                len[l] = f < ncell ? (int)cell[f].size() : 0;
-                mx = std::max(mx, len[l]);
-            }
-            double best = 1e300;
-            int bestc = mx;
-            for (int c = (mx > 0 ? 1 : 0); c <= mx; ++c) {
-                double cost = (double)c;
+        for (int sb = 0; sb < n_slab; ++sb)
+            for (int c = 0; c < ld; ++c) {
+                int len[32], mx = 0;
+                for (int l = 0; l < 32; ++l) {
+                    auto *p = cell_at(sb, c, l);
+                    len[l] = p ? (int)p->size() : 0;
+                    mx = std::max(mx, len[l]);
+                }
+                double best = 1e300;
+                int bestc = mx;
+                for (int cc = (mx > 0 ? 1 : 0); cc <= std::min(mx, 4); ++cc) {
+                    double cost = (double)cc;
+                    for (int l = 0; l < 32; ++l)
+                        if (len[l] > cc) cost += 1.25 * len[l] / 32.0 + lambda;
+                    if (cost < best) { best = cost; bestc = cc; }
+                }
+                cap[(size_t)sb * ld + c] = bestc;
                 for (int l = 0; l < 32; ++l)
-                    if (len[l] > c) cost += 1.25 * len[l] / 32.0 + lambda;
-                if (cost < best) { best = cost; bestc = c; }
+                    if (len[l] > bestc) { ++slots; any_overflow = true; }
             }
-            cap[t] = bestc;
-            for (int l = 0; l < 32; ++l)
-                if (len[l] > bestc) { ++slots; any_overflow = true; }
-        }
         if (slots <= e_limit) break;
         if (!any_overflow || lambda > 1e6) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
     }
-    (void)fixed_tasks;
-    for (int t = 0; t < o.n_mtask; ++t)
-        for (int l = 0; l < 32; ++l) {
-            const size_t f = (size_t)t * 32 + l;
-            if (f >= ncell || (int)cell[f].size() <= cap[t]) continue;
-            Task a;
-            a.kind = kAuxS1;
-            a.out = (uint32_t)next_slot++;
-            a.ent.swap(cell[f]);
-            tasks.push_back(a);
-            cell[f].push_back(pack_entry(tasks.back().out, 1));
-        }
+    for (int sb = 0; sb < n_slab; ++sb)
+        for (int c = 0; c < ld; ++c)
+            for (int l = 0; l < 32; ++l) {
+                auto *p = cell_at(sb, c, l);
+                if (!p || (int)p->size() <= cap[(size_t)sb * ld + c]) continue;
+                Task a;
+                a.kind = kAuxS1;
+                a.out = (uint32_t)next_slot++;
+                a.ent.swap(*p);
+                tasks.push_back(a);
+                p->push_back(pack_entry(tasks.back().out, 1));
+            }
     o.n_e = next_slot;
     if (o.n_e > e_limit) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
     const uint32_t pad1 = pack_entry((uint32_t)eZero, 0);
     const uint32_t pad2 = (uint32_t)eZero | (uint32_t)eZero << 16;
 
-    // ---- MAIN entries
-    o.mtask.assign((size_t)4 * o.n_mtask, 0u);
-    for (int t = 0; t < o.n_mtask; ++t) {
-        const uint32_t base = (uint32_t)o.m_ent.size();
-        const size_t f0 = (size_t)t * 32, f1 = std::min(ncell, f0 + 32) - 1;
-        const bool edge = f0 / ld == 0 || f1 / ld == (size_t)ns;       // touches column 0 or the zero column
-        o.mtask[4 * t + 0] = base;
-        o.mtask[4 * t + 1] = (uint32_t)cap[t] | (edge ? 1u << 16 : 0u);
-        o.mtask[4 * t + 2] = (uint32_t)(f0 % ld);
-        o.mtask[4 * t + 3] = (uint32_t)(f0 / ld);
-        o.m_ent.resize(o.m_ent.size() + (size_t)cap[t] * 32, pad1);
-        for (int l = 0; l < 32; ++l) {
-            const size_t f = f0 + l;
-            if (f >= ncell) continue;
-            for (size_t e = 0; e < cell[f].size(); ++e) o.m_ent[(size_t)base + e * 32 + l] = cell[f][e];
+    // ---- MAIN entries: m_hdr[slab][column] = (block index << 3) | steps; a block is 32 lanes x 4 entries
+    o.m_hdr.assign((size_t)n_slab * ld, 0u);
+    for (int sb = 0; sb < n_slab; ++sb)
+        for (int c = 0; c < ld; ++c) {
+            int steps = 0;
+            for (int l = 0; l < 32; ++l) {
+                auto *p = cell_at(sb, c, l);
+                if (p) steps = std::max(steps, (int)p->size());
+            }
+            if (steps == 0) continue;
+            const uint32_t blk = (uint32_t)(o.m_ent.size() / 128);
+            o.m_hdr[(size_t)sb * ld + c] = blk << 3 | (uint32_t)steps;
+            o.m_ent.resize(o.m_ent.size() + 128, pad1);
+            for (int l = 0; l < 32; ++l) {
+                auto *p = cell_at(sb, c, l);
+                if (!p) continue;
+                for (size_t e = 0; e < p->size(); ++e) o.m_ent[(size_t)blk * 128 + (size_t)l * 4 + e] = (*p)[e];
+            }
+            o.n_main_entries += (long long)steps * 32;
         }
-        o.n_main_entries += (long long)cap[t] * 32;
-    }
-    if (o.m_ent.empty()) o.m_ent.push_back(pad1);
+    if (o.m_ent.empty()) o.m_ent.assign(128, pad1);
 
     // ---- AUX chunks: sums of one kind, shared by equally many lanes and of similar length, fill the
-    // 32 lanes of a chunk; the warps take the chunks in a fixed round-robin order, longest first
+    // 32 lanes of a chunk; the warps take the chunks in a fixed round-robin order, longest first.
+    // Entries: step t of lane l at ent_base + (t / 8) * 256 + l * 8 + (t % 8) (two 16-byte loads per
+    // lane fetch eight steps).
     for (auto &t : tasks) t.rshift = pick_rshift(t.ent.size());
     struct Chunk { std::vector<size_t> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; };
     std::vector<Chunk> chunks;
@@ -547,18 +558,21 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
             o.a_const.push_back(0.0);
             continue;
         }
-        o.a_ent.resize(o.a_ent.size() + (size_t)c.steps * 32, c.kind == kAuxH2 ? pad2 : pad1);
+        const int rounds = (c.steps + 7) / 8;
+        o.a_ent.resize(o.a_ent.size() + (size_t)rounds * 256, c.kind == kAuxH2 ? pad2 : pad1);
         for (int l = 0; l < per; ++l) {
             if (l >= (int)c.t.size()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); continue; }
             const Task &t = tasks[c.t[l]];
             o.a_out.push_back(t.out);
             o.a_const.push_back(t.cst);
-            for (size_t e = 0; e < t.ent.size(); ++e)
-                o.a_ent[(size_t)base + (e / width) * 32 + (size_t)l * width + (e % width)] = t.ent[e];
+            for (size_t e = 0; e < t.ent.size(); ++e) {
+                const size_t step = e / width, lane = (size_t)l * width + (e % width);
+                o.a_ent[(size_t)base + (step / 8) * 256 + lane * 8 + (step % 8)] = t.ent[e];
+            }
         }
         o.n_aux_entries += (long long)c.steps * 32;
     }
-    if (o.a_ent.empty()) o.a_ent.push_back(pad1);
+    if (o.a_ent.empty()) o.a_ent.assign(256, pad1);
     if (o.achunk.empty()) { o.achunk.assign(4, 0u); }
     if (o.a_out.empty()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); }
 }

@@ -29,9 +29,9 @@ struct HostPack {
     std::vector<uint32_t> achunk;         // uint4 flattened
     std::vector<uint32_t> a_ent, a_out;
     std::vector<double> a_const;
-    int n_mtask = 0;
-    std::vector<uint32_t> mtask;          // uint4 flattened
-    std::vector<uint32_t> m_ent;
+    int n_slab = 0;
+    std::vector<uint32_t> m_hdr;          // [n_slab][ns+1]
+    std::vector<uint32_t> m_ent;          // blocks of 32 lanes x 4 entries
     int eQ = 0, eAr = 0, eTh = 0, eH = 0, eAlpha = 0, eGamma = 0, eWdot = 0, eTcol = 0, eG0 = 0, eZ = 0;
     int eS1 = 0, eA0 = 0, eS4 = 0, eZero = 0, eDump = 0, n_e = 0;
     // statistics (pyjac_pack_stats)
