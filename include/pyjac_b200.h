@@ -170,11 +170,12 @@ int pyjac_jacobian_launch_config(const pyjac_mech *mech, int64_t n, int32_t *thr
                                  int32_t *smem_bytes, int32_t *ctas_per_sm, int32_t *grid);
 
 /* Host-only: validates and packs `host_desc` exactly as pyjac_mech_create does (no CUDA call) and
- * reports the size of the evaluation tables.  stats[0..7] = doubles of shared memory per state for
- * the per-reaction products and gathered sums (array E), entries of all Jacobian cell lists, entry
- * slots of the MAIN pass (32 per step), entry slots of the AUX gathers, MAIN tasks (32 output
- * elements each), AUX chunks, shared-memory bytes of a CTA that evaluates one state at a time,
- * groups of 32 reactions.  Errors as pyjac_mech_create (PYJAC_EINVAL, PYJAC_ELIMIT, PYJAC_ENOMEM). */
+ * reports the size of the evaluation tables.  stats[0..11] = doubles of shared memory per state for
+ * the per-reaction products and gathered sums (array E, without the tile), entries of all Jacobian
+ * cell lists, gather steps of the cell chunks (32 lanes each), gather steps of the A1 chunks,
+ * Jacobian cells with a gather task, gather chunks, shared-memory bytes of one CTA, groups of 32
+ * reactions, states per CTA iteration (S), threads per CTA, column panels, columns per panel.
+ * Errors as pyjac_mech_create (PYJAC_EINVAL, PYJAC_ELIMIT, PYJAC_ENOMEM). */
 int pyjac_pack_stats(const pyjac_mech_desc *host_desc, int64_t *stats);
 
 /* Static, never-NULL description of an error code. */

@@ -113,15 +113,15 @@ def mech_desc(mech: Mechanism):
     return d, keep
 
 
-PACK_STAT_NAMES = ("e_doubles", "list_entries", "main_entry_slots", "aux_entry_slots", "main_tasks", "aux_chunks",
-                   "smem_bytes_one_state", "reaction_chunks")
+PACK_STAT_NAMES = ("e_doubles", "cell_entries", "cell_steps", "a1_steps", "cells", "chunks",
+                   "smem_bytes_per_cta", "reaction_chunks", "states_per_cta", "threads", "panels", "panel_columns")
 
 
 def pack_stats(mech: Mechanism) -> dict:
     """Host-only: sizes of the evaluation tables `pyjac_mech_create` would build (no CUDA call)."""
     lib = load_library()
     d, keep = mech_desc(mech)
-    out = (C.c_int64 * 8)()
+    out = (C.c_int64 * 12)()
     _check(lib.pyjac_pack_stats(C.byref(d), out), "pyjac_pack_stats")
     return dict(zip(PACK_STAT_NAMES, [int(v) for v in out]))
 

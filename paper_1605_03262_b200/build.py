@@ -2,21 +2,26 @@
 
     python -m paper_1605_03262_b200.build [--force] [--verbose]
 
-nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box.
+nvcc cross-compiles without a GPU.  kernels.cu is compiled once per CTA size (in parallel), the
+objects go to paper_1605_03262_b200/build/.  The .so is git-ignored but travels to the GPU box.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libpyjac_b200.so")
-SOURCES = ["api.cu", "mech_pack.cu", "kernels.cu"]
+HOST_SOURCES = ["api.cu", "mech_pack.cu", "dispatch.cu"]
+# (threads per CTA, CTAs per SM the register budget is set for) -- keep in step with csrc/dispatch.cu
+KERNEL_SIZES = [(128, 4), (256, 3), (384, 2), (512, 1), (768, 1), (1024, 1)]
 HEADERS = ["device_mech.h", "kernels.h", "mech_pack.h", os.path.join("..", "..", "include", "pyjac_b200.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC"]
 
 
 def _nvcc() -> str:
@@ -30,21 +35,42 @@ def is_stale() -> bool:
     if not os.path.exists(SO):
         return True
     t = os.path.getmtime(SO)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.abspath(__file__)]
+    deps = [os.path.join(CSRC, f) for f in HOST_SOURCES + ["kernels.cu"] + HEADERS] + [os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return SO
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
-    cmd += os.environ.get("PYJAC_NVCC_FLAGS", "").split()      # e.g. -DPYJAC_PROF (per-phase cycle print)
-    cmd += [os.path.join(CSRC, f) for f in SOURCES] + ["-o", SO]
-    res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+    os.makedirs(OBJ, exist_ok=True)
+    extra = (["-Xptxas", "-v"] if verbose else []) + os.environ.get("PYJAC_NVCC_FLAGS", "").split()
+    jobs = []      # (object, command)
+    for f in HOST_SOURCES:
+        o = os.path.join(OBJ, f[:-3] + ".o")
+        jobs.append((o, [_nvcc()] + NVCC_FLAGS + extra + ["-c", os.path.join(CSRC, f), "-o", o]))
+    for nt, mb in KERNEL_SIZES:
+        o = os.path.join(OBJ, "kernels_%d.o" % nt)
+        jobs.append((o, [_nvcc()] + NVCC_FLAGS + extra + ["-DPYJAC_NT=%d" % nt, "-DPYJAC_MB=%d" % mb, "-c",
+                                                          os.path.join(CSRC, "kernels.cu"), "-o", o]))
+
+    def run(job):
+        return subprocess.run(job[1], cwd=CSRC, capture_output=True, text=True)
+
+    with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+        results = list(ex.map(run, jobs))
+    failed = False
+    for (o, cmd), res in zip(jobs, results):
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        failed = failed or res.returncode != 0
+    if failed:
+        raise RuntimeError("nvcc failed building %s" % SO)
+    link = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + [j[0] for j in jobs] + ["-o", SO]
+    res = subprocess.run(link, cwd=CSRC, capture_output=True, text=True)
     if verbose or res.returncode != 0:
         sys.stderr.write(res.stdout + res.stderr)
     if res.returncode != 0:
-        raise RuntimeError("nvcc failed building %s" % SO)
+        raise RuntimeError("link failed for %s" % SO)
     return SO
 
 

@@ -2,6 +2,7 @@
 #include <cuda_runtime.h>
 
 #include <atomic>
+#include <cstdint>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -44,23 +45,17 @@ struct Uploader {
     }
 };
 
-// Launch shape: S states per CTA iteration and the CTA size, by the shared memory one state needs
-// (several small CTAs per SM overlap each other's phases; large mechanisms get one large CTA).
-// PYJAC_THREADS / PYJAC_S override it (tuning hooks); a pair that is not
-// instantiated or does not fit falls back to the default.
-void choose_shape(const SmemPlan &plan, size_t smem_max, int *threads, int *S)
+// Tuning hooks: PYJAC_S, PYJAC_THREADS, PYJAC_PW, PYJAC_CTAS override the launch shape
+// mech_pack.cu would choose; a value that is not instantiated or does not fit is an error at create.
+ShapeHints hints_from_env(long long smem_optin)
 {
-    auto fits = [&](int s) { return eval_smem_bytes(plan, s) <= smem_max; };
-    const size_t one = eval_smem_bytes(plan, 1);
-    int s = (fits(2) && 2 * one <= smem_max / 2) ? 2 : 1;
-    int nt = one <= 48 * 1024 ? 128 : one <= 110 * 1024 ? 256 : 512;
-    int es = 0, et = 0;
-    if (const char *e = std::getenv("PYJAC_S")) es = std::atoi(e);
-    if (const char *e = std::getenv("PYJAC_THREADS")) et = std::atoi(e);
-    if (es > 0 && fits(es) && eval_kernel_ptr(2, et > 0 ? et : nt, es)) s = es;
-    if (et > 0 && eval_kernel_ptr(2, et, s)) nt = et;
-    *threads = nt;
-    *S = s;
+    ShapeHints h;
+    if (smem_optin > 0) h.smem_bytes = smem_optin - 128;
+    if (const char *e = std::getenv("PYJAC_S")) h.S = std::atoi(e);
+    if (const char *e = std::getenv("PYJAC_THREADS")) h.threads = std::atoi(e);
+    if (const char *e = std::getenv("PYJAC_PW")) h.pw = std::atoi(e);
+    if (const char *e = std::getenv("PYJAC_CTAS")) h.ctas = std::atoi(e);
+    return h;
 }
 
 int check_eval_args(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
@@ -82,7 +77,9 @@ int launch(const pyjac_mech *m, int level, int64_t n, const double *T, const dou
     long long cap = (long long)m->n_sm * m->ctas_per_sm[level];
     const long long blocks = (n + m->S - 1) / m->S;
     int grid = (int)(blocks < cap ? blocks : cap);
-    cudaError_t e = launch_eval(level, m->threads, m->S, m->dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy,
+    DeviceMech dm = m->dm;
+    if (level == 2 && (reinterpret_cast<uintptr_t>(out.jac) & 15) != 0) dm.pair = 0;   // 8-byte stores
+    cudaError_t e = launch_eval(level, m->threads, m->S, dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy,
                                 out, (cudaStream_t)stream);
     if (dev != m->device) cudaSetDevice(dev);
     if (e != cudaSuccess) return PYJAC_ECUDA;
@@ -98,33 +95,42 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
 {
     if (!out) return PYJAC_EINVAL;
     *out = nullptr;
+    // validate and pack first (no CUDA call yet) with the architecture's shared-memory size; the
+    // real device's limit is checked below
     HostPack hp;
     const char *why = nullptr;
-    // validate and pack first (no CUDA call yet), with the architecture's shared-memory size; the
-    // real device's limit is checked below
-    const long long e_doubles = (long long)((size_t)227 * 1024 - 64 - eval_smem_bytes(make_smem_plan(d ? d->n_species : 1, 0), 1)) / 8;
-    int rc = pack_mechanism(d, hp, e_doubles, &why);
+    int rc = pack_mechanism(d, hp, hints_from_env(227 * 1024), &why);
     if (rc != PYJAC_OK) return rc;
-    pyjac_mech *m = new (std::nothrow) pyjac_mech();
-    if (!m) return PYJAC_ENOMEM;
-    m->device = device;
-    m->ns = hp.ns;
-    m->nr = hp.nr;
     int prev = -1;
     cudaDeviceProp prop{};
     if (cudaGetDevice(&prev) != cudaSuccess || cudaSetDevice(device) != cudaSuccess ||
         cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
-        delete m;
+        cudaGetLastError();
         return PYJAC_ECUDA;
     }
+    pyjac_mech *m = new (std::nothrow) pyjac_mech();
+    if (!m) { cudaSetDevice(prev); return PYJAC_ENOMEM; }
+    m->device = device;
+    m->ns = hp.ns;
+    m->nr = hp.nr;
     m->n_sm = prop.multiProcessorCount;
+    m->threads = hp.threads;
+    m->S = hp.S;
     DeviceMech &dm = m->dm;
     dm.ns = hp.ns; dm.nr = hp.nr; dm.ld = hp.ns + 1;
     dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk; dm.n_plain = (int)hp.n_plain_chunks;
-    dm.n_achunk = hp.n_achunk; dm.n_achunk01 = hp.n_achunk01; dm.n_slab = hp.n_slab; dm.m_seg = 8;
-    dm.eQ = hp.eQ; dm.eAr = hp.eAr; dm.eTh = hp.eTh; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;
-    dm.eWdot = hp.eWdot; dm.eTcol = hp.eTcol; dm.eG0 = hp.eG0; dm.eZ = hp.eZ;
+    dm.n_a1 = hp.n_a1; dm.n_a1_01 = hp.n_a1_01;
+    dm.n_panel = hp.n_panel; dm.pw = hp.pw; dm.nbuf = hp.nbuf; dm.eTile = hp.eTile; dm.pair = hp.pair;
+    dm.eQ = hp.eQ; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;
+    dm.eWdot = hp.eWdot; dm.eG0 = hp.eG0; dm.eZ = hp.eZ;
     dm.eS1 = hp.eS1; dm.eA0 = hp.eA0; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.eDump = hp.eDump; dm.n_e = hp.n_e;
+    {   // DENSE work items: about two per warp, 2..32 columns each
+        const int nw = m->threads / 32, n_slab = (dm.ld + (dm.pair ? 63 : 31)) / (dm.pair ? 64 : 32);
+        int seg = (n_slab * dm.pw + 2 * nw - 1) / (2 * nw);
+        seg = seg < 2 ? 2 : seg > 32 ? 32 : seg;
+        if (const char *e = std::getenv("PYJAC_SEG")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) seg = v; }
+        dm.d_seg = seg;
+    }
     Uploader up;
     try {
         up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.mw, hp.mw);
@@ -140,9 +146,8 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         up.add(&dm.fall_par, hp.fall_par);
         up.add(&dm.eff_ptr, hp.eff_ptr); up.add(&dm.eff_spec, hp.eff_spec); up.add(&dm.eff_eps, hp.eff_eps);
         up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
-        up.add((const uint32_t **)&dm.achunk, hp.achunk); up.add(&dm.a_ent, hp.a_ent);
-        up.add(&dm.a_out, hp.a_out); up.add(&dm.a_const, hp.a_const);
-        up.add(&dm.m_hdr, hp.m_hdr); up.add((const uint32_t **)&dm.m_ent, hp.m_ent);
+        up.add((const uint32_t **)&dm.achunk, hp.achunk); up.add((const uint32_t **)&dm.a_ent, hp.a_ent);
+        up.add((const uint32_t **)&dm.a_task, hp.a_task); up.add(&dm.panel_ptr, hp.panel_ptr);
     } catch (...) {
         delete m;
         cudaSetDevice(prev);
@@ -156,19 +161,11 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     }
     if (rc == PYJAC_OK) {
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
-        m->plan = make_smem_plan(hp.ns, hp.n_e);
-        choose_shape(m->plan, (size_t)prop.sharedMemPerBlockOptin - 64, &m->threads, &m->S);
-        {   // MAIN work items: about three per warp, 4..32 columns each
-            const int nw = m->threads / 32, cols = hp.ns + 1;
-            int seg = (hp.n_slab * cols + 3 * nw - 1) / (3 * nw);
-            seg = seg < 4 ? 4 : seg > 32 ? 32 : seg;
-            if (const char *e = std::getenv("PYJAC_SEG")) { const int v = std::atoi(e); if (v >= 1 && v <= 32) seg = v; }
-            dm.m_seg = seg;
-        }
-        m->stats[0] = hp.n_e; m->stats[1] = hp.n_list_entries; m->stats[2] = hp.n_main_entries;
-        m->stats[3] = hp.n_aux_entries; m->stats[4] = (long long)hp.n_slab * (hp.ns + 1); m->stats[5] = hp.n_achunk;
+        m->plan = make_smem_plan(hp.ns, hp.n_e + hp.nbuf * hp.pw * (hp.ns + 1));
+        m->stats[0] = hp.n_e; m->stats[1] = hp.n_cell_entries; m->stats[2] = hp.n_cell_steps;
+        m->stats[3] = hp.n_a1_steps; m->stats[4] = hp.n_cells; m->stats[5] = (long long)hp.achunk.size() / 4;
         const size_t bytes = eval_smem_bytes(m->plan, m->S);
-        if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin) {
+        if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->threads, m->S)) {
             rc = PYJAC_ELIMIT;
         } else {
             for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
@@ -263,12 +260,12 @@ int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
 {
     if (!stats) return PYJAC_EINVAL;
     HostPack hp;
-    const long long e_doubles = (long long)((size_t)227 * 1024 - 64 - eval_smem_bytes(make_smem_plan(d ? d->n_species : 1, 0), 1)) / 8;
-    const int rc = pack_mechanism(d, hp, e_doubles, nullptr);
+    const int rc = pack_mechanism(d, hp, hints_from_env(227 * 1024), nullptr);
     if (rc != PYJAC_OK) return rc;
-    const SmemPlan plan = make_smem_plan(hp.ns, hp.n_e);
-    stats[0] = hp.n_e; stats[1] = hp.n_list_entries; stats[2] = hp.n_main_entries; stats[3] = hp.n_aux_entries;
-    stats[4] = (int64_t)hp.n_slab * (hp.ns + 1); stats[5] = hp.n_achunk; stats[6] = (int64_t)eval_smem_bytes(plan, 1); stats[7] = hp.n_rchunk;
+    const SmemPlan plan = make_smem_plan(hp.ns, hp.n_e + hp.nbuf * hp.pw * (hp.ns + 1));
+    stats[0] = hp.n_e; stats[1] = hp.n_cell_entries; stats[2] = hp.n_cell_steps; stats[3] = hp.n_a1_steps;
+    stats[4] = hp.n_cells; stats[5] = (int64_t)hp.achunk.size() / 4; stats[6] = (int64_t)eval_smem_bytes(plan, hp.S);
+    stats[7] = hp.n_rchunk; stats[8] = hp.S; stats[9] = hp.threads; stats[10] = hp.n_panel; stats[11] = hp.pw;
     return PYJAC_OK;
 }
 

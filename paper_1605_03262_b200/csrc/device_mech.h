@@ -8,13 +8,14 @@
 //
 // The evaluation is a chain of fixed-order gathers over one per-state array `E` in shared memory:
 //   phase 1 writes, per reaction, the reusable products of Section 4.1:
-//           the sparse derivative terms s'_ij (region V), q_i, a_i, Theta_dT,i and the reaction
-//           enthalpy H_i (regions Q, Ar, Th, H);
-//   the AUX gathers sum them into per-species / per-column quantities (wdot_k, alpha_r, gamma_r,
-//           the T column, the column sums of the energy row, the sums of the long cell lists);
-//   a short FIX phase finishes the energy row (Eq. 113) into region Z;
-//   the MAIN pass owns the Jacobian as a flat array: lane <-> one output element, which gathers
-//           its (short) list from E, applies Eq. 112 and stores -- there is no Jacobian tile.
+//           the sparse derivative terms s'_ij (region V), q_i, a_i, Theta_dT,i (region Q,
+//           interleaved per reaction) and the reaction enthalpy H_i (region H);
+//   the A1 gathers sum them into per-species / per-column quantities (wdot_k, alpha_r, gamma_r,
+//           the T column, the column sums of the energy row);
+//   a short FIX step finishes the energy row (Eq. 113);
+//   the CELL gathers sum, for every structurally non-zero Jacobian entry, its list of s'_ij into a
+//           tile (a panel of Jacobian columns) that follows E in shared memory;
+//   the DENSE pass adds the rank-two part of Eq. 112 to the tile and streams it to HBM.
 #pragma once
 #include <cstdint>
 
@@ -35,22 +36,23 @@ __host__ __device__ inline int meta_rev(uint32_t m) { return (m >> 27) & 3; }
 __host__ __device__ inline int meta_form(uint32_t m) { return (m >> 29) & 3; }
 __host__ __device__ inline int meta_single(uint32_t m) { return (m >> 31) & 1; }
 
-// A gather entry: low 16 bits = index into E, high 16 bits = the top 16 bits of the fp64
-// coefficient (exact for the small integers that occur as stoichiometric factors).
-__host__ __device__ inline uint32_t pack_entry(uint32_t src, int coef)
+// A gather entry of the kAuxS1 / kAuxT3 lists: bits 0..18 = byte offset of the source element in
+// the CTA's interleaved E array (E index * S * 8), bits 19..31 = the top 13 bits of the fp64
+// coefficient (exact for +-1, 2, 3, 4, 6, 8; other small integers are split into two entries).
+constexpr uint32_t kEntOffMask = 0x7FFFFu;
+__host__ __device__ inline uint32_t coef_hi13(int coef)
 {
     uint32_t a = coef < 0 ? uint32_t(-coef) : uint32_t(coef);
-    uint32_t hi = a == 1 ? 0x3FF0u : a == 2 ? 0x4000u : a == 3 ? 0x4008u
-                : a == 4 ? 0x4010u : a == 5 ? 0x4014u : a == 6 ? 0x4018u
-                : a == 7 ? 0x401Cu : a == 8 ? 0x4020u : a == 9 ? 0x4022u : 0u;
+    uint32_t hi = a == 1 ? 0x3FF0u : a == 2 ? 0x4000u : a == 3 ? 0x4008u : a == 4 ? 0x4010u
+                : a == 6 ? 0x4018u : a == 8 ? 0x4020u : 0u;
     if (coef < 0) hi |= 0x8000u;
-    return (hi << 16) | (src & 0xFFFFu);
+    return (hi >> 3) << 19;
 }
 
-// kinds of AUX chunks (AuxChunk.z bits 0..7; bits 8..15 = log2 of the lanes that share one sum)
+// kinds of gather chunks (chunk.z bits 0..7; bits 8..15 = log2 of the lanes that share one sum)
 enum : uint32_t {
-    kAuxT3 = 0,    // entries {E index of q_i, nu_ki}: sums of nu q_i, nu a_i, nu Theta_i -> wdot_k, alpha_{k+1}, T column
-    kAuxS1 = 1,    // entries {E index, coef}: one sum, times a task constant -> E slot
+    kAuxT3 = 0,    // entries {q_i of reaction i, nu_ki}: sums of nu q_i, nu a_i, nu Theta_i -> wdot_k, alpha_{k+1}, T column
+    kAuxS1 = 1,    // entries {source, coef}: one sum, times a task constant -> E / tile slot
     kAuxH2 = 2,    // entries {index a | index b << 16}: sum of E[a] * E[b] -> E slot
     kAuxR3 = 3,    // no entries: sums over all reactions of H_i {q_i, a_i, Theta_i} -> S1, A0, S4
 };
@@ -61,9 +63,9 @@ struct DeviceMech {
     // ---- species tables
     const double *inv_mw;       // [ns]
     const double *mw;           // [ns]
-    const double *colc;         // [ns+1][4] column constants by Jacobian column c: {d_j, 1/W_j, 1, 0}, j = c - 1;
-                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51); the third
-                                //        entry switches gamma_r on; c = 0: {0, 1, 0, 0}; c = ns (zero column): zeros
+    const double *colc;         // [ns+1][2] column constants by Jacobian column c: {d_j, g_c}, j = c - 1;
+                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51); g_c = 1 where
+                                //        gamma_r applies (1 <= c < ns), else 0; c = 0 and c = ns: zeros
     const double *wrow;         // [ns+1] row factors by Jacobian row r: {1, W_0 .. W_{ns-1}}
     const double *nasa;         // [2][5][ns] a_0..a_4, range-major, coefficient-major (coalesced over k)
     const double *t_mid;        // [ns]
@@ -95,29 +97,31 @@ struct DeviceMech {
     const int32_t *pk_ptr;      // [n_pk+1] offsets into pk_data
     const double *pk_data;      // PLOG: n, then n x {p, ln p, ln A, beta, Ta};
                                 // Chebyshev: nT, nP, 1/Tmin, 1/Tmax, log10 pmin, log10 pmax, eta[nT*nP]
-    // ---- AUX gathers: chunks of 32 lanes, 32 >> rshift sums each, sorted by length at create time
-    int n_achunk;               // all chunks (Jacobian); the first n_achunk01 serve rates / dydt too
-    int n_achunk01;
-    const uint4 *achunk;        // {first entry, steps, kind | rshift << 8, first task}
-    const uint32_t *a_ent;      // entries at [first + step*32 + lane]
-    const uint32_t *a_out;      // [task] E slot of the result (kAuxT3: the species k)
-    const double *a_const;      // [task] constant factor (kAuxS1)
-    // ---- MAIN pass: the Jacobian in slabs of 32 rows, walked column by column
-    int n_slab;
-    int m_seg;                  // columns per work item (<= 32), chosen with the launch shape
-    const uint32_t *m_hdr;      // [n_slab][ns+1] (entry block << 3) | steps, steps <= 4
-    const uint4 *m_ent;         // blocks of 32 lanes x 4 entries: lane l of block b at [b*32 + l]
+    // ---- gathers: chunks of 32 lanes, 32 >> rshift sums each, sorted by length at create time.
+    // Chunks [0, n_a1) are the A1 phase (the first n_a1_01 of them serve rates / dydt too); the
+    // chunks of the cells of column panel p are [panel_ptr[p], panel_ptr[p+1]).
+    int n_a1, n_a1_01;
+    const uint4 *achunk;        // {first entry block, steps, kind | rshift << 8, first task}
+    const uint4 *a_ent;         // step t of lane l of a chunk: word (t & 3) of a_ent[first + (t >> 2) * 32 + l]
+    const uint4 *a_task;        // [task] {output E index (kAuxT3: species k; ~0 = none), 0, constant factor (fp64 bits)}
+    const int32_t *panel_ptr;   // [n_panel + 1]
+    // ---- the tile: column panels of the Jacobian, state-interleaved like E, element (r, c) of
+    // panel p at E index eTile + (p % nbuf) * pw * ld + (c - p * pw) * ld + r
+    int n_panel, pw, nbuf;
+    int eTile;
+    int pair;                   // 1: ld is even, the DENSE pass owns two rows per lane (16-byte stores)
+    int d_seg;                  // columns per DENSE work item
     // ---- regions of E (indices in doubles per state)
-    int eQ, eAr, eTh, eH;       // [nr] each, consecutive (eAr = eQ + nr, eTh = eQ + 2 nr, eH = eQ + 3 nr)
+    int eQ;                     // [nr][3] {q_i, a_i + W q_i, Theta_dT,i}
+    int eH;                     // [nr] reaction enthalpy H_i
     int eAlpha, eGamma;         // [ns+1] by Jacobian row; row 0 stays 0
     int eWdot;                  // [ns]
-    int eTcol;                  // [ns]   (1/rho) sum_i nu_ki Theta_i
     int eG0;                    // [ns]   sum_i H_i s'_ij per column species j
-    int eZ;                     // [ns+1] finished energy row: Z_c = J(0,c) W_j (c >= 1), Z_0 = J(0,0)
+    int eZ;                     // [ns+1] finished energy row J(0, c)
     int eS1, eA0, eS4;          // scalars: sum_i H_i q_i, sum_i H_i a_i, sum_i H_i Theta_i
     int eZero;                  // a slot that stays 0 (padding of the lists)
     int eDump;                  // a slot nobody reads (stores of empty reaction slots)
-    int n_e;                    // size of E
+    int n_e;                    // size of E without the tile
 };
 
 // per-state scalars (region Scal of the shared-memory plan)
@@ -130,14 +134,14 @@ enum {
 // (X, Cp, Scal) exists twice: the block of the next batch is filled while this one is in use.  After
 // the S interleaved state blocks come the state-independent tables (colc, wrow), loaded once per CTA.
 struct SmemPlan {
-    int E;                              // [n_e]
+    int E;                              // [n_e + tile]
     int P0;                             // two mixture blocks of p0size doubles
     int p0size;
     int oX;                             // within a mixture block: [ns+1] concentrations; slot ns = 1 (empty reaction slots)
     int oCp;                            // [ns] c_pk (mass based)
     int oScal;                          // [kNScal]
     int total;                          // doubles per state
-    int colc;                           // [ld][4], offset in doubles from the end of the state blocks
+    int colc;                           // [ld][2], offset in doubles from the end of the state blocks
     int wrow;                           // [ld]
     int shared_total;                   // doubles of the state-independent part
 };
@@ -159,7 +163,7 @@ inline SmemPlan make_smem_plan(int ns, int n_e)
     }
     p.total = o;
     o = 0;
-    p.colc = take(4 * (ns + 1));
+    p.colc = take(2 * (ns + 1));
     p.wrow = take(ns + 1);
     p.shared_total = o;
     return p;

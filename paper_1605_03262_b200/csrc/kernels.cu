@@ -3,27 +3,25 @@
 // One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop; the S
 // states are interleaved in shared memory (element i of a region for state q at (R + i) * S + q), so
 // whatever does not depend on the state -- decoding a reaction, a gather entry, a column constant --
-// is done once and applied to the S states with one vector load.  All work is assigned to the warps
-// statically (item i of a phase goes to warp i mod NW; the items were sorted by cost at create
-// time).  Per iteration:
+// is done once and applied to the S states with one vector load.  Per iteration:
 //   P0    mixture (Eqs. 3-5) and species, warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT
-//         (Eqs. 9-13, 54-55)
+//         (Eqs. 9-13, 54-55); computed one batch ahead, as an item of P1
 //   P1    reactions, lane <-> reaction, groups of 32: k_f, k_r (K_c from the per-reaction polynomial
 //         of device_mech.h `th_data`), R_f, R_r, c_i and the reusable per-reaction products of
 //         Section 4.1 into E: q_i, Theta_dT,i, a_i (the coefficient of d_j), the
 //         sparse terms s'_ij, the enthalpy H_i.  Groups made only of plain elementary reactions take
 //         a branch-free path that evaluates two states at a time.
-//   AUX   fixed-order gathers over E: wdot_k (Eq. 14), alpha_r, gamma_r of Eq. 112, the T column
-//         (Eq. 111), the column sums of the energy row (Eq. 113), the sums of long cell lists.
-//         2^rshift neighbouring lanes share one sum (butterfly at the end).
-//   FIX   the energy row, Eq. 113, per column into region Z
-//   MAIN  the Jacobian as a flat column-major array: lane <-> output element.  Each element
-//         gathers its short list from E and is stored straight from the register:
-//           J(r, c) = alpha_r d_j + (W_k / W_j) sum_i nu_ki s'_ij - gamma_r        (r = k+1, c = j+1)
-//         which is Eq. 112 with the per-reaction terms of Eqs. 118-127 regrouped by what they
-//         multiply.  Row 0 and column 0 are lists of one finished entry
-//         (Z_c, the T column), so the pass has no special cases.  A warp stores 256 contiguous bytes.
-// There are no atomics and no Jacobian tile: every sum has an order fixed at pyjac_mech_create.
+//   A1    fixed-order gathers over E, lane <-> sum: wdot_k (Eq. 14), alpha_r, gamma_r of Eq. 112, the
+//         T column (Eq. 111), the column sums of the energy row (Eq. 113).
+//   FIX   the energy row, Eq. 113
+//   CELLS lane <-> structurally non-zero Jacobian entry (sorted by list length, so the 32 lanes of a
+//         chunk walk lists of equal length): sum_i nu_ki s'_ij times W_k / W_j into the tile
+//   DENSE lane <-> two rows, walking columns:  J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c,
+//         which is Eq. 112 with the per-reaction terms of Eqs. 118-127 regrouped by what they multiply
+//         (DESIGN.md "Regrouping"); a warp stores 512 contiguous bytes per state and column.
+// Mechanisms whose tile does not fit are walked in column panels (two tile buffers: the cells of
+// panel p are gathered while panel p - 1 streams out).  There are no atomics on data: every sum
+// has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -45,7 +43,7 @@ namespace {
 constexpr double kLn10 = 2.302585092994045684;
 constexpr double kInvLn10 = 0.434294481903251828;
 
-__device__ __forceinline__ double entry_coef(uint32_t e) { return __hiloint2double((int)(e & 0xFFFF0000u), 0); }
+__device__ __forceinline__ double entry_coef(uint32_t e) { return __hiloint2double((int)(e & ~kEntOffMask), 0); }
 
 // exp(x) for the rate coefficients: Cody-Waite reduction by ln 2, degree-13 Taylor polynomial on
 // |r| <= ln2/2 (truncation 4e-18), scaling by 2^n in two steps so that results underflow to 0
@@ -99,16 +97,16 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
-// the S interleaved values of one element: one vector load / store
+// the S interleaved values of one element: 16-byte vector loads / stores
 template <int S>
 __device__ __forceinline__ void ldv(const double *p, double (&v)[S])
 {
-    if (S == 2) {
-        const double2 t = *reinterpret_cast<const double2 *>(p);
-        v[0] = t.x; v[1] = t.y;
-    } else if (S == 4) {
-        const double2 t = *reinterpret_cast<const double2 *>(p), u = *reinterpret_cast<const double2 *>(p + 2);
-        v[0] = t.x; v[1] = t.y; v[2] = u.x; v[3] = u.y;
+    if (S % 2 == 0) {
+#pragma unroll
+        for (int q = 0; q < S; q += 2) {
+            const double2 t = *reinterpret_cast<const double2 *>(p + q);
+            v[q] = t.x; v[q + 1 < S ? q + 1 : q] = t.y;
+        }
     } else {
 #pragma unroll
         for (int q = 0; q < S; ++q) v[q] = p[q];
@@ -117,11 +115,9 @@ __device__ __forceinline__ void ldv(const double *p, double (&v)[S])
 template <int S>
 __device__ __forceinline__ void stv(double *p, const double (&v)[S])
 {
-    if (S == 2) {
-        *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]);
-    } else if (S == 4) {
-        *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]);
-        *reinterpret_cast<double2 *>(p + 2) = make_double2(v[2], v[3]);
+    if (S % 2 == 0) {
+#pragma unroll
+        for (int q = 0; q < S; q += 2) *reinterpret_cast<double2 *>(p + q) = make_double2(v[q], v[q + 1 < S ? q + 1 : q]);
     } else {
 #pragma unroll
         for (int q = 0; q < S; ++q) p[q] = v[q];
@@ -185,7 +181,7 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
             const double p01 = c0 * c1, p34 = c3 * c4;
             const double Rf = kf[u] * (p01 * c2), Rr = kr[u] * (p34 * c5);       // Eqs. 18-19
             const double R = Rf - Rr;
-            E[(m.eQ + s) * S + q] = R;
+            E[(m.eQ + 3 * s) * S + q] = R;
             if (LEVEL >= 1) E[(m.eH + s) * S + q] = kRu * T[u] * fma(T[u], sdB[u], dnu);
             if (LEVEL == 0) {
                 const long long st = state0 + q;
@@ -202,8 +198,8 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
                 // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
                 const double dRf = Rf * fma(-snf, iT, L[u]);
                 const double dRr = Rr * (fma(-snr, iT, L[u]) - sdB[u]);
-                E[(m.eTh + s) * S + q] = fma(R, iT, dRf - dRr);
-                E[(m.eAr + s) * S + q] = W * (R - fma(Rf, snf, -Rr * snr));
+                E[(m.eQ + 3 * s + 2) * S + q] = fma(R, iT, dRf - dRr);
+                E[(m.eQ + 3 * s + 1) * S + q] = W * (R - fma(Rf, snf, -Rr * snr));
                 const double nkr = -kr[u];
                 E[v0 + q] = kf[u] * (c1 * c2); E[v1 + q] = kf[u] * (c0 * c2); E[v2 + q] = kf[u] * p01;   // Eq. 120
                 E[v3 + q] = nkr * (c4 * c5); E[v4 + q] = nkr * (c3 * c5); E[v5 + q] = nkr * p34;         // Eq. 121
@@ -402,7 +398,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             }
         }
         const double qi = c * R;
-        E[(m.eQ + s) * S + q] = qi;
+        E[(m.eQ + 3 * s) * S + q] = qi;
         if (LEVEL >= 1) E[(m.eH + s) * S + q] = H;
         if (LEVEL == 0) {
             const long long st = state0 + q;
@@ -418,13 +414,13 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             const double dcdT = pdep ? G * lPrT + c * fT : 0.0;
             const double dRfdT = Rf * (L - (double)snu_f * invT);                 // Eq. 66
             const double dRrdT = Rr * (Lr - (double)snu_r * invT);                // Eqs. 69, 75
-            E[(m.eTh + s) * S + q] = dcdT * R + c * (dRfdT - dRrdT + R * invT);
+            E[(m.eQ + 3 * s + 2) * S + q] = dcdT * R + c * (dRfdT - dRrdT + R * invT);
             // coefficient of d_j (Eqs. 119, 123, 127 regrouped), plus W q_i: the omega_k W d_j term of
             // Eq. 112 summed per reaction
             const double W = sc[kW * S + q];
             const double base = -W * (Rf * (double)snu_f - Rr * (double)snu_r);
             const double mix = (pdep && !meta_single(meta)) ? sc[kRho * S + q] : 0.0;
-            E[(m.eAr + s) * S + q] = c * base + b * (mix - W * Xi) + W * qi;
+            E[(m.eQ + 3 * s + 1) * S + q] = c * base + b * (mix - W * Xi) + W * qi;
             // sparse terms s'_ij = c (k_f S'_j - k_r S''_j) per slot, b (alpha_ij - 1) per efficiency
             const double ckf = c * kf, ckr = -c * kr;
             E[v0 + q] = ckf * sk0; E[v1 + q] = ckf * sk1; E[v2 + q] = ckf * sk2;
@@ -480,10 +476,170 @@ __device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double 
     }
 }
 
+// ---- one gather chunk: 32 lanes, 32 >> rshift sums (device_mech.h) ---------------------------------
+template <int LEVEL, int S>
+__device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, const double *sc, const uint4 ch, int lane)
+{
+    const uint32_t kind = ch.z & 0xFF;
+    const int rshift = (ch.z >> 8) & 0xFF, width = 1 << rshift;
+    const int steps = (int)ch.y;
+    const uint4 *ep = m.a_ent + ch.x + lane;
+    const uint4 task = m.a_task[ch.w + (lane >> rshift)];
+    const bool head = (lane & (width - 1)) == 0 && task.x != 0xFFFFFFFFu;
+    const char *Eb = reinterpret_cast<const char *>(E);
+    const uint4 ez = make_uint4(0u, 0u, 0u, 0u);
+    const int nr = m.nr;
+
+    if (kind == kAuxS1) {
+        if (LEVEL == 2) {
+            double acc[S];
+#pragma unroll
+            for (int q = 0; q < S; ++q) acc[q] = 0.0;
+            auto step = [&](uint32_t e) {
+                const double cf = entry_coef(e);
+                double a[S];
+                ldv<S>(reinterpret_cast<const double *>(Eb + (e & kEntOffMask)), a);
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
+            };
+            uint4 e = steps > 0 ? ep[0] : ez;
+            int t = 0;
+            for (; t + 4 < steps; t += 4) {
+                const uint4 en = ep[(t / 4 + 1) * 32];
+                step(e.x); step(e.y); step(e.z); step(e.w);
+                e = en;
+            }
+            const int rem = steps - t;
+            if (rem > 0) step(e.x);
+            if (rem > 1) step(e.y);
+            if (rem > 2) step(e.z);
+            if (rem > 3) step(e.w);
+            for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
+            if (head) {
+                const double cst = __hiloint2double((int)task.w, (int)task.z);
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[q] *= cst;
+                stv<S>(E + (size_t)task.x * S, acc);
+            }
+        }
+    } else if (kind == kAuxH2) {
+        if (LEVEL == 2) {
+            double acc[S];
+#pragma unroll
+            for (int q = 0; q < S; ++q) acc[q] = 0.0;
+            auto step = [&](uint32_t e) {
+                double a[S], b[S];
+                ldv<S>(E + (e & 0xFFFF) * S, a);
+                ldv<S>(E + (e >> 16) * S, b);
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
+            };
+            for (int t = 0; t < steps; t += 4) {
+                const uint4 e = ep[(t / 4) * 32];
+                step(e.x); step(e.y); step(e.z); step(e.w);      // padded with the zero slot
+            }
+            for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
+            if (head) stv<S>(E + (size_t)task.x * S, acc);
+        }
+    } else {
+        // kAuxT3 / kAuxR3: three sums at once (one for the rates / source-term kernels)
+        constexpr int NA = LEVEL == 2 ? 3 : 1;
+        double acc[NA][S];
+#pragma unroll
+        for (int w = 0; w < NA; ++w)
+#pragma unroll
+            for (int q = 0; q < S; ++q) acc[w][q] = 0.0;
+        if (kind == kAuxT3) {
+            auto step = [&](uint32_t e) {
+                const double cf = entry_coef(e);
+                const double *p = reinterpret_cast<const double *>(Eb + (e & kEntOffMask));
+#pragma unroll
+                for (int w = 0; w < NA; ++w) {
+                    double a[S];
+                    ldv<S>(p + w * S, a);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[w][q] = fma(cf, a[q], acc[w][q]);
+                }
+            };
+            for (int t = 0; t < steps; t += 4) {
+                const uint4 e = ep[(t / 4) * 32];
+                step(e.x); step(e.y); step(e.z); step(e.w);      // padded with the zero slots
+            }
+        } else {
+            for (int i = lane; i < nr; i += 32) {
+                double h[S];
+                ldv<S>(E + (m.eH + i) * S, h);
+#pragma unroll
+                for (int w = 0; w < NA; ++w) {
+                    double a[S];
+                    ldv<S>(E + (m.eQ + 3 * i + w) * S, a);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[w][q] = fma(h[q], a[q], acc[w][q]);
+                }
+            }
+        }
+        for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+            for (int w = 0; w < NA; ++w)
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[w][q], o);
+        constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
+        if (kind == kAuxR3) {
+            if ((lane & (width - 1)) == 0) {
+                stv<S>(E + m.eS1 * S, acc[0]);
+                if (LEVEL == 2) { stv<S>(E + m.eA0 * S, acc[iA]); stv<S>(E + m.eS4 * S, acc[iT]); }
+            }
+        } else if (head) {
+            const uint32_t k = task.x;
+            stv<S>(E + (m.eWdot + k) * S, acc[0]);
+            if (LEVEL == 2) {
+                // alpha_{k+1} of Eq. 112 regrouped, and the T column (Eq. 111) straight into the tile
+                const double wk = m.mw[k];
+                double al[S], tc[S];
+#pragma unroll
+                for (int q = 0; q < S; ++q) {
+                    const double wi = wk * sc[kIrho * S + q];
+                    al[q] = wi * acc[iA][q];
+                    tc[q] = wi * acc[iT][q];
+                }
+                stv<S>(E + (m.eAlpha + k + 1) * S, al);
+                stv<S>(E + (m.eTile + k + 1) * S, tc);
+            }
+        }
+    }
+}
+
+// the chunks [c0, c1) of a phase, round-robin over the warps; the next header is fetched early
+template <int LEVEL, int S, int NW>
+__device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, const double *sc, int c0, int c1, int warp,
+                                             int lane)
+{
+    int ch = c0 + warp;
+    if (ch >= c1) return;
+    uint4 h = m.achunk[ch];
+    for (; ch < c1; ch += NW) {
+        const uint4 hn = ch + NW < c1 ? m.achunk[ch + NW] : h;
+        gather_chunk<LEVEL, S>(m, E, sc, h, lane);
+        h = hn;
+    }
+}
+
+// 16-byte streaming store of two consecutive Jacobian rows
+__device__ __forceinline__ void st_cs_v2(double *p, double a, double b)
+{
+    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a), "d"(b) : "memory");
+}
+
 // ---- the kernel ------------------------------------------------------------------------------------
-// Shared memory: S interleaved state blocks of sp.total doubles, then the state-independent column
-// and row constants.  The mixture block (X, Cp, scalars) is double-buffered: P0 of the NEXT batch is
-// an item of this batch's P1 queue.
+// Shared memory: S interleaved state blocks of sp.total doubles (E with the tile behind it, two
+// mixture blocks), then the state-independent column and row constants.  The mixture block (X, Cp,
+// scalars) is double-buffered: P0 of the NEXT batch is an item of this batch's P1 queue.  The last
+// DENSE step of a batch is not followed by a barrier: P1 of the next batch only writes regions of E
+// that DENSE does not read, so the warps that finish early start it at once.
 template <int LEVEL, int NT, int S, int MB>
 __global__ void __launch_bounds__(NT, MB)
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
@@ -500,13 +656,17 @@ __global__ void __launch_bounds__(NT, MB)
     double *wrow = sm + (size_t)sp.total * S + sp.wrow;
     {
         double *cw = sm + (size_t)sp.total * S + sp.colc;
-        for (int i = tid; i < 4 * ld; i += NT) cw[i] = m.colc[i];
+        for (int i = tid; i < 2 * ld; i += NT) cw[i] = m.colc[i];
         for (int i = tid; i < ld; i += NT) wrow[i] = m.wrow[i];
+        if (LEVEL == 2)      // the tile: cells without a list stay zero
+            for (int i = tid; i < m.nbuf * m.pw * ld * S; i += NT) E[(size_t)m.eTile * S + i] = 0.0;
     }
-    if (tid < S) {   // the empty-slot dummy species, the zero slot, row 0 of alpha / gamma
+    if (tid < S) {   // the empty-slot dummy species, the zero slots, row 0 of alpha / gamma
         sm[(sp.P0 + sp.oX + ns) * S + tid] = 1.0;
         sm[(sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
         E[m.eZero * S + tid] = 0.0;
+        E[(m.eZero + 1) * S + tid] = 0.0;
+        E[(m.eZero + 2) * S + tid] = 0.0;
         E[m.eAlpha * S + tid] = 0.0;
         E[m.eGamma * S + tid] = 0.0;
         if (nr == 0) { E[m.eS1 * S + tid] = 0.0; E[m.eA0 * S + tid] = 0.0; E[m.eS4 * S + tid] = 0.0; }
@@ -523,6 +683,7 @@ __global__ void __launch_bounds__(NT, MB)
         mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oScal * S, warp,
                                       min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
     }
+    __syncthreads();
     int par = 0;
     for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x, par ^= 1) {
         const long long state0 = blk * S;
@@ -532,8 +693,6 @@ __global__ void __launch_bounds__(NT, MB)
         long long prof_t[12];
 #endif
         PROF_MARK(0);
-        __syncthreads();      // every warp has left the previous MAIN pass (and the first P0 is done)
-        PROF_MARK(1);
         // ---- P1: reactions (+ the mixture of the next batch)
         for (int it = grab(&ctr[0], lane); it < n_p1; it = grab(&ctr[0], lane)) {
             if (it < i_p0) {
@@ -550,144 +709,15 @@ __global__ void __launch_bounds__(NT, MB)
                 plain_reactions<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q0, out, state0, n);
             }
         }
-        PROF_MARK(2);
+        PROF_MARK(1);
         __syncthreads();
         if (tid == 0) ctr[0] = 0;
+        PROF_MARK(2);
+        // ---- A1: sums over the reactions per species / per column
+        gather_phase<LEVEL, S, NW>(m, E, sc, 0, LEVEL == 2 ? m.n_a1 : m.n_a1_01, warp, lane);
         PROF_MARK(3);
-        // ---- AUX gathers: chunk i of the list goes to warp i mod NW; the entries of a warp's next
-        // chunk are fetched before the current one is summed
-        {
-            const int nch = LEVEL == 2 ? m.n_achunk : m.n_achunk01;
-            const uint4 hz = make_uint4(0u, 0u, 0u, 0u);
-            int t0 = warp;
-            uint4 h0 = t0 < nch ? m.achunk[t0] : hz, h1 = t0 + NW < nch ? m.achunk[t0 + NW] : hz;
-            const uint4 *ap = reinterpret_cast<const uint4 *>(m.a_ent);
-            uint4 ea = hz, eb = hz;
-            if (h0.y > 0 && (h0.z & 0xFF) != kAuxR3) { ea = ap[h0.x / 4 + lane * 2]; if (h0.y > 4) eb = ap[h0.x / 4 + lane * 2 + 1]; }
-            for (; t0 < nch; t0 += NW) {
-                const uint4 h2 = t0 + 2 * NW < nch ? m.achunk[t0 + 2 * NW] : hz;
-                uint4 na = hz, nb = hz;
-                if (h1.y > 0 && (h1.z & 0xFF) != kAuxR3) { na = ap[h1.x / 4 + lane * 2]; if (h1.y > 4) nb = ap[h1.x / 4 + lane * 2 + 1]; }
-                // ---- chunk t0
-                const uint4 ch = h0;
-                const uint32_t kind = ch.z & 0xFF;
-                const int rshift = (ch.z >> 8) & 0xFF, width = 1 << rshift;
-                const bool head = (lane & (width - 1)) == 0;
-                const uint32_t task = ch.w + (lane >> rshift);
-                const uint32_t e0[8] = {ea.x, ea.y, ea.z, ea.w, eb.x, eb.y, eb.z, eb.w};
-                if (kind == kAuxT3 || kind == kAuxR3) {
-                    constexpr int NA = LEVEL == 2 ? 3 : 1;
-                    constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
-                    double acc[NA][S];
-#pragma unroll
-                    for (int w = 0; w < NA; ++w)
-#pragma unroll
-                        for (int q = 0; q < S; ++q) acc[w][q] = 0.0;
-                    if (kind == kAuxT3) {
-                        auto step = [&](uint32_t e) {
-                            const double cf = entry_coef(e);
-                            const double *p = E + (e & 0xFFFF) * S;
-#pragma unroll
-                            for (int w = 0; w < NA; ++w) {
-                                double a[S];
-                                ldv<S>(p + (size_t)w * nr * S, a);
-#pragma unroll
-                                for (int q = 0; q < S; ++q) acc[w][q] = fma(cf, a[q], acc[w][q]);
-                            }
-                        };
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            if ((uint32_t)j < ch.y) step(e0[j]);
-                        for (uint32_t t = 8; t < ch.y; ++t) step(m.a_ent[ch.x + (t >> 3) * 256 + lane * 8 + (t & 7)]);
-                    } else {
-                        for (int i = lane; i < nr; i += 32) {
-                            double h[S];
-                            ldv<S>(E + (m.eH + i) * S, h);
-#pragma unroll
-                            for (int w = 0; w < NA; ++w) {
-                                double a[S];
-                                ldv<S>(E + (m.eQ + w * nr + i) * S, a);
-#pragma unroll
-                                for (int q = 0; q < S; ++q) acc[w][q] = fma(h[q], a[q], acc[w][q]);
-                            }
-                        }
-                    }
-                    for (int o = 1; o < width; o <<= 1)
-#pragma unroll
-                        for (int w = 0; w < NA; ++w)
-#pragma unroll
-                            for (int q = 0; q < S; ++q) acc[w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[w][q], o);
-                    if (head) {
-                        if (kind == kAuxR3) {
-                            stv<S>(E + m.eS1 * S, acc[0]);
-                            if (LEVEL == 2) { stv<S>(E + m.eA0 * S, acc[iA]); stv<S>(E + m.eS4 * S, acc[iT]); }
-                        } else {
-                            const uint32_t k = m.a_out[task];
-                            if (k != 0xFFFFFFFFu) {
-                                stv<S>(E + (m.eWdot + k) * S, acc[0]);
-                                if (LEVEL == 2) {
-                                    const double wk = m.mw[k];
-                                    double al[S], tc[S];
-#pragma unroll
-                                    for (int q = 0; q < S; ++q) {
-                                        const double ir = sc[kIrho * S + q];
-                                        al[q] = wk * ir * acc[iA][q];
-                                        tc[q] = ir * acc[iT][q];
-                                    }
-                                    stv<S>(E + (m.eAlpha + k + 1) * S, al);
-                                    stv<S>(E + (m.eTcol + k) * S, tc);
-                                }
-                            }
-                        }
-                    }
-                } else if (LEVEL == 2) {
-                    double acc[S];
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[q] = 0.0;
-                    if (kind == kAuxH2) {
-                        auto step = [&](uint32_t e) {
-                            double a[S], b[S];
-                            ldv<S>(E + (e & 0xFFFF) * S, a);
-                            ldv<S>(E + (e >> 16) * S, b);
-#pragma unroll
-                            for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
-                        };
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            if ((uint32_t)j < ch.y) step(e0[j]);
-                        for (uint32_t t = 8; t < ch.y; ++t) step(m.a_ent[ch.x + (t >> 3) * 256 + lane * 8 + (t & 7)]);
-                    } else {
-                        auto step = [&](uint32_t e) {
-                            const double cf = entry_coef(e);
-                            double a[S];
-                            ldv<S>(E + (e & 0xFFFF) * S, a);
-#pragma unroll
-                            for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
-                        };
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            if ((uint32_t)j < ch.y) step(e0[j]);
-                        for (uint32_t t = 8; t < ch.y; ++t) step(m.a_ent[ch.x + (t >> 3) * 256 + lane * 8 + (t & 7)]);
-                    }
-                    for (int o = 1; o < width; o <<= 1)
-#pragma unroll
-                        for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
-                    const uint32_t slot = m.a_out[task];
-                    if (head && slot != 0xFFFFFFFFu) {
-                        if (kind == kAuxS1) {
-                            const double cst = m.a_const[task];
-#pragma unroll
-                            for (int q = 0; q < S; ++q) acc[q] *= cst;
-                        }
-                        stv<S>(E + slot * S, acc);
-                    }
-                }
-                h0 = h1; h1 = h2; ea = na; eb = nb;
-            }
-        }
-        PROF_MARK(4);
         __syncthreads();
-        PROF_MARK(5);
+        PROF_MARK(4);
         // ---- outputs of the rates / source-term kernels (Eqs. 7-8, 14)
         if (LEVEL == 0 && out.wdot) {
             for (int k = tid; k < ns; k += NT)
@@ -706,116 +736,137 @@ __global__ void __launch_bounds__(NT, MB)
                     out.dydt[(state0 + q) * ld + r] = v;
                 }
         }
-        if (LEVEL == 2) {
-            // ---- FIX: the energy row (Eq. 113).  Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 ..
-            const int nfix = 1 + (ns - 1 + 31) / 32;
-            for (int it = warp; it < nfix; it += NW) {
-                if (it == 0) {
-                    double s3[S];       // sum_k c_pk W_k wdot_k
+        if (LEVEL != 2) {
+            __syncthreads();      // the outputs above read E and the scalars
+            continue;
+        }
+        // ---- Jacobian: step p gathers the cells of panel p into its tile buffer (step 0 also
+        // finishes the energy row) and streams panel p - 1 out
+        const long long Jstate = (long long)ld * ld;
+        const int pw = m.pw, n_panel = m.n_panel;
+        for (int p = 0; p <= n_panel; ++p) {
+            if (p == 0) {
+                // FIX: the energy row (Eq. 113).  Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 ..
+                const int nfix = 1 + (ns - 1 + 31) / 32;
+                for (int it = NW - 1 - warp; it < nfix; it += NW) {
+                    if (it == 0) {
+                        double s3[S];       // sum_k c_pk W_k wdot_k
 #pragma unroll
-                    for (int q = 0; q < S; ++q) s3[q] = 0.0;
-                    for (int k = lane; k < ns; k += 32) {
-                        const double wk = wrow[k + 1];
-                        double cp[S], wd[S];
-                        ldv<S>(Cp + k * S, cp);
-                        ldv<S>(E + (m.eWdot + k) * S, wd);
+                        for (int q = 0; q < S; ++q) s3[q] = 0.0;
+                        for (int k = lane; k < ns; k += 32) {
+                            const double wk = wrow[k + 1];
+                            double cp[S], wd[S];
+                            ldv<S>(Cp + k * S, cp);
+                            ldv<S>(E + (m.eWdot + k) * S, wd);
 #pragma unroll
-                        for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
-                    }
+                            for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
+                        }
 #pragma unroll
-                    for (int o = 16; o > 0; o >>= 1)
+                        for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
-                        for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
-                    if (lane < S) {
-                        const int q = lane;
-                        double s = s3[0];
+                            for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
+                        if (lane < S) {
+                            const int q = lane;
+                            double s = s3[0];
 #pragma unroll
-                        for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
-                        const double icp = 1.0 / sc[kCpMix * S + q];
-                        E[m.eZ * S + q] = -icp * sc[kIrho * S + q] *
-                                          (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
-                    }
-                } else {
-                    const int c = (it - 1) * 32 + lane + 1;
-                    if (c < ns) {
-                        const double dx = colc[4 * c];
-                        const double wj = wrow[c], iwl = m.inv_mw[ns - 1];
+                            for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
+                            const double icp = 1.0 / sc[kCpMix * S + q];
+                            const double z = -icp * sc[kIrho * S + q] *
+                                             (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
+                            E[m.eZ * S + q] = z;
+                            E[m.eTile * S + q] = z;
+                        }
+                    } else {
+                        const int c = (it - 1) * 32 + lane + 1;
+                        if (c < ns) {
+                            const double dx = colc[2 * c];
+                            const double wj = wrow[c], iwj = m.inv_mw[c - 1], iwl = m.inv_mw[ns - 1];
 #pragma unroll
-                        for (int q = 0; q < S; ++q) {
-                            const double icp = 1.0 / sc[kCpMix * S + q], irho = sc[kIrho * S + q];
-                            const double a1 = irho * E[m.eS1 * S + q] * icp * icp;     // coefficient of c_pj - c_pNs
-                            const double alpha0 = -(irho * icp) * E[m.eA0 * S + q];
-                            const double gamma0 = -(iwl * icp) * E[(m.eG0 + ns - 1) * S + q];
-                            const double dcp = Cp[(c - 1) * S + q] - Cp[(ns - 1) * S + q];
-                            E[(m.eZ + c) * S + q] =
-                                wj * (alpha0 * dx - gamma0 + a1 * dcp) - icp * E[(m.eG0 + c - 1) * S + q];
+                            for (int q = 0; q < S; ++q) {
+                                const double icp = 1.0 / sc[kCpMix * S + q], irho = sc[kIrho * S + q];
+                                const double a1 = irho * E[m.eS1 * S + q] * icp * icp;     // coefficient of c_pj - c_pNs
+                                const double alpha0 = -(irho * icp) * E[m.eA0 * S + q];
+                                const double gamma0 = -(iwl * icp) * E[(m.eG0 + ns - 1) * S + q];
+                                const double dcp = Cp[(c - 1) * S + q] - Cp[(ns - 1) * S + q];
+                                const double z =
+                                    (wj * (alpha0 * dx - gamma0 + a1 * dcp) - icp * E[(m.eG0 + c - 1) * S + q]) * iwj;
+                                E[(m.eZ + c) * S + q] = z;
+                                if (c < pw) E[(m.eTile + c * ld) * S + q] = z;
+                            }
                         }
                     }
                 }
             }
-            PROF_MARK(6);
-            __syncthreads();
-            PROF_MARK(7);
-            // ---- MAIN pass: warp <-> (slab of 32 rows, segment of columns); lane <-> row.  alpha_r,
-            // gamma_r, W_r stay in registers; per column: one 16-byte load of the lane's entries (the
-            // next column's is in flight), gather, Eq. 112, store (32 consecutive rows = 256 bytes).
-            const long long Jstate = (long long)ld * ld;
-            const int seg = m.m_seg, nseg = (ld + seg - 1) / seg;
-            const int n_items = m.n_slab * nseg;
-            const uint4 ez = make_uint4(0u, 0u, 0u, 0u);
-            for (int it = warp; it < n_items; it += NW) {
-                const int slab = it % m.n_slab, sg = it / m.n_slab;
-                const int c0 = sg * seg, c1 = min(ld, c0 + seg);
-                const int r = slab * 32 + lane;
-                const bool rlive = r < ld;
-                const int rr = rlive ? r : 0;
-                const double wr = wrow[rr];
-                double alpha[S], gamma[S];
-                ldv<S>(E + (m.eAlpha + rr) * S, alpha);
-                ldv<S>(E + (m.eGamma + rr) * S, gamma);
-                const uint32_t hdrs = c0 + lane < c1 ? m.m_hdr[slab * ld + c0 + lane] : 0u;
-                double *Jp = out.jac + state0 * Jstate + (long long)c0 * ld + rr;
-                uint32_t h = __shfl_sync(0xFFFFFFFFu, hdrs, 0);
-                uint4 e = (h & 7) ? m.m_ent[(h >> 3) * 32 + lane] : ez;
-                for (int c = c0; c < c1; ++c, Jp += ld) {
-                    const uint32_t hn = __shfl_sync(0xFFFFFFFFu, hdrs, (c + 1 - c0) & 31);
-                    const uint4 en = (c + 1 < c1 && (hn & 7)) ? m.m_ent[(hn >> 3) * 32 + lane] : ez;
-                    const uint32_t steps = h & 7;
-                    double acc[S];
+            if (p < n_panel) gather_phase<2, S, NW>(m, E, sc, m.panel_ptr[p], m.panel_ptr[p + 1], warp, lane);
+            if (p >= 1) {
+                // DENSE: J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c  (Eq. 112 regrouped); a warp
+                // owns a slab of rows and walks a segment of columns
+                const int pp = p - 1;
+                const int c0 = pp * pw, ncol = min(ld, c0 + pw) - c0;
+                const double *tile = E + (size_t)(m.eTile + (pp % m.nbuf) * pw * ld) * S;
+                const int seg = m.d_seg, nseg = (ncol + seg - 1) / seg;
+                if (m.pair) {
+                    const int n_slab = (ld + 63) / 64;
+                    for (int it = warp; it < n_slab * nseg; it += NW) {
+                        const int slab = it % n_slab, sg = it / n_slab;
+                        const int ca = sg * seg, cb = min(ncol, ca + seg);
+                        const int r = slab * 64 + 2 * lane;
+                        const bool live = r < ld;
+                        const int rr = live ? r : 0;
+                        double al[2 * S], ga[2 * S];
+                        ldv<2 * S>(E + (m.eAlpha + rr) * S, al);
+                        ldv<2 * S>(E + (m.eGamma + rr) * S, ga);
+                        const double *tp = tile + ((size_t)ca * ld + rr) * S;
+                        const double *cc = colc + 2 * (c0 + ca);
+                        double *Jp = out.jac + state0 * Jstate + (long long)(c0 + ca) * ld + rr;
+                        for (int c = ca; c < cb; ++c, tp += (size_t)ld * S, cc += 2, Jp += ld) {
+                            const double2 dg = *reinterpret_cast<const double2 *>(cc);
+                            double t[2 * S];
+                            ldv<2 * S>(tp, t);
 #pragma unroll
-                    for (int q = 0; q < S; ++q) acc[q] = 0.0;
-                    auto step = [&](uint32_t w) {
-                        const double cf = entry_coef(w);
-                        double a[S];
-                        ldv<S>(E + (w & 0xFFFF) * S, a);
-#pragma unroll
-                        for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
-                    };
-                    if (steps > 0) step(e.x);
-                    if (steps > 1) step(e.y);
-                    if (steps > 2) step(e.z);
-                    if (steps > 3) step(e.w);
-                    const double2 c01 = *reinterpret_cast<const double2 *>(colc + 4 * c);
-                    const double gz = colc[4 * c + 2];
-                    const double wj = wr * c01.y;
-#pragma unroll
-                    for (int q = 0; q < S; ++q) {
-                        const double v = fma(wj, acc[q], fma(alpha[q], c01.x, -(gamma[q] * gz)));
-                        if (rlive && state0 + q < n) __stcs(Jp + q * Jstate, v);
+                            for (int q = 0; q < S; ++q) {
+                                const double v0 = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
+                                const double v1 = fma(-ga[S + q], dg.y, fma(al[S + q], dg.x, t[S + q]));
+                                if (live && state0 + q < n) st_cs_v2(Jp + q * Jstate, v0, v1);
+                            }
+                        }
                     }
-                    h = hn; e = en;
+                } else {
+                    const int n_slab = (ld + 31) / 32;
+                    for (int it = warp; it < n_slab * nseg; it += NW) {
+                        const int slab = it % n_slab, sg = it / n_slab;
+                        const int ca = sg * seg, cb = min(ncol, ca + seg);
+                        const int r = slab * 32 + lane;
+                        const bool live = r < ld;
+                        const int rr = live ? r : 0;
+                        double al[S], ga[S];
+                        ldv<S>(E + (m.eAlpha + rr) * S, al);
+                        ldv<S>(E + (m.eGamma + rr) * S, ga);
+                        const double *tp = tile + ((size_t)ca * ld + rr) * S;
+                        const double *cc = colc + 2 * (c0 + ca);
+                        double *Jp = out.jac + state0 * Jstate + (long long)(c0 + ca) * ld + rr;
+                        for (int c = ca; c < cb; ++c, tp += (size_t)ld * S, cc += 2, Jp += ld) {
+                            const double2 dg = *reinterpret_cast<const double2 *>(cc);
+                            double t[S];
+                            ldv<S>(tp, t);
+#pragma unroll
+                            for (int q = 0; q < S; ++q) {
+                                const double v = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
+                                if (live && state0 + q < n) __stcs(Jp + q * Jstate, v);
+                            }
+                        }
+                    }
                 }
             }
-            PROF_MARK(8);
-#ifdef PYJAC_PROF
-            if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x)
-                printf("PROF w%d wait %lld | P1 %lld wait %lld | AUX %lld wait %lld | FIX %lld wait %lld | MAIN %lld\n",
-                       warp, prof_t[1] - prof_t[0], prof_t[2] - prof_t[1], prof_t[3] - prof_t[2], prof_t[4] - prof_t[3],
-                       prof_t[5] - prof_t[4], prof_t[6] - prof_t[5], prof_t[7] - prof_t[6], prof_t[8] - prof_t[7]);
-#endif
-        } else {
-            __syncthreads();      // the outputs above read E and the scalars
+            PROF_MARK(5 + (p < 2 ? p : 2));
+            if (p < n_panel) __syncthreads();
         }
+#ifdef PYJAC_PROF
+        if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x)
+            printf("PROF w%d P1 %lld wait %lld | A1 %lld wait %lld | step0 %lld | rest %lld\n", warp,
+                   prof_t[1] - prof_t[0], prof_t[2] - prof_t[1], prof_t[3] - prof_t[2], prof_t[4] - prof_t[3],
+                   prof_t[5] - prof_t[4], prof_t[(n_panel >= 2 ? 7 : 6)] - prof_t[5]);
+#endif
     }
 }
 
@@ -830,35 +881,38 @@ cudaError_t launch_t(const DeviceMech &m, const SmemPlan &sp, int grid, size_t s
 
 }  // namespace
 
-size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + (size_t)sp.shared_total) * sizeof(double); }
+// This file is compiled once per CTA size: -DPYJAC_NT=<threads> -DPYJAC_MB=<CTAs per SM the register
+// budget is set for> (build.py); dispatch.cu switches over the sizes.
+#ifndef PYJAC_NT
+#error "compile with -DPYJAC_NT=<threads per CTA> -DPYJAC_MB=<CTAs per SM>"
+#endif
+#define PYJAC_CAT2(a, b) a##b
+#define PYJAC_CAT(a, b) PYJAC_CAT2(a, b)
+#define PYJAC_FOR_S(X) X(1) X(2) X(4)
 
-// (threads, S, CTAs per SM the register budget is set for)
-#define PYJAC_FOR_ALL(X) \
-    X(128, 1, 4) X(128, 2, 4) X(128, 4, 4) X(256, 1, 2) X(256, 2, 2) X(256, 4, 2) X(512, 1, 1) X(512, 2, 1) X(512, 4, 1) \
-    X(1024, 1, 1) X(1024, 2, 1) X(1024, 4, 1)
-
-const void *eval_kernel_ptr(int level, int nt, int S)
+const void *PYJAC_CAT(eval_kernel_ptr_, PYJAC_NT)(int level, int S)
 {
-#define PYJAC_PTR(N, SV, MB)                                                      \
-    if (nt == N && S == SV)                                                       \
-        return level == 0 ? (const void *)eval_kernel<0, N, SV, MB>               \
-             : level == 1 ? (const void *)eval_kernel<1, N, SV, MB> : (const void *)eval_kernel<2, N, SV, MB>;
-    PYJAC_FOR_ALL(PYJAC_PTR)
+#define PYJAC_PTR(SV)                                                                          \
+    if (S == SV)                                                                               \
+        return level == 0 ? (const void *)eval_kernel<0, PYJAC_NT, SV, PYJAC_MB>               \
+             : level == 1 ? (const void *)eval_kernel<1, PYJAC_NT, SV, PYJAC_MB>               \
+                          : (const void *)eval_kernel<2, PYJAC_NT, SV, PYJAC_MB>;
+    PYJAC_FOR_S(PYJAC_PTR)
 #undef PYJAC_PTR
     return nullptr;
 }
 
-cudaError_t launch_eval(int level, int nt, int S, const DeviceMech &m, const SmemPlan &sp, int grid, size_t smem,
-                        long long n, const double *T, const double *P, const double *Y, long long ldy,
-                        const EvalOut &out, cudaStream_t stream)
+cudaError_t PYJAC_CAT(launch_eval_, PYJAC_NT)(int level, int S, const DeviceMech &m, const SmemPlan &sp, int grid,
+                                              size_t smem, long long n, const double *T, const double *P,
+                                              const double *Y, long long ldy, const EvalOut &out, cudaStream_t stream)
 {
-#define PYJAC_CASE(N, SV, MB)                                                                                   \
-    if (nt == N && S == SV) {                                                                                   \
-        if (level == 0) return launch_t<0, N, SV, MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);         \
-        if (level == 1) return launch_t<1, N, SV, MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);         \
-        return launch_t<2, N, SV, MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);                         \
+#define PYJAC_CASE(SV)                                                                                                  \
+    if (S == SV) {                                                                                                      \
+        if (level == 0) return launch_t<0, PYJAC_NT, SV, PYJAC_MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);    \
+        if (level == 1) return launch_t<1, PYJAC_NT, SV, PYJAC_MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);    \
+        return launch_t<2, PYJAC_NT, SV, PYJAC_MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);                    \
     }
-    PYJAC_FOR_ALL(PYJAC_CASE)
+    PYJAC_FOR_S(PYJAC_CASE)
 #undef PYJAC_CASE
     return cudaErrorInvalidValue;
 }

@@ -8,6 +8,8 @@
 #include <algorithm>
 #include <array>
 #include <cmath>
+#include <cstring>
+#include <utility>
 #include <numeric>
 
 #include "device_mech.h"
@@ -32,15 +34,16 @@ struct ColEntry {
     uint32_t vi;   // E index of s'_ij
 };
 
-// one gathered sum of the AUX phase
+// one gathered sum (A1 phase or one Jacobian cell)
 struct Task {
-    std::vector<uint32_t> ent;
+    std::vector<std::pair<uint32_t, int>> ent;   // kAuxS1 / kAuxT3: (E index, coefficient); kAuxH2: (a | b << 16, 0)
     uint32_t kind = kAuxS1;
-    uint32_t out = 0;       // E slot (kAuxT3: species k)
+    uint32_t out = 0;       // E index of the result (kAuxT3: species k)
     double cst = 1.0;
     int rshift = 0;         // 2^rshift lanes share the sum
     bool lvl01 = false;     // needed by the rates / dydt kernels too
-    int steps() const { return (int)((ent.size() + (size_t(1) << rshift) - 1) >> rshift); }
+    size_t n_words = 0;     // entries after splitting coefficients
+    int steps() const { return (int)((n_words + (size_t(1) << rshift) - 1) >> rshift); }
 };
 
 // lanes that share one sum: enough that no lane walks more than 8 entries (kAuxPre of kernels.cu)
@@ -138,7 +141,7 @@ int n_eff_terms(const pyjac_mech_desc *d, int i)
 
 }  // namespace
 
-static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doubles)
+static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &hints)
 {
     validate(d);
     const int ns = d->n_species, nr = d->n_reactions, ld = ns + 1;
@@ -159,12 +162,10 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     const double iw_last = 1.0 / d->mol_wt[ns - 1];
     o.wrow.assign((size_t)ld, 1.0);
     for (int k = 0; k < ns; ++k) o.wrow[k + 1] = d->mol_wt[k];
-    o.colc.assign((size_t)4 * ld, 0.0);       // {d_j, 1/W_j, 1 (gamma_r applies), 0}; column 0: {0, 1, 0, 0}; column ns: zeros
-    o.colc[1] = 1.0;
+    o.colc.assign((size_t)2 * ld, 0.0);       // {d_j, 1 (gamma_r applies)}; columns 0 and ns: zeros
     for (int k = 0; k + 1 < ns; ++k) {
-        o.colc[4 * (k + 1)] = 1.0 / d->mol_wt[k] - iw_last;
-        o.colc[4 * (k + 1) + 1] = 1.0 / d->mol_wt[k];
-        o.colc[4 * (k + 1) + 2] = 1.0;
+        o.colc[2 * (k + 1)] = 1.0 / d->mol_wt[k] - iw_last;
+        o.colc[2 * (k + 1) + 1] = 1.0;
     }
 
     // ---- per reaction: molecules per side, breakpoints of its species' NASA ranges
@@ -250,11 +251,14 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
     }
     int next_slot = (int)nv;
     auto take = [&](int n) { int r = next_slot; next_slot += n; return r; };
-    const int eQ = take(nr), eAr = take(nr), eTh = take(nr), eH = take(nr);
-    const int eAlpha = take(ld), eGamma = take(ld), eWdot = take(ns), eTcol = take(ns), eG0 = take(ns), eZ = take(ld);
-    const int eS1 = take(1), eA0 = take(1), eS4 = take(1), eZero = take(1), eDump = take(1);
-    o.eQ = eQ; o.eAr = eAr; o.eTh = eTh; o.eH = eH; o.eAlpha = eAlpha; o.eGamma = eGamma; o.eWdot = eWdot;
-    o.eTcol = eTcol; o.eG0 = eG0; o.eZ = eZ; o.eS1 = eS1; o.eA0 = eA0; o.eS4 = eS4; o.eZero = eZero; o.eDump = eDump;
+    const int eQ = take(3 * nr), eH = take(nr);
+    auto take2 = [&](int n) { next_slot = (next_slot + 1) & ~1; return take(n); };      // even: read in pairs of rows
+    const int eAlpha = take2(ld), eGamma = take2(ld), eWdot = take(ns), eG0 = take(ns), eZ = take(ld);
+    const int eS1 = take(1), eA0 = take(1), eS4 = take(1), eZero = take(3), eDump = take(1);   // three zero slots: kAuxT3 pads read q, a, Theta
+    o.eQ = eQ; o.eH = eH; o.eAlpha = eAlpha; o.eGamma = eGamma; o.eWdot = eWdot;
+    o.eG0 = eG0; o.eZ = eZ; o.eS1 = eS1; o.eA0 = eA0; o.eS4 = eS4; o.eZero = eZero; o.eDump = eDump;
+    next_slot = (next_slot + 1) & ~1;
+    o.n_e = next_slot;
     if (next_slot > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-state table entries"};
 
     // ---- per-reaction tables in sorted order
@@ -394,141 +398,130 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
         }
     }
 
-    // ---- AUX sums that always exist
-    std::vector<Task> tasks;
+
+    // ---- launch shape: S states per CTA iteration, CTAs per SM, and the width of the column panels
+    // of the tile.  Everything lives in shared memory: S x (E + tile + two mixture blocks).
+    const long long sm_bytes = 228 * 1024;                       // shared memory of one sm_100 SM
+    auto bytes_for = [&](int S, int pw, int nbuf) {
+        const SmemPlan pl = make_smem_plan(ns, o.n_e + nbuf * pw * ld);
+        return ((long long)S * pl.total + pl.shared_total) * 8;
+    };
+    // each resident CTA also takes a 1 KB system reserve and the kernel's few static bytes
+    auto limit_for = [&](int ctas) { return std::min<long long>(sm_bytes / ctas - 1024 - 128, hints.smem_bytes); };
+    // widest panel (columns) that fits; 0 if not even one column does
+    auto widest = [&](int S, int ctas) {
+        const long long lim = limit_for(ctas);
+        if (bytes_for(S, ld, 1) <= lim) return ld;
+        int pw = 0;
+        for (int w = 1; w < ld; ++w)
+            if (bytes_for(S, w, 2) <= lim) pw = w;
+        return pw;
+    };
+    {
+        int S = 0, ctas = 0, pw = 0;
+        const int cand[][2] = {{2, 4}, {2, 2}, {2, 1}, {1, 2}, {1, 1}};
+        for (auto &c : cand) {
+            if (hints.S > 0 && c[0] != hints.S) continue;
+            if (hints.ctas > 0 && c[1] != hints.ctas) continue;
+            if (c[1] == 4 && ns > 24 && hints.ctas != 4) continue;     // four small CTAs only for tiny models
+            const int w = widest(c[0], c[1]);
+            const int want = hints.pw > 0 ? 1 : (c[1] > 1 || c[0] > 1) ? std::min(ld, 12) : 1;
+            if (w >= want) { S = c[0]; ctas = c[1]; pw = w; break; }
+        }
+        if (S == 0 && hints.S > 0) {            // a hinted S outside the candidate list (e.g. 4)
+            for (int c = (hints.ctas > 0 ? hints.ctas : 2); c >= 1 && S == 0; --c) {
+                const int w = widest(hints.S, c);
+                if (w >= 1) { S = hints.S; ctas = c; pw = w; }
+                if (hints.ctas > 0) break;
+            }
+        }
+        if (S == 0) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
+        if (hints.pw > 0 && hints.pw < pw) pw = hints.pw;
+        const int n_panel = (ld + pw - 1) / pw;
+        pw = (ld + n_panel - 1) / n_panel;
+        o.S = S; o.ctas_target = ctas; o.pw = pw; o.n_panel = n_panel; o.nbuf = n_panel > 1 ? 2 : 1;
+        o.threads = hints.threads > 0 ? hints.threads : ctas >= 4 ? 128 : ctas == 3 ? 256 : ctas == 2 ? 384 : 768;
+        o.eTile = o.n_e;
+        o.pair = (ld % 2 == 0) ? 1 : 0;
+        if ((long long)(o.n_e + o.nbuf * o.pw * ld) * o.S * 8 > (long long)kEntOffMask)
+            throw Fail{PYJAC_ELIMIT, "per-CTA tables exceed the 512 KB offset range of a gather entry"};
+    }
+    const int S = o.S, pw = o.pw, n_panel = o.n_panel, nbuf = o.nbuf, eTile = o.eTile;
+
+    // ---- A1 sums
+    std::vector<Task> a1;
     // (a) per species k: sums of nu_ki {q_i, a_i, Theta_i} (Eq. 14; the d_j coefficient of Eqs. 112, 119,
     //     123, 127 regrouped; the T column, Eq. 111).  The rates / dydt kernels need wdot too.
-    const size_t tT3 = tasks.size();
-    for (int k = 0; k < ns; ++k) { Task t; t.kind = kAuxT3; t.out = (uint32_t)k; t.lvl01 = true; tasks.push_back(t); }
+    const size_t tT3 = a1.size();
+    for (int k = 0; k < ns; ++k) { Task t; t.kind = kAuxT3; t.out = (uint32_t)k; t.lvl01 = true; a1.push_back(t); }
     // (b) gamma_r = (W_k / W_Ns) sum_i nu_ki s'_iNs
-    const size_t tGamma = tasks.size();
+    const size_t tGamma = a1.size();
     for (int k = 0; k < ns; ++k) {
         Task t; t.kind = kAuxS1; t.out = (uint32_t)(eGamma + k + 1); t.cst = d->mol_wt[k] * iw_last;
-        tasks.push_back(t);
+        a1.push_back(t);
     }
     // (c) energy row (Eq. 113): G0_j = sum_i H_i s'_ij per column species
-    const size_t tG0 = tasks.size();
-    for (int j = 0; j < ns; ++j) { Task t; t.kind = kAuxH2; t.out = (uint32_t)(eG0 + j); tasks.push_back(t); }
+    const size_t tG0 = a1.size();
+    for (int j = 0; j < ns; ++j) { Task t; t.kind = kAuxH2; t.out = (uint32_t)(eG0 + j); a1.push_back(t); }
 
     // ---- lists of the Jacobian cells, flat column-major index f = r + c * ld
-    std::vector<std::vector<uint32_t>> cell((size_t)ld * ld);
+    std::vector<std::vector<std::pair<uint32_t, int>>> cell((size_t)ld * ld);
     for (int s = 0; s < nr; ++s) {
         const uint32_t hs = (uint32_t)(eH + s);
-        for (auto &ce : cols[s]) tasks[tG0 + ce.spec].ent.push_back(ce.vi | hs << 16);
+        for (auto &ce : cols[s]) a1[tG0 + ce.spec].ent.push_back({ce.vi | hs << 16, 0});
         for (auto &pr : net[s]) {
             if (pr.second == 0) continue;
             const int k = pr.first;
-            tasks[tT3 + k].ent.push_back(pack_entry((uint32_t)(eQ + s), pr.second));
+            a1[tT3 + k].ent.push_back({(uint32_t)(eQ + 3 * s), pr.second});
             for (auto &ce : cols[s]) {
-                if (ce.spec == ns - 1) tasks[tGamma + k].ent.push_back(pack_entry(ce.vi, pr.second));
-                else cell[(size_t)(k + 1) + (size_t)(ce.spec + 1) * ld].push_back(pack_entry(ce.vi, pr.second));
+                if (ce.spec == ns - 1) a1[tGamma + k].ent.push_back({ce.vi, pr.second});
+                else cell[(size_t)(k + 1) + (size_t)(ce.spec + 1) * ld].push_back({ce.vi, pr.second});
             }
         }
     }
-    for (int k = 0; k < ns; ++k) cell[(size_t)(k + 1)].push_back(pack_entry((uint32_t)(eTcol + k), 1));   // column 0
-    for (int c = 0; c < ns; ++c) cell[(size_t)c * ld].push_back(pack_entry((uint32_t)(eZ + c), 1));        // row 0
-    for (auto &c : cell) o.n_list_entries += (long long)c.size();
 
-    // ---- MAIN pass: the Jacobian in slabs of 32 rows; a warp walks a slab column by column.  Per
-    // (slab, column) every lane (row) gathers at most `cap` <= 4 entries (one 16-byte load); longer
-    // lists are summed by an AUX task and enter as one entry.  The cap minimises (steps of the slab
-    // column) + (steps of the AUX chunks it causes); `lambda` prices the extra E slots and grows until
-    // E fits the shared memory.
-    const int n_slab = (ld + 31) / 32;
-    o.n_slab = n_slab;
-    auto cell_at = [&](int slab, int c, int l) -> std::vector<uint32_t> * {
-        const int r = 32 * slab + l;
-        return r < ld ? &cell[(size_t)r + (size_t)c * ld] : nullptr;
+    // ---- encoding of the entries (device_mech.h): coefficients outside {1,2,3,4,6,8} are split
+    auto encode = [&](const Task &t, std::vector<uint32_t> &w) {
+        w.clear();
+        for (auto &e : t.ent) {
+            if (t.kind == kAuxH2) { w.push_back(e.first); continue; }
+            int c = e.second;
+            const int sg = c < 0 ? -1 : 1;
+            c = c < 0 ? -c : c;
+            static const int parts[] = {8, 6, 4, 3, 2, 1};
+            while (c > 0)
+                for (int pz : parts)
+                    if (pz <= c) { w.push_back(coef_hi13(sg * pz) | (uint32_t)(e.first * S * 8)); c -= pz; break; }
+        }
     };
-    std::vector<int> cap((size_t)n_slab * ld, 0);
-    const long long e_limit = std::min<long long>(smem_doubles, 65535);
-    for (double lambda = 0.15;; lambda *= 2.0) {
-        int slots = next_slot;
-        bool any_overflow = false;
-        for (int sb = 0; sb < n_slab; ++sb)
-            for (int c = 0; c < ld; ++c) {
-                int len[32], mx = 0;
-                for (int l = 0; l < 32; ++l) {
-                    auto *p = cell_at(sb, c, l);
-                    len[l] = p ? (int)p->size() : 0;
-                    mx = std::max(mx, len[l]);
-                }
-                double best = 1e300;
-                int bestc = mx;
-                for (int cc = (mx > 0 ? 1 : 0); cc <= std::min(mx, 4); ++cc) {
-                    double cost = (double)cc;
-                    for (int l = 0; l < 32; ++l)
-                        if (len[l] > cc) cost += 1.25 * len[l] / 32.0 + lambda;
-                    if (cost < best) { best = cost; bestc = cc; }
-                }
-                cap[(size_t)sb * ld + c] = bestc;
-                for (int l = 0; l < 32; ++l)
-                    if (len[l] > bestc) { ++slots; any_overflow = true; }
-            }
-        if (slots <= e_limit) break;
-        if (!any_overflow || lambda > 1e6) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
-    }
-    for (int sb = 0; sb < n_slab; ++sb)
-        for (int c = 0; c < ld; ++c)
-            for (int l = 0; l < 32; ++l) {
-                auto *p = cell_at(sb, c, l);
-                if (!p || (int)p->size() <= cap[(size_t)sb * ld + c]) continue;
-                Task a;
-                a.kind = kAuxS1;
-                a.out = (uint32_t)next_slot++;
-                a.ent.swap(*p);
-                tasks.push_back(a);
-                p->push_back(pack_entry(tasks.back().out, 1));
-            }
-    o.n_e = next_slot;
-    if (o.n_e > e_limit) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
-    const uint32_t pad1 = pack_entry((uint32_t)eZero, 0);
+    const uint32_t pad1 = (uint32_t)(eZero * S * 8);                 // coefficient 0 times the zero slot
     const uint32_t pad2 = (uint32_t)eZero | (uint32_t)eZero << 16;
 
-    // ---- MAIN entries: m_hdr[slab][column] = (block index << 3) | steps; a block is 32 lanes x 4 entries
-    o.m_hdr.assign((size_t)n_slab * ld, 0u);
-    for (int sb = 0; sb < n_slab; ++sb)
-        for (int c = 0; c < ld; ++c) {
-            int steps = 0;
-            for (int l = 0; l < 32; ++l) {
-                auto *p = cell_at(sb, c, l);
-                if (p) steps = std::max(steps, (int)p->size());
-            }
-            if (steps == 0) continue;
-            const uint32_t blk = (uint32_t)(o.m_ent.size() / 128);
-            o.m_hdr[(size_t)sb * ld + c] = blk << 3 | (uint32_t)steps;
-            o.m_ent.resize(o.m_ent.size() + 128, pad1);
-            for (int l = 0; l < 32; ++l) {
-                auto *p = cell_at(sb, c, l);
-                if (!p) continue;
-                for (size_t e = 0; e < p->size(); ++e) o.m_ent[(size_t)blk * 128 + (size_t)l * 4 + e] = (*p)[e];
-            }
-            o.n_main_entries += (long long)steps * 32;
+    // ---- chunks: sums of one kind, shared by equally many lanes and of similar length, fill the 32
+    // lanes of a chunk; the warps take the chunks of a phase round-robin, most expensive first.
+    struct Chunk { std::vector<Task *> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; };
+    std::vector<uint32_t> words;
+    auto emit_phase = [&](std::vector<Task> &tasks, bool with_r3, long long &step_count) {
+        for (auto &t : tasks) {
+            encode(t, words);
+            t.n_words = words.size();
+            t.rshift = pick_rshift(t.n_words);
         }
-    if (o.m_ent.empty()) o.m_ent.assign(128, pad1);
-
-    // ---- AUX chunks: sums of one kind, shared by equally many lanes and of similar length, fill the
-    // 32 lanes of a chunk; the warps take the chunks in a fixed round-robin order, longest first.
-    // Entries: step t of lane l at ent_base + (t / 8) * 256 + l * 8 + (t % 8) (two 16-byte loads per
-    // lane fetch eight steps).
-    for (auto &t : tasks) t.rshift = pick_rshift(t.ent.size());
-    struct Chunk { std::vector<size_t> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; };
-    std::vector<Chunk> chunks;
-    if (nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0});
-    {
-        std::vector<size_t> idx(tasks.size());
-        std::iota(idx.begin(), idx.end(), 0);
-        std::stable_sort(idx.begin(), idx.end(), [&](size_t a, size_t b) {
-            if (tasks[a].kind != tasks[b].kind) return tasks[a].kind < tasks[b].kind;
-            if (tasks[a].rshift != tasks[b].rshift) return tasks[a].rshift > tasks[b].rshift;
-            return tasks[a].steps() > tasks[b].steps();
+        std::vector<Chunk> chunks;
+        if (with_r3 && nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0});
+        std::vector<Task *> idx;
+        for (auto &t : tasks) idx.push_back(&t);
+        std::stable_sort(idx.begin(), idx.end(), [&](const Task *a, const Task *b) {
+            if (a->kind != b->kind) return a->kind < b->kind;
+            if (a->rshift != b->rshift) return a->rshift > b->rshift;
+            return a->steps() > b->steps();
         });
         for (size_t p = 0; p < idx.size();) {
-            const Task &t0 = tasks[idx[p]];
+            const Task &t0 = *idx[p];
             Chunk c{{}, t0.kind, t0.rshift, 0, t0.lvl01, 0.0};
             const size_t per = (size_t)32 >> t0.rshift;
-            while (p < idx.size() && c.t.size() < per && tasks[idx[p]].kind == c.kind && tasks[idx[p]].rshift == c.rshift) {
-                c.steps = std::max(c.steps, tasks[idx[p]].steps());
+            while (p < idx.size() && c.t.size() < per && idx[p]->kind == c.kind && idx[p]->rshift == c.rshift) {
+                c.steps = std::max(c.steps, idx[p]->steps());
                 c.t.push_back(idx[p++]);
             }
             chunks.push_back(c);
@@ -542,45 +535,84 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, long long smem_doub
             if (a.lvl01 != b.lvl01) return a.lvl01;
             return a.cost > b.cost;
         });
-    }
-    o.n_achunk = (int)chunks.size();
-    o.n_achunk01 = 0;
-    for (auto &c : chunks) o.n_achunk01 += c.lvl01 ? 1 : 0;
-    for (auto &c : chunks) {
-        const uint32_t base = (uint32_t)o.a_ent.size();
-        const int per = 32 >> c.rshift, width = 1 << c.rshift;
-        o.achunk.push_back(base);
-        o.achunk.push_back((uint32_t)c.steps);
-        o.achunk.push_back(c.kind | (uint32_t)c.rshift << 8);
-        o.achunk.push_back((uint32_t)o.a_out.size());
-        if (c.kind == kAuxR3) {
-            o.a_out.push_back(0u);
-            o.a_const.push_back(0.0);
-            continue;
-        }
-        const int rounds = (c.steps + 7) / 8;
-        o.a_ent.resize(o.a_ent.size() + (size_t)rounds * 256, c.kind == kAuxH2 ? pad2 : pad1);
-        for (int l = 0; l < per; ++l) {
-            if (l >= (int)c.t.size()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); continue; }
-            const Task &t = tasks[c.t[l]];
-            o.a_out.push_back(t.out);
-            o.a_const.push_back(t.cst);
-            for (size_t e = 0; e < t.ent.size(); ++e) {
-                const size_t step = e / width, lane = (size_t)l * width + (e % width);
-                o.a_ent[(size_t)base + (step / 8) * 256 + lane * 8 + (step % 8)] = t.ent[e];
+        int n01 = 0;
+        for (auto &c : chunks) {
+            n01 += c.lvl01 ? 1 : 0;
+            const uint32_t base = (uint32_t)(o.a_ent.size() / 4);       // in uint4 units
+            const int per = 32 >> c.rshift, width = 1 << c.rshift;
+            o.achunk.push_back(base);
+            o.achunk.push_back((uint32_t)c.steps);
+            o.achunk.push_back(c.kind | (uint32_t)c.rshift << 8);
+            o.achunk.push_back((uint32_t)(o.a_task.size() / 4));
+            auto push_task = [&](uint32_t out, double cst) {
+                uint64_t bits;
+                std::memcpy(&bits, &cst, 8);
+                o.a_task.push_back(out);
+                o.a_task.push_back(0u);
+                o.a_task.push_back((uint32_t)bits);
+                o.a_task.push_back((uint32_t)(bits >> 32));
+            };
+            if (c.kind == kAuxR3) { push_task(0u, 0.0); continue; }
+            const int rounds = (c.steps + 3) / 4;
+            o.a_ent.resize(o.a_ent.size() + (size_t)rounds * 128, c.kind == kAuxH2 ? pad2 : pad1);
+            for (int l = 0; l < per; ++l) {
+                if (l >= (int)c.t.size()) { push_task(0xFFFFFFFFu, 0.0); continue; }
+                const Task &t = *c.t[l];
+                push_task(t.out, t.cst);
+                encode(t, words);
+                for (size_t e = 0; e < words.size(); ++e) {
+                    const size_t step = e / width, lane = (size_t)l * width + (e % width);
+                    o.a_ent[(size_t)base * 4 + ((step / 4) * 32 + lane) * 4 + (step % 4)] = words[e];
+                }
             }
+            step_count += c.steps;
         }
-        o.n_aux_entries += (long long)c.steps * 32;
+        return std::make_pair((int)chunks.size(), n01);
+    };
+
+    {
+        auto r = emit_phase(a1, true, o.n_a1_steps);
+        o.n_a1 = r.first;
+        o.n_a1_01 = r.second;
     }
-    if (o.a_ent.empty()) o.a_ent.assign(256, pad1);
-    if (o.achunk.empty()) { o.achunk.assign(4, 0u); }
-    if (o.a_out.empty()) { o.a_out.push_back(0xFFFFFFFFu); o.a_const.push_back(0.0); }
+
+    // ---- the cells, panel by panel.  Column 0 (rows >= 1) is written by the kAuxT3 sums and row 0 of
+    // panel 0 by the FIX step; with several panels every other cell of a panel gets a task (a cell
+    // that is structurally zero in this panel may not be in the panel that used the buffer before).
+    o.panel_ptr.assign(1, o.n_a1);
+    for (int p = 0; p < n_panel; ++p) {
+        std::vector<Task> tasks;
+        const int c0 = p * pw, c1 = std::min(ld, c0 + pw);
+        for (int c = c0; c < c1; ++c)
+            for (int r = 0; r < ld; ++r) {
+                if (c == 0 && r >= 1) continue;
+                if (r == 0 && p == 0) continue;
+                Task t;
+                t.kind = kAuxS1;
+                t.out = (uint32_t)(eTile + (p % nbuf) * pw * ld + (c - c0) * ld + r);
+                if (r == 0) {
+                    if (c < ns) t.ent.push_back({(uint32_t)(eZ + c), 1});
+                } else {
+                    t.ent = cell[(size_t)r + (size_t)c * ld];
+                    if (!t.ent.empty()) t.cst = d->mol_wt[r - 1] * (1.0 / d->mol_wt[c - 1]);
+                }
+                if (t.ent.empty() && n_panel == 1) continue;
+                o.n_cell_entries += (long long)t.ent.size();
+                tasks.push_back(t);
+            }
+        o.n_cells += (long long)tasks.size();
+        auto r = emit_phase(tasks, false, o.n_cell_steps);
+        o.panel_ptr.push_back(o.panel_ptr.back() + r.first);
+    }
+    if (o.a_ent.empty()) o.a_ent.assign(128, pad1);
+    if (o.achunk.empty()) o.achunk.assign(4, 0u);
+    if (o.a_task.empty()) o.a_task.assign(4, 0xFFFFFFFFu);
 }
 
-int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, long long smem_doubles, const char **why)
+int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const ShapeHints &hints, const char **why)
 {
     try {
-        pack_impl(d, out, smem_doubles);
+        pack_impl(d, out, hints);
     } catch (const Fail &f) {
         if (why) *why = f.why;
         return f.code;

@@ -25,22 +25,30 @@ struct HostPack {
     std::vector<int32_t> pk_ptr;
     std::vector<double> pk_data;
     int n_rchunk = 0;
-    int n_achunk = 0, n_achunk01 = 0;
+    // gathers (device_mech.h): A1 chunks first, then the cell chunks panel by panel
+    int n_a1 = 0, n_a1_01 = 0;
     std::vector<uint32_t> achunk;         // uint4 flattened
-    std::vector<uint32_t> a_ent, a_out;
-    std::vector<double> a_const;
-    int n_slab = 0;
-    std::vector<uint32_t> m_hdr;          // [n_slab][ns+1]
-    std::vector<uint32_t> m_ent;          // blocks of 32 lanes x 4 entries
-    int eQ = 0, eAr = 0, eTh = 0, eH = 0, eAlpha = 0, eGamma = 0, eWdot = 0, eTcol = 0, eG0 = 0, eZ = 0;
+    std::vector<uint32_t> a_ent;          // uint4 flattened
+    std::vector<uint32_t> a_task;         // uint4 flattened
+    std::vector<int32_t> panel_ptr;       // [n_panel + 1]
+    int n_panel = 1, pw = 0, nbuf = 1, eTile = 0, pair = 0;
+    int eQ = 0, eH = 0, eAlpha = 0, eGamma = 0, eWdot = 0, eG0 = 0, eZ = 0;
     int eS1 = 0, eA0 = 0, eS4 = 0, eZero = 0, eDump = 0, n_e = 0;
+    // launch shape chosen with the tables: S states per CTA iteration, threads per CTA, the CTAs
+    // per SM the shared-memory footprint was sized for
+    int S = 1, threads = 128, ctas_target = 1;
     // statistics (pyjac_pack_stats)
-    long long n_main_entries = 0, n_aux_entries = 0, n_list_entries = 0, n_plain_chunks = 0;
+    long long n_cell_entries = 0, n_cell_steps = 0, n_a1_steps = 0, n_cells = 0, n_plain_chunks = 0;
+};
+
+// What the launch-shape choice may use (api.cu fills it from the device properties and the
+// PYJAC_S / PYJAC_THREADS / PYJAC_PW / PYJAC_CTAS tuning hooks; 0 = choose).
+struct ShapeHints {
+    long long smem_bytes = 227 * 1024 - 1024;   // dynamic shared memory one CTA may use
+    int S = 0, threads = 0, pw = 0, ctas = 0;
 };
 
 // Returns PYJAC_OK, PYJAC_EINVAL or PYJAC_ELIMIT.  `why` (optional) receives a static message.
-// smem_doubles: doubles of shared memory one state may use for E (decides how many of the
-// Jacobian's cell lists are summed by AUX tasks instead of inline in the MAIN pass).
-int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, long long smem_doubles, const char **why);
+int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const ShapeHints &hints, const char **why);
 
 }  // namespace pyjac
