@@ -18,7 +18,7 @@ OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libpyjac_b200.so")
 HOST_SOURCES = ["api.cu", "mech_pack.cu", "dispatch.cu"]
 # (threads per CTA, CTAs per SM the register budget is set for) -- keep in step with csrc/dispatch.cu
-KERNEL_SIZES = [(128, 4), (256, 3), (384, 2), (512, 1), (768, 1), (1024, 1)]
+KERNEL_SIZES = [(128, 4), (256, 3), (384, 2), (512, 2), (768, 1), (1024, 1)]
 HEADERS = ["device_mech.h", "kernels.h", "mech_pack.h", os.path.join("..", "..", "include", "pyjac_b200.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]

@@ -144,10 +144,10 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         up.add(&dm.th_off, hp.th_off); up.add(&dm.th_data, hp.th_data); up.add(&dm.th_soa, hp.th_soa);
         up.add(&dm.lo_lnA, hp.lo_lnA); up.add(&dm.lo_beta, hp.lo_beta); up.add(&dm.lo_Ta, hp.lo_Ta);
         up.add(&dm.fall_par, hp.fall_par);
-        up.add(&dm.eff_ptr, hp.eff_ptr); up.add(&dm.eff_spec, hp.eff_spec); up.add(&dm.eff_eps, hp.eff_eps);
+        up.add(&dm.eff_base, hp.eff_base); up.add((const uint32_t **)&dm.eff_ent, hp.eff_ent);
         up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
         up.add((const uint32_t **)&dm.achunk, hp.achunk); up.add((const uint32_t **)&dm.a_ent, hp.a_ent);
-        up.add((const uint32_t **)&dm.a_task, hp.a_task); up.add(&dm.panel_ptr, hp.panel_ptr);
+        up.add(&dm.panel_ptr, hp.panel_ptr);
     } catch (...) {
         delete m;
         cudaSetDevice(prev);
@@ -163,7 +163,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
         m->plan = make_smem_plan(hp.ns, hp.n_e + hp.nbuf * hp.pw * (hp.ns + 1));
         m->stats[0] = hp.n_e; m->stats[1] = hp.n_cell_entries; m->stats[2] = hp.n_cell_steps;
-        m->stats[3] = hp.n_a1_steps; m->stats[4] = hp.n_cells; m->stats[5] = (long long)hp.achunk.size() / 4;
+        m->stats[3] = hp.n_a1_steps; m->stats[4] = hp.n_cells; m->stats[5] = (long long)hp.achunk.size() / 2;
         const size_t bytes = eval_smem_bytes(m->plan, m->S);
         if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->threads, m->S)) {
             rc = PYJAC_ELIMIT;
@@ -264,7 +264,7 @@ int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
     if (rc != PYJAC_OK) return rc;
     const SmemPlan plan = make_smem_plan(hp.ns, hp.n_e + hp.nbuf * hp.pw * (hp.ns + 1));
     stats[0] = hp.n_e; stats[1] = hp.n_cell_entries; stats[2] = hp.n_cell_steps; stats[3] = hp.n_a1_steps;
-    stats[4] = hp.n_cells; stats[5] = (int64_t)hp.achunk.size() / 4; stats[6] = (int64_t)eval_smem_bytes(plan, hp.S);
+    stats[4] = hp.n_cells; stats[5] = (int64_t)hp.achunk.size() / 2; stats[6] = (int64_t)eval_smem_bytes(plan, hp.S);
     stats[7] = hp.n_rchunk; stats[8] = hp.S; stats[9] = hp.threads; stats[10] = hp.n_panel; stats[11] = hp.pw;
     return PYJAC_OK;
 }

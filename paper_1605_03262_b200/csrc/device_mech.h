@@ -49,7 +49,7 @@ __host__ __device__ inline uint32_t coef_hi13(int coef)
     return (hi >> 3) << 19;
 }
 
-// kinds of gather chunks (chunk.z bits 0..7; bits 8..15 = log2 of the lanes that share one sum)
+// kinds of gather chunks
 enum : uint32_t {
     kAuxT3 = 0,    // entries {q_i of reaction i, nu_ki}: sums of nu q_i, nu a_i, nu Theta_i -> wdot_k, alpha_{k+1}, T column
     kAuxS1 = 1,    // entries {source, coef}: one sum, times a task constant -> E / tile slot
@@ -91,9 +91,10 @@ struct DeviceMech {
                                 // rows 8..14 g of the upper one
     const double *lo_lnA, *lo_beta, *lo_Ta;      // [n_pd] k_0
     const double *fall_par;                      // [n_pd][5]
-    const int32_t *eff_ptr;                      // [n_pd+1]
-    const uint32_t *eff_spec;                    // species of alpha_ij != 1 (or the single species) | E index of its term << 16
-    const double *eff_eps;                       // alpha_ij - 1      (1 for the single species)
+    const int32_t *eff_base;    // [general groups + 1] first efficiency entry of a group of 32 reactions
+    const uint4 *eff_ent;       // entry e of lane l of group c at [eff_base[c] + 32 e + l]: {species of alpha_ij != 1
+                                // (or the single species) | E index of its term << 16, 0, alpha_ij - 1 (fp64 bits;
+                                // 1 for the single species)}; padded with {dummy species | dump slot << 16, 0, 0.0}
     const int32_t *pk_ptr;      // [n_pk+1] offsets into pk_data
     const double *pk_data;      // PLOG: n, then n x {p, ln p, ln A, beta, Ta};
                                 // Chebyshev: nT, nP, 1/Tmin, 1/Tmax, log10 pmin, log10 pmax, eta[nT*nP]
@@ -101,9 +102,10 @@ struct DeviceMech {
     // Chunks [0, n_a1) are the A1 phase (the first n_a1_01 of them serve rates / dydt too); the
     // chunks of the cells of column panel p are [panel_ptr[p], panel_ptr[p+1]).
     int n_a1, n_a1_01;
-    const uint4 *achunk;        // {first entry block, steps, kind | rshift << 8, first task}
-    const uint4 *a_ent;         // step t of lane l of a chunk: word (t & 3) of a_ent[first + (t >> 2) * 32 + l]
-    const uint4 *a_task;        // [task] {output E index (kAuxT3: species k; ~0 = none), 0, constant factor (fp64 bits)}
+    const uint2 *achunk;        // {first block of a_ent, steps | kind << 16 | rshift << 20}
+    const uint4 *a_ent;         // block r of a chunk = a_ent[first + 32 r + lane].  Block 0: {output E index
+                                // (kAuxT3: species k; ~0 = none), constant factor (fp64 bits, 2 words), entry of
+                                // step 0}; block r >= 1: the entries of steps 4r-3 .. 4r
     const int32_t *panel_ptr;   // [n_panel + 1]
     // ---- the tile: column panels of the Jacobian, state-interleaved like E, element (r, c) of
     // panel p at E index eTile + (p % nbuf) * pw * ld + (c - p * pw) * ld + r
@@ -126,7 +128,7 @@ struct DeviceMech {
 
 // per-state scalars (region Scal of the shared-memory plan)
 enum {
-    kT = 0, kLnT, kInvT, kP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kNScal = 10
+    kT = 0, kLnT, kInvT, kP, kLnP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kIcp, kNScal = 12
 };
 
 // Shared-memory plan (offsets in doubles PER STATE).  A CTA evaluates S states at a time and

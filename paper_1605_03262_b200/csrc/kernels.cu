@@ -226,16 +226,18 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     double lnA = 0.0, beta = 0.0, Ta = 0.0;
     if (arrh) { lnA = m.lnA[s]; beta = m.beta[s]; Ta = m.Ta[s]; }
     const double dnu = (double)(snu_r - snu_f);
-    const double *th = m.th_data + m.th_off[s];
-    const int nint = (int)th[0];
+    const double brk = m.th_soa[s];             // NaN: more than two intervals, see th_data
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
     if (LEVEL == 2) {
         const uint4 vi = m.vidx[s];
         v0 = (vi.x & 0xFFFF) * S; v1 = (vi.x >> 16) * S; v2 = (vi.y & 0xFFFF) * S;
         v3 = (vi.y >> 16) * S; v4 = (vi.z & 0xFFFF) * S; v5 = (vi.z >> 16) * S;
     }
-    int eb = 0, ee = 0;
-    if (pdep) { eb = m.eff_ptr[s]; ee = m.eff_ptr[s + 1]; }
+    // efficiencies of the group's reactions, entry e of lane l at eff_ent[eff_base[group] + 32 e + l]
+    // (padded with eps = 0 on the dummy species, so the trip count is the group's)
+    const int grp = s >> 5;
+    const uint4 *ef = m.eff_ent + m.eff_base[grp] + (s & 31);
+    const int n_eff = m.eff_base[grp + 1] - m.eff_base[grp];        // 32 x entries per lane
 
     {
         const double T = sc[kT * S + q], lnT = sc[kLnT * S + q], invT = sc[kInvT * S + q];
@@ -265,10 +267,10 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             } else if (P >= row[5 * (np - 1)]) {
                 lo = hi = np - 1;
             } else {
-                int j = 0;
-                while (!(row[5 * j] <= P && P < row[5 * (j + 1)])) ++j;
+                int j = 0;                                           // p_j <= P < p_{j+1}
+                for (int k = 1; k < np - 1; ++k) j += P >= row[5 * k] ? 1 : 0;
                 lo = j; hi = j + 1;
-                wt = (log(P) - row[5 * j + 1]) / (row[5 * (j + 1) + 1] - row[5 * j + 1]);
+                wt = (sc[kLnP * S + q] - row[5 * j + 1]) / (row[5 * (j + 1) + 1] - row[5 * j + 1]);
             }
             const double *a1 = row + 5 * lo, *a2 = row + 5 * hi;
             const double lnk1 = a1[2] + a1[3] * lnT - a1[4] * invT;
@@ -282,7 +284,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             const double iTmin = pk[2], iTmax = pk[3], lpmin = pk[4], lpmax = pk[5];
             const double *eta = pk + 6;
             const double Tr = (2.0 * invT - iTmin - iTmax) / (iTmax - iTmin);
-            const double Pr = (2.0 * log10(P) - lpmin - lpmax) / (lpmax - lpmin);
+            const double Pr = (2.0 * (sc[kLnP * S + q] * kInvLn10) - lpmin - lpmax) / (lpmax - lpmin);
             double sum = 0.0, dsum = 0.0;
             double tm2 = 1.0, tm1 = Tr;          // T_{a-2}, T_{a-1}
             double um2 = 1.0, um1 = 2.0 * Tr;    // U_{a-3}, U_{a-2}
@@ -311,11 +313,20 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
 
         // ---- sum_k nu_ki B_k (Eq. 27 over the reaction), its T derivative (Eq. 74) and the reaction
         //      enthalpy H_i = sum_k nu_ki h_k W_k = R T (T d(sum nu B)/dT + sum nu)
-        int iv = 0;
-        for (int b = 1; b < nint; ++b) iv += T > th[b] ? 1 : 0;
-        const double *g = th + nint + 7 * iv;
-        const double g1 = g[1], g2 = g[2], g3 = g[3], g4 = g[4], g5 = g[5], g6 = g[6];
-        const double sB = fma(g1, lnT, g[0]) + fma(T, fma(T, fma(T, fma(T, g5, g4), g3), g2), g6 * invT);
+        double g0, g1, g2, g3, g4, g5, g6;
+        if (brk == brk) {
+            const double *g = m.th_soa + s + (size_t)(T > brk ? 8 : 1) * m.nr;
+            const size_t nrs = (size_t)m.nr;
+            g0 = g[0]; g1 = g[nrs]; g2 = g[2 * nrs]; g3 = g[3 * nrs]; g4 = g[4 * nrs]; g5 = g[5 * nrs]; g6 = g[6 * nrs];
+        } else {
+            const double *th = m.th_data + m.th_off[s];
+            const int nint = (int)th[0];
+            int iv = 0;
+            for (int b = 1; b < nint; ++b) iv += T > th[b] ? 1 : 0;
+            const double *g = th + nint + 7 * iv;
+            g0 = g[0]; g1 = g[1]; g2 = g[2]; g3 = g[3]; g4 = g[4]; g5 = g[5]; g6 = g[6];
+        }
+        const double sB = fma(g1, lnT, g0) + fma(T, fma(T, fma(T, fma(T, g5, g4), g3), g2), g6 * invT);
         const double sdB = fma(fma(-g6, invT, g1), invT, g2) + T * fma(T, fma(4.0 * g5, T, 3.0 * g4), 2.0 * g3);
         const double H = kRu * T * fma(T, sdB, dnu);
 
@@ -358,7 +369,14 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         double c = 1.0, G = 0.0, fT = 0.0, b = 0.0, Xi = 0.0;
         if (pdep) {
             Xi = meta_single(meta) ? 0.0 : sc[kM * S + q];               // Eqs. 28-30
-            for (int e = eb; e < ee; ++e) Xi += m.eff_eps[e] * X[(m.eff_spec[e] & 0xFFFF) * S + q];
+            for (int e = 0; e < n_eff; e += 128) {                       // four entries at a time, loads first
+                uint4 w[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.ns, 0u, 0u, 0u);
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    Xi = fma(__hiloint2double((int)w[u].w, (int)w[u].z), X[(w[u].x & 0xFFFF) * S + q], Xi);
+            }
             if (type == PYJAC_THIRD_BODY) {
                 c = Xi; G = Xi; lPrT = -invT; b = R;                     // Eqs. 79-80
             } else {
@@ -425,7 +443,14 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             const double ckf = c * kf, ckr = -c * kr;
             E[v0 + q] = ckf * sk0; E[v1 + q] = ckf * sk1; E[v2 + q] = ckf * sk2;
             E[v3 + q] = ckr * sk3; E[v4 + q] = ckr * sk4; E[v5 + q] = ckr * sk5;
-            for (int e = eb; e < ee; ++e) E[(m.eff_spec[e] >> 16) * S + q] = b * m.eff_eps[e];
+            if (pdep)
+                for (int e = 0; e < n_eff; e += 128) {
+                    uint4 w[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) E[(w[u].x >> 16) * S + q] = b * __hiloint2double((int)w[u].w, (int)w[u].z);
+                }
         }
     }
 }
@@ -470,58 +495,64 @@ __device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double 
     }
     if (LEVEL >= 1) { cp = warp_sum(cp); dcp = warp_sum(dcp); }
     if (lane == 0) {
-        sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P;
+        sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P; sc[kLnP * S + q] = log(P);
         sc[kM * S + q] = M; sc[kW * S + q] = W; sc[kRho * S + q] = rho; sc[kIrho * S + q] = 1.0 / rho;
-        sc[kCpMix * S + q] = cp; sc[kDcpDT * S + q] = dcp;
+        sc[kCpMix * S + q] = cp; sc[kDcpDT * S + q] = dcp; sc[kIcp * S + q] = 1.0 / cp;
     }
 }
 
-// ---- one gather chunk: 32 lanes, 32 >> rshift sums (device_mech.h) ---------------------------------
+// ---- one gather chunk: 32 lanes, 32 >> rshift sums (device_mech.h).  `r0` is block 0 of the chunk
+// (output index, constant, first entry) and `e1` block 1 (steps 1..4; anything if steps < 2), both
+// fetched by the caller one chunk ahead.
 template <int LEVEL, int S>
-__device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, const double *sc, const uint4 ch, int lane)
+__device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, const double *sc, const uint2 ch,
+                                             const uint4 r0, const uint4 e1, int lane)
 {
-    const uint32_t kind = ch.z & 0xFF;
-    const int rshift = (ch.z >> 8) & 0xFF, width = 1 << rshift;
-    const int steps = (int)ch.y;
+    const uint32_t kind = (ch.y >> 16) & 0xF;
+    const int rshift = (int)(ch.y >> 20), width = 1 << rshift;
+    const int steps = (int)(ch.y & 0xFFFF);
     const uint4 *ep = m.a_ent + ch.x + lane;
-    const uint4 task = m.a_task[ch.w + (lane >> rshift)];
-    const bool head = (lane & (width - 1)) == 0 && task.x != 0xFFFFFFFFu;
+    const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
     const char *Eb = reinterpret_cast<const char *>(E);
     const uint4 ez = make_uint4(0u, 0u, 0u, 0u);
     const int nr = m.nr;
+    int left = steps - 1;                                   // steps after the one in block 0
+    uint4 e = e1;
 
     if (kind == kAuxS1) {
         if (LEVEL == 2) {
             double acc[S];
 #pragma unroll
             for (int q = 0; q < S; ++q) acc[q] = 0.0;
-            auto step = [&](uint32_t e) {
-                const double cf = entry_coef(e);
+            auto step = [&](uint32_t w) {
+                const double cf = entry_coef(w);
                 double a[S];
-                ldv<S>(reinterpret_cast<const double *>(Eb + (e & kEntOffMask)), a);
+                ldv<S>(reinterpret_cast<const double *>(Eb + (w & kEntOffMask)), a);
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
             };
-            uint4 e = steps > 0 ? ep[0] : ez;
-            int t = 0;
-            for (; t + 4 < steps; t += 4) {
-                const uint4 en = ep[(t / 4 + 1) * 32];
-                step(e.x); step(e.y); step(e.z); step(e.w);
+            if (steps > 0) step(r0.w);
+            for (int r = 2; left > 0; ++r, left -= 4) {
+                const uint4 en = left > 4 ? ep[r * 32] : ez;
+                step(e.x);
+                if (left > 1) {
+                    step(e.y);
+                    if (left > 2) {
+                        step(e.z);
+                        if (left > 3) step(e.w);
+                    }
+                }
                 e = en;
             }
-            const int rem = steps - t;
-            if (rem > 0) step(e.x);
-            if (rem > 1) step(e.y);
-            if (rem > 2) step(e.z);
-            if (rem > 3) step(e.w);
-            for (int o = 1; o < width; o <<= 1)
+            if (rshift > 0)
+                for (int o = 1; o < width; o <<= 1)
 #pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
+                    for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
             if (head) {
-                const double cst = __hiloint2double((int)task.w, (int)task.z);
+                const double cst = __hiloint2double((int)r0.z, (int)r0.y);
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] *= cst;
-                stv<S>(E + (size_t)task.x * S, acc);
+                stv<S>(E + r0.x * S, acc);
             }
         }
     } else if (kind == kAuxH2) {
@@ -529,21 +560,23 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
             double acc[S];
 #pragma unroll
             for (int q = 0; q < S; ++q) acc[q] = 0.0;
-            auto step = [&](uint32_t e) {
+            auto step = [&](uint32_t w) {
                 double a[S], b[S];
-                ldv<S>(E + (e & 0xFFFF) * S, a);
-                ldv<S>(E + (e >> 16) * S, b);
+                ldv<S>(E + (w & 0xFFFF) * S, a);
+                ldv<S>(E + (w >> 16) * S, b);
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
             };
-            for (int t = 0; t < steps; t += 4) {
-                const uint4 e = ep[(t / 4) * 32];
+            if (steps > 0) step(r0.w);
+            for (int r = 2; left > 0; ++r, left -= 4) {
+                const uint4 en = left > 4 ? ep[r * 32] : ez;
                 step(e.x); step(e.y); step(e.z); step(e.w);      // padded with the zero slot
+                e = en;
             }
             for (int o = 1; o < width; o <<= 1)
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
-            if (head) stv<S>(E + (size_t)task.x * S, acc);
+            if (head) stv<S>(E + r0.x * S, acc);
         }
     } else {
         // kAuxT3 / kAuxR3: three sums at once (one for the rates / source-term kernels)
@@ -554,9 +587,9 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
 #pragma unroll
             for (int q = 0; q < S; ++q) acc[w][q] = 0.0;
         if (kind == kAuxT3) {
-            auto step = [&](uint32_t e) {
-                const double cf = entry_coef(e);
-                const double *p = reinterpret_cast<const double *>(Eb + (e & kEntOffMask));
+            auto step = [&](uint32_t w_) {
+                const double cf = entry_coef(w_);
+                const double *p = reinterpret_cast<const double *>(Eb + (w_ & kEntOffMask));
 #pragma unroll
                 for (int w = 0; w < NA; ++w) {
                     double a[S];
@@ -565,9 +598,11 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
                     for (int q = 0; q < S; ++q) acc[w][q] = fma(cf, a[q], acc[w][q]);
                 }
             };
-            for (int t = 0; t < steps; t += 4) {
-                const uint4 e = ep[(t / 4) * 32];
+            if (steps > 0) step(r0.w);
+            for (int r = 2; left > 0; ++r, left -= 4) {
+                const uint4 en = left > 4 ? ep[r * 32] : ez;
                 step(e.x); step(e.y); step(e.z); step(e.w);      // padded with the zero slots
+                e = en;
             }
         } else {
             for (int i = lane; i < nr; i += 32) {
@@ -589,12 +624,12 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
                 for (int q = 0; q < S; ++q) acc[w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[w][q], o);
         constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
         if (kind == kAuxR3) {
-            if ((lane & (width - 1)) == 0) {
+            if (lane == 0) {
                 stv<S>(E + m.eS1 * S, acc[0]);
                 if (LEVEL == 2) { stv<S>(E + m.eA0 * S, acc[iA]); stv<S>(E + m.eS4 * S, acc[iT]); }
             }
         } else if (head) {
-            const uint32_t k = task.x;
+            const uint32_t k = r0.x;
             stv<S>(E + (m.eWdot + k) * S, acc[0]);
             if (LEVEL == 2) {
                 // alpha_{k+1} of Eq. 112 regrouped, and the T column (Eq. 111) straight into the tile
@@ -613,18 +648,24 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
     }
 }
 
-// the chunks [c0, c1) of a phase, round-robin over the warps; the next header is fetched early
+// the chunks [c0, c1) of a phase, round-robin over the warps.  Headers are fetched two chunks
+// ahead, blocks 0 and 1 of a chunk one chunk ahead, so that short lists never wait for a table read.
 template <int LEVEL, int S, int NW>
 __device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, const double *sc, int c0, int c1, int warp,
                                              int lane)
 {
     int ch = c0 + warp;
     if (ch >= c1) return;
-    uint4 h = m.achunk[ch];
+    uint2 h = m.achunk[ch];
+    uint2 h1 = ch + NW < c1 ? m.achunk[ch + NW] : h;
+    uint4 r0 = m.a_ent[h.x + lane];
+    uint4 e1 = (h.y & 0xFFFF) > 1 ? m.a_ent[h.x + 32 + lane] : r0;
     for (; ch < c1; ch += NW) {
-        const uint4 hn = ch + NW < c1 ? m.achunk[ch + NW] : h;
-        gather_chunk<LEVEL, S>(m, E, sc, h, lane);
-        h = hn;
+        const uint2 h2 = ch + 2 * NW < c1 ? m.achunk[ch + 2 * NW] : h;
+        const uint4 r0n = m.a_ent[h1.x + lane];
+        const uint4 e1n = (h1.y & 0xFFFF) > 1 ? m.a_ent[h1.x + 32 + lane] : r0n;
+        gather_chunk<LEVEL, S>(m, E, sc, h, r0, e1, lane);
+        h = h1; h1 = h2; r0 = r0n; e1 = e1n;
     }
 }
 
@@ -742,8 +783,8 @@ __global__ void __launch_bounds__(NT, MB)
         }
         // ---- Jacobian: step p gathers the cells of panel p into its tile buffer (step 0 also
         // finishes the energy row) and streams panel p - 1 out
-        const long long Jstate = (long long)ld * ld;
         const int pw = m.pw, n_panel = m.n_panel;
+        const int nq = (int)min((long long)S, n - state0);       // states of this batch that exist
         for (int p = 0; p <= n_panel; ++p) {
             if (p == 0) {
                 // FIX: the energy row (Eq. 113).  Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 ..
@@ -770,7 +811,7 @@ __global__ void __launch_bounds__(NT, MB)
                             double s = s3[0];
 #pragma unroll
                             for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
-                            const double icp = 1.0 / sc[kCpMix * S + q];
+                            const double icp = sc[kIcp * S + q];
                             const double z = -icp * sc[kIrho * S + q] *
                                              (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
                             E[m.eZ * S + q] = z;
@@ -781,78 +822,79 @@ __global__ void __launch_bounds__(NT, MB)
                         if (c < ns) {
                             const double dx = colc[2 * c];
                             const double wj = wrow[c], iwj = m.inv_mw[c - 1], iwl = m.inv_mw[ns - 1];
+                            double icp[S], irho[S], s1[S], a0[S], gl[S], cpj[S], cpl[S], g0[S], z[S];
+                            ldv<S>(sc + kIcp * S, icp);
+                            ldv<S>(sc + kIrho * S, irho);
+                            ldv<S>(E + m.eS1 * S, s1);
+                            ldv<S>(E + m.eA0 * S, a0);
+                            ldv<S>(E + (m.eG0 + ns - 1) * S, gl);
+                            ldv<S>(Cp + (c - 1) * S, cpj);
+                            ldv<S>(Cp + (ns - 1) * S, cpl);
+                            ldv<S>(E + (m.eG0 + c - 1) * S, g0);
 #pragma unroll
                             for (int q = 0; q < S; ++q) {
-                                const double icp = 1.0 / sc[kCpMix * S + q], irho = sc[kIrho * S + q];
-                                const double a1 = irho * E[m.eS1 * S + q] * icp * icp;     // coefficient of c_pj - c_pNs
-                                const double alpha0 = -(irho * icp) * E[m.eA0 * S + q];
-                                const double gamma0 = -(iwl * icp) * E[(m.eG0 + ns - 1) * S + q];
-                                const double dcp = Cp[(c - 1) * S + q] - Cp[(ns - 1) * S + q];
-                                const double z =
-                                    (wj * (alpha0 * dx - gamma0 + a1 * dcp) - icp * E[(m.eG0 + c - 1) * S + q]) * iwj;
-                                E[(m.eZ + c) * S + q] = z;
-                                if (c < pw) E[(m.eTile + c * ld) * S + q] = z;
+                                const double a1 = irho[q] * s1[q] * icp[q] * icp[q];     // coefficient of c_pj - c_pNs
+                                const double alpha0 = -(irho[q] * icp[q]) * a0[q];
+                                const double gamma0 = -(iwl * icp[q]) * gl[q];
+                                z[q] = (wj * (alpha0 * dx - gamma0 + a1 * (cpj[q] - cpl[q])) - icp[q] * g0[q]) * iwj;
                             }
+                            stv<S>(E + (m.eZ + c) * S, z);
+                            if (c < pw) stv<S>(E + (m.eTile + c * ld) * S, z);
                         }
                     }
                 }
             }
             if (p < n_panel) gather_phase<2, S, NW>(m, E, sc, m.panel_ptr[p], m.panel_ptr[p + 1], warp, lane);
             if (p >= 1) {
-                // DENSE: J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c  (Eq. 112 regrouped); a warp
-                // owns a slab of rows and walks a segment of columns
+                // DENSE: J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c  (Eq. 112 regrouped).  A warp
+                // owns one slab of rows (two rows per lane when ld is even) and walks every
+                // (NW / n_slab)-th column of the panel; all offsets are 32-bit.
                 const int pp = p - 1;
                 const int c0 = pp * pw, ncol = min(ld, c0 + pw) - c0;
-                const double *tile = E + (size_t)(m.eTile + (pp % m.nbuf) * pw * ld) * S;
-                const int seg = m.d_seg, nseg = (ncol + seg - 1) / seg;
-                if (m.pair) {
-                    const int n_slab = (ld + 63) / 64;
-                    for (int it = warp; it < n_slab * nseg; it += NW) {
-                        const int slab = it % n_slab, sg = it / n_slab;
-                        const int ca = sg * seg, cb = min(ncol, ca + seg);
-                        const int r = slab * 64 + 2 * lane;
-                        const bool live = r < ld;
-                        const int rr = live ? r : 0;
+                const int RP = m.pair ? 2 : 1;
+                const int n_slab = (ld + 32 * RP - 1) / (32 * RP);
+                const int cstride = NW >= n_slab ? NW / n_slab : 1;
+                const int slab = NW >= n_slab ? warp % n_slab : 0, cfirst = warp / n_slab;
+                const int n_srep = NW >= n_slab ? 1 : n_slab;            // tiny CTAs: every warp walks all slabs
+                for (int sr = 0; sr < n_srep; ++sr) {
+                    const int r = (slab + sr) * 32 * RP + RP * lane;
+                    if (r >= ld || (NW >= n_slab && cfirst >= cstride)) continue;
+                    const int cbeg = NW >= n_slab ? cfirst : warp, cstep = NW >= n_slab ? cstride : NW;
+                    const uint32_t t_off = (uint32_t)((m.eTile + (pp % m.nbuf) * pw * ld + cbeg * ld + r) * S) * 8u;
+                    const uint32_t t_inc = (uint32_t)(cstep * ld * S) * 8u;
+                    const char *tp = reinterpret_cast<const char *>(E) + t_off;
+                    const char *cc = reinterpret_cast<const char *>(colc + 2 * (c0 + cbeg));
+                    char *Jp = reinterpret_cast<char *>(out.jac + state0 * ((long long)ld * ld) + (long long)(c0 + cbeg) * ld + r);
+                    const uint32_t j_inc = (uint32_t)(cstep * ld) * 8u, j_state = (uint32_t)(ld * ld) * 8u;
+                    if (RP == 2) {
                         double al[2 * S], ga[2 * S];
-                        ldv<2 * S>(E + (m.eAlpha + rr) * S, al);
-                        ldv<2 * S>(E + (m.eGamma + rr) * S, ga);
-                        const double *tp = tile + ((size_t)ca * ld + rr) * S;
-                        const double *cc = colc + 2 * (c0 + ca);
-                        double *Jp = out.jac + state0 * Jstate + (long long)(c0 + ca) * ld + rr;
-                        for (int c = ca; c < cb; ++c, tp += (size_t)ld * S, cc += 2, Jp += ld) {
+                        ldv<2 * S>(E + (m.eAlpha + r) * S, al);
+                        ldv<2 * S>(E + (m.eGamma + r) * S, ga);
+#pragma unroll 2
+                        for (int c = cbeg; c < ncol; c += cstep, tp += t_inc, cc += 16 * cstep, Jp += j_inc) {
                             const double2 dg = *reinterpret_cast<const double2 *>(cc);
                             double t[2 * S];
-                            ldv<2 * S>(tp, t);
+                            ldv<2 * S>(reinterpret_cast<const double *>(tp), t);
 #pragma unroll
                             for (int q = 0; q < S; ++q) {
                                 const double v0 = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
                                 const double v1 = fma(-ga[S + q], dg.y, fma(al[S + q], dg.x, t[S + q]));
-                                if (live && state0 + q < n) st_cs_v2(Jp + q * Jstate, v0, v1);
+                                if (q < nq) st_cs_v2(reinterpret_cast<double *>(Jp + q * j_state), v0, v1);
                             }
                         }
-                    }
-                } else {
-                    const int n_slab = (ld + 31) / 32;
-                    for (int it = warp; it < n_slab * nseg; it += NW) {
-                        const int slab = it % n_slab, sg = it / n_slab;
-                        const int ca = sg * seg, cb = min(ncol, ca + seg);
-                        const int r = slab * 32 + lane;
-                        const bool live = r < ld;
-                        const int rr = live ? r : 0;
+                    } else {
                         double al[S], ga[S];
-                        ldv<S>(E + (m.eAlpha + rr) * S, al);
-                        ldv<S>(E + (m.eGamma + rr) * S, ga);
-                        const double *tp = tile + ((size_t)ca * ld + rr) * S;
-                        const double *cc = colc + 2 * (c0 + ca);
-                        double *Jp = out.jac + state0 * Jstate + (long long)(c0 + ca) * ld + rr;
-                        for (int c = ca; c < cb; ++c, tp += (size_t)ld * S, cc += 2, Jp += ld) {
+                        ldv<S>(E + (m.eAlpha + r) * S, al);
+                        ldv<S>(E + (m.eGamma + r) * S, ga);
+#pragma unroll 2
+                        for (int c = cbeg; c < ncol; c += cstep, tp += t_inc, cc += 16 * cstep, Jp += j_inc) {
                             const double2 dg = *reinterpret_cast<const double2 *>(cc);
                             double t[S];
-                            ldv<S>(tp, t);
+                            ldv<S>(reinterpret_cast<const double *>(tp), t);
 #pragma unroll
                             for (int q = 0; q < S; ++q) {
                                 const double v = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
-                                if (live && state0 + q < n) __stcs(Jp + q * Jstate, v);
+                                if (q < nq) __stcs(reinterpret_cast<double *>(Jp + (size_t)q * j_state), v);
                             }
                         }
                     }

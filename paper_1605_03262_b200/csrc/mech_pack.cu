@@ -46,12 +46,12 @@ struct Task {
     int steps() const { return (int)((n_words + (size_t(1) << rshift) - 1) >> rshift); }
 };
 
-// lanes that share one sum: enough that no lane walks more than 8 entries (kAuxPre of kernels.cu)
+// lanes that share one sum: enough that no lane walks more than `kMaxSteps` entries
+constexpr size_t kMaxSteps = 12;
 int pick_rshift(size_t len)
 {
-    if (len <= 8) return 0;
-    for (int r = 2; r < 5; ++r)
-        if (((len + (size_t(1) << r) - 1) >> r) <= 8) return r;
+    for (int r = 0; r < 5; ++r)
+        if (((len + (size_t(1) << r) - 1) >> r) <= kMaxSteps) return r;
     return 5;
 }
 
@@ -328,7 +328,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             o.th_off[s] = (uint32_t)o.th_data.size();
             o.th_data.push_back((double)nint);
             for (double b : brk) o.th_data.push_back(b);
-            if (nint <= 2) o.th_soa[s] = nint == 2 ? brk[0] : HUGE_VAL;
+            o.th_soa[s] = nint == 2 ? brk[0] : nint == 1 ? HUGE_VAL : std::nan("");
             for (int iv = 0; iv < nint; ++iv) {
                 // interval iv: brk[iv-1] < T <= brk[iv]; species k is in its low range iff T <= t_mid[k]
                 double da[7] = {0, 0, 0, 0, 0, 0, 0};
@@ -398,6 +398,36 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         }
     }
 
+
+    // ---- efficiencies, regrouped per group of 32 reactions (device_mech.h `eff_ent`)
+    {
+        const int n_gen = o.n_rchunk - (int)o.n_plain_chunks;
+        o.eff_base.assign(1, 0);
+        for (int c = 0; c < n_gen; ++c) {
+            int gmax = 0;
+            for (int l = 0; l < 32; ++l) {
+                const int sr = 32 * c + l;
+                if (sr < o.n_pd) gmax = std::max(gmax, o.eff_ptr[sr + 1] - o.eff_ptr[sr]);
+            }
+            for (int e = 0; e < gmax; ++e)
+                for (int l = 0; l < 32; ++l) {
+                    const int sr = 32 * c + l;
+                    uint32_t w0 = (uint32_t)ns | (uint32_t)eDump << 16;
+                    double eps = 0.0;
+                    if (sr < o.n_pd && e < o.eff_ptr[sr + 1] - o.eff_ptr[sr]) {
+                        w0 = o.eff_spec[o.eff_ptr[sr] + e];
+                        eps = o.eff_eps[o.eff_ptr[sr] + e];
+                    }
+                    uint64_t bits;
+                    std::memcpy(&bits, &eps, 8);
+                    o.eff_ent.push_back(w0);
+                    o.eff_ent.push_back(0u);
+                    o.eff_ent.push_back((uint32_t)bits);
+                    o.eff_ent.push_back((uint32_t)(bits >> 32));
+                }
+            o.eff_base.push_back((int32_t)(o.eff_ent.size() / 4));
+        }
+    }
 
     // ---- launch shape: S states per CTA iteration, CTAs per SM, and the width of the column panels
     // of the tile.  Everything lives in shared memory: S x (E + tile + two mixture blocks).
@@ -538,33 +568,36 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         int n01 = 0;
         for (auto &c : chunks) {
             n01 += c.lvl01 ? 1 : 0;
+            // layout (device_mech.h): round 0 holds, per lane, {output index, constant (2 words), entry 0};
+            // round r >= 1 holds entries 4r-3 .. 4r
             const uint32_t base = (uint32_t)(o.a_ent.size() / 4);       // in uint4 units
             const int per = 32 >> c.rshift, width = 1 << c.rshift;
+            const uint32_t pad = c.kind == kAuxH2 ? pad2 : pad1;
             o.achunk.push_back(base);
-            o.achunk.push_back((uint32_t)c.steps);
-            o.achunk.push_back(c.kind | (uint32_t)c.rshift << 8);
-            o.achunk.push_back((uint32_t)(o.a_task.size() / 4));
-            auto push_task = [&](uint32_t out, double cst) {
+            o.achunk.push_back((uint32_t)c.steps | c.kind << 16 | (uint32_t)c.rshift << 20);
+            const int rounds = 1 + (c.steps > 1 ? (c.steps - 1 + 3) / 4 : 0);
+            o.a_ent.resize(o.a_ent.size() + (size_t)rounds * 128, pad);
+            uint32_t *blk = o.a_ent.data() + (size_t)base * 4;
+            for (int lane = 0; lane < 32; ++lane) {
+                const int l = lane / width;
+                uint32_t out = 0xFFFFFFFFu;
+                double cst = 0.0;
+                if (c.kind != kAuxR3 && l < (int)c.t.size()) { out = c.t[l]->out; cst = c.t[l]->cst; }
                 uint64_t bits;
                 std::memcpy(&bits, &cst, 8);
-                o.a_task.push_back(out);
-                o.a_task.push_back(0u);
-                o.a_task.push_back((uint32_t)bits);
-                o.a_task.push_back((uint32_t)(bits >> 32));
-            };
-            if (c.kind == kAuxR3) { push_task(0u, 0.0); continue; }
-            const int rounds = (c.steps + 3) / 4;
-            o.a_ent.resize(o.a_ent.size() + (size_t)rounds * 128, c.kind == kAuxH2 ? pad2 : pad1);
-            for (int l = 0; l < per; ++l) {
-                if (l >= (int)c.t.size()) { push_task(0xFFFFFFFFu, 0.0); continue; }
-                const Task &t = *c.t[l];
-                push_task(t.out, t.cst);
-                encode(t, words);
-                for (size_t e = 0; e < words.size(); ++e) {
-                    const size_t step = e / width, lane = (size_t)l * width + (e % width);
-                    o.a_ent[(size_t)base * 4 + ((step / 4) * 32 + lane) * 4 + (step % 4)] = words[e];
-                }
+                blk[lane * 4 + 0] = out;
+                blk[lane * 4 + 1] = (uint32_t)bits;
+                blk[lane * 4 + 2] = (uint32_t)(bits >> 32);
             }
+            if (c.kind != kAuxR3)
+                for (int l = 0; l < (int)c.t.size(); ++l) {
+                    encode(*c.t[l], words);
+                    for (size_t e = 0; e < words.size(); ++e) {
+                        const size_t step = e / width, lane = (size_t)l * width + (e % width);
+                        const size_t at = step == 0 ? lane * 4 + 3 : ((1 + (step - 1) / 4) * 32 + lane) * 4 + (step - 1) % 4;
+                        blk[at] = words[e];
+                    }
+                }
             step_count += c.steps;
         }
         return std::make_pair((int)chunks.size(), n01);
@@ -605,8 +638,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         o.panel_ptr.push_back(o.panel_ptr.back() + r.first);
     }
     if (o.a_ent.empty()) o.a_ent.assign(128, pad1);
-    if (o.achunk.empty()) o.achunk.assign(4, 0u);
-    if (o.a_task.empty()) o.a_task.assign(4, 0xFFFFFFFFu);
+    if (o.achunk.empty()) o.achunk.assign(2, 0u);
 }
 
 int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const ShapeHints &hints, const char **why)

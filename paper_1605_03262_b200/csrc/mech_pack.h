@@ -22,14 +22,15 @@ struct HostPack {
     std::vector<int32_t> eff_ptr;
     std::vector<uint32_t> eff_spec;
     std::vector<double> eff_eps;
+    std::vector<int32_t> eff_base;        // per general group
+    std::vector<uint32_t> eff_ent;        // uint4 flattened
     std::vector<int32_t> pk_ptr;
     std::vector<double> pk_data;
     int n_rchunk = 0;
     // gathers (device_mech.h): A1 chunks first, then the cell chunks panel by panel
     int n_a1 = 0, n_a1_01 = 0;
-    std::vector<uint32_t> achunk;         // uint4 flattened
+    std::vector<uint32_t> achunk;         // uint2 flattened
     std::vector<uint32_t> a_ent;          // uint4 flattened
-    std::vector<uint32_t> a_task;         // uint4 flattened
     std::vector<int32_t> panel_ptr;       // [n_panel + 1]
     int n_panel = 1, pw = 0, nbuf = 1, eTile = 0, pair = 0;
     int eQ = 0, eH = 0, eAlpha = 0, eGamma = 0, eWdot = 0, eG0 = 0, eZ = 0;
