@@ -102,10 +102,12 @@ struct DeviceMech {
     // Chunks [0, n_a1) are the A1 phase (the first n_a1_01 of them serve rates / dydt too); the
     // chunks of the cells of column panel p are [panel_ptr[p], panel_ptr[p+1]).
     int n_a1, n_a1_01;
-    const uint2 *achunk;        // {first block of a_ent, steps | kind << 16 | rshift << 20}
-    const uint4 *a_ent;         // block r of a chunk = a_ent[first + 32 r + lane].  Block 0: {output E index
-                                // (kAuxT3: species k; ~0 = none), constant factor (fp64 bits, 2 words), entry of
-                                // step 0}; block r >= 1: the entries of steps 4r-3 .. 4r
+    const uint2 *achunk;        // {first block of a_ent, steps | kind << 16 | rshift << 20 | sums per lane << 24}
+    const uint4 *a_ent;         // block r of a chunk = a_ent[first + 32 r + lane].  One sum per lane: block 0 =
+                                // {output E index (kAuxT3: species k; ~0 = none), constant factor (fp64 bits, 2
+                                // words), entry of step 0}; block r >= 1: the entries of steps 4r-3 .. 4r.  Two
+                                // sums A, B per lane (kAuxS1 only): blocks 0 and 1 are the records of A and B,
+                                // block r >= 2 = {A, B of step 2r-3, A, B of step 2r-2}
     const int32_t *panel_ptr;   // [n_panel + 1]
     // ---- the tile: column panels of the Jacobian, state-interleaved like E, element (r, c) of
     // panel p at E index eTile + (p % nbuf) * pw * ld + (c - p * pw) * ld + r

@@ -509,7 +509,8 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
                                              const uint4 r0, const uint4 e1, int lane)
 {
     const uint32_t kind = (ch.y >> 16) & 0xF;
-    const int rshift = (int)(ch.y >> 20), width = 1 << rshift;
+    const int rshift = (int)(ch.y >> 20) & 0xF, width = 1 << rshift;
+    const bool two = (ch.y >> 24) == 2;                  // two sums per lane: `e1` is the record of the second
     const int steps = (int)(ch.y & 0xFFFF);
     const uint4 *ep = m.a_ent + ch.x + lane;
     const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
@@ -521,6 +522,40 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
 
     if (kind == kAuxS1) {
         if (LEVEL == 2) {
+            if (two) {
+                double accA[S], accB[S];
+#pragma unroll
+                for (int q = 0; q < S; ++q) { accA[q] = 0.0; accB[q] = 0.0; }
+                auto step2 = [&](uint32_t wa, uint32_t wb) {
+                    const double ca = entry_coef(wa), cb = entry_coef(wb);
+                    double a[S], b[S];
+                    ldv<S>(reinterpret_cast<const double *>(Eb + (wa & kEntOffMask)), a);
+                    ldv<S>(reinterpret_cast<const double *>(Eb + (wb & kEntOffMask)), b);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) { accA[q] = fma(ca, a[q], accA[q]); accB[q] = fma(cb, b[q], accB[q]); }
+                };
+                uint4 w = left > 0 ? ep[64] : ez;
+                if (steps > 0) step2(r0.w, e1.w);
+                for (int r = 3; left > 0; ++r, left -= 2) {
+                    const uint4 wn = left > 2 ? ep[r * 32] : ez;
+                    step2(w.x, w.y);
+                    if (left > 1) step2(w.z, w.w);
+                    w = wn;
+                }
+                if (r0.x != 0xFFFFFFFFu) {
+                    const double cst = __hiloint2double((int)r0.z, (int)r0.y);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) accA[q] *= cst;
+                    stv<S>(E + r0.x * S, accA);
+                }
+                if (e1.x != 0xFFFFFFFFu) {
+                    const double cst = __hiloint2double((int)e1.z, (int)e1.y);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) accB[q] *= cst;
+                    stv<S>(E + e1.x * S, accB);
+                }
+                return;
+            }
             double acc[S];
 #pragma unroll
             for (int q = 0; q < S; ++q) acc[q] = 0.0;
@@ -648,8 +683,14 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
     }
 }
 
-// the chunks [c0, c1) of a phase, round-robin over the warps.  Headers are fetched two chunks
-// ahead, blocks 0 and 1 of a chunk one chunk ahead, so that short lists never wait for a table read.
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// blocks 0 and 1 of a chunk are needed as soon as it starts (block 1: steps 1..4, or the second record)
+__device__ __forceinline__ bool has_block1(uint2 h) { return (h.y & 0xFFFF) > 1 || (h.y >> 24) == 2; }
+
+// the chunks [c0, c1) of a phase, round-robin over the warps.  Headers run three chunks ahead, an
+// L1 prefetch of a chunk's first blocks two chunks ahead, its blocks 0 and 1 (registers) one chunk
+// ahead: no table read sits on the critical path of a short list.
 template <int LEVEL, int S, int NW>
 __device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, const double *sc, int c0, int c1, int warp,
                                              int lane)
@@ -658,14 +699,20 @@ __device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, con
     if (ch >= c1) return;
     uint2 h = m.achunk[ch];
     uint2 h1 = ch + NW < c1 ? m.achunk[ch + NW] : h;
+    uint2 h2 = ch + 2 * NW < c1 ? m.achunk[ch + 2 * NW] : h;
     uint4 r0 = m.a_ent[h.x + lane];
-    uint4 e1 = (h.y & 0xFFFF) > 1 ? m.a_ent[h.x + 32 + lane] : r0;
+    uint4 e1 = has_block1(h) ? m.a_ent[h.x + 32 + lane] : r0;
     for (; ch < c1; ch += NW) {
-        const uint2 h2 = ch + 2 * NW < c1 ? m.achunk[ch + 2 * NW] : h;
+        const uint2 h3 = ch + 3 * NW < c1 ? m.achunk[ch + 3 * NW] : h;
+        if (ch + 2 * NW < c1) {
+            prefetch_l1(m.a_ent + h2.x + lane);
+            prefetch_l1(m.a_ent + h2.x + 32 + lane);
+            prefetch_l1(m.a_ent + h2.x + 64 + lane);
+        }
         const uint4 r0n = m.a_ent[h1.x + lane];
-        const uint4 e1n = (h1.y & 0xFFFF) > 1 ? m.a_ent[h1.x + 32 + lane] : r0n;
+        const uint4 e1n = has_block1(h1) ? m.a_ent[h1.x + 32 + lane] : r0n;
         gather_chunk<LEVEL, S>(m, E, sc, h, r0, e1, lane);
-        h = h1; h1 = h2; r0 = r0n; e1 = e1n;
+        h = h1; h1 = h2; h2 = h3; r0 = r0n; e1 = e1n;
     }
 }
 
@@ -705,9 +752,7 @@ __global__ void __launch_bounds__(NT, MB)
     if (tid < S) {   // the empty-slot dummy species, the zero slots, row 0 of alpha / gamma
         sm[(sp.P0 + sp.oX + ns) * S + tid] = 1.0;
         sm[(sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
-        E[m.eZero * S + tid] = 0.0;
-        E[(m.eZero + 1) * S + tid] = 0.0;
-        E[(m.eZero + 2) * S + tid] = 0.0;
+        for (int z = 0; z < 18; ++z) E[(m.eZero + z) * S + tid] = 0.0;      // mech_pack.cu kZeroSlots
         E[m.eAlpha * S + tid] = 0.0;
         E[m.eGamma * S + tid] = 0.0;
         if (nr == 0) { E[m.eS1 * S + tid] = 0.0; E[m.eA0 * S + tid] = 0.0; E[m.eS4 * S + tid] = 0.0; }

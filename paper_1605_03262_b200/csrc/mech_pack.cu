@@ -48,6 +48,7 @@ struct Task {
 
 // lanes that share one sum: enough that no lane walks more than `kMaxSteps` entries
 constexpr size_t kMaxSteps = 12;
+constexpr int kZeroSlots = 18;     // >= lanes of one shared-memory wavefront (16 at S = 1) + 2
 int pick_rshift(size_t len)
 {
     for (int r = 0; r < 5; ++r)
@@ -254,7 +255,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     const int eQ = take(3 * nr), eH = take(nr);
     auto take2 = [&](int n) { next_slot = (next_slot + 1) & ~1; return take(n); };      // even: read in pairs of rows
     const int eAlpha = take2(ld), eGamma = take2(ld), eWdot = take(ns), eG0 = take(ns), eZ = take(ld);
-    const int eS1 = take(1), eA0 = take(1), eS4 = take(1), eZero = take(3), eDump = take(1);   // three zero slots: kAuxT3 pads read q, a, Theta
+    const int eS1 = take(1), eA0 = take(1), eS4 = take(1), eZero = take(kZeroSlots), eDump = take(1);   // zero slots: one per bank group, plus two (kAuxT3 pads read q, a, Theta)
     o.eQ = eQ; o.eH = eH; o.eAlpha = eAlpha; o.eGamma = eGamma; o.eWdot = eWdot;
     o.eG0 = eG0; o.eZ = eZ; o.eS1 = eS1; o.eA0 = eA0; o.eS4 = eS4; o.eZero = eZero; o.eDump = eDump;
     next_slot = (next_slot + 1) & ~1;
@@ -529,7 +530,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
 
     // ---- chunks: sums of one kind, shared by equally many lanes and of similar length, fill the 32
     // lanes of a chunk; the warps take the chunks of a phase round-robin, most expensive first.
-    struct Chunk { std::vector<Task *> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; };
+    struct Chunk { std::vector<Task *> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; int tpl; };
     std::vector<uint32_t> words;
     auto emit_phase = [&](std::vector<Task> &tasks, bool with_r3, long long &step_count) {
         for (auto &t : tasks) {
@@ -538,7 +539,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             t.rshift = pick_rshift(t.n_words);
         }
         std::vector<Chunk> chunks;
-        if (with_r3 && nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0});
+        if (with_r3 && nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0, 1});
         std::vector<Task *> idx;
         for (auto &t : tasks) idx.push_back(&t);
         std::stable_sort(idx.begin(), idx.end(), [&](const Task *a, const Task *b) {
@@ -548,18 +549,20 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         });
         for (size_t p = 0; p < idx.size();) {
             const Task &t0 = *idx[p];
-            Chunk c{{}, t0.kind, t0.rshift, 0, t0.lvl01, 0.0};
-            const size_t per = (size_t)32 >> t0.rshift;
+            Chunk c{{}, t0.kind, t0.rshift, 0, t0.lvl01, 0.0, 1};
+            // single-sum lists without lane sharing: two sums per lane (independent accumulators)
+            const size_t per = (t0.kind == kAuxS1 && t0.rshift == 0) ? 64 : (size_t)32 >> t0.rshift;
             while (p < idx.size() && c.t.size() < per && idx[p]->kind == c.kind && idx[p]->rshift == c.rshift) {
                 c.steps = std::max(c.steps, idx[p]->steps());
                 c.t.push_back(idx[p++]);
             }
+            c.tpl = c.t.size() > 32 ? 2 : 1;
             chunks.push_back(c);
         }
         for (auto &c : chunks) {
             const double per_step = c.kind == kAuxT3 ? 3.0 : c.kind == kAuxR3 ? 4.0 : c.kind == kAuxH2 ? 1.5 : 1.0;
             const double sums = (c.kind == kAuxT3 || c.kind == kAuxR3) ? 3.0 : 1.0;
-            c.cost = per_step * c.steps + 1.0 * sums * c.rshift + 3.0;
+            c.cost = per_step * c.steps * c.tpl + 1.0 * sums * c.rshift + 3.0;
         }
         std::stable_sort(chunks.begin(), chunks.end(), [&](const Chunk &a, const Chunk &b) {
             if (a.lvl01 != b.lvl01) return a.lvl01;
@@ -568,36 +571,140 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         int n01 = 0;
         for (auto &c : chunks) {
             n01 += c.lvl01 ? 1 : 0;
-            // layout (device_mech.h): round 0 holds, per lane, {output index, constant (2 words), entry 0};
-            // round r >= 1 holds entries 4r-3 .. 4r
+            // layout (device_mech.h)
             const uint32_t base = (uint32_t)(o.a_ent.size() / 4);       // in uint4 units
-            const int per = 32 >> c.rshift, width = 1 << c.rshift;
+            const int width = 1 << c.rshift;
             const uint32_t pad = c.kind == kAuxH2 ? pad2 : pad1;
             o.achunk.push_back(base);
-            o.achunk.push_back((uint32_t)c.steps | c.kind << 16 | (uint32_t)c.rshift << 20);
-            const int rounds = 1 + (c.steps > 1 ? (c.steps - 1 + 3) / 4 : 0);
+            o.achunk.push_back((uint32_t)c.steps | c.kind << 16 | (uint32_t)c.rshift << 20 | (uint32_t)c.tpl << 24);
+            const int rounds = c.tpl == 2 ? 2 + (c.steps > 1 ? (c.steps - 1 + 1) / 2 : 0)
+                                          : 1 + (c.steps > 1 ? (c.steps - 1 + 3) / 4 : 0);
             o.a_ent.resize(o.a_ent.size() + (size_t)rounds * 128, pad);
             uint32_t *blk = o.a_ent.data() + (size_t)base * 4;
-            for (int lane = 0; lane < 32; ++lane) {
-                const int l = lane / width;
-                uint32_t out = 0xFFFFFFFFu;
-                double cst = 0.0;
-                if (c.kind != kAuxR3 && l < (int)c.t.size()) { out = c.t[l]->out; cst = c.t[l]->cst; }
-                uint64_t bits;
-                std::memcpy(&bits, &cst, 8);
-                blk[lane * 4 + 0] = out;
-                blk[lane * 4 + 1] = (uint32_t)bits;
-                blk[lane * 4 + 2] = (uint32_t)(bits >> 32);
-            }
+            // ---- which sum sits on which lane(s), and in which order its entries are walked, is free:
+            // both are chosen greedily so that the lanes of one shared-memory wavefront (LP lanes, one
+            // load granule each) hit different bank groups at every step
+            const int per_row = 32 / width, nslot = c.tpl * per_row;
+            const int gsz = std::min(8 * S, 16), LP = 128 / gsz, nq = 32 / LP;
+            const int nstream = c.kind == kAuxH2 ? 2 : 1;
+            auto granules = [&](uint32_t w, uint32_t g[2]) {
+                if (c.kind == kAuxH2) { g[0] = (w & 0xFFFF) * S * 8 / gsz; g[1] = (w >> 16) * S * 8 / gsz; }
+                else g[0] = (w & kEntOffMask) / gsz;
+            };
+            // occ[((row * steps + step) * nq + quarter) * nstream + stream] = granules read there
+            std::vector<std::vector<uint32_t>> occ((size_t)c.tpl * std::max(c.steps, 1) * nq * nstream);
+            auto cell_of = [&](int row, int step, int lane, int st) -> std::vector<uint32_t> & {
+                return occ[(((size_t)row * c.steps + step) * nq + lane / LP) * nstream + st];
+            };
+            auto clash = [&](const std::vector<uint32_t> &v, uint32_t g) {
+                bool same_bank = false;
+                for (uint32_t x : v) {
+                    if (x == g) return 0;                  // same address: broadcast
+                    same_bank = same_bank || (x % LP == g % LP);
+                }
+                return same_bank ? 1 : 0;
+            };
+            std::vector<int> slot_task(nslot, -1);
+            std::vector<char> taken(c.t.size(), 0);
+            std::vector<std::vector<uint32_t>> tw(c.t.size());
             if (c.kind != kAuxR3)
-                for (int l = 0; l < (int)c.t.size(); ++l) {
-                    encode(*c.t[l], words);
-                    for (size_t e = 0; e < words.size(); ++e) {
-                        const size_t step = e / width, lane = (size_t)l * width + (e % width);
-                        const size_t at = step == 0 ? lane * 4 + 3 : ((1 + (step - 1) / 4) * 32 + lane) * 4 + (step - 1) % 4;
-                        blk[at] = words[e];
+                for (size_t i = 0; i < c.t.size(); ++i) { encode(*c.t[i], words); tw[i] = words; }
+            std::vector<std::vector<int>> where(c.t.size());     // per task: slot (lane * steps + step) of each entry
+            std::vector<char> used;
+            auto place = [&](int ti, int sl, bool commit) {
+                const int row = sl / per_row, lane0 = (sl % per_row) * width;
+                used.assign((size_t)width * std::max(c.steps, 1), 0);
+                int cost = 0;
+                if (commit) where[ti].clear();
+                for (uint32_t w : tw[ti]) {
+                    uint32_t g[2];
+                    granules(w, g);
+                    int best = -1, bc = 1 << 30;
+                    for (int st = 0; st < c.steps && bc > 0; ++st)
+                        for (int j = 0; j < width; ++j) {
+                            if (used[(size_t)j * c.steps + st]) continue;
+                            int cc = 0;
+                            for (int k = 0; k < nstream; ++k) cc += clash(cell_of(row, st, lane0 + j, k), g[k]);
+                            if (cc < bc) { bc = cc; best = j * c.steps + st; }
+                            if (bc == 0) break;
+                        }
+                    used[best] = 1;
+                    cost += bc;
+                    if (commit) {
+                        where[ti].push_back(best);
+                        for (int k = 0; k < nstream; ++k) cell_of(row, best % c.steps, lane0 + best / c.steps, k).push_back(g[k]);
                     }
                 }
+                return cost;
+            };
+            if (c.kind != kAuxR3) {
+                size_t first_free = 0;
+                for (int sl = 0; sl < nslot && first_free < c.t.size(); ++sl) {
+                    int pick = -1, pc = 1 << 30, seen = 0;
+                    for (size_t i = first_free; i < c.t.size() && seen < 12 && pc > 0; ++i) {
+                        if (taken[i]) continue;
+                        ++seen;
+                        const int cc = place((int)i, sl, false);
+                        if (cc < pc) { pc = cc; pick = (int)i; }
+                    }
+                    if (pick < 0) break;
+                    place(pick, sl, true);
+                    taken[pick] = 1;
+                    slot_task[sl] = pick;
+                    while (first_free < c.t.size() && taken[first_free]) ++first_free;
+                }
+            }
+            auto word_at = [&](int row, int lane, int step) -> uint32_t & {
+                size_t at;
+                if (c.tpl == 2)
+                    at = step == 0 ? ((size_t)row * 32 + lane) * 4 + 3
+                                   : ((size_t)(2 + (step - 1) / 2) * 32 + lane) * 4 + 2 * ((step - 1) % 2) + row;
+                else
+                    at = step == 0 ? (size_t)lane * 4 + 3 : ((size_t)(1 + (step - 1) / 4) * 32 + lane) * 4 + (step - 1) % 4;
+                return blk[at];
+            };
+            for (int row = 0; row < c.tpl; ++row)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const int sl = row * per_row + lane / width, ti = slot_task[sl];
+                    uint32_t out = 0xFFFFFFFFu;
+                    double cst = 0.0;
+                    if (ti >= 0) { out = c.t[ti]->out; cst = c.t[ti]->cst; }
+                    uint64_t bits;
+                    std::memcpy(&bits, &cst, 8);
+                    uint32_t *rec = blk + ((size_t)row * 32 + lane) * 4;
+                    rec[0] = out;
+                    rec[1] = (uint32_t)bits;
+                    rec[2] = (uint32_t)(bits >> 32);
+                }
+            if (c.kind != kAuxR3) {
+                std::vector<char> filled((size_t)c.tpl * 32 * std::max(c.steps, 1), 0);
+                for (int sl = 0; sl < nslot; ++sl) {
+                    const int ti = slot_task[sl];
+                    if (ti < 0) continue;
+                    const int row = sl / per_row, lane0 = (sl % per_row) * width;
+                    for (size_t e = 0; e < tw[ti].size(); ++e) {
+                        const int lane = lane0 + where[ti][e] / c.steps, step = where[ti][e] % c.steps;
+                        word_at(row, lane, step) = tw[ti][e];
+                        filled[((size_t)row * 32 + lane) * c.steps + step] = 1;
+                    }
+                }
+                // pads: coefficient 0 (kAuxH2: zero times zero) on the zero slot whose bank group is free
+                for (int row = 0; row < c.tpl; ++row)
+                    for (int step = 0; step < c.steps; ++step)
+                        for (int lane = 0; lane < 32; ++lane) {
+                            if (filled[((size_t)row * 32 + lane) * c.steps + step]) continue;
+                            int z = 0;
+                            for (int t = 0; t < LP; ++t) {
+                                const uint32_t g = (uint32_t)(eZero + t) * S * 8 / gsz;
+                                bool ok = true;
+                                for (int k = 0; k < nstream; ++k) ok = ok && clash(cell_of(row, step, lane, k), g) == 0;
+                                if (ok) { z = t; break; }
+                            }
+                            const uint32_t zi = (uint32_t)(eZero + z);
+                            for (int k = 0; k < nstream; ++k) cell_of(row, step, lane, k).push_back(zi * S * 8 / gsz);
+                            word_at(row, lane, step) = c.kind == kAuxH2 ? (zi | zi << 16) : zi * S * 8;
+                        }
+            }
             step_count += c.steps;
         }
         return std::make_pair((int)chunks.size(), n01);
