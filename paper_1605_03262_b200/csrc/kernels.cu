@@ -223,10 +223,17 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     const int snu_r = meta_nu(meta, 3) + meta_nu(meta, 4) + meta_nu(meta, 5);
     const bool pdep = type == PYJAC_THIRD_BODY || type == PYJAC_FALLOFF || type == PYJAC_CHEM_ACTIVATED;
     const bool arrh = type != PYJAC_PLOG && type != PYJAC_CHEBYSHEV;
-    double lnA = 0.0, beta = 0.0, Ta = 0.0;
-    if (arrh) { lnA = m.lnA[s]; beta = m.beta[s]; Ta = m.Ta[s]; }
-    const double dnu = (double)(snu_r - snu_f);
+    // every table read of the reaction is issued here, before the first use, so that the reads
+    // overlap (one L2 round trip instead of one per parameter group); indices are clamped, the values
+    // of reactions that do not use them are ignored
     const double brk = m.th_soa[s];             // NaN: more than two intervals, see th_data
+    const double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
+    const int s_pd = min(s, max(m.n_pd, 1) - 1);
+    const double lo_lnA = m.lo_lnA[s_pd], lo_beta = m.lo_beta[s_pd], lo_Ta = m.lo_Ta[s_pd];
+    double fp[5];
+#pragma unroll
+    for (int i = 0; i < 5; ++i) fp[i] = m.fall_par[5 * s_pd + i];
+    const double dnu = (double)(snu_r - snu_f);
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
     if (LEVEL == 2) {
         const uint4 vi = m.vidx[s];
@@ -250,8 +257,8 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             lnkf = lnkinf;
             L = (beta + Ta * invT) * invT;                          // Eq. 65
             if (type == PYJAC_FALLOFF || type == PYJAC_CHEM_ACTIVATED) {
-                const double b0 = m.lo_beta[s], Ta0 = m.lo_Ta[s];
-                lnk0 = m.lo_lnA[s] + b0 * lnT - Ta0 * invT;
+                const double b0 = lo_beta, Ta0 = lo_Ta;
+                lnk0 = lo_lnA + b0 * lnT - Ta0 * invT;
                 lPrT = invT * (b0 - beta + (Ta0 - Ta) * invT - 1.0);   // Eq. 84 / P_r
                 if (type == PYJAC_CHEM_ACTIVATED) { lnkf = lnk0; L = (b0 + Ta0 * invT) * invT; }
             }
@@ -381,7 +388,6 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
                 c = Xi; G = Xi; lPrT = -invT; b = R;                     // Eqs. 79-80
             } else {
                 const double Pr = exp_rate(lnk0 - lnkinf) * Xi;          // Eq. 31
-                const double *fp = m.fall_par + 5 * s;
                 const int form = meta_form(meta);
                 double F = 1.0, gF = 0.0;                                // gF = (P_r/F) dF/dP_r
                 if (form == PYJAC_TROE) {                                // Eqs. 33-35, 90-96
@@ -685,9 +691,6 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
 
 __device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
-// blocks 0 and 1 of a chunk are needed as soon as it starts (block 1: steps 1..4, or the second record)
-__device__ __forceinline__ bool has_block1(uint2 h) { return (h.y & 0xFFFF) > 1 || (h.y >> 24) == 2; }
-
 // the chunks [c0, c1) of a phase, round-robin over the warps.  Headers run three chunks ahead, an
 // L1 prefetch of a chunk's first blocks two chunks ahead, its blocks 0 and 1 (registers) one chunk
 // ahead: no table read sits on the critical path of a short list.
@@ -701,16 +704,18 @@ __device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, con
     uint2 h1 = ch + NW < c1 ? m.achunk[ch + NW] : h;
     uint2 h2 = ch + 2 * NW < c1 ? m.achunk[ch + 2 * NW] : h;
     uint4 r0 = m.a_ent[h.x + lane];
-    uint4 e1 = has_block1(h) ? m.a_ent[h.x + 32 + lane] : r0;
+    uint4 e1 = m.a_ent[h.x + 32 + lane];        // unconditional (a_ent is padded): a select would wait for r0
     for (; ch < c1; ch += NW) {
         const uint2 h3 = ch + 3 * NW < c1 ? m.achunk[ch + 3 * NW] : h;
+#ifdef PYJAC_L1_PREFETCH
         if (ch + 2 * NW < c1) {
             prefetch_l1(m.a_ent + h2.x + lane);
             prefetch_l1(m.a_ent + h2.x + 32 + lane);
             prefetch_l1(m.a_ent + h2.x + 64 + lane);
         }
+#endif
         const uint4 r0n = m.a_ent[h1.x + lane];
-        const uint4 e1n = has_block1(h1) ? m.a_ent[h1.x + 32 + lane] : r0n;
+        const uint4 e1n = m.a_ent[h1.x + 32 + lane];
         gather_chunk<LEVEL, S>(m, E, sc, h, r0, e1, lane);
         h = h1; h1 = h2; h2 = h3; r0 = r0n; e1 = e1n;
     }
@@ -802,7 +807,7 @@ __global__ void __launch_bounds__(NT, MB)
         // ---- A1: sums over the reactions per species / per column
         gather_phase<LEVEL, S, NW>(m, E, sc, 0, LEVEL == 2 ? m.n_a1 : m.n_a1_01, warp, lane);
         PROF_MARK(3);
-        __syncthreads();
+        if (LEVEL != 2) __syncthreads();   // the Jacobian's cell gathers do not read what A1 writes: no barrier
         PROF_MARK(4);
         // ---- outputs of the rates / source-term kernels (Eqs. 7-8, 14)
         if (LEVEL == 0 && out.wdot) {
@@ -831,9 +836,11 @@ __global__ void __launch_bounds__(NT, MB)
         const int pw = m.pw, n_panel = m.n_panel;
         const int nq = (int)min((long long)S, n - state0);       // states of this batch that exist
         for (int p = 0; p <= n_panel; ++p) {
-            if (p == 0) {
-                // FIX: the energy row (Eq. 113).  Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 ..
-                const int nfix = 1 + (ns - 1 + 31) / 32;
+            if (p == 1) {
+                // FIX: the energy row (Eq. 113), stored by the lanes that finish it (DENSE skips row 0).
+                // Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 .. (column ns is zero)
+                const int nfix = 1 + (ns + 31) / 32;
+                double *J0 = out.jac + state0 * ((long long)ld * ld);
                 for (int it = NW - 1 - warp; it < nfix; it += NW) {
                     if (it == 0) {
                         double s3[S];       // sum_k c_pk W_k wdot_k
@@ -859,8 +866,7 @@ __global__ void __launch_bounds__(NT, MB)
                             const double icp = sc[kIcp * S + q];
                             const double z = -icp * sc[kIrho * S + q] *
                                              (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
-                            E[m.eZ * S + q] = z;
-                            E[m.eTile * S + q] = z;
+                            if (q < nq) J0[(long long)q * ld * ld] = z;
                         }
                     } else {
                         const int c = (it - 1) * 32 + lane + 1;
@@ -883,8 +889,13 @@ __global__ void __launch_bounds__(NT, MB)
                                 const double gamma0 = -(iwl * icp[q]) * gl[q];
                                 z[q] = (wj * (alpha0 * dx - gamma0 + a1 * (cpj[q] - cpl[q])) - icp[q] * g0[q]) * iwj;
                             }
-                            stv<S>(E + (m.eZ + c) * S, z);
-                            if (c < pw) stv<S>(E + (m.eTile + c * ld) * S, z);
+#pragma unroll
+                            for (int q = 0; q < S; ++q)
+                                if (q < nq) J0[(long long)q * ld * ld + (long long)c * ld] = z[q];
+                        } else if (c == ns) {
+#pragma unroll
+                            for (int q = 0; q < S; ++q)
+                                if (q < nq) J0[(long long)q * ld * ld + (long long)c * ld] = 0.0;
                         }
                     }
                 }
@@ -924,7 +935,10 @@ __global__ void __launch_bounds__(NT, MB)
                             for (int q = 0; q < S; ++q) {
                                 const double v0 = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
                                 const double v1 = fma(-ga[S + q], dg.y, fma(al[S + q], dg.x, t[S + q]));
-                                if (q < nq) st_cs_v2(reinterpret_cast<double *>(Jp + q * j_state), v0, v1);
+                                if (q < nq) {
+                                    if (r != 0) st_cs_v2(reinterpret_cast<double *>(Jp + q * j_state), v0, v1);
+                                    else __stcs(reinterpret_cast<double *>(Jp + q * j_state) + 1, v1);
+                                }
                             }
                         }
                     } else {
@@ -939,7 +953,7 @@ __global__ void __launch_bounds__(NT, MB)
 #pragma unroll
                             for (int q = 0; q < S; ++q) {
                                 const double v = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
-                                if (q < nq) __stcs(reinterpret_cast<double *>(Jp + (size_t)q * j_state), v);
+                                if (q < nq && r != 0) __stcs(reinterpret_cast<double *>(Jp + (size_t)q * j_state), v);
                             }
                         }
                     }

@@ -532,7 +532,9 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     // lanes of a chunk; the warps take the chunks of a phase round-robin, most expensive first.
     struct Chunk { std::vector<Task *> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; int tpl; };
     std::vector<uint32_t> words;
-    auto emit_phase = [&](std::vector<Task> &tasks, bool with_r3, long long &step_count) {
+    const int NW = o.threads / 32;
+    std::vector<double> a1_load;
+    auto emit_phase = [&](std::vector<Task> &tasks, bool with_r3, long long &step_count, std::vector<double> &load) {
         for (auto &t : tasks) {
             encode(t, words);
             t.n_words = words.size();
@@ -559,15 +561,42 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             c.tpl = c.t.size() > 32 ? 2 : 1;
             chunks.push_back(c);
         }
+        // cost in units of about six instructions: a chunk's fixed part, its steps, its shuffle reduction
         for (auto &c : chunks) {
-            const double per_step = c.kind == kAuxT3 ? 3.0 : c.kind == kAuxR3 ? 4.0 : c.kind == kAuxH2 ? 1.5 : 1.0;
+            const double per_step = c.kind == kAuxT3 ? 2.0 : c.kind == kAuxR3 ? 2.5 : c.kind == kAuxH2 ? 1.5 : 1.0;
             const double sums = (c.kind == kAuxT3 || c.kind == kAuxR3) ? 3.0 : 1.0;
-            c.cost = per_step * c.steps * c.tpl + 1.0 * sums * c.rshift + 3.0;
+            c.cost = 7.0 + per_step * c.steps * c.tpl + 1.0 * sums * c.rshift;
         }
-        std::stable_sort(chunks.begin(), chunks.end(), [&](const Chunk &a, const Chunk &b) {
-            if (a.lvl01 != b.lvl01) return a.lvl01;
-            return a.cost > b.cost;
-        });
+        // the warps take chunk (k * NW + w) in round k: arrange the chunks so that every warp gets about
+        // the same cost (longest first onto the least loaded warp; rows padded with empty chunks).
+        // The chunks the rates / source-term kernels need too come first, in rows of their own.
+        {
+            std::vector<Chunk> arranged;
+            load.resize(NW, 0.0);
+            for (int pass = 0; pass < 2; ++pass) {
+                std::vector<Chunk *> grp;
+                for (auto &c : chunks)
+                    if (c.lvl01 == (pass == 0)) grp.push_back(&c);
+                if (grp.empty()) continue;
+                std::stable_sort(grp.begin(), grp.end(), [](const Chunk *a, const Chunk *b) { return a->cost > b->cost; });
+                std::vector<std::vector<Chunk *>> mine(NW);
+                for (Chunk *c : grp) {
+                    int w = 0;
+                    for (int i = 1; i < NW; ++i)
+                        if (load[i] < load[w]) w = i;
+                    mine[w].push_back(c);
+                    load[w] += c->cost;
+                }
+                size_t rows = 0;
+                for (auto &v : mine) rows = std::max(rows, v.size());
+                for (size_t k = 0; k < rows; ++k)
+                    for (int w = 0; w < NW; ++w) {
+                        if (k < mine[w].size()) arranged.push_back(*mine[w][k]);
+                        else arranged.push_back(Chunk{{}, kAuxS1, 0, 0, pass == 0, 0.0, 1});      // empty chunk
+                    }
+            }
+            chunks.swap(arranged);
+        }
         int n01 = 0;
         for (auto &c : chunks) {
             n01 += c.lvl01 ? 1 : 0;
@@ -711,14 +740,15 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     };
 
     {
-        auto r = emit_phase(a1, true, o.n_a1_steps);
+        auto r = emit_phase(a1, true, o.n_a1_steps, a1_load);
         o.n_a1 = r.first;
         o.n_a1_01 = r.second;
     }
 
-    // ---- the cells, panel by panel.  Column 0 (rows >= 1) is written by the kAuxT3 sums and row 0 of
-    // panel 0 by the FIX step; with several panels every other cell of a panel gets a task (a cell
-    // that is structurally zero in this panel may not be in the panel that used the buffer before).
+    // ---- the cells, panel by panel.  Column 0 (rows >= 1) is written by the kAuxT3 sums; row 0 (the
+    // energy row) never enters the tile, the FIX step stores it.  With several panels every other
+    // cell of a panel gets a task (a cell that is structurally zero in this panel may not be in the
+    // panel that used the buffer before).
     o.panel_ptr.assign(1, o.n_a1);
     for (int p = 0; p < n_panel; ++p) {
         std::vector<Task> tasks;
@@ -726,25 +756,23 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         for (int c = c0; c < c1; ++c)
             for (int r = 0; r < ld; ++r) {
                 if (c == 0 && r >= 1) continue;
-                if (r == 0 && p == 0) continue;
+                if (r == 0) continue;
                 Task t;
                 t.kind = kAuxS1;
                 t.out = (uint32_t)(eTile + (p % nbuf) * pw * ld + (c - c0) * ld + r);
-                if (r == 0) {
-                    if (c < ns) t.ent.push_back({(uint32_t)(eZ + c), 1});
-                } else {
-                    t.ent = cell[(size_t)r + (size_t)c * ld];
-                    if (!t.ent.empty()) t.cst = d->mol_wt[r - 1] * (1.0 / d->mol_wt[c - 1]);
-                }
+                t.ent = cell[(size_t)r + (size_t)c * ld];
+                if (!t.ent.empty()) t.cst = d->mol_wt[r - 1] * (1.0 / d->mol_wt[c - 1]);
                 if (t.ent.empty() && n_panel == 1) continue;
                 o.n_cell_entries += (long long)t.ent.size();
                 tasks.push_back(t);
             }
         o.n_cells += (long long)tasks.size();
-        auto r = emit_phase(tasks, false, o.n_cell_steps);
+        // the cells of panel 0 are gathered in the same phase as the A1 sums: continue their balance
+        std::vector<double> load = p == 0 ? a1_load : std::vector<double>(NW, 0.0);
+        auto r = emit_phase(tasks, false, o.n_cell_steps, load);
         o.panel_ptr.push_back(o.panel_ptr.back() + r.first);
     }
-    if (o.a_ent.empty()) o.a_ent.assign(128, pad1);
+    o.a_ent.resize(o.a_ent.size() + 256, pad1);      // the kernels read one or two blocks past a chunk's last
     if (o.achunk.empty()) o.achunk.assign(2, 0u);
 }
 
