@@ -139,7 +139,7 @@ enum {
 // the S interleaved state blocks come the state-independent tables (colc, wrow), loaded once per CTA.
 struct SmemPlan {
     int E;                              // [n_e + tile]
-    int P0;                             // two mixture blocks of p0size doubles
+    int P0;                             // three mixture blocks of p0size doubles
     int p0size;
     int oX;                             // within a mixture block: [ns+1] concentrations; slot ns = 1 (empty reaction slots)
     int oCp;                            // [ns] c_pk (mass based)
@@ -163,7 +163,7 @@ inline SmemPlan make_smem_plan(int ns, int n_e)
         p.oCp = take(ns) - base;
         p.oScal = take(kNScal) - base;
         p.p0size = o - base;
-        o += p.p0size;
+        o += 2 * p.p0size;
     }
     p.total = o;
     o = 0;

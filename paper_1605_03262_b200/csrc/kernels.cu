@@ -727,12 +727,136 @@ __device__ __forceinline__ void st_cs_v2(double *p, double a, double b)
     asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a), "d"(b) : "memory");
 }
 
+// ---- FIX item `it` of one batch: the energy row (Eq. 113), stored by the lanes that finish it (DENSE
+// skips row 0).  Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 .. (column ns is zero)
+template <int S>
+__device__ __forceinline__ void fix_item(const DeviceMech &m, const double *E, const double *Cp, const double *sc,
+                                         const double *colc, const double *wrow, int it, int lane, double *J0, int nq)
+{
+    const int ns = m.ns, ld = m.ld;
+    const long long Jstate = (long long)ld * ld;
+    if (it == 0) {
+        double s3[S];       // sum_k c_pk W_k wdot_k
+#pragma unroll
+        for (int q = 0; q < S; ++q) s3[q] = 0.0;
+        for (int k = lane; k < ns; k += 32) {
+            const double wk = wrow[k + 1];
+            double cp[S], wd[S];
+            ldv<S>(Cp + k * S, cp);
+            ldv<S>(E + (m.eWdot + k) * S, wd);
+#pragma unroll
+            for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+            for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
+        if (lane < S) {
+            const int q = lane;
+            double s = s3[0];
+#pragma unroll
+            for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
+            const double icp = sc[kIcp * S + q];
+            const double z = -icp * sc[kIrho * S + q] *
+                             (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
+            if (q < nq) J0[q * Jstate] = z;
+        }
+        return;
+    }
+    const int c = (it - 1) * 32 + lane + 1;
+    if (c < ns) {
+        const double dx = colc[2 * c];
+        const double wj = wrow[c], iwj = m.inv_mw[c - 1], iwl = m.inv_mw[ns - 1];
+        double icp[S], irho[S], s1[S], a0[S], gl[S], cpj[S], cpl[S], g0[S];
+        ldv<S>(sc + kIcp * S, icp);
+        ldv<S>(sc + kIrho * S, irho);
+        ldv<S>(E + m.eS1 * S, s1);
+        ldv<S>(E + m.eA0 * S, a0);
+        ldv<S>(E + (m.eG0 + ns - 1) * S, gl);
+        ldv<S>(Cp + (c - 1) * S, cpj);
+        ldv<S>(Cp + (ns - 1) * S, cpl);
+        ldv<S>(E + (m.eG0 + c - 1) * S, g0);
+#pragma unroll
+        for (int q = 0; q < S; ++q) {
+            const double a1 = irho[q] * s1[q] * icp[q] * icp[q];     // coefficient of c_pj - c_pNs
+            const double alpha0 = -(irho[q] * icp[q]) * a0[q];
+            const double gamma0 = -(iwl * icp[q]) * gl[q];
+            const double z = (wj * (alpha0 * dx - gamma0 + a1 * (cpj[q] - cpl[q])) - icp[q] * g0[q]) * iwj;
+            if (q < nq) J0[q * Jstate + (long long)c * ld] = z;
+        }
+    } else if (c == ns) {
+#pragma unroll
+        for (int q = 0; q < S; ++q)
+            if (q < nq) J0[q * Jstate + (long long)c * ld] = 0.0;
+    }
+}
+
+// ---- DENSE item `it` of panel pp: J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c  (Eq. 112 regrouped)
+// for one slab of rows (two rows per lane when ld is even) and m.d_seg columns; 32-bit offsets
+template <int S>
+__device__ __forceinline__ void dense_item(const DeviceMech &m, const double *E, const double *colc, int pp, int it,
+                                           int lane, double *J0, int nq)
+{
+    const int ld = m.ld, pw = m.pw;
+    const int c0 = pp * pw, ncol = min(ld, c0 + pw) - c0;
+    const int RP = m.pair ? 2 : 1;
+    const int n_slab = (ld + 32 * RP - 1) / (32 * RP);
+    const int slab = it % n_slab, cbeg = (it / n_slab) * m.d_seg, cend = min(ncol, cbeg + m.d_seg);
+    const int r = slab * 32 * RP + RP * lane;
+    if (r >= ld) return;
+    const char *tp = reinterpret_cast<const char *>(E) +
+                     (uint32_t)((m.eTile + (pp % m.nbuf) * pw * ld + cbeg * ld + r) * S) * 8u;
+    const uint32_t t_inc = (uint32_t)(ld * S) * 8u, j_inc = (uint32_t)ld * 8u, j_state = (uint32_t)(ld * ld) * 8u;
+    const char *cc = reinterpret_cast<const char *>(colc + 2 * (c0 + cbeg));
+    char *Jp = reinterpret_cast<char *>(J0 + (long long)(c0 + cbeg) * ld + r);
+    if (RP == 2) {
+        double al[2 * S], ga[2 * S];
+        ldv<2 * S>(E + (m.eAlpha + r) * S, al);
+        ldv<2 * S>(E + (m.eGamma + r) * S, ga);
+#pragma unroll 2
+        for (int c = cbeg; c < cend; ++c, tp += t_inc, cc += 16, Jp += j_inc) {
+            const double2 dg = *reinterpret_cast<const double2 *>(cc);
+            double t[2 * S];
+            ldv<2 * S>(reinterpret_cast<const double *>(tp), t);
+#pragma unroll
+            for (int q = 0; q < S; ++q) {
+                const double v0 = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
+                const double v1 = fma(-ga[S + q], dg.y, fma(al[S + q], dg.x, t[S + q]));
+                if (q < nq) {
+                    if (r != 0) st_cs_v2(reinterpret_cast<double *>(Jp + q * j_state), v0, v1);
+                    else __stcs(reinterpret_cast<double *>(Jp + q * j_state) + 1, v1);
+                }
+            }
+        }
+    } else {
+        double al[S], ga[S];
+        ldv<S>(E + (m.eAlpha + r) * S, al);
+        ldv<S>(E + (m.eGamma + r) * S, ga);
+#pragma unroll 2
+        for (int c = cbeg; c < cend; ++c, tp += t_inc, cc += 16, Jp += j_inc) {
+            const double2 dg = *reinterpret_cast<const double2 *>(cc);
+            double t[S];
+            ldv<S>(reinterpret_cast<const double *>(tp), t);
+#pragma unroll
+            for (int q = 0; q < S; ++q) {
+                const double v = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
+                if (q < nq && r != 0) __stcs(reinterpret_cast<double *>(Jp + (size_t)q * j_state), v);
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ int dense_items(const DeviceMech &m, int pp)
+{
+    const int ld = m.ld, c0 = pp * m.pw, ncol = min(ld, c0 + m.pw) - c0;
+    const int RP = m.pair ? 2 : 1;
+    return ((ld + 32 * RP - 1) / (32 * RP)) * ((ncol + m.d_seg - 1) / m.d_seg);
+}
+
 // ---- the kernel ------------------------------------------------------------------------------------
-// Shared memory: S interleaved state blocks of sp.total doubles (E with the tile behind it, two
+// Shared memory: S interleaved state blocks of sp.total doubles (E with the tile behind it, three
 // mixture blocks), then the state-independent column and row constants.  The mixture block (X, Cp,
-// scalars) is double-buffered: P0 of the NEXT batch is an item of this batch's P1 queue.  The last
-// DENSE step of a batch is not followed by a barrier: P1 of the next batch only writes regions of E
-// that DENSE does not read, so the warps that finish early start it at once.
+// scalars) of the NEXT batch is filled as an item of this batch's reaction queue.
 template <int LEVEL, int NT, int S, int MB>
 __global__ void __launch_bounds__(NT, MB)
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
@@ -757,6 +881,7 @@ __global__ void __launch_bounds__(NT, MB)
     if (tid < S) {   // the empty-slot dummy species, the zero slots, row 0 of alpha / gamma
         sm[(sp.P0 + sp.oX + ns) * S + tid] = 1.0;
         sm[(sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
+        sm[(sp.P0 + 2 * sp.p0size + sp.oX + ns) * S + tid] = 1.0;
         for (int z = 0; z < 18; ++z) E[(m.eZero + z) * S + tid] = 0.0;      // mech_pack.cu kZeroSlots
         E[m.eAlpha * S + tid] = 0.0;
         E[m.eGamma * S + tid] = 0.0;
@@ -775,6 +900,90 @@ __global__ void __launch_bounds__(NT, MB)
                                       min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
     }
     __syncthreads();
+    if (LEVEL == 2) {
+        // ---- Jacobian.  Per batch b two kinds of phase alternate:
+        //   Q(b)  one dynamic queue: the reactions of batch b (P1), the mixture of batch b + 1 (P0) and,
+        //         of batch b - 1, the last DENSE step (and the FIX step if there is one panel).  The
+        //         long general-reaction items start first, the short DENSE items fill the tail.
+        //   G(b)  the gathers of batch b: A1 sums and the cells of panel 0 (further panels: cells of
+        //         panel p with the DENSE step of panel p - 1, a barrier after each).
+        // Three mixture blocks rotate: Q(b) reads block b (P1), writes block b + 1 and reads block b - 1 (FIX).
+        const int n_panel = m.n_panel, nfix = 1 + (ns + 31) / 32;
+        const long long Jstate = (long long)ld * ld;
+        long long blk = blockIdx.x, prev = -1;
+        int par = 0, ppar = 0;
+        for (;;) {
+            const bool has_cur = blk < nblk, has_prev = prev >= 0;
+            if (!has_cur && !has_prev) break;
+            const long long state0 = blk * S;
+            double *P0 = sm + (sp.P0 + par * sp.p0size) * S;
+            double *P0n = sm + (sp.P0 + (par == 2 ? 0 : par + 1) * sp.p0size) * S;
+            const double *P0p = sm + (sp.P0 + ppar * sp.p0size) * S;
+            const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S;
+            double *Jprev = out.jac + prev * S * Jstate;
+            const int nq_prev = (int)min((long long)S, n - prev * S);
+#ifdef PYJAC_PROF
+            long long prof_t[12];
+#endif
+            PROF_MARK(0);
+            // ---- Q(blk)
+            const int n_g = has_cur ? n_gen * S : 0;
+            const int i_pl = n_g, i_m = i_pl + (has_cur ? m.n_plain * (S / SP) : 0);
+            const int i_fix = i_m + ((has_cur && blk + gridDim.x < nblk) ? S : 0);
+            const int i_d = i_fix + ((has_prev && n_panel == 1) ? nfix : 0);
+            const int n_q = i_d + (has_prev ? dense_items(m, n_panel - 1) : 0);
+            for (int it = grab(&ctr[0], lane); it < n_q; it = grab(&ctr[0], lane)) {
+                if (it < i_pl) {
+                    const int c = it / S, q = it - c * S;
+                    reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q, out, state0, n);
+                } else if (it < i_m) {
+                    const int j = it - i_pl;
+                    const int c = n_gen + j / (S / SP), q0 = (j % (S / SP)) * SP;
+                    plain_reactions<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q0, out, state0, n);
+                } else if (it < i_fix) {
+                    const int q = it - i_m;
+                    mixture_and_species<LEVEL, S>(m, P0n + sp.oX * S, P0n + sp.oCp * S, P0n + sp.oScal * S, q,
+                                                  min((blk + gridDim.x) * S + q, n - 1), Tg, Pg, Yg, ldy, lane);
+                } else if (it < i_d) {
+                    fix_item<S>(m, E, P0p + sp.oCp * S, P0p + sp.oScal * S, colc, wrow, it - i_fix, lane, Jprev, nq_prev);
+                } else {
+                    dense_item<S>(m, E, colc, n_panel - 1, it - i_d, lane, Jprev, nq_prev);
+                }
+            }
+            PROF_MARK(1);
+            __syncthreads();
+            if (tid == 0) ctr[0] = 0;
+            PROF_MARK(2);
+            if (!has_cur) break;
+            // ---- G(blk)
+            gather_phase<2, S, NW>(m, E, sc, 0, m.n_a1, warp, lane);
+            gather_phase<2, S, NW>(m, E, sc, m.panel_ptr[0], m.panel_ptr[1], warp, lane);
+            PROF_MARK(3);
+            __syncthreads();
+            PROF_MARK(4);
+            if (n_panel > 1) {
+                double *Jcur = out.jac + state0 * Jstate;
+                const int nq = (int)min((long long)S, n - state0);
+                for (int p = 1; p < n_panel; ++p) {
+                    if (p == 1)
+                        for (int it = NW - 1 - warp; it < nfix; it += NW)
+                            fix_item<S>(m, E, P0 + sp.oCp * S, sc, colc, wrow, it, lane, Jcur, nq);
+                    gather_phase<2, S, NW>(m, E, sc, m.panel_ptr[p], m.panel_ptr[p + 1], warp, lane);
+                    const int nd = dense_items(m, p - 1);
+                    for (int it = warp; it < nd; it += NW) dense_item<S>(m, E, colc, p - 1, it, lane, Jcur, nq);
+                    __syncthreads();
+                }
+            }
+#ifdef PYJAC_PROF
+            if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x)
+                printf("PROF w%d Q %lld wait %lld | G %lld wait %lld\n", warp, prof_t[1] - prof_t[0],
+                       prof_t[2] - prof_t[1], prof_t[3] - prof_t[2], prof_t[4] - prof_t[3]);
+#endif
+            prev = blk; ppar = par;
+            blk += gridDim.x; par = par == 2 ? 0 : par + 1;
+        }
+        return;
+    }
     int par = 0;
     for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x, par ^= 1) {
         const long long state0 = blk * S;
@@ -805,9 +1014,9 @@ __global__ void __launch_bounds__(NT, MB)
         if (tid == 0) ctr[0] = 0;
         PROF_MARK(2);
         // ---- A1: sums over the reactions per species / per column
-        gather_phase<LEVEL, S, NW>(m, E, sc, 0, LEVEL == 2 ? m.n_a1 : m.n_a1_01, warp, lane);
+        gather_phase<LEVEL, S, NW>(m, E, sc, 0, m.n_a1_01, warp, lane);
         PROF_MARK(3);
-        if (LEVEL != 2) __syncthreads();   // the Jacobian's cell gathers do not read what A1 writes: no barrier
+        __syncthreads();
         PROF_MARK(4);
         // ---- outputs of the rates / source-term kernels (Eqs. 7-8, 14)
         if (LEVEL == 0 && out.wdot) {
@@ -827,147 +1036,7 @@ __global__ void __launch_bounds__(NT, MB)
                     out.dydt[(state0 + q) * ld + r] = v;
                 }
         }
-        if (LEVEL != 2) {
-            __syncthreads();      // the outputs above read E and the scalars
-            continue;
-        }
-        // ---- Jacobian: step p gathers the cells of panel p into its tile buffer (step 0 also
-        // finishes the energy row) and streams panel p - 1 out
-        const int pw = m.pw, n_panel = m.n_panel;
-        const int nq = (int)min((long long)S, n - state0);       // states of this batch that exist
-        for (int p = 0; p <= n_panel; ++p) {
-            if (p == 1) {
-                // FIX: the energy row (Eq. 113), stored by the lanes that finish it (DENSE skips row 0).
-                // Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 .. (column ns is zero)
-                const int nfix = 1 + (ns + 31) / 32;
-                double *J0 = out.jac + state0 * ((long long)ld * ld);
-                for (int it = NW - 1 - warp; it < nfix; it += NW) {
-                    if (it == 0) {
-                        double s3[S];       // sum_k c_pk W_k wdot_k
-#pragma unroll
-                        for (int q = 0; q < S; ++q) s3[q] = 0.0;
-                        for (int k = lane; k < ns; k += 32) {
-                            const double wk = wrow[k + 1];
-                            double cp[S], wd[S];
-                            ldv<S>(Cp + k * S, cp);
-                            ldv<S>(E + (m.eWdot + k) * S, wd);
-#pragma unroll
-                            for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
-                        }
-#pragma unroll
-                        for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-                            for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
-                        if (lane < S) {
-                            const int q = lane;
-                            double s = s3[0];
-#pragma unroll
-                            for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
-                            const double icp = sc[kIcp * S + q];
-                            const double z = -icp * sc[kIrho * S + q] *
-                                             (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
-                            if (q < nq) J0[(long long)q * ld * ld] = z;
-                        }
-                    } else {
-                        const int c = (it - 1) * 32 + lane + 1;
-                        if (c < ns) {
-                            const double dx = colc[2 * c];
-                            const double wj = wrow[c], iwj = m.inv_mw[c - 1], iwl = m.inv_mw[ns - 1];
-                            double icp[S], irho[S], s1[S], a0[S], gl[S], cpj[S], cpl[S], g0[S], z[S];
-                            ldv<S>(sc + kIcp * S, icp);
-                            ldv<S>(sc + kIrho * S, irho);
-                            ldv<S>(E + m.eS1 * S, s1);
-                            ldv<S>(E + m.eA0 * S, a0);
-                            ldv<S>(E + (m.eG0 + ns - 1) * S, gl);
-                            ldv<S>(Cp + (c - 1) * S, cpj);
-                            ldv<S>(Cp + (ns - 1) * S, cpl);
-                            ldv<S>(E + (m.eG0 + c - 1) * S, g0);
-#pragma unroll
-                            for (int q = 0; q < S; ++q) {
-                                const double a1 = irho[q] * s1[q] * icp[q] * icp[q];     // coefficient of c_pj - c_pNs
-                                const double alpha0 = -(irho[q] * icp[q]) * a0[q];
-                                const double gamma0 = -(iwl * icp[q]) * gl[q];
-                                z[q] = (wj * (alpha0 * dx - gamma0 + a1 * (cpj[q] - cpl[q])) - icp[q] * g0[q]) * iwj;
-                            }
-#pragma unroll
-                            for (int q = 0; q < S; ++q)
-                                if (q < nq) J0[(long long)q * ld * ld + (long long)c * ld] = z[q];
-                        } else if (c == ns) {
-#pragma unroll
-                            for (int q = 0; q < S; ++q)
-                                if (q < nq) J0[(long long)q * ld * ld + (long long)c * ld] = 0.0;
-                        }
-                    }
-                }
-            }
-            if (p < n_panel) gather_phase<2, S, NW>(m, E, sc, m.panel_ptr[p], m.panel_ptr[p + 1], warp, lane);
-            if (p >= 1) {
-                // DENSE: J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c  (Eq. 112 regrouped).  A warp
-                // owns one slab of rows (two rows per lane when ld is even) and walks every
-                // (NW / n_slab)-th column of the panel; all offsets are 32-bit.
-                const int pp = p - 1;
-                const int c0 = pp * pw, ncol = min(ld, c0 + pw) - c0;
-                const int RP = m.pair ? 2 : 1;
-                const int n_slab = (ld + 32 * RP - 1) / (32 * RP);
-                const int cstride = NW >= n_slab ? NW / n_slab : 1;
-                const int slab = NW >= n_slab ? warp % n_slab : 0, cfirst = warp / n_slab;
-                const int n_srep = NW >= n_slab ? 1 : n_slab;            // tiny CTAs: every warp walks all slabs
-                for (int sr = 0; sr < n_srep; ++sr) {
-                    const int r = (slab + sr) * 32 * RP + RP * lane;
-                    if (r >= ld || (NW >= n_slab && cfirst >= cstride)) continue;
-                    const int cbeg = NW >= n_slab ? cfirst : warp, cstep = NW >= n_slab ? cstride : NW;
-                    const uint32_t t_off = (uint32_t)((m.eTile + (pp % m.nbuf) * pw * ld + cbeg * ld + r) * S) * 8u;
-                    const uint32_t t_inc = (uint32_t)(cstep * ld * S) * 8u;
-                    const char *tp = reinterpret_cast<const char *>(E) + t_off;
-                    const char *cc = reinterpret_cast<const char *>(colc + 2 * (c0 + cbeg));
-                    char *Jp = reinterpret_cast<char *>(out.jac + state0 * ((long long)ld * ld) + (long long)(c0 + cbeg) * ld + r);
-                    const uint32_t j_inc = (uint32_t)(cstep * ld) * 8u, j_state = (uint32_t)(ld * ld) * 8u;
-                    if (RP == 2) {
-                        double al[2 * S], ga[2 * S];
-                        ldv<2 * S>(E + (m.eAlpha + r) * S, al);
-                        ldv<2 * S>(E + (m.eGamma + r) * S, ga);
-#pragma unroll 2
-                        for (int c = cbeg; c < ncol; c += cstep, tp += t_inc, cc += 16 * cstep, Jp += j_inc) {
-                            const double2 dg = *reinterpret_cast<const double2 *>(cc);
-                            double t[2 * S];
-                            ldv<2 * S>(reinterpret_cast<const double *>(tp), t);
-#pragma unroll
-                            for (int q = 0; q < S; ++q) {
-                                const double v0 = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
-                                const double v1 = fma(-ga[S + q], dg.y, fma(al[S + q], dg.x, t[S + q]));
-                                if (q < nq) {
-                                    if (r != 0) st_cs_v2(reinterpret_cast<double *>(Jp + q * j_state), v0, v1);
-                                    else __stcs(reinterpret_cast<double *>(Jp + q * j_state) + 1, v1);
-                                }
-                            }
-                        }
-                    } else {
-                        double al[S], ga[S];
-                        ldv<S>(E + (m.eAlpha + r) * S, al);
-                        ldv<S>(E + (m.eGamma + r) * S, ga);
-#pragma unroll 2
-                        for (int c = cbeg; c < ncol; c += cstep, tp += t_inc, cc += 16 * cstep, Jp += j_inc) {
-                            const double2 dg = *reinterpret_cast<const double2 *>(cc);
-                            double t[S];
-                            ldv<S>(reinterpret_cast<const double *>(tp), t);
-#pragma unroll
-                            for (int q = 0; q < S; ++q) {
-                                const double v = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
-                                if (q < nq && r != 0) __stcs(reinterpret_cast<double *>(Jp + (size_t)q * j_state), v);
-                            }
-                        }
-                    }
-                }
-            }
-            PROF_MARK(5 + (p < 2 ? p : 2));
-            if (p < n_panel) __syncthreads();
-        }
-#ifdef PYJAC_PROF
-        if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x)
-            printf("PROF w%d P1 %lld wait %lld | A1 %lld wait %lld | step0 %lld | rest %lld\n", warp,
-                   prof_t[1] - prof_t[0], prof_t[2] - prof_t[1], prof_t[3] - prof_t[2], prof_t[4] - prof_t[3],
-                   prof_t[5] - prof_t[4], prof_t[(n_panel >= 2 ? 7 : 6)] - prof_t[5]);
-#endif
+        __syncthreads();      // the outputs above read E and the scalars
     }
 }
 
