@@ -34,7 +34,7 @@ FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallba
 CPU_SAMPLE = {0: 1024, 1: 8192, 2: 2048, 3: 256}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the Jacobian kernel from the committed
 # `ncu --set full` capture (profiles/), or None where no capture exists for that workload
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {"cfg1_53sp_325rx": 2355041800, "cfg2_111sp_784rx": 10179383432}      # profiles/r1_v8_cfg1_cfg2.md
 
 
 def measured_peaks():
@@ -245,7 +245,7 @@ def main():
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_BYTES.get(c.name), "peak_source": peak_src,
-                "kernel": "pyjac::eval_kernel<2,%d>" % pj.launch_config(r["per_launch"])["threads"],
+                "kernel": "pyjac::eval_kernel<2 (Jacobian), %d threads>" % pj.launch_config(r["per_launch"])["threads"],
                 "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": launch_ms,
                 "launch_config": pj.launch_config(r["per_launch"])}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

@@ -293,3 +293,44 @@ def test_host_buffer_variant_matches_device_variant(torch, PyJac):
     before = pj.kernel_launches()
     pj.eval_jacobian(dT, dP, dY)
     assert pj.kernel_launches() == before + 1
+
+
+# ---------------------------------------------------------------------------------- launch shapes
+@pytest.mark.gpu
+@pytest.mark.parametrize("cfg,n,env", [
+    (1, 301, {"PYJAC_S": "1"}),                                     # one state per CTA iteration
+    (1, 301, {"PYJAC_S": "2", "PYJAC_PW": "7"}),                    # eight column panels, two tile buffers
+    (1, 301, {"PYJAC_S": "4", "PYJAC_CTAS": "1"}),                  # four interleaved states
+    (1, 301, {"PYJAC_S": "2", "PYJAC_CTAS": "1", "PYJAC_THREADS": "1024"}),
+    (0, 1024, {"PYJAC_S": "1", "PYJAC_PW": "5", "PYJAC_THREADS": "128"}),
+    (2, 65, {"PYJAC_S": "1", "PYJAC_CTAS": "2"}),
+])
+def test_launch_shapes(torch, PyJac, monkeypatch, cfg, n, env):
+    """Every launch shape the tuning hooks can select (states per CTA iteration, column panels of the
+    tile, CTA size) evaluates the same Jacobian: parity with the oracle within the same tolerance,
+    ragged last batch included."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    m = synth.make_mechanism(cfg)
+    T, P, Y = synth.config_states(cfg, n)
+    pj = PyJac(m)
+    o = Oracle(m)
+    check_jacobian(torch, pj, o, T, P, Y)
+    check_rates(torch, pj, o, T[:64], P[:64], Y[:64])
+
+
+@pytest.mark.gpu
+def test_output_pointer_not_16_byte_aligned(torch, PyJac):
+    """An output pointer that is only 8-byte aligned takes the 8-byte store path; same numbers."""
+    m = synth.make_mechanism(0)
+    pj = PyJac(m)
+    T, P, Y = synth.config_states(0, 257)
+    dT, dP, dY = dev(torch, T, P, Y)
+    J = pj.eval_jacobian(dT, dP, dY)
+    ld = m.n_species + 1
+    buf = torch.zeros(257 * ld * ld + 1, dtype=torch.float64, device="cuda")
+    view = buf[1:]
+    assert view.data_ptr() % 16 == 8
+    pj.eval_jacobian(dT, dP, dY, out=view)
+    assert torch.equal(view.reshape(257, ld * ld), J)
+    assert float(buf[0]) == 0.0
