@@ -174,15 +174,20 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
         for (int u = 0; u < SP; ++u) kf[u] = exp_rate(lnkf[u]);
 #pragma unroll
         for (int u = 0; u < SP; ++u) { kr[u] = exp_rate(lnkf[u] - sB[u]); kr[u] = rev ? kr[u] : 0.0; }   // Eqs. 23-27
+        // the SP states of one element are neighbours in shared memory: one 16-byte access for both
+        double c[6][SP], W[SP], vq[3][SP], vh[SP], vs[6][SP];
+        ldv<SP>(X + x0 + q0, c[0]); ldv<SP>(X + x1 + q0, c[1]); ldv<SP>(X + x2 + q0, c[2]);
+        ldv<SP>(X + x3 + q0, c[3]); ldv<SP>(X + x4 + q0, c[4]); ldv<SP>(X + x5 + q0, c[5]);
+        if (LEVEL == 2) ldv<SP>(sc + kW * S + q0, W);
 #pragma unroll
         for (int u = 0; u < SP; ++u) {
             const int q = q0 + u;
-            const double c0 = X[x0 + q], c1 = X[x1 + q], c2 = X[x2 + q], c3 = X[x3 + q], c4 = X[x4 + q], c5 = X[x5 + q];
+            const double c0 = c[0][u], c1 = c[1][u], c2 = c[2][u], c3 = c[3][u], c4 = c[4][u], c5 = c[5][u];
             const double p01 = c0 * c1, p34 = c3 * c4;
             const double Rf = kf[u] * (p01 * c2), Rr = kr[u] * (p34 * c5);       // Eqs. 18-19
             const double R = Rf - Rr;
-            E[(m.eQ + 3 * s) * S + q] = R;
-            if (LEVEL >= 1) E[(m.eH + s) * S + q] = kRu * T[u] * fma(T[u], sdB[u], dnu);
+            vq[0][u] = R;
+            vh[u] = kRu * T[u] * fma(T[u], sdB[u], dnu);
             if (LEVEL == 0) {
                 const long long st = state0 + q;
                 if (st < n) {
@@ -193,17 +198,24 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
                 }
             }
             if (LEVEL == 2) {
-                const double W = sc[kW * S + q];
                 const double iT = invT[u];
                 // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
                 const double dRf = Rf * fma(-snf, iT, L[u]);
                 const double dRr = Rr * (fma(-snr, iT, L[u]) - sdB[u]);
-                E[(m.eQ + 3 * s + 2) * S + q] = fma(R, iT, dRf - dRr);
-                E[(m.eQ + 3 * s + 1) * S + q] = W * (R - fma(Rf, snf, -Rr * snr));
+                vq[2][u] = fma(R, iT, dRf - dRr);
+                vq[1][u] = W[u] * (R - fma(Rf, snf, -Rr * snr));
                 const double nkr = -kr[u];
-                E[v0 + q] = kf[u] * (c1 * c2); E[v1 + q] = kf[u] * (c0 * c2); E[v2 + q] = kf[u] * p01;   // Eq. 120
-                E[v3 + q] = nkr * (c4 * c5); E[v4 + q] = nkr * (c3 * c5); E[v5 + q] = nkr * p34;         // Eq. 121
+                vs[0][u] = kf[u] * (c1 * c2); vs[1][u] = kf[u] * (c0 * c2); vs[2][u] = kf[u] * p01;   // Eq. 120
+                vs[3][u] = nkr * (c4 * c5); vs[4][u] = nkr * (c3 * c5); vs[5][u] = nkr * p34;         // Eq. 121
             }
+        }
+        stv<SP>(E + (m.eQ + 3 * s) * S + q0, vq[0]);
+        if (LEVEL >= 1) stv<SP>(E + (m.eH + s) * S + q0, vh);
+        if (LEVEL == 2) {
+            stv<SP>(E + (m.eQ + 3 * s + 1) * S + q0, vq[1]);
+            stv<SP>(E + (m.eQ + 3 * s + 2) * S + q0, vq[2]);
+            stv<SP>(E + v0 + q0, vs[0]); stv<SP>(E + v1 + q0, vs[1]); stv<SP>(E + v2 + q0, vs[2]);
+            stv<SP>(E + v3 + q0, vs[3]); stv<SP>(E + v4 + q0, vs[4]); stv<SP>(E + v5 + q0, vs[5]);
         }
     }
 }

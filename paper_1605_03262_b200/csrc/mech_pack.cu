@@ -46,15 +46,17 @@ struct Task {
     int steps() const { return (int)((n_words + (size_t(1) << rshift) - 1) >> rshift); }
 };
 
-// lanes that share one sum: enough that no lane walks more than `kMaxSteps` entries
-constexpr size_t kMaxSteps = 12;
-constexpr int kZeroSlots = 18;     // >= lanes of one shared-memory wavefront (16 at S = 1) + 2
-int pick_rshift(size_t len)
+// lanes that share one sum: enough that no lane walks more than `cap` entries.  Long lists on one
+// lane cost the fewest instructions (no padding, no shuffle reduction) but make long chunks: with two
+// CTAs per SM the other CTA fills the tail (measured: cfg1 2.79 -> 2.77 ms with cap 32), with one CTA
+// per SM and a barrier per column panel they do not (cfg2 10.8 -> 13.8 ms), so the cap follows the shape.
+int pick_rshift(size_t len, size_t cap)
 {
     for (int r = 0; r < 5; ++r)
-        if (((len + (size_t(1) << r) - 1) >> r) <= kMaxSteps) return r;
+        if (((len + (size_t(1) << r) - 1) >> r) <= cap) return r;
     return 5;
 }
+constexpr int kZeroSlots = 18;     // >= lanes of one shared-memory wavefront (16 at S = 1) + 2
 
 void validate(const pyjac_mech_desc *d)
 {
@@ -538,7 +540,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         for (auto &t : tasks) {
             encode(t, words);
             t.n_words = words.size();
-            t.rshift = pick_rshift(t.n_words);
+            t.rshift = pick_rshift(t.n_words, o.ctas_target >= 2 ? 32 : 12);
         }
         std::vector<Chunk> chunks;
         if (with_r3 && nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0, 1});
