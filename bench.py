@@ -184,6 +184,22 @@ def bench_config(torch, cfg, steps, warmup, n_states=None, chunk=None):
                 per_step_ms=per, launches=launches, launches_per_step=len(views), per_launch=per_launch)
 
 
+def max_over_ranks(ms: float, dist, device: str) -> float:
+    """Device-timed milliseconds of the timed region, MAX over the ranks (the only collective of the
+    run: states are independent, every rank evaluates its own replica)."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world: int, n_states_per_rank: int, ms_per_step: float) -> float:
+    """States all ranks evaluated per second ("scaling": "weak": n per rank is fixed)."""
+    return world * n_states_per_rank / (ms_per_step * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -231,14 +247,10 @@ def main():
     r = bench_config(torch, cfg, args.steps, args.warmup, chunk=chunk)
     barrier()
     clocks = sampler.stop()
-    total_ms = r["total_ms"]
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(r["total_ms"], dist, "cuda")
     c, n, pj = r["cfg"], r["n"], r["pj"]
     ms_per_step = total_ms / args.steps
-    value = world * n / (ms_per_step * 1e-3)
+    value = whole_job_value(world, n, ms_per_step)
     peak, peak_src = measured_peaks()
     launch_ms = r["total_ms"] / (args.steps * r["launches_per_step"])
     alg_bytes = algorithmic_bytes(c.n_species, r["per_launch"])

@@ -624,6 +624,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             };
             // occ[((row * steps + step) * nq + quarter) * nstream + stream] = granules read there
             std::vector<std::vector<uint32_t>> occ((size_t)c.tpl * std::max(c.steps, 1) * nq * nstream);
+            // the 16-byte stores of the results (kAuxS1: one per sum, all lanes of a row at once)
+            std::vector<std::vector<uint32_t>> occ_st((size_t)c.tpl * nq);
             auto cell_of = [&](int row, int step, int lane, int st) -> std::vector<uint32_t> & {
                 return occ[(((size_t)row * c.steps + step) * nq + lane / LP) * nstream + st];
             };
@@ -647,6 +649,12 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                 used.assign((size_t)width * std::max(c.steps, 1), 0);
                 int cost = 0;
                 if (commit) where[ti].clear();
+                if (c.kind == kAuxS1) {
+                    auto &st_cell = occ_st[(size_t)row * nq + lane0 / LP];
+                    const uint32_t g = c.t[ti]->out * S * 8 / gsz;
+                    cost += 2 * clash(st_cell, g);
+                    if (commit) st_cell.push_back(g);
+                }
                 for (uint32_t w : tw[ti]) {
                     uint32_t g[2];
                     granules(w, g);
