@@ -124,9 +124,11 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     dm.eQ = hp.eQ; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;
     dm.eWdot = hp.eWdot; dm.eG0 = hp.eG0; dm.eZ = hp.eZ;
     dm.eS1 = hp.eS1; dm.eA0 = hp.eA0; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.eDump = hp.eDump; dm.n_e = hp.n_e;
-    {   // DENSE work items: about two per warp, 2..32 columns each
+    {   // DENSE work items (one slab of rows x seg columns).  Measured (profiles/r1_v8_cfg1_cfg2.md): with one
+        // panel the items sit in the dynamic queue and fewer, longer items win (less set-up per column);
+        // with several panels they are dealt round-robin next to the cell gathers and about 3 columns win.
         const int nw = m->threads / 32, n_slab = (dm.ld + (dm.pair ? 63 : 31)) / (dm.pair ? 64 : 32);
-        int seg = (n_slab * dm.pw + 2 * nw - 1) / (2 * nw);
+        int seg = dm.n_panel == 1 ? (3 * n_slab * dm.pw + 2 * nw - 1) / (2 * nw) : 3;
         seg = seg < 2 ? 2 : seg > 32 ? 32 : seg;
         if (const char *e = std::getenv("PYJAC_SEG")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) seg = v; }
         dm.d_seg = seg;

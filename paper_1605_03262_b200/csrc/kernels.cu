@@ -701,33 +701,20 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
     }
 }
 
-__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-
-// the chunks [c0, c1) of a phase, round-robin over the warps.  Headers run three chunks ahead, an
-// L1 prefetch of a chunk's first blocks two chunks ahead, its blocks 0 and 1 (registers) one chunk
-// ahead: no table read sits on the critical path of a short list.
+// the chunks [c0, c1) of a phase: warp w takes chunk c0 + w + k NW in round k (mech_pack.cu arranged
+// the chunks in full rows of NW, balanced by cost, and padded the header table, so there are no
+// bounds checks).  Headers run three chunks ahead, a chunk's blocks 0 and 1 one chunk ahead.
 template <int LEVEL, int S, int NW>
 __device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, const double *sc, int c0, int c1, int warp,
                                              int lane)
 {
-    int ch = c0 + warp;
-    if (ch >= c1) return;
-    uint2 h = m.achunk[ch];
-    uint2 h1 = ch + NW < c1 ? m.achunk[ch + NW] : h;
-    uint2 h2 = ch + 2 * NW < c1 ? m.achunk[ch + 2 * NW] : h;
-    uint4 r0 = m.a_ent[h.x + lane];
-    uint4 e1 = m.a_ent[h.x + 32 + lane];        // unconditional (a_ent is padded): a select would wait for r0
-    for (; ch < c1; ch += NW) {
-        const uint2 h3 = ch + 3 * NW < c1 ? m.achunk[ch + 3 * NW] : h;
-#ifdef PYJAC_L1_PREFETCH
-        if (ch + 2 * NW < c1) {
-            prefetch_l1(m.a_ent + h2.x + lane);
-            prefetch_l1(m.a_ent + h2.x + 32 + lane);
-            prefetch_l1(m.a_ent + h2.x + 64 + lane);
-        }
-#endif
-        const uint4 r0n = m.a_ent[h1.x + lane];
-        const uint4 e1n = m.a_ent[h1.x + 32 + lane];
+    const uint2 *hp = m.achunk + c0 + warp;
+    const uint4 *ent = m.a_ent + lane;
+    uint2 h = hp[0], h1 = hp[NW], h2 = hp[2 * NW];
+    uint4 r0 = ent[h.x], e1 = ent[h.x + 32];
+    for (int ch = c0; ch < c1; ch += NW, hp += NW) {
+        const uint2 h3 = hp[3 * NW];
+        const uint4 r0n = ent[h1.x], e1n = ent[h1.x + 32];
         gather_chunk<LEVEL, S>(m, E, sc, h, r0, e1, lane);
         h = h1; h1 = h2; h2 = h3; r0 = r0n; e1 = e1n;
     }

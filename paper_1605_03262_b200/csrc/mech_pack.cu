@@ -783,7 +783,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         o.panel_ptr.push_back(o.panel_ptr.back() + r.first);
     }
     o.a_ent.resize(o.a_ent.size() + 256, pad1);      // the kernels read one or two blocks past a chunk's last
-    if (o.achunk.empty()) o.achunk.assign(2, 0u);
+    o.achunk.resize(o.achunk.size() + (size_t)2 * 3 * NW, 0u);       // headers are read three rounds ahead
 }
 
 int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const ShapeHints &hints, const char **why)
