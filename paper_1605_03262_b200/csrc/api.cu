@@ -78,7 +78,7 @@ int launch(const pyjac_mech *m, int level, int64_t n, const double *T, const dou
     const long long blocks = (n + m->S - 1) / m->S;
     int grid = (int)(blocks < cap ? blocks : cap);
     DeviceMech dm = m->dm;
-    if (level == 2 && (reinterpret_cast<uintptr_t>(out.jac) & 15) != 0) dm.pair = 0;   // 8-byte stores
+    if (level == 2 && (reinterpret_cast<uintptr_t>(out.jac) & 15) != 0) { dm.pair = 0; dm.n_slab = (dm.ld + 31) / 32; }   // 8-byte stores
     cudaError_t e = launch_eval(level, m->threads, m->S, dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy,
                                 out, (cudaStream_t)stream);
     if (dev != m->device) cudaSetDevice(dev);
@@ -132,6 +132,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         seg = seg < 2 ? 2 : seg > 32 ? 32 : seg;
         if (const char *e = std::getenv("PYJAC_SEG")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) seg = v; }
         dm.d_seg = seg;
+        dm.n_slab = n_slab;
     }
     Uploader up;
     try {

@@ -115,6 +115,7 @@ struct DeviceMech {
     int eTile;
     int pair;                   // 1: ld is even, the DENSE pass owns two rows per lane (16-byte stores)
     int d_seg;                  // columns per DENSE work item
+    int n_slab;                 // slabs of rows of the DENSE pass: 64 rows each if pair, else 32
     // ---- regions of E (indices in doubles per state)
     int eQ;                     // [nr][3] {q_i, a_i + W q_i, Theta_dT,i}
     int eH;                     // [nr] reaction enthalpy H_i

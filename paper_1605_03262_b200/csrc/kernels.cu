@@ -799,12 +799,13 @@ __device__ __forceinline__ void dense_item(const DeviceMech &m, const double *E,
     const int ld = m.ld, pw = m.pw;
     const int c0 = pp * pw, ncol = min(ld, c0 + pw) - c0;
     const int RP = m.pair ? 2 : 1;
-    const int n_slab = (ld + 32 * RP - 1) / (32 * RP);
-    const int slab = it % n_slab, cbeg = (it / n_slab) * m.d_seg, cend = min(ncol, cbeg + m.d_seg);
+    const int n_slab = m.n_slab;                              // slabs of 32 RP rows; no integer divisions here
+    const int sg = n_slab == 1 ? it : it / n_slab, slab = it - sg * n_slab;
+    const int cbeg = sg * m.d_seg, cend = min(ncol, cbeg + m.d_seg);
     const int r = slab * 32 * RP + RP * lane;
     if (r >= ld) return;
     const char *tp = reinterpret_cast<const char *>(E) +
-                     (uint32_t)((m.eTile + (pp % m.nbuf) * pw * ld + cbeg * ld + r) * S) * 8u;
+                     (uint32_t)((m.eTile + (m.nbuf == 2 ? (pp & 1) : 0) * pw * ld + cbeg * ld + r) * S) * 8u;
     const uint32_t t_inc = (uint32_t)(ld * S) * 8u, j_inc = (uint32_t)ld * 8u, j_state = (uint32_t)(ld * ld) * 8u;
     const char *cc = reinterpret_cast<const char *>(colc + 2 * (c0 + cbeg));
     char *Jp = reinterpret_cast<char *>(J0 + (long long)(c0 + cbeg) * ld + r);
@@ -848,8 +849,7 @@ __device__ __forceinline__ void dense_item(const DeviceMech &m, const double *E,
 __device__ __forceinline__ int dense_items(const DeviceMech &m, int pp)
 {
     const int ld = m.ld, c0 = pp * m.pw, ncol = min(ld, c0 + m.pw) - c0;
-    const int RP = m.pair ? 2 : 1;
-    return ((ld + 32 * RP - 1) / (32 * RP)) * ((ncol + m.d_seg - 1) / m.d_seg);
+    return m.n_slab * ((ncol + m.d_seg - 1) / m.d_seg);
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------
@@ -911,6 +911,9 @@ __global__ void __launch_bounds__(NT, MB)
         const long long Jstate = (long long)ld * ld;
         long long blk = blockIdx.x, prev = -1;
         int par = 0, ppar = 0;
+        const int nd_last = dense_items(m, n_panel - 1);         // loop invariants (integer divisions)
+        const int n_fixq = n_panel == 1 ? nfix : 0;
+        const int n_plq = m.n_plain * (S / SP);
         for (;;) {
             const bool has_cur = blk < nblk, has_prev = prev >= 0;
             if (!has_cur && !has_prev) break;
@@ -927,10 +930,10 @@ __global__ void __launch_bounds__(NT, MB)
             PROF_MARK(0);
             // ---- Q(blk)
             const int n_g = has_cur ? n_gen * S : 0;
-            const int i_pl = n_g, i_m = i_pl + (has_cur ? m.n_plain * (S / SP) : 0);
+            const int i_pl = n_g, i_m = i_pl + (has_cur ? n_plq : 0);
             const int i_fix = i_m + ((has_cur && blk + gridDim.x < nblk) ? S : 0);
-            const int i_d = i_fix + ((has_prev && n_panel == 1) ? nfix : 0);
-            const int n_q = i_d + (has_prev ? dense_items(m, n_panel - 1) : 0);
+            const int i_d = i_fix + (has_prev ? n_fixq : 0);
+            const int n_q = i_d + (has_prev ? nd_last : 0);
             for (int it = grab(&ctr[0], lane); it < n_q; it = grab(&ctr[0], lane)) {
                 if (it < i_pl) {
                     const int c = it / S, q = it - c * S;
