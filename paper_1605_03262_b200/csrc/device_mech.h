@@ -73,6 +73,10 @@ struct DeviceMech {
     int n_pd;                   // pressure-dependent reactions (third body, falloff, chem. activated): [0, n_pd)
     int n_pk;                   // PLOG / Chebyshev reactions: [n_pd, n_pd + n_pk)
     int n_rchunk;               // groups of 32 reactions
+    int split_general;          // 1: the group that holds reaction n_pd is two work items (pressure-dependent lanes /
+                                // the others).  Shortens the longest item; set when one CTA per SM leaves the
+                                // reaction queue latency-bound (cfg2: 10.51 -> 10.23 ms), not otherwise (cfg1:
+                                // 2.69 -> 2.83 ms, the extra item costs issue slots the other CTA would use)
     int n_plain;                // the last n_plain groups hold only plain reactions
     const uint32_t *rchunk;     // [n_rchunk] 1 = every reaction of the group takes the plain path
     const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}

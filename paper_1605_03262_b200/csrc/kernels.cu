@@ -912,6 +912,8 @@ __global__ void __launch_bounds__(NT, MB)
         long long blk = blockIdx.x, prev = -1;
         int par = 0, ppar = 0;
         const int nd_last = dense_items(m, n_panel - 1);         // loop invariants (integer divisions)
+        const int split_l = m.n_pd & 31, split_c = (m.split_general && split_l != 0 && (m.n_pd >> 5) < n_gen) ? (m.n_pd >> 5) : -1;
+        const int n_genq = n_gen + (split_c >= 0 ? 1 : 0);
         const int n_fixq = n_panel == 1 ? nfix : 0;
         const int n_plq = m.n_plain * (S / SP);
         for (;;) {
@@ -929,15 +931,20 @@ __global__ void __launch_bounds__(NT, MB)
 #endif
             PROF_MARK(0);
             // ---- Q(blk)
-            const int n_g = has_cur ? n_gen * S : 0;
+            const int n_g = has_cur ? n_genq * S : 0;
             const int i_pl = n_g, i_m = i_pl + (has_cur ? n_plq : 0);
             const int i_fix = i_m + ((has_cur && blk + gridDim.x < nblk) ? S : 0);
             const int i_d = i_fix + (has_prev ? n_fixq : 0);
             const int n_q = i_d + (has_prev ? nd_last : 0);
             for (int it = grab(&ctr[0], lane); it < n_q; it = grab(&ctr[0], lane)) {
                 if (it < i_pl) {
-                    const int c = it / S, q = it - c * S;
-                    reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q, out, state0, n);
+                    // general groups, one state at a time; the group that holds both pressure-dependent and
+                    // other reactions is two items (each runs only its own code paths)
+                    const int gi = it / S, q = it - gi * S;
+                    const int c = gi < n_gen ? gi : split_c;
+                    int sl = lane;              // lanes of the other part repeat this part's first reaction
+                    if (c == split_c) sl = gi < n_gen ? (lane < split_l ? lane : 0) : (lane >= split_l ? lane : split_l);
+                    reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + sl, nr - 1), q, out, state0, n);
                 } else if (it < i_m) {
                     const int j = it - i_pl;
                     const int c = n_gen + j / (S / SP), q0 = (j % (S / SP)) * SP;

@@ -206,6 +206,28 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     std::vector<int> order(nr);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key[a] < key[b]; });
+    // A group of 32 lanes runs every code path one of its reactions needs, one after the other, and the
+    // longest group is the critical path of the reaction queue.  The expensive falloff forms (Troe, SRI)
+    // therefore never share a group: after each of them the group is filled up with third-body /
+    // Lindemann reactions, which add almost nothing to a falloff group (same common part).
+    {
+        auto rank_of = [&](int i) { return key[i] / (4 * 8 * 64); };
+        std::vector<int> troe, sri, fill, rest;
+        for (int i : order) {
+            const int r = rank_of(i);
+            (r == 0 ? troe : r == 1 ? sri : (r == 2 || r == 3) ? fill : rest).push_back(i);
+        }
+        std::vector<int> out;
+        size_t f = 0;
+        for (auto *blk : {&troe, &sri}) {
+            if (blk->empty()) continue;
+            out.insert(out.end(), blk->begin(), blk->end());
+            while (out.size() % 32 != 0 && f < fill.size()) out.push_back(fill[f++]);
+        }
+        while (f < fill.size()) out.push_back(fill[f++]);
+        out.insert(out.end(), rest.begin(), rest.end());
+        order.swap(out);
+    }
     o.n_rchunk = (nr + 31) / 32;
     o.rchunk.assign(std::max(o.n_rchunk, 1), 0u);
     for (int c = 0; c < o.n_rchunk; ++c) {
