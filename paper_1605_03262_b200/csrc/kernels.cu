@@ -701,23 +701,47 @@ __device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, con
     }
 }
 
-// the chunks [c0, c1) of a phase: warp w takes chunk c0 + w + k NW in round k (mech_pack.cu arranged
-// the chunks in full rows of NW, balanced by cost, and padded the header table, so there are no
-// bounds checks).  Headers run three chunks ahead, a chunk's blocks 0 and 1 one chunk ahead.
+// The gather chunks of a batch are one table in execution order (A1, then the cells panel by panel),
+// arranged by mech_pack.cu in full rows of NW chunks balanced by cost, the header table padded: warp w
+// takes chunk c + w of the row that starts at c, without bounds checks.  The pipe carries the table
+// reads across phases and barriers: headers three rows ahead, a chunk's blocks 0 and 1 one row ahead,
+// so that only the first chunk of a batch waits for its tables.
+struct GatherPipe {
+    const uint2 *hp;
+    uint2 h, h1, h2;
+    uint4 r0, e1;
+};
+
+template <int NW>
+__device__ __forceinline__ void gather_start(GatherPipe &g, const DeviceMech &m, int c0, int warp, int lane)
+{
+    g.hp = m.achunk + c0 + warp;
+    g.h = g.hp[0]; g.h1 = g.hp[NW]; g.h2 = g.hp[2 * NW];
+    g.r0 = m.a_ent[g.h.x + lane];
+    g.e1 = m.a_ent[g.h.x + 32 + lane];
+}
+
+// the chunks [c0, c1) (whole rows), continuing where the pipe stands
+template <int LEVEL, int S, int NW>
+__device__ __forceinline__ void gather_run(GatherPipe &g, const DeviceMech &m, double *E, const double *sc, int c0,
+                                           int c1, int lane)
+{
+    const uint4 *ent = m.a_ent + lane;
+    for (int ch = c0; ch < c1; ch += NW, g.hp += NW) {
+        const uint2 h3 = g.hp[3 * NW];
+        const uint4 r0n = ent[g.h1.x], e1n = ent[g.h1.x + 32];
+        gather_chunk<LEVEL, S>(m, E, sc, g.h, g.r0, g.e1, lane);
+        g.h = g.h1; g.h1 = g.h2; g.h2 = h3; g.r0 = r0n; g.e1 = e1n;
+    }
+}
+
 template <int LEVEL, int S, int NW>
 __device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, const double *sc, int c0, int c1, int warp,
                                              int lane)
 {
-    const uint2 *hp = m.achunk + c0 + warp;
-    const uint4 *ent = m.a_ent + lane;
-    uint2 h = hp[0], h1 = hp[NW], h2 = hp[2 * NW];
-    uint4 r0 = ent[h.x], e1 = ent[h.x + 32];
-    for (int ch = c0; ch < c1; ch += NW, hp += NW) {
-        const uint2 h3 = hp[3 * NW];
-        const uint4 r0n = ent[h1.x], e1n = ent[h1.x + 32];
-        gather_chunk<LEVEL, S>(m, E, sc, h, r0, e1, lane);
-        h = h1; h1 = h2; h2 = h3; r0 = r0n; e1 = e1n;
-    }
+    GatherPipe g;
+    gather_start<NW>(g, m, c0, warp, lane);
+    gather_run<LEVEL, S, NW>(g, m, E, sc, c0, c1, lane);
 }
 
 // 16-byte streaming store of two consecutive Jacobian rows
@@ -965,8 +989,9 @@ __global__ void __launch_bounds__(NT, MB)
             PROF_MARK(2);
             if (!has_cur) break;
             // ---- G(blk)
-            gather_phase<2, S, NW>(m, E, sc, 0, m.n_a1, warp, lane);
-            gather_phase<2, S, NW>(m, E, sc, m.panel_ptr[0], m.panel_ptr[1], warp, lane);
+            GatherPipe gp;
+            gather_start<NW>(gp, m, 0, warp, lane);
+            gather_run<2, S, NW>(gp, m, E, sc, 0, m.panel_ptr[1], lane);      // A1 and the cells of panel 0
             PROF_MARK(3);
             __syncthreads();
             PROF_MARK(4);
@@ -977,7 +1002,7 @@ __global__ void __launch_bounds__(NT, MB)
                     if (p == 1)
                         for (int it = NW - 1 - warp; it < nfix; it += NW)
                             fix_item<S>(m, E, P0 + sp.oCp * S, sc, colc, wrow, it, lane, Jcur, nq);
-                    gather_phase<2, S, NW>(m, E, sc, m.panel_ptr[p], m.panel_ptr[p + 1], warp, lane);
+                    gather_run<2, S, NW>(gp, m, E, sc, m.panel_ptr[p], m.panel_ptr[p + 1], lane);
                     const int nd = dense_items(m, p - 1);
                     for (int it = warp; it < nd; it += NW) dense_item<S>(m, E, colc, p - 1, it, lane, Jcur, nq);
                     __syncthreads();
