@@ -55,6 +55,7 @@ ShapeHints hints_from_env(long long smem_optin)
     if (const char *e = std::getenv("PYJAC_THREADS")) h.threads = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_PW")) h.pw = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_CTAS")) h.ctas = std::atoi(e);
+    if (const char *e = std::getenv("PYJAC_CAP")) h.cap = std::atoi(e);
     return h;
 }
 

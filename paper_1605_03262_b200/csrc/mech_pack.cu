@@ -48,8 +48,9 @@ struct Task {
 
 // lanes that share one sum: enough that no lane walks more than `cap` entries.  Long lists on one
 // lane cost the fewest instructions (no padding, no shuffle reduction) but make long chunks: with two
-// CTAs per SM the other CTA fills the tail (measured: cfg1 2.79 -> 2.77 ms with cap 32), with one CTA
-// per SM and a barrier per column panel they do not (cfg2 10.8 -> 13.8 ms), so the cap follows the shape.
+// CTAs per SM the other CTA fills the tail, with one CTA per SM and a barrier per column panel it does
+// not.  Measured (PYJAC_CAP sweep): cfg1 2.60 / 2.55 / 2.68 / 2.91 ms at cap 16 / 24 / 32 / 48; cfg2
+// 9.80 / 9.41 / 9.50 / 9.54 / 11.16 ms at cap 6 / 8 / 12 / 16 / 24.  So the cap follows the shape: 24 / 10.
 int pick_rshift(size_t len, size_t cap)
 {
     for (int r = 0; r < 5; ++r)
@@ -562,7 +563,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         for (auto &t : tasks) {
             encode(t, words);
             t.n_words = words.size();
-            t.rshift = pick_rshift(t.n_words, o.ctas_target >= 2 ? 32 : 12);
+            t.rshift = pick_rshift(t.n_words, hints.cap > 0 ? (size_t)hints.cap : o.ctas_target >= 2 ? 24 : 10);
         }
         std::vector<Chunk> chunks;
         if (with_r3 && nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0, 1});

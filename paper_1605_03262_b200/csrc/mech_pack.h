@@ -46,7 +46,7 @@ struct HostPack {
 // PYJAC_S / PYJAC_THREADS / PYJAC_PW / PYJAC_CTAS tuning hooks; 0 = choose).
 struct ShapeHints {
     long long smem_bytes = 227 * 1024 - 1024;   // dynamic shared memory one CTA may use
-    int S = 0, threads = 0, pw = 0, ctas = 0;
+    int S = 0, threads = 0, pw = 0, ctas = 0, cap = 0;      // cap: longest list one lane walks
 };
 
 // Returns PYJAC_OK, PYJAC_EINVAL or PYJAC_ELIMIT.  `why` (optional) receives a static message.
