@@ -817,7 +817,7 @@ __device__ __forceinline__ void fix_item(const DeviceMech &m, const double *E, c
 // ---- DENSE item `it` of panel pp: J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c  (Eq. 112 regrouped)
 // for one slab of rows (two rows per lane when ld is even) and m.d_seg columns; 32-bit offsets
 template <int S>
-__device__ __forceinline__ void dense_item(const DeviceMech &m, const double *E, const double *colc, int pp, int it,
+__device__ __forceinline__ void dense_item(const DeviceMech &m, double *E, const double *colc, int pp, int it,
                                            int lane, double *J0, int nq)
 {
     const int ld = m.ld, pw = m.pw;
@@ -833,6 +833,14 @@ __device__ __forceinline__ void dense_item(const DeviceMech &m, const double *E,
     const uint32_t t_inc = (uint32_t)(ld * S) * 8u, j_inc = (uint32_t)ld * 8u, j_state = (uint32_t)(ld * ld) * 8u;
     const char *cc = reinterpret_cast<const char *>(colc + 2 * (c0 + cbeg));
     char *Jp = reinterpret_cast<char *>(J0 + (long long)(c0 + cbeg) * ld + r);
+    // several panels share a tile buffer: zero it behind the read, so that cells without a list are zero
+    // for the next panel that uses the buffer (column 0 of panel 0 is rewritten by the kAuxT3 sums)
+    const bool zero = m.n_panel > 1;
+    double zeros[2 * S], zeros1[S];
+#pragma unroll
+    for (int q = 0; q < 2 * S; ++q) zeros[q] = 0.0;
+#pragma unroll
+    for (int q = 0; q < S; ++q) zeros1[q] = 0.0;
     if (RP == 2) {
         double al[2 * S], ga[2 * S];
         ldv<2 * S>(E + (m.eAlpha + r) * S, al);
@@ -842,6 +850,7 @@ __device__ __forceinline__ void dense_item(const DeviceMech &m, const double *E,
             const double2 dg = *reinterpret_cast<const double2 *>(cc);
             double t[2 * S];
             ldv<2 * S>(reinterpret_cast<const double *>(tp), t);
+            if (zero) stv<2 * S>(reinterpret_cast<double *>(const_cast<char *>(tp)), zeros);
 #pragma unroll
             for (int q = 0; q < S; ++q) {
                 const double v0 = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
@@ -861,6 +870,7 @@ __device__ __forceinline__ void dense_item(const DeviceMech &m, const double *E,
             const double2 dg = *reinterpret_cast<const double2 *>(cc);
             double t[S];
             ldv<S>(reinterpret_cast<const double *>(tp), t);
+            if (zero) stv<S>(reinterpret_cast<double *>(const_cast<char *>(tp)), zeros1);
 #pragma unroll
             for (int q = 0; q < S; ++q) {
                 const double v = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));

@@ -779,9 +779,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     }
 
     // ---- the cells, panel by panel.  Column 0 (rows >= 1) is written by the kAuxT3 sums; row 0 (the
-    // energy row) never enters the tile, the FIX step stores it.  With several panels every other
-    // cell of a panel gets a task (a cell that is structurally zero in this panel may not be in the
-    // panel that used the buffer before).
+    // energy row) never enters the tile, the FIX step stores it.  Cells without a list get no task: the
+    // tile starts as zeros and, with several panels, the DENSE pass zeroes each buffer behind itself.
     o.panel_ptr.assign(1, o.n_a1);
     for (int p = 0; p < n_panel; ++p) {
         std::vector<Task> tasks;
@@ -795,7 +794,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                 t.out = (uint32_t)(eTile + (p % nbuf) * pw * ld + (c - c0) * ld + r);
                 t.ent = cell[(size_t)r + (size_t)c * ld];
                 if (!t.ent.empty()) t.cst = d->mol_wt[r - 1] * (1.0 / d->mol_wt[c - 1]);
-                if (t.ent.empty() && n_panel == 1) continue;
+                if (t.ent.empty()) continue;        // stays zero: the DENSE pass zeroes a tile buffer behind itself
                 o.n_cell_entries += (long long)t.ent.size();
                 tasks.push_back(t);
             }
