@@ -56,6 +56,7 @@ ShapeHints hints_from_env(long long smem_optin)
     if (const char *e = std::getenv("PYJAC_PW")) h.pw = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_CTAS")) h.ctas = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_CAP")) h.cap = std::atoi(e);
+    if (const char *e = std::getenv("PYJAC_SEG")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) h.seg = v; }
     return h;
 }
 
@@ -126,16 +127,8 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     dm.eQ = hp.eQ; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;
     dm.eWdot = hp.eWdot; dm.eG0 = hp.eG0; dm.eZ = hp.eZ;
     dm.eS1 = hp.eS1; dm.eA0 = hp.eA0; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.eDump = hp.eDump; dm.n_e = hp.n_e;
-    {   // DENSE work items (one slab of rows x seg columns).  Measured (profiles/r1_v8_cfg1_cfg2.md): with one
-        // panel the items sit in the dynamic queue and fewer, longer items win (less set-up per column);
-        // with several panels they are dealt round-robin next to the cell gathers and about 3 columns win.
-        const int nw = m->threads / 32, n_slab = (dm.ld + (dm.pair ? 63 : 31)) / (dm.pair ? 64 : 32);
-        int seg = dm.n_panel == 1 ? (3 * n_slab * dm.pw + 2 * nw - 1) / (2 * nw) : 3;
-        seg = seg < 2 ? 2 : seg > 32 ? 32 : seg;
-        if (const char *e = std::getenv("PYJAC_SEG")) { const int v = std::atoi(e); if (v >= 1 && v <= 64) seg = v; }
-        dm.d_seg = seg;
-        dm.n_slab = n_slab;
-    }
+    dm.d_seg = hp.d_seg;
+    dm.n_slab = (dm.ld + (dm.pair ? 63 : 31)) / (dm.pair ? 64 : 32);
     Uploader up;
     try {
         up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.mw, hp.mw);

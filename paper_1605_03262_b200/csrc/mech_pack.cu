@@ -502,6 +502,15 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         if ((long long)(o.n_e + o.nbuf * o.pw * ld) * o.S * 8 > (long long)kEntOffMask)
             throw Fail{PYJAC_ELIMIT, "per-CTA tables exceed the 512 KB offset range of a gather entry"};
     }
+    {   // DENSE work items (one slab of rows x d_seg columns).  Measured: with one panel the items sit in the
+        // dynamic queue and fewer, longer items win (less set-up per column); with several panels they are
+        // dealt round-robin next to the cell gathers and about 3 columns win.
+        const int nw = o.threads / 32, n_slab = (ld + (o.pair ? 63 : 31)) / (o.pair ? 64 : 32);
+        int seg = o.n_panel == 1 ? (3 * n_slab * o.pw + 2 * nw - 1) / (2 * nw) : 3;
+        seg = seg < 2 ? 2 : seg > 32 ? 32 : seg;
+        if (hints.seg > 0) seg = hints.seg;
+        o.d_seg = seg;
+    }
     const int S = o.S, pw = o.pw, n_panel = o.n_panel, nbuf = o.nbuf, eTile = o.eTile;
 
     // ---- A1 sums
@@ -799,8 +808,17 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                 tasks.push_back(t);
             }
         o.n_cells += (long long)tasks.size();
-        // the cells of panel 0 are gathered in the same phase as the A1 sums: continue their balance
+        // the cells of panel 0 are gathered in the same phase as the A1 sums: continue their balance;
+        // the cells of panel p >= 1 share their step with the DENSE items of panel p - 1, dealt round-robin
         std::vector<double> load = p == 0 ? a1_load : std::vector<double>(NW, 0.0);
+        if (p >= 1) {
+            const int RP = o.pair ? 2 : 1, n_slab = (ld + 32 * RP - 1) / (32 * RP);
+            const int ncol_prev = std::min(ld, p * pw) - (p - 1) * pw;
+            const int nd = n_slab * ((ncol_prev + o.d_seg - 1) / o.d_seg);
+            // cost of a DENSE item in the units of emit_phase; measured on cfg2: 9.53 / 9.39 / 9.62 / 10.33 ms
+            // with 0 / 0.5 / 1 / 1.5 times (10 + 5 d_seg)
+            for (int it = 0; it < nd; ++it) load[it % NW] += 5.0 + 2.5 * o.d_seg;
+        }
         auto r = emit_phase(tasks, false, o.n_cell_steps, load);
         o.panel_ptr.push_back(o.panel_ptr.back() + r.first);
     }

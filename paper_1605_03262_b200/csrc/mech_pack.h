@@ -32,7 +32,7 @@ struct HostPack {
     std::vector<uint32_t> achunk;         // uint2 flattened
     std::vector<uint32_t> a_ent;          // uint4 flattened
     std::vector<int32_t> panel_ptr;       // [n_panel + 1]
-    int n_panel = 1, pw = 0, nbuf = 1, eTile = 0, pair = 0;
+    int n_panel = 1, pw = 0, nbuf = 1, eTile = 0, pair = 0, d_seg = 3;
     int eQ = 0, eH = 0, eAlpha = 0, eGamma = 0, eWdot = 0, eG0 = 0, eZ = 0;
     int eS1 = 0, eA0 = 0, eS4 = 0, eZero = 0, eDump = 0, n_e = 0;
     // launch shape chosen with the tables: S states per CTA iteration, threads per CTA, the CTAs
@@ -46,7 +46,7 @@ struct HostPack {
 // PYJAC_S / PYJAC_THREADS / PYJAC_PW / PYJAC_CTAS tuning hooks; 0 = choose).
 struct ShapeHints {
     long long smem_bytes = 227 * 1024 - 1024;   // dynamic shared memory one CTA may use
-    int S = 0, threads = 0, pw = 0, ctas = 0, cap = 0;      // cap: longest list one lane walks
+    int S = 0, threads = 0, pw = 0, ctas = 0, cap = 0, seg = 0;      // cap: longest list one lane walks; seg: columns per DENSE item
 };
 
 // Returns PYJAC_OK, PYJAC_EINVAL or PYJAC_ELIMIT.  `why` (optional) receives a static message.
