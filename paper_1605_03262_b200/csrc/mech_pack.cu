@@ -824,6 +824,50 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     }
     o.a_ent.resize(o.a_ent.size() + 256, pad1);      // the kernels read one or two blocks past a chunk's last
     o.achunk.resize(o.achunk.size() + (size_t)2 * 3 * NW, 0u);       // headers are read three rounds ahead
+
+    // ---- self-check of what the kernels rely on without bounds checks (kernels.cu gather_run /
+    // gather_chunk): whole rows of NW chunks per phase, every block a chunk reads inside a_ent (its own
+    // blocks and the unconditional block 1), every header the pipe reads ahead inside achunk, every
+    // source offset and output index inside the CTA's E + tile array
+    {
+        const size_t n_chunks = o.achunk.size() / 2 - (size_t)3 * NW, n_blocks = o.a_ent.size() / 4;
+        const uint32_t e_total = (uint32_t)(o.n_e + nbuf * pw * ld);
+        auto bad = [](const char *w) { throw Fail{PYJAC_ELIMIT, w}; };
+        if (o.n_a1 % NW || o.n_a1_01 % NW || (size_t)o.panel_ptr.back() != n_chunks || o.panel_ptr[0] != o.n_a1)
+            bad("internal: gather phases are not whole rows of chunks");
+        for (size_t p = 0; p + 1 < o.panel_ptr.size(); ++p)
+            if (o.panel_ptr[p + 1] < o.panel_ptr[p] || (o.panel_ptr[p + 1] - o.panel_ptr[p]) % NW)
+                bad("internal: a panel's chunks are not whole rows");
+        for (size_t c = 0; c < o.achunk.size() / 2; ++c) {
+            const uint32_t base = o.achunk[2 * c], meta = o.achunk[2 * c + 1];
+            const int steps = (int)(meta & 0xFFFF), kind = (int)((meta >> 16) & 0xF), tpl = (int)(meta >> 24);
+            const int rounds = c >= n_chunks ? 1
+                             : tpl == 2 ? 2 + (steps > 1 ? steps / 2 : 0) : 1 + (steps > 1 ? (steps + 2) / 4 : 0);
+            if ((size_t)base + 32 * (size_t)std::max(rounds, 2) > n_blocks) bad("internal: a chunk reads past the entry table");
+            if (c >= n_chunks || kind == (int)kAuxR3) continue;
+            const uint32_t *blk = o.a_ent.data() + (size_t)base * 4;
+            for (int row = 0; row < std::max(tpl, 1); ++row)
+                for (int lane = 0; lane < 32; ++lane) {
+                    const uint32_t out = blk[((size_t)row * 32 + lane) * 4];
+                    if (out != 0xFFFFFFFFu && out >= (kind == (int)kAuxT3 ? (uint32_t)ns : e_total))
+                        bad("internal: a gather result lies outside E");
+                    for (int st = 0; st < steps; ++st) {
+                        size_t at;
+                        if (tpl == 2)
+                            at = st == 0 ? ((size_t)row * 32 + lane) * 4 + 3
+                                         : ((size_t)(2 + (st - 1) / 2) * 32 + lane) * 4 + 2 * ((st - 1) % 2) + row;
+                        else
+                            at = st == 0 ? (size_t)lane * 4 + 3 : ((size_t)(1 + (st - 1) / 4) * 32 + lane) * 4 + (st - 1) % 4;
+                        const uint32_t w = blk[at];
+                        const bool ok = kind == (int)kAuxH2
+                                            ? ((w & 0xFFFF) < e_total && (w >> 16) < e_total)
+                                            : ((w & kEntOffMask) % (8u * S) == 0 &&
+                                               (w & kEntOffMask) / (8u * S) + (kind == (int)kAuxT3 ? 2u : 0u) < e_total);
+                        if (!ok) bad("internal: a gather entry points outside E");
+                    }
+                }
+        }
+    }
 }
 
 int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const ShapeHints &hints, const char **why)

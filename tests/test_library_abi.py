@@ -124,3 +124,25 @@ def test_binding_refuses_cpu_tensors():
     with pytest.raises(TypeError):
         pj._dev_inputs(torch.zeros(2, dtype=torch.float64), torch.zeros(2, dtype=torch.float64),
                        torch.zeros(2, 3, dtype=torch.float64))
+
+
+@pytest.mark.parametrize("env", [
+    {}, {"PYJAC_S": "1"}, {"PYJAC_S": "2", "PYJAC_PW": "7"}, {"PYJAC_S": "4", "PYJAC_CTAS": "1"},
+    {"PYJAC_S": "1", "PYJAC_PW": "5", "PYJAC_THREADS": "128"}, {"PYJAC_CAP": "6"}, {"PYJAC_CAP": "64"},
+])
+def test_pack_self_check_over_launch_shapes(monkeypatch, env):
+    """pyjac_pack_stats packs exactly as pyjac_mech_create does, including the self-check of everything
+    the kernels read without bounds checks (whole rows of chunks, table blocks, entry offsets); it must
+    hold for every configuration and every shape the tuning hooks can select."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    for cfg in (0, 1, 2, 3):
+        try:
+            st = binding.pack_stats(synth.make_mechanism(cfg))
+        except binding.PyJacError as e:
+            # a forced shape that does not fit the shared memory of one CTA is refused, loudly
+            assert e.code == binding.PYJAC_ELIMIT and "PYJAC_S" in env and cfg >= 2
+            continue
+        assert st["chunks"] > 0 and st["panels"] >= 1 and st["smem_bytes_per_cta"] <= 227 * 1024
+    for seed in range(4):
+        binding.pack_stats(synth.make_tiny_mechanism(seed))
