@@ -94,7 +94,7 @@ struct DeviceMech {
                                 // row 0 the breakpoint (+inf if n_int = 1), rows 1..7 g of the lower interval,
                                 // rows 8..14 g of the upper one
     const double *lo_lnA, *lo_beta, *lo_Ta;      // [n_pd] k_0
-    const double *fall_par;                      // [n_pd][5]
+    const double *fall_par;                      // [n_pd][5]; Troe: {a, 1/T***, 1/T*, T**, has T**}; SRI: {a, b, 1/c, d, e}
     const int32_t *eff_base;    // [general groups + 1] first efficiency entry of a group of 32 reactions
     const uint4 *eff_ent;       // entry e of lane l of group c at [eff_base[c] + 32 e + l]: {species of alpha_ij != 1
                                 // (or the single species) | E index of its term << 16, 0, alpha_ij - 1 (fp64 bits;

@@ -403,27 +403,29 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
                 const int form = meta_form(meta);
                 double F = 1.0, gF = 0.0;                                // gF = (P_r/F) dF/dP_r
                 if (form == PYJAC_TROE) {                                // Eqs. 33-35, 90-96
-                    const double a = fp[0];
-                    const double e3 = exp_rate(-T / fp[1]), e1 = exp_rate(-T / fp[2]);
+                    // fp[1], fp[2] hold 1/T***, 1/T* (mech_pack.cu); three reciprocals serve every quotient
+                    const double a = fp[0], i3 = fp[1], i1 = fp[2];
+                    const double e3 = exp_rate(-T * i3), e1 = exp_rate(-T * i1);
                     const double e2 = fp[4] != 0.0 ? exp_rate(-fp[3] * invT) : 0.0;
                     const double Fc = (1.0 - a) * e3 + a * e1 + e2;
-                    const double dFc = -(1.0 - a) / fp[1] * e3 - a / fp[2] * e1 + fp[3] * invT * invT * e2;
+                    const double dFc = -(1.0 - a) * i3 * e3 - a * i1 * e1 + fp[3] * invT * invT * e2;
                     const double lnFc = log(Fc);
                     const double lF = lnFc * kInvLn10, lP = log10(Pr);
                     const double At = lP - 0.67 * lF - 0.4;
                     const double Bt = 0.806 - 1.1762 * lF - 0.14 * lP;
-                    const double AB = At / Bt, qq = 1.0 + AB * AB;
-                    F = exp_rate(lnFc / qq);
-                    const double k2 = lnFc * 2.0 * At / (Bt * Bt * Bt) / (kLn10 * qq * qq);
+                    const double rB = 1.0 / Bt, rF = 1.0 / Fc;
+                    const double AB = At * rB, rq = 1.0 / (1.0 + AB * AB);
+                    F = exp_rate(lnFc * rq);
+                    const double k2 = lnFc * 2.0 * At * (rB * rB * rB) * (kInvLn10 * rq * rq);
                     gF = -k2 * (Bt + 0.14 * At);
-                    fT = (1.0 / (Fc * qq) - k2 * (1.1762 * At - 0.67 * Bt) / Fc) * dFc;
+                    fT = (rq - k2 * (1.1762 * At - 0.67 * Bt)) * rF * dFc;
                 } else if (form == PYJAC_SRI) {                          // Eqs. 36, 97-100
-                    const double ea = exp_rate(-fp[1] * invT), ec = exp_rate(-T / fp[2]);
+                    const double ea = exp_rate(-fp[1] * invT), ec = exp_rate(-T * fp[2]);       // fp[2] holds 1/c
                     const double base = fp[0] * ea + ec, lnb = log(base);
                     const double lP = log10(Pr), Xs = 1.0 / (1.0 + lP * lP);
                     F = fp[3] * exp_rate(fp[4] * lnT + Xs * lnb);
                     gF = -Xs * Xs * 2.0 * lP * lnb * kInvLn10;
-                    fT = fp[4] * invT + Xs * (fp[0] * fp[1] * invT * invT * ea - ec / fp[2]) / base;
+                    fT = fp[4] * invT + Xs * (fp[0] * fp[1] * invT * invT * ea - ec * fp[2]) / base;
                 }
                 const double i1p = 1.0 / (1.0 + Pr);
                 double Theta;

@@ -380,7 +380,15 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             o.lo_lnA.push_back(fall ? std::log(d->arr_lo[3 * i]) : 0.0);
             o.lo_beta.push_back(fall ? d->arr_lo[3 * i + 1] : 0.0);
             o.lo_Ta.push_back(fall ? d->arr_lo[3 * i + 2] : 0.0);
-            for (int c = 0; c < 5; ++c) o.fall_par.push_back(fall ? d->falloff_par[5 * i + c] : 0.0);
+            for (int c = 0; c < 5; ++c) {
+                double v = fall ? d->falloff_par[5 * i + c] : 0.0;
+                // the temperatures that only ever divide are stored as reciprocals: Troe T***, T* (Eq. 33),
+                // SRI c (Eq. 36)
+                if (fall && ((d->falloff_form[i] == PYJAC_TROE && (c == 1 || c == 2)) ||
+                             (d->falloff_form[i] == PYJAC_SRI && c == 2)))
+                    v = 1.0 / v;
+                o.fall_par.push_back(v);
+            }
             size_t e = 0;
             const int m = d->tb_species[i];
             if (m >= 0) {       // Eq. 30: [X]_i = [X_m]; one entry with "alpha - 1" = 1 and no [M] term
