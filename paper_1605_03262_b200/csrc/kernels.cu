@@ -388,13 +388,17 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         double c = 1.0, G = 0.0, fT = 0.0, b = 0.0, Xi = 0.0;
         if (pdep) {
             Xi = meta_single(meta) ? 0.0 : sc[kM * S + q];               // Eqs. 28-30
-            for (int e = 0; e < n_eff; e += 128) {                       // four entries at a time, loads first
-                uint4 w[4];
+            for (int e = 0; e < n_eff; e += 256) {                       // eight entries at a time, all reads first
+                uint4 w[8];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.ns, 0u, 0u, 0u);
+                for (int u = 0; u < 8; ++u) w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.ns, 0u, 0u, 0u);
+                double xa = 0.0, xb = 0.0;
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    Xi = fma(__hiloint2double((int)w[u].w, (int)w[u].z), X[(w[u].x & 0xFFFF) * S + q], Xi);
+                for (int u = 0; u < 8; u += 2) {
+                    xa = fma(__hiloint2double((int)w[u].w, (int)w[u].z), X[(w[u].x & 0xFFFF) * S + q], xa);
+                    xb = fma(__hiloint2double((int)w[u + 1].w, (int)w[u + 1].z), X[(w[u + 1].x & 0xFFFF) * S + q], xb);
+                }
+                Xi += xa + xb;
             }
             if (type == PYJAC_THIRD_BODY) {
                 c = Xi; G = Xi; lPrT = -invT; b = R;                     // Eqs. 79-80
@@ -464,12 +468,12 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             E[v0 + q] = ckf * sk0; E[v1 + q] = ckf * sk1; E[v2 + q] = ckf * sk2;
             E[v3 + q] = ckr * sk3; E[v4 + q] = ckr * sk4; E[v5 + q] = ckr * sk5;
             if (pdep)
-                for (int e = 0; e < n_eff; e += 128) {
-                    uint4 w[4];
+                for (int e = 0; e < n_eff; e += 256) {
+                    uint4 w[8];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
+                    for (int u = 0; u < 8; ++u) w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) E[(w[u].x >> 16) * S + q] = b * __hiloint2double((int)w[u].w, (int)w[u].z);
+                    for (int u = 0; u < 8; ++u) E[(w[u].x >> 16) * S + q] = b * __hiloint2double((int)w[u].w, (int)w[u].z);
                 }
         }
     }
