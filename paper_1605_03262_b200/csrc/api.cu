@@ -122,6 +122,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     dm.ns = hp.ns; dm.nr = hp.nr; dm.ld = hp.ns + 1;
     dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk; dm.n_plain = (int)hp.n_plain_chunks;
     dm.n_a1 = hp.n_a1; dm.n_a1_01 = hp.n_a1_01;
+    dm.brk_common = hp.brk_common;
     dm.split_general = hp.ctas_target == 1 ? 1 : 0;
     dm.n_panel = hp.n_panel; dm.pw = hp.pw; dm.nbuf = hp.nbuf; dm.eTile = hp.eTile; dm.pair = hp.pair;
     dm.eQ = hp.eQ; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma;

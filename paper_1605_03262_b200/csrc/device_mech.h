@@ -90,6 +90,7 @@ struct DeviceMech {
                                 // sum_k nu_ki B_k(T) = g0 + g1 ln T + T (g2 + T (g3 + T (g4 + T g5))) + g6 / T
                                 // (Eq. 27 summed over the reaction, one set per interval between the t_mid of
                                 // its species; g0 includes (sum nu) ln(p_atm / R) of Eq. 26)
+    double brk_common;          // the breakpoint every reaction shares (all n_int <= 2, one t_mid), else NaN
     const double *th_soa;       // [15][nr] the same for reactions with n_int <= 2, coalesced over reactions:
                                 // row 0 the breakpoint (+inf if n_int = 1), rows 1..7 g of the lower interval,
                                 // rows 8..14 g of the upper one

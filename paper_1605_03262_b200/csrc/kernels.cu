@@ -143,7 +143,9 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
     const bool rev = meta_rev(meta) != PYJAC_IRREVERSIBLE;
     const double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
     const double *th = m.th_soa + s;
-    const double brk = th[0];
+    // one breakpoint for the whole mechanism (the usual case): the interval is known without a table read,
+    // so the coefficient reads go out with the other tables instead of one L2 round trip later
+    const double brk = m.brk_common == m.brk_common ? m.brk_common : th[0];
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
     if (LEVEL == 2) {
         const uint4 vi = m.vidx[s];
@@ -238,7 +240,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     // every table read of the reaction is issued here, before the first use, so that the reads
     // overlap (one L2 round trip instead of one per parameter group); indices are clamped, the values
     // of reactions that do not use them are ignored
-    const double brk = m.th_soa[s];             // NaN: more than two intervals, see th_data
+    const double brk = m.brk_common == m.brk_common ? m.brk_common : m.th_soa[s];   // NaN: more than two intervals, see th_data
     const double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
     const int s_pd = min(s, max(m.n_pd, 1) - 1);
     const double lo_lnA = m.lo_lnA[s_pd], lo_beta = m.lo_beta[s_pd], lo_Ta = m.lo_Ta[s_pd];

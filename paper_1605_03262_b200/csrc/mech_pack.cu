@@ -433,6 +433,22 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     }
 
 
+    // ---- one breakpoint for all reactions?  (reactions with a single interval carry the same
+    // coefficients in both rows of th_soa, so any breakpoint is right for them)
+    {
+        double common = HUGE_VAL;
+        bool ok = true;
+        for (int sr = 0; sr < nr && ok; ++sr) {
+            const double b = o.th_soa[sr];
+            if (b != b) ok = false;
+            else if (b != HUGE_VAL) {
+                if (common == HUGE_VAL) common = b;
+                else if (common != b) ok = false;
+            }
+        }
+        o.brk_common = ok ? common : std::nan("");
+    }
+
     // ---- efficiencies, regrouped per group of 32 reactions (device_mech.h `eff_ent`)
     {
         const int n_gen = o.n_rchunk - (int)o.n_plain_chunks;

@@ -18,6 +18,7 @@ struct HostPack {
     std::vector<int32_t> rxn_orig;
     std::vector<uint32_t> th_off;
     std::vector<double> th_data, th_soa;
+    double brk_common = 0.0;              // NaN unless every reaction has at most two intervals and one breakpoint
     std::vector<double> lo_lnA, lo_beta, lo_Ta, fall_par;
     std::vector<int32_t> eff_ptr;
     std::vector<uint32_t> eff_spec;
