@@ -34,7 +34,7 @@ FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallba
 CPU_SAMPLE = {0: 1024, 1: 8192, 2: 2048, 3: 256}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the Jacobian kernel from the committed
 # `ncu --set full` capture (profiles/), or None where no capture exists for that workload
-NCU_TRAFFIC_BYTES = {"cfg1_53sp_325rx": 2356203160, "cfg2_111sp_784rx": 10170013216}      # profiles/r1_v8_cfg1_cfg2.md
+NCU_TRAFFIC_BYTES = {"cfg1_53sp_325rx": 2376411408, "cfg2_111sp_784rx": 10179931272}      # profiles/r1_v8_cfg1_cfg2.md
 
 
 def measured_peaks():
