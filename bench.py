@@ -184,6 +184,49 @@ def bench_config(torch, cfg, steps, warmup, n_states=None, chunk=None):
                 per_step_ms=per, launches=launches, launches_per_step=len(views), per_launch=per_launch)
 
 
+def run_peaks():
+    """The two machine peaks SURVEY.md section 8(d) asks for beside MEASURED_PEAKS.json's copy bandwidth:
+    a write-only stream with the DENSE pass's store instruction, and the fp64 FMA rate (8 independent
+    chains per thread, full occupancy).  CUDA events, 3 warm-up + 10 timed launches, best and mean."""
+    import torch
+    from paper_1605_03262_b200 import build, binding
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    sp = torch.cuda.current_stream().cuda_stream
+    buf = torch.empty(1 << 29, dtype=torch.float64, device="cuda")          # 4 GiB, far beyond L2
+    out = torch.empty(148 * 4096, dtype=torch.float64, device="cuda")
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(11)]
+        ev[0].record()
+        for i in range(10):
+            fn()
+            ev[i + 1].record()
+        torch.cuda.synchronize()
+        per = [ev[i].elapsed_time(ev[i + 1]) for i in range(10)]
+        return min(per), sum(per) / len(per)
+
+    best, mean = timed(lambda: binding.peak_store_stream(buf, sp))
+    nbytes = buf.numel() * 8
+    flops = [0]
+    iters = 1 << 16
+
+    def dfma():
+        flops[0] = binding.peak_dfma(out, iters, sp)
+    fbest, fmean = timed(dfma)
+    peak, src = measured_peaks()
+    print(json.dumps({"store_stream": {"bytes": nbytes, "best_gbs": nbytes / best / 1e6, "mean_gbs": nbytes / mean / 1e6,
+                                       "instruction": "st.global.cs.v2.f64"},
+                      "fp64_fma": {"flops": flops[0], "best_tflops": flops[0] / fbest / 1e9, "mean_tflops": flops[0] / fmean / 1e9,
+                                   "chains_per_thread": 8},
+                      "hbm_copy_gbs": peak, "hbm_copy_source": src}))
+
+
 def max_over_ranks(ms: float, dist, device: str) -> float:
     """Device-timed milliseconds of the timed region, MAX over the ranks (the only collective of the
     run: states are independent, every rank evaluates its own replica)."""
@@ -210,10 +253,15 @@ def main():
     ap.add_argument("--also", default="2", help="comma list of further configs reported under per_config")
     ap.add_argument("--sweep", action="store_true", help="config 4: state-count sweep, three kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--peaks", action="store_true",
+                    help="measure the write-only store stream and the fp64 FMA rate (SURVEY.md 8(d)) and exit")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.peaks:
+        run_peaks()
         return
     args.warmup = max(3, args.warmup)
 

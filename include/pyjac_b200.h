@@ -178,6 +178,16 @@ int pyjac_jacobian_launch_config(const pyjac_mech *mech, int64_t n, int32_t *thr
  * Errors as pyjac_mech_create (PYJAC_EINVAL, PYJAC_ELIMIT, PYJAC_ENOMEM). */
 int pyjac_pack_stats(const pyjac_mech_desc *host_desc, int64_t *stats);
 
+/* Machine peaks the roofline discussion refers to (bench.py --peaks), measured with
+ * the same instructions the Jacobian kernel uses.  Device pointers, enqueued on `stream`, no allocation.
+ *   pyjac_peak_store_stream: writes n_doubles (a multiple of 2) doubles of `buf` once with 16-byte
+ *     streaming stores (st.global.cs.v2.f64), the store of the DENSE pass; bytes moved = 8 n_doubles.
+ *   pyjac_peak_dfma: every thread of a full-occupancy grid runs 8 independent chains of `iters` fp64
+ *     FMAs and writes one result per thread to out[0 .. *n_threads) (out must hold 148 * 2048 doubles
+ *     at least; the thread count used is returned); flops = 2 * 8 * iters * *n_threads. */
+int pyjac_peak_store_stream(double *buf, int64_t n_doubles, void *stream);
+int pyjac_peak_dfma(double *out, int64_t iters, int64_t *n_threads, void *stream);
+
 /* Static, never-NULL description of an error code. */
 const char *pyjac_strerror(int code);
 

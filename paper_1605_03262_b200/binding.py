@@ -40,7 +40,7 @@ class MechDesc(C.Structure):
 EXPORTS = ("pyjac_mech_create", "pyjac_mech_destroy", "pyjac_mech_sizes", "pyjac_eval_rates",
            "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
            "pyjac_eval_dydt_host", "pyjac_kernel_launches", "pyjac_jacobian_launch_config",
-           "pyjac_pack_stats", "pyjac_strerror")
+           "pyjac_pack_stats", "pyjac_peak_store_stream", "pyjac_peak_dfma", "pyjac_strerror")
 
 _lib = None
 
@@ -68,6 +68,8 @@ def load_library(path: str | None = None):
     lib.pyjac_kernel_launches.restype = i64
     lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 4
     lib.pyjac_pack_stats.argtypes = [C.POINTER(MechDesc), C.POINTER(i64)]
+    lib.pyjac_peak_store_stream.argtypes = [vp, i64, vp]
+    lib.pyjac_peak_dfma.argtypes = [vp, i64, C.POINTER(i64), vp]
     lib.pyjac_strerror.argtypes = [C.c_int]
     lib.pyjac_strerror.restype = C.c_char_p
     for name in EXPORTS:
@@ -124,6 +126,18 @@ def pack_stats(mech: Mechanism) -> dict:
     out = (C.c_int64 * 12)()
     _check(lib.pyjac_pack_stats(C.byref(d), out), "pyjac_pack_stats")
     return dict(zip(PACK_STAT_NAMES, [int(v) for v in out]))
+
+
+def peak_store_stream(buf, stream_ptr):
+    """Enqueues one write-only pass over the CUDA float64 tensor `buf` (pyjac_peak_store_stream)."""
+    _check(load_library().pyjac_peak_store_stream(buf.data_ptr(), int(buf.numel()), stream_ptr), "pyjac_peak_store_stream")
+
+
+def peak_dfma(out, iters, stream_ptr):
+    """Enqueues the fp64 FMA probe (pyjac_peak_dfma); returns the flops it executes."""
+    n = C.c_int64()
+    _check(load_library().pyjac_peak_dfma(out.data_ptr(), int(iters), C.byref(n), stream_ptr), "pyjac_peak_dfma")
+    return 2 * 8 * int(iters) * n.value
 
 
 class PyJac:

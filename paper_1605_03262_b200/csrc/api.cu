@@ -268,6 +268,33 @@ int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
     return PYJAC_OK;
 }
 
+int pyjac_peak_store_stream(double *buf, int64_t n_doubles, void *stream)
+{
+    if (!buf || n_doubles < 2 || (n_doubles & 1) || (reinterpret_cast<uintptr_t>(buf) & 15)) return PYJAC_EINVAL;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return PYJAC_ECUDA;
+    const cudaError_t e = launch_peak_store(buf, n_doubles, n_sm * 8, (cudaStream_t)stream);
+    if (e != cudaSuccess) return PYJAC_ECUDA;
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return PYJAC_OK;
+}
+
+int pyjac_peak_dfma(double *out, int64_t iters, int64_t *n_threads, void *stream)
+{
+    if (!out || iters < 1 || !n_threads) return PYJAC_EINVAL;
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return PYJAC_ECUDA;
+    *n_threads = (int64_t)n_sm * 2048;
+    const cudaError_t e = launch_peak_dfma(out, iters, n_sm * 8, (cudaStream_t)stream);
+    if (e != cudaSuccess) return PYJAC_ECUDA;
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return PYJAC_OK;
+}
+
 const char *pyjac_strerror(int code)
 {
     switch (code) {

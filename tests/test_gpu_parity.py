@@ -334,3 +334,23 @@ def test_output_pointer_not_16_byte_aligned(torch, PyJac):
     pj.eval_jacobian(dT, dP, dY, out=view)
     assert torch.equal(view.reshape(257, ld * ld), J)
     assert float(buf[0]) == 0.0
+
+
+@pytest.mark.gpu
+def test_peak_probes(torch):
+    """The roofline probes: the store stream writes every element once, the FMA probe
+    reports the flops it ran; bad arguments are refused."""
+    from paper_1605_03262_b200 import binding
+    sp = torch.cuda.current_stream().cuda_stream
+    buf = torch.full((1 << 16,), -1.0, dtype=torch.float64, device="cuda")
+    binding.peak_store_stream(buf, sp)
+    torch.cuda.synchronize()
+    assert torch.equal(buf[0::2], torch.arange(1 << 15, dtype=torch.float64, device="cuda"))
+    assert bool((buf[1::2] == 1.0).all())
+    out = torch.zeros(148 * 4096, dtype=torch.float64, device="cuda")
+    flops = binding.peak_dfma(out, 128, sp)
+    torch.cuda.synchronize()
+    assert flops > 0 and flops % (2 * 8 * 128) == 0 and bool(torch.isfinite(out).all())
+    lib = binding.load_library()
+    assert lib.pyjac_peak_store_stream(None, 16, None) == binding.PYJAC_EINVAL
+    assert lib.pyjac_peak_store_stream(buf.data_ptr() + 8, 16, None) == binding.PYJAC_EINVAL
