@@ -473,3 +473,29 @@ def test_batch_independence_and_threads(tiny_mechs):
     o1 = Oracle(m, threads=1)
     b = np.concatenate([o1.jacobian(T[:5], P[:5], Y[:5]), o1.jacobian(T[5:], P[5:], Y[5:])])
     np.testing.assert_array_equal(a, b)
+
+
+def test_oracle_regression_fixture():
+    """tests/golden/oracle_tiny_jacobian.txt (written by tests/golden/make_golden.py, which calls only
+    oracle/) freezes the oracle's arithmetic: an accidental change of oracle.c shows up here.  It is not
+    a pin to the paper (which prints no worked example)."""
+    import os
+    from paper_1605_03262_b200 import synth as _synth
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "oracle_tiny_jacobian.txt")
+    rows = [l for l in open(path).read().splitlines() if l and not l.startswith("#")]
+    i = 0
+    while i < len(rows):
+        tag, seed, n, ns = rows[i].split()
+        assert tag == "case"
+        seed, n, ns = int(seed), int(n), int(ns)
+        m = _synth.make_tiny_mechanism(seed)
+        assert m.n_species == ns
+        T, P, Y = _synth.make_states(ns, n, 4242 + seed)
+        o = Oracle(m)
+        src, J = o.source(T, P, Y), o.jacobian(T, P, Y)
+        for s in range(n):
+            dy = np.array([float(x) for x in rows[i + 1 + 2 * s].split()])
+            Js = np.array([float(x) for x in rows[i + 2 + 2 * s].split()])
+            assert np.allclose(src["dydt"][s], dy, rtol=1e-12, atol=1e-12 * np.abs(dy).max())
+            assert np.linalg.norm(J[s] - Js) <= 1e-12 * np.linalg.norm(Js)
+        i += 1 + 2 * n
