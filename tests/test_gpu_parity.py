@@ -47,25 +47,38 @@ def kr_tol(oracle, T):
     return max(RATE_TOL, 8.0 * 6 * EPS * bmax)
 
 
-def check_rates(torch, pj, o, T, P, Y):
+RATES_OBSERVED = {}     # label -> largest relative errors of the rate arrays, next to the tolerance in force
+
+
+def check_rates(torch, pj, o, T, P, Y, label=None):
     dT, dP, dY = dev(torch, T, P, Y)
     got = {k: v.cpu().numpy() for k, v in pj.eval_rates(dT, dP, dY).items()}
     dy = pj.eval_dydt(dT, dP, dY).cpu().numpy()
     ref = o.source(T, P, Y)
     tiny = 1e-300
     tol_r = kr_tol(o, T)
-    assert np.all(np.abs(got["rf"] - ref["rf"]) <= RATE_TOL * np.abs(ref["rf"]) + tiny)
-    assert np.all(np.abs(got["rr"] - ref["rr"]) <= tol_r * np.abs(ref["rr"]) + tiny)
-    assert np.all(np.abs(got["cmod"] - ref["cmod"]) <= RATE_TOL * np.abs(ref["cmod"]) + tiny)
+    rel = lambda a, b: float((np.abs(a - b) / np.maximum(np.abs(b), tiny))[np.abs(b) > 0].max(initial=0.0))
     # production rates and source term: against the size of what was summed (C19); with reverse
     # rates entering, the bound is the reverse-rate one
     q = np.abs(ref["cmod"]) * (np.abs(ref["rf"]) + np.abs(ref["rr"]))
     scale_w = q.max(axis=1, keepdims=True)
+    seen = dict(rf=rel(got["rf"], ref["rf"]), rr=rel(got["rr"], ref["rr"]), cmod=rel(got["cmod"], ref["cmod"]),
+                wdot=float((np.abs(got["wdot"] - ref["wdot"]) / np.maximum(scale_w, tiny)).max(initial=0.0)),
+                kr_tol=tol_r)
+    assert np.all(np.abs(got["rf"] - ref["rf"]) <= RATE_TOL * np.abs(ref["rf"]) + tiny)
+    assert np.all(np.abs(got["rr"] - ref["rr"]) <= tol_r * np.abs(ref["rr"]) + tiny)
+    assert np.all(np.abs(got["cmod"] - ref["cmod"]) <= RATE_TOL * np.abs(ref["cmod"]) + tiny)
     assert np.all(np.abs(got["wdot"] - ref["wdot"]) <= tol_r * scale_w + tiny)
-    for part in (slice(0, 1), slice(1, None)):
+    for name, part in (("dTdt", slice(0, 1)), ("dYdt", slice(1, None))):
         scale = np.abs(ref["dydt"][:, part]).max(axis=1, keepdims=True)
-        bound = max(tol_r, RATE_TOL) * np.maximum(scale, _dydt_term_scale(o, ref, T, P, Y, part))
+        term = np.maximum(scale, _dydt_term_scale(o, ref, T, P, Y, part))
+        bound = max(tol_r, RATE_TOL) * term
+        seen[name] = float((np.abs(dy[:, part] - ref["dydt"][:, part]) / np.maximum(term, tiny)).max(initial=0.0))
         assert np.all(np.abs(dy[:, part] - ref["dydt"][:, part]) <= bound + tiny)
+    if label is not None:
+        best = RATES_OBSERVED.setdefault(label, dict(seen))
+        for k, v in seen.items():
+            best[k] = max(best[k], v)
     return got, dy
 
 
@@ -85,17 +98,92 @@ def _dydt_term_scale(o, ref, T, P, Y, part):
     return out[:, None]
 
 
-def check_jacobian(torch, pj, o, T, P, Y, tol=JAC_TOL):
+OBSERVED = {}       # label -> largest errors seen, printed at the end of the module (pytest -s) and written to gpurun_out/
+
+
+def jacobian_errors(J, Jr, ns):
+    """Errors of a batch of GPU Jacobians against the oracle's, each as a maximum over the batch:
+      fro   ||J - Jr||_F / ||Jr||_F per state (Eq. 132, north_star's wording).  On the seeded states the
+            energy row carries 0.9999998 of ||Jr||_F, so this alone says nothing about the species block;
+      row   per row r: ||J[r,:] - Jr[r,:]||_2 / ||Jr[r,:]||_2 (rows of the reference that are exactly
+            zero -- an inert species, Eq. 112 with nu_ki = 0 -- must be exactly zero: counted in `zero_bad`);
+      elem  per element: |J_rc - Jr_rc| / max_c' |Jr_rc'|.  An element of row r is a rounded sum of terms of
+            the size of the row's largest entries (the alpha_r d_c part of Eq. 112 is in every column), so
+            the row's largest entry is the scale rounding works at; elements far below it are cancelled
+            sums that no evaluation order reproduces to a relative 1e-10;
+      col   per column c with the energy row EXCLUDED: (||dJ[1:,c]||_2 - floor) / ||Jr[1:,c]||_2, floor =
+            1e-13 ||rowmax[1:]||_2: a column can consist of cancelled elements only, the floor is their
+            rounding (450 eps times the row scales)."""
+    ld = ns + 1
+    A = np.asarray(J).reshape(-1, ld, ld).transpose(0, 2, 1)      # [n][row][col]
+    B = np.asarray(Jr).reshape(-1, ld, ld).transpose(0, 2, 1)
+    D = A - B
+    tiny = 1e-300
+    fro = np.linalg.norm(D, axis=(1, 2)) / np.maximum(np.linalg.norm(B, axis=(1, 2)), tiny)
+    row_den = np.linalg.norm(B, axis=2)
+    row_num = np.linalg.norm(D, axis=2)
+    zero_rows = row_den == 0.0
+    zero_bad = int(np.count_nonzero(zero_rows & (np.abs(A).max(axis=2) != 0.0)))
+    row = np.where(zero_rows, 0.0, row_num / np.maximum(row_den, tiny))
+    rowmax = np.abs(B).max(axis=2, keepdims=True)
+    elem = np.abs(D) / np.maximum(rowmax, tiny)
+    elem = np.where(rowmax == 0.0, 0.0, elem)
+    col_den = np.linalg.norm(B[:, 1:, :], axis=1)
+    col_num = np.linalg.norm(D[:, 1:, :], axis=1)
+    floor = 1e-13 * np.linalg.norm(rowmax[:, 1:, 0], axis=1)[:, None]
+    col = np.maximum(col_num - floor, 0.0) / np.maximum(col_den, tiny)
+    col = np.where(col_den == 0.0, np.where(col_num > floor, np.inf, 0.0), col)
+    tcol = np.linalg.norm(D[:, 1:, 0], axis=1) / np.maximum(np.linalg.norm(B[:, 1:, 0], axis=1), tiny)
+    return dict(fro=float(fro.max(initial=0.0)), row=float(row.max(initial=0.0)), elem=float(elem.max(initial=0.0)),
+                col=float(col.max(initial=0.0)), tcol=float(tcol.max(initial=0.0)), zero_bad=zero_bad)
+
+
+def assert_jacobian(J, Jr, ns, tol=JAC_TOL, label=None):
+    """North_star's bound (Frobenius, 1e-10 per state) AND the same bound per row, per element against
+    its row's scale, per species-block column and on the T column (Eq. 111) alone."""
+    e = jacobian_errors(J, Jr, ns)
+    if label is not None:
+        best = OBSERVED.setdefault(label, dict(e))
+        for k, v in e.items():
+            best[k] = max(best[k], v)
+    assert e["zero_bad"] == 0, e
+    for k in ("fro", "row", "elem", "col", "tcol"):
+        assert e[k] <= tol, (k, e)
+    return e
+
+
+def check_jacobian(torch, pj, o, T, P, Y, tol=JAC_TOL, label=None):
     dT, dP, dY = dev(torch, T, P, Y)
     J = pj.eval_jacobian(dT, dP, dY).cpu().numpy()
     Jr = o.jacobian(T, P, Y)
-    num = np.linalg.norm(J - Jr, axis=1)
-    den = np.linalg.norm(Jr, axis=1)
     assert np.all(np.isfinite(J))
-    assert np.all(num <= tol * den), (num / den).max()
+    e = assert_jacobian(J, Jr, o.ns, tol, label)
     ld = o.ns + 1
     assert np.all(J.reshape(-1, ld, ld)[:, ld - 1, :] == 0.0)      # column Nsp is zero (C1)
-    return J, (num / np.maximum(den, 1e-300)).max()
+    return J, e["fro"]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _report_observed():
+    yield
+    if not OBSERVED and not RATES_OBSERVED:
+        return
+    import json
+    import os
+    if RATES_OBSERVED:
+        print("\nobserved maxima of the rate arrays, GPU vs oracle (R_f, c_i: 1e-12; the others: kr_tol):")
+        for k, v in sorted(RATES_OBSERVED.items()):
+            print("%-28s " % k + " ".join("%s=%.2e" % (n, x) for n, x in sorted(v.items())))
+    lines = ["%-28s " % k + " ".join("%s=%.2e" % (n, v[n]) for n in ("fro", "row", "elem", "col", "tcol"))
+             for k, v in sorted(OBSERVED.items())]
+    print("\nobserved maxima, GPU vs oracle (tolerance %.0e):\n" % JAC_TOL + "\n".join(lines))
+    out = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    try:
+        os.makedirs(out, exist_ok=True)
+        with open(os.path.join(out, "parity_observed.json"), "w") as f:
+            json.dump(dict(jacobian=OBSERVED, rates=RATES_OBSERVED), f, indent=1, sort_keys=True)
+    except OSError:
+        pass
 
 
 # ---------------------------------------------------------------------------------- small cases
@@ -104,8 +192,8 @@ def test_tiny_mechanisms_all_reaction_types(torch, PyJac, tiny_mechs):
     for m in tiny_mechs:
         o, pj = Oracle(m), PyJac(m)
         T, P, Y = synth.make_states(m.n_species, 257, 5, t_range=(500.0, 2800.0), p_range_atm=(0.05, 80.0))
-        check_rates(torch, pj, o, T, P, Y)
-        check_jacobian(torch, pj, o, T, P, Y)
+        check_rates(torch, pj, o, T, P, Y, label="tiny")
+        check_jacobian(torch, pj, o, T, P, Y, label="tiny")
 
 
 def test_tiny_mechanism_last_species_inert(torch, PyJac):
@@ -121,8 +209,8 @@ def test_config0_all_states(torch, PyJac):
     o, pj = Oracle(m), PyJac(m)
     T, P, Y = synth.config_states(0)
     assert len(T) == 1024
-    check_rates(torch, pj, o, T, P, Y)
-    check_jacobian(torch, pj, o, T, P, Y)
+    check_rates(torch, pj, o, T, P, Y, label="cfg0_all")
+    check_jacobian(torch, pj, o, T, P, Y, label="cfg0_all")
 
 
 @pytest.mark.parametrize("cfg,n", [(1, 1500), (2, 300), (3, 24)])
@@ -131,8 +219,8 @@ def test_config_prefix(torch, PyJac, cfg, n):
     m = synth.make_mechanism(cfg)
     o, pj = Oracle(m), PyJac(m)
     T, P, Y = synth.config_states(cfg, n)
-    check_rates(torch, pj, o, T, P, Y)
-    check_jacobian(torch, pj, o, T, P, Y)
+    check_rates(torch, pj, o, T, P, Y, label="cfg%d_prefix" % cfg)
+    check_jacobian(torch, pj, o, T, P, Y, label="cfg%d_prefix" % cfg)
 
 
 # ---------------------------------------------------------------------------------- full sizes
@@ -161,8 +249,7 @@ def test_config_full_size_sampled(torch, PyJac, cfg, chunk, n_sample):
         pick = np.sort(rng.choice(s1 - s0, size=min(n_sample, s1 - s0), replace=False))
         Jr = o.jacobian(T[s0:s1][pick], P[s0:s1][pick], Y[s0:s1][pick])
         Jg = J.reshape(-1, ld * ld)[torch.from_numpy(pick).cuda()].cpu().numpy()
-        err = np.linalg.norm(Jg - Jr, axis=1) / np.linalg.norm(Jr, axis=1)
-        assert err.max() <= JAC_TOL, err.max()
+        assert_jacobian(Jg, Jr, ns, label="cfg%d_full_sampled" % cfg)
     del buf
 
 
@@ -184,7 +271,7 @@ def test_state_count_sweep_rates_and_dydt(torch, PyJac):
         assert np.all(np.abs(dy[pick][:, 1:] - ref["dydt"][:, 1:]) <= bound)
         Jr = o.jacobian(T[pick], P[pick], Y[pick])
         Jg = J[torch.from_numpy(pick).cuda()].cpu().numpy()
-        assert (np.linalg.norm(Jg - Jr, axis=1) <= JAC_TOL * np.linalg.norm(Jr, axis=1)).all()
+        assert_jacobian(Jg, Jr, m.n_species, label="cfg4_sweep")
 
 
 # ---------------------------------------------------------------------------------- edge cases
@@ -315,7 +402,7 @@ def test_launch_shapes(torch, PyJac, monkeypatch, cfg, n, env):
     T, P, Y = synth.config_states(cfg, n)
     pj = PyJac(m)
     o = Oracle(m)
-    check_jacobian(torch, pj, o, T, P, Y)
+    check_jacobian(torch, pj, o, T, P, Y, label="launch_shapes")
     check_rates(torch, pj, o, T[:64], P[:64], Y[:64])
 
 

@@ -298,6 +298,36 @@ def test_falloff_pressure_limits():
     assert lo == pytest.approx(d["Pr"][0, 0], rel=1e-6)
 
 
+def test_sri_blending_by_its_special_cases():
+    """Eq. 36 pinned by what it reduces to, not by re-typing it:
+      P_r = 1       =>  X = 1 and F = d T^e (a e^{-b/T} + e^{-T/c}), no exponent left;
+      P_r -> 0, oo  =>  X -> 0 and F -> d T^e;
+      a = 1, b = 0, c -> oo, d = 1, e = 0  =>  F = 2^X, so 1/log2(F) - 1 = (log10 P_r)^2, which fixes
+                        the form of X and that its logarithm is base 10 (reading C13)."""
+    sri = (1.2, 500.0, 1800.0, 0.9, 0.15)
+    a, b, c, d, e = sri
+    Y = [[0.3, 0.2, 0.5]]
+    for rtype in (FALLOFF, CHEM_ACTIVATED):
+        o = Oracle(_falloff_mech(SRI, sri, rtype))
+        for T in (700.0, 1300.0, 2400.0):
+            P0 = 2.0 * PATM
+            Pr0 = o.details([T], [P0], Y)["Pr"][0, 0]
+            det = o.details([T], [P0 / Pr0], Y)                     # P_r is linear in P at fixed T, Y
+            assert det["Pr"][0, 0] == pytest.approx(1.0, rel=1e-13)
+            assert det["F"][0, 0] == pytest.approx(d * T ** e * (a * np.exp(-b / T) + np.exp(-T / c)), rel=1e-12)
+            for P in (1e-200, 1e200):                               # |log10 P_r| ~ 200: X ~ 2.5e-5
+                det = o.details([T], [P], Y)
+                X = 1.0 / (1.0 + np.log10(det["Pr"][0, 0]) ** 2)
+                assert X < 1e-4
+                assert det["F"][0, 0] == pytest.approx(d * T ** e, rel=2e-4)
+        o = Oracle(_falloff_mech(SRI, (1.0, 0.0, 1e300, 1.0, 0.0), rtype))
+        T, P, Yr = synth.make_states(3, 16, 9, p_range_atm=(1e-3, 1e3))
+        det = o.details(T, P, Yr)
+        F, Pr = det["F"][:, 0], det["Pr"][:, 0]
+        np.testing.assert_allclose(1.0 / np.log2(F) - 1.0, np.log10(Pr) ** 2, rtol=1e-9, atol=1e-11)
+
+
+
 # ------------------------------------------------------------------ P9 conservation
 @pytest.mark.parametrize("cfg", [0, 1])
 def test_mass_and_element_conservation(cfg):
@@ -406,21 +436,51 @@ def test_isomerisation_jacobian_by_hand():
 
 
 # ------------------------------------------------------------------ P11, P12, P14 whole Jacobian
+def _erel_paper(J, Jref):
+    """Eq. 131 over the elements the paper keeps, |J_ij| >= ||J||_F / 1e20."""
+    mask = np.abs(Jref) >= np.linalg.norm(Jref) / 1e20
+    return np.linalg.norm((Jref[mask] - J[mask]) / Jref[mask]), int(mask.sum())
+
+
 def _erel_filtered(J, Jref):
-    """Eq. 131 over the elements the paper keeps, |J_ij| >= ||J||_F / 1e20, and that
-    carry significant digits at all: |J_ij| >= 1e-8 max_j' |J_ij'| (reading C19b).  Every
-    element of row i is a sum of terms of the size of that row's largest entries, so an element
-    1e-8 below them has lost 8 of fp64's 16 digits to cancellation in BOTH Jacobians; on the
-    seeded far-from-equilibrium states (norms ~1e24) the paper's filter alone keeps such noise
-    (elements ~1e6 in rows ~1e21) and E_rel then measures rounding, not the formulas."""
+    """Eq. 131 over the elements the paper keeps AND that carry significant digits at all:
+    |J_ij| >= 1e-8 max_j' |J_ij'| (reading C19b).  Every element of row i is a
+    sum of terms of the size of that row's largest entries, so an element 1e-8 below them has lost 8
+    of fp64's 16 digits to cancellation in BOTH Jacobians; on the seeded far-from-equilibrium states
+    (norms ~1e24) the paper's filter alone keeps such noise (elements ~1e6 in rows ~1e21) and E_rel
+    then measures rounding, not the formulas."""
     mask = np.abs(Jref) >= np.linalg.norm(Jref) / 1e20
     mask &= np.abs(Jref) >= 1e-8 * np.abs(Jref).max(axis=1, keepdims=True)
-    return np.linalg.norm((Jref[mask] - J[mask]) / Jref[mask])
+    return np.linalg.norm((Jref[mask] - J[mask]) / Jref[mask]), int(mask.sum())
+
+
+def _assert_rows_and_columns(Ja, Jc, tol):
+    """Per ROW and per COLUMN relative 2-norms (the whole-matrix norm is the energy row: it carries
+    0.9999998 of ||J||_F on these states, so it says nothing about the species block, Eqs. 111-112).
+    The column check leaves the energy row out.  A row or column of the reference that is exactly
+    zero (inert species, the dependent column N_sp) must be exactly zero: no floor applies to it."""
+    row_den = np.linalg.norm(Jc, axis=1)
+    row_num = np.linalg.norm(Ja - Jc, axis=1)
+    assert np.all(row_num <= tol * row_den), (row_num / np.maximum(row_den, 1e-300)).max()
+    # element-wise against the largest entry of the element's row: an element is a rounded sum of terms
+    # of the size of its row's largest entries (the alpha_k d_j part of Eq. 112 is in every column), so
+    # this is what rounding allows; observed 7e-15 over all configurations
+    rowmax = np.abs(Jc).max(axis=1, keepdims=True)
+    assert np.all(np.abs(Ja - Jc) <= tol * rowmax)
+    # columns of the species block: a column can consist of cancelled elements only (each far below its
+    # row's scale), so the floor is the rounding of its elements, 64 eps ||rowmax||_2
+    col_den = np.linalg.norm(Jc[1:], axis=0)
+    col_num = np.linalg.norm(Ja[1:] - Jc[1:], axis=0)
+    floor = 64 * 2.220446049250313e-16 * np.linalg.norm(rowmax[1:])
+    assert np.all(col_num <= tol * col_den + floor), ((col_num - floor) / np.maximum(col_den, 1e-300)).max()
 
 
 def test_jacobian_vs_complex_step_tiny(tiny_mechs):
     """Every reaction type / falloff form / reverse treatment: analytic columns match the
-    complex-step derivative within 1e-8 relative (north_star; observed ~1e-14)."""
+    complex-step derivative within 1e-8 relative (north_star; observed ~1e-14).  Per row and per
+    column (energy row excluded) within 1e-12, so that the explicit-reverse (Eq. 69), irreversible and
+    single-species third-body (Eq. 85) terms -- which only these mechanisms contain -- are pinned in the
+    species rows themselves and not through their weight in the energy row."""
     for m in tiny_mechs:
         o = Oracle(m)
         T, P, Y = synth.make_states(m.n_species, 24, 21, t_range=(500.0, 2800.0),
@@ -432,13 +492,17 @@ def test_jacobian_vs_complex_step_tiny(tiny_mechs):
                 den = np.linalg.norm(Jc[s][:, c])
                 assert np.linalg.norm(Ja[s][:, c] - Jc[s][:, c]) <= 1e-8 * den + 1e-300
             assert np.linalg.norm(Ja[s] - Jc[s]) <= 1e-12 * np.linalg.norm(Jc[s])
+            _assert_rows_and_columns(Ja[s], Jc[s], 1e-12)
             assert np.all(Ja[s][:, -1] == 0.0) and np.all(Jc[s][:, -1] == 0.0)
 
 
 @pytest.mark.parametrize("cfg,n", [(0, 32), (1, 8), (2, 4), (3, 2)])
 def test_jacobian_paper_criterion_on_configs(cfg, n):
-    """agreement within 0.001 % (filtered E_rel <= 1e-5) between the
-    analytical Jacobian and the reference derivative, on every benchmark configuration."""
+    """agreement within 0.001 % (E_rel <= 1e-5) between the analytical Jacobian
+    and the reference derivative, on every benchmark configuration -- under reading C19b's filter;
+    under the paper's filter alone the cancelled elements' rounding noise dominates E_rel (observed up
+    to 3.5e-5 on single states), so that figure is only bounded loosely here and the per-row,
+    per-column and per-element checks carry the weight (observed < 1e-14)."""
     m = synth.make_mechanism(cfg)
     o = Oracle(m)
     T, P, Y = synth.config_states(cfg, n)
@@ -446,7 +510,11 @@ def test_jacobian_paper_criterion_on_configs(cfg, n):
     Jc = as_matrix(o.jacobian_complex_step(T, P, Y), m.n_species)
     for s in range(n):
         assert np.linalg.norm(Ja[s] - Jc[s]) <= 1e-11 * np.linalg.norm(Jc[s])
-        assert _erel_filtered(Ja[s], Jc[s]) <= 1e-5
+        _assert_rows_and_columns(Ja[s], Jc[s], 1e-12)
+        e_c19b, _ = _erel_filtered(Ja[s], Jc[s])
+        e_paper, _ = _erel_paper(Ja[s], Jc[s])
+        assert e_c19b <= 1e-5
+        assert e_paper <= 1e-3
 
 
 def test_jacobian_species_columns_sum_to_zero(tiny_mechs):
