@@ -6,16 +6,16 @@
 // modification (Eq. 20).  Reactions are stored in a SORTED order (most expensive rate form first,
 // the plain elementary ones last); `rxn_orig` maps back to the caller's order.
 //
-// The evaluation is a chain of fixed-order gathers over one per-state array `E` in shared memory:
-//   phase 1 writes, per reaction, the reusable products of Section 4.1:
-//           the sparse derivative terms s'_ij (region V), q_i, a_i, Theta_dT,i (region Q,
-//           interleaved per reaction) and the reaction enthalpy H_i (region H);
-//   the A1 gathers sum them into per-species / per-column quantities (wdot_k, alpha_r, gamma_r,
-//           the T column, the column sums of the energy row);
-//   a short FIX step finishes the energy row (Eq. 113);
-//   the CELL gathers sum, for every structurally non-zero Jacobian entry, its list of s'_ij into a
-//           tile (a panel of Jacobian columns) that follows E in shared memory;
-//   the DENSE pass adds the rank-two part of Eq. 112 to the tile and streams it to HBM.
+// One CTA evaluates NP blocks of S states at a time.  Every block owns one array `E` in shared memory
+// (element e of state q at (e * S + q) doubles); the evaluation is a chain of fixed-order gathers over it:
+//   P1  writes, per reaction, the reusable products of Section 4.1: the sparse
+//       derivative terms s'_ij (region V), q_i, a_i, Theta_dT,i (region Q, interleaved per reaction)
+//       and the reaction enthalpy H_i (region H);
+//   A   sums them into per-species / per-column quantities (wdot_k, alpha'_r, gamma'_r, the T column,
+//       the column sums of the energy row) and sums the long Jacobian-cell lists piecewise (region Hs);
+//   B   walks the Jacobian column by column, lane <-> two rows: each cell gathers its (short) list,
+//       adds the rank-two part of Eq. 112 and is streamed to HBM; the energy row (Eq. 113) is finished
+//       and stored by the FIX items of the same phase.
 #pragma once
 #include <cstdint>
 
@@ -24,6 +24,8 @@ namespace pyjac {
 constexpr double kRu = 8314.46261815324;   // J kmol^-1 K^-1
 constexpr double kPatm = 101325.0;         // Pa
 constexpr int kMaxSide = 3;                // species per reaction side
+constexpr int kMaxNP = 4;                  // blocks of S states per CTA iteration
+constexpr int kMaxThreads = 512;           // threads per CTA the kernels are compiled for
 
 // meta word of a reaction: bits 0..23 six 4-bit nu (slots 0-2 reactants, 3-5 products; 0 = empty
 // slot), 24..26 rxn_type, 27..28 rev_type, 29..30 falloff_form, 31 third body is a single species.
@@ -36,25 +38,28 @@ __host__ __device__ inline int meta_rev(uint32_t m) { return (m >> 27) & 3; }
 __host__ __device__ inline int meta_form(uint32_t m) { return (m >> 29) & 3; }
 __host__ __device__ inline int meta_single(uint32_t m) { return (m >> 31) & 1; }
 
-// A gather entry of the kAuxS1 / kAuxT3 lists: bits 0..18 = byte offset of the source element in
-// the CTA's interleaved E array (E index * S * 8), bits 19..31 = the top 13 bits of the fp64
-// coefficient (exact for +-1, 2, 3, 4, 6, 8; other small integers are split into two entries).
-constexpr uint32_t kEntOffMask = 0x7FFFFu;
-__host__ __device__ inline uint32_t coef_hi13(int coef)
+// A gather entry of the kSum1 / kSum3 lists and of the Jacobian cells: bits 0..17 = byte offset of the
+// source element in the block's E array (E index * S * 8, below 256 KB), bits 18..31 = the top 14 bits
+// of the fp64 coefficient (sign, exponent, two mantissa bits: exact for every integer up to 8 in
+// magnitude; larger ones are split into two entries).  Coefficient bits 0 = the padding entry.
+constexpr uint32_t kEntOffMask = 0x3FFFFu;
+__host__ __device__ inline uint32_t coef_hi14(int coef)
 {
     uint32_t a = coef < 0 ? uint32_t(-coef) : uint32_t(coef);
-    uint32_t hi = a == 1 ? 0x3FF0u : a == 2 ? 0x4000u : a == 3 ? 0x4008u : a == 4 ? 0x4010u
-                : a == 6 ? 0x4018u : a == 8 ? 0x4020u : 0u;
-    if (coef < 0) hi |= 0x8000u;
-    return (hi >> 3) << 19;
+    // high word of the double a, for 1 <= a <= 8
+    static const uint32_t hi[9] = {0u,          0x3FF00000u, 0x40000000u, 0x40080000u, 0x40100000u,
+                                   0x40140000u, 0x40180000u, 0x401C0000u, 0x40200000u};
+    uint32_t h = a <= 8 ? hi[a] : 0u;
+    if (coef < 0) h |= 0x80000000u;
+    return h & ~kEntOffMask;
 }
 
-// kinds of gather chunks
+// kinds of phase-A chunks (32 lanes, 32 >> rshift sums each)
 enum : uint32_t {
-    kAuxT3 = 0,    // entries {q_i of reaction i, nu_ki}: sums of nu q_i, nu a_i, nu Theta_i -> wdot_k, alpha_{k+1}, T column
-    kAuxS1 = 1,    // entries {source, coef}: one sum, times a task constant -> E / tile slot
-    kAuxH2 = 2,    // entries {index a | index b << 16}: sum of E[a] * E[b] -> E slot
-    kAuxR3 = 3,    // no entries: sums over all reactions of H_i {q_i, a_i, Theta_i} -> S1, A0, S4
+    kSum3 = 0,     // entries {q_i of reaction i, nu_ki}: sums of nu q_i, nu a_i, nu Theta_i -> wdot_k, alpha'_{k+1}, T column
+    kSum1 = 1,     // entries {source, coef}: one sum, times a task constant -> E slot
+    kProd = 2,     // entries {index a | index b << 16}: sum of E[a] * E[b] -> E slot
+    kAll3 = 3,     // no entries: sums over all reactions of H_i {q_i, a_i, Theta_i} -> S1, A0, S4
 };
 
 struct DeviceMech {
@@ -63,9 +68,9 @@ struct DeviceMech {
     // ---- species tables
     const double *inv_mw;       // [ns]
     const double *mw;           // [ns]
-    const double *colc;         // [ns+1][2] column constants by Jacobian column c: {d_j, g_c}, j = c - 1;
-                                //        d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51); g_c = 1 where
-                                //        gamma_r applies (1 <= c < ns), else 0; c = 0 and c = ns: zeros
+    const double *colc;         // [ns+1][4] column constants by Jacobian column c: {u_c, v_c, 1/W_j, 0}, j = c - 1:
+                                //        u_c = W_j d_j with d_j = 1/W_j - 1/W_Ns (the d rho / d Y_j factor, Eq. 51);
+                                //        v_c = W_j where gamma_r applies (1 <= c < ns); c = 0: {0, 0, 1}; c = ns: zeros
     const double *wrow;         // [ns+1] row factors by Jacobian row r: {1, W_0 .. W_{ns-1}}
     const double *nasa;         // [2][5][ns] a_0..a_4, range-major, coefficient-major (coalesced over k)
     const double *t_mid;        // [ns]
@@ -74,11 +79,8 @@ struct DeviceMech {
     int n_pk;                   // PLOG / Chebyshev reactions: [n_pd, n_pd + n_pk)
     int n_rchunk;               // groups of 32 reactions
     int split_general;          // 1: the group that holds reaction n_pd is two work items (pressure-dependent lanes /
-                                // the others).  Shortens the longest item; set when one CTA per SM leaves the
-                                // reaction queue latency-bound (cfg2: 10.51 -> 10.23 ms), not otherwise (cfg1:
-                                // 2.69 -> 2.83 ms, the extra item costs issue slots the other CTA would use)
+                                // the others); shortens the longest item of the reaction queue
     int n_plain;                // the last n_plain groups hold only plain reactions
-    const uint32_t *rchunk;     // [n_rchunk] 1 = every reaction of the group takes the plain path
     const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
     const uint4 *vidx;          // [nr] E indices of the slots' s'_ij: {v0|v1<<16, v2|v3<<16, v4|v5<<16, 0}
                                 //      (empty slots point at the dump slot)
@@ -103,35 +105,33 @@ struct DeviceMech {
     const int32_t *pk_ptr;      // [n_pk+1] offsets into pk_data
     const double *pk_data;      // PLOG: n, then n x {p, ln p, ln A, beta, Ta};
                                 // Chebyshev: nT, nP, 1/Tmin, 1/Tmax, log10 pmin, log10 pmax, eta[nT*nP]
-    // ---- gathers: chunks of 32 lanes, 32 >> rshift sums each, sorted by length at create time.
-    // Chunks [0, n_a1) are the A1 phase (the first n_a1_01 of them serve rates / dydt too); the
-    // chunks of the cells of column panel p are [panel_ptr[p], panel_ptr[p+1]).
-    int n_a1, n_a1_01;
-    const uint2 *achunk;        // {first block of a_ent, steps | kind << 16 | rshift << 20 | sums per lane << 24}
-    const uint4 *a_ent;         // block r of a chunk = a_ent[first + 32 r + lane].  One sum per lane: block 0 =
-                                // {output E index (kAuxT3: species k; ~0 = none), constant factor (fp64 bits, 2
-                                // words), entry of step 0}; block r >= 1: the entries of steps 4r-3 .. 4r.  Two
-                                // sums A, B per lane (kAuxS1 only): blocks 0 and 1 are the records of A and B,
-                                // block r >= 2 = {A, B of step 2r-3, A, B of step 2r-2}
-    const int32_t *panel_ptr;   // [n_panel + 1]
-    // ---- the tile: column panels of the Jacobian, state-interleaved like E, element (r, c) of
-    // panel p at E index eTile + (p % nbuf) * pw * ld + (c - p * pw) * ld + r
-    int n_panel, pw, nbuf;
-    int eTile;
-    int pair;                   // 1: ld is even, the DENSE pass owns two rows per lane (16-byte stores)
-    int d_seg;                  // columns per DENSE work item
-    int n_slab;                 // slabs of rows of the DENSE pass: 64 rows each if pair, else 32
-    // ---- regions of E (indices in doubles per state)
+    // ---- phase A: chunks of 32 lanes, 32 >> rshift sums each, sorted by length at create time and
+    // arranged in rows of NW chunks (warp w takes chunk row * NW + w); rows [0, n_arow01) serve the
+    // rates / source-term kernels too
+    int n_arow, n_arow01;
+    const uint2 *achunk;        // {first block of a_ent, steps | kind << 8 | rshift << 12}
+    const uint4 *a_ent;         // block 0 of a chunk = a_ent[first + lane] = {output E index (kSum3: species k;
+                                // ~0 = none), constant factor (fp64 bits, 2 words), 0}; block b >= 1 =
+                                // a_ent[first + 32 b + lane] = the lane's entries of steps 4b-4 .. 4b-1
+    // ---- phase B: one item per (slab of rows, Jacobian column), slab-major.  A lane owns `rp` rows
+    // (rp = 2: rows 64 slab + 2 lane, + 1, stored with one 16-byte store; rp = 1 when ld is odd).
+    int rp, n_slab;
+    const uint2 *bitem;         // [n_slab * ld] {first block of b_ent, steps of the first row | steps of the second << 8}
+    const uint4 *b_ent;         // b_ent[first + lane] = up to four entries of the lane's first cell,
+                                // b_ent[first + 32 + lane] of its second cell (rp = 2)
+    const int32_t *bsplit;      // [NW + 1] the items of warp w are [bsplit[w], bsplit[w + 1])
+    // ---- regions of E (indices in elements per state)
     int eQ;                     // [nr][3] {q_i, a_i + W q_i, Theta_dT,i}
     int eH;                     // [nr] reaction enthalpy H_i
-    int eAlpha, eGamma;         // [ns+1] by Jacobian row; row 0 stays 0
+    int eAlpha, eGamma;         // [ns+1] alpha'_r = A_k / rho, gamma'_r = Gamma_k / W_Ns by Jacobian row r = k + 1
+    int eTc;                    // [ns+1] the T column by row: sum_i nu_ki Theta_i / rho (Eq. 111 without W_k)
     int eWdot;                  // [ns]
     int eG0;                    // [ns]   sum_i H_i s'_ij per column species j
-    int eZ;                     // [ns+1] finished energy row J(0, c)
     int eS1, eA0, eS4;          // scalars: sum_i H_i q_i, sum_i H_i a_i, sum_i H_i Theta_i
-    int eZero;                  // a slot that stays 0 (padding of the lists)
+    int eZero;                  // slots that stay 0 (padding of the lists)
     int eDump;                  // a slot nobody reads (stores of empty reaction slots)
-    int n_e;                    // size of E without the tile
+    int eHs;                    // partial sums of the long Jacobian-cell lists
+    int n_e;                    // size of E
 };
 
 // per-state scalars (region Scal of the shared-memory plan)
@@ -139,19 +139,19 @@ enum {
     kT = 0, kLnT, kInvT, kP, kLnP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kIcp, kNScal = 12
 };
 
-// Shared-memory plan (offsets in doubles PER STATE).  A CTA evaluates S states at a time and
-// interleaves them: element i of region R of state q lives at (R + i) * S + q.  The mixture block
-// (X, Cp, Scal) exists twice: the block of the next batch is filled while this one is in use.  After
-// the S interleaved state blocks come the state-independent tables (colc, wrow), loaded once per CTA.
+// Shared-memory plan (offsets in doubles PER STATE).  A block of S states is interleaved: element i of
+// region R of state q lives at (R + i) * S + q within the block; NP blocks follow one another.  The
+// mixture part (X, Cp, Scal) exists twice: the one of the next batch is filled while this one is in
+// use.  After the NP blocks come the state-independent tables (colc, wrow), loaded once per CTA.
 struct SmemPlan {
-    int E;                              // [n_e + tile]
-    int P0;                             // three mixture blocks of p0size doubles
+    int E;                              // [n_e]
+    int P0;                             // two mixture parts of p0size doubles
     int p0size;
-    int oX;                             // within a mixture block: [ns+1] concentrations; slot ns = 1 (empty reaction slots)
+    int oX;                             // within a mixture part: [ns+1] concentrations; slot ns = 1 (empty reaction slots)
     int oCp;                            // [ns] c_pk (mass based)
     int oScal;                          // [kNScal]
     int total;                          // doubles per state
-    int colc;                           // [ld][2], offset in doubles from the end of the state blocks
+    int colc;                           // [ld][4], offset in doubles from the end of the blocks
     int wrow;                           // [ld]
     int shared_total;                   // doubles of the state-independent part
 };
@@ -169,11 +169,11 @@ inline SmemPlan make_smem_plan(int ns, int n_e)
         p.oCp = take(ns) - base;
         p.oScal = take(kNScal) - base;
         p.p0size = o - base;
-        o += 2 * p.p0size;
+        o += p.p0size;
     }
     p.total = o;
     o = 0;
-    p.colc = take(2 * (ns + 1));
+    p.colc = take(4 * (ns + 1));
     p.wrow = take(ns + 1);
     p.shared_total = o;
     return p;

@@ -1,30 +1,27 @@
 // kernels.cu -- sm_100a kernels for the batched source term and analytical Jacobian.
 //
-// One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop; the S
-// states are interleaved in shared memory (element i of a region for state q at (R + i) * S + q), so
-// whatever does not depend on the state -- decoding a reaction, a gather entry, a column constant --
-// is done once and applied to the S states with one vector load.  Per iteration:
-//   P0    mixture (Eqs. 3-5) and species, warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT
-//         (Eqs. 9-13, 54-55); computed one batch ahead, as an item of P1
-//   P1    reactions, lane <-> reaction, groups of 32: k_f, k_r (K_c from the per-reaction polynomial
-//         of device_mech.h `th_data`), R_f, R_r, c_i and the reusable per-reaction products of
-//         Section 4.1 into E: q_i, Theta_dT,i, a_i (the coefficient of d_j), the
-//         sparse terms s'_ij, the enthalpy H_i.  Groups made only of plain elementary reactions take
-//         a branch-free path that evaluates two states at a time.
-//   A1    fixed-order gathers over E, lane <-> sum: wdot_k (Eq. 14), alpha_r, gamma_r of Eq. 112, the
-//         T column (Eq. 111), the column sums of the energy row (Eq. 113).
-//   FIX   the energy row, Eq. 113
-//   CELLS lane <-> structurally non-zero Jacobian entry (sorted by list length, so the 32 lanes of a
-//         chunk walk lists of equal length): sum_i nu_ki s'_ij times W_k / W_j into the tile
-//   DENSE lane <-> two rows, walking columns:  J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c,
-//         which is Eq. 112 with the per-reaction terms of Eqs. 118-127 regrouped by what they multiply
-//         (DESIGN.md "Regrouping"); a warp stores 512 contiguous bytes per state and column.
-// Mechanisms whose tile does not fit are walked in column panels (two tile buffers: the cells of
-// panel p are gathered while panel p - 1 streams out).  There are no atomics on data: every sum
-// has an order fixed at pyjac_mech_create.
+// One CTA evaluates NP blocks of S thermochemical states per iteration of a persistent grid-stride loop.
+// The S states of a block are interleaved in shared memory (element i of a region for state q at
+// (R + i) * S + q), so whatever does not depend on the state -- decoding a reaction, a gather entry, a
+// column constant -- is done once per lane and applied to the S states of each of the NP blocks with
+// vector loads.  Per iteration, separated by CTA barriers:
+//   P0  mixture (Eqs. 3-5) and species, warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT
+//       (Eqs. 9-13, 54-55); computed one iteration ahead, at the end of phase B
+//   P1  reactions, lane <-> reaction, groups of 32 from one dynamic queue: k_f, k_r (K_c from the
+//       per-reaction polynomial of device_mech.h `th_data`), R_f, R_r, c_i and the reusable per-reaction
+//       products of Section 4.1 into E: q_i, Theta_dT,i, a_i (the coefficient of d_j),
+//       the sparse terms s'_ij, the enthalpy H_i.  Groups made only of plain elementary reactions take a
+//       branch-free path that evaluates two states at a time.
+//   A   fixed-order gathers over E, lane <-> sum (or a share of one): wdot_k (Eq. 14), alpha'_r, gamma'_r
+//       of Eq. 112, the T column (Eq. 111), the column sums of the energy row (Eq. 113), and the long
+//       Jacobian-cell lists piece by piece
+//   B   the Jacobian, column by column, lane <-> two rows: every cell gathers its (at most four) entries
+//       on top of alpha'_r u_c - gamma'_r v_c, which is Eq. 112 with the per-reaction terms of Eqs.
+//       118-127 regrouped by what they multiply, and is stored at once: a warp
+//       stores 512 contiguous bytes per state and column, nothing is staged.  FIX items of the same phase
+//       finish and store the energy row (Eq. 113).
+// There are no atomics on data: every sum has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
-
-#include <cstdio>
 
 #include "device_mech.h"
 #include "kernels.h"
@@ -32,13 +29,6 @@
 namespace pyjac {
 
 namespace {
-
-// -DPYJAC_PROF: CTA 0 prints the cycles warp 0 spends in each phase of its fourth iteration
-#ifdef PYJAC_PROF
-#define PROF_MARK(i) do { if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x) prof_t[i] = clock64(); } while (0)
-#else
-#define PROF_MARK(i) do { } while (0)
-#endif
 
 constexpr double kLn10 = 2.302585092994045684;
 constexpr double kInvLn10 = 0.434294481903251828;
@@ -527,616 +517,536 @@ __device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double 
     }
 }
 
-// ---- one gather chunk: 32 lanes, 32 >> rshift sums (device_mech.h).  `r0` is block 0 of the chunk
-// (output index, constant, first entry) and `e1` block 1 (steps 1..4; anything if steps < 2), both
-// fetched by the caller one chunk ahead.
-template <int LEVEL, int S>
-__device__ __forceinline__ void gather_chunk(const DeviceMech &m, double *E, const double *sc, const uint2 ch,
-                                             const uint4 r0, const uint4 e1, int lane)
-{
-    const uint32_t kind = (ch.y >> 16) & 0xF;
-    const int rshift = (int)(ch.y >> 20) & 0xF, width = 1 << rshift;
-    const bool two = (ch.y >> 24) == 2;                  // two sums per lane: `e1` is the record of the second
-    const int steps = (int)(ch.y & 0xFFFF);
-    const uint4 *ep = m.a_ent + ch.x + lane;
-    const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
-    const char *Eb = reinterpret_cast<const char *>(E);
-    const uint4 ez = make_uint4(0u, 0u, 0u, 0u);
-    const int nr = m.nr;
-    int left = steps - 1;                                   // steps after the one in block 0
-    uint4 e = e1;
-
-    if (kind == kAuxS1) {
-        if (LEVEL == 2) {
-            if (two) {
-                double accA[S], accB[S];
-#pragma unroll
-                for (int q = 0; q < S; ++q) { accA[q] = 0.0; accB[q] = 0.0; }
-                auto step2 = [&](uint32_t wa, uint32_t wb) {
-                    const double ca = entry_coef(wa), cb = entry_coef(wb);
-                    double a[S], b[S];
-                    ldv<S>(reinterpret_cast<const double *>(Eb + (wa & kEntOffMask)), a);
-                    ldv<S>(reinterpret_cast<const double *>(Eb + (wb & kEntOffMask)), b);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) { accA[q] = fma(ca, a[q], accA[q]); accB[q] = fma(cb, b[q], accB[q]); }
-                };
-                uint4 w = left > 0 ? ep[64] : ez;
-                if (steps > 0) step2(r0.w, e1.w);
-                for (int r = 3; left > 0; ++r, left -= 2) {
-                    const uint4 wn = left > 2 ? ep[r * 32] : ez;
-                    step2(w.x, w.y);
-                    if (left > 1) step2(w.z, w.w);
-                    w = wn;
-                }
-                if (r0.x != 0xFFFFFFFFu) {
-                    const double cst = __hiloint2double((int)r0.z, (int)r0.y);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) accA[q] *= cst;
-                    stv<S>(E + r0.x * S, accA);
-                }
-                if (e1.x != 0xFFFFFFFFu) {
-                    const double cst = __hiloint2double((int)e1.z, (int)e1.y);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) accB[q] *= cst;
-                    stv<S>(E + e1.x * S, accB);
-                }
-                return;
-            }
-            double acc[S];
-#pragma unroll
-            for (int q = 0; q < S; ++q) acc[q] = 0.0;
-            auto step = [&](uint32_t w) {
-                const double cf = entry_coef(w);
-                double a[S];
-                ldv<S>(reinterpret_cast<const double *>(Eb + (w & kEntOffMask)), a);
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
-            };
-            if (steps > 0) step(r0.w);
-            for (int r = 2; left > 0; ++r, left -= 4) {
-                const uint4 en = left > 4 ? ep[r * 32] : ez;
-                step(e.x);
-                if (left > 1) {
-                    step(e.y);
-                    if (left > 2) {
-                        step(e.z);
-                        if (left > 3) step(e.w);
-                    }
-                }
-                e = en;
-            }
-            if (rshift > 0)
-                for (int o = 1; o < width; o <<= 1)
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
-            if (head) {
-                const double cst = __hiloint2double((int)r0.z, (int)r0.y);
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] *= cst;
-                stv<S>(E + r0.x * S, acc);
-            }
-        }
-    } else if (kind == kAuxH2) {
-        if (LEVEL == 2) {
-            double acc[S];
-#pragma unroll
-            for (int q = 0; q < S; ++q) acc[q] = 0.0;
-            auto step = [&](uint32_t w) {
-                double a[S], b[S];
-                ldv<S>(E + (w & 0xFFFF) * S, a);
-                ldv<S>(E + (w >> 16) * S, b);
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
-            };
-            if (steps > 0) step(r0.w);
-            for (int r = 2; left > 0; ++r, left -= 4) {
-                const uint4 en = left > 4 ? ep[r * 32] : ez;
-                step(e.x); step(e.y); step(e.z); step(e.w);      // padded with the zero slot
-                e = en;
-            }
-            for (int o = 1; o < width; o <<= 1)
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
-            if (head) stv<S>(E + r0.x * S, acc);
-        }
-    } else {
-        // kAuxT3 / kAuxR3: three sums at once (one for the rates / source-term kernels)
-        constexpr int NA = LEVEL == 2 ? 3 : 1;
-        double acc[NA][S];
-#pragma unroll
-        for (int w = 0; w < NA; ++w)
-#pragma unroll
-            for (int q = 0; q < S; ++q) acc[w][q] = 0.0;
-        if (kind == kAuxT3) {
-            auto step = [&](uint32_t w_) {
-                const double cf = entry_coef(w_);
-                const double *p = reinterpret_cast<const double *>(Eb + (w_ & kEntOffMask));
-#pragma unroll
-                for (int w = 0; w < NA; ++w) {
-                    double a[S];
-                    ldv<S>(p + w * S, a);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[w][q] = fma(cf, a[q], acc[w][q]);
-                }
-            };
-            if (steps > 0) step(r0.w);
-            for (int r = 2; left > 0; ++r, left -= 4) {
-                const uint4 en = left > 4 ? ep[r * 32] : ez;
-                step(e.x); step(e.y); step(e.z); step(e.w);      // padded with the zero slots
-                e = en;
-            }
-        } else {
-            for (int i = lane; i < nr; i += 32) {
-                double h[S];
-                ldv<S>(E + (m.eH + i) * S, h);
-#pragma unroll
-                for (int w = 0; w < NA; ++w) {
-                    double a[S];
-                    ldv<S>(E + (m.eQ + 3 * i + w) * S, a);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[w][q] = fma(h[q], a[q], acc[w][q]);
-                }
-            }
-        }
-        for (int o = 1; o < width; o <<= 1)
-#pragma unroll
-            for (int w = 0; w < NA; ++w)
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[w][q], o);
-        constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
-        if (kind == kAuxR3) {
-            if (lane == 0) {
-                stv<S>(E + m.eS1 * S, acc[0]);
-                if (LEVEL == 2) { stv<S>(E + m.eA0 * S, acc[iA]); stv<S>(E + m.eS4 * S, acc[iT]); }
-            }
-        } else if (head) {
-            const uint32_t k = r0.x;
-            stv<S>(E + (m.eWdot + k) * S, acc[0]);
-            if (LEVEL == 2) {
-                // alpha_{k+1} of Eq. 112 regrouped, and the T column (Eq. 111) straight into the tile
-                const double wk = m.mw[k];
-                double al[S], tc[S];
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    const double wi = wk * sc[kIrho * S + q];
-                    al[q] = wi * acc[iA][q];
-                    tc[q] = wi * acc[iT][q];
-                }
-                stv<S>(E + (m.eAlpha + k + 1) * S, al);
-                stv<S>(E + (m.eTile + k + 1) * S, tc);
-            }
-        }
-    }
-}
-
-// The gather chunks of a batch are one table in execution order (A1, then the cells panel by panel),
-// arranged by mech_pack.cu in full rows of NW chunks balanced by cost, the header table padded: warp w
-// takes chunk c + w of the row that starts at c, without bounds checks.  The pipe carries the table
-// reads across phases and barriers: headers three rows ahead, a chunk's blocks 0 and 1 one row ahead,
-// so that only the first chunk of a batch waits for its tables.
-struct GatherPipe {
-    const uint2 *hp;
-    uint2 h, h1, h2;
-    uint4 r0, e1;
-};
-
-template <int NW>
-__device__ __forceinline__ void gather_start(GatherPipe &g, const DeviceMech &m, int c0, int warp, int lane)
-{
-    g.hp = m.achunk + c0 + warp;
-    g.h = g.hp[0]; g.h1 = g.hp[NW]; g.h2 = g.hp[2 * NW];
-    g.r0 = m.a_ent[g.h.x + lane];
-    g.e1 = m.a_ent[g.h.x + 32 + lane];
-}
-
-// the chunks [c0, c1) (whole rows), continuing where the pipe stands
-template <int LEVEL, int S, int NW>
-__device__ __forceinline__ void gather_run(GatherPipe &g, const DeviceMech &m, double *E, const double *sc, int c0,
-                                           int c1, int lane)
-{
-    const uint4 *ent = m.a_ent + lane;
-    for (int ch = c0; ch < c1; ch += NW, g.hp += NW) {
-        const uint2 h3 = g.hp[3 * NW];
-        const uint4 r0n = ent[g.h1.x], e1n = ent[g.h1.x + 32];
-        gather_chunk<LEVEL, S>(m, E, sc, g.h, g.r0, g.e1, lane);
-        g.h = g.h1; g.h1 = g.h2; g.h2 = h3; g.r0 = r0n; g.e1 = e1n;
-    }
-}
-
-template <int LEVEL, int S, int NW>
-__device__ __forceinline__ void gather_phase(const DeviceMech &m, double *E, const double *sc, int c0, int c1, int warp,
-                                             int lane)
-{
-    GatherPipe g;
-    gather_start<NW>(g, m, c0, warp, lane);
-    gather_run<LEVEL, S, NW>(g, m, E, sc, c0, c1, lane);
-}
-
 // 16-byte streaming store of two consecutive Jacobian rows
 __device__ __forceinline__ void st_cs_v2(double *p, double a, double b)
 {
     asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a), "d"(b) : "memory");
 }
 
-// ---- FIX item `it` of one batch: the energy row (Eq. 113), stored by the lanes that finish it (DENSE
-// skips row 0).  Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 .. (column ns is zero)
-template <int S>
-__device__ __forceinline__ void fix_item(const DeviceMech &m, const double *E, const double *Cp, const double *sc,
-                                         const double *colc, const double *wrow, int it, int lane, double *J0, int nq)
+// ---- phase A, one chunk: 32 lanes, 32 >> rshift sums (device_mech.h), for the NP blocks at once:
+// an entry is decoded once and applied to every block
+template <int LEVEL, int S, int NP>
+__device__ __forceinline__ void a_chunk(const DeviceMech &m, double *E0, uint32_t blk_bytes, const double *sc0,
+                                        const uint2 ch, int lane)
 {
-    const int ns = m.ns, ld = m.ld;
-    const long long Jstate = (long long)ld * ld;
-    if (it == 0) {
-        double s3[S];       // sum_k c_pk W_k wdot_k
-#pragma unroll
-        for (int q = 0; q < S; ++q) s3[q] = 0.0;
-        for (int k = lane; k < ns; k += 32) {
-            const double wk = wrow[k + 1];
-            double cp[S], wd[S];
-            ldv<S>(Cp + k * S, cp);
-            ldv<S>(E + (m.eWdot + k) * S, wd);
-#pragma unroll
-            for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-            for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
-        if (lane < S) {
-            const int q = lane;
-            double s = s3[0];
-#pragma unroll
-            for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
-            const double icp = sc[kIcp * S + q];
-            const double z = -icp * sc[kIrho * S + q] *
-                             (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
-            if (q < nq) J0[q * Jstate] = z;
-        }
-        return;
-    }
-    const int c = (it - 1) * 32 + lane + 1;
-    if (c < ns) {
-        const double dx = colc[2 * c];
-        const double wj = wrow[c], iwj = m.inv_mw[c - 1], iwl = m.inv_mw[ns - 1];
-        double icp[S], irho[S], s1[S], a0[S], gl[S], cpj[S], cpl[S], g0[S];
-        ldv<S>(sc + kIcp * S, icp);
-        ldv<S>(sc + kIrho * S, irho);
-        ldv<S>(E + m.eS1 * S, s1);
-        ldv<S>(E + m.eA0 * S, a0);
-        ldv<S>(E + (m.eG0 + ns - 1) * S, gl);
-        ldv<S>(Cp + (c - 1) * S, cpj);
-        ldv<S>(Cp + (ns - 1) * S, cpl);
-        ldv<S>(E + (m.eG0 + c - 1) * S, g0);
-#pragma unroll
-        for (int q = 0; q < S; ++q) {
-            const double a1 = irho[q] * s1[q] * icp[q] * icp[q];     // coefficient of c_pj - c_pNs
-            const double alpha0 = -(irho[q] * icp[q]) * a0[q];
-            const double gamma0 = -(iwl * icp[q]) * gl[q];
-            const double z = (wj * (alpha0 * dx - gamma0 + a1 * (cpj[q] - cpl[q])) - icp[q] * g0[q]) * iwj;
-            if (q < nq) J0[q * Jstate + (long long)c * ld] = z;
-        }
-    } else if (c == ns) {
-#pragma unroll
-        for (int q = 0; q < S; ++q)
-            if (q < nq) J0[q * Jstate + (long long)c * ld] = 0.0;
-    }
-}
+    const uint32_t kind = (ch.y >> 8) & 0xF;
+    const int steps = (int)(ch.y & 0xFF), rshift = (int)(ch.y >> 12) & 0xF, width = 1 << rshift;
+    const uint4 *ep = m.a_ent + ch.x + lane;
+    const uint4 r0 = ep[0];
+    const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
+    const char *Eb = reinterpret_cast<const char *>(E0);
+    const int nr = m.nr;
 
-// ---- DENSE item `it` of panel pp: J(r, c) = tile(r, c) + alpha_r d_c - gamma_r g_c  (Eq. 112 regrouped)
-// for one slab of rows (two rows per lane when ld is even) and m.d_seg columns; 32-bit offsets
-template <int S>
-__device__ __forceinline__ void dense_item(const DeviceMech &m, double *E, const double *colc, int pp, int it,
-                                           int lane, double *J0, int nq)
-{
-    const int ld = m.ld, pw = m.pw;
-    const int c0 = pp * pw, ncol = min(ld, c0 + pw) - c0;
-    const int RP = m.pair ? 2 : 1;
-    const int n_slab = m.n_slab;                              // slabs of 32 RP rows; no integer divisions here
-    const int sg = n_slab == 1 ? it : it / n_slab, slab = it - sg * n_slab;
-    const int cbeg = sg * m.d_seg, cend = min(ncol, cbeg + m.d_seg);
-    const int r = slab * 32 * RP + RP * lane;
-    if (r >= ld) return;
-    const char *tp = reinterpret_cast<const char *>(E) +
-                     (uint32_t)((m.eTile + (m.nbuf == 2 ? (pp & 1) : 0) * pw * ld + cbeg * ld + r) * S) * 8u;
-    const uint32_t t_inc = (uint32_t)(ld * S) * 8u, j_inc = (uint32_t)ld * 8u, j_state = (uint32_t)(ld * ld) * 8u;
-    const char *cc = reinterpret_cast<const char *>(colc + 2 * (c0 + cbeg));
-    char *Jp = reinterpret_cast<char *>(J0 + (long long)(c0 + cbeg) * ld + r);
-    // several panels share a tile buffer: zero it behind the read, so that cells without a list are zero
-    // for the next panel that uses the buffer (column 0 of panel 0 is rewritten by the kAuxT3 sums)
-    const bool zero = m.n_panel > 1;
-    double zeros[2 * S], zeros1[S];
+    if (kind == kSum1) {
+        if (LEVEL == 2) {
+            double acc[NP][S];
 #pragma unroll
-    for (int q = 0; q < 2 * S; ++q) zeros[q] = 0.0;
+            for (int p = 0; p < NP; ++p)
 #pragma unroll
-    for (int q = 0; q < S; ++q) zeros1[q] = 0.0;
-    if (RP == 2) {
-        double al[2 * S], ga[2 * S];
-        ldv<2 * S>(E + (m.eAlpha + r) * S, al);
-        ldv<2 * S>(E + (m.eGamma + r) * S, ga);
-#pragma unroll 2
-        for (int c = cbeg; c < cend; ++c, tp += t_inc, cc += 16, Jp += j_inc) {
-            const double2 dg = *reinterpret_cast<const double2 *>(cc);
-            double t[2 * S];
-            ldv<2 * S>(reinterpret_cast<const double *>(tp), t);
-            if (zero) stv<2 * S>(reinterpret_cast<double *>(const_cast<char *>(tp)), zeros);
+                for (int q = 0; q < S; ++q) acc[p][q] = 0.0;
+            auto step = [&](uint32_t w) {
+                const double cf = entry_coef(w);
+                const char *src = Eb + (w & kEntOffMask);
 #pragma unroll
-            for (int q = 0; q < S; ++q) {
-                const double v0 = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
-                const double v1 = fma(-ga[S + q], dg.y, fma(al[S + q], dg.x, t[S + q]));
-                if (q < nq) {
-                    if (r != 0) st_cs_v2(reinterpret_cast<double *>(Jp + q * j_state), v0, v1);
-                    else __stcs(reinterpret_cast<double *>(Jp + q * j_state) + 1, v1);
+                for (int p = 0; p < NP; ++p) {
+                    double a[S];
+                    ldv<S>(reinterpret_cast<const double *>(src + p * blk_bytes), a);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[p][q] = fma(cf, a[q], acc[p][q]);
+                }
+            };
+            uint4 w = ep[32];
+            for (int s = 0; s < steps; s += 4) {
+                const uint4 wn = ep[32 * (2 + (s >> 2))];          // one block ahead (the table is padded)
+                step(w.x);
+                if (s + 1 < steps) step(w.y);
+                if (s + 2 < steps) step(w.z);
+                if (s + 3 < steps) step(w.w);
+                w = wn;
+            }
+            for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+                for (int p = 0; p < NP; ++p)
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[p][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[p][q], o);
+            if (head) {
+                const double cst = __hiloint2double((int)r0.z, (int)r0.y);
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[p][q] *= cst;
+                    stv<S>(reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes) + r0.x * S, acc[p]);
                 }
             }
         }
-    } else {
-        double al[S], ga[S];
-        ldv<S>(E + (m.eAlpha + r) * S, al);
-        ldv<S>(E + (m.eGamma + r) * S, ga);
-#pragma unroll 2
-        for (int c = cbeg; c < cend; ++c, tp += t_inc, cc += 16, Jp += j_inc) {
-            const double2 dg = *reinterpret_cast<const double2 *>(cc);
-            double t[S];
-            ldv<S>(reinterpret_cast<const double *>(tp), t);
-            if (zero) stv<S>(reinterpret_cast<double *>(const_cast<char *>(tp)), zeros1);
+    } else if (kind == kProd) {
+        if (LEVEL == 2) {
+            double acc[NP][S];
 #pragma unroll
-            for (int q = 0; q < S; ++q) {
-                const double v = fma(-ga[q], dg.y, fma(al[q], dg.x, t[q]));
-                if (q < nq && r != 0) __stcs(reinterpret_cast<double *>(Jp + (size_t)q * j_state), v);
+            for (int p = 0; p < NP; ++p)
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[p][q] = 0.0;
+            auto step = [&](uint32_t w) {
+                const char *sa = Eb + (w & 0xFFFF) * (S * 8), *sb = Eb + (w >> 16) * (S * 8);
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    double a[S], b[S];
+                    ldv<S>(reinterpret_cast<const double *>(sa + p * blk_bytes), a);
+                    ldv<S>(reinterpret_cast<const double *>(sb + p * blk_bytes), b);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[p][q] = fma(a[q], b[q], acc[p][q]);
+                }
+            };
+            uint4 w = ep[32];
+            for (int s = 0; s < steps; s += 4) {
+                const uint4 wn = ep[32 * (2 + (s >> 2))];
+                step(w.x);
+                if (s + 1 < steps) step(w.y);
+                if (s + 2 < steps) step(w.z);
+                if (s + 3 < steps) step(w.w);
+                w = wn;
+            }
+            for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+                for (int p = 0; p < NP; ++p)
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[p][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[p][q], o);
+            if (head)
+#pragma unroll
+                for (int p = 0; p < NP; ++p)
+                    stv<S>(reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes) + r0.x * S, acc[p]);
+        }
+    } else {
+        // kSum3 / kAll3: three sums at once (one for the rates / source-term kernels)
+        constexpr int NA = LEVEL == 2 ? 3 : 1;
+        double acc[NP][NA][S];
+#pragma unroll
+        for (int p = 0; p < NP; ++p)
+#pragma unroll
+            for (int w = 0; w < NA; ++w)
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[p][w][q] = 0.0;
+        if (kind == kSum3) {
+            auto step = [&](uint32_t w_) {
+                const double cf = entry_coef(w_);
+                const char *src = Eb + (w_ & kEntOffMask);
+#pragma unroll
+                for (int p = 0; p < NP; ++p)
+#pragma unroll
+                    for (int w = 0; w < NA; ++w) {
+                        double a[S];
+                        ldv<S>(reinterpret_cast<const double *>(src + p * blk_bytes) + w * S, a);
+#pragma unroll
+                        for (int q = 0; q < S; ++q) acc[p][w][q] = fma(cf, a[q], acc[p][w][q]);
+                    }
+            };
+            uint4 w = ep[32];
+            for (int s = 0; s < steps; s += 4) {
+                const uint4 wn = ep[32 * (2 + (s >> 2))];
+                step(w.x);
+                if (s + 1 < steps) step(w.y);
+                if (s + 2 < steps) step(w.z);
+                if (s + 3 < steps) step(w.w);
+                w = wn;
+            }
+        } else {
+            for (int i = lane; i < nr; i += 32)
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    const double *Ep = reinterpret_cast<const double *>(Eb + p * blk_bytes);
+                    double h[S];
+                    ldv<S>(Ep + (m.eH + i) * S, h);
+#pragma unroll
+                    for (int w = 0; w < NA; ++w) {
+                        double a[S];
+                        ldv<S>(Ep + (m.eQ + 3 * i + w) * S, a);
+#pragma unroll
+                        for (int q = 0; q < S; ++q) acc[p][w][q] = fma(h[q], a[q], acc[p][w][q]);
+                    }
+                }
+        }
+        for (int o = 1; o < width; o <<= 1)
+#pragma unroll
+            for (int p = 0; p < NP; ++p)
+#pragma unroll
+                for (int w = 0; w < NA; ++w)
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[p][w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[p][w][q], o);
+        constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
+        if (kind == kAll3) {
+            if (lane == 0)
+#pragma unroll
+                for (int p = 0; p < NP; ++p) {
+                    double *Ep = reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes);
+                    stv<S>(Ep + m.eS1 * S, acc[p][0]);
+                    if (LEVEL == 2) { stv<S>(Ep + m.eA0 * S, acc[p][iA]); stv<S>(Ep + m.eS4 * S, acc[p][iT]); }
+                }
+        } else if (head) {
+            const uint32_t k = r0.x;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                double *Ep = reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes);
+                stv<S>(Ep + (m.eWdot + k) * S, acc[p][0]);
+                if (LEVEL == 2) {
+                    // alpha'_{k+1} of Eq. 112 regrouped and the T column (Eq. 111), both without W_k
+                    const double *scp = reinterpret_cast<const double *>(reinterpret_cast<const char *>(sc0) + p * blk_bytes);
+                    double al[S], tc[S];
+#pragma unroll
+                    for (int q = 0; q < S; ++q) {
+                        const double ir = scp[kIrho * S + q];
+                        al[q] = ir * acc[p][iA][q];
+                        tc[q] = ir * acc[p][iT][q];
+                    }
+                    stv<S>(Ep + (m.eAlpha + k + 1) * S, al);
+                    stv<S>(Ep + (m.eTc + k + 1) * S, tc);
+                }
             }
         }
     }
 }
 
-__device__ __forceinline__ int dense_items(const DeviceMech &m, int pp)
+// ---- FIX item `it`: the energy row (Eq. 113), stored by the lanes that finish it (phase B skips row 0).
+// Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 .. (column ns is zero)
+template <int S, int NP>
+__device__ __forceinline__ void fix_item(const DeviceMech &m, const double *E0, uint32_t blk_bytes, const double *Cp0,
+                                         const double *sc0, const double *colc, const double *wrow, int it, int lane,
+                                         double *J0, int nvalid)
 {
-    const int ld = m.ld, c0 = pp * m.pw, ncol = min(ld, c0 + m.pw) - c0;
-    return m.n_slab * ((ncol + m.d_seg - 1) / m.d_seg);
+    const int ns = m.ns, ld = m.ld;
+    const long long Jstate = (long long)ld * ld;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const double *E = reinterpret_cast<const double *>(reinterpret_cast<const char *>(E0) + p * blk_bytes);
+        const double *Cp = reinterpret_cast<const double *>(reinterpret_cast<const char *>(Cp0) + p * blk_bytes);
+        const double *sc = reinterpret_cast<const double *>(reinterpret_cast<const char *>(sc0) + p * blk_bytes);
+        double *Jp = J0 + (long long)p * S * Jstate;
+        const int nq = nvalid - p * S;
+        if (it == 0) {
+            double s3[S];       // sum_k c_pk W_k wdot_k
+#pragma unroll
+            for (int q = 0; q < S; ++q) s3[q] = 0.0;
+            for (int k = lane; k < ns; k += 32) {
+                const double wk = wrow[k + 1];
+                double cp[S], wd[S];
+                ldv<S>(Cp + k * S, cp);
+                ldv<S>(E + (m.eWdot + k) * S, wd);
+#pragma unroll
+                for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
+            if (lane < S) {
+                const int q = lane;
+                double s = s3[0];
+#pragma unroll
+                for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
+                const double icp = sc[kIcp * S + q];
+                const double z = -icp * sc[kIrho * S + q] *
+                                 (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
+                if (q < nq) Jp[q * Jstate] = z;
+            }
+            continue;
+        }
+        const int c = (it - 1) * 32 + lane + 1;
+        if (c < ns) {
+            const double uc = colc[4 * c], wj = colc[4 * c + 1], iwj = colc[4 * c + 2], iwl = m.inv_mw[ns - 1];
+            double icp[S], irho[S], s1[S], a0[S], gl[S], cpj[S], cpl[S], g0[S];
+            ldv<S>(sc + kIcp * S, icp);
+            ldv<S>(sc + kIrho * S, irho);
+            ldv<S>(E + m.eS1 * S, s1);
+            ldv<S>(E + m.eA0 * S, a0);
+            ldv<S>(E + (m.eG0 + ns - 1) * S, gl);
+            ldv<S>(Cp + (c - 1) * S, cpj);
+            ldv<S>(Cp + (ns - 1) * S, cpl);
+            ldv<S>(E + (m.eG0 + c - 1) * S, g0);
+#pragma unroll
+            for (int q = 0; q < S; ++q) {
+                const double a1 = irho[q] * s1[q] * icp[q] * icp[q];     // coefficient of c_pj - c_pNs
+                const double alpha0 = -(irho[q] * icp[q]) * a0[q];
+                const double gamma0 = -(iwl * icp[q]) * gl[q];
+                const double z = (alpha0 * uc + wj * (a1 * (cpj[q] - cpl[q]) - gamma0) - icp[q] * g0[q]) * iwj;
+                if (q < nq) Jp[q * Jstate + (long long)c * ld] = z;
+            }
+        } else if (c == ns) {
+#pragma unroll
+            for (int q = 0; q < S; ++q)
+                if (q < nq) Jp[q * Jstate + (long long)c * ld] = 0.0;
+        }
+    }
+}
+
+// ---- phase B: the items [it0, it1) of one warp (one item = one Jacobian column for one slab of rows).
+// J(r, c) = W_r / W_j (sum of the cell's entries + alpha'_r u_c - gamma'_r v_c)  (Eq. 112 regrouped), RP rows
+// per lane; alpha', gamma' and W_r stay in registers while the slab does not change, the entries of a
+// cell are decoded once for the NP blocks.  Headers are read two items ahead, entries one item ahead.
+template <int S, int NP, int RP>
+__device__ __forceinline__ void b_run(const DeviceMech &m, const double *E0, uint32_t blk_bytes, const double *colc,
+                                      const double *wrow, int it0, int it1, int lane, double *J0, int nvalid,
+                                      bool aligned16)
+{
+    if (it0 >= it1) return;
+    const int ld = m.ld;
+    const uint32_t j_state = (uint32_t)(ld * ld) * 8u;
+    const char *Eb = reinterpret_cast<const char *>(E0);
+    int slab = it0 / ld, c = it0 - slab * ld;
+    int cur = -1, r = 0;
+    bool rowok = false;
+    double al[NP][RP * S], ga[NP][RP * S], wr[RP];
+    uint2 h = m.bitem[it0], h1 = m.bitem[it0 + 1];
+    uint4 wA = m.b_ent[h.x + lane], wB = make_uint4(0u, 0u, 0u, 0u);
+    if (RP == 2) wB = m.b_ent[h.x + 32 + lane];
+    for (int it = it0; it < it1; ++it) {
+        const uint2 h2 = m.bitem[it + 2];
+        const uint4 wAn = m.b_ent[h1.x + lane];
+        uint4 wBn = make_uint4(0u, 0u, 0u, 0u);
+        if (RP == 2) wBn = m.b_ent[h1.x + 32 + lane];
+        if (slab != cur) {
+            cur = slab;
+            r = RP * (32 * slab + lane);
+            rowok = r < ld;
+            const int rr = rowok ? r : 0;
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                const double *Ep = reinterpret_cast<const double *>(Eb + p * blk_bytes);
+                ldv<RP * S>(Ep + (m.eAlpha + rr) * S, al[p]);
+                ldv<RP * S>(Ep + (m.eGamma + rr) * S, ga[p]);
+            }
+#pragma unroll
+            for (int hh = 0; hh < RP; ++hh) wr[hh] = wrow[rr + hh];
+        }
+        const double2 uv = *reinterpret_cast<const double2 *>(colc + 4 * c);
+        const double iw = colc[4 * c + 2];
+        const int nA = (int)(h.y & 0xFF), nB = (int)(h.y >> 8) & 0xFF;
+        double acc[NP][RP * S];
+#pragma unroll
+        for (int p = 0; p < NP; ++p)
+#pragma unroll
+            for (int e = 0; e < RP * S; ++e) acc[p][e] = fma(-ga[p][e], uv.y, al[p][e] * uv.x);
+        auto step = [&](uint32_t w, int hh) {
+            const double cf = entry_coef(w);
+            const char *src = Eb + (w & kEntOffMask);
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                double a[S];
+                ldv<S>(reinterpret_cast<const double *>(src + p * blk_bytes), a);
+#pragma unroll
+                for (int q = 0; q < S; ++q) acc[p][hh * S + q] = fma(cf, a[q], acc[p][hh * S + q]);
+            }
+        };
+        if (nA > 0) {
+            step(wA.x, 0);
+            if (nA > 1) {
+                step(wA.y, 0);
+                if (nA > 2) {
+                    step(wA.z, 0);
+                    if (nA > 3) step(wA.w, 0);
+                }
+            }
+        }
+        if (RP == 2 && nB > 0) {
+            step(wB.x, RP - 1);
+            if (nB > 1) {
+                step(wB.y, RP - 1);
+                if (nB > 2) {
+                    step(wB.z, RP - 1);
+                    if (nB > 3) step(wB.w, RP - 1);
+                }
+            }
+        }
+        if (rowok) {
+            char *Jp = reinterpret_cast<char *>(J0 + (long long)c * ld + r);
+            double f[RP];
+#pragma unroll
+            for (int hh = 0; hh < RP; ++hh) f[hh] = wr[hh] * iw;
+#pragma unroll
+            for (int p = 0; p < NP; ++p)
+#pragma unroll
+                for (int q = 0; q < S; ++q) {
+                    if (p * S + q >= nvalid) continue;
+                    double *dst = reinterpret_cast<double *>(Jp + (uint32_t)(p * S + q) * j_state);
+                    if (RP == 2) {
+                        const double v0 = acc[p][q] * f[0], v1 = acc[p][S + q] * f[RP - 1];
+                        if (r != 0 && aligned16) st_cs_v2(dst, v0, v1);
+                        else {
+                            if (r != 0) __stcs(dst, v0);
+                            __stcs(dst + 1, v1);
+                        }
+                    } else {
+                        if (r != 0) __stcs(dst, acc[p][q] * f[0]);
+                    }
+                }
+        }
+        h = h1; h1 = h2; wA = wAn; wB = wBn;
+        if (++c == ld) { c = 0; ++slab; }
+    }
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------
-// Shared memory: S interleaved state blocks of sp.total doubles (E with the tile behind it, three
-// mixture blocks), then the state-independent column and row constants.  The mixture block (X, Cp,
-// scalars) of the NEXT batch is filled as an item of this batch's reaction queue.
-template <int LEVEL, int NT, int S, int MB>
-__global__ void __launch_bounds__(NT, MB)
+// Shared memory: NP blocks of S interleaved states, sp.total doubles per state (E, two mixture parts),
+// then the state-independent column and row constants.
+template <int LEVEL, int S, int NP>
+__global__ void __launch_bounds__(kMaxThreads, 1)
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
                 const double *__restrict__ Pg, const double *__restrict__ Yg, long long ldy, const EvalOut out)
 {
     extern __shared__ __align__(16) double sm[];
     __shared__ int ctr[2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NW = NT / 32;
+    const int NT = blockDim.x, NW = NT >> 5;
     constexpr int SP = S >= 2 ? 2 : 1;
+    constexpr int NS = S * NP;                           // states per CTA iteration
     const int ns = m.ns, ld = m.ld, nr = m.nr;
-    double *E = sm + sp.E * S;
-    const double *colc = sm + (size_t)sp.total * S + sp.colc;
-    double *wrow = sm + (size_t)sp.total * S + sp.wrow;
+    const int blkd = sp.total * S;                       // doubles per block
+    const uint32_t blk_bytes = (uint32_t)blkd * 8u;
+    double *E0 = sm + sp.E * S;
+    const double *colc = sm + (size_t)NP * blkd + sp.colc;
+    double *wrow = sm + (size_t)NP * blkd + sp.wrow;
     {
-        double *cw = sm + (size_t)sp.total * S + sp.colc;
-        for (int i = tid; i < 2 * ld; i += NT) cw[i] = m.colc[i];
+        double *cw = sm + (size_t)NP * blkd + sp.colc;
+        for (int i = tid; i < 4 * ld; i += NT) cw[i] = m.colc[i];
         for (int i = tid; i < ld; i += NT) wrow[i] = m.wrow[i];
-        if (LEVEL == 2)      // the tile: cells without a list stay zero
-            for (int i = tid; i < m.nbuf * m.pw * ld * S; i += NT) E[(size_t)m.eTile * S + i] = 0.0;
+        // E starts as zeros: sums without a list, the zero slots and row 0 of alpha' / gamma' stay zero
+        for (int p = 0; p < NP; ++p)
+            for (int i = tid; i < m.n_e * S; i += NT) E0[(size_t)p * blkd + i] = 0.0;
     }
-    if (tid < S) {   // the empty-slot dummy species, the zero slots, row 0 of alpha / gamma
-        sm[(sp.P0 + sp.oX + ns) * S + tid] = 1.0;
-        sm[(sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
-        sm[(sp.P0 + 2 * sp.p0size + sp.oX + ns) * S + tid] = 1.0;
-        for (int z = 0; z < 18; ++z) E[(m.eZero + z) * S + tid] = 0.0;      // mech_pack.cu kZeroSlots
-        E[m.eAlpha * S + tid] = 0.0;
-        E[m.eGamma * S + tid] = 0.0;
-        if (nr == 0) { E[m.eS1 * S + tid] = 0.0; E[m.eA0 * S + tid] = 0.0; E[m.eS4 * S + tid] = 0.0; }
-    }
+    if (tid < S)       // the empty-slot dummy species of both mixture parts
+        for (int p = 0; p < NP; ++p) {
+            sm[(size_t)p * blkd + (sp.P0 + sp.oX + ns) * S + tid] = 1.0;
+            sm[(size_t)p * blkd + (sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
+        }
     if (tid == 0) ctr[0] = 0;
-    const long long nblk = (n + S - 1) / S;
-    // work items of P1: the general groups one state at a time (most expensive first), P0 of the next
-    // batch (one state each), then the plain groups SP states at a time
+    const long long nbatch = (n + NS - 1) / NS;
+    // work items of P1: the general groups one state at a time (most expensive first), then the plain
+    // groups SP states at a time; each for every block
     const int n_gen = m.n_rchunk - m.n_plain;
-    const int i_p0 = n_gen * S, i_plain = i_p0 + S;
-    const int n_p1 = i_plain + m.n_plain * (S / SP);
-    if (warp < S && (long long)blockIdx.x < nblk) {
-        double *P0 = sm + sp.P0 * S;
-        mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oScal * S, warp,
-                                      min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
-    }
-    __syncthreads();
-    if (LEVEL == 2) {
-        // ---- Jacobian.  Per batch b two kinds of phase alternate:
-        //   Q(b)  one dynamic queue: the reactions of batch b (P1), the mixture of batch b + 1 (P0) and,
-        //         of batch b - 1, the last DENSE step (and the FIX step if there is one panel).  The
-        //         long general-reaction items start first, the short DENSE items fill the tail.
-        //   G(b)  the gathers of batch b: A1 sums and the cells of panel 0 (further panels: cells of
-        //         panel p with the DENSE step of panel p - 1, a barrier after each).
-        // Three mixture blocks rotate: Q(b) reads block b (P1), writes block b + 1 and reads block b - 1 (FIX).
-        const int n_panel = m.n_panel, nfix = 1 + (ns + 31) / 32;
-        const long long Jstate = (long long)ld * ld;
-        long long blk = blockIdx.x, prev = -1;
-        int par = 0, ppar = 0;
-        const int nd_last = dense_items(m, n_panel - 1);         // loop invariants (integer divisions)
-        const int split_l = m.n_pd & 31, split_c = (m.split_general && split_l != 0 && (m.n_pd >> 5) < n_gen) ? (m.n_pd >> 5) : -1;
-        const int n_genq = n_gen + (split_c >= 0 ? 1 : 0);
-        const int n_fixq = n_panel == 1 ? nfix : 0;
-        const int n_plq = m.n_plain * (S / SP);
-        for (;;) {
-            const bool has_cur = blk < nblk, has_prev = prev >= 0;
-            if (!has_cur && !has_prev) break;
-            const long long state0 = blk * S;
-            double *P0 = sm + (sp.P0 + par * sp.p0size) * S;
-            double *P0n = sm + (sp.P0 + (par == 2 ? 0 : par + 1) * sp.p0size) * S;
-            const double *P0p = sm + (sp.P0 + ppar * sp.p0size) * S;
-            const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S;
-            double *Jprev = out.jac + prev * S * Jstate;
-            const int nq_prev = (int)min((long long)S, n - prev * S);
-#ifdef PYJAC_PROF
-            long long prof_t[12];
-#endif
-            PROF_MARK(0);
-            // ---- Q(blk)
-            const int n_g = has_cur ? n_genq * S : 0;
-            const int i_pl = n_g, i_m = i_pl + (has_cur ? n_plq : 0);
-            const int i_fix = i_m + ((has_cur && blk + gridDim.x < nblk) ? S : 0);
-            const int i_d = i_fix + (has_prev ? n_fixq : 0);
-            const int n_q = i_d + (has_prev ? nd_last : 0);
-            for (int it = grab(&ctr[0], lane); it < n_q; it = grab(&ctr[0], lane)) {
-                if (it < i_pl) {
-                    // general groups, one state at a time; the group that holds both pressure-dependent and
-                    // other reactions is two items (each runs only its own code paths)
-                    const int gi = it / S, q = it - gi * S;
-                    const int c = gi < n_gen ? gi : split_c;
-                    int sl = lane;              // lanes of the other part repeat this part's first reaction
-                    if (c == split_c) sl = gi < n_gen ? (lane < split_l ? lane : 0) : (lane >= split_l ? lane : split_l);
-                    reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + sl, nr - 1), q, out, state0, n);
-                } else if (it < i_m) {
-                    const int j = it - i_pl;
-                    const int c = n_gen + j / (S / SP), q0 = (j % (S / SP)) * SP;
-                    plain_reactions<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q0, out, state0, n);
-                } else if (it < i_fix) {
-                    const int q = it - i_m;
-                    mixture_and_species<LEVEL, S>(m, P0n + sp.oX * S, P0n + sp.oCp * S, P0n + sp.oScal * S, q,
-                                                  min((blk + gridDim.x) * S + q, n - 1), Tg, Pg, Yg, ldy, lane);
-                } else if (it < i_d) {
-                    fix_item<S>(m, E, P0p + sp.oCp * S, P0p + sp.oScal * S, colc, wrow, it - i_fix, lane, Jprev, nq_prev);
-                } else {
-                    dense_item<S>(m, E, colc, n_panel - 1, it - i_d, lane, Jprev, nq_prev);
-                }
-            }
-            PROF_MARK(1);
-            __syncthreads();
-            if (tid == 0) ctr[0] = 0;
-            PROF_MARK(2);
-            if (!has_cur) break;
-            // ---- G(blk)
-            GatherPipe gp;
-            gather_start<NW>(gp, m, 0, warp, lane);
-            gather_run<2, S, NW>(gp, m, E, sc, 0, m.panel_ptr[1], lane);      // A1 and the cells of panel 0
-            PROF_MARK(3);
-            __syncthreads();
-            PROF_MARK(4);
-            if (n_panel > 1) {
-                double *Jcur = out.jac + state0 * Jstate;
-                const int nq = (int)min((long long)S, n - state0);
-                for (int p = 1; p < n_panel; ++p) {
-                    if (p == 1)
-                        for (int it = NW - 1 - warp; it < nfix; it += NW)
-                            fix_item<S>(m, E, P0 + sp.oCp * S, sc, colc, wrow, it, lane, Jcur, nq);
-                    gather_run<2, S, NW>(gp, m, E, sc, m.panel_ptr[p], m.panel_ptr[p + 1], lane);
-                    const int nd = dense_items(m, p - 1);
-                    for (int it = warp; it < nd; it += NW) dense_item<S>(m, E, colc, p - 1, it, lane, Jcur, nq);
-                    __syncthreads();
-                }
-            }
-#ifdef PYJAC_PROF
-            if (blockIdx.x == 0 && (tid & 31) == 0 && blk == blockIdx.x + 3 * (long long)gridDim.x)
-                printf("PROF w%d Q %lld wait %lld | G %lld wait %lld\n", warp, prof_t[1] - prof_t[0],
-                       prof_t[2] - prof_t[1], prof_t[3] - prof_t[2], prof_t[4] - prof_t[3]);
-#endif
-            prev = blk; ppar = par;
-            blk += gridDim.x; par = par == 2 ? 0 : par + 1;
-        }
-        return;
-    }
+    const int split_l = m.n_pd & 31, split_c = (m.split_general && split_l != 0 && (m.n_pd >> 5) < n_gen) ? (m.n_pd >> 5) : -1;
+    const int n_genq = n_gen + (split_c >= 0 ? 1 : 0);
+    const int n_plq = m.n_plain * (S / SP);
+    const int i_plain = n_genq * S * NP, n_p1 = i_plain + n_plq * NP;
     int par = 0;
-    for (long long blk = blockIdx.x; blk < nblk; blk += gridDim.x, par ^= 1) {
-        const long long state0 = blk * S;
-        double *P0 = sm + (sp.P0 + par * sp.p0size) * S, *P0n = sm + (sp.P0 + (par ^ 1) * sp.p0size) * S;
-        const double *X = P0 + sp.oX * S, *Cp = P0 + sp.oCp * S, *sc = P0 + sp.oScal * S;
-#ifdef PYJAC_PROF
-        long long prof_t[12];
-#endif
-        PROF_MARK(0);
-        // ---- P1: reactions (+ the mixture of the next batch)
+    if ((long long)blockIdx.x < nbatch)
+        for (int it = warp; it < NS; it += NW) {
+            const int p = it / S, q = it - p * S;
+            double *P0 = sm + (size_t)p * blkd + sp.P0 * S;
+            mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oScal * S, q,
+                                          min((long long)blockIdx.x * NS + it, n - 1), Tg, Pg, Yg, ldy, lane);
+        }
+    __syncthreads();
+    for (long long b = blockIdx.x; b < nbatch; b += gridDim.x, par ^= 1) {
+        const long long state0 = b * NS;
+        double *P0 = sm + (sp.P0 + par * sp.p0size) * S;             // block 0's mixture part of this iteration
+        const double *sc0 = P0 + sp.oScal * S;
+        // ---- P1: reactions
         for (int it = grab(&ctr[0], lane); it < n_p1; it = grab(&ctr[0], lane)) {
-            if (it < i_p0) {
-                const int c = it / S, q = it - c * S;
-                reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q, out, state0, n);
-            } else if (it < i_plain) {
-                const int q = it - i_p0;
-                if (blk + gridDim.x < nblk)
-                    mixture_and_species<LEVEL, S>(m, P0n + sp.oX * S, P0n + sp.oCp * S, P0n + sp.oScal * S, q,
-                                                  min((blk + gridDim.x) * S + q, n - 1), Tg, Pg, Yg, ldy, lane);
+            if (it < i_plain) {
+                // general groups, one state at a time; the group that holds both pressure-dependent and
+                // other reactions is two items (each runs only its own code paths)
+                const int p = it % NP, j = it / NP;
+                const int gi = j / S, q = j - gi * S;
+                const int c = gi < n_gen ? gi : split_c;
+                int sl = lane;              // lanes of the other part repeat this part's first reaction
+                if (c == split_c) sl = gi < n_gen ? (lane < split_l ? lane : 0) : (lane >= split_l ? lane : split_l);
+                const double *Pp = P0 + (size_t)p * blkd;
+                reaction<LEVEL, S>(m, sp, E0 + (size_t)p * blkd, Pp + sp.oX * S, Pp + sp.oScal * S,
+                                   min(c * 32 + sl, nr - 1), q, out, state0 + p * S, n);
             } else {
-                const int j = it - i_plain;
+                const int i2 = it - i_plain;
+                const int p = i2 % NP, j = i2 / NP;
                 const int c = n_gen + j / (S / SP), q0 = (j % (S / SP)) * SP;
-                plain_reactions<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q0, out, state0, n);
+                const double *Pp = P0 + (size_t)p * blkd;
+                plain_reactions<LEVEL, S>(m, sp, E0 + (size_t)p * blkd, Pp + sp.oX * S, Pp + sp.oScal * S,
+                                          min(c * 32 + lane, nr - 1), q0, out, state0 + p * S, n);
             }
         }
-        PROF_MARK(1);
         __syncthreads();
         if (tid == 0) ctr[0] = 0;
-        PROF_MARK(2);
-        // ---- A1: sums over the reactions per species / per column
-        gather_phase<LEVEL, S, NW>(m, E, sc, 0, m.n_a1_01, warp, lane);
-        PROF_MARK(3);
+        // ---- A: sums over the reactions per species / per column, pieces of the long cell lists
+        {
+            const int rows = LEVEL == 2 ? m.n_arow : m.n_arow01;
+            const uint2 *hp = m.achunk + warp;
+            uint2 h = hp[0];
+            for (int row = 0; row < rows; ++row) {
+                const uint2 hn = hp[(size_t)(row + 1 < rows ? row + 1 : row) * NW];
+                a_chunk<LEVEL, S, NP>(m, E0, blk_bytes, sc0, h, lane);
+                h = hn;
+            }
+        }
         __syncthreads();
-        PROF_MARK(4);
+        const int nvalid = (int)min((long long)NS, n - state0);
+        if (LEVEL == 2) {
+            // ---- B: the Jacobian column by column, the energy row
+            double *J0 = out.jac + state0 * ((long long)ld * ld);
+            const bool aligned16 = (reinterpret_cast<uintptr_t>(out.jac) & 15) == 0;
+            const int it0 = m.bsplit[warp], it1 = m.bsplit[warp + 1];
+            if (m.rp == 2) b_run<S, NP, 2>(m, E0, blk_bytes, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
+            else b_run<S, NP, 1>(m, E0, blk_bytes, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
+            const int nfix = 1 + (ns + 31) / 32;
+            for (int it = NW - 1 - warp; it < nfix; it += NW)
+                fix_item<S, NP>(m, E0, blk_bytes, P0 + sp.oCp * S, sc0, colc, wrow, it, lane, J0, nvalid);
+        }
         // ---- outputs of the rates / source-term kernels (Eqs. 7-8, 14)
         if (LEVEL == 0 && out.wdot) {
-            for (int k = tid; k < ns; k += NT)
+            for (int i = tid; i < ns * NP; i += NT) {
+                const int p = i / ns, k = i - p * ns;
 #pragma unroll
                 for (int q = 0; q < S; ++q)
-                    if (state0 + q < n) out.wdot[(state0 + q) * ns + k] = E[(m.eWdot + k) * S + q];
+                    if (p * S + q < nvalid) out.wdot[(state0 + p * S + q) * ns + k] = E0[(size_t)p * blkd + (m.eWdot + k) * S + q];
+            }
         }
         if (LEVEL == 1) {
-            for (int r = tid; r < ld; r += NT)
+            for (int i = tid; i < ld * NP; i += NT) {
+                const int p = i / ld, r = i - p * ld;
+                const double *E = E0 + (size_t)p * blkd, *sc = sc0 + (size_t)p * blkd;
 #pragma unroll
                 for (int q = 0; q < S; ++q) {
-                    if (state0 + q >= n) continue;
+                    if (p * S + q >= nvalid) continue;
                     const double irho = sc[kIrho * S + q];
                     const double v = r == 0 ? -E[m.eS1 * S + q] * irho / sc[kCpMix * S + q]
                                             : wrow[r] * E[(m.eWdot + r - 1) * S + q] * irho;
-                    out.dydt[(state0 + q) * ld + r] = v;
+                    out.dydt[(state0 + p * S + q) * ld + r] = v;
                 }
+            }
         }
-        __syncthreads();      // the outputs above read E and the scalars
+        // ---- P0 of the next iteration into the other mixture part
+        if (b + gridDim.x < nbatch)
+            for (int it = warp; it < NS; it += NW) {
+                const int p = it / S, q = it - p * S;
+                double *Pn = sm + (size_t)p * blkd + (sp.P0 + (par ^ 1) * sp.p0size) * S;
+                mixture_and_species<LEVEL, S>(m, Pn + sp.oX * S, Pn + sp.oCp * S, Pn + sp.oScal * S, q,
+                                              min((b + gridDim.x) * NS + it, n - 1), Tg, Pg, Yg, ldy, lane);
+            }
+        __syncthreads();
     }
-}
-
-template <int LEVEL, int NT, int S, int MB>
-cudaError_t launch_t(const DeviceMech &m, const SmemPlan &sp, int grid, size_t smem, long long n,
-                     const double *T, const double *P, const double *Y, long long ldy, const EvalOut &out,
-                     cudaStream_t stream)
-{
-    eval_kernel<LEVEL, NT, S, MB><<<grid, NT, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
-    return cudaGetLastError();
 }
 
 }  // namespace
 
-// This file is compiled once per CTA size: -DPYJAC_NT=<threads> -DPYJAC_MB=<CTAs per SM the register
-// budget is set for> (build.py); dispatch.cu switches over the sizes.
-#ifndef PYJAC_NT
-#error "compile with -DPYJAC_NT=<threads per CTA> -DPYJAC_MB=<CTAs per SM>"
+// This file is compiled once per (S, NP): -DPYJAC_S=<states per block> -DPYJAC_NP=<blocks per CTA
+// iteration> (build.py); dispatch.cu switches over them.
+#if !defined(PYJAC_S) || !defined(PYJAC_NP)
+#error "compile with -DPYJAC_S=<1|2> -DPYJAC_NP=<1..4>"
 #endif
-#define PYJAC_CAT2(a, b) a##b
-#define PYJAC_CAT(a, b) PYJAC_CAT2(a, b)
-#define PYJAC_FOR_S(X) X(1) X(2) X(4)
+#define PYJAC_CAT3(a, b, c, d) a##b##c##d
+#define PYJAC_NAME(a, s, np) PYJAC_CAT3(a, s, _, np)
 
-const void *PYJAC_CAT(eval_kernel_ptr_, PYJAC_NT)(int level, int S)
+const void *PYJAC_NAME(eval_kernel_ptr_, PYJAC_S, PYJAC_NP)(int level)
 {
-#define PYJAC_PTR(SV)                                                                          \
-    if (S == SV)                                                                               \
-        return level == 0 ? (const void *)eval_kernel<0, PYJAC_NT, SV, PYJAC_MB>               \
-             : level == 1 ? (const void *)eval_kernel<1, PYJAC_NT, SV, PYJAC_MB>               \
-                          : (const void *)eval_kernel<2, PYJAC_NT, SV, PYJAC_MB>;
-    PYJAC_FOR_S(PYJAC_PTR)
-#undef PYJAC_PTR
-    return nullptr;
+    return level == 0 ? (const void *)eval_kernel<0, PYJAC_S, PYJAC_NP>
+         : level == 1 ? (const void *)eval_kernel<1, PYJAC_S, PYJAC_NP>
+                      : (const void *)eval_kernel<2, PYJAC_S, PYJAC_NP>;
 }
 
-cudaError_t PYJAC_CAT(launch_eval_, PYJAC_NT)(int level, int S, const DeviceMech &m, const SmemPlan &sp, int grid,
-                                              size_t smem, long long n, const double *T, const double *P,
-                                              const double *Y, long long ldy, const EvalOut &out, cudaStream_t stream)
+cudaError_t PYJAC_NAME(launch_eval_, PYJAC_S, PYJAC_NP)(int level, int threads, const DeviceMech &m, const SmemPlan &sp,
+                                                         int grid, size_t smem, long long n, const double *T,
+                                                         const double *P, const double *Y, long long ldy,
+                                                         const EvalOut &out, cudaStream_t stream)
 {
-#define PYJAC_CASE(SV)                                                                                                  \
-    if (S == SV) {                                                                                                      \
-        if (level == 0) return launch_t<0, PYJAC_NT, SV, PYJAC_MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);    \
-        if (level == 1) return launch_t<1, PYJAC_NT, SV, PYJAC_MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);    \
-        return launch_t<2, PYJAC_NT, SV, PYJAC_MB>(m, sp, grid, smem, n, T, P, Y, ldy, out, stream);                    \
-    }
-    PYJAC_FOR_S(PYJAC_CASE)
-#undef PYJAC_CASE
-    return cudaErrorInvalidValue;
+    if (level == 0) eval_kernel<0, PYJAC_S, PYJAC_NP><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+    else if (level == 1) eval_kernel<1, PYJAC_S, PYJAC_NP><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+    else eval_kernel<2, PYJAC_S, PYJAC_NP><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+    return cudaGetLastError();
 }
 
 }  // namespace pyjac

@@ -36,9 +36,9 @@ struct ColEntry {
 
 // one gathered sum (A1 phase or one Jacobian cell)
 struct Task {
-    std::vector<std::pair<uint32_t, int>> ent;   // kAuxS1 / kAuxT3: (E index, coefficient); kAuxH2: (a | b << 16, 0)
-    uint32_t kind = kAuxS1;
-    uint32_t out = 0;       // E index of the result (kAuxT3: species k)
+    std::vector<std::pair<uint32_t, int>> ent;   // kSum1 / kSum3: (E index, coefficient); kProd: (a | b << 16, 0)
+    uint32_t kind = kSum1;
+    uint32_t out = 0;       // E index of the result (kSum3: species k)
     double cst = 1.0;
     int rshift = 0;         // 2^rshift lanes share the sum
     bool lvl01 = false;     // needed by the rates / dydt kernels too
@@ -166,10 +166,12 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     const double iw_last = 1.0 / d->mol_wt[ns - 1];
     o.wrow.assign((size_t)ld, 1.0);
     for (int k = 0; k < ns; ++k) o.wrow[k + 1] = d->mol_wt[k];
-    o.colc.assign((size_t)2 * ld, 0.0);       // {d_j, 1 (gamma_r applies)}; columns 0 and ns: zeros
+    o.colc.assign((size_t)4 * ld, 0.0);       // {u_c, v_c, 1/W_j, 0} (device_mech.h); column ns: zeros
+    o.colc[2] = 1.0;
     for (int k = 0; k + 1 < ns; ++k) {
-        o.colc[2 * (k + 1)] = 1.0 / d->mol_wt[k] - iw_last;
-        o.colc[2 * (k + 1) + 1] = 1.0;
+        o.colc[4 * (k + 1) + 0] = d->mol_wt[k] * (1.0 / d->mol_wt[k] - iw_last);
+        o.colc[4 * (k + 1) + 1] = d->mol_wt[k];
+        o.colc[4 * (k + 1) + 2] = 1.0 / d->mol_wt[k];
     }
 
     // ---- per reaction: molecules per side, breakpoints of its species' NASA ranges
@@ -279,13 +281,11 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     auto take = [&](int n) { int r = next_slot; next_slot += n; return r; };
     const int eQ = take(3 * nr), eH = take(nr);
     auto take2 = [&](int n) { next_slot = (next_slot + 1) & ~1; return take(n); };      // even: read in pairs of rows
-    const int eAlpha = take2(ld), eGamma = take2(ld), eWdot = take(ns), eG0 = take(ns), eZ = take(ld);
-    const int eS1 = take(1), eA0 = take(1), eS4 = take(1), eZero = take(kZeroSlots), eDump = take(1);   // zero slots: one per bank group, plus two (kAuxT3 pads read q, a, Theta)
-    o.eQ = eQ; o.eH = eH; o.eAlpha = eAlpha; o.eGamma = eGamma; o.eWdot = eWdot;
-    o.eG0 = eG0; o.eZ = eZ; o.eS1 = eS1; o.eA0 = eA0; o.eS4 = eS4; o.eZero = eZero; o.eDump = eDump;
-    next_slot = (next_slot + 1) & ~1;
-    o.n_e = next_slot;
-    if (next_slot > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-state table entries"};
+    const int eAlpha = take2(ld), eGamma = take2(ld), eTc = take2(ld), eWdot = take(ns), eG0 = take(ns);
+    const int eS1 = take(1), eA0 = take(1), eS4 = take(1), eZero = take(kZeroSlots), eDump = take(1);   // zero slots: one per bank group, plus two (kSum3 pads read q, a, Theta)
+    o.eQ = eQ; o.eH = eH; o.eAlpha = eAlpha; o.eGamma = eGamma; o.eTc = eTc; o.eWdot = eWdot;
+    o.eG0 = eG0; o.eS1 = eS1; o.eA0 = eA0; o.eS4 = eS4; o.eZero = eZero; o.eDump = eDump;
+    const int eHs = next_slot;          // the partial sums of the long cell lists follow (sized below)
 
     // ---- per-reaction tables in sorted order
     o.lnA.assign(nr, 0.0); o.beta.assign(nr, 0.0); o.Ta.assign(nr, 0.0);
@@ -479,129 +479,210 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         }
     }
 
-    // ---- launch shape: S states per CTA iteration, CTAs per SM, and the width of the column panels
-    // of the tile.  Everything lives in shared memory: S x (E + tile + two mixture blocks).
-    const long long sm_bytes = 228 * 1024;                       // shared memory of one sm_100 SM
-    auto bytes_for = [&](int S, int pw, int nbuf) {
-        const SmemPlan pl = make_smem_plan(ns, o.n_e + nbuf * pw * ld);
-        return ((long long)S * pl.total + pl.shared_total) * 8;
-    };
-    // each resident CTA also takes a 1 KB system reserve and the kernel's few static bytes
-    auto limit_for = [&](int ctas) { return std::min<long long>(sm_bytes / ctas - 1024 - 128, hints.smem_bytes); };
-    // widest panel (columns) that fits; 0 if not even one column does
-    auto widest = [&](int S, int ctas) {
-        const long long lim = limit_for(ctas);
-        if (bytes_for(S, ld, 1) <= lim) return ld;
-        int pw = 0;
-        for (int w = 1; w < ld; ++w)
-            if (bytes_for(S, w, 2) <= lim) pw = w;
-        return pw;
-    };
-    {
-        int S = 0, ctas = 0, pw = 0;
-        const int cand[][2] = {{2, 4}, {2, 2}, {2, 1}, {1, 2}, {1, 1}};
-        for (auto &c : cand) {
-            if (hints.S > 0 && c[0] != hints.S) continue;
-            if (hints.ctas > 0 && c[1] != hints.ctas) continue;
-            if (c[1] == 4 && ns > 24 && hints.ctas != 4) continue;     // four small CTAs only for tiny models
-            const int w = widest(c[0], c[1]);
-            const int want = hints.pw > 0 ? 1 : (c[1] > 1 || c[0] > 1) ? std::min(ld, 12) : 1;
-            if (w >= want) { S = c[0]; ctas = c[1]; pw = w; break; }
-        }
-        if (S == 0 && hints.S > 0) {            // a hinted S outside the candidate list (e.g. 4)
-            for (int c = (hints.ctas > 0 ? hints.ctas : 2); c >= 1 && S == 0; --c) {
-                const int w = widest(hints.S, c);
-                if (w >= 1) { S = hints.S; ctas = c; pw = w; }
-                if (hints.ctas > 0) break;
-            }
-        }
-        if (S == 0) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
-        if (hints.pw > 0 && hints.pw < pw) pw = hints.pw;
-        const int n_panel = (ld + pw - 1) / pw;
-        pw = (ld + n_panel - 1) / n_panel;
-        o.S = S; o.ctas_target = ctas; o.pw = pw; o.n_panel = n_panel; o.nbuf = n_panel > 1 ? 2 : 1;
-        o.threads = hints.threads > 0 ? hints.threads : ctas >= 4 ? 128 : ctas == 3 ? 256 : ctas == 2 ? 384 : 768;
-        o.eTile = o.n_e;
-        o.pair = (ld % 2 == 0) ? 1 : 0;
-        if ((long long)(o.n_e + o.nbuf * o.pw * ld) * o.S * 8 > (long long)kEntOffMask)
-            throw Fail{PYJAC_ELIMIT, "per-CTA tables exceed the 512 KB offset range of a gather entry"};
-    }
-    {   // DENSE work items (one slab of rows x d_seg columns).  Measured: with one panel the items sit in the
-        // dynamic queue and fewer, longer items win (less set-up per column); with several panels they are
-        // dealt round-robin next to the cell gathers and about 3 columns win.
-        const int nw = o.threads / 32, n_slab = (ld + (o.pair ? 63 : 31)) / (o.pair ? 64 : 32);
-        int seg = o.n_panel == 1 ? (3 * n_slab * o.pw + 2 * nw - 1) / (2 * nw) : 3;
-        seg = seg < 2 ? 2 : seg > 32 ? 32 : seg;
-        if (hints.seg > 0) seg = hints.seg;
-        o.d_seg = seg;
-    }
-    const int S = o.S, pw = o.pw, n_panel = o.n_panel, nbuf = o.nbuf, eTile = o.eTile;
-
-    // ---- A1 sums
-    std::vector<Task> a1;
+    // ---- which per-reaction products feed which sums: Algorithm 2's scatter written
+    // as fixed-order gathers
+    std::vector<Task> sums;
     // (a) per species k: sums of nu_ki {q_i, a_i, Theta_i} (Eq. 14; the d_j coefficient of Eqs. 112, 119,
     //     123, 127 regrouped; the T column, Eq. 111).  The rates / dydt kernels need wdot too.
-    const size_t tT3 = a1.size();
-    for (int k = 0; k < ns; ++k) { Task t; t.kind = kAuxT3; t.out = (uint32_t)k; t.lvl01 = true; a1.push_back(t); }
-    // (b) gamma_r = (W_k / W_Ns) sum_i nu_ki s'_iNs
-    const size_t tGamma = a1.size();
+    const size_t tS3 = sums.size();
+    for (int k = 0; k < ns; ++k) { Task t; t.kind = kSum3; t.out = (uint32_t)k; t.lvl01 = true; sums.push_back(t); }
+    // (b) gamma'_r = (1 / W_Ns) sum_i nu_ki s'_iNs
+    const size_t tGamma = sums.size();
     for (int k = 0; k < ns; ++k) {
-        Task t; t.kind = kAuxS1; t.out = (uint32_t)(eGamma + k + 1); t.cst = d->mol_wt[k] * iw_last;
-        a1.push_back(t);
+        Task t; t.kind = kSum1; t.out = (uint32_t)(eGamma + k + 1); t.cst = iw_last;
+        sums.push_back(t);
     }
     // (c) energy row (Eq. 113): G0_j = sum_i H_i s'_ij per column species
-    const size_t tG0 = a1.size();
-    for (int j = 0; j < ns; ++j) { Task t; t.kind = kAuxH2; t.out = (uint32_t)(eG0 + j); a1.push_back(t); }
+    const size_t tG0 = sums.size();
+    for (int j = 0; j < ns; ++j) { Task t; t.kind = kProd; t.out = (uint32_t)(eG0 + j); sums.push_back(t); }
 
-    // ---- lists of the Jacobian cells, flat column-major index f = r + c * ld
+    // ---- lists of the Jacobian cells, flat column-major index f = r + c * ld.  Column 0 (the T column,
+    // Eq. 111) reads the finished sum of its row; row 0 (the energy row) and column ns have no list.
     std::vector<std::vector<std::pair<uint32_t, int>>> cell((size_t)ld * ld);
     for (int s = 0; s < nr; ++s) {
         const uint32_t hs = (uint32_t)(eH + s);
-        for (auto &ce : cols[s]) a1[tG0 + ce.spec].ent.push_back({ce.vi | hs << 16, 0});
+        for (auto &ce : cols[s]) sums[tG0 + ce.spec].ent.push_back({ce.vi | hs << 16, 0});
         for (auto &pr : net[s]) {
             if (pr.second == 0) continue;
             const int k = pr.first;
-            a1[tT3 + k].ent.push_back({(uint32_t)(eQ + 3 * s), pr.second});
+            sums[tS3 + k].ent.push_back({(uint32_t)(eQ + 3 * s), pr.second});
             for (auto &ce : cols[s]) {
-                if (ce.spec == ns - 1) a1[tGamma + k].ent.push_back({ce.vi, pr.second});
+                if (ce.spec == ns - 1) sums[tGamma + k].ent.push_back({ce.vi, pr.second});
                 else cell[(size_t)(k + 1) + (size_t)(ce.spec + 1) * ld].push_back({ce.vi, pr.second});
             }
         }
     }
+    for (int r = 1; r < ld; ++r) cell[(size_t)r].push_back({(uint32_t)(eTc + r), 1});
 
-    // ---- encoding of the entries (device_mech.h): coefficients outside {1,2,3,4,6,8} are split
-    auto encode = [&](const Task &t, std::vector<uint32_t> &w) {
+    // ---- entries after splitting coefficients beyond +-8 (device_mech.h); E indices, not yet offsets
+    auto split = [&](const std::vector<std::pair<uint32_t, int>> &ent, std::vector<std::pair<uint32_t, int>> &w) {
         w.clear();
-        for (auto &e : t.ent) {
-            if (t.kind == kAuxH2) { w.push_back(e.first); continue; }
+        for (auto &e : ent) {
             int c = e.second;
             const int sg = c < 0 ? -1 : 1;
             c = c < 0 ? -c : c;
-            static const int parts[] = {8, 6, 4, 3, 2, 1};
-            while (c > 0)
-                for (int pz : parts)
-                    if (pz <= c) { w.push_back(coef_hi13(sg * pz) | (uint32_t)(e.first * S * 8)); c -= pz; break; }
+            while (c > 0) { const int pz = std::min(c, 8); w.push_back({e.first, sg * pz}); c -= pz; }
         }
     };
-    const uint32_t pad1 = (uint32_t)(eZero * S * 8);                 // coefficient 0 times the zero slot
-    const uint32_t pad2 = (uint32_t)eZero | (uint32_t)eZero << 16;
 
-    // ---- chunks: sums of one kind, shared by equally many lanes and of similar length, fill the 32
-    // lanes of a chunk; the warps take the chunks of a phase round-robin, most expensive first.
-    struct Chunk { std::vector<Task *> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; int tpl; };
-    std::vector<uint32_t> words;
-    const int NW = o.threads / 32;
-    std::vector<double> a1_load;
-    auto emit_phase = [&](std::vector<Task> &tasks, bool with_r3, long long &step_count, std::vector<double> &load) {
-        for (auto &t : tasks) {
-            encode(t, words);
-            t.n_words = words.size();
-            t.rshift = pick_rshift(t.n_words, hints.cap > 0 ? (size_t)hints.cap : o.ctas_target >= 2 ? 24 : 10);
+    // ---- long cell lists are summed piecewise in phase A (balanced over the lanes: lists sorted by
+    // length); phase B then reads at most `cell_cap` entries per cell, all lanes of a warp alike
+    const int cell_cap = hints.cell_cap >= 1 && hints.cell_cap <= 4 ? hints.cell_cap : 3;
+    constexpr int kPiece = 8;
+    std::vector<std::vector<std::pair<uint32_t, int>>> cell_w((size_t)ld * ld);
+    {
+        std::vector<std::pair<uint32_t, int>> w;
+        int n_hs = 0;
+        for (size_t f = 0; f < cell.size(); ++f) {
+            if (cell[f].empty()) continue;
+            split(cell[f], w);
+            o.n_cells += 1;
+            o.n_cell_entries += (long long)w.size();
+            if ((int)w.size() <= cell_cap) { cell_w[f] = w; continue; }
+            const int np = std::min(cell_cap, ((int)w.size() + kPiece - 1) / kPiece);
+            o.n_heavy_cells += 1;
+            size_t at = 0;
+            for (int p = 0; p < np; ++p) {
+                const size_t len = (w.size() - at + (np - p) - 1) / (np - p);
+                Task t; t.kind = kSum1; t.out = (uint32_t)(eHs + n_hs); t.cst = 1.0;
+                t.ent.assign(w.begin() + at, w.begin() + at + len);
+                at += len;
+                sums.push_back(t);
+                cell_w[f].push_back({(uint32_t)(eHs + n_hs), 1});
+                ++n_hs;
+            }
         }
+        o.n_heavy_pieces = n_hs;
+        o.eHs = eHs;
+        o.n_e = (eHs + n_hs + 1) & ~1;
+        if (o.n_e > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-state table entries"};
+    }
+
+    // ---- launch shape: NP blocks of S states per CTA iteration, threads per CTA, CTAs per SM.
+    // Everything lives in shared memory: NP x S x (E + two mixture parts) + the column / row constants.
+    {
+        const long long sm_bytes = 228 * 1024;                       // shared memory of one sm_100 SM
+        const SmemPlan pl = make_smem_plan(ns, o.n_e);
+        auto bytes_for = [&](int S, int NP) { return ((long long)S * NP * pl.total + pl.shared_total) * 8; };
+        // each resident CTA also takes a 1 KB system reserve and the kernel's few static bytes
+        auto limit_for = [&](int ctas) { return std::min<long long>(sm_bytes / ctas - 1024 - 128, hints.smem_bytes); };
+        int S = hints.S > 0 ? hints.S : (bytes_for(2, 1) <= limit_for(1) ? 2 : 1);
+        if (S != 1 && S != 2) throw Fail{PYJAC_EINVAL, "states per block must be 1 or 2"};
+        if (bytes_for(S, 1) > limit_for(1)) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
+        int ctas = hints.ctas > 0 ? hints.ctas : 0, NP = hints.NP > 0 ? hints.NP : 0;
+        if (NP > kMaxNP) throw Fail{PYJAC_EINVAL, "more blocks per CTA than the kernels are compiled for"};
+        if (ctas == 0 && NP == 0) {
+            // default: as many states in flight per SM as fit, in the fewest CTAs (tables are read once per CTA
+            // iteration and amortised over its NP blocks)
+            const long long per_block = (long long)S * pl.total * 8;
+            const int fit = (int)std::max<long long>(1, (limit_for(1) - pl.shared_total * 8) / per_block);
+            if (fit <= kMaxNP) { NP = fit; ctas = 1; }
+            else {
+                NP = kMaxNP;
+                ctas = 1;
+                while (ctas < 4 && bytes_for(S, NP) <= limit_for(ctas + 1)) ++ctas;
+            }
+        } else if (NP == 0) {
+            NP = 1;
+            while (NP < kMaxNP && bytes_for(S, NP + 1) <= limit_for(ctas)) ++NP;
+        } else if (ctas == 0) {
+            ctas = 1;
+            while (ctas < 4 && bytes_for(S, NP) <= limit_for(ctas + 1)) ++ctas;
+        }
+        if (bytes_for(S, NP) > limit_for(ctas)) throw Fail{PYJAC_ELIMIT, "the requested launch shape exceeds shared memory"};
+        int threads = hints.threads > 0 ? hints.threads : (kMaxThreads / ctas) & ~31;
+        if (threads < 64) threads = 64;
+        if (threads > kMaxThreads || threads % 32) throw Fail{PYJAC_EINVAL, "threads per CTA must be a multiple of 32 up to 512"};
+        o.S = S; o.NP = NP; o.threads = threads; o.ctas_target = ctas;
+        if ((long long)o.n_e * S * 8 > (long long)kEntOffMask + 1)
+            throw Fail{PYJAC_ELIMIT, "per-block tables exceed the 256 KB offset range of a gather entry"};
+    }
+    const int S = o.S, NW = o.threads / 32;
+    o.rp = (hints.rp == 1 || hints.rp == 2) ? hints.rp : (ld % 2 == 0 ? 2 : 1);
+    if (ld % 2 != 0) o.rp = 1;
+    const int rp = o.rp;
+    o.n_slab = (ld + 32 * rp - 1) / (32 * rp);
+
+    // ---- encoding (device_mech.h) and bank-aware placement.  Which step of a lane reads which of its
+    // entries, and which zero slot a padding entry reads, is free: both are chosen greedily so that the
+    // lanes of one shared-memory wavefront hit different bank groups at every step.
+    auto enc = [&](const std::pair<uint32_t, int> &e) { return coef_hi14(e.second) | (uint32_t)(e.first * S * 8); };
+    const int gsz = std::min(8 * S, 16), LP = 128 / gsz, nq = 32 / LP;     // bytes per lane access, lanes per wavefront
+    // lists[slot] sits on lanes [slot * width, (slot + 1) * width); returns grid[lane * steps + step]
+    auto place = [&](const std::vector<std::vector<uint32_t>> &lists, int width, int steps, uint32_t kind) {
+        const int nstream = kind == kProd ? 2 : 1;
+        std::vector<uint32_t> grid((size_t)32 * std::max(steps, 1), 0u);
+        if (steps == 0) return grid;
+        std::vector<char> filled((size_t)32 * steps, 0);
+        std::vector<std::vector<uint32_t>> occ((size_t)steps * nq * nstream);
+        auto occ_of = [&](int step, int lane, int st) -> std::vector<uint32_t> & {
+            return occ[((size_t)step * nq + lane / LP) * nstream + st];
+        };
+        auto granules = [&](uint32_t w, uint32_t g[2]) {
+            if (kind == kProd) { g[0] = (w & 0xFFFF) * S * 8 / gsz; g[1] = (w >> 16) * S * 8 / gsz; }
+            else { g[0] = (w & kEntOffMask) / gsz; g[1] = 0; }
+        };
+        auto clash = [&](const std::vector<uint32_t> &v, uint32_t g) {
+            bool same_bank = false;
+            for (uint32_t x : v) {
+                if (x == g) return 0;                  // same address: broadcast
+                same_bank = same_bank || (x % LP == g % LP);
+            }
+            return same_bank ? 1 : 0;
+        };
+        for (size_t sl = 0; sl < lists.size(); ++sl) {
+            const int lane0 = (int)sl * width;
+            for (uint32_t w : lists[sl]) {
+                uint32_t g[2];
+                granules(w, g);
+                int best = -1, bc = 1 << 30;
+                for (int st = 0; st < steps && bc > 0; ++st)
+                    for (int j = 0; j < width; ++j) {
+                        if (filled[(size_t)(lane0 + j) * steps + st]) continue;
+                        int cc = 0;
+                        for (int k = 0; k < nstream; ++k) cc += clash(occ_of(st, lane0 + j, k), g[k]);
+                        if (cc < bc) { bc = cc; best = (lane0 + j) * steps + st; }
+                        if (bc == 0) break;
+                    }
+                REQUIRE(best >= 0, "internal: a gather list does not fit its lanes");
+                filled[best] = 1;
+                grid[best] = w;
+                for (int k = 0; k < nstream; ++k) occ_of(best % steps, best / steps, k).push_back(g[k]);
+            }
+        }
+        // pads: coefficient 0 (kProd: zero times zero) on a zero slot whose bank group is free
+        for (int st = 0; st < steps; ++st)
+            for (int lane = 0; lane < 32; ++lane) {
+                if (filled[(size_t)lane * steps + st]) continue;
+                int z = 0;
+                for (int t = 0; t < LP; ++t) {
+                    const uint32_t g = (uint32_t)(eZero + t) * S * 8 / gsz;
+                    bool ok = true;
+                    for (int k = 0; k < nstream; ++k) ok = ok && clash(occ_of(st, lane, k), g) == 0;
+                    if (ok) { z = t; break; }
+                }
+                const uint32_t zi = (uint32_t)(eZero + z);
+                for (int k = 0; k < nstream; ++k) occ_of(st, lane, k).push_back(zi * S * 8 / gsz);
+                grid[(size_t)lane * steps + st] = kind == kProd ? (zi | zi << 16) : zi * S * 8;
+            }
+        return grid;
+    };
+
+    // ---- phase A chunks: sums of one kind, shared by equally many lanes and of similar length, fill the
+    // 32 lanes of a chunk; the warps take the chunks row by row, most expensive first.
+    {
+        std::vector<std::pair<uint32_t, int>> w;
+        for (auto &t : sums) {
+            if (t.kind == kProd) t.n_words = t.ent.size();
+            else { split(t.ent, w); t.n_words = w.size(); }
+            t.rshift = pick_rshift(t.n_words, hints.cap > 0 ? (size_t)hints.cap : 12);
+        }
+        struct Chunk { std::vector<Task *> t; uint32_t kind; int rshift; int steps; bool lvl01; double cost; };
         std::vector<Chunk> chunks;
-        if (with_r3 && nr > 0) chunks.push_back({{}, kAuxR3, 5, (nr + 31) / 32, true, 0.0, 1});
+        if (nr > 0) chunks.push_back({{}, kAll3, 5, (nr + 31) / 32, true, 0.0});
         std::vector<Task *> idx;
-        for (auto &t : tasks) idx.push_back(&t);
+        for (auto &t : sums)
+            if (t.kind == kSum3 || !t.ent.empty()) idx.push_back(&t);
         std::stable_sort(idx.begin(), idx.end(), [&](const Task *a, const Task *b) {
             if (a->kind != b->kind) return a->kind < b->kind;
             if (a->rshift != b->rshift) return a->rshift > b->rshift;
@@ -609,288 +690,179 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         });
         for (size_t p = 0; p < idx.size();) {
             const Task &t0 = *idx[p];
-            Chunk c{{}, t0.kind, t0.rshift, 0, t0.lvl01, 0.0, 1};
-            // single-sum lists without lane sharing: two sums per lane (independent accumulators)
-            const size_t per = (t0.kind == kAuxS1 && t0.rshift == 0) ? 64 : (size_t)32 >> t0.rshift;
+            Chunk c{{}, t0.kind, t0.rshift, 0, t0.lvl01, 0.0};
+            const size_t per = (size_t)32 >> t0.rshift;
             while (p < idx.size() && c.t.size() < per && idx[p]->kind == c.kind && idx[p]->rshift == c.rshift) {
                 c.steps = std::max(c.steps, idx[p]->steps());
                 c.t.push_back(idx[p++]);
             }
-            c.tpl = c.t.size() > 32 ? 2 : 1;
             chunks.push_back(c);
         }
-        // cost in units of about six instructions: a chunk's fixed part, its steps, its shuffle reduction
+        // cost in loads per block: a chunk's fixed part, its steps, its shuffle reduction
         for (auto &c : chunks) {
-            const double per_step = c.kind == kAuxT3 ? 2.0 : c.kind == kAuxR3 ? 2.5 : c.kind == kAuxH2 ? 1.5 : 1.0;
-            const double sums = (c.kind == kAuxT3 || c.kind == kAuxR3) ? 3.0 : 1.0;
-            c.cost = 7.0 + per_step * c.steps * c.tpl + 1.0 * sums * c.rshift;
+            const double per_step = c.kind == kSum3 ? 3.0 : c.kind == kAll3 ? 4.0 : c.kind == kProd ? 2.0 : 1.0;
+            const double nsum = (c.kind == kSum3 || c.kind == kAll3) ? 3.0 : 1.0;
+            c.cost = 4.0 + per_step * c.steps + 1.5 * nsum * c.rshift;
         }
-        // the warps take chunk (k * NW + w) in round k: arrange the chunks so that every warp gets about
-        // the same cost (longest first onto the least loaded warp; rows padded with empty chunks).
-        // The chunks the rates / source-term kernels need too come first, in rows of their own.
-        {
-            std::vector<Chunk> arranged;
-            load.resize(NW, 0.0);
-            for (int pass = 0; pass < 2; ++pass) {
-                std::vector<Chunk *> grp;
-                for (auto &c : chunks)
-                    if (c.lvl01 == (pass == 0)) grp.push_back(&c);
-                if (grp.empty()) continue;
-                std::stable_sort(grp.begin(), grp.end(), [](const Chunk *a, const Chunk *b) { return a->cost > b->cost; });
-                std::vector<std::vector<Chunk *>> mine(NW);
-                for (Chunk *c : grp) {
-                    int w = 0;
-                    for (int i = 1; i < NW; ++i)
-                        if (load[i] < load[w]) w = i;
-                    mine[w].push_back(c);
-                    load[w] += c->cost;
-                }
-                size_t rows = 0;
-                for (auto &v : mine) rows = std::max(rows, v.size());
-                for (size_t k = 0; k < rows; ++k)
-                    for (int w = 0; w < NW; ++w) {
-                        if (k < mine[w].size()) arranged.push_back(*mine[w][k]);
-                        else arranged.push_back(Chunk{{}, kAuxS1, 0, 0, pass == 0, 0.0, 1});      // empty chunk
-                    }
+        // the warps take chunk (row * NW + w): arrange the chunks so that every warp gets about the same
+        // cost (longest first onto the least loaded warp; rows padded with empty chunks).  The chunks the
+        // rates / source-term kernels need too come first, in rows of their own.
+        std::vector<Chunk> arranged;
+        std::vector<double> load(NW, 0.0);
+        int rows01 = 0;
+        for (int pass = 0; pass < 2; ++pass) {
+            std::vector<Chunk *> grp;
+            for (auto &c : chunks)
+                if (c.lvl01 == (pass == 0)) grp.push_back(&c);
+            if (grp.empty()) continue;
+            std::stable_sort(grp.begin(), grp.end(), [](const Chunk *a, const Chunk *b) { return a->cost > b->cost; });
+            std::vector<std::vector<Chunk *>> mine(NW);
+            for (Chunk *c : grp) {
+                int wmin = 0;
+                for (int i = 1; i < NW; ++i)
+                    if (load[i] < load[wmin]) wmin = i;
+                mine[wmin].push_back(c);
+                load[wmin] += c->cost;
             }
-            chunks.swap(arranged);
+            size_t rows = 0;
+            for (auto &v : mine) rows = std::max(rows, v.size());
+            for (size_t k = 0; k < rows; ++k)
+                for (int wi = 0; wi < NW; ++wi) {
+                    if (k < mine[wi].size()) arranged.push_back(*mine[wi][k]);
+                    else arranged.push_back(Chunk{{}, kSum1, 0, 0, pass == 0, 0.0});      // empty chunk
+                }
+            if (pass == 0) rows01 = (int)rows;
         }
-        int n01 = 0;
-        for (auto &c : chunks) {
-            n01 += c.lvl01 ? 1 : 0;
-            // layout (device_mech.h)
+        o.n_arow = (int)(arranged.size() / NW);
+        o.n_arow01 = rows01;
+        for (auto &c : arranged) {
             const uint32_t base = (uint32_t)(o.a_ent.size() / 4);       // in uint4 units
-            const int width = 1 << c.rshift;
-            const uint32_t pad = c.kind == kAuxH2 ? pad2 : pad1;
+            const int width = 1 << c.rshift, per_row = 32 / width;
             o.achunk.push_back(base);
-            o.achunk.push_back((uint32_t)c.steps | c.kind << 16 | (uint32_t)c.rshift << 20 | (uint32_t)c.tpl << 24);
-            const int rounds = c.tpl == 2 ? 2 + (c.steps > 1 ? (c.steps - 1 + 1) / 2 : 0)
-                                          : 1 + (c.steps > 1 ? (c.steps - 1 + 3) / 4 : 0);
-            o.a_ent.resize(o.a_ent.size() + (size_t)rounds * 128, pad);
+            o.achunk.push_back((uint32_t)c.steps | c.kind << 8 | (uint32_t)c.rshift << 12);
+            REQUIRE(c.steps < 256, "internal: a phase-A chunk has more than 255 steps");
+            const int nblk = 1 + (c.kind == kAll3 ? 0 : (c.steps + 3) / 4);
+            o.a_ent.resize(o.a_ent.size() + (size_t)nblk * 128, 0u);
             uint32_t *blk = o.a_ent.data() + (size_t)base * 4;
-            // ---- which sum sits on which lane(s), and in which order its entries are walked, is free:
-            // both are chosen greedily so that the lanes of one shared-memory wavefront (LP lanes, one
-            // load granule each) hit different bank groups at every step
-            const int per_row = 32 / width, nslot = c.tpl * per_row;
-            const int gsz = std::min(8 * S, 16), LP = 128 / gsz, nq = 32 / LP;
-            const int nstream = c.kind == kAuxH2 ? 2 : 1;
-            auto granules = [&](uint32_t w, uint32_t g[2]) {
-                if (c.kind == kAuxH2) { g[0] = (w & 0xFFFF) * S * 8 / gsz; g[1] = (w >> 16) * S * 8 / gsz; }
-                else g[0] = (w & kEntOffMask) / gsz;
-            };
-            // occ[((row * steps + step) * nq + quarter) * nstream + stream] = granules read there
-            std::vector<std::vector<uint32_t>> occ((size_t)c.tpl * std::max(c.steps, 1) * nq * nstream);
-            // the 16-byte stores of the results (kAuxS1: one per sum, all lanes of a row at once)
-            std::vector<std::vector<uint32_t>> occ_st((size_t)c.tpl * nq);
-            auto cell_of = [&](int row, int step, int lane, int st) -> std::vector<uint32_t> & {
-                return occ[(((size_t)row * c.steps + step) * nq + lane / LP) * nstream + st];
-            };
-            auto clash = [&](const std::vector<uint32_t> &v, uint32_t g) {
-                bool same_bank = false;
-                for (uint32_t x : v) {
-                    if (x == g) return 0;                  // same address: broadcast
-                    same_bank = same_bank || (x % LP == g % LP);
-                }
-                return same_bank ? 1 : 0;
-            };
-            std::vector<int> slot_task(nslot, -1);
-            std::vector<char> taken(c.t.size(), 0);
-            std::vector<std::vector<uint32_t>> tw(c.t.size());
-            if (c.kind != kAuxR3)
-                for (size_t i = 0; i < c.t.size(); ++i) { encode(*c.t[i], words); tw[i] = words; }
-            std::vector<std::vector<int>> where(c.t.size());     // per task: slot (lane * steps + step) of each entry
-            std::vector<char> used;
-            auto place = [&](int ti, int sl, bool commit) {
-                const int row = sl / per_row, lane0 = (sl % per_row) * width;
-                used.assign((size_t)width * std::max(c.steps, 1), 0);
-                int cost = 0;
-                if (commit) where[ti].clear();
-                if (c.kind == kAuxS1) {
-                    auto &st_cell = occ_st[(size_t)row * nq + lane0 / LP];
-                    const uint32_t g = c.t[ti]->out * S * 8 / gsz;
-                    cost += 2 * clash(st_cell, g);
-                    if (commit) st_cell.push_back(g);
-                }
-                for (uint32_t w : tw[ti]) {
-                    uint32_t g[2];
-                    granules(w, g);
-                    int best = -1, bc = 1 << 30;
-                    for (int st = 0; st < c.steps && bc > 0; ++st)
-                        for (int j = 0; j < width; ++j) {
-                            if (used[(size_t)j * c.steps + st]) continue;
-                            int cc = 0;
-                            for (int k = 0; k < nstream; ++k) cc += clash(cell_of(row, st, lane0 + j, k), g[k]);
-                            if (cc < bc) { bc = cc; best = j * c.steps + st; }
-                            if (bc == 0) break;
-                        }
-                    used[best] = 1;
-                    cost += bc;
-                    if (commit) {
-                        where[ti].push_back(best);
-                        for (int k = 0; k < nstream; ++k) cell_of(row, best % c.steps, lane0 + best / c.steps, k).push_back(g[k]);
-                    }
-                }
-                return cost;
-            };
-            if (c.kind != kAuxR3) {
-                size_t first_free = 0;
-                for (int sl = 0; sl < nslot && first_free < c.t.size(); ++sl) {
-                    int pick = -1, pc = 1 << 30, seen = 0;
-                    for (size_t i = first_free; i < c.t.size() && seen < 12 && pc > 0; ++i) {
-                        if (taken[i]) continue;
-                        ++seen;
-                        const int cc = place((int)i, sl, false);
-                        if (cc < pc) { pc = cc; pick = (int)i; }
-                    }
-                    if (pick < 0) break;
-                    place(pick, sl, true);
-                    taken[pick] = 1;
-                    slot_task[sl] = pick;
-                    while (first_free < c.t.size() && taken[first_free]) ++first_free;
+            for (int lane = 0; lane < 32; ++lane) {
+                const size_t sl = (size_t)lane / width;
+                uint32_t out = 0xFFFFFFFFu;
+                double cst = 0.0;
+                if (c.kind != kAll3 && sl < c.t.size()) { out = c.t[sl]->out; cst = c.t[sl]->cst; }
+                uint64_t bits;
+                std::memcpy(&bits, &cst, 8);
+                blk[(size_t)lane * 4 + 0] = out;
+                blk[(size_t)lane * 4 + 1] = (uint32_t)bits;
+                blk[(size_t)lane * 4 + 2] = (uint32_t)(bits >> 32);
+            }
+            if (c.kind == kAll3) { o.n_a_steps += c.steps; continue; }
+            std::vector<std::vector<uint32_t>> lists((size_t)per_row);
+            for (size_t i = 0; i < c.t.size(); ++i) {
+                if (c.kind == kProd) {
+                    for (auto &e : c.t[i]->ent) lists[i].push_back(e.first);
+                } else {
+                    split(c.t[i]->ent, w);
+                    for (auto &e : w) lists[i].push_back(enc(e));
                 }
             }
-            auto word_at = [&](int row, int lane, int step) -> uint32_t & {
-                size_t at;
-                if (c.tpl == 2)
-                    at = step == 0 ? ((size_t)row * 32 + lane) * 4 + 3
-                                   : ((size_t)(2 + (step - 1) / 2) * 32 + lane) * 4 + 2 * ((step - 1) % 2) + row;
-                else
-                    at = step == 0 ? (size_t)lane * 4 + 3 : ((size_t)(1 + (step - 1) / 4) * 32 + lane) * 4 + (step - 1) % 4;
-                return blk[at];
-            };
-            for (int row = 0; row < c.tpl; ++row)
-                for (int lane = 0; lane < 32; ++lane) {
-                    const int sl = row * per_row + lane / width, ti = slot_task[sl];
-                    uint32_t out = 0xFFFFFFFFu;
-                    double cst = 0.0;
-                    if (ti >= 0) { out = c.t[ti]->out; cst = c.t[ti]->cst; }
-                    uint64_t bits;
-                    std::memcpy(&bits, &cst, 8);
-                    uint32_t *rec = blk + ((size_t)row * 32 + lane) * 4;
-                    rec[0] = out;
-                    rec[1] = (uint32_t)bits;
-                    rec[2] = (uint32_t)(bits >> 32);
-                }
-            if (c.kind != kAuxR3) {
-                std::vector<char> filled((size_t)c.tpl * 32 * std::max(c.steps, 1), 0);
-                for (int sl = 0; sl < nslot; ++sl) {
-                    const int ti = slot_task[sl];
-                    if (ti < 0) continue;
-                    const int row = sl / per_row, lane0 = (sl % per_row) * width;
-                    for (size_t e = 0; e < tw[ti].size(); ++e) {
-                        const int lane = lane0 + where[ti][e] / c.steps, step = where[ti][e] % c.steps;
-                        word_at(row, lane, step) = tw[ti][e];
-                        filled[((size_t)row * 32 + lane) * c.steps + step] = 1;
-                    }
-                }
-                // pads: coefficient 0 (kAuxH2: zero times zero) on the zero slot whose bank group is free
-                for (int row = 0; row < c.tpl; ++row)
-                    for (int step = 0; step < c.steps; ++step)
-                        for (int lane = 0; lane < 32; ++lane) {
-                            if (filled[((size_t)row * 32 + lane) * c.steps + step]) continue;
-                            int z = 0;
-                            for (int t = 0; t < LP; ++t) {
-                                const uint32_t g = (uint32_t)(eZero + t) * S * 8 / gsz;
-                                bool ok = true;
-                                for (int k = 0; k < nstream; ++k) ok = ok && clash(cell_of(row, step, lane, k), g) == 0;
-                                if (ok) { z = t; break; }
-                            }
-                            const uint32_t zi = (uint32_t)(eZero + z);
-                            for (int k = 0; k < nstream; ++k) cell_of(row, step, lane, k).push_back(zi * S * 8 / gsz);
-                            word_at(row, lane, step) = c.kind == kAuxH2 ? (zi | zi << 16) : zi * S * 8;
-                        }
-            }
-            step_count += c.steps;
+            // blocks of four steps; the words behind the chunk's last step are never read
+            const std::vector<uint32_t> grid = place(lists, width, c.steps, c.kind);
+            for (int lane = 0; lane < 32; ++lane)
+                for (int st = 0; st < c.steps; ++st)
+                    blk[((size_t)(1 + st / 4) * 32 + lane) * 4 + st % 4] = grid[(size_t)lane * c.steps + st];
+            o.n_a_steps += c.steps;
         }
-        return std::make_pair((int)chunks.size(), n01);
-    };
-
-    {
-        auto r = emit_phase(a1, true, o.n_a1_steps, a1_load);
-        o.n_a1 = r.first;
-        o.n_a1_01 = r.second;
+        o.a_ent.resize(o.a_ent.size() + 128, 0u);        // the kernels read one block past a chunk's last
     }
 
-    // ---- the cells, panel by panel.  Column 0 (rows >= 1) is written by the kAuxT3 sums; row 0 (the
-    // energy row) never enters the tile, the FIX step stores it.  Cells without a list get no task: the
-    // tile starts as zeros and, with several panels, the DENSE pass zeroes each buffer behind itself.
-    o.panel_ptr.assign(1, o.n_a1);
-    for (int p = 0; p < n_panel; ++p) {
-        std::vector<Task> tasks;
-        const int c0 = p * pw, c1 = std::min(ld, c0 + pw);
-        for (int c = c0; c < c1; ++c)
-            for (int r = 0; r < ld; ++r) {
-                if (c == 0 && r >= 1) continue;
-                if (r == 0) continue;
-                Task t;
-                t.kind = kAuxS1;
-                t.out = (uint32_t)(eTile + (p % nbuf) * pw * ld + (c - c0) * ld + r);
-                t.ent = cell[(size_t)r + (size_t)c * ld];
-                if (!t.ent.empty()) t.cst = d->mol_wt[r - 1] * (1.0 / d->mol_wt[c - 1]);
-                if (t.ent.empty()) continue;        // stays zero: the DENSE pass zeroes a tile buffer behind itself
-                o.n_cell_entries += (long long)t.ent.size();
-                tasks.push_back(t);
-            }
-        o.n_cells += (long long)tasks.size();
-        // the cells of panel 0 are gathered in the same phase as the A1 sums: continue their balance;
-        // the cells of panel p >= 1 share their step with the DENSE items of panel p - 1, dealt round-robin
-        std::vector<double> load = p == 0 ? a1_load : std::vector<double>(NW, 0.0);
-        if (p >= 1) {
-            const int RP = o.pair ? 2 : 1, n_slab = (ld + 32 * RP - 1) / (32 * RP);
-            const int ncol_prev = std::min(ld, p * pw) - (p - 1) * pw;
-            const int nd = n_slab * ((ncol_prev + o.d_seg - 1) / o.d_seg);
-            // cost of a DENSE item in the units of emit_phase; measured on cfg2: 9.53 / 9.39 / 9.62 / 10.33 ms
-            // with 0 / 0.5 / 1 / 1.5 times (10 + 5 d_seg)
-            for (int it = 0; it < nd; ++it) load[it % NW] += 5.0 + 2.5 * o.d_seg;
-        }
-        auto r = emit_phase(tasks, false, o.n_cell_steps, load);
-        o.panel_ptr.push_back(o.panel_ptr.back() + r.first);
-    }
-    o.a_ent.resize(o.a_ent.size() + 256, pad1);      // the kernels read one or two blocks past a chunk's last
-    o.achunk.resize(o.achunk.size() + (size_t)2 * 3 * NW, 0u);       // headers are read three rounds ahead
-
-    // ---- self-check of what the kernels rely on without bounds checks (kernels.cu gather_run /
-    // gather_chunk): whole rows of NW chunks per phase, every block a chunk reads inside a_ent (its own
-    // blocks and the unconditional block 1), every header the pipe reads ahead inside achunk, every
-    // source offset and output index inside the CTA's E + tile array
+    // ---- phase B items: one per (slab, column); a lane's cells are rows rp * (32 slab + lane) .. + rp - 1
     {
-        const size_t n_chunks = o.achunk.size() / 2 - (size_t)3 * NW, n_blocks = o.a_ent.size() / 4;
-        const uint32_t e_total = (uint32_t)(o.n_e + nbuf * pw * ld);
-        auto bad = [](const char *w) { throw Fail{PYJAC_ELIMIT, w}; };
-        if (o.n_a1 % NW || o.n_a1_01 % NW || (size_t)o.panel_ptr.back() != n_chunks || o.panel_ptr[0] != o.n_a1)
-            bad("internal: gather phases are not whole rows of chunks");
-        for (size_t p = 0; p + 1 < o.panel_ptr.size(); ++p)
-            if (o.panel_ptr[p + 1] < o.panel_ptr[p] || (o.panel_ptr[p + 1] - o.panel_ptr[p]) % NW)
-                bad("internal: a panel's chunks are not whole rows");
+        o.bitem.assign((size_t)2 * (o.n_slab * ld + 2), 0u);     // headers are read two items ahead
+        o.b_ent.assign(128, 0u);                                  // block 0: what empty items point at
+        std::vector<double> cost((size_t)o.n_slab * ld, 0.0);
+        for (int slab = 0; slab < o.n_slab; ++slab)
+            for (int c = 0; c < ld; ++c) {
+                const size_t it = (size_t)slab * ld + c;
+                int nst[2] = {0, 0};
+                std::vector<std::vector<uint32_t>> lists[2];
+                for (int h = 0; h < rp; ++h) {
+                    lists[h].resize(32);
+                    for (int lane = 0; lane < 32; ++lane) {
+                        const int r = rp * (32 * slab + lane) + h;
+                        if (r >= ld) continue;
+                        for (auto &e : cell_w[(size_t)r + (size_t)c * ld]) lists[h][lane].push_back(enc(e));
+                        nst[h] = std::max(nst[h], (int)lists[h][lane].size());
+                    }
+                }
+                REQUIRE(nst[0] <= 4 && nst[1] <= 4, "internal: a phase-B cell list is longer than four entries");
+                cost[it] = 6.0 + 2.0 * rp + nst[0] + nst[1];
+                o.n_b_steps += nst[0] + nst[1];
+                if (nst[0] + nst[1] == 0) continue;
+                const uint32_t base = (uint32_t)(o.b_ent.size() / 4);
+                o.bitem[2 * it] = base;
+                o.bitem[2 * it + 1] = (uint32_t)nst[0] | (uint32_t)nst[1] << 8;
+                o.b_ent.resize(o.b_ent.size() + (size_t)rp * 128, 0u);
+                for (int h = 0; h < rp; ++h) {
+                    // all four words are filled (pads beyond the item's steps are never read)
+                    const std::vector<uint32_t> grid = place(lists[h], 1, std::max(nst[h], 1), kSum1);
+                    const int ns_h = std::max(nst[h], 1);
+                    for (int lane = 0; lane < 32; ++lane)
+                        for (int st = 0; st < 4; ++st)
+                            o.b_ent[((size_t)base + 32 * h + lane) * 4 + st] =
+                                st < ns_h ? grid[(size_t)lane * ns_h + st] : (uint32_t)(eZero * S * 8);
+                }
+            }
+        // contiguous ranges of items per warp, balanced by cost
+        double total = 0.0;
+        for (double c : cost) total += c;
+        o.bsplit.assign(NW + 1, 0);
+        double acc = 0.0;
+        int wi = 1;
+        for (size_t it = 0; it < cost.size(); ++it) {
+            acc += cost[it];
+            while (wi < NW && acc >= total * wi / NW) o.bsplit[wi++] = (int32_t)(it + 1);
+        }
+        while (wi <= NW) o.bsplit[wi++] = (int32_t)cost.size();
+    }
+
+    // ---- self-check of what the kernels rely on without bounds checks: every source offset and every
+    // output index inside the block's E array, every block a chunk or an item reads inside its table
+    {
+        auto bad = [](const char *wh) { throw Fail{PYJAC_ELIMIT, wh}; };
+        const uint32_t e_total = (uint32_t)o.n_e;
+        const size_t na_blocks = o.a_ent.size() / 4, nb_blocks = o.b_ent.size() / 4;
+        if (o.achunk.size() / 2 != (size_t)o.n_arow * NW) bad("internal: phase A is not whole rows of chunks");
         for (size_t c = 0; c < o.achunk.size() / 2; ++c) {
             const uint32_t base = o.achunk[2 * c], meta = o.achunk[2 * c + 1];
-            const int steps = (int)(meta & 0xFFFF), kind = (int)((meta >> 16) & 0xF), tpl = (int)(meta >> 24);
-            const int rounds = c >= n_chunks ? 1
-                             : tpl == 2 ? 2 + (steps > 1 ? steps / 2 : 0) : 1 + (steps > 1 ? (steps + 2) / 4 : 0);
-            if ((size_t)base + 32 * (size_t)std::max(rounds, 2) > n_blocks) bad("internal: a chunk reads past the entry table");
-            if (c >= n_chunks || kind == (int)kAuxR3) continue;
+            const int steps = (int)(meta & 0xFF), kind = (int)((meta >> 8) & 0xF);
+            const int nblk = 1 + (kind == (int)kAll3 ? 0 : (steps + 3) / 4);
+            if ((size_t)base + 32 * (size_t)(nblk + 1) > na_blocks) bad("internal: a chunk reads past the entry table");
+            if (kind == (int)kAll3) continue;
             const uint32_t *blk = o.a_ent.data() + (size_t)base * 4;
-            for (int row = 0; row < std::max(tpl, 1); ++row)
-                for (int lane = 0; lane < 32; ++lane) {
-                    const uint32_t out = blk[((size_t)row * 32 + lane) * 4];
-                    if (out != 0xFFFFFFFFu && out >= (kind == (int)kAuxT3 ? (uint32_t)ns : e_total))
-                        bad("internal: a gather result lies outside E");
-                    for (int st = 0; st < steps; ++st) {
-                        size_t at;
-                        if (tpl == 2)
-                            at = st == 0 ? ((size_t)row * 32 + lane) * 4 + 3
-                                         : ((size_t)(2 + (st - 1) / 2) * 32 + lane) * 4 + 2 * ((st - 1) % 2) + row;
-                        else
-                            at = st == 0 ? (size_t)lane * 4 + 3 : ((size_t)(1 + (st - 1) / 4) * 32 + lane) * 4 + (st - 1) % 4;
-                        const uint32_t w = blk[at];
-                        const bool ok = kind == (int)kAuxH2
-                                            ? ((w & 0xFFFF) < e_total && (w >> 16) < e_total)
-                                            : ((w & kEntOffMask) % (8u * S) == 0 &&
-                                               (w & kEntOffMask) / (8u * S) + (kind == (int)kAuxT3 ? 2u : 0u) < e_total);
-                        if (!ok) bad("internal: a gather entry points outside E");
-                    }
+            for (int lane = 0; lane < 32; ++lane) {
+                const uint32_t out = blk[(size_t)lane * 4];
+                if (out != 0xFFFFFFFFu && out >= (kind == (int)kSum3 ? (uint32_t)ns : e_total))
+                    bad("internal: a gather result lies outside E");
+                for (int st = 0; st < steps; ++st) {
+                    const uint32_t wd = blk[((size_t)(1 + st / 4) * 32 + lane) * 4 + st % 4];
+                    const bool ok = kind == (int)kProd
+                                        ? ((wd & 0xFFFF) < e_total && (wd >> 16) < e_total)
+                                        : ((wd & kEntOffMask) % (8u * S) == 0 &&
+                                           (wd & kEntOffMask) / (8u * S) + (kind == (int)kSum3 ? 2u : 0u) < e_total);
+                    if (!ok) bad("internal: a gather entry points outside E");
                 }
+            }
         }
+        for (size_t it = 0; it < o.bitem.size() / 2; ++it) {
+            const uint32_t base = o.bitem[2 * it];
+            if ((size_t)base + 32 * (size_t)rp > nb_blocks) bad("internal: an item reads past the entry table");
+            for (size_t k = 0; k < (size_t)rp * 128; ++k) {
+                const uint32_t wd = o.b_ent[(size_t)base * 4 + k];
+                if ((wd & kEntOffMask) % (8u * S) != 0 || (wd & kEntOffMask) / (8u * S) >= e_total)
+                    bad("internal: a cell entry points outside E");
+            }
+        }
+        if (o.bsplit[0] != 0 || o.bsplit[NW] != o.n_slab * ld) bad("internal: phase B ranges do not cover the items");
     }
 }
 
