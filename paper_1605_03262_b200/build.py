@@ -2,7 +2,7 @@
 
     python -m paper_1605_03262_b200.build [--force] [--verbose]
 
-nvcc cross-compiles without a GPU.  kernels.cu is compiled once per launch shape (S, NP) (in parallel), the
+nvcc cross-compiles without a GPU.  kernels.cu is compiled once per S (states a CTA interleaves; in parallel), the
 objects go to paper_1605_03262_b200/build/.  The .so is git-ignored but travels to the GPU box.
 """
 from __future__ import annotations
@@ -17,8 +17,8 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libpyjac_b200.so")
 HOST_SOURCES = ["api.cu", "mech_pack.cu", "dispatch.cu"]
-# (states per block, blocks per CTA iteration) -- keep in step with csrc/dispatch.cu
-KERNEL_SHAPES = [(s, np_) for s in (1, 2) for np_ in (1, 2, 3, 4)]
+# states a CTA interleaves per iteration -- keep in step with csrc/dispatch.cu
+KERNEL_S = [1, 2, 3, 4, 6]
 HEADERS = ["device_mech.h", "kernels.h", "mech_pack.h", os.path.join("..", "..", "include", "pyjac_b200.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]
@@ -48,9 +48,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for f in HOST_SOURCES:
         o = os.path.join(OBJ, f[:-3] + ".o")
         jobs.append((o, [_nvcc()] + NVCC_FLAGS + extra + ["-c", os.path.join(CSRC, f), "-o", o]))
-    for sv, npv in KERNEL_SHAPES:
-        o = os.path.join(OBJ, "kernels_%d_%d.o" % (sv, npv))
-        jobs.append((o, [_nvcc()] + NVCC_FLAGS + extra + ["-DPYJAC_S=%d" % sv, "-DPYJAC_NP=%d" % npv, "-c",
+    for sv in KERNEL_S:
+        o = os.path.join(OBJ, "kernels_s%d.o" % sv)
+        jobs.append((o, [_nvcc()] + NVCC_FLAGS + extra + ["-DPYJAC_S=%d" % sv, "-c",
                                                           os.path.join(CSRC, "kernels.cu"), "-o", o]))
 
     def run(job):

@@ -21,7 +21,7 @@ struct pyjac_mech {
     DeviceMech dm{};
     SmemPlan plan{};
     int threads = 128;
-    int S = 1, NP = 1;          // NP blocks of S states per CTA iteration
+    int S = 1;                  // states per CTA iteration
     size_t smem[3] = {0, 0, 0}; // dynamic shared memory per level
     int ctas_per_sm[3] = {1, 1, 1};
     int n_sm = 1;
@@ -45,7 +45,7 @@ struct Uploader {
     }
 };
 
-// Tuning hooks, read at pyjac_mech_create / pyjac_pack_stats: PYJAC_S, PYJAC_NP, PYJAC_THREADS,
+// Tuning hooks, read at pyjac_mech_create / pyjac_pack_stats: PYJAC_S, PYJAC_THREADS,
 // PYJAC_CTAS override the launch shape mech_pack.cu would choose, PYJAC_CAP / PYJAC_CELL_CAP the list
 // lengths of phases A / B, PYJAC_RP the rows per lane of phase B; a value that is not instantiated or
 // does not fit is an error at create.
@@ -54,7 +54,6 @@ ShapeHints hints_from_env(long long smem_optin)
     ShapeHints h;
     if (smem_optin > 0) h.smem_bytes = smem_optin - 128;
     if (const char *e = std::getenv("PYJAC_S")) h.S = std::atoi(e);
-    if (const char *e = std::getenv("PYJAC_NP")) h.NP = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_THREADS")) h.threads = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_CTAS")) h.ctas = std::atoi(e);
     if (const char *e = std::getenv("PYJAC_CAP")) h.cap = std::atoi(e);
@@ -80,10 +79,9 @@ int launch(const pyjac_mech *m, int level, int64_t n, const double *T, const dou
     if (cudaGetDevice(&dev) != cudaSuccess) return PYJAC_ECUDA;
     if (dev != m->device && cudaSetDevice(m->device) != cudaSuccess) return PYJAC_ECUDA;
     long long cap = (long long)m->n_sm * m->ctas_per_sm[level];
-    const long long per = (long long)m->S * m->NP;
-    const long long blocks = (n + per - 1) / per;
+    const long long blocks = (n + m->S - 1) / m->S;
     int grid = (int)(blocks < cap ? blocks : cap);
-    cudaError_t e = launch_eval(level, m->threads, m->S, m->NP, m->dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy,
+    cudaError_t e = launch_eval(level, m->threads, m->S, m->dm, m->plan, grid, m->smem[level], n, T, P, Y, ldy,
                                 out, (cudaStream_t)stream);
     if (dev != m->device) cudaSetDevice(dev);
     if (e != cudaSuccess) return PYJAC_ECUDA;
@@ -120,7 +118,6 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     m->n_sm = prop.multiProcessorCount;
     m->threads = hp.threads;
     m->S = hp.S;
-    m->NP = hp.NP;
     DeviceMech &dm = m->dm;
     dm.ns = hp.ns; dm.nr = hp.nr; dm.ld = hp.ns + 1;
     dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk; dm.n_plain = (int)hp.n_plain_chunks;
@@ -147,7 +144,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         up.add(&dm.eff_base, hp.eff_base); up.add((const uint32_t **)&dm.eff_ent, hp.eff_ent);
         up.add(&dm.pk_ptr, hp.pk_ptr); up.add(&dm.pk_data, hp.pk_data);
         up.add((const uint32_t **)&dm.achunk, hp.achunk); up.add((const uint32_t **)&dm.a_ent, hp.a_ent);
-        up.add((const uint32_t **)&dm.bitem, hp.bitem); up.add((const uint32_t **)&dm.b_ent, hp.b_ent);
+        up.add((const uint32_t **)&dm.b_ent, hp.b_ent);
         up.add(&dm.bsplit, hp.bsplit);
     } catch (...) {
         delete m;
@@ -166,13 +163,13 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         m->stats[0] = hp.n_e; m->stats[1] = hp.n_cell_entries; m->stats[2] = hp.n_b_steps;
         m->stats[3] = hp.n_a_steps; m->stats[4] = hp.n_cells; m->stats[5] = (long long)hp.achunk.size() / 2;
         m->stats[6] = hp.n_heavy_cells; m->stats[7] = hp.n_heavy_pieces;
-        const size_t bytes = eval_smem_bytes(m->plan, m->S, m->NP);
-        if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->S, m->NP)) {
+        const size_t bytes = eval_smem_bytes(m->plan, m->S);
+        if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->S)) {
             rc = PYJAC_ELIMIT;
         } else {
             for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
                 m->smem[level] = bytes;
-                const void *k = eval_kernel_ptr(level, m->S, m->NP);
+                const void *k = eval_kernel_ptr(level, m->S);
                 // the kernel function is shared by every handle of this shape: its dynamic shared-memory limit
                 // is raised to what the device allows, once and for all, never to one handle's size
                 cudaFuncAttributes fa{};
@@ -258,8 +255,7 @@ int pyjac_jacobian_launch_config(const pyjac_mech *m, int64_t n, int32_t *thread
     if (smem_bytes) *smem_bytes = (int32_t)m->smem[2];
     if (ctas_per_sm) *ctas_per_sm = m->ctas_per_sm[2];
     long long cap = (long long)m->n_sm * m->ctas_per_sm[2];
-    const long long per = (long long)m->S * m->NP;
-    const long long blocks = (n + per - 1) / per;
+    const long long blocks = (n + m->S - 1) / m->S;
     if (grid) *grid = (int32_t)(blocks < cap ? blocks : cap);
     return PYJAC_OK;
 }
@@ -272,8 +268,8 @@ int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
     if (rc != PYJAC_OK) return rc;
     const SmemPlan plan = make_smem_plan(hp.ns, hp.n_e);
     stats[0] = hp.n_e; stats[1] = hp.n_cell_entries; stats[2] = hp.n_b_steps; stats[3] = hp.n_a_steps;
-    stats[4] = hp.n_cells; stats[5] = (int64_t)hp.achunk.size() / 2; stats[6] = (int64_t)eval_smem_bytes(plan, hp.S, hp.NP);
-    stats[7] = hp.n_rchunk; stats[8] = hp.S; stats[9] = hp.threads; stats[10] = hp.NP; stats[11] = hp.ctas_target;
+    stats[4] = hp.n_cells; stats[5] = (int64_t)hp.achunk.size() / 2; stats[6] = (int64_t)eval_smem_bytes(plan, hp.S);
+    stats[7] = hp.n_rchunk; stats[8] = hp.S; stats[9] = hp.threads; stats[10] = 1; stats[11] = hp.ctas_target;
     stats[12] = hp.n_heavy_cells; stats[13] = hp.n_heavy_pieces; stats[14] = (int64_t)hp.a_ent.size() * 4;
     stats[15] = (int64_t)hp.b_ent.size() * 4;
     return PYJAC_OK;

@@ -6,8 +6,8 @@
 // modification (Eq. 20).  Reactions are stored in a SORTED order (most expensive rate form first,
 // the plain elementary ones last); `rxn_orig` maps back to the caller's order.
 //
-// One CTA evaluates NP blocks of S states at a time.  Every block owns one array `E` in shared memory
-// (element e of state q at (e * S + q) doubles); the evaluation is a chain of fixed-order gathers over it:
+// One CTA evaluates S states at a time, interleaved in one array `E` in shared memory (element e of
+// state q at (e * S + q) doubles); the evaluation is a chain of fixed-order gathers over it:
 //   P1  writes, per reaction, the reusable products of Section 4.1: the sparse
 //       derivative terms s'_ij (region V), q_i, a_i, Theta_dT,i (region Q, interleaved per reaction)
 //       and the reaction enthalpy H_i (region H);
@@ -24,7 +24,6 @@ namespace pyjac {
 constexpr double kRu = 8314.46261815324;   // J kmol^-1 K^-1
 constexpr double kPatm = 101325.0;         // Pa
 constexpr int kMaxSide = 3;                // species per reaction side
-constexpr int kMaxNP = 4;                  // blocks of S states per CTA iteration
 constexpr int kMaxThreads = 512;           // threads per CTA the kernels are compiled for
 
 // meta word of a reaction: bits 0..23 six 4-bit nu (slots 0-2 reactants, 3-5 products; 0 = empty
@@ -39,7 +38,7 @@ __host__ __device__ inline int meta_form(uint32_t m) { return (m >> 29) & 3; }
 __host__ __device__ inline int meta_single(uint32_t m) { return (m >> 31) & 1; }
 
 // A gather entry of the kSum1 / kSum3 lists and of the Jacobian cells: bits 0..17 = byte offset of the
-// source element in the block's E array (E index * S * 8, below 256 KB), bits 18..31 = the top 14 bits
+// source element in the CTA's E array (E index * S * 8, below 256 KB), bits 18..31 = the top 14 bits
 // of the fp64 coefficient (sign, exponent, two mantissa bits: exact for every integer up to 8 in
 // magnitude; larger ones are split into two entries).  Coefficient bits 0 = the padding entry.
 constexpr uint32_t kEntOffMask = 0x3FFFFu;
@@ -116,9 +115,8 @@ struct DeviceMech {
     // ---- phase B: one item per (slab of rows, Jacobian column), slab-major.  A lane owns `rp` rows
     // (rp = 2: rows 64 slab + 2 lane, + 1, stored with one 16-byte store; rp = 1 when ld is odd).
     int rp, n_slab;
-    const uint2 *bitem;         // [n_slab * ld] {first block of b_ent, steps of the first row | steps of the second << 8}
-    const uint4 *b_ent;         // b_ent[first + lane] = up to four entries of the lane's first cell,
-                                // b_ent[first + 32 + lane] of its second cell (rp = 2)
+    const uint4 *b_ent;         // item it = slab * ld + c: b_ent[(it * rp + h) * 32 + lane] = {three entries of the lane's
+                                // cell h (padded with the zero slot), steps of the item's cells h: 0 none, 1 one, 2 three}
     const int32_t *bsplit;      // [NW + 1] the items of warp w are [bsplit[w], bsplit[w + 1])
     // ---- regions of E (indices in elements per state)
     int eQ;                     // [nr][3] {q_i, a_i + W q_i, Theta_dT,i}
@@ -139,10 +137,10 @@ enum {
     kT = 0, kLnT, kInvT, kP, kLnP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kIcp, kNScal = 12
 };
 
-// Shared-memory plan (offsets in doubles PER STATE).  A block of S states is interleaved: element i of
-// region R of state q lives at (R + i) * S + q within the block; NP blocks follow one another.  The
-// mixture part (X, Cp, Scal) exists twice: the one of the next batch is filled while this one is in
-// use.  After the NP blocks come the state-independent tables (colc, wrow), loaded once per CTA.
+// Shared-memory plan (offsets in doubles PER STATE).  The S states of a CTA iteration are interleaved:
+// element i of region R of state q lives at (R + i) * S + q.  The mixture part (X, Cp, Scal) exists
+// twice: the one of the next iteration is filled while this one is in use.  After the S states come the
+// state-independent tables (colc, wrow), loaded once per CTA.
 struct SmemPlan {
     int E;                              // [n_e]
     int P0;                             // two mixture parts of p0size doubles
@@ -151,7 +149,7 @@ struct SmemPlan {
     int oCp;                            // [ns] c_pk (mass based)
     int oScal;                          // [kNScal]
     int total;                          // doubles per state
-    int colc;                           // [ld][4], offset in doubles from the end of the blocks
+    int colc;                           // [ld][4], offset in doubles from the end of the state part
     int wrow;                           // [ld]
     int shared_total;                   // doubles of the state-independent part
 };

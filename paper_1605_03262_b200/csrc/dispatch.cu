@@ -1,17 +1,17 @@
-// dispatch.cu -- switches over the (S, NP) shapes kernels.cu was compiled for (build.py: one object per shape).
+// dispatch.cu -- switches over the S (states per CTA iteration) kernels.cu was compiled for (build.py: one object per S).
 #include "kernels.h"
 
 namespace pyjac {
 
-// (states per block, blocks per CTA iteration) -- keep in step with build.py
-#define PYJAC_FOR_SHAPE(X) X(1, 1) X(1, 2) X(1, 3) X(1, 4) X(2, 1) X(2, 2) X(2, 3) X(2, 4)
+// states a CTA interleaves per iteration -- keep in step with build.py
+#define PYJAC_FOR_S(X) X(1) X(2) X(3) X(4) X(6)
 
-#define PYJAC_DECL(SV, NPV)                                                                                         \
-    const void *eval_kernel_ptr_##SV##_##NPV(int level);                                                           \
-    cudaError_t launch_eval_##SV##_##NPV(int level, int threads, const DeviceMech &m, const SmemPlan &sp, int grid, \
-                                         size_t smem, long long n, const double *T, const double *P,               \
-                                         const double *Y, long long ldy, const EvalOut &out, cudaStream_t stream);
-PYJAC_FOR_SHAPE(PYJAC_DECL)
+#define PYJAC_DECL(SV)                                                                                             \
+    const void *eval_kernel_ptr_##SV(int level);                                                                   \
+    cudaError_t launch_eval_##SV(int level, int threads, const DeviceMech &m, const SmemPlan &sp, int grid,        \
+                                 size_t smem, long long n, const double *T, const double *P, const double *Y,      \
+                                 long long ldy, const EvalOut &out, cudaStream_t stream);
+PYJAC_FOR_S(PYJAC_DECL)
 #undef PYJAC_DECL
 
 namespace {
@@ -48,27 +48,24 @@ cudaError_t launch_peak_dfma(double *out, long long iters, int grid, cudaStream_
     return cudaGetLastError();
 }
 
-size_t eval_smem_bytes(const SmemPlan &sp, int S, int NP)
-{
-    return ((size_t)S * NP * sp.total + (size_t)sp.shared_total) * sizeof(double);
-}
+size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + (size_t)sp.shared_total) * sizeof(double); }
 
-const void *eval_kernel_ptr(int level, int S, int NP)
+const void *eval_kernel_ptr(int level, int S)
 {
-#define PYJAC_PTR(SV, NPV) \
-    if (S == SV && NP == NPV) return eval_kernel_ptr_##SV##_##NPV(level);
-    PYJAC_FOR_SHAPE(PYJAC_PTR)
+#define PYJAC_PTR(SV) \
+    if (S == SV) return eval_kernel_ptr_##SV(level);
+    PYJAC_FOR_S(PYJAC_PTR)
 #undef PYJAC_PTR
     return nullptr;
 }
 
-cudaError_t launch_eval(int level, int threads, int S, int NP, const DeviceMech &m, const SmemPlan &sp, int grid,
-                        size_t smem, long long n, const double *T, const double *P, const double *Y, long long ldy,
+cudaError_t launch_eval(int level, int threads, int S, const DeviceMech &m, const SmemPlan &sp, int grid, size_t smem,
+                        long long n, const double *T, const double *P, const double *Y, long long ldy,
                         const EvalOut &out, cudaStream_t stream)
 {
-#define PYJAC_CASE(SV, NPV) \
-    if (S == SV && NP == NPV) return launch_eval_##SV##_##NPV(level, threads, m, sp, grid, smem, n, T, P, Y, ldy, out, stream);
-    PYJAC_FOR_SHAPE(PYJAC_CASE)
+#define PYJAC_CASE(SV) \
+    if (S == SV) return launch_eval_##SV(level, threads, m, sp, grid, smem, n, T, P, Y, ldy, out, stream);
+    PYJAC_FOR_S(PYJAC_CASE)
 #undef PYJAC_CASE
     return cudaErrorInvalidValue;
 }

@@ -1,10 +1,10 @@
 // kernels.cu -- sm_100a kernels for the batched source term and analytical Jacobian.
 //
-// One CTA evaluates NP blocks of S thermochemical states per iteration of a persistent grid-stride loop.
-// The S states of a block are interleaved in shared memory (element i of a region for state q at
-// (R + i) * S + q), so whatever does not depend on the state -- decoding a reaction, a gather entry, a
-// column constant -- is done once per lane and applied to the S states of each of the NP blocks with
-// vector loads.  Per iteration, separated by CTA barriers:
+// One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop.  The S
+// states are interleaved in shared memory (element i of a region for state q at (R + i) * S + q), so
+// whatever does not depend on the state -- decoding a reaction, a gather entry, a column constant -- is
+// done once per lane and applied to the S states with vector loads.  Per iteration, separated by CTA
+// barriers:
 //   P0  mixture (Eqs. 3-5) and species, warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT
 //       (Eqs. 9-13, 54-55); computed one iteration ahead, at the end of phase B
 //   P1  reactions, lane <-> reaction, groups of 32 from one dynamic queue: k_f, k_r (K_c from the
@@ -15,7 +15,7 @@
 //   A   fixed-order gathers over E, lane <-> sum (or a share of one): wdot_k (Eq. 14), alpha'_r, gamma'_r
 //       of Eq. 112, the T column (Eq. 111), the column sums of the energy row (Eq. 113), and the long
 //       Jacobian-cell lists piece by piece
-//   B   the Jacobian, column by column, lane <-> two rows: every cell gathers its (at most four) entries
+//   B   the Jacobian, column by column, lane <-> two rows: every cell gathers its (at most three) entries
 //       on top of alpha'_r u_c - gamma'_r v_c, which is Eq. 112 with the per-reaction terms of Eqs.
 //       118-127 regrouped by what they multiply, and is stored at once: a warp
 //       stores 512 contiguous bytes per state and column, nothing is staged.  FIX items of the same phase
@@ -121,7 +121,7 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
                                                 const double *sc, int s, int q0, const EvalOut &out, long long state0,
                                                 long long n)
 {
-    constexpr int SP = S >= 2 ? 2 : 1;
+    constexpr int SP = S % 2 == 0 ? 2 : 1;
     const int nr = m.nr;
     const uint4 sl = m.slots[s];
     const uint32_t meta = sl.w;
@@ -523,370 +523,309 @@ __device__ __forceinline__ void st_cs_v2(double *p, double a, double b)
     asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a), "d"(b) : "memory");
 }
 
-// ---- phase A, one chunk: 32 lanes, 32 >> rshift sums (device_mech.h), for the NP blocks at once:
-// an entry is decoded once and applied to every block
-template <int LEVEL, int S, int NP>
-__device__ __forceinline__ void a_chunk(const DeviceMech &m, double *E0, uint32_t blk_bytes, const double *sc0,
-                                        const uint2 ch, int lane)
+// ---- phase A, one chunk: 32 lanes, 32 >> rshift sums (device_mech.h).  An entry is decoded once and
+// applied to the S states; whole blocks of four steps run without a branch, the chunk's last block by
+// its step count.
+template <int LEVEL, int S>
+__device__ __forceinline__ void a_chunk(const DeviceMech &m, double *E, const double *sc, const uint2 ch, int lane)
 {
     const uint32_t kind = (ch.y >> 8) & 0xF;
     const int steps = (int)(ch.y & 0xFF), rshift = (int)(ch.y >> 12) & 0xF, width = 1 << rshift;
     const uint4 *ep = m.a_ent + ch.x + lane;
     const uint4 r0 = ep[0];
     const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
-    const char *Eb = reinterpret_cast<const char *>(E0);
+    const char *Eb = reinterpret_cast<const char *>(E);
     const int nr = m.nr;
+    const int nfull = steps >> 2, rem = steps & 3;
+
+    // walks the chunk's blocks: `step` is applied to every entry of the lane
+#define PYJAC_WALK(step)                                                   \
+    {                                                                      \
+        const uint4 *bp = ep + 32;                                         \
+        uint4 w = *bp;                                                     \
+        for (int b = 0; b < nfull; ++b) {                                  \
+            bp += 32;                                                      \
+            const uint4 wn = *bp; /* one block ahead (the table is padded) */ \
+            step(w.x); step(w.y); step(w.z); step(w.w);                    \
+            w = wn;                                                        \
+        }                                                                  \
+        if (rem > 0) {                                                     \
+            step(w.x);                                                     \
+            if (rem > 1) {                                                 \
+                step(w.y);                                                 \
+                if (rem > 2) step(w.z);                                    \
+            }                                                              \
+        }                                                                  \
+    }
 
     if (kind == kSum1) {
         if (LEVEL == 2) {
-            double acc[NP][S];
+            double acc[S];
 #pragma unroll
-            for (int p = 0; p < NP; ++p)
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[p][q] = 0.0;
+            for (int q = 0; q < S; ++q) acc[q] = 0.0;
             auto step = [&](uint32_t w) {
                 const double cf = entry_coef(w);
-                const char *src = Eb + (w & kEntOffMask);
+                double a[S];
+                ldv<S>(reinterpret_cast<const double *>(Eb + (w & kEntOffMask)), a);
 #pragma unroll
-                for (int p = 0; p < NP; ++p) {
-                    double a[S];
-                    ldv<S>(reinterpret_cast<const double *>(src + p * blk_bytes), a);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[p][q] = fma(cf, a[q], acc[p][q]);
-                }
+                for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
             };
-            uint4 w = ep[32];
-            for (int s = 0; s < steps; s += 4) {
-                const uint4 wn = ep[32 * (2 + (s >> 2))];          // one block ahead (the table is padded)
-                step(w.x);
-                if (s + 1 < steps) step(w.y);
-                if (s + 2 < steps) step(w.z);
-                if (s + 3 < steps) step(w.w);
-                w = wn;
-            }
+            PYJAC_WALK(step)
             for (int o = 1; o < width; o <<= 1)
 #pragma unroll
-                for (int p = 0; p < NP; ++p)
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[p][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[p][q], o);
+                for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
             if (head) {
                 const double cst = __hiloint2double((int)r0.z, (int)r0.y);
 #pragma unroll
-                for (int p = 0; p < NP; ++p) {
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[p][q] *= cst;
-                    stv<S>(reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes) + r0.x * S, acc[p]);
-                }
+                for (int q = 0; q < S; ++q) acc[q] *= cst;
+                stv<S>(E + r0.x * S, acc);
             }
         }
     } else if (kind == kProd) {
         if (LEVEL == 2) {
-            double acc[NP][S];
+            double acc[S];
 #pragma unroll
-            for (int p = 0; p < NP; ++p)
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[p][q] = 0.0;
+            for (int q = 0; q < S; ++q) acc[q] = 0.0;
             auto step = [&](uint32_t w) {
-                const char *sa = Eb + (w & 0xFFFF) * (S * 8), *sb = Eb + (w >> 16) * (S * 8);
+                double a[S], b[S];
+                ldv<S>(reinterpret_cast<const double *>(Eb + (w & 0xFFFF) * (S * 8)), a);
+                ldv<S>(reinterpret_cast<const double *>(Eb + (w >> 16) * (S * 8)), b);
 #pragma unroll
-                for (int p = 0; p < NP; ++p) {
-                    double a[S], b[S];
-                    ldv<S>(reinterpret_cast<const double *>(sa + p * blk_bytes), a);
-                    ldv<S>(reinterpret_cast<const double *>(sb + p * blk_bytes), b);
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[p][q] = fma(a[q], b[q], acc[p][q]);
-                }
+                for (int q = 0; q < S; ++q) acc[q] = fma(a[q], b[q], acc[q]);
             };
-            uint4 w = ep[32];
-            for (int s = 0; s < steps; s += 4) {
-                const uint4 wn = ep[32 * (2 + (s >> 2))];
-                step(w.x);
-                if (s + 1 < steps) step(w.y);
-                if (s + 2 < steps) step(w.z);
-                if (s + 3 < steps) step(w.w);
-                w = wn;
-            }
+            PYJAC_WALK(step)
             for (int o = 1; o < width; o <<= 1)
 #pragma unroll
-                for (int p = 0; p < NP; ++p)
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[p][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[p][q], o);
-            if (head)
-#pragma unroll
-                for (int p = 0; p < NP; ++p)
-                    stv<S>(reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes) + r0.x * S, acc[p]);
+                for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
+            if (head) stv<S>(E + r0.x * S, acc);
         }
     } else {
         // kSum3 / kAll3: three sums at once (one for the rates / source-term kernels)
         constexpr int NA = LEVEL == 2 ? 3 : 1;
-        double acc[NP][NA][S];
+        double acc[NA][S];
 #pragma unroll
-        for (int p = 0; p < NP; ++p)
+        for (int w = 0; w < NA; ++w)
 #pragma unroll
-            for (int w = 0; w < NA; ++w)
-#pragma unroll
-                for (int q = 0; q < S; ++q) acc[p][w][q] = 0.0;
+            for (int q = 0; q < S; ++q) acc[w][q] = 0.0;
         if (kind == kSum3) {
             auto step = [&](uint32_t w_) {
                 const double cf = entry_coef(w_);
-                const char *src = Eb + (w_ & kEntOffMask);
+                const double *src = reinterpret_cast<const double *>(Eb + (w_ & kEntOffMask));
 #pragma unroll
-                for (int p = 0; p < NP; ++p)
+                for (int w = 0; w < NA; ++w) {
+                    double a[S];
+                    ldv<S>(src + w * S, a);
 #pragma unroll
-                    for (int w = 0; w < NA; ++w) {
-                        double a[S];
-                        ldv<S>(reinterpret_cast<const double *>(src + p * blk_bytes) + w * S, a);
-#pragma unroll
-                        for (int q = 0; q < S; ++q) acc[p][w][q] = fma(cf, a[q], acc[p][w][q]);
-                    }
-            };
-            uint4 w = ep[32];
-            for (int s = 0; s < steps; s += 4) {
-                const uint4 wn = ep[32 * (2 + (s >> 2))];
-                step(w.x);
-                if (s + 1 < steps) step(w.y);
-                if (s + 2 < steps) step(w.z);
-                if (s + 3 < steps) step(w.w);
-                w = wn;
-            }
-        } else {
-            for (int i = lane; i < nr; i += 32)
-#pragma unroll
-                for (int p = 0; p < NP; ++p) {
-                    const double *Ep = reinterpret_cast<const double *>(Eb + p * blk_bytes);
-                    double h[S];
-                    ldv<S>(Ep + (m.eH + i) * S, h);
-#pragma unroll
-                    for (int w = 0; w < NA; ++w) {
-                        double a[S];
-                        ldv<S>(Ep + (m.eQ + 3 * i + w) * S, a);
-#pragma unroll
-                        for (int q = 0; q < S; ++q) acc[p][w][q] = fma(h[q], a[q], acc[p][w][q]);
-                    }
+                    for (int q = 0; q < S; ++q) acc[w][q] = fma(cf, a[q], acc[w][q]);
                 }
+            };
+            PYJAC_WALK(step)
+        } else {
+            for (int i = lane; i < nr; i += 32) {
+                double h[S];
+                ldv<S>(E + (m.eH + i) * S, h);
+#pragma unroll
+                for (int w = 0; w < NA; ++w) {
+                    double a[S];
+                    ldv<S>(E + (m.eQ + 3 * i + w) * S, a);
+#pragma unroll
+                    for (int q = 0; q < S; ++q) acc[w][q] = fma(h[q], a[q], acc[w][q]);
+                }
+            }
         }
         for (int o = 1; o < width; o <<= 1)
 #pragma unroll
-            for (int p = 0; p < NP; ++p)
+            for (int w = 0; w < NA; ++w)
 #pragma unroll
-                for (int w = 0; w < NA; ++w)
-#pragma unroll
-                    for (int q = 0; q < S; ++q) acc[p][w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[p][w][q], o);
+                for (int q = 0; q < S; ++q) acc[w][q] += __shfl_xor_sync(0xFFFFFFFFu, acc[w][q], o);
         constexpr int iA = NA > 1 ? 1 : 0, iT = NA > 2 ? 2 : 0;
         if (kind == kAll3) {
-            if (lane == 0)
-#pragma unroll
-                for (int p = 0; p < NP; ++p) {
-                    double *Ep = reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes);
-                    stv<S>(Ep + m.eS1 * S, acc[p][0]);
-                    if (LEVEL == 2) { stv<S>(Ep + m.eA0 * S, acc[p][iA]); stv<S>(Ep + m.eS4 * S, acc[p][iT]); }
-                }
+            if (lane == 0) {
+                stv<S>(E + m.eS1 * S, acc[0]);
+                if (LEVEL == 2) { stv<S>(E + m.eA0 * S, acc[iA]); stv<S>(E + m.eS4 * S, acc[iT]); }
+            }
         } else if (head) {
             const uint32_t k = r0.x;
+            stv<S>(E + (m.eWdot + k) * S, acc[0]);
+            if (LEVEL == 2) {
+                // alpha'_{k+1} of Eq. 112 regrouped and the T column (Eq. 111), both without W_k
+                double ir[S], al[S], tc[S];
+                ldv<S>(sc + kIrho * S, ir);
 #pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                double *Ep = reinterpret_cast<double *>(const_cast<char *>(Eb) + p * blk_bytes);
-                stv<S>(Ep + (m.eWdot + k) * S, acc[p][0]);
-                if (LEVEL == 2) {
-                    // alpha'_{k+1} of Eq. 112 regrouped and the T column (Eq. 111), both without W_k
-                    const double *scp = reinterpret_cast<const double *>(reinterpret_cast<const char *>(sc0) + p * blk_bytes);
-                    double al[S], tc[S];
-#pragma unroll
-                    for (int q = 0; q < S; ++q) {
-                        const double ir = scp[kIrho * S + q];
-                        al[q] = ir * acc[p][iA][q];
-                        tc[q] = ir * acc[p][iT][q];
-                    }
-                    stv<S>(Ep + (m.eAlpha + k + 1) * S, al);
-                    stv<S>(Ep + (m.eTc + k + 1) * S, tc);
+                for (int q = 0; q < S; ++q) {
+                    al[q] = ir[q] * acc[iA][q];
+                    tc[q] = ir[q] * acc[iT][q];
                 }
+                stv<S>(E + (m.eAlpha + k + 1) * S, al);
+                stv<S>(E + (m.eTc + k + 1) * S, tc);
             }
         }
     }
+#undef PYJAC_WALK
 }
 
 // ---- FIX item `it`: the energy row (Eq. 113), stored by the lanes that finish it (phase B skips row 0).
 // Item 0 is J(0,0); item i >= 1 the columns 32(i-1)+1 .. (column ns is zero)
-template <int S, int NP>
-__device__ __forceinline__ void fix_item(const DeviceMech &m, const double *E0, uint32_t blk_bytes, const double *Cp0,
-                                         const double *sc0, const double *colc, const double *wrow, int it, int lane,
-                                         double *J0, int nvalid)
+template <int S>
+__device__ __forceinline__ void fix_item(const DeviceMech &m, const double *E, const double *Cp, const double *sc,
+                                         const double *colc, const double *wrow, int it, int lane, double *J0, int nq)
 {
     const int ns = m.ns, ld = m.ld;
     const long long Jstate = (long long)ld * ld;
+    if (it == 0) {
+        double s3[S];       // sum_k c_pk W_k wdot_k
 #pragma unroll
-    for (int p = 0; p < NP; ++p) {
-        const double *E = reinterpret_cast<const double *>(reinterpret_cast<const char *>(E0) + p * blk_bytes);
-        const double *Cp = reinterpret_cast<const double *>(reinterpret_cast<const char *>(Cp0) + p * blk_bytes);
-        const double *sc = reinterpret_cast<const double *>(reinterpret_cast<const char *>(sc0) + p * blk_bytes);
-        double *Jp = J0 + (long long)p * S * Jstate;
-        const int nq = nvalid - p * S;
-        if (it == 0) {
-            double s3[S];       // sum_k c_pk W_k wdot_k
+        for (int q = 0; q < S; ++q) s3[q] = 0.0;
+        for (int k = lane; k < ns; k += 32) {
+            const double wk = wrow[k + 1];
+            double cp[S], wd[S];
+            ldv<S>(Cp + k * S, cp);
+            ldv<S>(E + (m.eWdot + k) * S, wd);
 #pragma unroll
-            for (int q = 0; q < S; ++q) s3[q] = 0.0;
-            for (int k = lane; k < ns; k += 32) {
-                const double wk = wrow[k + 1];
-                double cp[S], wd[S];
-                ldv<S>(Cp + k * S, cp);
-                ldv<S>(E + (m.eWdot + k) * S, wd);
-#pragma unroll
-                for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1)
-#pragma unroll
-                for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
-            if (lane < S) {
-                const int q = lane;
-                double s = s3[0];
-#pragma unroll
-                for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
-                const double icp = sc[kIcp * S + q];
-                const double z = -icp * sc[kIrho * S + q] *
-                                 (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
-                if (q < nq) Jp[q * Jstate] = z;
-            }
-            continue;
+            for (int q = 0; q < S; ++q) s3[q] = fma(cp[q] * wk, wd[q], s3[q]);
         }
-        const int c = (it - 1) * 32 + lane + 1;
-        if (c < ns) {
-            const double uc = colc[4 * c], wj = colc[4 * c + 1], iwj = colc[4 * c + 2], iwl = m.inv_mw[ns - 1];
-            double icp[S], irho[S], s1[S], a0[S], gl[S], cpj[S], cpl[S], g0[S];
-            ldv<S>(sc + kIcp * S, icp);
-            ldv<S>(sc + kIrho * S, irho);
-            ldv<S>(E + m.eS1 * S, s1);
-            ldv<S>(E + m.eA0 * S, a0);
-            ldv<S>(E + (m.eG0 + ns - 1) * S, gl);
-            ldv<S>(Cp + (c - 1) * S, cpj);
-            ldv<S>(Cp + (ns - 1) * S, cpl);
-            ldv<S>(E + (m.eG0 + c - 1) * S, g0);
 #pragma unroll
-            for (int q = 0; q < S; ++q) {
-                const double a1 = irho[q] * s1[q] * icp[q] * icp[q];     // coefficient of c_pj - c_pNs
-                const double alpha0 = -(irho[q] * icp[q]) * a0[q];
-                const double gamma0 = -(iwl * icp[q]) * gl[q];
-                const double z = (alpha0 * uc + wj * (a1 * (cpj[q] - cpl[q]) - gamma0) - icp[q] * g0[q]) * iwj;
-                if (q < nq) Jp[q * Jstate + (long long)c * ld] = z;
-            }
-        } else if (c == ns) {
+        for (int o = 16; o > 0; o >>= 1)
 #pragma unroll
-            for (int q = 0; q < S; ++q)
-                if (q < nq) Jp[q * Jstate + (long long)c * ld] = 0.0;
+            for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
+        if (lane < S) {
+            const int q = lane;
+            double s = s3[0];
+#pragma unroll
+            for (int u = 1; u < S; ++u) s = q == u ? s3[u] : s;
+            const double icp = sc[kIcp * S + q];
+            const double z = -icp * sc[kIrho * S + q] *
+                             (s - sc[kDcpDT * S + q] * icp * E[m.eS1 * S + q] + E[m.eS4 * S + q]);
+            if (q < nq) J0[q * Jstate] = z;
         }
+        return;
+    }
+    const int c = (it - 1) * 32 + lane + 1;
+    if (c < ns) {
+        const double uc = colc[4 * c], wj = colc[4 * c + 1], iwj = colc[4 * c + 2], iwl = m.inv_mw[ns - 1];
+        double icp[S], irho[S], s1[S], a0[S], gl[S], cpj[S], cpl[S], g0[S];
+        ldv<S>(sc + kIcp * S, icp);
+        ldv<S>(sc + kIrho * S, irho);
+        ldv<S>(E + m.eS1 * S, s1);
+        ldv<S>(E + m.eA0 * S, a0);
+        ldv<S>(E + (m.eG0 + ns - 1) * S, gl);
+        ldv<S>(Cp + (c - 1) * S, cpj);
+        ldv<S>(Cp + (ns - 1) * S, cpl);
+        ldv<S>(E + (m.eG0 + c - 1) * S, g0);
+#pragma unroll
+        for (int q = 0; q < S; ++q) {
+            const double a1 = irho[q] * s1[q] * icp[q] * icp[q];     // coefficient of c_pj - c_pNs
+            const double alpha0 = -(irho[q] * icp[q]) * a0[q];
+            const double gamma0 = -(iwl * icp[q]) * gl[q];
+            const double z = (alpha0 * uc + wj * (a1 * (cpj[q] - cpl[q]) - gamma0) - icp[q] * g0[q]) * iwj;
+            if (q < nq) J0[q * Jstate + (long long)c * ld] = z;
+        }
+    } else if (c == ns) {
+#pragma unroll
+        for (int q = 0; q < S; ++q)
+            if (q < nq) J0[q * Jstate + (long long)c * ld] = 0.0;
     }
 }
 
 // ---- phase B: the items [it0, it1) of one warp (one item = one Jacobian column for one slab of rows).
 // J(r, c) = W_r / W_j (sum of the cell's entries + alpha'_r u_c - gamma'_r v_c)  (Eq. 112 regrouped), RP rows
-// per lane; alpha', gamma' and W_r stay in registers while the slab does not change, the entries of a
-// cell are decoded once for the NP blocks.  Headers are read two items ahead, entries one item ahead.
-template <int S, int NP, int RP>
-__device__ __forceinline__ void b_run(const DeviceMech &m, const double *E0, uint32_t blk_bytes, const double *colc,
-                                      const double *wrow, int it0, int it1, int lane, double *J0, int nvalid,
-                                      bool aligned16)
+// per lane; alpha', gamma' and W_r stay in registers while the slab does not change.  A cell has three
+// entry words (padded with the zero slot) and the item's step count; the entries of the next item are
+// fetched while this one is summed.  FAST: all S states are stored and the output is 16-byte aligned.
+template <int S, int RP, bool FAST>
+__device__ __forceinline__ void b_run(const DeviceMech &m, const double *E, const double *colc, const double *wrow,
+                                      int it0, int it1, int lane, double *J0, int nvalid, bool aligned16)
 {
-    if (it0 >= it1) return;
     const int ld = m.ld;
-    const uint32_t j_state = (uint32_t)(ld * ld) * 8u;
-    const char *Eb = reinterpret_cast<const char *>(E0);
-    int slab = it0 / ld, c = it0 - slab * ld;
-    int cur = -1, r = 0;
-    bool rowok = false;
-    double al[NP][RP * S], ga[NP][RP * S], wr[RP];
-    uint2 h = m.bitem[it0], h1 = m.bitem[it0 + 1];
-    uint4 wA = m.b_ent[h.x + lane], wB = make_uint4(0u, 0u, 0u, 0u);
-    if (RP == 2) wB = m.b_ent[h.x + 32 + lane];
-    for (int it = it0; it < it1; ++it) {
-        const uint2 h2 = m.bitem[it + 2];
-        const uint4 wAn = m.b_ent[h1.x + lane];
-        uint4 wBn = make_uint4(0u, 0u, 0u, 0u);
-        if (RP == 2) wBn = m.b_ent[h1.x + 32 + lane];
-        if (slab != cur) {
-            cur = slab;
-            r = RP * (32 * slab + lane);
-            rowok = r < ld;
-            const int rr = rowok ? r : 0;
+    const uint32_t j_state = (uint32_t)(ld * ld);
+    const char *Eb = reinterpret_cast<const char *>(E);
+    const uint4 *ebase = m.b_ent + lane;
+    int it = it0;
+    while (it < it1) {
+        const int slab = it / ld, c0 = it - slab * ld;
+        const int c1 = min(ld, c0 + (it1 - it));
+        const int r = RP * (32 * slab + lane);
+        const bool rowok = r < ld;
+        const int rr = rowok ? r : 0;
+        double al[RP * S], ga[RP * S], wr[RP];
+        ldv<RP * S>(E + (m.eAlpha + rr) * S, al);
+        ldv<RP * S>(E + (m.eGamma + rr) * S, ga);
 #pragma unroll
-            for (int p = 0; p < NP; ++p) {
-                const double *Ep = reinterpret_cast<const double *>(Eb + p * blk_bytes);
-                ldv<RP * S>(Ep + (m.eAlpha + rr) * S, al[p]);
-                ldv<RP * S>(Ep + (m.eGamma + rr) * S, ga[p]);
-            }
+        for (int hh = 0; hh < RP; ++hh) wr[hh] = wrow[rr + hh];
+        const uint4 *ep = ebase + (size_t)it * (32 * RP);
+        const double *cc = colc + 4 * c0;
+        uint32_t off = (uint32_t)(c0 * ld + r);                  // element (r, c) of the batch's first state
+        uint4 wA = ep[0], wB = wA;
+        if (RP == 2) wB = ep[32];
+        for (int c = c0; c < c1; ++c, cc += 4, off += (uint32_t)ld) {
+            ep += 32 * RP;
+            const uint4 wAn = ep[0];                              // the table is padded by one item
+            uint4 wBn = wAn;
+            if (RP == 2) wBn = ep[32];
+            const double2 uv = *reinterpret_cast<const double2 *>(cc);
+            const double iw = cc[2];
+            double acc[RP * S];
 #pragma unroll
-            for (int hh = 0; hh < RP; ++hh) wr[hh] = wrow[rr + hh];
-        }
-        const double2 uv = *reinterpret_cast<const double2 *>(colc + 4 * c);
-        const double iw = colc[4 * c + 2];
-        const int nA = (int)(h.y & 0xFF), nB = (int)(h.y >> 8) & 0xFF;
-        double acc[NP][RP * S];
-#pragma unroll
-        for (int p = 0; p < NP; ++p)
-#pragma unroll
-            for (int e = 0; e < RP * S; ++e) acc[p][e] = fma(-ga[p][e], uv.y, al[p][e] * uv.x);
-        auto step = [&](uint32_t w, int hh) {
-            const double cf = entry_coef(w);
-            const char *src = Eb + (w & kEntOffMask);
-#pragma unroll
-            for (int p = 0; p < NP; ++p) {
+            for (int e = 0; e < RP * S; ++e) acc[e] = fma(-ga[e], uv.y, al[e] * uv.x);
+            auto step = [&](uint32_t w, int hh) {
+                const double cf = entry_coef(w);
                 double a[S];
-                ldv<S>(reinterpret_cast<const double *>(src + p * blk_bytes), a);
+                ldv<S>(reinterpret_cast<const double *>(Eb + (w & kEntOffMask)), a);
 #pragma unroll
-                for (int q = 0; q < S; ++q) acc[p][hh * S + q] = fma(cf, a[q], acc[p][hh * S + q]);
+                for (int q = 0; q < S; ++q) acc[hh * S + q] = fma(cf, a[q], acc[hh * S + q]);
+            };
+            if (wA.w != 0u) {
+                step(wA.x, 0);
+                if (wA.w > 1u) { step(wA.y, 0); step(wA.z, 0); }
             }
-        };
-        if (nA > 0) {
-            step(wA.x, 0);
-            if (nA > 1) {
-                step(wA.y, 0);
-                if (nA > 2) {
-                    step(wA.z, 0);
-                    if (nA > 3) step(wA.w, 0);
-                }
+            if (RP == 2 && wB.w != 0u) {
+                step(wB.x, RP - 1);
+                if (wB.w > 1u) { step(wB.y, RP - 1); step(wB.z, RP - 1); }
             }
-        }
-        if (RP == 2 && nB > 0) {
-            step(wB.x, RP - 1);
-            if (nB > 1) {
-                step(wB.y, RP - 1);
-                if (nB > 2) {
-                    step(wB.z, RP - 1);
-                    if (nB > 3) step(wB.w, RP - 1);
-                }
-            }
-        }
-        if (rowok) {
-            char *Jp = reinterpret_cast<char *>(J0 + (long long)c * ld + r);
             double f[RP];
 #pragma unroll
             for (int hh = 0; hh < RP; ++hh) f[hh] = wr[hh] * iw;
+            if (FAST) {
+                if (rowok) {
 #pragma unroll
-            for (int p = 0; p < NP; ++p)
+                    for (int q = 0; q < S; ++q) {
+                        double *dst = J0 + (off + (uint32_t)q * j_state);
+                        if (RP == 2) {
+                            const double v0 = acc[q] * f[0], v1 = acc[S + q] * f[RP - 1];
+                            if (r != 0) st_cs_v2(dst, v0, v1);
+                            else __stcs(dst + 1, v1);
+                        } else {
+                            if (r != 0) __stcs(dst, acc[q] * f[0]);
+                        }
+                    }
+                }
+            } else if (rowok) {
 #pragma unroll
                 for (int q = 0; q < S; ++q) {
-                    if (p * S + q >= nvalid) continue;
-                    double *dst = reinterpret_cast<double *>(Jp + (uint32_t)(p * S + q) * j_state);
+                    if (q >= nvalid) continue;
+                    double *dst = J0 + (off + (uint32_t)q * j_state);
                     if (RP == 2) {
-                        const double v0 = acc[p][q] * f[0], v1 = acc[p][S + q] * f[RP - 1];
+                        const double v0 = acc[q] * f[0], v1 = acc[S + q] * f[RP - 1];
                         if (r != 0 && aligned16) st_cs_v2(dst, v0, v1);
                         else {
                             if (r != 0) __stcs(dst, v0);
                             __stcs(dst + 1, v1);
                         }
                     } else {
-                        if (r != 0) __stcs(dst, acc[p][q] * f[0]);
+                        if (r != 0) __stcs(dst, acc[q] * f[0]);
                     }
                 }
+            }
+            wA = wAn; wB = wBn;
         }
-        h = h1; h1 = h2; wA = wAn; wB = wBn;
-        if (++c == ld) { c = 0; ++slab; }
+        it += c1 - c0;
     }
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------
-// Shared memory: NP blocks of S interleaved states, sp.total doubles per state (E, two mixture parts),
-// then the state-independent column and row constants.
-template <int LEVEL, int S, int NP>
+// Shared memory: S interleaved states of sp.total doubles each (E, two mixture parts), then the
+// state-independent column and row constants.
+template <int LEVEL, int S>
 __global__ void __launch_bounds__(kMaxThreads, 1)
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
                 const double *__restrict__ Pg, const double *__restrict__ Yg, long long ldy, const EvalOut out)
@@ -895,157 +834,142 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
     __shared__ int ctr[2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int NT = blockDim.x, NW = NT >> 5;
-    constexpr int SP = S >= 2 ? 2 : 1;
-    constexpr int NS = S * NP;                           // states per CTA iteration
+    constexpr int SP = S % 2 == 0 ? 2 : 1;
     const int ns = m.ns, ld = m.ld, nr = m.nr;
-    const int blkd = sp.total * S;                       // doubles per block
-    const uint32_t blk_bytes = (uint32_t)blkd * 8u;
-    double *E0 = sm + sp.E * S;
-    const double *colc = sm + (size_t)NP * blkd + sp.colc;
-    double *wrow = sm + (size_t)NP * blkd + sp.wrow;
+    double *E = sm + sp.E * S;
+    const double *colc = sm + (size_t)sp.total * S + sp.colc;
+    double *wrow = sm + (size_t)sp.total * S + sp.wrow;
     {
-        double *cw = sm + (size_t)NP * blkd + sp.colc;
+        double *cw = sm + (size_t)sp.total * S + sp.colc;
         for (int i = tid; i < 4 * ld; i += NT) cw[i] = m.colc[i];
         for (int i = tid; i < ld; i += NT) wrow[i] = m.wrow[i];
         // E starts as zeros: sums without a list, the zero slots and row 0 of alpha' / gamma' stay zero
-        for (int p = 0; p < NP; ++p)
-            for (int i = tid; i < m.n_e * S; i += NT) E0[(size_t)p * blkd + i] = 0.0;
+        for (int i = tid; i < m.n_e * S; i += NT) E[i] = 0.0;
     }
-    if (tid < S)       // the empty-slot dummy species of both mixture parts
-        for (int p = 0; p < NP; ++p) {
-            sm[(size_t)p * blkd + (sp.P0 + sp.oX + ns) * S + tid] = 1.0;
-            sm[(size_t)p * blkd + (sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
-        }
+    if (tid < S) {     // the empty-slot dummy species of both mixture parts
+        sm[(sp.P0 + sp.oX + ns) * S + tid] = 1.0;
+        sm[(sp.P0 + sp.p0size + sp.oX + ns) * S + tid] = 1.0;
+    }
     if (tid == 0) ctr[0] = 0;
-    const long long nbatch = (n + NS - 1) / NS;
+    const long long nbatch = (n + S - 1) / S;
     // work items of P1: the general groups one state at a time (most expensive first), then the plain
-    // groups SP states at a time; each for every block
+    // groups SP states at a time
     const int n_gen = m.n_rchunk - m.n_plain;
     const int split_l = m.n_pd & 31, split_c = (m.split_general && split_l != 0 && (m.n_pd >> 5) < n_gen) ? (m.n_pd >> 5) : -1;
     const int n_genq = n_gen + (split_c >= 0 ? 1 : 0);
-    const int n_plq = m.n_plain * (S / SP);
-    const int i_plain = n_genq * S * NP, n_p1 = i_plain + n_plq * NP;
+    const int i_plain = n_genq * S, n_p1 = i_plain + m.n_plain * (S / SP);
+    const int arows = LEVEL == 2 ? m.n_arow : m.n_arow01;
+    const int it0 = m.bsplit[warp], it1 = m.bsplit[warp + 1];
+    const int nfix = 1 + (ns + 31) / 32;
+    const bool aligned16 = (reinterpret_cast<uintptr_t>(out.jac) & 15) == 0;
     int par = 0;
-    if ((long long)blockIdx.x < nbatch)
-        for (int it = warp; it < NS; it += NW) {
-            const int p = it / S, q = it - p * S;
-            double *P0 = sm + (size_t)p * blkd + sp.P0 * S;
-            mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oScal * S, q,
-                                          min((long long)blockIdx.x * NS + it, n - 1), Tg, Pg, Yg, ldy, lane);
-        }
+    if ((long long)blockIdx.x < nbatch && warp < S) {
+        double *P0 = sm + sp.P0 * S;
+        mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oScal * S, warp,
+                                      min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
+    }
     __syncthreads();
     for (long long b = blockIdx.x; b < nbatch; b += gridDim.x, par ^= 1) {
-        const long long state0 = b * NS;
-        double *P0 = sm + (sp.P0 + par * sp.p0size) * S;             // block 0's mixture part of this iteration
-        const double *sc0 = P0 + sp.oScal * S;
+        const long long state0 = b * S;
+        double *P0 = sm + (sp.P0 + par * sp.p0size) * S;
+        const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S;
         // ---- P1: reactions
         for (int it = grab(&ctr[0], lane); it < n_p1; it = grab(&ctr[0], lane)) {
             if (it < i_plain) {
                 // general groups, one state at a time; the group that holds both pressure-dependent and
                 // other reactions is two items (each runs only its own code paths)
-                const int p = it % NP, j = it / NP;
-                const int gi = j / S, q = j - gi * S;
+                const int gi = it / S, q = it - gi * S;
                 const int c = gi < n_gen ? gi : split_c;
                 int sl = lane;              // lanes of the other part repeat this part's first reaction
                 if (c == split_c) sl = gi < n_gen ? (lane < split_l ? lane : 0) : (lane >= split_l ? lane : split_l);
-                const double *Pp = P0 + (size_t)p * blkd;
-                reaction<LEVEL, S>(m, sp, E0 + (size_t)p * blkd, Pp + sp.oX * S, Pp + sp.oScal * S,
-                                   min(c * 32 + sl, nr - 1), q, out, state0 + p * S, n);
+                reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + sl, nr - 1), q, out, state0, n);
             } else {
-                const int i2 = it - i_plain;
-                const int p = i2 % NP, j = i2 / NP;
+                const int j = it - i_plain;
                 const int c = n_gen + j / (S / SP), q0 = (j % (S / SP)) * SP;
-                const double *Pp = P0 + (size_t)p * blkd;
-                plain_reactions<LEVEL, S>(m, sp, E0 + (size_t)p * blkd, Pp + sp.oX * S, Pp + sp.oScal * S,
-                                          min(c * 32 + lane, nr - 1), q0, out, state0 + p * S, n);
+                plain_reactions<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q0, out, state0, n);
             }
         }
         __syncthreads();
         if (tid == 0) ctr[0] = 0;
         // ---- A: sums over the reactions per species / per column, pieces of the long cell lists
         {
-            const int rows = LEVEL == 2 ? m.n_arow : m.n_arow01;
             const uint2 *hp = m.achunk + warp;
-            uint2 h = hp[0];
-            for (int row = 0; row < rows; ++row) {
-                const uint2 hn = hp[(size_t)(row + 1 < rows ? row + 1 : row) * NW];
-                a_chunk<LEVEL, S, NP>(m, E0, blk_bytes, sc0, h, lane);
+            uint2 h = *hp;
+            for (int row = 0; row < arows; ++row) {
+                hp += NW;
+                const uint2 hn = *hp;                 // the header table is padded by one row
+                a_chunk<LEVEL, S>(m, E, sc, h, lane);
                 h = hn;
             }
         }
         __syncthreads();
-        const int nvalid = (int)min((long long)NS, n - state0);
+        const int nvalid = (int)min((long long)S, n - state0);
         if (LEVEL == 2) {
             // ---- B: the Jacobian column by column, the energy row
             double *J0 = out.jac + state0 * ((long long)ld * ld);
-            const bool aligned16 = (reinterpret_cast<uintptr_t>(out.jac) & 15) == 0;
-            const int it0 = m.bsplit[warp], it1 = m.bsplit[warp + 1];
-            if (m.rp == 2) b_run<S, NP, 2>(m, E0, blk_bytes, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
-            else b_run<S, NP, 1>(m, E0, blk_bytes, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
-            const int nfix = 1 + (ns + 31) / 32;
+            if (nvalid == S && aligned16) {
+                if (m.rp == 2) b_run<S, 2, true>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, true);
+                else b_run<S, 1, true>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, true);
+            } else {
+                if (m.rp == 2) b_run<S, 2, false>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
+                else b_run<S, 1, false>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
+            }
             for (int it = NW - 1 - warp; it < nfix; it += NW)
-                fix_item<S, NP>(m, E0, blk_bytes, P0 + sp.oCp * S, sc0, colc, wrow, it, lane, J0, nvalid);
+                fix_item<S>(m, E, P0 + sp.oCp * S, sc, colc, wrow, it, lane, J0, nvalid);
         }
         // ---- outputs of the rates / source-term kernels (Eqs. 7-8, 14)
         if (LEVEL == 0 && out.wdot) {
-            for (int i = tid; i < ns * NP; i += NT) {
-                const int p = i / ns, k = i - p * ns;
+            for (int k = tid; k < ns; k += NT)
 #pragma unroll
                 for (int q = 0; q < S; ++q)
-                    if (p * S + q < nvalid) out.wdot[(state0 + p * S + q) * ns + k] = E0[(size_t)p * blkd + (m.eWdot + k) * S + q];
-            }
+                    if (q < nvalid) out.wdot[(state0 + q) * ns + k] = E[(m.eWdot + k) * S + q];
         }
         if (LEVEL == 1) {
-            for (int i = tid; i < ld * NP; i += NT) {
-                const int p = i / ld, r = i - p * ld;
-                const double *E = E0 + (size_t)p * blkd, *sc = sc0 + (size_t)p * blkd;
+            for (int r = tid; r < ld; r += NT)
 #pragma unroll
                 for (int q = 0; q < S; ++q) {
-                    if (p * S + q >= nvalid) continue;
+                    if (q >= nvalid) continue;
                     const double irho = sc[kIrho * S + q];
                     const double v = r == 0 ? -E[m.eS1 * S + q] * irho / sc[kCpMix * S + q]
                                             : wrow[r] * E[(m.eWdot + r - 1) * S + q] * irho;
-                    out.dydt[(state0 + p * S + q) * ld + r] = v;
+                    out.dydt[(state0 + q) * ld + r] = v;
                 }
-            }
         }
-        // ---- P0 of the next iteration into the other mixture part
-        if (b + gridDim.x < nbatch)
-            for (int it = warp; it < NS; it += NW) {
-                const int p = it / S, q = it - p * S;
-                double *Pn = sm + (size_t)p * blkd + (sp.P0 + (par ^ 1) * sp.p0size) * S;
-                mixture_and_species<LEVEL, S>(m, Pn + sp.oX * S, Pn + sp.oCp * S, Pn + sp.oScal * S, q,
-                                              min((b + gridDim.x) * NS + it, n - 1), Tg, Pg, Yg, ldy, lane);
-            }
+        // ---- P0 of the next iteration into the other mixture part, by the last warps
+        if (b + gridDim.x < nbatch && warp >= NW - S) {
+            const int q = warp - (NW - S);
+            double *Pn = sm + (sp.P0 + (par ^ 1) * sp.p0size) * S;
+            mixture_and_species<LEVEL, S>(m, Pn + sp.oX * S, Pn + sp.oCp * S, Pn + sp.oScal * S, q,
+                                          min((b + gridDim.x) * S + q, n - 1), Tg, Pg, Yg, ldy, lane);
+        }
         __syncthreads();
     }
 }
 
 }  // namespace
 
-// This file is compiled once per (S, NP): -DPYJAC_S=<states per block> -DPYJAC_NP=<blocks per CTA
-// iteration> (build.py); dispatch.cu switches over them.
-#if !defined(PYJAC_S) || !defined(PYJAC_NP)
-#error "compile with -DPYJAC_S=<1|2> -DPYJAC_NP=<1..4>"
+// This file is compiled once per S (states a CTA interleaves): -DPYJAC_S=<1|2|3|4|6> (build.py);
+// dispatch.cu switches over them.
+#if !defined(PYJAC_S)
+#error "compile with -DPYJAC_S=<1|2|3|4|6>"
 #endif
-#define PYJAC_CAT3(a, b, c, d) a##b##c##d
-#define PYJAC_NAME(a, s, np) PYJAC_CAT3(a, s, _, np)
+#define PYJAC_CAT2(a, b) a##b
+#define PYJAC_NAME(a, s) PYJAC_CAT2(a, s)
 
-const void *PYJAC_NAME(eval_kernel_ptr_, PYJAC_S, PYJAC_NP)(int level)
+const void *PYJAC_NAME(eval_kernel_ptr_, PYJAC_S)(int level)
 {
-    return level == 0 ? (const void *)eval_kernel<0, PYJAC_S, PYJAC_NP>
-         : level == 1 ? (const void *)eval_kernel<1, PYJAC_S, PYJAC_NP>
-                      : (const void *)eval_kernel<2, PYJAC_S, PYJAC_NP>;
+    return level == 0 ? (const void *)eval_kernel<0, PYJAC_S>
+         : level == 1 ? (const void *)eval_kernel<1, PYJAC_S>
+                      : (const void *)eval_kernel<2, PYJAC_S>;
 }
 
-cudaError_t PYJAC_NAME(launch_eval_, PYJAC_S, PYJAC_NP)(int level, int threads, const DeviceMech &m, const SmemPlan &sp,
-                                                         int grid, size_t smem, long long n, const double *T,
-                                                         const double *P, const double *Y, long long ldy,
-                                                         const EvalOut &out, cudaStream_t stream)
+cudaError_t PYJAC_NAME(launch_eval_, PYJAC_S)(int level, int threads, const DeviceMech &m, const SmemPlan &sp, int grid,
+                                               size_t smem, long long n, const double *T, const double *P,
+                                               const double *Y, long long ldy, const EvalOut &out, cudaStream_t stream)
 {
-    if (level == 0) eval_kernel<0, PYJAC_S, PYJAC_NP><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
-    else if (level == 1) eval_kernel<1, PYJAC_S, PYJAC_NP><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
-    else eval_kernel<2, PYJAC_S, PYJAC_NP><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+    if (level == 0) eval_kernel<0, PYJAC_S><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+    else if (level == 1) eval_kernel<1, PYJAC_S><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+    else eval_kernel<2, PYJAC_S><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
     return cudaGetLastError();
 }
 

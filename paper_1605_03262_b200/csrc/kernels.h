@@ -14,12 +14,12 @@ struct EvalOut {
     double *jac;                     // level 2
 };
 
-// level: 0 rates, 1 source term, 2 Jacobian.  S: states per block (1, 2); NP: blocks a CTA evaluates per
-// iteration (1 .. kMaxNP); threads: a multiple of 32 up to kMaxThreads.
-const void *eval_kernel_ptr(int level, int S, int NP);
-size_t eval_smem_bytes(const SmemPlan &sp, int S, int NP);
-cudaError_t launch_eval(int level, int threads, int S, int NP, const DeviceMech &m, const SmemPlan &sp, int grid,
-                        size_t smem, long long n, const double *T, const double *P, const double *Y, long long ldy,
+// level: 0 rates, 1 source term, 2 Jacobian.  S: states a CTA interleaves per iteration (1, 2, 3, 4, 6);
+// threads: a multiple of 32, at least 32 S, up to kMaxThreads.
+const void *eval_kernel_ptr(int level, int S);
+size_t eval_smem_bytes(const SmemPlan &sp, int S);
+cudaError_t launch_eval(int level, int threads, int S, const DeviceMech &m, const SmemPlan &sp, int grid, size_t smem,
+                        long long n, const double *T, const double *P, const double *Y, long long ldy,
                         const EvalOut &out, cudaStream_t stream);
 
 // peak probes (dispatch.cu): a write-only stream of 16-byte streaming stores; 8 independent DFMA chains

@@ -527,7 +527,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
 
     // ---- long cell lists are summed piecewise in phase A (balanced over the lanes: lists sorted by
     // length); phase B then reads at most `cell_cap` entries per cell, all lanes of a warp alike
-    const int cell_cap = hints.cell_cap >= 1 && hints.cell_cap <= 4 ? hints.cell_cap : 3;
+    const int cell_cap = hints.cell_cap >= 1 && hints.cell_cap <= 3 ? hints.cell_cap : 3;
     constexpr int kPiece = 8;
     std::vector<std::vector<std::pair<uint32_t, int>>> cell_w((size_t)ld * ld);
     {
@@ -558,44 +558,41 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         if (o.n_e > 65535) throw Fail{PYJAC_ELIMIT, "more than 65535 per-state table entries"};
     }
 
-    // ---- launch shape: NP blocks of S states per CTA iteration, threads per CTA, CTAs per SM.
-    // Everything lives in shared memory: NP x S x (E + two mixture parts) + the column / row constants.
+    // ---- launch shape: S states per CTA iteration, threads per CTA, CTAs per SM.  Everything lives in
+    // shared memory: S x (E + two mixture parts) + the column / row constants.  S = 6 (48-byte elements)
+    // and S = 2 (16-byte elements) let the 16-byte loads of a quarter warp fall into eight different bank
+    // groups; S = 4 cannot (its elements cover only every other bank group), S = 3 uses 8-byte loads.
     {
         const long long sm_bytes = 228 * 1024;                       // shared memory of one sm_100 SM
         const SmemPlan pl = make_smem_plan(ns, o.n_e);
-        auto bytes_for = [&](int S, int NP) { return ((long long)S * NP * pl.total + pl.shared_total) * 8; };
+        auto bytes_for = [&](int S) { return ((long long)S * pl.total + pl.shared_total) * 8; };
         // each resident CTA also takes a 1 KB system reserve and the kernel's few static bytes
         auto limit_for = [&](int ctas) { return std::min<long long>(sm_bytes / ctas - 1024 - 128, hints.smem_bytes); };
-        int S = hints.S > 0 ? hints.S : (bytes_for(2, 1) <= limit_for(1) ? 2 : 1);
-        if (S != 1 && S != 2) throw Fail{PYJAC_EINVAL, "states per block must be 1 or 2"};
-        if (bytes_for(S, 1) > limit_for(1)) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
-        int ctas = hints.ctas > 0 ? hints.ctas : 0, NP = hints.NP > 0 ? hints.NP : 0;
-        if (NP > kMaxNP) throw Fail{PYJAC_EINVAL, "more blocks per CTA than the kernels are compiled for"};
-        if (ctas == 0 && NP == 0) {
-            // default: as many states in flight per SM as fit, in the fewest CTAs (tables are read once per CTA
-            // iteration and amortised over its NP blocks)
-            const long long per_block = (long long)S * pl.total * 8;
-            const int fit = (int)std::max<long long>(1, (limit_for(1) - pl.shared_total * 8) / per_block);
-            if (fit <= kMaxNP) { NP = fit; ctas = 1; }
-            else {
-                NP = kMaxNP;
-                ctas = 1;
-                while (ctas < 4 && bytes_for(S, NP) <= limit_for(ctas + 1)) ++ctas;
+        int S = hints.S, ctas = hints.ctas;
+        if (S == 0) {
+            if (ctas > 0) {
+                for (int cand : {6, 4, 3, 2, 1})
+                    if (S == 0 && bytes_for(cand) <= limit_for(ctas)) S = cand;
+            } else {
+                for (int cand : {6, 2, 1})
+                    if (S == 0 && bytes_for(cand) <= limit_for(1)) S = cand;
             }
-        } else if (NP == 0) {
-            NP = 1;
-            while (NP < kMaxNP && bytes_for(S, NP + 1) <= limit_for(ctas)) ++NP;
-        } else if (ctas == 0) {
-            ctas = 1;
-            while (ctas < 4 && bytes_for(S, NP) <= limit_for(ctas + 1)) ++ctas;
+            if (S == 0) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
         }
-        if (bytes_for(S, NP) > limit_for(ctas)) throw Fail{PYJAC_ELIMIT, "the requested launch shape exceeds shared memory"};
+        if (S != 1 && S != 2 && S != 3 && S != 4 && S != 6) throw Fail{PYJAC_EINVAL, "states per CTA iteration must be 1, 2, 3, 4 or 6"};
+        if (bytes_for(S) > limit_for(1)) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
+        if (ctas == 0) {
+            ctas = 1;
+            while (ctas < 4 && bytes_for(S) <= limit_for(ctas + 1)) ++ctas;
+        }
+        if (bytes_for(S) > limit_for(ctas)) throw Fail{PYJAC_ELIMIT, "the requested launch shape exceeds shared memory"};
         int threads = hints.threads > 0 ? hints.threads : (kMaxThreads / ctas) & ~31;
+        if (threads < 32 * S) threads = 32 * S;
         if (threads < 64) threads = 64;
         if (threads > kMaxThreads || threads % 32) throw Fail{PYJAC_EINVAL, "threads per CTA must be a multiple of 32 up to 512"};
-        o.S = S; o.NP = NP; o.threads = threads; o.ctas_target = ctas;
+        o.S = S; o.threads = threads; o.ctas_target = ctas;
         if ((long long)o.n_e * S * 8 > (long long)kEntOffMask + 1)
-            throw Fail{PYJAC_ELIMIT, "per-block tables exceed the 256 KB offset range of a gather entry"};
+            throw Fail{PYJAC_ELIMIT, "per-CTA tables exceed the 256 KB offset range of a gather entry"};
     }
     const int S = o.S, NW = o.threads / 32;
     o.rp = (hints.rp == 1 || hints.rp == 2) ? hints.rp : (ld % 2 == 0 ? 2 : 1);
@@ -607,7 +604,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     // entries, and which zero slot a padding entry reads, is free: both are chosen greedily so that the
     // lanes of one shared-memory wavefront hit different bank groups at every step.
     auto enc = [&](const std::pair<uint32_t, int> &e) { return coef_hi14(e.second) | (uint32_t)(e.first * S * 8); };
-    const int gsz = std::min(8 * S, 16), LP = 128 / gsz, nq = 32 / LP;     // bytes per lane access, lanes per wavefront
+    const int gsz = S % 2 == 0 ? 16 : 8, LP = 128 / gsz, nq = 32 / LP;     // bytes per lane access, lanes per wavefront
     // lists[slot] sits on lanes [slot * width, (slot + 1) * width); returns grid[lane * steps + step]
     auto place = [&](const std::vector<std::vector<uint32_t>> &lists, int width, int steps, uint32_t kind) {
         const int nstream = kind == kProd ? 2 : 1;
@@ -773,45 +770,42 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             o.n_a_steps += c.steps;
         }
         o.a_ent.resize(o.a_ent.size() + 128, 0u);        // the kernels read one block past a chunk's last
+        o.achunk.resize(o.achunk.size() + (size_t)2 * NW, 0u);      // ... and the headers one row ahead
     }
 
-    // ---- phase B items: one per (slab, column); a lane's cells are rows rp * (32 slab + lane) .. + rp - 1
+    // ---- phase B items: one per (slab, column); a lane's cells are rows rp * (32 slab + lane) .. + rp - 1.
+    // Every cell has three entry words (padded with a zero slot); the fourth word of every lane is the
+    // step count of the item's cells h: 0 (no lane has an entry), 1 (one step), 2 (three steps).
     {
-        o.bitem.assign((size_t)2 * (o.n_slab * ld + 2), 0u);     // headers are read two items ahead
-        o.b_ent.assign(128, 0u);                                  // block 0: what empty items point at
-        std::vector<double> cost((size_t)o.n_slab * ld, 0.0);
+        const size_t n_item = (size_t)o.n_slab * ld;
+        o.b_ent.assign((n_item + 1) * rp * 128, (uint32_t)(eZero * S * 8));     // one item of padding: read ahead
+        std::vector<double> cost(n_item, 0.0);
         for (int slab = 0; slab < o.n_slab; ++slab)
             for (int c = 0; c < ld; ++c) {
                 const size_t it = (size_t)slab * ld + c;
-                int nst[2] = {0, 0};
-                std::vector<std::vector<uint32_t>> lists[2];
+                cost[it] = 8.0 + 3.0 * rp;
                 for (int h = 0; h < rp; ++h) {
-                    lists[h].resize(32);
+                    std::vector<std::vector<uint32_t>> lists(32);
+                    int nst = 0;
                     for (int lane = 0; lane < 32; ++lane) {
                         const int r = rp * (32 * slab + lane) + h;
                         if (r >= ld) continue;
-                        for (auto &e : cell_w[(size_t)r + (size_t)c * ld]) lists[h][lane].push_back(enc(e));
-                        nst[h] = std::max(nst[h], (int)lists[h][lane].size());
+                        for (auto &e : cell_w[(size_t)r + (size_t)c * ld]) lists[lane].push_back(enc(e));
+                        nst = std::max(nst, (int)lists[lane].size());
                     }
-                }
-                REQUIRE(nst[0] <= 4 && nst[1] <= 4, "internal: a phase-B cell list is longer than four entries");
-                cost[it] = 6.0 + 2.0 * rp + nst[0] + nst[1];
-                o.n_b_steps += nst[0] + nst[1];
-                if (nst[0] + nst[1] == 0) continue;
-                const uint32_t base = (uint32_t)(o.b_ent.size() / 4);
-                o.bitem[2 * it] = base;
-                o.bitem[2 * it + 1] = (uint32_t)nst[0] | (uint32_t)nst[1] << 8;
-                o.b_ent.resize(o.b_ent.size() + (size_t)rp * 128, 0u);
-                for (int h = 0; h < rp; ++h) {
-                    // all four words are filled (pads beyond the item's steps are never read)
-                    const std::vector<uint32_t> grid = place(lists[h], 1, std::max(nst[h], 1), kSum1);
-                    const int ns_h = std::max(nst[h], 1);
-                    for (int lane = 0; lane < 32; ++lane)
-                        for (int st = 0; st < 4; ++st)
-                            o.b_ent[((size_t)base + 32 * h + lane) * 4 + st] =
-                                st < ns_h ? grid[(size_t)lane * ns_h + st] : (uint32_t)(eZero * S * 8);
+                    REQUIRE(nst <= 3, "internal: a phase-B cell list is longer than three entries");
+                    const int run = nst == 0 ? 0 : nst == 1 ? 1 : 3;          // steps the kernel executes
+                    const std::vector<uint32_t> grid = place(lists, 1, std::max(run, 1), kSum1);
+                    uint32_t *blk = o.b_ent.data() + (it * rp + h) * 128;
+                    for (int lane = 0; lane < 32; ++lane) {
+                        for (int st = 0; st < std::max(run, 1); ++st) blk[lane * 4 + st] = grid[(size_t)lane * std::max(run, 1) + st];
+                        blk[lane * 4 + 3] = nst == 0 ? 0u : nst == 1 ? 1u : 2u;
+                    }
+                    cost[it] += run;
+                    o.n_b_steps += run;
                 }
             }
+        for (size_t k = n_item * rp * 128 + 3; k < o.b_ent.size(); k += 4) o.b_ent[k] = 0u;
         // contiguous ranges of items per warp, balanced by cost
         double total = 0.0;
         for (double c : cost) total += c;
@@ -830,9 +824,9 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     {
         auto bad = [](const char *wh) { throw Fail{PYJAC_ELIMIT, wh}; };
         const uint32_t e_total = (uint32_t)o.n_e;
-        const size_t na_blocks = o.a_ent.size() / 4, nb_blocks = o.b_ent.size() / 4;
-        if (o.achunk.size() / 2 != (size_t)o.n_arow * NW) bad("internal: phase A is not whole rows of chunks");
-        for (size_t c = 0; c < o.achunk.size() / 2; ++c) {
+        const size_t na_blocks = o.a_ent.size() / 4;
+        if (o.achunk.size() / 2 != (size_t)(o.n_arow + 1) * NW) bad("internal: phase A is not whole rows of chunks");
+        for (size_t c = 0; c < (size_t)o.n_arow * NW; ++c) {
             const uint32_t base = o.achunk[2 * c], meta = o.achunk[2 * c + 1];
             const int steps = (int)(meta & 0xFF), kind = (int)((meta >> 8) & 0xF);
             const int nblk = 1 + (kind == (int)kAll3 ? 0 : (steps + 3) / 4);
@@ -853,14 +847,12 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                 }
             }
         }
-        for (size_t it = 0; it < o.bitem.size() / 2; ++it) {
-            const uint32_t base = o.bitem[2 * it];
-            if ((size_t)base + 32 * (size_t)rp > nb_blocks) bad("internal: an item reads past the entry table");
-            for (size_t k = 0; k < (size_t)rp * 128; ++k) {
-                const uint32_t wd = o.b_ent[(size_t)base * 4 + k];
-                if ((wd & kEntOffMask) % (8u * S) != 0 || (wd & kEntOffMask) / (8u * S) >= e_total)
-                    bad("internal: a cell entry points outside E");
-            }
+        if (o.b_ent.size() != ((size_t)o.n_slab * ld + 1) * rp * 128) bad("internal: phase B table has the wrong size");
+        for (size_t k = 0; k < o.b_ent.size(); ++k) {
+            const uint32_t wd = o.b_ent[k];
+            if (k % 4 == 3) { if (wd > 2u) bad("internal: a phase-B step count is out of range"); continue; }
+            if ((wd & kEntOffMask) % (8u * S) != 0 || (wd & kEntOffMask) / (8u * S) >= e_total)
+                bad("internal: a cell entry points outside E");
         }
         if (o.bsplit[0] != 0 || o.bsplit[NW] != o.n_slab * ld) bad("internal: phase B ranges do not cover the items");
     }

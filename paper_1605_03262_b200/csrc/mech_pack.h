@@ -34,26 +34,25 @@ struct HostPack {
     std::vector<uint32_t> a_ent;          // uint4 flattened
     // phase B items, one per (slab, column)
     int rp = 1, n_slab = 1;
-    std::vector<uint32_t> bitem;          // uint2 flattened
     std::vector<uint32_t> b_ent;          // uint4 flattened
     std::vector<int32_t> bsplit;          // [NW + 1]
     int eQ = 0, eH = 0, eAlpha = 0, eGamma = 0, eTc = 0, eWdot = 0, eG0 = 0;
     int eS1 = 0, eA0 = 0, eS4 = 0, eZero = 0, eDump = 0, eHs = 0, n_e = 0;
-    // launch shape chosen with the tables: NP blocks of S states per CTA iteration, threads per CTA,
-    // the CTAs per SM the shared-memory footprint was sized for
-    int S = 1, NP = 1, threads = 128, ctas_target = 1;
+    // launch shape chosen with the tables: S states per CTA iteration, threads per CTA, the CTAs per SM
+    // the shared-memory footprint was sized for
+    int S = 1, threads = 128, ctas_target = 1;
     // statistics (pyjac_pack_stats)
     long long n_cell_entries = 0, n_cells = 0, n_heavy_cells = 0, n_heavy_pieces = 0, n_a_steps = 0, n_b_steps = 0;
     long long n_plain_chunks = 0;
 };
 
 // What the launch-shape choice may use (api.cu fills it from the device properties and the
-// PYJAC_S / PYJAC_NP / PYJAC_THREADS / PYJAC_CTAS tuning hooks; 0 = choose).
+// PYJAC_S / PYJAC_THREADS / PYJAC_CTAS tuning hooks; 0 = choose).
 struct ShapeHints {
     long long smem_bytes = 227 * 1024 - 1024;   // dynamic shared memory one CTA may use
-    int S = 0, NP = 0, threads = 0, ctas = 0;
+    int S = 0, threads = 0, ctas = 0;
     int cap = 0;        // longest list one lane walks in phase A
-    int cell_cap = 0;   // longest Jacobian-cell list gathered in phase B (1..4); longer ones are summed piecewise in phase A
+    int cell_cap = 0;   // longest Jacobian-cell list gathered in phase B (1..3); longer ones are summed piecewise in phase A
     int rp = 0;         // rows per lane in phase B (1 or 2)
 };
 

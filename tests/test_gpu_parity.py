@@ -385,17 +385,19 @@ def test_host_buffer_variant_matches_device_variant(torch, PyJac):
 # ---------------------------------------------------------------------------------- launch shapes
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg,n,env", [
-    (1, 301, {"PYJAC_S": "1", "PYJAC_NP": "2"}),                                   # one state per block
-    (1, 301, {"PYJAC_S": "2", "PYJAC_NP": "1", "PYJAC_CTAS": "3", "PYJAC_THREADS": "128"}),   # three small CTAs per SM
-    (1, 301, {"PYJAC_NP": "2", "PYJAC_THREADS": "256"}),
-    (1, 301, {"PYJAC_CELL_CAP": "4"}),                                             # longer cell lists in phase B
+    (1, 301, {"PYJAC_S": "1", "PYJAC_CTAS": "4"}),                                 # one state per CTA iteration
+    (1, 301, {"PYJAC_S": "2", "PYJAC_CTAS": "3", "PYJAC_THREADS": "160"}),         # three small CTAs per SM
+    (1, 301, {"PYJAC_S": "3"}),                                                    # odd S: 8-byte shared loads
+    (1, 301, {"PYJAC_S": "4", "PYJAC_THREADS": "256"}),
+    (1, 301, {"PYJAC_S": "6", "PYJAC_THREADS": "384"}),
     (1, 301, {"PYJAC_CELL_CAP": "1", "PYJAC_CAP": "4"}),                           # everything summed in phase A, short lane lists
+    (1, 301, {"PYJAC_CELL_CAP": "2", "PYJAC_CAP": "30"}),
     (1, 301, {"PYJAC_RP": "1"}),                                                   # one row per lane, 8-byte stores
-    (0, 1024, {"PYJAC_S": "1", "PYJAC_NP": "4", "PYJAC_THREADS": "64"}),
-    (2, 65, {"PYJAC_S": "1", "PYJAC_NP": "3"}),
+    (0, 1024, {"PYJAC_S": "1", "PYJAC_THREADS": "64"}),
+    (2, 65, {"PYJAC_S": "3"}),
 ])
 def test_launch_shapes(torch, PyJac, monkeypatch, cfg, n, env):
-    """Every launch shape the tuning hooks can select (states per block, blocks per CTA iteration, CTA
+    """Every launch shape the tuning hooks can select (states per CTA iteration, CTAs per SM, CTA
     size, list lengths of the two gather phases, rows per lane) evaluates the same Jacobian: parity with
     the oracle within the same tolerance, ragged last batch included."""
     for k, v in env.items():
