@@ -123,7 +123,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     dm.n_pd = hp.n_pd; dm.n_pk = hp.n_pk; dm.n_rchunk = hp.n_rchunk; dm.n_plain = (int)hp.n_plain_chunks;
     dm.n_arow = hp.n_arow; dm.n_arow01 = hp.n_arow01;
     dm.brk_common = hp.brk_common;
-    dm.split_general = hp.threads * hp.ctas_target <= 256 ? 0 : 1;
+    dm.n_p1item = (int)hp.p1item.size();
     dm.rp = hp.rp; dm.n_slab = hp.n_slab;
     dm.eQ = hp.eQ; dm.eH = hp.eH; dm.eAlpha = hp.eAlpha; dm.eGamma = hp.eGamma; dm.eTc = hp.eTc;
     dm.eWdot = hp.eWdot; dm.eG0 = hp.eG0;
@@ -136,7 +136,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         up.add(&dm.nasa, hp.nasa); up.add(&dm.t_mid, hp.t_mid);
         up.add((const uint32_t **)&dm.slots, hp.slots); up.add((const uint32_t **)&dm.vidx, hp.vidx);
         up.add(&dm.lnA, hp.lnA); up.add(&dm.beta, hp.beta); up.add(&dm.Ta, hp.Ta);
-        up.add(&dm.rxn_orig, hp.rxn_orig);
+        up.add(&dm.rxn_orig, hp.rxn_orig); up.add(&dm.p1item, hp.p1item);
         up.add(&dm.rev_lnA, hp.rev_lnA); up.add(&dm.rev_beta, hp.rev_beta); up.add(&dm.rev_Ta, hp.rev_Ta);
         up.add(&dm.th_off, hp.th_off); up.add(&dm.th_data, hp.th_data); up.add(&dm.th_soa, hp.th_soa);
         up.add(&dm.lo_lnA, hp.lo_lnA); up.add(&dm.lo_beta, hp.lo_beta); up.add(&dm.lo_Ta, hp.lo_Ta);
@@ -167,6 +167,11 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
         if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->S)) {
             rc = PYJAC_ELIMIT;
         } else {
+            // shared-memory carve-out: what the CTAs this shape was sized for need, the rest of the 256 KB
+            // stays L1 (the gather tables are re-read from L1 / L2 by every CTA iteration)
+            int carveout = (int)((100 * ((long long)hp.ctas_target * (long long)(bytes + 1024 + 16)) + 228 * 1024 - 1) / (228 * 1024));
+            if (const char *e = std::getenv("PYJAC_CARVEOUT")) carveout = std::atoi(e);
+            carveout = carveout > 100 ? 100 : carveout < 0 ? 0 : carveout;
             for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
                 m->smem[level] = bytes;
                 const void *k = eval_kernel_ptr(level, m->S);
@@ -176,8 +181,7 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
                 if (cudaFuncGetAttributes(&fa, k) != cudaSuccess ||
                     cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)prop.sharedMemPerBlockOptin - (int)fa.sharedSizeBytes) != cudaSuccess ||
-                    cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                         cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
+                    cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, carveout) != cudaSuccess ||
                     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&m->ctas_per_sm[level], k, m->threads, bytes) !=
                         cudaSuccess ||
                     m->ctas_per_sm[level] < 1)
@@ -272,6 +276,7 @@ int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
     stats[7] = hp.n_rchunk; stats[8] = hp.S; stats[9] = hp.threads; stats[10] = 1; stats[11] = hp.ctas_target;
     stats[12] = hp.n_heavy_cells; stats[13] = hp.n_heavy_pieces; stats[14] = (int64_t)hp.a_ent.size() * 4;
     stats[15] = (int64_t)hp.b_ent.size() * 4;
+    for (int k = 0; k < 4; ++k) stats[16 + k] = hp.n_a_steps_kind[k];
     return PYJAC_OK;
 }
 

@@ -77,9 +77,11 @@ struct DeviceMech {
     int n_pd;                   // pressure-dependent reactions (third body, falloff, chem. activated): [0, n_pd)
     int n_pk;                   // PLOG / Chebyshev reactions: [n_pd, n_pd + n_pk)
     int n_rchunk;               // groups of 32 reactions
-    int split_general;          // 1: the group that holds reaction n_pd is two work items (pressure-dependent lanes /
-                                // the others); shortens the longest item of the reaction queue
     int n_plain;                // the last n_plain groups hold only plain reactions
+    int n_p1item;
+    const uint32_t *p1item;     // work items of P1, most expensive first: group | path << 16 | first state << 20; path 0 =
+                                // any reaction, one state (q); 1 = plain elementary reactions, 2 = any rate form with
+                                // at most three molecules per side, k_r from K_c and one NASA breakpoint: two states
     const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
     const uint4 *vidx;          // [nr] E indices of the slots' s'_ij: {v0|v1<<16, v2|v3<<16, v4|v5<<16, 0}
                                 //      (empty slots point at the dump slot)

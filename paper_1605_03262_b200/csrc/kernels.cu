@@ -1,21 +1,21 @@
 // kernels.cu -- sm_100a kernels for the batched source term and analytical Jacobian.
 //
-// One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop.  The S
-// states are interleaved in shared memory (element i of a region for state q at (R + i) * S + q), so
-// whatever does not depend on the state -- decoding a reaction, a gather entry, a column constant -- is
-// done once per lane and applied to the S states with vector loads.  Per iteration, separated by CTA
-// barriers:
+// One CTA evaluates NP blocks of S thermochemical states per iteration of a persistent grid-stride loop.
+// The S states of a block are interleaved in shared memory (element i of a region for state q at
+// (R + i) * S + q), so whatever does not depend on the state -- decoding a reaction, a gather entry, a
+// column constant -- is done once per lane and applied to the S states of each of the NP blocks with
+// vector loads.  Per iteration, separated by CTA barriers:
 //   P0  mixture (Eqs. 3-5) and species, warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT
 //       (Eqs. 9-13, 54-55); computed one iteration ahead, at the end of phase B
 //   P1  reactions, lane <-> reaction, groups of 32 from one dynamic queue: k_f, k_r (K_c from the
 //       per-reaction polynomial of device_mech.h `th_data`), R_f, R_r, c_i and the reusable per-reaction
 //       products of Section 4.1 into E: q_i, Theta_dT,i, a_i (the coefficient of d_j),
-//       the sparse terms s'_ij, the enthalpy H_i.  Groups made only of plain elementary reactions take a
-//       branch-free path that evaluates two states at a time.
+//       the sparse terms s'_ij, the enthalpy H_i.  Two states at a time; the common part of every rate
+//       form is branch-free, pressure-dependent lanes add the c_i tail.
 //   A   fixed-order gathers over E, lane <-> sum (or a share of one): wdot_k (Eq. 14), alpha'_r, gamma'_r
 //       of Eq. 112, the T column (Eq. 111), the column sums of the energy row (Eq. 113), and the long
 //       Jacobian-cell lists piece by piece
-//   B   the Jacobian, column by column, lane <-> two rows: every cell gathers its (at most three) entries
+//   B   the Jacobian, column by column, lane <-> two rows: every cell gathers its (at most four) entries
 //       on top of alpha'_r u_c - gamma'_r v_c, which is Eq. 112 with the per-reaction terms of Eqs.
 //       118-127 regrouped by what they multiply, and is stored at once: a warp
 //       stores 512 contiguous bytes per state and column, nothing is staged.  FIX items of the same phase
@@ -62,9 +62,12 @@ __device__ __forceinline__ double exp_rate(double x)
     const double nd = s - c_exp_red[1];
     double r = fma(nd, c_exp_red[2], x);
     r = fma(nd, c_exp_red[3], r);
-    double p = c_exp[0];
+    // even and odd powers as two independent Horner chains in r^2 (half the dependent depth)
+    const double r2 = r * r;
+    double po = c_exp[0], pe = c_exp[1];
 #pragma unroll
-    for (int i = 1; i < 14; ++i) p = fma(p, r, c_exp[i]);
+    for (int i = 2; i < 14; i += 2) { po = fma(po, r2, c_exp[i]); pe = fma(pe, r2, c_exp[i + 1]); }
+    double p = fma(po, r, pe);
     n = max(-1080, min(1030, n));
     const int n1 = n >> 1, n2 = n - n1;
     p *= __hiloint2double((n1 + 1023) << 20, 0);
@@ -114,12 +117,71 @@ __device__ __forceinline__ void stv(double *p, const double (&v)[S])
     }
 }
 
-// ---- P1, plain path: 32 elementary reactions with at most three molecules per side (one slot per
-// molecule), k_r from K_c or irreversible, one NASA breakpoint.  Two states at a time (q0, q0 + 1), no branches.
-template <int LEVEL, int S>
-__device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemPlan &sp, double *E, const double *X,
-                                                const double *sc, int s, int q0, const EvalOut &out, long long state0,
-                                                long long n)
+// ---- rate coefficient of a PLOG or Chebyshev reaction (Eqs. 37-43) and L = d ln k_f / dT (Eqs. 105, 110)
+__device__ __forceinline__ void special_rate(const DeviceMech &m, int s, int type, double P, double lnP, double lnT,
+                                             double invT, double &lnkf, double &L)
+{
+    const double *pk = m.pk_data + m.pk_ptr[s - m.n_pd];
+    if (type == PYJAC_PLOG) {                                       // Eqs. 37-39, 105
+        const int np = (int)pk[0];
+        const double *row = pk + 1;                              // {p, ln p, ln A, beta, Ta}
+        int lo = 0, hi = 0;
+        double wt = 0.0;
+        if (P <= row[0]) {
+            lo = hi = 0;
+        } else if (P >= row[5 * (np - 1)]) {
+            lo = hi = np - 1;
+        } else {
+            int j = 0;                                           // p_j <= P < p_{j+1}
+            for (int k = 1; k < np - 1; ++k) j += P >= row[5 * k] ? 1 : 0;
+            lo = j; hi = j + 1;
+            wt = (lnP - row[5 * j + 1]) / (row[5 * (j + 1) + 1] - row[5 * j + 1]);
+        }
+        const double *a1 = row + 5 * lo, *a2 = row + 5 * hi;
+        const double lnk1 = a1[2] + a1[3] * lnT - a1[4] * invT;
+        const double lnk2 = a2[2] + a2[3] * lnT - a2[4] * invT;
+        lnkf = lnk1 + (lnk2 - lnk1) * wt;
+        L = (a1[3] + a1[4] * invT + (a2[3] - a1[3] + (a2[4] - a1[4]) * invT) * wt) * invT;
+    } else {                                                        // Chebyshev, Eqs. 40-43, 110
+        const int nT = (int)pk[0], nP = (int)pk[1];
+        const double iTmin = pk[2], iTmax = pk[3], lpmin = pk[4], lpmax = pk[5];
+        const double *eta = pk + 6;
+        const double Tr = (2.0 * invT - iTmin - iTmax) / (iTmax - iTmin);
+        const double Pr = (2.0 * (lnP * kInvLn10) - lpmin - lpmax) / (lpmax - lpmin);
+        double sum = 0.0, dsum = 0.0;
+        double tm2 = 1.0, tm1 = Tr;          // T_{a-2}, T_{a-1}
+        double um2 = 1.0, um1 = 2.0 * Tr;    // U_{a-3}, U_{a-2}
+        for (int a = 0; a < nT; ++a) {
+            const double phiT = a == 0 ? 1.0 : a == 1 ? Tr : 2.0 * Tr * tm1 - tm2;
+            if (a >= 2) { tm2 = tm1; tm1 = phiT; }
+            double U = 0.0;                                       // U_{a-1}
+            if (a >= 1) {
+                const int nn = a - 1;
+                U = nn == 0 ? 1.0 : nn == 1 ? 2.0 * Tr : 2.0 * Tr * um1 - um2;
+                if (nn >= 2) { um2 = um1; um1 = U; }
+            }
+            double pm2 = 1.0, pm1 = Pr, rowsum = 0.0;
+            for (int b = 0; b < nP; ++b) {
+                const double phiP = b == 0 ? 1.0 : b == 1 ? Pr : 2.0 * Pr * pm1 - pm2;
+                if (b >= 2) { pm2 = pm1; pm1 = phiP; }
+                rowsum += eta[a * nP + b] * phiP;
+            }
+            sum += rowsum * phiT;
+            dsum += rowsum * (double)a * U;
+        }
+        lnkf = sum * kLn10;
+        L = kLn10 * invT * dsum * (-2.0 * invT) / (iTmax - iTmin);
+    }
+}
+
+// ---- P1, fast path: 32 reactions with at most three molecules per side (one slot per molecule), k_r from
+// K_c or irreversible, one NASA breakpoint; SP states at a time (q0 ..), the common part without branches.
+// GEN = false: plain elementary reactions only.  GEN = true: any rate form -- PLOG / Chebyshev lanes
+// replace ln k_f and L, pressure-dependent lanes (third body, falloff, chemically activated) scale the
+// products of the common part by c_i and add the derivative terms of c_i (Eqs. 77-100).
+template <int LEVEL, int S, bool GEN>
+__device__ __forceinline__ void fast_reactions(const DeviceMech &m, double *E, const double *X, const double *sc, int s,
+                                               int q0, const EvalOut &out, long long state0, long long n)
 {
     constexpr int SP = S % 2 == 0 ? 2 : 1;
     const int nr = m.nr;
@@ -131,7 +193,22 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
     const int nb = ((meta >> 12) & 0xF) + ((meta >> 16) & 0xF) + ((meta >> 20) & 0xF);
     const double snf = (double)nf, snr = (double)nb, dnu = (double)(nb - nf);
     const bool rev = meta_rev(meta) != PYJAC_IRREVERSIBLE;
-    const double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
+    const int type = GEN ? meta_type(meta) : PYJAC_ELEMENTARY;
+    const bool pdep = GEN && (type == PYJAC_THIRD_BODY || type == PYJAC_FALLOFF || type == PYJAC_CHEM_ACTIVATED);
+    const bool fall = GEN && (type == PYJAC_FALLOFF || type == PYJAC_CHEM_ACTIVATED);
+    const bool special = GEN && (type == PYJAC_PLOG || type == PYJAC_CHEBYSHEV);
+    double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
+    double dlnA = 0.0, dbeta = 0.0, dTa = 0.0, fp[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (GEN) {
+        // k_0 - k_inf of the falloff forms (Eq. 31); a chemically activated reaction multiplies its
+        // concentrations by k_0 (reading C5)
+        const int s_pd = min(s, max(m.n_pd, 1) - 1);
+        const double l0 = m.lo_lnA[s_pd], b0 = m.lo_beta[s_pd], t0 = m.lo_Ta[s_pd];
+#pragma unroll
+        for (int i = 0; i < 5; ++i) fp[i] = m.fall_par[5 * s_pd + i];
+        if (fall) { dlnA = l0 - lnA; dbeta = b0 - beta; dTa = t0 - Ta; }
+        if (type == PYJAC_CHEM_ACTIVATED) { lnA = l0; beta = b0; Ta = t0; }
+    }
     const double *th = m.th_soa + s;
     // one breakpoint for the whole mechanism (the usual case): the interval is known without a table read,
     // so the coefficient reads go out with the other tables instead of one L2 round trip later
@@ -143,72 +220,187 @@ __device__ __forceinline__ void plain_reactions(const DeviceMech &m, const SmemP
         v3 = (vi.y >> 16) * S; v4 = (vi.z & 0xFFFF) * S; v5 = (vi.z >> 16) * S;
     }
     const int orig = LEVEL == 0 ? m.rxn_orig[s] : 0;
+    // efficiencies of the group's reactions, entry e of lane l at eff_ent[eff_base[group] + 32 e + l]
+    // (padded with eps = 0 on the dummy species, so the trip count is the group's)
+    const uint4 *ef = nullptr;
+    int n_eff = 0;
+    if (GEN) {
+        const int grp = s >> 5;
+        ef = m.eff_ent + m.eff_base[grp] + (s & 31);
+        n_eff = m.eff_base[grp + 1] - m.eff_base[grp];
+    }
 
-    {
-        double T[SP], lnT[SP], invT[SP], lnkf[SP], L[SP], sB[SP], sdB[SP], kf[SP], kr[SP];
+    double T[SP], lnT[SP], invT[SP], lnkf[SP], L[SP], sB[SP], sdB[SP], kf[SP], kr[SP];
 #pragma unroll
-        for (int u = 0; u < SP; ++u) {
-            T[u] = sc[kT * S + q0 + u]; lnT[u] = sc[kLnT * S + q0 + u]; invT[u] = sc[kInvT * S + q0 + u];
-            lnkf[u] = fma(beta, lnT[u], fma(-Ta, invT[u], lnA));                 // Eq. 21
-            L[u] = fma(Ta, invT[u], beta) * invT[u];                             // Eq. 65
+    for (int u = 0; u < SP; ++u) {
+        T[u] = sc[kT * S + q0 + u]; lnT[u] = sc[kLnT * S + q0 + u]; invT[u] = sc[kInvT * S + q0 + u];
+        lnkf[u] = fma(beta, lnT[u], fma(-Ta, invT[u], lnA));                 // Eq. 21
+        L[u] = fma(Ta, invT[u], beta) * invT[u];                             // Eq. 65
+    }
+    if (GEN && special) {
+#pragma unroll
+        for (int u = 0; u < SP; ++u)
+            special_rate(m, s, type, sc[kP * S + q0 + u], sc[kLnP * S + q0 + u], lnT[u], invT[u], lnkf[u], L[u]);
+    }
+    // sum_k nu_ki B_k (Eq. 27 over the reaction) and its T derivative (Eq. 74)
+#pragma unroll
+    for (int u = 0; u < SP; ++u) {
+        const double *g = th + (size_t)(T[u] > brk ? 8 : 1) * nr;
+        const double g0 = g[0], g1 = g[nr], g2 = g[2 * (size_t)nr], g3 = g[3 * (size_t)nr], g4 = g[4 * (size_t)nr],
+                     g5 = g[5 * (size_t)nr], g6 = g[6 * (size_t)nr];
+        const double t = T[u];
+        sB[u] = fma(g1, lnT[u], g0) + fma(t, fma(t, fma(t, fma(t, g5, g4), g3), g2), g6 * invT[u]);
+        sdB[u] = fma(fma(-g6, invT[u], g1), invT[u], g2) + t * fma(t, fma(4.0 * g5, t, 3.0 * g4), 2.0 * g3);
+    }
+#pragma unroll
+    for (int u = 0; u < SP; ++u) kf[u] = exp_rate(lnkf[u]);
+#pragma unroll
+    for (int u = 0; u < SP; ++u) { kr[u] = exp_rate(lnkf[u] - sB[u]); kr[u] = rev ? kr[u] : 0.0; }   // Eqs. 23-27
+    // the SP states of one element are neighbours in shared memory: one 16-byte access for both
+    double c[6][SP], W[SP], vq[3][SP], vh[SP], vs[6][SP];
+    ldv<SP>(X + x0 + q0, c[0]); ldv<SP>(X + x1 + q0, c[1]); ldv<SP>(X + x2 + q0, c[2]);
+    ldv<SP>(X + x3 + q0, c[3]); ldv<SP>(X + x4 + q0, c[4]); ldv<SP>(X + x5 + q0, c[5]);
+    if (LEVEL == 2) ldv<SP>(sc + kW * S + q0, W);
+    double Rfv[SP], Rrv[SP];
+#pragma unroll
+    for (int u = 0; u < SP; ++u) {
+        const double c0 = c[0][u], c1 = c[1][u], c2 = c[2][u], c3 = c[3][u], c4 = c[4][u], c5 = c[5][u];
+        const double p01 = c0 * c1, p34 = c3 * c4;
+        const double Rf = kf[u] * (p01 * c2), Rr = kr[u] * (p34 * c5);       // Eqs. 18-19
+        const double R = Rf - Rr;
+        Rfv[u] = Rf; Rrv[u] = Rr;
+        vq[0][u] = R;
+        vh[u] = kRu * T[u] * fma(T[u], sdB[u], dnu);
+        if (LEVEL == 2) {
+            const double iT = invT[u];
+            // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
+            const double dRf = Rf * fma(-snf, iT, L[u]);
+            const double dRr = Rr * (fma(-snr, iT, L[u]) - sdB[u]);
+            vq[2][u] = fma(R, iT, dRf - dRr);
+            vq[1][u] = W[u] * (R - fma(Rf, snf, -Rr * snr));
+            const double nkr = -kr[u];
+            vs[0][u] = kf[u] * (c1 * c2); vs[1][u] = kf[u] * (c0 * c2); vs[2][u] = kf[u] * p01;   // Eq. 120
+            vs[3][u] = nkr * (c4 * c5); vs[4][u] = nkr * (c3 * c5); vs[5][u] = nkr * p34;         // Eq. 121
         }
-        // sum_k nu_ki B_k (Eq. 27 over the reaction) and its T derivative (Eq. 74)
+    }
+    double cm[SP];
 #pragma unroll
-        for (int u = 0; u < SP; ++u) {
-            const double *g = th + (size_t)(T[u] > brk ? 8 : 1) * nr;
-            const double g0 = g[0], g1 = g[nr], g2 = g[2 * (size_t)nr], g3 = g[3 * (size_t)nr], g4 = g[4 * (size_t)nr],
-                         g5 = g[5 * (size_t)nr], g6 = g[6 * (size_t)nr];
-            const double t = T[u];
-            sB[u] = fma(g1, lnT[u], g0) + fma(t, fma(t, fma(t, fma(t, g5, g4), g3), g2), g6 * invT[u]);
-            sdB[u] = fma(fma(-g6, invT[u], g1), invT[u], g2) + t * fma(t, fma(4.0 * g5, t, 3.0 * g4), 2.0 * g3);
+    for (int u = 0; u < SP; ++u) cm[u] = 1.0;
+    if (GEN) {
+        // ---- pressure modification c_i (Eq. 20) and its derivatives (Eqs. 77-100): q_i = c R,
+        // Theta = dc/dT R + c Theta0, a = c a0 + b (rho - W [X]_i), s'_ij = c s0_ij, and b (alpha_ij - 1)
+        // per efficiency; lanes without a pressure dependence keep c = 1, b = 0
+        double Xi[SP], bb[SP], dcdT[SP], mixW[SP];
+#pragma unroll
+        for (int u = 0; u < SP; ++u) { Xi[u] = (pdep && !meta_single(meta)) ? sc[kM * S + q0 + u] : 0.0; bb[u] = 0.0; dcdT[u] = 0.0; }
+        for (int e = 0; e < n_eff; e += 128) {                       // Eqs. 28-30, four entries at a time
+            uint4 w[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.ns, 0u, 0u, 0u);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
+                double x[SP];
+                ldv<SP>(X + (w[k].x & 0xFFFF) * S + q0, x);
+#pragma unroll
+                for (int u = 0; u < SP; ++u) Xi[u] = fma(eps, x[u], Xi[u]);
+            }
         }
+        if (pdep) {
 #pragma unroll
-        for (int u = 0; u < SP; ++u) kf[u] = exp_rate(lnkf[u]);
+            for (int u = 0; u < SP; ++u) {
+                const double R = vq[0][u], iT = invT[u], Tu = T[u];
+                double cc, G, lPrT, fT = 0.0;
+                if (type == PYJAC_THIRD_BODY) {
+                    cc = Xi[u]; G = Xi[u]; lPrT = -iT; bb[u] = R;            // Eqs. 79-80
+                } else {
+                    const double Pr = exp_rate(fma(dbeta, lnT[u], fma(-dTa, iT, dlnA))) * Xi[u];   // Eq. 31
+                    lPrT = iT * (dbeta + dTa * iT - 1.0);                    // Eq. 84 / P_r
+                    const int form = meta_form(meta);
+                    double F = 1.0, gF = 0.0;                                // gF = (P_r/F) dF/dP_r
+                    if (form == PYJAC_TROE) {                                // Eqs. 33-35, 90-96
+                        // fp[1], fp[2] hold 1/T***, 1/T* (mech_pack.cu); three reciprocals serve every quotient
+                        const double a = fp[0], i3 = fp[1], i1 = fp[2];
+                        const double e3 = exp_rate(-Tu * i3), e1 = exp_rate(-Tu * i1);
+                        const double e2 = fp[4] != 0.0 ? exp_rate(-fp[3] * iT) : 0.0;
+                        const double Fc = (1.0 - a) * e3 + a * e1 + e2;
+                        const double dFc = -(1.0 - a) * i3 * e3 - a * i1 * e1 + fp[3] * iT * iT * e2;
+                        const double lnFc = log(Fc);
+                        const double lF = lnFc * kInvLn10, lP = log10(Pr);
+                        const double At = lP - 0.67 * lF - 0.4;
+                        const double Bt = 0.806 - 1.1762 * lF - 0.14 * lP;
+                        const double rB = 1.0 / Bt, rF = 1.0 / Fc;
+                        const double AB = At * rB, rq = 1.0 / (1.0 + AB * AB);
+                        F = exp_rate(lnFc * rq);
+                        const double k2 = lnFc * 2.0 * At * (rB * rB * rB) * (kInvLn10 * rq * rq);
+                        gF = -k2 * (Bt + 0.14 * At);
+                        fT = (rq - k2 * (1.1762 * At - 0.67 * Bt)) * rF * dFc;
+                    } else if (form == PYJAC_SRI) {                          // Eqs. 36, 97-100
+                        const double ea = exp_rate(-fp[1] * iT), ec = exp_rate(-Tu * fp[2]);       // fp[2] holds 1/c
+                        const double base = fp[0] * ea + ec, lnb = log(base);
+                        const double lP = log10(Pr), Xs = 1.0 / (1.0 + lP * lP);
+                        F = fp[3] * exp_rate(fp[4] * lnT[u] + Xs * lnb);
+                        gF = -Xs * Xs * 2.0 * lP * lnb * kInvLn10;
+                        fT = fp[4] * iT + Xs * (fp[0] * fp[1] * iT * iT * ea - ec * fp[2]) / base;
+                    }
+                    const double i1p = 1.0 / (1.0 + Pr);
+                    double Theta;
+                    if (type == PYJAC_FALLOFF) { cc = Pr * i1p * F; Theta = i1p; }       // Eqs. 82-83
+                    else                       { cc = i1p * F;      Theta = -Pr * i1p; } // Eqs. 86-87
+                    G = cc * (Theta + gF);
+                    bb[u] = R * G / Xi[u];
+                }
+                cm[u] = cc;
+                dcdT[u] = G * lPrT + cc * fT;
+            }
+        }
+        if (LEVEL == 2) {
 #pragma unroll
-        for (int u = 0; u < SP; ++u) { kr[u] = exp_rate(lnkf[u] - sB[u]); kr[u] = rev ? kr[u] : 0.0; }   // Eqs. 23-27
-        // the SP states of one element are neighbours in shared memory: one 16-byte access for both
-        double c[6][SP], W[SP], vq[3][SP], vh[SP], vs[6][SP];
-        ldv<SP>(X + x0 + q0, c[0]); ldv<SP>(X + x1 + q0, c[1]); ldv<SP>(X + x2 + q0, c[2]);
-        ldv<SP>(X + x3 + q0, c[3]); ldv<SP>(X + x4 + q0, c[4]); ldv<SP>(X + x5 + q0, c[5]);
-        if (LEVEL == 2) ldv<SP>(sc + kW * S + q0, W);
+            for (int u = 0; u < SP; ++u) mixW[u] = (pdep && !meta_single(meta)) ? sc[kRho * S + q0 + u] - W[u] * Xi[u] : -W[u] * Xi[u];
 #pragma unroll
-        for (int u = 0; u < SP; ++u) {
-            const int q = q0 + u;
-            const double c0 = c[0][u], c1 = c[1][u], c2 = c[2][u], c3 = c[3][u], c4 = c[4][u], c5 = c[5][u];
-            const double p01 = c0 * c1, p34 = c3 * c4;
-            const double Rf = kf[u] * (p01 * c2), Rr = kr[u] * (p34 * c5);       // Eqs. 18-19
-            const double R = Rf - Rr;
-            vq[0][u] = R;
-            vh[u] = kRu * T[u] * fma(T[u], sdB[u], dnu);
-            if (LEVEL == 0) {
-                const long long st = state0 + q;
-                if (st < n) {
-                    const long long o = st * nr + orig;
-                    if (out.rf) out.rf[o] = Rf;
-                    if (out.rr) out.rr[o] = Rr;
-                    if (out.cmod) out.cmod[o] = 1.0;
+            for (int u = 0; u < SP; ++u) {
+                const double R = vq[0][u];
+                vq[2][u] = fma(dcdT[u], R, cm[u] * vq[2][u]);
+                vq[1][u] = fma(bb[u], mixW[u], cm[u] * vq[1][u]);
+#pragma unroll
+                for (int k = 0; k < 6; ++k) vs[k][u] *= cm[u];
+            }
+            for (int e = 0; e < n_eff; e += 128) {
+                uint4 w[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
+                    double t[SP];
+#pragma unroll
+                    for (int u = 0; u < SP; ++u) t[u] = bb[u] * eps;
+                    stv<SP>(E + (w[k].x >> 16) * S + q0, t);
                 }
             }
-            if (LEVEL == 2) {
-                const double iT = invT[u];
-                // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
-                const double dRf = Rf * fma(-snf, iT, L[u]);
-                const double dRr = Rr * (fma(-snr, iT, L[u]) - sdB[u]);
-                vq[2][u] = fma(R, iT, dRf - dRr);
-                vq[1][u] = W[u] * (R - fma(Rf, snf, -Rr * snr));
-                const double nkr = -kr[u];
-                vs[0][u] = kf[u] * (c1 * c2); vs[1][u] = kf[u] * (c0 * c2); vs[2][u] = kf[u] * p01;   // Eq. 120
-                vs[3][u] = nkr * (c4 * c5); vs[4][u] = nkr * (c3 * c5); vs[5][u] = nkr * p34;         // Eq. 121
+        }
+#pragma unroll
+        for (int u = 0; u < SP; ++u) vq[0][u] *= cm[u];
+    }
+    if (LEVEL == 0) {
+#pragma unroll
+        for (int u = 0; u < SP; ++u) {
+            const long long st = state0 + q0 + u;
+            if (st < n) {
+                const long long o = st * nr + orig;
+                if (out.rf) out.rf[o] = Rfv[u];
+                if (out.rr) out.rr[o] = Rrv[u];
+                if (out.cmod) out.cmod[o] = cm[u];
             }
         }
-        stv<SP>(E + (m.eQ + 3 * s) * S + q0, vq[0]);
-        if (LEVEL >= 1) stv<SP>(E + (m.eH + s) * S + q0, vh);
-        if (LEVEL == 2) {
-            stv<SP>(E + (m.eQ + 3 * s + 1) * S + q0, vq[1]);
-            stv<SP>(E + (m.eQ + 3 * s + 2) * S + q0, vq[2]);
-            stv<SP>(E + v0 + q0, vs[0]); stv<SP>(E + v1 + q0, vs[1]); stv<SP>(E + v2 + q0, vs[2]);
-            stv<SP>(E + v3 + q0, vs[3]); stv<SP>(E + v4 + q0, vs[4]); stv<SP>(E + v5 + q0, vs[5]);
-        }
+    }
+    stv<SP>(E + (m.eQ + 3 * s) * S + q0, vq[0]);
+    if (LEVEL >= 1) stv<SP>(E + (m.eH + s) * S + q0, vh);
+    if (LEVEL == 2) {
+        stv<SP>(E + (m.eQ + 3 * s + 1) * S + q0, vq[1]);
+        stv<SP>(E + (m.eQ + 3 * s + 2) * S + q0, vq[2]);
+        stv<SP>(E + v0 + q0, vs[0]); stv<SP>(E + v1 + q0, vs[1]); stv<SP>(E + v2 + q0, vs[2]);
+        stv<SP>(E + v3 + q0, vs[3]); stv<SP>(E + v4 + q0, vs[4]); stv<SP>(E + v5 + q0, vs[5]);
     }
 }
 
@@ -834,7 +1026,6 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
     __shared__ int ctr[2];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int NT = blockDim.x, NW = NT >> 5;
-    constexpr int SP = S % 2 == 0 ? 2 : 1;
     const int ns = m.ns, ld = m.ld, nr = m.nr;
     double *E = sm + sp.E * S;
     const double *colc = sm + (size_t)sp.total * S + sp.colc;
@@ -852,12 +1043,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
     }
     if (tid == 0) ctr[0] = 0;
     const long long nbatch = (n + S - 1) / S;
-    // work items of P1: the general groups one state at a time (most expensive first), then the plain
-    // groups SP states at a time
-    const int n_gen = m.n_rchunk - m.n_plain;
-    const int split_l = m.n_pd & 31, split_c = (m.split_general && split_l != 0 && (m.n_pd >> 5) < n_gen) ? (m.n_pd >> 5) : -1;
-    const int n_genq = n_gen + (split_c >= 0 ? 1 : 0);
-    const int i_plain = n_genq * S, n_p1 = i_plain + m.n_plain * (S / SP);
+    const int n_p1 = m.n_p1item;
     const int arows = LEVEL == 2 ? m.n_arow : m.n_arow01;
     const int it0 = m.bsplit[warp], it1 = m.bsplit[warp + 1];
     const int nfix = 1 + (ns + 31) / 32;
@@ -875,19 +1061,13 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
         const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S;
         // ---- P1: reactions
         for (int it = grab(&ctr[0], lane); it < n_p1; it = grab(&ctr[0], lane)) {
-            if (it < i_plain) {
-                // general groups, one state at a time; the group that holds both pressure-dependent and
-                // other reactions is two items (each runs only its own code paths)
-                const int gi = it / S, q = it - gi * S;
-                const int c = gi < n_gen ? gi : split_c;
-                int sl = lane;              // lanes of the other part repeat this part's first reaction
-                if (c == split_c) sl = gi < n_gen ? (lane < split_l ? lane : 0) : (lane >= split_l ? lane : split_l);
-                reaction<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + sl, nr - 1), q, out, state0, n);
-            } else {
-                const int j = it - i_plain;
-                const int c = n_gen + j / (S / SP), q0 = (j % (S / SP)) * SP;
-                plain_reactions<LEVEL, S>(m, sp, E, X, sc, min(c * 32 + lane, nr - 1), q0, out, state0, n);
-            }
+            // item = {group of 32 reactions, path, first state}: most expensive first (device_mech.h `p1item`)
+            const uint32_t w = m.p1item[it];
+            const int c = (int)(w & 0xFFFF), kind = (int)(w >> 16) & 0xF, q = (int)(w >> 20);
+            const int s = min(c * 32 + lane, nr - 1);
+            if (kind == 1) fast_reactions<LEVEL, S, false>(m, E, X, sc, s, q, out, state0, n);
+            else if (kind == 2) fast_reactions<LEVEL, S, true>(m, E, X, sc, s, q, out, state0, n);
+            else reaction<LEVEL, S>(m, sp, E, X, sc, s, q, out, state0, n);
         }
         __syncthreads();
         if (tid == 0) ctr[0] = 0;

@@ -231,13 +231,23 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         out.insert(out.end(), rest.begin(), rest.end());
         order.swap(out);
     }
+    // ---- P1 path of every group of 32 reactions (device_mech.h `p1item`)
+    auto fastgen = [&](int i) { return d->rev_type[i] != PYJAC_REV_EXPLICIT && expandable(i) && n_brk[i] <= 1; };
     o.n_rchunk = (nr + 31) / 32;
     o.rchunk.assign(std::max(o.n_rchunk, 1), 0u);
     for (int c = 0; c < o.n_rchunk; ++c) {
-        bool all = true;
-        for (int s = 32 * c; s < std::min(nr, 32 * c + 32); ++s) all = all && plain(order[s]);
-        o.rchunk[c] = all ? 1u : 0u;
-        o.n_plain_chunks += all ? 1 : 0;
+        bool all_plain = true, all_fast = true;
+        for (int s = 32 * c; s < std::min(nr, 32 * c + 32); ++s) {
+            all_plain = all_plain && plain(order[s]);
+            all_fast = all_fast && fastgen(order[s]);
+        }
+        o.rchunk[c] = all_plain ? 1u : all_fast ? 2u : 0u;
+    }
+    // the plain groups are the last ones (sorted order); a plain group in front of a non-plain one takes path 2
+    for (int c = o.n_rchunk - 1, tail = 1; c >= 0; --c) {
+        if (o.rchunk[c] != 1u) tail = 0;
+        else if (!tail) o.rchunk[c] = 2u;
+        o.n_plain_chunks += o.rchunk[c] == 1u ? 1 : 0;
     }
 
     // ---- slots of every reaction (sorted order): species and nu per slot
@@ -589,7 +599,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         int threads = hints.threads > 0 ? hints.threads : (kMaxThreads / ctas) & ~31;
         if (threads < 32 * S) threads = 32 * S;
         if (threads < 64) threads = 64;
-        if (threads > kMaxThreads || threads % 32) throw Fail{PYJAC_EINVAL, "threads per CTA must be a multiple of 32 up to 512"};
+        if (threads > kMaxThreads || threads % 32) throw Fail{PYJAC_EINVAL, "threads per CTA must be a multiple of 32 up to kMaxThreads"};
         o.S = S; o.threads = threads; o.ctas_target = ctas;
         if ((long long)o.n_e * S * 8 > (long long)kEntOffMask + 1)
             throw Fail{PYJAC_ELIMIT, "per-CTA tables exceed the 256 KB offset range of a gather entry"};
@@ -599,6 +609,17 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     if (ld % 2 != 0) o.rp = 1;
     const int rp = o.rp;
     o.n_slab = (ld + 32 * rp - 1) / (32 * rp);
+
+    // ---- work items of P1: the groups that need the one-state path first, then the pressure-dependent
+    // groups, then the plain ones, each for every state (pair)
+    {
+        const int SP = S % 2 == 0 ? 2 : 1;
+        for (uint32_t kind : {0u, 2u, 1u})
+            for (int c = 0; c < o.n_rchunk; ++c) {
+                if (o.rchunk[c] != kind) continue;
+                for (int q = 0; q < S; q += (kind == 0u ? 1 : SP)) o.p1item.push_back((uint32_t)c | kind << 16 | (uint32_t)q << 20);
+            }
+    }
 
     // ---- encoding (device_mech.h) and bank-aware placement.  Which step of a lane reads which of its
     // entries, and which zero slot a padding entry reads, is free: both are chosen greedily so that the
@@ -752,6 +773,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                 blk[(size_t)lane * 4 + 1] = (uint32_t)bits;
                 blk[(size_t)lane * 4 + 2] = (uint32_t)(bits >> 32);
             }
+            o.n_a_steps_kind[c.kind] += c.steps;
             if (c.kind == kAll3) { o.n_a_steps += c.steps; continue; }
             std::vector<std::vector<uint32_t>> lists((size_t)per_row);
             for (size_t i = 0; i < c.t.size(); ++i) {

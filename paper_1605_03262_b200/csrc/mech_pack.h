@@ -11,7 +11,8 @@ struct HostPack {
     int ns = 0, nr = 0;
     std::vector<double> inv_mw, mw, colc, wrow, nasa, t_mid;
     int n_pd = 0, n_pk = 0;
-    std::vector<uint32_t> rchunk;
+    std::vector<uint32_t> rchunk;         // per group of 32 reactions: the P1 path (device_mech.h `p1item`)
+    std::vector<uint32_t> p1item;
     std::vector<uint32_t> slots;          // 4 words per reaction
     std::vector<uint32_t> vidx;           // 4 words per reaction
     std::vector<double> lnA, beta, Ta, rev_lnA, rev_beta, rev_Ta;
@@ -44,6 +45,7 @@ struct HostPack {
     // statistics (pyjac_pack_stats)
     long long n_cell_entries = 0, n_cells = 0, n_heavy_cells = 0, n_heavy_pieces = 0, n_a_steps = 0, n_b_steps = 0;
     long long n_plain_chunks = 0;
+    long long n_a_steps_kind[4] = {0, 0, 0, 0};     // phase-A steps by chunk kind
 };
 
 // What the launch-shape choice may use (api.cu fills it from the device properties and the
