@@ -118,14 +118,14 @@ def mech_desc(mech: Mechanism):
 PACK_STAT_NAMES = ("e_doubles", "cell_entries", "b_steps", "a_steps", "cells", "chunks",
                    "smem_bytes_per_cta", "reaction_chunks", "states_per_block", "threads", "blocks_per_cta",
                    "ctas_per_sm_target", "heavy_cells", "heavy_pieces", "a_table_bytes", "b_table_bytes",
-                   "a_steps_sum3", "a_steps_sum1", "a_steps_prod", "a_steps_all3")
+                   "a_steps_sum3", "a_steps_sum1", "a_steps_prod", "a_steps_all3", "a_conflict_wf", "b_conflict_wf")
 
 
 def pack_stats(mech: Mechanism) -> dict:
     """Host-only: sizes of the evaluation tables `pyjac_mech_create` would build (no CUDA call)."""
     lib = load_library()
     d, keep = mech_desc(mech)
-    out = (C.c_int64 * 20)()
+    out = (C.c_int64 * 22)()
     _check(lib.pyjac_pack_stats(C.byref(d), out), "pyjac_pack_stats")
     return dict(zip(PACK_STAT_NAMES, [int(v) for v in out]))
 

@@ -277,6 +277,7 @@ int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
     stats[12] = hp.n_heavy_cells; stats[13] = hp.n_heavy_pieces; stats[14] = (int64_t)hp.a_ent.size() * 4;
     stats[15] = (int64_t)hp.b_ent.size() * 4;
     for (int k = 0; k < 4; ++k) stats[16 + k] = hp.n_a_steps_kind[k];
+    stats[20] = hp.n_conflict_wf[0]; stats[21] = hp.n_conflict_wf[1];
     return PYJAC_OK;
 }
 

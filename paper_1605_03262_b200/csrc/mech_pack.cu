@@ -8,6 +8,7 @@
 #include <algorithm>
 #include <array>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <utility>
 #include <numeric>
@@ -580,13 +581,11 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         auto limit_for = [&](int ctas) { return std::min<long long>(sm_bytes / ctas - 1024 - 128, hints.smem_bytes); };
         int S = hints.S, ctas = hints.ctas;
         if (S == 0) {
-            if (ctas > 0) {
-                for (int cand : {6, 4, 3, 2, 1})
-                    if (S == 0 && bytes_for(cand) <= limit_for(ctas)) S = cand;
-            } else {
-                for (int cand : {6, 2, 1})
-                    if (S == 0 && bytes_for(cand) <= limit_for(1)) S = cand;
-            }
+            // measured on B200 (profiles/): three interleaved states beat two, four and six on every
+            // benchmark mechanism they fit (finer work items of the reaction queue, conflict-free 8-byte
+            // gathers over sixteen bank pairs); then two, then one
+            for (int cand : {3, 2, 1})
+                if (S == 0 && bytes_for(cand) <= limit_for(ctas > 0 ? ctas : 1)) S = cand;
             if (S == 0) throw Fail{PYJAC_ELIMIT, "per-state tables exceed the shared memory of one CTA"};
         }
         if (S != 1 && S != 2 && S != 3 && S != 4 && S != 6) throw Fail{PYJAC_EINVAL, "states per CTA iteration must be 1, 2, 3, 4 or 6"};
@@ -626,62 +625,117 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     // lanes of one shared-memory wavefront hit different bank groups at every step.
     auto enc = [&](const std::pair<uint32_t, int> &e) { return coef_hi14(e.second) | (uint32_t)(e.first * S * 8); };
     const int gsz = S % 2 == 0 ? 16 : 8, LP = 128 / gsz, nq = 32 / LP;     // bytes per lane access, lanes per wavefront
-    // lists[slot] sits on lanes [slot * width, (slot + 1) * width); returns grid[lane * steps + step]
-    auto place = [&](const std::vector<std::vector<uint32_t>> &lists, int width, int steps, uint32_t kind) {
+    // lists[slot] sits on lanes [perm[slot] * width, (perm[slot] + 1) * width); returns grid[lane * steps + step].
+    // Local search over two kinds of moves: two steps of one lane trade places; two sums of a chunk trade
+    // lanes (`swap_slots`; not for phase B, whose lanes are tied to Jacobian rows).  The cost of a (step,
+    // wavefront group of LP lanes) is the number of wavefronts beyond the first: the largest number of
+    // different addresses in one bank group.
+    auto place = [&](const std::vector<std::vector<uint32_t>> &lists, int width, int steps, uint32_t kind,
+                     bool swap_slots, std::vector<int> *perm_out) {
         const int nstream = kind == kProd ? 2 : 1;
+        const int nslot = 32 / width;
         std::vector<uint32_t> grid((size_t)32 * std::max(steps, 1), 0u);
+        std::vector<int> perm(nslot);
+        for (int i = 0; i < nslot; ++i) perm[i] = i;
+        if (perm_out) *perm_out = perm;
         if (steps == 0) return grid;
-        std::vector<char> filled((size_t)32 * steps, 0);
-        std::vector<std::vector<uint32_t>> occ((size_t)steps * nq * nstream);
-        auto occ_of = [&](int step, int lane, int st) -> std::vector<uint32_t> & {
-            return occ[((size_t)step * nq + lane / LP) * nstream + st];
+        constexpr uint32_t kPad = 0xFFFFFFFFu;                 // a padding position (reads a zero slot chosen at the end)
+        std::fill(grid.begin(), grid.end(), kPad);
+        auto granule = [&](uint32_t w, int k) -> uint32_t {
+            if (kind == kProd) return (k == 0 ? (w & 0xFFFF) : (w >> 16)) * (uint32_t)(S * 8 / gsz);
+            return (w & kEntOffMask) / (uint32_t)gsz;
         };
-        auto granules = [&](uint32_t w, uint32_t g[2]) {
-            if (kind == kProd) { g[0] = (w & 0xFFFF) * S * 8 / gsz; g[1] = (w >> 16) * S * 8 / gsz; }
-            else { g[0] = (w & kEntOffMask) / gsz; g[1] = 0; }
-        };
-        auto clash = [&](const std::vector<uint32_t> &v, uint32_t g) {
-            bool same_bank = false;
-            for (uint32_t x : v) {
-                if (x == g) return 0;                  // same address: broadcast
-                same_bank = same_bank || (x % LP == g % LP);
-            }
-            return same_bank ? 1 : 0;
-        };
+        // initial layout: the words of a list go round its lanes
         for (size_t sl = 0; sl < lists.size(); ++sl) {
-            const int lane0 = (int)sl * width;
-            for (uint32_t w : lists[sl]) {
-                uint32_t g[2];
-                granules(w, g);
-                int best = -1, bc = 1 << 30;
-                for (int st = 0; st < steps && bc > 0; ++st)
-                    for (int j = 0; j < width; ++j) {
-                        if (filled[(size_t)(lane0 + j) * steps + st]) continue;
-                        int cc = 0;
-                        for (int k = 0; k < nstream; ++k) cc += clash(occ_of(st, lane0 + j, k), g[k]);
-                        if (cc < bc) { bc = cc; best = (lane0 + j) * steps + st; }
-                        if (bc == 0) break;
-                    }
-                REQUIRE(best >= 0, "internal: a gather list does not fit its lanes");
-                filled[best] = 1;
-                grid[best] = w;
-                for (int k = 0; k < nstream; ++k) occ_of(best % steps, best / steps, k).push_back(g[k]);
+            REQUIRE((int)lists[sl].size() <= width * steps, "internal: a gather list does not fit its lanes");
+            for (size_t e = 0; e < lists[sl].size(); ++e)
+                grid[(size_t)((int)sl * width + (int)(e % width)) * steps + e / width] = lists[sl][e];
+        }
+        auto cell_cost = [&](int step, int quarter) {
+            int cost = 0;
+            for (int k = 0; k < nstream; ++k) {
+                uint32_t seen[32];
+                int nseen = 0, cnt[32] = {0};
+                int worst = 1;
+                for (int j = 0; j < LP; ++j) {
+                    const uint32_t w = grid[(size_t)(quarter * LP + j) * steps + step];
+                    if (w == kPad) continue;
+                    const uint32_t g = granule(w, k);
+                    bool dup = false;
+                    for (int i = 0; i < nseen; ++i) dup = dup || seen[i] == g;
+                    if (dup) continue;
+                    seen[nseen++] = g;
+                    worst = std::max(worst, ++cnt[g % LP]);
+                }
+                cost += worst - 1;
             }
+            return cost;
+        };
+        for (int pass = 0; pass < 6; ++pass) {
+            bool improved = false;
+            for (int lane = 0; lane < 32; ++lane) {
+                const int q = lane / LP;
+                for (int s1 = 0; s1 < steps; ++s1)
+                    for (int s2 = s1 + 1; s2 < steps; ++s2) {
+                        uint32_t &a = grid[(size_t)lane * steps + s1], &b = grid[(size_t)lane * steps + s2];
+                        if (a == b) continue;
+                        const int before = cell_cost(s1, q) + cell_cost(s2, q);
+                        if (before == 0) continue;
+                        std::swap(a, b);
+                        const int after = cell_cost(s1, q) + cell_cost(s2, q);
+                        if (after < before) improved = true;
+                        else std::swap(a, b);
+                    }
+            }
+            if (swap_slots && width <= LP)
+                for (int a = 0; a < nslot; ++a)
+                    for (int b = a + 1; b < nslot; ++b) {
+                        const int qa = a * width / LP, qb = b * width / LP;
+                        if (qa == qb) continue;
+                        int before = 0;
+                        for (int st = 0; st < steps; ++st) before += cell_cost(st, qa) + cell_cost(st, qb);
+                        if (before == 0) continue;
+                        auto swap_all = [&]() {
+                            for (int j = 0; j < width; ++j)
+                                for (int st = 0; st < steps; ++st)
+                                    std::swap(grid[(size_t)(a * width + j) * steps + st], grid[(size_t)(b * width + j) * steps + st]);
+                        };
+                        swap_all();
+                        int after = 0;
+                        for (int st = 0; st < steps; ++st) after += cell_cost(st, qa) + cell_cost(st, qb);
+                        if (after < before) { improved = true; std::swap(perm[a], perm[b]); }
+                        else swap_all();
+                    }
+            if (!improved) break;
+        }
+        for (int st = 0; st < steps; ++st)
+            for (int q = 0; q < nq; ++q) o.n_conflict_wf[swap_slots ? 0 : 1] += cell_cost(st, q);
+        // perm[position] = list that sits there; callers want list -> position
+        if (perm_out) {
+            perm_out->assign(nslot, 0);
+            for (int pos = 0; pos < nslot; ++pos) (*perm_out)[perm[pos]] = pos;
         }
         // pads: coefficient 0 (kProd: zero times zero) on a zero slot whose bank group is free
         for (int st = 0; st < steps; ++st)
-            for (int lane = 0; lane < 32; ++lane) {
-                if (filled[(size_t)lane * steps + st]) continue;
+            for (int q = 0; q < nq; ++q) {
+                bool used[2][32] = {{false}};
+                for (int j = 0; j < LP; ++j) {
+                    const uint32_t w = grid[(size_t)(q * LP + j) * steps + st];
+                    if (w == kPad) continue;
+                    for (int k = 0; k < nstream; ++k) used[k][granule(w, k) % LP] = true;
+                }
                 int z = 0;
                 for (int t = 0; t < LP; ++t) {
-                    const uint32_t g = (uint32_t)(eZero + t) * S * 8 / gsz;
+                    const uint32_t g = (uint32_t)(eZero + t) * (uint32_t)(S * 8 / gsz);
                     bool ok = true;
-                    for (int k = 0; k < nstream; ++k) ok = ok && clash(occ_of(st, lane, k), g) == 0;
+                    for (int k = 0; k < nstream; ++k) ok = ok && !used[k][g % LP];
                     if (ok) { z = t; break; }
                 }
                 const uint32_t zi = (uint32_t)(eZero + z);
-                for (int k = 0; k < nstream; ++k) occ_of(st, lane, k).push_back(zi * S * 8 / gsz);
-                grid[(size_t)lane * steps + st] = kind == kProd ? (zi | zi << 16) : zi * S * 8;
+                for (int j = 0; j < LP; ++j) {
+                    uint32_t &w = grid[(size_t)(q * LP + j) * steps + st];
+                    if (w == kPad) w = kind == kProd ? (zi | zi << 16) : zi * (uint32_t)(S * 8);
+                }
             }
         return grid;
     };
@@ -762,37 +816,44 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             const int nblk = 1 + (c.kind == kAll3 ? 0 : (c.steps + 3) / 4);
             o.a_ent.resize(o.a_ent.size() + (size_t)nblk * 128, 0u);
             uint32_t *blk = o.a_ent.data() + (size_t)base * 4;
+            std::vector<std::vector<uint32_t>> lists((size_t)per_row);
+            if (c.kind != kAll3)
+                for (size_t i = 0; i < c.t.size(); ++i) {
+                    if (c.kind == kProd) {
+                        for (auto &e : c.t[i]->ent) lists[i].push_back(e.first);
+                    } else {
+                        split(c.t[i]->ent, w);
+                        for (auto &e : w) lists[i].push_back(enc(e));
+                    }
+                }
+            // blocks of four steps; the words behind the chunk's last step are never read
+            std::vector<int> pos;
+            const std::vector<uint32_t> grid = place(lists, width, c.kind == kAll3 ? 0 : c.steps, c.kind, true, &pos);
             for (int lane = 0; lane < 32; ++lane) {
-                const size_t sl = (size_t)lane / width;
-                uint32_t out = 0xFFFFFFFFu;
-                double cst = 0.0;
-                if (c.kind != kAll3 && sl < c.t.size()) { out = c.t[sl]->out; cst = c.t[sl]->cst; }
-                uint64_t bits;
-                std::memcpy(&bits, &cst, 8);
-                blk[(size_t)lane * 4 + 0] = out;
-                blk[(size_t)lane * 4 + 1] = (uint32_t)bits;
-                blk[(size_t)lane * 4 + 2] = (uint32_t)(bits >> 32);
+                blk[(size_t)lane * 4 + 0] = 0xFFFFFFFFu;
+                blk[(size_t)lane * 4 + 1] = 0u;
+                blk[(size_t)lane * 4 + 2] = 0u;
             }
+            if (c.kind != kAll3)
+                for (size_t i = 0; i < c.t.size(); ++i) {
+                    uint64_t bits;
+                    std::memcpy(&bits, &c.t[i]->cst, 8);
+                    for (int j = 0; j < width; ++j) {
+                        const size_t lane = (size_t)pos[i] * width + j;
+                        blk[lane * 4 + 0] = c.t[i]->out;
+                        blk[lane * 4 + 1] = (uint32_t)bits;
+                        blk[lane * 4 + 2] = (uint32_t)(bits >> 32);
+                    }
+                }
             o.n_a_steps_kind[c.kind] += c.steps;
             if (c.kind == kAll3) { o.n_a_steps += c.steps; continue; }
-            std::vector<std::vector<uint32_t>> lists((size_t)per_row);
-            for (size_t i = 0; i < c.t.size(); ++i) {
-                if (c.kind == kProd) {
-                    for (auto &e : c.t[i]->ent) lists[i].push_back(e.first);
-                } else {
-                    split(c.t[i]->ent, w);
-                    for (auto &e : w) lists[i].push_back(enc(e));
-                }
-            }
-            // blocks of four steps; the words behind the chunk's last step are never read
-            const std::vector<uint32_t> grid = place(lists, width, c.steps, c.kind);
             for (int lane = 0; lane < 32; ++lane)
                 for (int st = 0; st < c.steps; ++st)
                     blk[((size_t)(1 + st / 4) * 32 + lane) * 4 + st % 4] = grid[(size_t)lane * c.steps + st];
             o.n_a_steps += c.steps;
         }
         o.a_ent.resize(o.a_ent.size() + 128, 0u);        // the kernels read one block past a chunk's last
-        o.achunk.resize(o.achunk.size() + (size_t)2 * NW, 0u);      // ... and the headers one row ahead
+        o.achunk.resize(o.achunk.size() + (size_t)2 * 2 * NW, 0u);  // ... and the headers two rows ahead
     }
 
     // ---- phase B items: one per (slab, column); a lane's cells are rows rp * (32 slab + lane) .. + rp - 1.
@@ -816,8 +877,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                         nst = std::max(nst, (int)lists[lane].size());
                     }
                     REQUIRE(nst <= 3, "internal: a phase-B cell list is longer than three entries");
-                    const int run = nst == 0 ? 0 : nst == 1 ? 1 : 3;          // steps the kernel executes
-                    const std::vector<uint32_t> grid = place(lists, 1, std::max(run, 1), kSum1);
+                    const int run = nst == 0 ? 0 : nst == 1 ? 1 : 3;          // steps the kernel executes (1 or 3)
+                    const std::vector<uint32_t> grid = place(lists, 1, std::max(run, 1), kSum1, false, nullptr);
                     uint32_t *blk = o.b_ent.data() + (it * rp + h) * 128;
                     for (int lane = 0; lane < 32; ++lane) {
                         for (int st = 0; st < std::max(run, 1); ++st) blk[lane * 4 + st] = grid[(size_t)lane * std::max(run, 1) + st];
@@ -847,7 +908,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         auto bad = [](const char *wh) { throw Fail{PYJAC_ELIMIT, wh}; };
         const uint32_t e_total = (uint32_t)o.n_e;
         const size_t na_blocks = o.a_ent.size() / 4;
-        if (o.achunk.size() / 2 != (size_t)(o.n_arow + 1) * NW) bad("internal: phase A is not whole rows of chunks");
+        if (o.achunk.size() / 2 != (size_t)(o.n_arow + 2) * NW) bad("internal: phase A is not whole rows of chunks");
         for (size_t c = 0; c < (size_t)o.n_arow * NW; ++c) {
             const uint32_t base = o.achunk[2 * c], meta = o.achunk[2 * c + 1];
             const int steps = (int)(meta & 0xFF), kind = (int)((meta >> 8) & 0xF);

@@ -46,6 +46,8 @@ struct HostPack {
     long long n_cell_entries = 0, n_cells = 0, n_heavy_cells = 0, n_heavy_pieces = 0, n_a_steps = 0, n_b_steps = 0;
     long long n_plain_chunks = 0;
     long long n_a_steps_kind[4] = {0, 0, 0, 0};     // phase-A steps by chunk kind
+    long long n_conflict_wf[2] = {0, 0};            // shared-memory wavefronts beyond one per lane group and step that the
+                                                    // placement leaves (phase A, phase B; model of mech_pack.cu `place`)
 };
 
 // What the launch-shape choice may use (api.cu fills it from the device properties and the
