@@ -19,6 +19,10 @@
  *   - the dense analytical Jacobian d(dPhi/dt)/dPhi           PAPER.md:288-570 Eqs. 44-113,
  *     in the reaction-wise evaluation order of Section 4      PAPER.md:609-744 Alg. 2, Eqs. 115-130
  *
+ * Bench / test helpers (table statistics, machine-peak probes) are NOT part of this interface:
+ * they live in include/pyjac_b200_tools.h and a library of their own.  The library reads no
+ * environment variable; everything it does follows from the call arguments.
+ *
  * Conventions
  *   - Every function returns 0 (PYJAC_OK) or a negative error code; nothing throws or exits.
  *   - `pyjac_mech_desc` holds HOST pointers; the library copies what it needs during
@@ -113,12 +117,35 @@ typedef struct pyjac_mech pyjac_mech; /* opaque, owned by the library */
 
 /* Validates the description, sorts and packs it into device-resident SoA tables (precomputing
  * ln A, sum nu, the reaction-wise contribution lists of Algorithm 2) and
- * uploads them to CUDA device `device`.
+ * uploads them to CUDA device `device`.  The launch shape (states a CTA interleaves, threads per
+ * CTA, CTAs per SM) is chosen from the size of the per-state tables.
  * Errors: PYJAC_EINVAL (NULL pointers, counts < 0, indices out of range, nu outside 1..3, more than
  * 3 species on a side, A <= 0, non-ascending PLOG pressures, T_min >= T_max, ...), PYJAC_ELIMIT
- * (more than 65534 species, 65535 reactions or 65535 per-reaction derivative entries, or per-state
+ * (more than 65534 species, 65535 reactions or 65535 per-state table entries, or per-state
  * tables that exceed the 227 KB of shared memory of one CTA), PYJAC_ENOMEM, PYJAC_ECUDA. */
 int pyjac_mech_create(const pyjac_mech_desc *host_desc, int device, pyjac_mech **out);
+
+/* Launch shape of the evaluation kernels; 0 in a field = let the library choose.  The kernels
+ * evaluate `states_per_cta` states per CTA iteration, interleaved in shared memory (PAPER.md:857
+ * names cache capacity as what limits its one-thread-per-state layout; here the per-state
+ * reaction products stay in shared memory instead). */
+typedef struct pyjac_launch_shape {
+    int32_t states_per_cta; /* 1, 2, 3, 4 or 6 */
+    int32_t threads;        /* per CTA: a multiple of 32, at least 32 * states_per_cta, at most 512 */
+    int32_t ctas_per_sm;    /* resident CTAs the shared-memory footprint is sized for, 1..4 */
+    int32_t list_cap;       /* longest list one lane sums in the per-species / per-column phase; longer
+                               lists are shared by 2, 4, .. lanes and combined by warp shuffles */
+    int32_t cell_cap;       /* 1..3: longest contribution list of a Jacobian entry summed while the
+                               column is streamed out; longer lists are summed piecewise before */
+    int32_t rows_per_lane;  /* 1 or 2 Jacobian rows per lane in the streaming phase (2 needs N_sp odd,
+                               i.e. an even leading dimension; 16-byte stores) */
+} pyjac_launch_shape;
+
+/* As pyjac_mech_create with an explicit launch shape (tuning and tests; `shape` may be NULL).
+ * Every shape evaluates the same numbers up to the order of a sum.  PYJAC_EINVAL for a value out
+ * of range, PYJAC_ELIMIT if the shape does not fit the shared memory of one SM. */
+int pyjac_mech_create_shaped(const pyjac_mech_desc *host_desc, int device,
+                             const pyjac_launch_shape *shape, pyjac_mech **out);
 
 /* Frees the device tables.  NULL is a no-op returning PYJAC_OK. */
 int pyjac_mech_destroy(pyjac_mech *mech);
@@ -153,8 +180,10 @@ int pyjac_eval_jacobian(const pyjac_mech *mech, int64_t n, const double *T, cons
  * asynchronous; pageable memory works but serialises them).  The call copies the inputs to the
  * device, runs the same kernels as above in chunks of at most `chunk_states` states (<= 0: a
  * default sized to the device's free memory), copies the result back with copies of one chunk
- * overlapping the evaluation of the next, and returns after the last byte has arrived.  Device
- * staging buffers are allocated and freed inside the call. */
+ * overlapping the evaluation of the next, and returns after the last byte has arrived.  The two
+ * device staging buffers and the two streams are kept with the handle and reused by later calls
+ * (grown when a call needs more; freed by pyjac_mech_destroy); a second thread that calls while
+ * they are in use gets temporary ones. */
 int pyjac_eval_jacobian_host(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
                              const double *Y, int64_t ldy, double *jac, int64_t chunk_states);
 int pyjac_eval_dydt_host(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
@@ -168,25 +197,6 @@ int64_t pyjac_kernel_launches(void);
  * states.  Reported by bench.py next to the roofline numbers. */
 int pyjac_jacobian_launch_config(const pyjac_mech *mech, int64_t n, int32_t *threads,
                                  int32_t *smem_bytes, int32_t *ctas_per_sm, int32_t *grid);
-
-/* Host-only: validates and packs `host_desc` exactly as pyjac_mech_create does (no CUDA call) and
- * reports the size of the evaluation tables.  stats[0..11] = doubles of shared memory per state for
- * the per-reaction products and gathered sums (array E, without the tile), entries of all Jacobian
- * cell lists, gather steps of the cell chunks (32 lanes each), gather steps of the A1 chunks,
- * Jacobian cells with a gather task, gather chunks, shared-memory bytes of one CTA, groups of 32
- * reactions, states per CTA iteration (S), threads per CTA, column panels, columns per panel.
- * Errors as pyjac_mech_create (PYJAC_EINVAL, PYJAC_ELIMIT, PYJAC_ENOMEM). */
-int pyjac_pack_stats(const pyjac_mech_desc *host_desc, int64_t *stats);
-
-/* Machine peaks the roofline discussion refers to (bench.py --peaks), measured with
- * the same instructions the Jacobian kernel uses.  Device pointers, enqueued on `stream`, no allocation.
- *   pyjac_peak_store_stream: writes n_doubles (a multiple of 2) doubles of `buf` once with 16-byte
- *     streaming stores (st.global.cs.v2.f64), the store of the DENSE pass; bytes moved = 8 n_doubles.
- *   pyjac_peak_dfma: every thread of a full-occupancy grid runs 8 independent chains of `iters` fp64
- *     FMAs and writes one result per thread to out[0 .. *n_threads) (out must hold 148 * 2048 doubles
- *     at least; the thread count used is returned); flops = 2 * 8 * iters * *n_threads. */
-int pyjac_peak_store_stream(double *buf, int64_t n_doubles, void *stream);
-int pyjac_peak_dfma(double *out, int64_t iters, int64_t *n_threads, void *stream);
 
 /* Static, never-NULL description of an error code. */
 const char *pyjac_strerror(int code);

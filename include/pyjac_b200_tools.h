@@ -1,0 +1,52 @@
+/* pyjac_b200_tools.h -- bench / test helpers beside the product library (libpyjac_b200_tools.so).
+ *
+ * Nothing here is on the evaluation path of include/pyjac_b200.h: table statistics for the
+ * design notes and the host-side tests, and the two machine-peak probes the roofline discussion
+ * refers to (`bench.py --peaks`).
+ */
+#ifndef PYJAC_B200_TOOLS_H
+#define PYJAC_B200_TOOLS_H
+
+#include "pyjac_b200.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PYJAC_TOOLS_NSTATS 24
+
+/* Host-only: validates and packs `host_desc` exactly as pyjac_mech_create_shaped does (no CUDA
+ * call, the same self-check of everything the kernels read without bounds checks) and reports the
+ * size of the evaluation tables.  stats[0..23] =
+ *   0 elements of the per-state array E      1 entries of all Jacobian cell lists
+ *   2 gather steps of the streaming phase    3 gather steps of the summing phase
+ *   4 Jacobian cells with a list             5 chunks of the summing phase
+ *   6 shared-memory bytes of one CTA         7 groups of 32 reactions
+ *   8 states per CTA iteration               9 threads per CTA
+ *  10 reserved (1)                          11 CTAs per SM the footprint is sized for
+ *  12 cells summed piecewise                13 pieces
+ *  14 bytes of the summing-phase tables     15 bytes of the streaming-phase tables
+ *  16..19 summing-phase steps by kind (three sums at once, one sum, products, all reactions)
+ *  20, 21 shared-memory wavefronts beyond the minimum that the entry placement leaves, per CTA
+ *         iteration (summing phase, streaming phase; the bank model of mech_pack.cu)
+ *  22, 23 reserved (0)
+ * Errors as pyjac_mech_create_shaped (PYJAC_EINVAL, PYJAC_ELIMIT, PYJAC_ENOMEM). */
+int pyjac_tools_pack_stats(const pyjac_mech_desc *host_desc, const pyjac_launch_shape *shape,
+                           int64_t *stats);
+
+/* Machine peaks measured with the same instructions the Jacobian kernel uses.  Device pointers,
+ * enqueued on `stream` (a cudaStream_t), no allocation.
+ *   pyjac_tools_peak_store_stream: writes n_doubles (a multiple of 2) doubles of `buf` once with
+ *     16-byte streaming stores (st.global.cs.v2.f64), the store of the streaming phase; bytes
+ *     moved = 8 n_doubles.
+ *   pyjac_tools_peak_dfma: every thread of a full-occupancy grid runs 8 independent chains of
+ *     `iters` fp64 FMAs and writes one result per thread to out[0 .. *n_threads) (out must hold
+ *     148 * 2048 doubles at least; the thread count used is returned); flops = 2 * 8 * iters *
+ *     *n_threads. */
+int pyjac_tools_peak_store_stream(double *buf, int64_t n_doubles, void *stream);
+int pyjac_tools_peak_dfma(double *out, int64_t iters, int64_t *n_threads, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYJAC_B200_TOOLS_H */

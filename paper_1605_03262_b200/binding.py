@@ -15,6 +15,7 @@ from .mechanism import Mechanism
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpyjac_b200.so")
+TOOLS_LIB_PATH = os.path.join(_HERE, "libpyjac_b200_tools.so")     # include/pyjac_b200_tools.h: bench / test helpers
 
 PYJAC_OK, PYJAC_EINVAL, PYJAC_ENOMEM, PYJAC_ECUDA, PYJAC_ELIMIT = 0, -1, -2, -3, -4
 
@@ -37,12 +38,19 @@ class MechDesc(C.Structure):
                 ("cheb_lim", _pd), ("cheb_eta", _pd)]
 
 
-EXPORTS = ("pyjac_mech_create", "pyjac_mech_destroy", "pyjac_mech_sizes", "pyjac_eval_rates",
-           "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
-           "pyjac_eval_dydt_host", "pyjac_kernel_launches", "pyjac_jacobian_launch_config",
-           "pyjac_pack_stats", "pyjac_peak_store_stream", "pyjac_peak_dfma", "pyjac_strerror")
+class LaunchShape(C.Structure):
+    """struct pyjac_launch_shape (0 = let the library choose)"""
+    _fields_ = [("states_per_cta", C.c_int32), ("threads", C.c_int32), ("ctas_per_sm", C.c_int32),
+                ("list_cap", C.c_int32), ("cell_cap", C.c_int32), ("rows_per_lane", C.c_int32)]
+
+
+EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_sizes",
+           "pyjac_eval_rates", "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
+           "pyjac_eval_dydt_host", "pyjac_kernel_launches", "pyjac_jacobian_launch_config", "pyjac_strerror")
+TOOLS_EXPORTS = ("pyjac_tools_pack_stats", "pyjac_tools_peak_store_stream", "pyjac_tools_peak_dfma")
 
 _lib = None
+_tools = None
 
 
 def load_library(path: str | None = None):
@@ -57,6 +65,7 @@ def load_library(path: str | None = None):
     lib = C.CDLL(p)
     vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
     lib.pyjac_mech_create.argtypes = [C.POINTER(MechDesc), C.c_int, C.POINTER(vp)]
+    lib.pyjac_mech_create_shaped.argtypes = [C.POINTER(MechDesc), C.c_int, C.POINTER(LaunchShape), C.POINTER(vp)]
     lib.pyjac_mech_destroy.argtypes = [vp]
     lib.pyjac_mech_sizes.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     lib.pyjac_eval_rates.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp]
@@ -67,9 +76,6 @@ def load_library(path: str | None = None):
     lib.pyjac_kernel_launches.argtypes = []
     lib.pyjac_kernel_launches.restype = i64
     lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 4
-    lib.pyjac_pack_stats.argtypes = [C.POINTER(MechDesc), C.POINTER(i64)]
-    lib.pyjac_peak_store_stream.argtypes = [vp, i64, vp]
-    lib.pyjac_peak_dfma.argtypes = [vp, i64, C.POINTER(i64), vp]
     lib.pyjac_strerror.argtypes = [C.c_int]
     lib.pyjac_strerror.restype = C.c_char_p
     for name in EXPORTS:
@@ -77,6 +83,26 @@ def load_library(path: str | None = None):
             getattr(lib, name).restype = C.c_int
     if path is None:
         _lib = lib
+    return lib
+
+
+def load_tools(path: str | None = None):
+    """Loads libpyjac_b200_tools.so (table statistics, machine-peak probes; not the product)."""
+    global _tools
+    if _tools is not None and path is None:
+        return _tools
+    p = path or TOOLS_LIB_PATH
+    if not os.path.exists(p):
+        raise RuntimeError("%s is missing: run `python -m paper_1605_03262_b200.build`" % p)
+    lib = C.CDLL(p)
+    vp, i64 = C.c_void_p, C.c_int64
+    lib.pyjac_tools_pack_stats.argtypes = [C.POINTER(MechDesc), C.POINTER(LaunchShape), C.POINTER(i64)]
+    lib.pyjac_tools_peak_store_stream.argtypes = [vp, i64, vp]
+    lib.pyjac_tools_peak_dfma.argtypes = [vp, i64, C.POINTER(i64), vp]
+    for name in TOOLS_EXPORTS:
+        getattr(lib, name).restype = C.c_int
+    if path is None:
+        _tools = lib
     return lib
 
 
@@ -115,41 +141,59 @@ def mech_desc(mech: Mechanism):
     return d, keep
 
 
-PACK_STAT_NAMES = ("e_doubles", "cell_entries", "b_steps", "a_steps", "cells", "chunks",
-                   "smem_bytes_per_cta", "reaction_chunks", "states_per_block", "threads", "blocks_per_cta",
+def launch_shape(shape):
+    """None, a LaunchShape or a dict with the fields of `pyjac_launch_shape` -> LaunchShape or None."""
+    if shape is None or isinstance(shape, LaunchShape):
+        return shape
+    unknown = set(shape) - {f[0] for f in LaunchShape._fields_}
+    if unknown:
+        raise ValueError("unknown launch-shape fields: %s" % sorted(unknown))
+    return LaunchShape(**{k: int(v) for k, v in shape.items()})
+
+
+PACK_STAT_NAMES = ("e_elements", "cell_entries", "b_steps", "a_steps", "cells", "chunks",
+                   "smem_bytes_per_cta", "reaction_groups", "states_per_cta", "threads", "reserved10",
                    "ctas_per_sm_target", "heavy_cells", "heavy_pieces", "a_table_bytes", "b_table_bytes",
-                   "a_steps_sum3", "a_steps_sum1", "a_steps_prod", "a_steps_all3", "a_conflict_wf", "b_conflict_wf")
+                   "a_steps_sum3", "a_steps_sum1", "a_steps_prod", "a_steps_all3", "a_conflict_wf", "b_conflict_wf",
+                   "reserved22", "reserved23")
 
 
-def pack_stats(mech: Mechanism) -> dict:
-    """Host-only: sizes of the evaluation tables `pyjac_mech_create` would build (no CUDA call)."""
-    lib = load_library()
+def pack_stats(mech: Mechanism, shape=None) -> dict:
+    """Host-only (tools library): sizes of the evaluation tables `pyjac_mech_create_shaped` would build."""
+    lib = load_tools()
     d, keep = mech_desc(mech)
-    out = (C.c_int64 * 22)()
-    _check(lib.pyjac_pack_stats(C.byref(d), out), "pyjac_pack_stats")
+    out = (C.c_int64 * len(PACK_STAT_NAMES))()
+    sh = launch_shape(shape)
+    _check(lib.pyjac_tools_pack_stats(C.byref(d), C.byref(sh) if sh is not None else None, out), "pyjac_tools_pack_stats")
     return dict(zip(PACK_STAT_NAMES, [int(v) for v in out]))
 
 
 def peak_store_stream(buf, stream_ptr):
-    """Enqueues one write-only pass over the CUDA float64 tensor `buf` (pyjac_peak_store_stream)."""
-    _check(load_library().pyjac_peak_store_stream(buf.data_ptr(), int(buf.numel()), stream_ptr), "pyjac_peak_store_stream")
+    """Enqueues one write-only pass over the CUDA float64 tensor `buf` (pyjac_tools_peak_store_stream)."""
+    _check(load_tools().pyjac_tools_peak_store_stream(buf.data_ptr(), int(buf.numel()), stream_ptr),
+           "pyjac_tools_peak_store_stream")
 
 
 def peak_dfma(out, iters, stream_ptr):
-    """Enqueues the fp64 FMA probe (pyjac_peak_dfma); returns the flops it executes."""
+    """Enqueues the fp64 FMA probe (pyjac_tools_peak_dfma); returns the flops it executes."""
     n = C.c_int64()
-    _check(load_library().pyjac_peak_dfma(out.data_ptr(), int(iters), C.byref(n), stream_ptr), "pyjac_peak_dfma")
+    _check(load_tools().pyjac_tools_peak_dfma(out.data_ptr(), int(iters), C.byref(n), stream_ptr), "pyjac_tools_peak_dfma")
     return 2 * 8 * int(iters) * n.value
 
 
 class PyJac:
     """A kinetic model resident on one CUDA device (wraps `pyjac_mech*`)."""
 
-    def __init__(self, mech: Mechanism, device: int = 0):
+    def __init__(self, mech: Mechanism, device: int = 0, shape=None):
         self.lib = load_library()
         d, keep = mech_desc(mech)
         h = C.c_void_p()
-        _check(self.lib.pyjac_mech_create(C.byref(d), int(device), C.byref(h)), "pyjac_mech_create")
+        sh = launch_shape(shape)
+        if sh is None:
+            _check(self.lib.pyjac_mech_create(C.byref(d), int(device), C.byref(h)), "pyjac_mech_create")
+        else:
+            _check(self.lib.pyjac_mech_create_shaped(C.byref(d), int(device), C.byref(sh), C.byref(h)),
+                   "pyjac_mech_create_shaped")
         self._h = h
         self.device = int(device)
         ns, nr = C.c_int32(), C.c_int32()
@@ -175,9 +219,14 @@ class PyJac:
                 raise TypeError("T, P, Y must be float64 CUDA tensors")
         if Y.dim() != 2 or Y.stride(1) != 1 or not T.is_contiguous() or not P.is_contiguous():
             raise ValueError("Y must be [n][>=Nsp] with unit inner stride; T, P contiguous")
+        if any(t.device.index != self.device for t in (T, P, Y)):
+            raise ValueError("T, P, Y must live on the handle's device (cuda:%d)" % self.device)
         n = T.numel()
         if P.numel() != n or Y.shape[0] != n or Y.shape[1] < self.ns:
             raise ValueError("inconsistent state arrays")
+        import torch
+        if torch.cuda.current_device() != self.device:
+            raise ValueError("the current CUDA device (whose stream the call is enqueued on) is not cuda:%d" % self.device)
         ldy = Y.stride(0) if n > 1 else max(Y.shape[1], self.ns)
         return n, ldy
 
@@ -185,6 +234,18 @@ class PyJac:
     def _stream():
         import torch
         return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+    def _dev_out(self, out, n, per_state, like):
+        """A caller's output tensor is written in place: it must be a contiguous float64 CUDA tensor on the
+        handle's device with at least n * per_state elements (nothing is ever copied or converted)."""
+        import torch
+        if out is None:
+            return torch.empty((n, per_state), dtype=torch.float64, device=like.device)
+        if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.is_contiguous()
+                and out.device.index == self.device and out.numel() >= n * per_state):
+            raise ValueError("out must be a contiguous float64 CUDA tensor on cuda:%d with at least %d elements"
+                             % (self.device, n * per_state))
+        return out
 
     # ---- device-pointer calls (enqueue on torch's current stream)
     def eval_rates(self, T, P, Y, want=("rf", "rr", "cmod", "wdot")):
@@ -206,8 +267,7 @@ class PyJac:
         """[n][Nsp+1] source term (pyjac_eval_dydt)."""
         import torch
         n, ldy = self._dev_inputs(T, P, Y)
-        if out is None:
-            out = torch.empty((n, self.ns + 1), dtype=torch.float64, device=T.device)
+        out = self._dev_out(out, n, self.ns + 1, T)
         _check(self.lib.pyjac_eval_dydt(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
                                         out.data_ptr(), self._stream()), "pyjac_eval_dydt")
         return out
@@ -217,40 +277,57 @@ class PyJac:
         import torch
         n, ldy = self._dev_inputs(T, P, Y)
         ld = self.ns + 1
-        if out is None:
-            out = torch.empty((n, ld * ld), dtype=torch.float64, device=T.device)
-        elif out.numel() < n * ld * ld or not out.is_contiguous():
-            raise ValueError("output buffer too small or not contiguous")
+        out = self._dev_out(out, n, ld * ld, T)
         _check(self.lib.pyjac_eval_jacobian(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
                                             out.data_ptr(), self._stream()), "pyjac_eval_jacobian")
         return out
 
     # ---- host-pointer calls (copies inside; synchronous)
     @staticmethod
-    def _host_ptr(a):
+    def _host_in(a):
+        """Host input: a CPU float64 torch tensor or anything numpy can view as C-contiguous float64 (inputs
+        may be converted; the converted copy is kept alive for the call)."""
         import torch
         if isinstance(a, torch.Tensor):
-            assert not a.is_cuda and a.dtype == torch.float64 and a.is_contiguous()
+            if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous():
+                raise ValueError("host inputs must be contiguous float64 CPU tensors")
             return a.data_ptr(), a
         a = np.ascontiguousarray(a, dtype=np.float64)
         return a.ctypes.data, a
 
-    def eval_jacobian_host(self, T, P, Y, out, chunk_states: int = 0):
-        """Host buffers in, host buffer out (numpy arrays or CPU torch tensors, pinned or not)."""
-        (pT, kT), (pP, kP), (pY, kY), (pO, kO) = map(self._host_ptr, (T, P, Y, out))
+    @staticmethod
+    def _host_out(a, n_elements):
+        """Host output, written in place: never copied or converted, so it must already be C-contiguous float64
+        with room for the result."""
+        import torch
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous() or a.numel() < n_elements:
+                raise ValueError("out must be a contiguous float64 CPU tensor with at least %d elements" % n_elements)
+            return a.data_ptr()
+        if not (isinstance(a, np.ndarray) and a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+                and a.flags["WRITEABLE"] and a.size >= n_elements):
+            raise ValueError("out must be a writeable C-contiguous float64 numpy array with at least %d elements"
+                             % n_elements)
+        return a.ctypes.data
+
+    def _host_call(self, fn, what, T, P, Y, out, per_state, chunk_states):
+        (pT, kT), (pP, kP), (pY, kY) = map(self._host_in, (T, P, Y))
         n = int(kT.shape[0])
-        ldy = int(kY.shape[1])
-        _check(self.lib.pyjac_eval_jacobian_host(self._h, n, pT, pP, pY, ldy, pO, int(chunk_states)),
-               "pyjac_eval_jacobian_host")
+        if kY.ndim != 2 or int(kY.shape[0]) != n or int(kP.shape[0]) != n or int(kY.shape[1]) < self.ns:
+            raise ValueError("inconsistent state arrays")
+        pO = self._host_out(out, n * per_state)
+        _check(fn(self._h, n, pT, pP, pY, int(kY.shape[1]), pO, int(chunk_states)), what)
         return out
 
+    def eval_jacobian_host(self, T, P, Y, out, chunk_states: int = 0):
+        """Host buffers in, host buffer out (numpy arrays or CPU torch tensors, pinned or not)."""
+        ld = self.ns + 1
+        return self._host_call(self.lib.pyjac_eval_jacobian_host, "pyjac_eval_jacobian_host", T, P, Y, out, ld * ld,
+                               chunk_states)
+
     def eval_dydt_host(self, T, P, Y, out, chunk_states: int = 0):
-        (pT, kT), (pP, kP), (pY, kY), (pO, kO) = map(self._host_ptr, (T, P, Y, out))
-        n = int(kT.shape[0])
-        ldy = int(kY.shape[1])
-        _check(self.lib.pyjac_eval_dydt_host(self._h, n, pT, pP, pY, ldy, pO, int(chunk_states)),
-               "pyjac_eval_dydt_host")
-        return out
+        return self._host_call(self.lib.pyjac_eval_dydt_host, "pyjac_eval_dydt_host", T, P, Y, out, self.ns + 1,
+                               chunk_states)
 
     def launch_config(self, n: int):
         v = [C.c_int32() for _ in range(4)]

@@ -1,4 +1,5 @@
-"""Builds the C-ABI CUDA library in-tree: paper_1605_03262_b200/libpyjac_b200.so (sm_100a only).
+"""Builds the C-ABI CUDA library in-tree: paper_1605_03262_b200/libpyjac_b200.so (sm_100a only), and the
+bench / test helper library libpyjac_b200_tools.so beside it (include/pyjac_b200_tools.h).
 
     python -m paper_1605_03262_b200.build [--force] [--verbose]
 
@@ -16,10 +17,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libpyjac_b200.so")
-HOST_SOURCES = ["api.cu", "mech_pack.cu", "dispatch.cu"]
+TOOLS_SO = os.path.join(HERE, "libpyjac_b200_tools.so")          # bench / test helpers, not the product
+HOST_SOURCES = ["api.cu", "mech_pack.cu", "dispatch.cu", "tools.cu"]
 # states a CTA interleaves per iteration -- keep in step with csrc/dispatch.cu
 KERNEL_S = [1, 2, 3, 4, 6]
-HEADERS = ["device_mech.h", "kernels.h", "mech_pack.h", os.path.join("..", "..", "include", "pyjac_b200.h")]
+HEADERS = ["device_mech.h", "kernels.h", "mech_pack.h", os.path.join("..", "..", "include", "pyjac_b200.h"),
+           os.path.join("..", "..", "include", "pyjac_b200_tools.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC"]
 
@@ -32,7 +35,7 @@ def _nvcc() -> str:
 
 
 def is_stale() -> bool:
-    if not os.path.exists(SO):
+    if not os.path.exists(SO) or not os.path.exists(TOOLS_SO):
         return True
     t = os.path.getmtime(SO)
     deps = [os.path.join(CSRC, f) for f in HOST_SOURCES + ["kernels.cu"] + HEADERS] + [os.path.abspath(__file__)]
@@ -65,12 +68,16 @@ def build(force: bool = False, verbose: bool = False) -> str:
         failed = failed or res.returncode != 0
     if failed:
         raise RuntimeError("nvcc failed building %s" % SO)
-    link = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + [j[0] for j in jobs] + ["-o", SO]
-    res = subprocess.run(link, cwd=CSRC, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
-        raise RuntimeError("link failed for %s" % SO)
+    objs = [j[0] for j in jobs]
+    tools_obj = os.path.join(OBJ, "tools.o")
+    pack_obj = os.path.join(OBJ, "mech_pack.o")
+    for so, parts in ((SO, [o for o in objs if o != tools_obj]), (TOOLS_SO, [tools_obj, pack_obj])):
+        link = [_nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a"] + parts + ["-o", so]
+        res = subprocess.run(link, cwd=CSRC, capture_output=True, text=True)
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        if res.returncode != 0:
+            raise RuntimeError("link failed for %s" % so)
     return SO
 
 

@@ -25,7 +25,13 @@ struct pyjac_mech {
     size_t smem[3] = {0, 0, 0}; // dynamic shared memory per level
     int ctas_per_sm[3] = {1, 1, 1};
     int n_sm = 1;
-    long long stats[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    // staging of the *_host calls: two device buffer pairs and two streams, kept between calls.  The handle
+    // is otherwise immutable; this part is guarded by `ws_busy` (a caller that finds it taken stages with
+    // temporary buffers instead).
+    mutable std::atomic_flag ws_busy = ATOMIC_FLAG_INIT;
+    mutable double *ws_in[2] = {nullptr, nullptr}, *ws_out[2] = {nullptr, nullptr};
+    mutable size_t ws_in_cap = 0, ws_out_cap = 0;          // doubles per buffer
+    mutable cudaStream_t ws_stream[2] = {nullptr, nullptr};
 };
 
 namespace {
@@ -44,23 +50,6 @@ struct Uploader {
         fix.push_back({(const void **)field, off});
     }
 };
-
-// Tuning hooks, read at pyjac_mech_create / pyjac_pack_stats: PYJAC_S, PYJAC_THREADS,
-// PYJAC_CTAS override the launch shape mech_pack.cu would choose, PYJAC_CAP / PYJAC_CELL_CAP the list
-// lengths of phases A / B, PYJAC_RP the rows per lane of phase B; a value that is not instantiated or
-// does not fit is an error at create.
-ShapeHints hints_from_env(long long smem_optin)
-{
-    ShapeHints h;
-    if (smem_optin > 0) h.smem_bytes = smem_optin - 128;
-    if (const char *e = std::getenv("PYJAC_S")) h.S = std::atoi(e);
-    if (const char *e = std::getenv("PYJAC_THREADS")) h.threads = std::atoi(e);
-    if (const char *e = std::getenv("PYJAC_CTAS")) h.ctas = std::atoi(e);
-    if (const char *e = std::getenv("PYJAC_CAP")) h.cap = std::atoi(e);
-    if (const char *e = std::getenv("PYJAC_CELL_CAP")) h.cell_cap = std::atoi(e);
-    if (const char *e = std::getenv("PYJAC_RP")) h.rp = std::atoi(e);
-    return h;
-}
 
 int check_eval_args(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
                     int64_t ldy)
@@ -95,13 +84,18 @@ extern "C" {
 
 int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
 {
+    return pyjac_mech_create_shaped(d, device, nullptr, out);
+}
+
+int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_launch_shape *shape, pyjac_mech **out)
+{
     if (!out) return PYJAC_EINVAL;
     *out = nullptr;
     // validate and pack first (no CUDA call yet) with the architecture's shared-memory size; the
     // real device's limit is checked below
     HostPack hp;
     const char *why = nullptr;
-    int rc = pack_mechanism(d, hp, hints_from_env(227 * 1024), &why);
+    int rc = pack_mechanism(d, hp, hints_from_shape(shape, 227 * 1024), &why);
     if (rc != PYJAC_OK) return rc;
     int prev = -1;
     cudaDeviceProp prop{};
@@ -160,9 +154,6 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
     if (rc == PYJAC_OK) {
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
         m->plan = make_smem_plan(hp.ns, hp.n_e);
-        m->stats[0] = hp.n_e; m->stats[1] = hp.n_cell_entries; m->stats[2] = hp.n_b_steps;
-        m->stats[3] = hp.n_a_steps; m->stats[4] = hp.n_cells; m->stats[5] = (long long)hp.achunk.size() / 2;
-        m->stats[6] = hp.n_heavy_cells; m->stats[7] = hp.n_heavy_pieces;
         const size_t bytes = eval_smem_bytes(m->plan, m->S);
         if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->S)) {
             rc = PYJAC_ELIMIT;
@@ -170,7 +161,6 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
             // shared-memory carve-out: what the CTAs this shape was sized for need, the rest of the 256 KB
             // stays L1 (the gather tables are re-read from L1 / L2 by every CTA iteration)
             int carveout = (int)((100 * ((long long)hp.ctas_target * (long long)(bytes + 1024 + 16)) + 228 * 1024 - 1) / (228 * 1024));
-            if (const char *e = std::getenv("PYJAC_CARVEOUT")) carveout = std::atoi(e);
             carveout = carveout > 100 ? 100 : carveout < 0 ? 0 : carveout;
             for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
                 m->smem[level] = bytes;
@@ -207,6 +197,11 @@ int pyjac_mech_destroy(pyjac_mech *m)
     cudaGetDevice(&prev);
     cudaSetDevice(m->device);
     cudaError_t e = cudaFree(m->blob);
+    for (int b = 0; b < 2; ++b) {
+        if (m->ws_stream[b]) cudaStreamDestroy(m->ws_stream[b]);
+        if (m->ws_in[b]) cudaFree(m->ws_in[b]);
+        if (m->ws_out[b]) cudaFree(m->ws_out[b]);
+    }
     if (prev >= 0) cudaSetDevice(prev);
     delete m;
     return e == cudaSuccess ? PYJAC_OK : PYJAC_ECUDA;
@@ -264,50 +259,6 @@ int pyjac_jacobian_launch_config(const pyjac_mech *m, int64_t n, int32_t *thread
     return PYJAC_OK;
 }
 
-int pyjac_pack_stats(const pyjac_mech_desc *d, int64_t *stats)
-{
-    if (!stats) return PYJAC_EINVAL;
-    HostPack hp;
-    const int rc = pack_mechanism(d, hp, hints_from_env(227 * 1024), nullptr);
-    if (rc != PYJAC_OK) return rc;
-    const SmemPlan plan = make_smem_plan(hp.ns, hp.n_e);
-    stats[0] = hp.n_e; stats[1] = hp.n_cell_entries; stats[2] = hp.n_b_steps; stats[3] = hp.n_a_steps;
-    stats[4] = hp.n_cells; stats[5] = (int64_t)hp.achunk.size() / 2; stats[6] = (int64_t)eval_smem_bytes(plan, hp.S);
-    stats[7] = hp.n_rchunk; stats[8] = hp.S; stats[9] = hp.threads; stats[10] = 1; stats[11] = hp.ctas_target;
-    stats[12] = hp.n_heavy_cells; stats[13] = hp.n_heavy_pieces; stats[14] = (int64_t)hp.a_ent.size() * 4;
-    stats[15] = (int64_t)hp.b_ent.size() * 4;
-    for (int k = 0; k < 4; ++k) stats[16 + k] = hp.n_a_steps_kind[k];
-    stats[20] = hp.n_conflict_wf[0]; stats[21] = hp.n_conflict_wf[1];
-    return PYJAC_OK;
-}
-
-int pyjac_peak_store_stream(double *buf, int64_t n_doubles, void *stream)
-{
-    if (!buf || n_doubles < 2 || (n_doubles & 1) || (reinterpret_cast<uintptr_t>(buf) & 15)) return PYJAC_EINVAL;
-    int dev = 0, n_sm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-        return PYJAC_ECUDA;
-    const cudaError_t e = launch_peak_store(buf, n_doubles, n_sm * 8, (cudaStream_t)stream);
-    if (e != cudaSuccess) return PYJAC_ECUDA;
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return PYJAC_OK;
-}
-
-int pyjac_peak_dfma(double *out, int64_t iters, int64_t *n_threads, void *stream)
-{
-    if (!out || iters < 1 || !n_threads) return PYJAC_EINVAL;
-    int dev = 0, n_sm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-        return PYJAC_ECUDA;
-    *n_threads = (int64_t)n_sm * 2048;
-    const cudaError_t e = launch_peak_dfma(out, iters, n_sm * 8, (cudaStream_t)stream);
-    if (e != cudaSuccess) return PYJAC_ECUDA;
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return PYJAC_OK;
-}
-
 const char *pyjac_strerror(int code)
 {
     switch (code) {
@@ -352,12 +303,34 @@ int eval_host(const pyjac_mech *m, int level, int64_t n, const double *T, const 
     double *din[2] = {nullptr, nullptr}, *dout[2] = {nullptr, nullptr};
     cudaStream_t st[2] = {nullptr, nullptr};
     rc = PYJAC_OK;
-    for (int b = 0; b < 2 && rc == PYJAC_OK; ++b) {
-        if (cudaMalloc(&din[b], C * in_per * sizeof(double)) != cudaSuccess ||
-            cudaMalloc(&dout[b], C * out_per * sizeof(double)) != cudaSuccess)
-            rc = PYJAC_ENOMEM;
-        else if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess)
-            rc = PYJAC_ECUDA;
+    // the handle's staging buffers if nobody else is using them (grown on demand), else temporary ones
+    const bool cached = !m->ws_busy.test_and_set(std::memory_order_acquire);
+    if (cached) {
+        for (int b = 0; b < 2 && rc == PYJAC_OK; ++b)
+            if (!m->ws_stream[b] && cudaStreamCreateWithFlags(&m->ws_stream[b], cudaStreamNonBlocking) != cudaSuccess)
+                rc = PYJAC_ECUDA;
+        if (rc == PYJAC_OK && (m->ws_in_cap < C * in_per || m->ws_out_cap < C * out_per)) {
+            for (int b = 0; b < 2; ++b) {
+                if (m->ws_in[b]) cudaFree(m->ws_in[b]);
+                if (m->ws_out[b]) cudaFree(m->ws_out[b]);
+                m->ws_in[b] = m->ws_out[b] = nullptr;
+            }
+            m->ws_in_cap = m->ws_out_cap = 0;
+            for (int b = 0; b < 2 && rc == PYJAC_OK; ++b)
+                if (cudaMalloc(&m->ws_in[b], C * in_per * sizeof(double)) != cudaSuccess ||
+                    cudaMalloc(&m->ws_out[b], C * out_per * sizeof(double)) != cudaSuccess)
+                    rc = PYJAC_ENOMEM;
+            if (rc == PYJAC_OK) { m->ws_in_cap = C * in_per; m->ws_out_cap = C * out_per; }
+        }
+        for (int b = 0; b < 2; ++b) { din[b] = m->ws_in[b]; dout[b] = m->ws_out[b]; st[b] = m->ws_stream[b]; }
+    } else {
+        for (int b = 0; b < 2 && rc == PYJAC_OK; ++b) {
+            if (cudaMalloc(&din[b], C * in_per * sizeof(double)) != cudaSuccess ||
+                cudaMalloc(&dout[b], C * out_per * sizeof(double)) != cudaSuccess)
+                rc = PYJAC_ENOMEM;
+            else if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess)
+                rc = PYJAC_ECUDA;
+        }
     }
     int b = 0;
     for (int64_t s0 = 0; s0 < n && rc == PYJAC_OK; s0 += chunk_states, b ^= 1) {
@@ -377,13 +350,14 @@ int eval_host(const pyjac_mech *m, int level, int64_t n, const double *T, const 
         if (e != cudaSuccess) { rc = PYJAC_ECUDA; break; }
     }
     for (int q = 0; q < 2; ++q) {
-        if (st[q]) {
-            if (cudaStreamSynchronize(st[q]) != cudaSuccess && rc == PYJAC_OK) rc = PYJAC_ECUDA;
-            cudaStreamDestroy(st[q]);
+        if (st[q] && cudaStreamSynchronize(st[q]) != cudaSuccess && rc == PYJAC_OK) rc = PYJAC_ECUDA;
+        if (!cached) {
+            if (st[q]) cudaStreamDestroy(st[q]);
+            if (din[q]) cudaFree(din[q]);
+            if (dout[q]) cudaFree(dout[q]);
         }
-        if (din[q]) cudaFree(din[q]);
-        if (dout[q]) cudaFree(dout[q]);
     }
+    if (cached) m->ws_busy.clear(std::memory_order_release);
     if (rc != PYJAC_OK) cudaGetLastError();
     cudaSetDevice(prev);
     return rc;

@@ -14,40 +14,6 @@ namespace pyjac {
 PYJAC_FOR_S(PYJAC_DECL)
 #undef PYJAC_DECL
 
-namespace {
-
-__global__ void __launch_bounds__(256) peak_store_kernel(double *buf, long long n_pairs)
-{
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_pairs; i += stride)
-        asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(buf + 2 * i), "d"((double)i), "d"(1.0) : "memory");
-}
-
-__global__ void __launch_bounds__(256) peak_dfma_kernel(double *out, long long iters)
-{
-    const double x = 1.0 + 1e-9 * threadIdx.x, y = 1e-12 * blockIdx.x;
-    double a0 = 0.1, a1 = 0.2, a2 = 0.3, a3 = 0.4, a4 = 0.5, a5 = 0.6, a6 = 0.7, a7 = 0.8;
-    for (long long i = 0; i < iters; ++i) {
-        a0 = fma(a0, x, y); a1 = fma(a1, x, y); a2 = fma(a2, x, y); a3 = fma(a3, x, y);
-        a4 = fma(a4, x, y); a5 = fma(a5, x, y); a6 = fma(a6, x, y); a7 = fma(a7, x, y);
-    }
-    out[(long long)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
-}
-
-}  // namespace
-
-cudaError_t launch_peak_store(double *buf, long long n_doubles, int grid, cudaStream_t stream)
-{
-    peak_store_kernel<<<grid, 256, 0, stream>>>(buf, n_doubles / 2);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_peak_dfma(double *out, long long iters, int grid, cudaStream_t stream)
-{
-    peak_dfma_kernel<<<grid, 256, 0, stream>>>(out, iters);
-    return cudaGetLastError();
-}
-
 size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + (size_t)sp.shared_total) * sizeof(double); }
 
 const void *eval_kernel_ptr(int level, int S)

@@ -22,9 +22,4 @@ cudaError_t launch_eval(int level, int threads, int S, const DeviceMech &m, cons
                         long long n, const double *T, const double *P, const double *Y, long long ldy,
                         const EvalOut &out, cudaStream_t stream);
 
-// peak probes (dispatch.cu): a write-only stream of 16-byte streaming stores; 8 independent DFMA chains
-// per thread, 256 threads per CTA
-cudaError_t launch_peak_store(double *buf, long long n_doubles, int grid, cudaStream_t stream);
-cudaError_t launch_peak_dfma(double *out, long long iters, int grid, cudaStream_t stream);
-
 }  // namespace pyjac

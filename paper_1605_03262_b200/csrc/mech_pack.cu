@@ -538,7 +538,10 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
 
     // ---- long cell lists are summed piecewise in phase A (balanced over the lanes: lists sorted by
     // length); phase B then reads at most `cell_cap` entries per cell, all lanes of a warp alike
-    const int cell_cap = hints.cell_cap >= 1 && hints.cell_cap <= 3 ? hints.cell_cap : 3;
+    REQUIRE(hints.cell_cap >= 0 && hints.cell_cap <= 3, "cell_cap must be 0 (choose) or 1..3");
+    REQUIRE(hints.cap >= 0 && hints.rp >= 0 && hints.rp <= 2 && hints.ctas >= 0 && hints.ctas <= 4 && hints.threads >= 0 && hints.S >= 0,
+            "launch shape out of range");
+    const int cell_cap = hints.cell_cap >= 1 ? hints.cell_cap : 3;
     constexpr int kPiece = 8;
     std::vector<std::vector<std::pair<uint32_t, int>>> cell_w((size_t)ld * ld);
     {
@@ -939,6 +942,17 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         }
         if (o.bsplit[0] != 0 || o.bsplit[NW] != o.n_slab * ld) bad("internal: phase B ranges do not cover the items");
     }
+}
+
+ShapeHints hints_from_shape(const pyjac_launch_shape *shape, long long smem_optin)
+{
+    ShapeHints h;
+    if (smem_optin > 0) h.smem_bytes = smem_optin - 128;
+    if (shape) {
+        h.S = shape->states_per_cta; h.threads = shape->threads; h.ctas = shape->ctas_per_sm;
+        h.cap = shape->list_cap; h.cell_cap = shape->cell_cap; h.rp = shape->rows_per_lane;
+    }
+    return h;
 }
 
 int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const ShapeHints &hints, const char **why)

@@ -50,8 +50,8 @@ struct HostPack {
                                                     // placement leaves (phase A, phase B; model of mech_pack.cu `place`)
 };
 
-// What the launch-shape choice may use (api.cu fills it from the device properties and the
-// PYJAC_S / PYJAC_THREADS / PYJAC_CTAS tuning hooks; 0 = choose).
+// What the launch-shape choice may use (filled from the device properties and a pyjac_launch_shape;
+// 0 = choose).
 struct ShapeHints {
     long long smem_bytes = 227 * 1024 - 1024;   // dynamic shared memory one CTA may use
     int S = 0, threads = 0, ctas = 0;
@@ -59,6 +59,10 @@ struct ShapeHints {
     int cell_cap = 0;   // longest Jacobian-cell list gathered in phase B (1..3); longer ones are summed piecewise in phase A
     int rp = 0;         // rows per lane in phase B (1 or 2)
 };
+
+// The hints of an explicit launch shape (NULL: all zeros = choose); `smem_optin` = the device's opt-in
+// shared memory per CTA (0: the architecture's 227 KB).
+ShapeHints hints_from_shape(const pyjac_launch_shape *shape, long long smem_optin);
 
 // Returns PYJAC_OK, PYJAC_EINVAL or PYJAC_ELIMIT.  `why` (optional) receives a static message.
 int pack_mechanism(const pyjac_mech_desc *d, HostPack &out, const ShapeHints &hints, const char **why);

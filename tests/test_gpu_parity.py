@@ -384,30 +384,103 @@ def test_host_buffer_variant_matches_device_variant(torch, PyJac):
 
 # ---------------------------------------------------------------------------------- launch shapes
 @pytest.mark.gpu
-@pytest.mark.parametrize("cfg,n,env", [
-    (1, 301, {"PYJAC_S": "1", "PYJAC_CTAS": "4"}),                                 # one state per CTA iteration
-    (1, 301, {"PYJAC_S": "2", "PYJAC_CTAS": "3", "PYJAC_THREADS": "160"}),         # three small CTAs per SM
-    (1, 301, {"PYJAC_S": "3"}),                                                    # odd S: 8-byte shared loads
-    (1, 301, {"PYJAC_S": "4", "PYJAC_THREADS": "256"}),
-    (1, 301, {"PYJAC_S": "6", "PYJAC_THREADS": "384"}),
-    (1, 301, {"PYJAC_CELL_CAP": "1", "PYJAC_CAP": "4"}),                           # everything summed in phase A, short lane lists
-    (1, 301, {"PYJAC_CELL_CAP": "2", "PYJAC_CAP": "30"}),
-    (1, 301, {"PYJAC_RP": "1"}),                                                   # one row per lane, 8-byte stores
-    (0, 1024, {"PYJAC_S": "1", "PYJAC_THREADS": "64"}),
-    (2, 65, {"PYJAC_S": "3"}),
+@pytest.mark.parametrize("cfg,n,shape", [
+    (1, 301, dict(states_per_cta=1, ctas_per_sm=4)),                                # one state per CTA iteration
+    (1, 301, dict(states_per_cta=2, ctas_per_sm=3, threads=160)),                   # three small CTAs per SM
+    (1, 301, dict(states_per_cta=3, ctas_per_sm=1, threads=512)),                   # odd S: 8-byte shared loads
+    (1, 301, dict(states_per_cta=4, threads=256)),
+    (1, 301, dict(states_per_cta=6, threads=384)),
+    (1, 301, dict(cell_cap=1, list_cap=4)),                    # everything summed in the summing phase, short lane lists
+    (1, 301, dict(states_per_cta=2, cell_cap=2, list_cap=30)),
+    (1, 301, dict(rows_per_lane=1)),                                                # one row per lane, 8-byte stores
+    (0, 1024, dict(states_per_cta=1, threads=64)),
+    (2, 65, dict(states_per_cta=2)),
 ])
-def test_launch_shapes(torch, PyJac, monkeypatch, cfg, n, env):
-    """Every launch shape the tuning hooks can select (states per CTA iteration, CTAs per SM, CTA
+def test_launch_shapes(torch, PyJac, cfg, n, shape):
+    """Every launch shape pyjac_mech_create_shaped accepts (states per CTA iteration, CTAs per SM, CTA
     size, list lengths of the two gather phases, rows per lane) evaluates the same Jacobian: parity with
     the oracle within the same tolerance, ragged last batch included."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
     m = synth.make_mechanism(cfg)
     T, P, Y = synth.config_states(cfg, n)
-    pj = PyJac(m)
+    pj = PyJac(m, shape=shape)
     o = Oracle(m)
     check_jacobian(torch, pj, o, T, P, Y, label="launch_shapes")
     check_rates(torch, pj, o, T[:64], P[:64], Y[:64])
+
+
+@pytest.mark.gpu
+def test_two_live_handles_share_a_kernel(torch, PyJac):
+    """A handle is immutable after creation: creating a second, smaller mechanism that uses the same kernel
+    function must not disturb the first one's launches (the kernel's dynamic shared-memory limit is set to
+    what the device allows, never to one handle's size)."""
+    big, small = synth.make_mechanism(1), synth.make_mechanism(0)
+    shape = dict(states_per_cta=2, ctas_per_sm=1, threads=256)
+    T, P, Y = synth.config_states(1, 130)
+    dT, dP, dY = dev(torch, T, P, Y)
+    pj_big = PyJac(big, shape=shape)
+    J0 = pj_big.eval_jacobian(dT, dP, dY).clone()
+    pj_small = PyJac(small, shape=shape)                      # same kernel function, 8 KB instead of 67 KB
+    Ts, Ps, Ys = synth.config_states(0, 64)
+    check_jacobian(torch, pj_small, Oracle(small), Ts, Ps, Ys)
+    assert torch.equal(pj_big.eval_jacobian(dT, dP, dY), J0)
+    check_jacobian(torch, pj_big, Oracle(big), T, P, Y)
+
+
+@pytest.mark.gpu
+def test_one_handle_from_two_host_threads(torch, PyJac):
+    """Evaluation on a handle is re-entrant (the paper's complaint about TChem): two host
+    threads evaluate on the same handle at once, each on its own stream, device-pointer and host-buffer
+    calls mixed; every result is bit-identical to the serial one."""
+    import threading
+    m = synth.make_mechanism(0)
+    pj = PyJac(m)
+    ld = m.n_species + 1
+    T, P, Y = synth.config_states(0, 1024)
+    dT, dP, dY = dev(torch, T, P, Y)
+    ref = pj.eval_jacobian(dT, dP, dY).cpu()
+    torch.cuda.synchronize()
+    errors = []
+
+    def work(k):
+        try:
+            torch.cuda.set_device(0)
+            s = torch.cuda.Stream()
+            for it in range(6):
+                with torch.cuda.stream(s):
+                    J = pj.eval_jacobian(dT, dP, dY)
+                s.synchronize()
+                assert torch.equal(J.cpu(), ref)
+                out = np.empty((1024, ld * ld))
+                pj.eval_jacobian_host(T, P, Y, out, chunk_states=300 + 37 * k)
+                assert np.array_equal(out, ref.numpy())
+        except Exception as e:                                  # noqa: BLE001
+            errors.append(repr(e))
+
+    threads = [threading.Thread(target=work, args=(k,)) for k in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+
+
+@pytest.mark.gpu
+def test_binding_rejects_bad_output_tensors(torch, PyJac):
+    m = synth.make_mechanism(0)
+    pj = PyJac(m)
+    ld = m.n_species + 1
+    T, P, Y = synth.config_states(0, 8)
+    dT, dP, dY = dev(torch, T, P, Y)
+    for bad in (torch.empty((8, ld * ld), dtype=torch.float32, device="cuda"),
+                torch.empty((8, ld * ld - 1), dtype=torch.float64, device="cuda"),
+                torch.empty((8, 2 * ld * ld), dtype=torch.float64, device="cuda")[:, ::2],
+                torch.empty((8, ld * ld), dtype=torch.float64)):
+        with pytest.raises(ValueError):
+            pj.eval_jacobian(dT, dP, dY, out=bad)
+    with pytest.raises(ValueError):
+        pj.eval_dydt(dT, dP, dY, out=torch.empty((8, ld - 1), dtype=torch.float64, device="cuda"))
+    with pytest.raises(ValueError):
+        pj.eval_jacobian_host(T, P, Y, np.empty((8, ld * ld), dtype=np.float32))
 
 
 @pytest.mark.gpu
@@ -429,8 +502,8 @@ def test_output_pointer_not_16_byte_aligned(torch, PyJac):
 
 @pytest.mark.gpu
 def test_peak_probes(torch):
-    """The roofline probes: the store stream writes every element once, the FMA probe
-    reports the flops it ran; bad arguments are refused."""
+    """The roofline probes of the helper library: the store stream writes every element
+    once, the FMA probe reports the flops it ran; bad arguments are refused."""
     from paper_1605_03262_b200 import binding
     sp = torch.cuda.current_stream().cuda_stream
     buf = torch.full((1 << 16,), -1.0, dtype=torch.float64, device="cuda")
@@ -442,6 +515,6 @@ def test_peak_probes(torch):
     flops = binding.peak_dfma(out, 128, sp)
     torch.cuda.synchronize()
     assert flops > 0 and flops % (2 * 8 * 128) == 0 and bool(torch.isfinite(out).all())
-    lib = binding.load_library()
-    assert lib.pyjac_peak_store_stream(None, 16, None) == binding.PYJAC_EINVAL
-    assert lib.pyjac_peak_store_stream(buf.data_ptr() + 8, 16, None) == binding.PYJAC_EINVAL
+    lib = binding.load_tools()
+    assert lib.pyjac_tools_peak_store_stream(None, 16, None) == binding.PYJAC_EINVAL
+    assert lib.pyjac_tools_peak_store_stream(buf.data_ptr() + 8, 16, None) == binding.PYJAC_EINVAL

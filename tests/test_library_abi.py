@@ -20,17 +20,39 @@ def lib():
     return binding.load_library()
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "pyjac_b200.h")).read()
+def declared_symbols(header):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(pyjac_[a-z_]+)\s*\(", text)))
 
 
 def test_header_symbols_are_exported(lib):
-    names = declared_symbols()
+    """Every function include/pyjac_b200.h declares is exported by the product library, and nothing of
+    the bench / test helper interface is; the helper library exports exactly its own header."""
+    names = declared_symbols("pyjac_b200.h")
     assert set(names) == set(binding.EXPORTS)
     for n in names:
         assert hasattr(lib, n), n
+    tools = binding.load_tools()
+    tnames = declared_symbols("pyjac_b200_tools.h")
+    assert set(tnames) == set(binding.TOOLS_EXPORTS)
+    for n in tnames:
+        assert hasattr(tools, n), n
+        assert not hasattr(lib, n), n
+
+
+def test_product_library_reads_no_environment(lib):
+    """no runtime flags beyond the call arguments -- none of the product's own object
+    files references getenv (launch shapes are an explicit argument of pyjac_mech_create_shaped; the CUDA
+    runtime linked into the .so reads its own variables, which is not ours to change)."""
+    import glob
+    import subprocess
+    objs = [o for o in glob.glob(os.path.join(os.path.dirname(binding.LIB_PATH), "build", "*.o"))
+            if not o.endswith("tools.o")]
+    assert len(objs) >= 4
+    for o in objs:
+        out = subprocess.run(["nm", "--undefined-only", o], capture_output=True, text=True).stdout
+        assert "getenv" not in out, o
 
 
 def test_strerror(lib):
@@ -126,23 +148,45 @@ def test_binding_refuses_cpu_tensors():
                        torch.zeros(2, 3, dtype=torch.float64))
 
 
-@pytest.mark.parametrize("env", [
-    {}, {"PYJAC_S": "1"}, {"PYJAC_S": "2", "PYJAC_PW": "7"}, {"PYJAC_S": "4", "PYJAC_CTAS": "1"},
-    {"PYJAC_S": "1", "PYJAC_PW": "5", "PYJAC_THREADS": "128"}, {"PYJAC_CAP": "6"}, {"PYJAC_CAP": "64"},
+@pytest.mark.parametrize("shape", [
+    None, dict(states_per_cta=1), dict(states_per_cta=2, ctas_per_sm=3, threads=160), dict(states_per_cta=6),
+    dict(states_per_cta=4, ctas_per_sm=1), dict(states_per_cta=1, threads=64), dict(list_cap=6), dict(list_cap=64),
+    dict(cell_cap=1), dict(cell_cap=2, rows_per_lane=1),
 ])
-def test_pack_self_check_over_launch_shapes(monkeypatch, env):
-    """pyjac_pack_stats packs exactly as pyjac_mech_create does, including the self-check of everything
-    the kernels read without bounds checks (whole rows of chunks, table blocks, entry offsets); it must
-    hold for every configuration and every shape the tuning hooks can select."""
-    for k, v in env.items():
-        monkeypatch.setenv(k, v)
+def test_pack_self_check_over_launch_shapes(shape):
+    """pyjac_tools_pack_stats packs exactly as pyjac_mech_create_shaped does, including the self-check of
+    everything the kernels read without bounds checks (whole rows of chunks, table blocks, entry offsets);
+    it must hold for every configuration and every launch shape."""
     for cfg in (0, 1, 2, 3):
         try:
-            st = binding.pack_stats(synth.make_mechanism(cfg))
+            st = binding.pack_stats(synth.make_mechanism(cfg), shape)
         except binding.PyJacError as e:
             # a forced shape that does not fit the shared memory of one CTA is refused, loudly
-            assert e.code == binding.PYJAC_ELIMIT and "PYJAC_S" in env and cfg >= 2
+            assert e.code == binding.PYJAC_ELIMIT and shape is not None and cfg >= 1
             continue
-        assert st["chunks"] > 0 and st["panels"] >= 1 and st["smem_bytes_per_cta"] <= 227 * 1024
+        assert st["chunks"] > 0 and st["states_per_cta"] >= 1 and st["smem_bytes_per_cta"] <= 227 * 1024
+        assert st["threads"] % 32 == 0 and st["threads"] >= 32 * st["states_per_cta"]
     for seed in range(4):
-        binding.pack_stats(synth.make_tiny_mechanism(seed))
+        binding.pack_stats(synth.make_tiny_mechanism(seed), shape)
+
+
+def test_launch_shape_validation():
+    m = synth.make_mechanism(0)
+    for bad in (dict(states_per_cta=5), dict(threads=100), dict(threads=1024), dict(ctas_per_sm=9),
+                dict(cell_cap=4), dict(rows_per_lane=3), dict(states_per_cta=-1)):
+        with pytest.raises(binding.PyJacError) as e:
+            binding.pack_stats(m, bad)
+        assert e.value.code == binding.PYJAC_EINVAL
+    with pytest.raises(ValueError):
+        binding.launch_shape(dict(no_such_field=1))
+
+
+def test_binding_validates_outputs():
+    """Outputs are written in place and never copied or converted: a wrong dtype, a non-contiguous view or a
+    buffer that is too small is an error, not a silent temporary."""
+    pj = binding.PyJac.__new__(binding.PyJac)
+    pj.ns, pj.nr, pj.device = 3, 1, 0
+    for bad in (np.zeros((4, 16), dtype=np.float32), np.zeros((4, 32))[:, ::2], np.zeros((4, 15)), [[0.0] * 16] * 4):
+        with pytest.raises(ValueError):
+            pj._host_out(bad, 4 * 16)
+    assert pj._host_out(np.zeros((4, 16)), 4 * 16) != 0
