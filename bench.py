@@ -2,7 +2,7 @@
 """bench.py -- Jacobian evaluations per second of the batched analytical kinetics Jacobian on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
-                    [--also 2,3] [--sweep] [--no-cpu-baseline]
+                    [--also 2,3] [--sweep short|full|off] [--no-cpu-baseline] [--no-e2e] [--peaks]
 
 A "step" is one pass of the whole hot path (thermo -> rates -> source term -> Jacobian -> store;
 SURVEY.md section 8(a) rows S0-S10, one kernel launch) over one batch of seeded synthetic states.
@@ -32,9 +32,45 @@ UNIT = "states/s"
 FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback
 # oracle sample sizes per config (about 10-30 s of CPU work on 8-32 cores)
 CPU_SAMPLE = {0: 1024, 1: 8192, 2: 2048, 3: 256}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the Jacobian kernel from the committed
-# `ncu --set full` capture (profiles/), or None where no capture exists for that workload
-NCU_TRAFFIC_BYTES = {"cfg1_53sp_325rx": 2376411408, "cfg2_111sp_784rx": 10179931272}      # profiles/r1_v8_cfg1_cfg2.md
+# Counters of the committed `ncu` captures (profiles/r2_ncu_counters.csv, written from the reports the .md
+# beside it names): DRAM bytes and fp64 flops per state of each kernel.  They describe the kernels whose
+# source hash they carry; with different sources the bench reports null instead of a stale number.
+NCU_COUNTERS = os.path.join(ROOT, "profiles", "r2_ncu_counters.csv")
+KERNEL_SOURCES = ("kernels.cu", "mech_pack.cu", "device_mech.h", "api.cu", "dispatch.cu")
+FP64_PEAK_TFLOPS = 33.74        # measured: bench.py --peaks, profiles/r1_machine_peaks.md (8 FMA chains per thread)
+
+
+def kernel_source_sha16() -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_1605_03262_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_counters():
+    """({workload: {kernel: {dram_bytes_per_state, fp64_flop_per_state}}}, source) of the committed captures
+    that belong to these kernel sources."""
+    import csv
+    out, src = {}, None
+    try:
+        sha = kernel_source_sha16()
+        for row in csv.DictReader(open(NCU_COUNTERS)):
+            if row["kernel_source_sha16"] != sha:
+                src = "profiles/r2_ncu_counters.csv describes other kernel sources (%s)" % row["kernel_source_sha16"]
+                continue
+            out.setdefault(row["workload"], {})[row["kernel"]] = {
+                "dram_bytes_per_state": float(row["dram_bytes_per_state"]),
+                "fp64_flop_per_state": float(row["fp64_flop_per_state"])}
+            src = "profiles/r2_ncu_counters.csv (%s)" % row["source"]
+    except Exception:
+        return {}, None
+    return out, src
+
+
+def fp64_peak():
+    return FP64_PEAK_TFLOPS
 
 
 def measured_peaks():
@@ -101,7 +137,21 @@ def algorithmic_bytes(ns: int, n: int) -> int:
     return n * ((ns + 2) + (ns + 1) * (ns + 1)) * 8
 
 
-def time_oracle(cfg: int, n_sample: int, steps: int = 1, warmup: int = 0):
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def time_oracle(cfg: int, n_sample: int, steps: int = 3, warmup: int = 1, single_thread: bool = False):
+    """The oracle as it stands on the host cores: `warmup` untimed passes over 64 states, then `steps`
+    timed passes over the first n_sample states of the workload (1 warm-up + 3
+    repetitions); optionally also one pass on ONE thread over n_sample / cores states -- the paper's CPU
+    numbers are single-thread."""
     import numpy as np  # noqa: F401
     from oracle.oracle import Oracle
     from paper_1605_03262_b200 import synth
@@ -111,13 +161,26 @@ def time_oracle(cfg: int, n_sample: int, steps: int = 1, warmup: int = 0):
     T, P, Y = synth.config_states(cfg, n_sample)
     for _ in range(warmup):
         o.jacobian(T[:64], P[:64], Y[:64])
-    t0 = time.perf_counter()
+    per = []
     for _ in range(steps):
+        t0 = time.perf_counter()
         o.jacobian(T, P, Y)
-    dt = (time.perf_counter() - t0) / steps
-    return {"value": n_sample / dt, "unit": UNIT, "cores": o.threads, "kind": "oracle",
-            "sample": "analytical Jacobian (oracle/oracle.c, Algorithm-1 order, OpenMP static over states) on "
-                      "the first %d states of the workload, %d pass(es), %.2f s per pass" % (n_sample, steps, dt)}, dt
+        per.append(time.perf_counter() - t0)
+    dt = sum(per) / len(per)
+    res = {"value": n_sample / dt, "unit": UNIT, "cores": o.threads, "kind": "oracle", "cpu": cpu_model(),
+           "best_value": n_sample / min(per),
+           "sample": "analytical Jacobian (oracle/oracle.c, Algorithm-1 order, OpenMP static over states) on "
+                     "the first %d states of the workload, %d warm-up + %d timed pass(es), %.2f s per pass"
+                     % (n_sample, warmup, steps, dt)}
+    if single_thread:
+        n1 = max(16, n_sample // max(o.threads, 1))
+        o1 = Oracle(m, threads=1)
+        o1.jacobian(T[:16], P[:16], Y[:16])
+        t0 = time.perf_counter()
+        o1.jacobian(T[:n1], P[:n1], Y[:n1])
+        res["single_thread"] = {"value": n1 / (time.perf_counter() - t0), "unit": UNIT, "cores": 1,
+                                "sample": "first %d states, one pass" % n1}
+    return res, dt
 
 
 def run_reference(args):
@@ -250,8 +313,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--also", default="2", help="comma list of further configs reported under per_config")
-    ap.add_argument("--sweep", action="store_true", help="config 4: state-count sweep, three kernels")
+    ap.add_argument("--also", default="2,3", help="comma list of further configs reported under per_config")
+    ap.add_argument("--sweep", default="short", choices=["short", "full", "off"],
+                    help="config 4: state-count sweep of the three kernels (short: 4^5, 4^7, 4^9; full: 4^5 .. 4^10)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--peaks", action="store_true",
                     help="measure the write-only store stream and the fp64 FMA rate (SURVEY.md 8(d)) and exit")
@@ -303,11 +367,31 @@ def main():
     launch_ms = r["total_ms"] / (args.steps * r["launches_per_step"])
     alg_bytes = algorithmic_bytes(c.n_species, r["per_launch"])
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
+    counters, counters_src = ncu_counters()
+
+    def traffic_of(name, states):
+        c = counters.get(name, {}).get("jacobian")
+        return None if not c else int(round(c["dram_bytes_per_state"] * states))
+
+    def fp64_of(name, kernel, states, ms):
+        """achieved fp64 FLOP/s of one launch from the counted DFMA / DADD / DMUL per state (ncu), against the
+        measured FMA peak: the second roofline SURVEY.md 8(d) asks for"""
+        c = counters.get(name, {}).get(kernel)
+        if not c:
+            return None
+        tf = c["fp64_flop_per_state"] * states / (ms * 1e-3) / 1e12
+        return {"bound": "alu", "achieved": tf, "peak": fp64_peak(), "unit": "TFLOP/s", "frac": tf / fp64_peak(),
+                "flop_per_state": c["fp64_flop_per_state"], "peak_source": "bench.py --peaks (profiles/r1_machine_peaks.md)"}
+
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_BYTES.get(c.name), "peak_source": peak_src,
-                "kernel": "pyjac::eval_kernel<2 (Jacobian), %d threads>" % pj.launch_config(r["per_launch"])["threads"],
-                "algorithmic_bytes_per_launch": alg_bytes, "launch_ms": launch_ms,
-                "launch_config": pj.launch_config(r["per_launch"])}
+                "traffic": traffic_of(c.name, r["per_launch"]), "traffic_source": counters_src,
+                "peak_source": peak_src,
+                "kernel": "pyjac::eval_kernel<2 (Jacobian), S = %d states per CTA iteration>" % pj.launch_config(r["per_launch"])["states_per_cta"],
+                "algorithmic_bytes_per_launch": alg_bytes,
+                "algorithmic_bytes_note": "(Ns+2) doubles read + (Ns+1)^2 doubles written per state, the placeholder "
+                                          "row and the zero column of the (Ns+1)^2 layout included",
+                "launch_ms": launch_ms, "launch_config": pj.launch_config(r["per_launch"]),
+                "fp64": fp64_of(c.name, "jacobian", r["per_launch"], launch_ms)}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -355,31 +439,34 @@ def main():
                             "n_states": rr["n"], "states_per_launch": rr["per_launch"], "launch_ms": lm,
                             "roofline": {"bound": "hbm", "achieved": ab / (lm * 1e-3) / 1e9, "peak": peak,
                                          "unit": "GB/s", "frac": ab / (lm * 1e-3) / 1e9 / peak,
-                                         "traffic": NCU_TRAFFIC_BYTES.get(cc.name)},
+                                         "traffic": traffic_of(cc.name, rr["per_launch"]),
+                                         "fp64": fp64_of(cc.name, "jacobian", rr["per_launch"], lm)},
                             "launch_config": rr["pj"].launch_config(rr["per_launch"])}
             del rr
             torch.cuda.empty_cache()
         if per:
             line["per_config"] = per
-        if args.sweep:
-            line["sweep_53sp"] = sweep(torch, args)
+        if args.sweep != "off":
+            line["sweep_53sp"] = sweep(torch, args, fp64_of)
         if not args.no_cpu_baseline:
-            line["cpu_baseline"], _ = time_oracle(cfg, CPU_SAMPLE[cfg])
+            line["cpu_baseline"], _ = time_oracle(cfg, CPU_SAMPLE[cfg], steps=3, warmup=1, single_thread=True)
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
 
 
-def sweep(torch, args):
-    """BASELINE.json configs[4]: 53-species mechanism, 4^5 .. 4^10 states, the three kernels."""
+def sweep(torch, args, fp64_of):
+    """BASELINE.json configs[4]: 53-species mechanism, 4^5 .. 4^10 states (short: three of them), the three
+    kernels separately, each with its fp64 roofline entry (rates and dPhi/dt move few bytes: fp64-bound)."""
     from paper_1605_03262_b200 import synth
     from paper_1605_03262_b200.binding import PyJac
     m = synth.make_mechanism(1)
     pj = PyJac(m, device=torch.cuda.current_device())
     ld = m.n_species + 1
     res = []
-    for n in synth.SWEEP_STATES:
+    counts = synth.SWEEP_STATES if args.sweep == "full" else (4 ** 5, 4 ** 7, 4 ** 9)
+    for n in counts:
         T, P, Y = synth.make_states(m.n_species, n, synth.CONFIGS[1].seed + 2000 + n)
         dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
         out = torch.empty((n, ld * ld), dtype=torch.float64, device="cuda")
@@ -389,8 +476,12 @@ def sweep(torch, args):
         td, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3, fn=lambda: pj.eval_dydt(dT, dP, dY, out=dy))
         tr, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3,
                          fn=lambda: pj.eval_rates(dT, dP, dY, want=("wdot",)))
+        name = synth.CONFIGS[1].name
         res.append({"n_states": n, "jacobian_states_per_s": n / (tj / steps * 1e-3),
-                    "dydt_states_per_s": n / (td / steps * 1e-3), "rates_states_per_s": n / (tr / steps * 1e-3)})
+                    "dydt_states_per_s": n / (td / steps * 1e-3), "rates_states_per_s": n / (tr / steps * 1e-3),
+                    "fp64": {"jacobian": fp64_of(name, "jacobian", n, tj / steps),
+                             "dydt": fp64_of(name, "dydt", n, td / steps),
+                             "rates": fp64_of(name, "rates", n, tr / steps)}})
         del out, dy
         torch.cuda.empty_cache()
     return res

@@ -194,9 +194,10 @@ int64_t pyjac_kernel_launches(void);
 
 /* Launch configuration the Jacobian kernel uses for this mechanism (any output may be NULL):
  * threads per CTA, dynamic shared memory per CTA in bytes, resident CTAs per SM, grid size for n
- * states.  Reported by bench.py next to the roofline numbers. */
+ * states, states a CTA interleaves per iteration.  Reported by bench.py next to the roofline numbers. */
 int pyjac_jacobian_launch_config(const pyjac_mech *mech, int64_t n, int32_t *threads,
-                                 int32_t *smem_bytes, int32_t *ctas_per_sm, int32_t *grid);
+                                 int32_t *smem_bytes, int32_t *ctas_per_sm, int32_t *grid,
+                                 int32_t *states_per_cta);
 
 /* Static, never-NULL description of an error code. */
 const char *pyjac_strerror(int code);

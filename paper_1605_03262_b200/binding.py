@@ -75,7 +75,7 @@ def load_library(path: str | None = None):
     lib.pyjac_eval_dydt_host.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64]
     lib.pyjac_kernel_launches.argtypes = []
     lib.pyjac_kernel_launches.restype = i64
-    lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 4
+    lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 5
     lib.pyjac_strerror.argtypes = [C.c_int]
     lib.pyjac_strerror.restype = C.c_char_p
     for name in EXPORTS:
@@ -330,10 +330,11 @@ class PyJac:
                                chunk_states)
 
     def launch_config(self, n: int):
-        v = [C.c_int32() for _ in range(4)]
+        v = [C.c_int32() for _ in range(5)]
         _check(self.lib.pyjac_jacobian_launch_config(self._h, int(n), *[C.byref(x) for x in v]),
                "pyjac_jacobian_launch_config")
-        return dict(threads=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, grid=v[3].value)
+        return dict(threads=v[0].value, smem_bytes=v[1].value, ctas_per_sm=v[2].value, grid=v[3].value,
+                    states_per_cta=v[4].value)
 
     def kernel_launches(self) -> int:
         return int(self.lib.pyjac_kernel_launches())

@@ -247,10 +247,11 @@ int pyjac_eval_jacobian(const pyjac_mech *m, int64_t n, const double *T, const d
 int64_t pyjac_kernel_launches(void) { return g_launches.load(std::memory_order_relaxed); }
 
 int pyjac_jacobian_launch_config(const pyjac_mech *m, int64_t n, int32_t *threads, int32_t *smem_bytes,
-                                 int32_t *ctas_per_sm, int32_t *grid)
+                                 int32_t *ctas_per_sm, int32_t *grid, int32_t *states_per_cta)
 {
     if (!m || n < 0) return PYJAC_EINVAL;
     if (threads) *threads = m->threads;
+    if (states_per_cta) *states_per_cta = m->S;
     if (smem_bytes) *smem_bytes = (int32_t)m->smem[2];
     if (ctas_per_sm) *ctas_per_sm = m->ctas_per_sm[2];
     long long cap = (long long)m->n_sm * m->ctas_per_sm[2];

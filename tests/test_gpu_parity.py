@@ -1,7 +1,9 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
 same seeded inputs.  Tolerances (BASELINE.json north_star):
-  rates R_f, R_r, c_i      element-wise relative 1e-12 (reverse rates: see KR_TOL below)
-  wdot, dPhi/dt            1e-12 of max_k |.| per state (C19: do not judge cancellation)
+  rates R_f, R_r, c_i      element-wise relative 1e-12 (north_star), R_r included: the conditioning bound
+                           of k_r = k_f / K_c, `kr_bound`, is several 1e-12, but the observed maximum is
+                           3e-13, so the plain 1e-12 holds and is what is asserted
+  wdot, dPhi/dt            1e-12 of the largest term summed, per state (C19: do not judge cancellation)
   Jacobian                 Frobenius-norm relative error per state <= 1e-10 (Eq. 132)
 """
 import numpy as np
@@ -39,10 +41,11 @@ def dev(torch, *arrays):
     return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrays]
 
 
-def kr_tol(oracle, T):
-    """k_r = k_f / K_c with K_c from exp(sum_k nu_ki B_k) (Eqs. 23-27): each B_k is rounded at
-    eps |B_k| (its a_5/T term reaches several hundred for large species), so two correct
-    evaluation orders differ by up to ~eps * sum|nu| * max|B_k| in the exponent."""
+def kr_bound(oracle, T):
+    """Conditioning of k_r = k_f / K_c with K_c from exp(sum_k nu_ki B_k) (Eqs. 23-27): each B_k is
+    rounded at eps |B_k| (its a_5/T term reaches several hundred for large species), so two correct
+    evaluation orders may differ by up to ~eps * sum|nu| * max|B_k| in the exponent.  Reported beside
+    the observed error; NOT the tolerance (that is RATE_TOL)."""
     bmax = max(np.abs(oracle.species_thermo(float(t))[0][3]).max() for t in (T.min(), T.max()))
     return max(RATE_TOL, 8.0 * 6 * EPS * bmax)
 
@@ -56,7 +59,7 @@ def check_rates(torch, pj, o, T, P, Y, label=None):
     dy = pj.eval_dydt(dT, dP, dY).cpu().numpy()
     ref = o.source(T, P, Y)
     tiny = 1e-300
-    tol_r = kr_tol(o, T)
+    tol_r = RATE_TOL
     rel = lambda a, b: float((np.abs(a - b) / np.maximum(np.abs(b), tiny))[np.abs(b) > 0].max(initial=0.0))
     # production rates and source term: against the size of what was summed (C19); with reverse
     # rates entering, the bound is the reverse-rate one
@@ -64,7 +67,7 @@ def check_rates(torch, pj, o, T, P, Y, label=None):
     scale_w = q.max(axis=1, keepdims=True)
     seen = dict(rf=rel(got["rf"], ref["rf"]), rr=rel(got["rr"], ref["rr"]), cmod=rel(got["cmod"], ref["cmod"]),
                 wdot=float((np.abs(got["wdot"] - ref["wdot"]) / np.maximum(scale_w, tiny)).max(initial=0.0)),
-                kr_tol=tol_r)
+                kr_bound=kr_bound(o, T))
     assert np.all(np.abs(got["rf"] - ref["rf"]) <= RATE_TOL * np.abs(ref["rf"]) + tiny)
     assert np.all(np.abs(got["rr"] - ref["rr"]) <= tol_r * np.abs(ref["rr"]) + tiny)
     assert np.all(np.abs(got["cmod"] - ref["cmod"]) <= RATE_TOL * np.abs(ref["cmod"]) + tiny)
@@ -171,7 +174,7 @@ def _report_observed():
     import json
     import os
     if RATES_OBSERVED:
-        print("\nobserved maxima of the rate arrays, GPU vs oracle (R_f, c_i: 1e-12; the others: kr_tol):")
+        print("\nobserved maxima of the rate arrays, GPU vs oracle (tolerance 1e-12; kr_bound = conditioning bound of k_r):")
         for k, v in sorted(RATES_OBSERVED.items()):
             print("%-28s " % k + " ".join("%s=%.2e" % (n, x) for n, x in sorted(v.items())))
     lines = ["%-28s " % k + " ".join("%s=%.2e" % (n, v[n]) for n in ("fro", "row", "elem", "col", "tcol"))
@@ -266,7 +269,7 @@ def test_state_count_sweep_rates_and_dydt(torch, PyJac):
         pick = np.sort(np.random.default_rng(n).choice(n, size=48, replace=False))
         ref = o.source(T[pick], P[pick], Y[pick])
         scale = np.abs(ref["dydt"][:, 1:]).max(axis=1, keepdims=True)
-        tol = kr_tol(o, T[pick])
+        tol = RATE_TOL
         bound = tol * np.maximum(scale, _dydt_term_scale(o, ref, T[pick], P[pick], Y[pick], slice(1, None)))
         assert np.all(np.abs(dy[pick][:, 1:] - ref["dydt"][:, 1:]) <= bound)
         Jr = o.jacobian(T[pick], P[pick], Y[pick])
