@@ -139,6 +139,10 @@ typedef struct pyjac_launch_shape {
                                column is streamed out; longer lists are summed piecewise before */
     int32_t rows_per_lane;  /* 1 or 2 Jacobian rows per lane in the streaming phase (2 needs N_sp odd,
                                i.e. an even leading dimension; 16-byte stores) */
+    int32_t p1_states;      /* states one work item of the reaction phase evaluates with the reaction's
+                               constants held in registers (0: all states_per_cta) */
+    int32_t stage_tables;   /* 1: copy the gather tables to shared memory once per CTA (PYJAC_ELIMIT if they
+                               do not fit this shape); 0: read them through L1 / L2 */
 } pyjac_launch_shape;
 
 /* As pyjac_mech_create with an explicit launch shape (tuning and tests; `shape` may be NULL).

@@ -41,7 +41,8 @@ class MechDesc(C.Structure):
 class LaunchShape(C.Structure):
     """struct pyjac_launch_shape (0 = let the library choose)"""
     _fields_ = [("states_per_cta", C.c_int32), ("threads", C.c_int32), ("ctas_per_sm", C.c_int32),
-                ("list_cap", C.c_int32), ("cell_cap", C.c_int32), ("rows_per_lane", C.c_int32)]
+                ("list_cap", C.c_int32), ("cell_cap", C.c_int32), ("rows_per_lane", C.c_int32),
+                ("p1_states", C.c_int32), ("stage_tables", C.c_int32)]
 
 
 EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_sizes",

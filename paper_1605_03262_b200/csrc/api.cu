@@ -153,9 +153,11 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
     }
     if (rc == PYJAC_OK) {
         for (auto &f : up.fix) *f.first = (const unsigned char *)m->blob + f.second;
-        m->plan = make_smem_plan(hp.ns, hp.n_e);
+        m->plan = hp.stage ? make_smem_plan(hp.ns, hp.n_e, (int)((hp.achunk.size() / 2 + 1) / 2), (int)(hp.a_ent.size() / 4),
+                                            (int)(hp.b_ent.size() / 4))
+                           : make_smem_plan(hp.ns, hp.n_e);
         const size_t bytes = eval_smem_bytes(m->plan, m->S);
-        if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->S)) {
+        if (bytes + 64 > (size_t)prop.sharedMemPerBlockOptin || !eval_kernel_ptr(2, m->S, hp.stage)) {
             rc = PYJAC_ELIMIT;
         } else {
             // shared-memory carve-out: what the CTAs this shape was sized for need, the rest of the 256 KB
@@ -164,7 +166,7 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
             carveout = carveout > 100 ? 100 : carveout < 0 ? 0 : carveout;
             for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
                 m->smem[level] = bytes;
-                const void *k = eval_kernel_ptr(level, m->S);
+                const void *k = eval_kernel_ptr(level, m->S, hp.stage);
                 // the kernel function is shared by every handle of this shape: its dynamic shared-memory limit
                 // is raised to what the device allows, once and for all, never to one handle's size
                 cudaFuncAttributes fa{};

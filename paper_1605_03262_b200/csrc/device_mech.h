@@ -79,9 +79,10 @@ struct DeviceMech {
     int n_rchunk;               // groups of 32 reactions
     int n_plain;                // the last n_plain groups hold only plain reactions
     int n_p1item;
-    const uint32_t *p1item;     // work items of P1, most expensive first: group | path << 16 | first state << 20; path 0 =
-                                // any reaction, one state (q); 1 = plain elementary reactions, 2 = any rate form with
-                                // at most three molecules per side, k_r from K_c and one NASA breakpoint: two states
+    const uint32_t *p1item;     // work items of P1, most expensive first: group | path << 16 | first state << 20 |
+                                // states << 24; path 0 = any reaction (one state); 1 = plain elementary reactions,
+                                // 2 = any rate form with at most three molecules per side, k_r from K_c and one NASA
+                                // breakpoint: the item's states one after the other, the reaction's constants in registers
     const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
     const uint4 *vidx;          // [nr] E indices of the slots' s'_ij: {v0|v1<<16, v2|v3<<16, v4|v5<<16, 0}
                                 //      (empty slots point at the dump slot)
@@ -153,10 +154,14 @@ struct SmemPlan {
     int total;                          // doubles per state
     int colc;                           // [ld][4], offset in doubles from the end of the state part
     int wrow;                           // [ld]
+    int etab;                           // [32] 2^(j/32), the table of exp_rate (kernels.cu)
+    int staged;                         // 1: the gather tables of phases A and B are copied to shared memory once per CTA
+    int t_achunk, t_aent, t_bent;       // their offsets (doubles from the end of the state part), sizes in 16-byte units
+    int n_achunk16, n_aent16, n_bent16;
     int shared_total;                   // doubles of the state-independent part
 };
 
-inline SmemPlan make_smem_plan(int ns, int n_e)
+inline SmemPlan make_smem_plan(int ns, int n_e, int n_achunk16 = 0, int n_aent16 = 0, int n_bent16 = 0)
 {
     SmemPlan p{};
     int o = 0;
@@ -175,6 +180,12 @@ inline SmemPlan make_smem_plan(int ns, int n_e)
     o = 0;
     p.colc = take(4 * (ns + 1));
     p.wrow = take(ns + 1);
+    p.etab = take(32);
+    p.staged = n_bent16 > 0 ? 1 : 0;
+    p.n_achunk16 = n_achunk16; p.n_aent16 = n_aent16; p.n_bent16 = n_bent16;
+    p.t_achunk = take(2 * n_achunk16);
+    p.t_aent = take(2 * n_aent16);
+    p.t_bent = take(2 * n_bent16);
     p.shared_total = o;
     return p;
 }

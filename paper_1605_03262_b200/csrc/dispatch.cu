@@ -7,7 +7,7 @@ namespace pyjac {
 #define PYJAC_FOR_S(X) X(1) X(2) X(3) X(4) X(6)
 
 #define PYJAC_DECL(SV)                                                                                             \
-    const void *eval_kernel_ptr_##SV(int level);                                                                   \
+    const void *eval_kernel_ptr_##SV(int level, bool stage);                                                                   \
     cudaError_t launch_eval_##SV(int level, int threads, const DeviceMech &m, const SmemPlan &sp, int grid,        \
                                  size_t smem, long long n, const double *T, const double *P, const double *Y,      \
                                  long long ldy, const EvalOut &out, cudaStream_t stream);
@@ -16,10 +16,10 @@ PYJAC_FOR_S(PYJAC_DECL)
 
 size_t eval_smem_bytes(const SmemPlan &sp, int S) { return ((size_t)S * sp.total + (size_t)sp.shared_total) * sizeof(double); }
 
-const void *eval_kernel_ptr(int level, int S)
+const void *eval_kernel_ptr(int level, int S, bool stage)
 {
 #define PYJAC_PTR(SV) \
-    if (S == SV) return eval_kernel_ptr_##SV(level);
+    if (S == SV) return eval_kernel_ptr_##SV(level, stage);
     PYJAC_FOR_S(PYJAC_PTR)
 #undef PYJAC_PTR
     return nullptr;

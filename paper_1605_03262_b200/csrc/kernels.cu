@@ -22,6 +22,9 @@
 //       finish and store the energy row (Eq. 113).
 // There are no atomics on data: every sum has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
+#ifdef PYJAC_PROF
+#include <cstdio>
+#endif
 
 #include "device_mech.h"
 #include "kernels.h"
@@ -35,43 +38,46 @@ constexpr double kInvLn10 = 0.434294481903251828;
 
 __device__ __forceinline__ double entry_coef(uint32_t e) { return __hiloint2double((int)(e & ~kEntOffMask), 0); }
 
-// exp(x) for the rate coefficients: Cody-Waite reduction by ln 2, degree-13 Taylor polynomial on
-// |r| <= ln2/2 (truncation 4e-18), scaling by 2^n in two steps so that results underflow to 0
-// and overflow to +inf like exp().  About 1 ulp; no special-case branches.  The coefficients sit
-// in constant memory so that each Horner step is one DFMA with a constant-bank operand.
-__constant__ double c_exp[14] = {
-    1.6059043836821613e-10,  // 1/13!
-    2.08767569878681e-09,    // 1/12!
-    2.505210838544172e-08,   // 1/11!
-    2.755731922398589e-07,   // 1/10!
-    2.7557319223985893e-06,  // 1/9!
-    2.48015873015873e-05,    // 1/8!
-    1.984126984126984e-04,   // 1/7!
-    1.388888888888889e-03,   // 1/6!
-    8.333333333333333e-03,   // 1/5!
-    4.1666666666666664e-02,  // 1/4!
-    1.6666666666666666e-01,  // 1/3!
-    0.5, 1.0, 1.0};
-__constant__ double c_exp_red[4] = {1.4426950408889634074, 6755399441055744.0, -6.93147180369123816490e-01,
-                                    -1.90821492927058770002e-10};
+// exp(x) for the rate coefficients: x = (32 k + j) ln2/32 + r with |r| <= ln2/64, so that
+// exp(x) = 2^k 2^(j/32) exp(r): a 32-entry table (staged in shared memory; the index differs per lane), a
+// degree-6 polynomial (truncation 4e-18) and the power of two added to the exponent field.  About 1.5 ulp;
+// x <= -708 gives 0 and x >= 708 gives +inf (the rate is outside the normal range either way).
+__constant__ double c_exp2_32[32] = {
+    0x1.0000000000000p+0, 0x1.059b0d3158574p+0, 0x1.0b5586cf9890fp+0, 0x1.11301d0125b51p+0,
+    0x1.172b83c7d517bp+0, 0x1.1d4873168b9aap+0, 0x1.2387a6e756238p+0, 0x1.29e9df51fdee1p+0,
+    0x1.306fe0a31b715p+0, 0x1.371a7373aa9cbp+0, 0x1.3dea64c123422p+0, 0x1.44e086061892dp+0,
+    0x1.4bfdad5362a27p+0, 0x1.5342b569d4f82p+0, 0x1.5ab07dd485429p+0, 0x1.6247eb03a5585p+0,
+    0x1.6a09e667f3bcdp+0, 0x1.71f75e8ec5f74p+0, 0x1.7a11473eb0187p+0, 0x1.82589994cce13p+0,
+    0x1.8ace5422aa0dbp+0, 0x1.93737b0cdc5e5p+0, 0x1.9c49182a3f090p+0, 0x1.a5503b23e255dp+0,
+    0x1.ae89f995ad3adp+0, 0x1.b7f76f2fb5e47p+0, 0x1.c199bdd85529cp+0, 0x1.cb720dcef9069p+0,
+    0x1.d5818dcfba487p+0, 0x1.dfc97337b9b5fp+0, 0x1.ea4afa2a490dap+0, 0x1.f50765b6e4540p+0};
+// {32/ln2, 1.5 2^52, -(ln2/32) high part (29 bits), -(ln2/32) low part}
+__constant__ double c_exp_red[4] = {0x1.71547652b82fep+5, 6755399441055744.0, -0x1.62e42fe000000p-6,
+                                    -0x1.f473de6af278fp-35};
+// 1/6!, 1/5!, 1/4!, 1/3!, 1/2
+__constant__ double c_exp[5] = {1.388888888888889e-03, 8.333333333333333e-03, 4.1666666666666664e-02,
+                                1.6666666666666666e-01, 0.5};
 
-__device__ __forceinline__ double exp_rate(double x)
+__device__ __forceinline__ double exp_rate(double x, const double *etab)
 {
     const double s = fma(x, c_exp_red[0], c_exp_red[1]);
-    int n = __double2loint(s);
+    const int n = __double2loint(s);
     const double nd = s - c_exp_red[1];
     double r = fma(nd, c_exp_red[2], x);
     r = fma(nd, c_exp_red[3], r);
-    // even and odd powers as two independent Horner chains in r^2 (half the dependent depth)
-    const double r2 = r * r;
-    double po = c_exp[0], pe = c_exp[1];
-#pragma unroll
-    for (int i = 2; i < 14; i += 2) { po = fma(po, r2, c_exp[i]); pe = fma(pe, r2, c_exp[i + 1]); }
-    double p = fma(po, r, pe);
-    n = max(-1080, min(1030, n));
-    const int n1 = n >> 1, n2 = n - n1;
-    p *= __hiloint2double((n1 + 1023) << 20, 0);
-    return p * __hiloint2double((n2 + 1023) << 20, 0);
+    const double t = etab[n & 31];
+    double p = fma(c_exp[0], r, c_exp[1]);
+    p = fma(p, r, c_exp[2]);
+    p = fma(p, r, c_exp[3]);
+    p = fma(p, r, c_exp[4]);
+    p = fma(p, r, 1.0);
+    p = fma(p, r, 1.0);
+    p *= t;                                            // in [1, 2)
+    const int hx = __double2hiint(x), ax = hx & 0x7FFFFFFF;
+    double v = __hiloint2double(__double2hiint(p) + ((n >> 5) << 20), __double2loint(p));
+    // |x| >= 708 (2^k would leave the normal range), infinities and NaN
+    if (ax >= 0x40862000) v = ax > 0x7FF00000 ? x : hx < 0 ? 0.0 : __longlong_as_double(0x7FF0000000000000ll);
+    return v;
 }
 
 // x^nu and nu x^(nu-1) for nu in 0..3 by repeated multiplication (Eqs. 18-19, 120-121; never a
@@ -82,6 +88,9 @@ __device__ __forceinline__ void int_pow(double x, int nu, double &p, double &pm)
     p = nu == 0 ? 1.0 : nu == 1 ? x : nu == 2 ? x2 : x2 * x;
     pm = nu == 0 ? 0.0 : nu == 1 ? 1.0 : nu == 2 ? 2.0 * x : 3.0 * x2;
 }
+
+template <int N>
+struct IntC { static constexpr int value = N; };
 
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -175,15 +184,17 @@ __device__ __forceinline__ void special_rate(const DeviceMech &m, int s, int typ
 }
 
 // ---- P1, fast path: 32 reactions with at most three molecules per side (one slot per molecule), k_r from
-// K_c or irreversible, one NASA breakpoint; SP states at a time (q0 ..), the common part without branches.
+// K_c or irreversible, one NASA breakpoint; the states [q0, q1) of the block one after the other.  Everything
+// that does not depend on the state -- the reaction's constants, its slots' addresses -- is read once and
+// kept in registers over the states.
 // GEN = false: plain elementary reactions only.  GEN = true: any rate form -- PLOG / Chebyshev lanes
 // replace ln k_f and L, pressure-dependent lanes (third body, falloff, chemically activated) scale the
 // products of the common part by c_i and add the derivative terms of c_i (Eqs. 77-100).
 template <int LEVEL, int S, bool GEN>
-__device__ __forceinline__ void fast_reactions(const DeviceMech &m, double *E, const double *X, const double *sc, int s,
-                                               int q0, const EvalOut &out, long long state0, long long n)
+__device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const double *X, const double *sc,
+                                         const double *etab, int s, int q0, int q1, const EvalOut &out,
+                                         long long state0, long long n)
 {
-    constexpr int SP = S % 2 == 0 ? 2 : 1;
     const int nr = m.nr;
     const uint4 sl = m.slots[s];
     const uint32_t meta = sl.w;
@@ -197,6 +208,7 @@ __device__ __forceinline__ void fast_reactions(const DeviceMech &m, double *E, c
     const bool pdep = GEN && (type == PYJAC_THIRD_BODY || type == PYJAC_FALLOFF || type == PYJAC_CHEM_ACTIVATED);
     const bool fall = GEN && (type == PYJAC_FALLOFF || type == PYJAC_CHEM_ACTIVATED);
     const bool special = GEN && (type == PYJAC_PLOG || type == PYJAC_CHEBYSHEV);
+    const bool mixM = pdep && !meta_single(meta);
     double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
     double dlnA = 0.0, dbeta = 0.0, dTa = 0.0, fp[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (GEN) {
@@ -209,9 +221,8 @@ __device__ __forceinline__ void fast_reactions(const DeviceMech &m, double *E, c
         if (fall) { dlnA = l0 - lnA; dbeta = b0 - beta; dTa = t0 - Ta; }
         if (type == PYJAC_CHEM_ACTIVATED) { lnA = l0; beta = b0; Ta = t0; }
     }
+    // sum_k nu_ki B_k (Eq. 27 over the reaction): both intervals
     const double *th = m.th_soa + s;
-    // one breakpoint for the whole mechanism (the usual case): the interval is known without a table read,
-    // so the coefficient reads go out with the other tables instead of one L2 round trip later
     const double brk = m.brk_common == m.brk_common ? m.brk_common : th[0];
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
     if (LEVEL == 2) {
@@ -229,185 +240,186 @@ __device__ __forceinline__ void fast_reactions(const DeviceMech &m, double *E, c
         ef = m.eff_ent + m.eff_base[grp] + (s & 31);
         n_eff = m.eff_base[grp + 1] - m.eff_base[grp];
     }
+    const int eq = (m.eQ + 3 * s) * S, eh = (m.eH + s) * S;
 
-    double T[SP], lnT[SP], invT[SP], lnkf[SP], L[SP], sB[SP], sdB[SP], kf[SP], kr[SP];
+    // NQ states at a time (independent chains: the fp64 pipe sees several of them)
+    auto body = [&](auto nq_c, const int q) {
+        constexpr int NQ = decltype(nq_c)::value;
+        double T[NQ], lnT[NQ], invT[NQ], lnkf[NQ], L[NQ], sB[NQ], sdB[NQ], kf[NQ], kr[NQ];
 #pragma unroll
-    for (int u = 0; u < SP; ++u) {
-        T[u] = sc[kT * S + q0 + u]; lnT[u] = sc[kLnT * S + q0 + u]; invT[u] = sc[kInvT * S + q0 + u];
-        lnkf[u] = fma(beta, lnT[u], fma(-Ta, invT[u], lnA));                 // Eq. 21
-        L[u] = fma(Ta, invT[u], beta) * invT[u];                             // Eq. 65
-    }
-    if (GEN && special) {
-#pragma unroll
-        for (int u = 0; u < SP; ++u)
-            special_rate(m, s, type, sc[kP * S + q0 + u], sc[kLnP * S + q0 + u], lnT[u], invT[u], lnkf[u], L[u]);
-    }
-    // sum_k nu_ki B_k (Eq. 27 over the reaction) and its T derivative (Eq. 74)
-#pragma unroll
-    for (int u = 0; u < SP; ++u) {
-        const double *g = th + (size_t)(T[u] > brk ? 8 : 1) * nr;
-        const double g0 = g[0], g1 = g[nr], g2 = g[2 * (size_t)nr], g3 = g[3 * (size_t)nr], g4 = g[4 * (size_t)nr],
-                     g5 = g[5 * (size_t)nr], g6 = g[6 * (size_t)nr];
-        const double t = T[u];
-        sB[u] = fma(g1, lnT[u], g0) + fma(t, fma(t, fma(t, fma(t, g5, g4), g3), g2), g6 * invT[u]);
-        sdB[u] = fma(fma(-g6, invT[u], g1), invT[u], g2) + t * fma(t, fma(4.0 * g5, t, 3.0 * g4), 2.0 * g3);
-    }
-#pragma unroll
-    for (int u = 0; u < SP; ++u) kf[u] = exp_rate(lnkf[u]);
-#pragma unroll
-    for (int u = 0; u < SP; ++u) { kr[u] = exp_rate(lnkf[u] - sB[u]); kr[u] = rev ? kr[u] : 0.0; }   // Eqs. 23-27
-    // the SP states of one element are neighbours in shared memory: one 16-byte access for both
-    double c[6][SP], W[SP], vq[3][SP], vh[SP], vs[6][SP];
-    ldv<SP>(X + x0 + q0, c[0]); ldv<SP>(X + x1 + q0, c[1]); ldv<SP>(X + x2 + q0, c[2]);
-    ldv<SP>(X + x3 + q0, c[3]); ldv<SP>(X + x4 + q0, c[4]); ldv<SP>(X + x5 + q0, c[5]);
-    if (LEVEL == 2) ldv<SP>(sc + kW * S + q0, W);
-    double Rfv[SP], Rrv[SP];
-#pragma unroll
-    for (int u = 0; u < SP; ++u) {
-        const double c0 = c[0][u], c1 = c[1][u], c2 = c[2][u], c3 = c[3][u], c4 = c[4][u], c5 = c[5][u];
-        const double p01 = c0 * c1, p34 = c3 * c4;
-        const double Rf = kf[u] * (p01 * c2), Rr = kr[u] * (p34 * c5);       // Eqs. 18-19
-        const double R = Rf - Rr;
-        Rfv[u] = Rf; Rrv[u] = Rr;
-        vq[0][u] = R;
-        vh[u] = kRu * T[u] * fma(T[u], sdB[u], dnu);
-        if (LEVEL == 2) {
-            const double iT = invT[u];
-            // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
-            const double dRf = Rf * fma(-snf, iT, L[u]);
-            const double dRr = Rr * (fma(-snr, iT, L[u]) - sdB[u]);
-            vq[2][u] = fma(R, iT, dRf - dRr);
-            vq[1][u] = W[u] * (R - fma(Rf, snf, -Rr * snr));
-            const double nkr = -kr[u];
-            vs[0][u] = kf[u] * (c1 * c2); vs[1][u] = kf[u] * (c0 * c2); vs[2][u] = kf[u] * p01;   // Eq. 120
-            vs[3][u] = nkr * (c4 * c5); vs[4][u] = nkr * (c3 * c5); vs[5][u] = nkr * p34;         // Eq. 121
+        for (int u = 0; u < NQ; ++u) {
+            T[u] = sc[kT * S + q + u]; lnT[u] = sc[kLnT * S + q + u]; invT[u] = sc[kInvT * S + q + u];
+            lnkf[u] = fma(beta, lnT[u], fma(-Ta, invT[u], lnA));                  // Eq. 21
+            L[u] = fma(Ta, invT[u], beta) * invT[u];                              // Eq. 65
         }
-    }
-    double cm[SP];
+        if (GEN && special) {
 #pragma unroll
-    for (int u = 0; u < SP; ++u) cm[u] = 1.0;
-    if (GEN) {
-        // ---- pressure modification c_i (Eq. 20) and its derivatives (Eqs. 77-100): q_i = c R,
-        // Theta = dc/dT R + c Theta0, a = c a0 + b (rho - W [X]_i), s'_ij = c s0_ij, and b (alpha_ij - 1)
-        // per efficiency; lanes without a pressure dependence keep c = 1, b = 0
-        double Xi[SP], bb[SP], dcdT[SP], mixW[SP];
+            for (int u = 0; u < NQ; ++u)
+                special_rate(m, s, type, sc[kP * S + q + u], sc[kLnP * S + q + u], lnT[u], invT[u], lnkf[u], L[u]);
+        }
+        // sum_k nu_ki B_k and its T derivative (Eq. 74)
 #pragma unroll
-        for (int u = 0; u < SP; ++u) { Xi[u] = (pdep && !meta_single(meta)) ? sc[kM * S + q0 + u] : 0.0; bb[u] = 0.0; dcdT[u] = 0.0; }
-        for (int e = 0; e < n_eff; e += 128) {                       // Eqs. 28-30, four entries at a time
-            uint4 w[4];
+        for (int u = 0; u < NQ; ++u) {
+            const double *g = th + (T[u] > brk ? 8 : 1) * nr;
+            const double g0 = g[0], g1 = g[nr], g2 = g[2 * nr], g3 = g[3 * nr], g4 = g[4 * nr], g5 = g[5 * nr], g6 = g[6 * nr];
+            const double t = T[u];
+            sB[u] = fma(g1, lnT[u], g0) + fma(t, fma(t, fma(t, fma(t, g5, g4), g3), g2), g6 * invT[u]);
+            sdB[u] = fma(fma(-g6, invT[u], g1), invT[u], g2) + t * fma(t, fma(4.0 * g5, t, 3.0 * g4), 2.0 * g3);
+        }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.ns, 0u, 0u, 0u);
+        for (int u = 0; u < NQ; ++u) kf[u] = exp_rate(lnkf[u], etab);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
-                double x[SP];
-                ldv<SP>(X + (w[k].x & 0xFFFF) * S + q0, x);
+        for (int u = 0; u < NQ; ++u) { kr[u] = exp_rate(lnkf[u] - sB[u], etab); kr[u] = rev ? kr[u] : 0.0; }   // Eqs. 23-27
+        double Rf[NQ], Rr[NQ], W[NQ], vq0[NQ], vq1[NQ], vq2[NQ], vh[NQ], vs[6][NQ], cm[NQ];
 #pragma unroll
-                for (int u = 0; u < SP; ++u) Xi[u] = fma(eps, x[u], Xi[u]);
+        for (int u = 0; u < NQ; ++u) {
+            const double c0 = X[x0 + q + u], c1 = X[x1 + q + u], c2 = X[x2 + q + u], c3 = X[x3 + q + u],
+                         c4 = X[x4 + q + u], c5 = X[x5 + q + u];
+            const double p01 = c0 * c1, p34 = c3 * c4;
+            Rf[u] = kf[u] * (p01 * c2); Rr[u] = kr[u] * (p34 * c5);           // Eqs. 18-19
+            const double R = Rf[u] - Rr[u];
+            vq0[u] = R; vq1[u] = 0.0; vq2[u] = 0.0; W[u] = 0.0; cm[u] = 1.0;
+            vh[u] = kRu * T[u] * fma(T[u], sdB[u], dnu);
+            if (LEVEL == 2) {
+                W[u] = sc[kW * S + q + u];
+                const double iT = invT[u];
+                // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
+                const double dRf = Rf[u] * fma(-snf, iT, L[u]);
+                const double dRr = Rr[u] * (fma(-snr, iT, L[u]) - sdB[u]);
+                vq2[u] = fma(R, iT, dRf - dRr);
+                vq1[u] = W[u] * (R - fma(Rf[u], snf, -Rr[u] * snr));
+                const double nkr = -kr[u];
+                vs[0][u] = kf[u] * (c1 * c2); vs[1][u] = kf[u] * (c0 * c2); vs[2][u] = kf[u] * p01;     // Eq. 120
+                vs[3][u] = nkr * (c4 * c5); vs[4][u] = nkr * (c3 * c5); vs[5][u] = nkr * p34;           // Eq. 121
             }
         }
-        if (pdep) {
+        if (GEN) {
+            // ---- pressure modification c_i (Eq. 20) and its derivatives (Eqs. 77-100): q_i = c R,
+            // Theta = dc/dT R + c Theta0, a = c a0 + b (rho - W [X]_i), s'_ij = c s0_ij, and b (alpha_ij - 1)
+            // per efficiency; lanes without a pressure dependence keep c = 1, b = 0
+            double Xi[NQ], bb[NQ], dcdT[NQ];
 #pragma unroll
-            for (int u = 0; u < SP; ++u) {
-                const double R = vq[0][u], iT = invT[u], Tu = T[u];
-                double cc, G, lPrT, fT = 0.0;
-                if (type == PYJAC_THIRD_BODY) {
-                    cc = Xi[u]; G = Xi[u]; lPrT = -iT; bb[u] = R;            // Eqs. 79-80
-                } else {
-                    const double Pr = exp_rate(fma(dbeta, lnT[u], fma(-dTa, iT, dlnA))) * Xi[u];   // Eq. 31
-                    lPrT = iT * (dbeta + dTa * iT - 1.0);                    // Eq. 84 / P_r
-                    const int form = meta_form(meta);
-                    double F = 1.0, gF = 0.0;                                // gF = (P_r/F) dF/dP_r
-                    if (form == PYJAC_TROE) {                                // Eqs. 33-35, 90-96
-                        // fp[1], fp[2] hold 1/T***, 1/T* (mech_pack.cu); three reciprocals serve every quotient
-                        const double a = fp[0], i3 = fp[1], i1 = fp[2];
-                        const double e3 = exp_rate(-Tu * i3), e1 = exp_rate(-Tu * i1);
-                        const double e2 = fp[4] != 0.0 ? exp_rate(-fp[3] * iT) : 0.0;
-                        const double Fc = (1.0 - a) * e3 + a * e1 + e2;
-                        const double dFc = -(1.0 - a) * i3 * e3 - a * i1 * e1 + fp[3] * iT * iT * e2;
-                        const double lnFc = log(Fc);
-                        const double lF = lnFc * kInvLn10, lP = log10(Pr);
-                        const double At = lP - 0.67 * lF - 0.4;
-                        const double Bt = 0.806 - 1.1762 * lF - 0.14 * lP;
-                        const double rB = 1.0 / Bt, rF = 1.0 / Fc;
-                        const double AB = At * rB, rq = 1.0 / (1.0 + AB * AB);
-                        F = exp_rate(lnFc * rq);
-                        const double k2 = lnFc * 2.0 * At * (rB * rB * rB) * (kInvLn10 * rq * rq);
-                        gF = -k2 * (Bt + 0.14 * At);
-                        fT = (rq - k2 * (1.1762 * At - 0.67 * Bt)) * rF * dFc;
-                    } else if (form == PYJAC_SRI) {                          // Eqs. 36, 97-100
-                        const double ea = exp_rate(-fp[1] * iT), ec = exp_rate(-Tu * fp[2]);       // fp[2] holds 1/c
-                        const double base = fp[0] * ea + ec, lnb = log(base);
-                        const double lP = log10(Pr), Xs = 1.0 / (1.0 + lP * lP);
-                        F = fp[3] * exp_rate(fp[4] * lnT[u] + Xs * lnb);
-                        gF = -Xs * Xs * 2.0 * lP * lnb * kInvLn10;
-                        fT = fp[4] * iT + Xs * (fp[0] * fp[1] * iT * iT * ea - ec * fp[2]) / base;
-                    }
-                    const double i1p = 1.0 / (1.0 + Pr);
-                    double Theta;
-                    if (type == PYJAC_FALLOFF) { cc = Pr * i1p * F; Theta = i1p; }       // Eqs. 82-83
-                    else                       { cc = i1p * F;      Theta = -Pr * i1p; } // Eqs. 86-87
-                    G = cc * (Theta + gF);
-                    bb[u] = R * G / Xi[u];
-                }
-                cm[u] = cc;
-                dcdT[u] = G * lPrT + cc * fT;
-            }
-        }
-        if (LEVEL == 2) {
-#pragma unroll
-            for (int u = 0; u < SP; ++u) mixW[u] = (pdep && !meta_single(meta)) ? sc[kRho * S + q0 + u] - W[u] * Xi[u] : -W[u] * Xi[u];
-#pragma unroll
-            for (int u = 0; u < SP; ++u) {
-                const double R = vq[0][u];
-                vq[2][u] = fma(dcdT[u], R, cm[u] * vq[2][u]);
-                vq[1][u] = fma(bb[u], mixW[u], cm[u] * vq[1][u]);
-#pragma unroll
-                for (int k = 0; k < 6; ++k) vs[k][u] *= cm[u];
-            }
-            for (int e = 0; e < n_eff; e += 128) {
+            for (int u = 0; u < NQ; ++u) { Xi[u] = mixM ? sc[kM * S + q + u] : 0.0; bb[u] = 0.0; dcdT[u] = 0.0; }
+            for (int e = 0; e < n_eff; e += 128) {                       // Eqs. 28-30, four entries at a time
                 uint4 w[4];
 #pragma unroll
-                for (int k = 0; k < 4; ++k) w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
+                for (int k = 0; k < 4; ++k) w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.ns, 0u, 0u, 0u);
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
-                    double t[SP];
+                    const int xo = (w[k].x & 0xFFFF) * S + q;
 #pragma unroll
-                    for (int u = 0; u < SP; ++u) t[u] = bb[u] * eps;
-                    stv<SP>(E + (w[k].x >> 16) * S + q0, t);
+                    for (int u = 0; u < NQ; ++u) Xi[u] = fma(eps, X[xo + u], Xi[u]);
                 }
             }
+            if (pdep) {
+#pragma unroll
+                for (int u = 0; u < NQ; ++u) {
+                    const double R = vq0[u], iT = invT[u], Tu = T[u];
+                    double cc, G, lPrT, fT = 0.0;
+                    if (type == PYJAC_THIRD_BODY) {
+                        cc = Xi[u]; G = Xi[u]; lPrT = -iT; bb[u] = R;            // Eqs. 79-80
+                    } else {
+                        const double Pr = exp_rate(fma(dbeta, lnT[u], fma(-dTa, iT, dlnA)), etab) * Xi[u];   // Eq. 31
+                        lPrT = iT * (dbeta + dTa * iT - 1.0);                    // Eq. 84 / P_r
+                        const int form = meta_form(meta);
+                        double F = 1.0, gF = 0.0;                                // gF = (P_r/F) dF/dP_r
+                        if (form == PYJAC_TROE) {                                // Eqs. 33-35, 90-96
+                            // fp[1], fp[2] hold 1/T***, 1/T* (mech_pack.cu); three reciprocals serve every quotient
+                            const double a = fp[0], i3 = fp[1], i1 = fp[2];
+                            const double e3 = exp_rate(-Tu * i3, etab), e1 = exp_rate(-Tu * i1, etab);
+                            const double e2 = fp[4] != 0.0 ? exp_rate(-fp[3] * iT, etab) : 0.0;
+                            const double Fc = (1.0 - a) * e3 + a * e1 + e2;
+                            const double dFc = -(1.0 - a) * i3 * e3 - a * i1 * e1 + fp[3] * iT * iT * e2;
+                            const double lnFc = log(Fc);
+                            const double lF = lnFc * kInvLn10, lP = log10(Pr);
+                            const double At = lP - 0.67 * lF - 0.4;
+                            const double Bt = 0.806 - 1.1762 * lF - 0.14 * lP;
+                            const double rB = 1.0 / Bt, rF = 1.0 / Fc;
+                            const double AB = At * rB, rq = 1.0 / (1.0 + AB * AB);
+                            F = exp_rate(lnFc * rq, etab);
+                            const double k2 = lnFc * 2.0 * At * (rB * rB * rB) * (kInvLn10 * rq * rq);
+                            gF = -k2 * (Bt + 0.14 * At);
+                            fT = (rq - k2 * (1.1762 * At - 0.67 * Bt)) * rF * dFc;
+                        } else if (form == PYJAC_SRI) {                          // Eqs. 36, 97-100
+                            const double ea = exp_rate(-fp[1] * iT, etab), ec = exp_rate(-Tu * fp[2], etab);   // fp[2] holds 1/c
+                            const double base = fp[0] * ea + ec, lnb = log(base);
+                            const double lP = log10(Pr), Xs = 1.0 / (1.0 + lP * lP);
+                            F = fp[3] * exp_rate(fp[4] * lnT[u] + Xs * lnb, etab);
+                            gF = -Xs * Xs * 2.0 * lP * lnb * kInvLn10;
+                            fT = fp[4] * iT + Xs * (fp[0] * fp[1] * iT * iT * ea - ec * fp[2]) / base;
+                        }
+                        const double i1p = 1.0 / (1.0 + Pr);
+                        double Theta;
+                        if (type == PYJAC_FALLOFF) { cc = Pr * i1p * F; Theta = i1p; }       // Eqs. 82-83
+                        else                       { cc = i1p * F;      Theta = -Pr * i1p; } // Eqs. 86-87
+                        G = cc * (Theta + gF);
+                        bb[u] = R * G / Xi[u];
+                    }
+                    cm[u] = cc;
+                    dcdT[u] = G * lPrT + cc * fT;
+                }
+            }
+            if (LEVEL == 2) {
+#pragma unroll
+                for (int u = 0; u < NQ; ++u) {
+                    const double mixW = mixM ? sc[kRho * S + q + u] - W[u] * Xi[u] : -W[u] * Xi[u];
+                    const double R = vq0[u];
+                    vq2[u] = fma(dcdT[u], R, cm[u] * vq2[u]);
+                    vq1[u] = fma(bb[u], mixW, cm[u] * vq1[u]);
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) vs[k][u] *= cm[u];
+                }
+                for (int e = 0; e < n_eff; e += 128) {
+                    uint4 w[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
+                        const int eo = (w[k].x >> 16) * S + q;
+#pragma unroll
+                        for (int u = 0; u < NQ; ++u) E[eo + u] = bb[u] * eps;
+                    }
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < NQ; ++u) vq0[u] *= cm[u];
         }
 #pragma unroll
-        for (int u = 0; u < SP; ++u) vq[0][u] *= cm[u];
-    }
-    if (LEVEL == 0) {
-#pragma unroll
-        for (int u = 0; u < SP; ++u) {
-            const long long st = state0 + q0 + u;
-            if (st < n) {
-                const long long o = st * nr + orig;
-                if (out.rf) out.rf[o] = Rfv[u];
-                if (out.rr) out.rr[o] = Rrv[u];
-                if (out.cmod) out.cmod[o] = cm[u];
+        for (int u = 0; u < NQ; ++u) {
+            if (LEVEL == 0) {
+                const long long st = state0 + q + u;
+                if (st < n) {
+                    const long long o = st * nr + orig;
+                    if (out.rf) out.rf[o] = Rf[u];
+                    if (out.rr) out.rr[o] = Rr[u];
+                    if (out.cmod) out.cmod[o] = cm[u];
+                }
+            }
+            E[eq + q + u] = vq0[u];
+            if (LEVEL >= 1) E[eh + q + u] = vh[u];
+            if (LEVEL == 2) {
+                E[eq + S + q + u] = vq1[u];
+                E[eq + 2 * S + q + u] = vq2[u];
+                E[v0 + q + u] = vs[0][u]; E[v1 + q + u] = vs[1][u]; E[v2 + q + u] = vs[2][u];
+                E[v3 + q + u] = vs[3][u]; E[v4 + q + u] = vs[4][u]; E[v5 + q + u] = vs[5][u];
             }
         }
-    }
-    stv<SP>(E + (m.eQ + 3 * s) * S + q0, vq[0]);
-    if (LEVEL >= 1) stv<SP>(E + (m.eH + s) * S + q0, vh);
-    if (LEVEL == 2) {
-        stv<SP>(E + (m.eQ + 3 * s + 1) * S + q0, vq[1]);
-        stv<SP>(E + (m.eQ + 3 * s + 2) * S + q0, vq[2]);
-        stv<SP>(E + v0 + q0, vs[0]); stv<SP>(E + v1 + q0, vs[1]); stv<SP>(E + v2 + q0, vs[2]);
-        stv<SP>(E + v3 + q0, vs[3]); stv<SP>(E + v4 + q0, vs[4]); stv<SP>(E + v5 + q0, vs[5]);
-    }
+    };
+    int q = q0;
+#pragma unroll 1
+    for (; !GEN && q + 2 <= q1; q += 2) body(IntC<2>{}, q);
+#pragma unroll 1
+    for (; GEN && q + 1 < q1; ++q) body(IntC<1>{}, q);
+    if (q < q1) body(IntC<1>{}, q);
 }
 
 // ---- P1, general path: one reaction of any type, one state (q) ----------------------------------------
 template <int LEVEL, int S>
 __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *E, const double *X,
-                                         const double *sc, int s, int q, const EvalOut &out, long long state0, long long n)
+                                         const double *sc, const double *etab, int s, int q, const EvalOut &out,
+                                         long long state0, long long n)
 {
     const uint4 sl = m.slots[s];
     const uint32_t meta = sl.w;
@@ -512,7 +524,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             lnkf = sum * kLn10;
             L = kLn10 * invT * dsum * (-2.0 * invT) / (iTmax - iTmin);
         }
-        const double kf = exp_rate(lnkf);
+        const double kf = exp_rate(lnkf, etab);
 
         // ---- sum_k nu_ki B_k (Eq. 27 over the reaction), its T derivative (Eq. 74) and the reaction
         //      enthalpy H_i = sum_k nu_ki h_k W_k = R T (T d(sum nu B)/dT + sum nu)
@@ -557,11 +569,11 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         // ---- reverse rate coefficient (Eqs. 23-27, 69, 75)
         double kr = 0.0, Lr = 0.0;
         if (rev == PYJAC_REV_FROM_KC) {
-            kr = exp_rate(lnkf - sB);
+            kr = exp_rate(lnkf - sB, etab);
             Lr = L - sdB;
         } else if (rev == PYJAC_REV_EXPLICIT) {
             const double rb = m.rev_beta[s], rTa = m.rev_Ta[s];
-            kr = exp_rate(m.rev_lnA[s] + rb * lnT - rTa * invT);
+            kr = exp_rate(m.rev_lnA[s] + rb * lnT - rTa * invT, etab);
             Lr = (rb + rTa * invT) * invT;
         }
         const double Rf = kf * Pf;
@@ -587,14 +599,14 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             if (type == PYJAC_THIRD_BODY) {
                 c = Xi; G = Xi; lPrT = -invT; b = R;                     // Eqs. 79-80
             } else {
-                const double Pr = exp_rate(lnk0 - lnkinf) * Xi;          // Eq. 31
+                const double Pr = exp_rate(lnk0 - lnkinf, etab) * Xi;          // Eq. 31
                 const int form = meta_form(meta);
                 double F = 1.0, gF = 0.0;                                // gF = (P_r/F) dF/dP_r
                 if (form == PYJAC_TROE) {                                // Eqs. 33-35, 90-96
                     // fp[1], fp[2] hold 1/T***, 1/T* (mech_pack.cu); three reciprocals serve every quotient
                     const double a = fp[0], i3 = fp[1], i1 = fp[2];
-                    const double e3 = exp_rate(-T * i3), e1 = exp_rate(-T * i1);
-                    const double e2 = fp[4] != 0.0 ? exp_rate(-fp[3] * invT) : 0.0;
+                    const double e3 = exp_rate(-T * i3, etab), e1 = exp_rate(-T * i1, etab);
+                    const double e2 = fp[4] != 0.0 ? exp_rate(-fp[3] * invT, etab) : 0.0;
                     const double Fc = (1.0 - a) * e3 + a * e1 + e2;
                     const double dFc = -(1.0 - a) * i3 * e3 - a * i1 * e1 + fp[3] * invT * invT * e2;
                     const double lnFc = log(Fc);
@@ -603,15 +615,15 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
                     const double Bt = 0.806 - 1.1762 * lF - 0.14 * lP;
                     const double rB = 1.0 / Bt, rF = 1.0 / Fc;
                     const double AB = At * rB, rq = 1.0 / (1.0 + AB * AB);
-                    F = exp_rate(lnFc * rq);
+                    F = exp_rate(lnFc * rq, etab);
                     const double k2 = lnFc * 2.0 * At * (rB * rB * rB) * (kInvLn10 * rq * rq);
                     gF = -k2 * (Bt + 0.14 * At);
                     fT = (rq - k2 * (1.1762 * At - 0.67 * Bt)) * rF * dFc;
                 } else if (form == PYJAC_SRI) {                          // Eqs. 36, 97-100
-                    const double ea = exp_rate(-fp[1] * invT), ec = exp_rate(-T * fp[2]);       // fp[2] holds 1/c
+                    const double ea = exp_rate(-fp[1] * invT, etab), ec = exp_rate(-T * fp[2], etab);       // fp[2] holds 1/c
                     const double base = fp[0] * ea + ec, lnb = log(base);
                     const double lP = log10(Pr), Xs = 1.0 / (1.0 + lP * lP);
-                    F = fp[3] * exp_rate(fp[4] * lnT + Xs * lnb);
+                    F = fp[3] * exp_rate(fp[4] * lnT + Xs * lnb, etab);
                     gF = -Xs * Xs * 2.0 * lP * lnb * kInvLn10;
                     fT = fp[4] * invT + Xs * (fp[0] * fp[1] * invT * invT * ea - ec * fp[2]) / base;
                 }
@@ -719,11 +731,11 @@ __device__ __forceinline__ void st_cs_v2(double *p, double a, double b)
 // applied to the S states; whole blocks of four steps run without a branch, the chunk's last block by
 // its step count.
 template <int LEVEL, int S>
-__device__ __forceinline__ void a_chunk(const DeviceMech &m, double *E, const double *sc, const uint2 ch, int lane)
+__device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent, double *E, const double *sc, const uint2 ch, int lane)
 {
     const uint32_t kind = (ch.y >> 8) & 0xF;
     const int steps = (int)(ch.y & 0xFF), rshift = (int)(ch.y >> 12) & 0xF, width = 1 << rshift;
-    const uint4 *ep = m.a_ent + ch.x + lane;
+    const uint4 *ep = a_ent + ch.x + lane;
     const uint4 r0 = ep[0];
     const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
     const char *Eb = reinterpret_cast<const char *>(E);
@@ -925,13 +937,13 @@ __device__ __forceinline__ void fix_item(const DeviceMech &m, const double *E, c
 // entry words (padded with the zero slot) and the item's step count; the entries of the next item are
 // fetched while this one is summed.  FAST: all S states are stored and the output is 16-byte aligned.
 template <int S, int RP, bool FAST>
-__device__ __forceinline__ void b_run(const DeviceMech &m, const double *E, const double *colc, const double *wrow,
+__device__ __forceinline__ void b_run(const DeviceMech &m, const uint4 *b_ent, const double *E, const double *colc, const double *wrow,
                                       int it0, int it1, int lane, double *J0, int nvalid, bool aligned16)
 {
     const int ld = m.ld;
     const uint32_t j_state = (uint32_t)(ld * ld);
     const char *Eb = reinterpret_cast<const char *>(E);
-    const uint4 *ebase = m.b_ent + lane;
+    const uint4 *ebase = b_ent + lane;
     int it = it0;
     while (it < it1) {
         const int slab = it / ld, c0 = it - slab * ld;
@@ -1017,7 +1029,7 @@ __device__ __forceinline__ void b_run(const DeviceMech &m, const double *E, cons
 // ---- the kernel ------------------------------------------------------------------------------------
 // Shared memory: S interleaved states of sp.total doubles each (E, two mixture parts), then the
 // state-independent column and row constants.
-template <int LEVEL, int S>
+template <int LEVEL, int S, bool STAGE>
 __global__ void __launch_bounds__(kMaxThreads, 1)
     eval_kernel(const DeviceMech m, const SmemPlan sp, long long n, const double *__restrict__ Tg,
                 const double *__restrict__ Pg, const double *__restrict__ Yg, long long ldy, const EvalOut out)
@@ -1030,12 +1042,26 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
     double *E = sm + sp.E * S;
     const double *colc = sm + (size_t)sp.total * S + sp.colc;
     double *wrow = sm + (size_t)sp.total * S + sp.wrow;
+    const double *etab = sm + (size_t)sp.total * S + sp.etab;
     {
+        if (tid < 32) sm[(size_t)sp.total * S + sp.etab + tid] = c_exp2_32[tid];
         double *cw = sm + (size_t)sp.total * S + sp.colc;
         for (int i = tid; i < 4 * ld; i += NT) cw[i] = m.colc[i];
         for (int i = tid; i < ld; i += NT) wrow[i] = m.wrow[i];
         // E starts as zeros: sums without a list, the zero slots and row 0 of alpha' / gamma' stay zero
         for (int i = tid; i < m.n_e * S; i += NT) E[i] = 0.0;
+    }
+    // the gather tables of phases A and B: from global memory (L1 / L2), or staged here once per CTA
+    const uint2 *achunk = m.achunk;
+    const uint4 *a_ent = m.a_ent, *b_ent = m.b_ent;
+    if (STAGE) {
+        uint4 *base = reinterpret_cast<uint4 *>(sm + (size_t)sp.total * S);
+        uint4 *d0 = base + sp.t_achunk / 2, *d1 = base + sp.t_aent / 2, *d2 = base + sp.t_bent / 2;
+        const uint4 *s0 = reinterpret_cast<const uint4 *>(m.achunk);
+        for (int i = tid; i < sp.n_achunk16; i += NT) d0[i] = s0[i];
+        for (int i = tid; i < sp.n_aent16; i += NT) d1[i] = m.a_ent[i];
+        for (int i = tid; i < sp.n_bent16; i += NT) d2[i] = m.b_ent[i];
+        achunk = reinterpret_cast<const uint2 *>(d0); a_ent = d1; b_ent = d2;
     }
     if (tid < S) {     // the empty-slot dummy species of both mixture parts
         sm[(sp.P0 + sp.oX + ns) * S + tid] = 1.0;
@@ -1055,44 +1081,69 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
                                       min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
     }
     __syncthreads();
+#ifdef PYJAC_PROF
+    long long tP1 = 0, tP1w = 0, tA = 0, tAw = 0, tB = 0, tBw = 0, t0, t1;
+    int nb_ = 0;
+#define PROF_T(x) x = clock64();
+#define PROF_ACC(acc, a, b_) acc += (b_) - (a);
+#else
+#define PROF_T(x)
+#define PROF_ACC(acc, a, b_)
+#endif
     for (long long b = blockIdx.x; b < nbatch; b += gridDim.x, par ^= 1) {
         const long long state0 = b * S;
+        PROF_T(t0)
         double *P0 = sm + (sp.P0 + par * sp.p0size) * S;
         const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S;
         // ---- P1: reactions
-        for (int it = grab(&ctr[0], lane); it < n_p1; it = grab(&ctr[0], lane)) {
+        // the queue starts with the mixtures of the NEXT batch (into the other mixture part, which nobody reads
+        // during this iteration): their input reads from HBM overlap the reactions
+        const bool more = b + gridDim.x < nbatch;
+        for (int it = grab(&ctr[0], lane); it < n_p1 + S; it = grab(&ctr[0], lane)) {
+            if (it < S) {
+                if (more) {
+                    double *Pn = sm + (sp.P0 + (par ^ 1) * sp.p0size) * S;
+                    mixture_and_species<LEVEL, S>(m, Pn + sp.oX * S, Pn + sp.oCp * S, Pn + sp.oScal * S, it,
+                                                  min((b + gridDim.x) * S + it, n - 1), Tg, Pg, Yg, ldy, lane);
+                }
+                continue;
+            }
             // item = {group of 32 reactions, path, first state}: most expensive first (device_mech.h `p1item`)
-            const uint32_t w = m.p1item[it];
-            const int c = (int)(w & 0xFFFF), kind = (int)(w >> 16) & 0xF, q = (int)(w >> 20);
+            const uint32_t w = m.p1item[it - S];
+            const int c = (int)(w & 0xFFFF), kind = (int)(w >> 16) & 0xF, q = (int)(w >> 20) & 0xF, nq = (int)(w >> 24);
             const int s = min(c * 32 + lane, nr - 1);
-            if (kind == 1) fast_reactions<LEVEL, S, false>(m, E, X, sc, s, q, out, state0, n);
-            else if (kind == 2) fast_reactions<LEVEL, S, true>(m, E, X, sc, s, q, out, state0, n);
-            else reaction<LEVEL, S>(m, sp, E, X, sc, s, q, out, state0, n);
+            if (kind == 1) p1_group<LEVEL, S, false>(m, E, X, sc, etab, s, q, q + nq, out, state0, n);
+            else if (kind == 2) p1_group<LEVEL, S, true>(m, E, X, sc, etab, s, q, q + nq, out, state0, n);
+            else reaction<LEVEL, S>(m, sp, E, X, sc, etab, s, q, out, state0, n);
         }
+        PROF_T(t1) PROF_ACC(tP1w, t0, t1)
         __syncthreads();
+        PROF_T(t1) PROF_ACC(tP1, t0, t1) PROF_T(t0)
         if (tid == 0) ctr[0] = 0;
         // ---- A: sums over the reactions per species / per column, pieces of the long cell lists
         {
-            const uint2 *hp = m.achunk + warp;
+            const uint2 *hp = achunk + warp;
             uint2 h = *hp;
             for (int row = 0; row < arows; ++row) {
                 hp += NW;
                 const uint2 hn = *hp;                 // the header table is padded by one row
-                a_chunk<LEVEL, S>(m, E, sc, h, lane);
+                a_chunk<LEVEL, S>(m, a_ent, E, sc, h, lane);
                 h = hn;
             }
         }
+        PROF_T(t1) PROF_ACC(tAw, t0, t1)
         __syncthreads();
+        PROF_T(t1) PROF_ACC(tA, t0, t1) PROF_T(t0)
         const int nvalid = (int)min((long long)S, n - state0);
         if (LEVEL == 2) {
             // ---- B: the Jacobian column by column, the energy row
             double *J0 = out.jac + state0 * ((long long)ld * ld);
             if (nvalid == S && aligned16) {
-                if (m.rp == 2) b_run<S, 2, true>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, true);
-                else b_run<S, 1, true>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, true);
+                if (m.rp == 2) b_run<S, 2, true>(m, b_ent, E, colc, wrow, it0, it1, lane, J0, nvalid, true);
+                else b_run<S, 1, true>(m, b_ent, E, colc, wrow, it0, it1, lane, J0, nvalid, true);
             } else {
-                if (m.rp == 2) b_run<S, 2, false>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
-                else b_run<S, 1, false>(m, E, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
+                if (m.rp == 2) b_run<S, 2, false>(m, b_ent, E, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
+                else b_run<S, 1, false>(m, b_ent, E, colc, wrow, it0, it1, lane, J0, nvalid, aligned16);
             }
             for (int it = NW - 1 - warp; it < nfix; it += NW)
                 fix_item<S>(m, E, P0 + sp.oCp * S, sc, colc, wrow, it, lane, J0, nvalid);
@@ -1115,15 +1166,18 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
                     out.dydt[(state0 + q) * ld + r] = v;
                 }
         }
-        // ---- P0 of the next iteration into the other mixture part, by the last warps
-        if (b + gridDim.x < nbatch && warp >= NW - S) {
-            const int q = warp - (NW - S);
-            double *Pn = sm + (sp.P0 + (par ^ 1) * sp.p0size) * S;
-            mixture_and_species<LEVEL, S>(m, Pn + sp.oX * S, Pn + sp.oCp * S, Pn + sp.oScal * S, q,
-                                          min((b + gridDim.x) * S + q, n - 1), Tg, Pg, Yg, ldy, lane);
-        }
+        PROF_T(t1) PROF_ACC(tBw, t0, t1)
         __syncthreads();
+        PROF_T(t1) PROF_ACC(tB, t0, t1)
+#ifdef PYJAC_PROF
+        ++nb_;
+#endif
     }
+#ifdef PYJAC_PROF
+    if (blockIdx.x == 0 && lane == 0)
+        printf("warp %2d batches %d  P1 %lld (own %lld)  A %lld (own %lld)  B+P0 %lld (own %lld) cycles per batch\n", warp, nb_,
+               tP1 / nb_, tP1w / nb_, tA / nb_, tAw / nb_, tB / nb_, tBw / nb_);
+#endif
 }
 
 }  // namespace
@@ -1136,20 +1190,32 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
 #define PYJAC_CAT2(a, b) a##b
 #define PYJAC_NAME(a, s) PYJAC_CAT2(a, s)
 
-const void *PYJAC_NAME(eval_kernel_ptr_, PYJAC_S)(int level)
+const void *PYJAC_NAME(eval_kernel_ptr_, PYJAC_S)(int level, bool stage)
 {
-    return level == 0 ? (const void *)eval_kernel<0, PYJAC_S>
-         : level == 1 ? (const void *)eval_kernel<1, PYJAC_S>
-                      : (const void *)eval_kernel<2, PYJAC_S>;
+    if (stage)
+        return level == 0 ? (const void *)eval_kernel<0, PYJAC_S, true>
+             : level == 1 ? (const void *)eval_kernel<1, PYJAC_S, true>
+                          : (const void *)eval_kernel<2, PYJAC_S, true>;
+    return level == 0 ? (const void *)eval_kernel<0, PYJAC_S, false>
+         : level == 1 ? (const void *)eval_kernel<1, PYJAC_S, false>
+                      : (const void *)eval_kernel<2, PYJAC_S, false>;
 }
 
 cudaError_t PYJAC_NAME(launch_eval_, PYJAC_S)(int level, int threads, const DeviceMech &m, const SmemPlan &sp, int grid,
                                                size_t smem, long long n, const double *T, const double *P,
                                                const double *Y, long long ldy, const EvalOut &out, cudaStream_t stream)
 {
-    if (level == 0) eval_kernel<0, PYJAC_S><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
-    else if (level == 1) eval_kernel<1, PYJAC_S><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
-    else eval_kernel<2, PYJAC_S><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out);
+#define PYJAC_LAUNCH(L, ST) eval_kernel<L, PYJAC_S, ST><<<grid, threads, smem, stream>>>(m, sp, n, T, P, Y, ldy, out)
+    if (sp.staged) {
+        if (level == 0) PYJAC_LAUNCH(0, true);
+        else if (level == 1) PYJAC_LAUNCH(1, true);
+        else PYJAC_LAUNCH(2, true);
+    } else {
+        if (level == 0) PYJAC_LAUNCH(0, false);
+        else if (level == 1) PYJAC_LAUNCH(1, false);
+        else PYJAC_LAUNCH(2, false);
+    }
+#undef PYJAC_LAUNCH
     return cudaGetLastError();
 }
 

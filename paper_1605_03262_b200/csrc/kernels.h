@@ -16,7 +16,7 @@ struct EvalOut {
 
 // level: 0 rates, 1 source term, 2 Jacobian.  S: states a CTA interleaves per iteration (1, 2, 3, 4, 6);
 // threads: a multiple of 32, at least 32 S, up to kMaxThreads.
-const void *eval_kernel_ptr(int level, int S);
+const void *eval_kernel_ptr(int level, int S, bool stage);
 size_t eval_smem_bytes(const SmemPlan &sp, int S);
 cudaError_t launch_eval(int level, int threads, int S, const DeviceMech &m, const SmemPlan &sp, int grid, size_t smem,
                         long long n, const double *T, const double *P, const double *Y, long long ldy,

@@ -541,6 +541,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     REQUIRE(hints.cell_cap >= 0 && hints.cell_cap <= 3, "cell_cap must be 0 (choose) or 1..3");
     REQUIRE(hints.cap >= 0 && hints.rp >= 0 && hints.rp <= 2 && hints.ctas >= 0 && hints.ctas <= 4 && hints.threads >= 0 && hints.S >= 0,
             "launch shape out of range");
+    REQUIRE(hints.p1_states >= 0 && hints.p1_states <= 15, "p1_states out of range");
     const int cell_cap = hints.cell_cap >= 1 ? hints.cell_cap : 3;
     constexpr int kPiece = 8;
     std::vector<std::vector<std::pair<uint32_t, int>>> cell_w((size_t)ld * ld);
@@ -598,7 +599,9 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             while (ctas < 4 && bytes_for(S) <= limit_for(ctas + 1)) ++ctas;
         }
         if (bytes_for(S) > limit_for(ctas)) throw Fail{PYJAC_ELIMIT, "the requested launch shape exceeds shared memory"};
-        int threads = hints.threads > 0 ? hints.threads : (kMaxThreads / ctas) & ~31;
+        // measured on B200 (profiles/r2_shape_sweeps.md): with one state per CTA (the 360-species mechanism)
+        // 384 threads beat 512 (1.55 M against 1.40 M states/s): fewer warps share the one-state queue tails
+        int threads = hints.threads > 0 ? hints.threads : S == 1 && ctas == 1 ? 384 : (kMaxThreads / ctas) & ~31;
         if (threads < 32 * S) threads = 32 * S;
         if (threads < 64) threads = 64;
         if (threads > kMaxThreads || threads % 32) throw Fail{PYJAC_EINVAL, "threads per CTA must be a multiple of 32 up to kMaxThreads"};
@@ -615,11 +618,16 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     // ---- work items of P1: the groups that need the one-state path first, then the pressure-dependent
     // groups, then the plain ones, each for every state (pair)
     {
-        const int SP = S % 2 == 0 ? 2 : 1;
+        // states per fast-path item: all S (the reaction's constants are read once per batch) when several CTAs
+        // share an SM and fill each other's queue tails; one state per item when a single CTA has the SM to
+        // itself (111 species: 6.5 against 8.1 ms per 100,000 states)
+        const int per = hints.p1_states > 0 ? std::min(hints.p1_states, S) : o.ctas_target > 1 ? S : 1;
         for (uint32_t kind : {0u, 2u, 1u})
             for (int c = 0; c < o.n_rchunk; ++c) {
                 if (o.rchunk[c] != kind) continue;
-                for (int q = 0; q < S; q += (kind == 0u ? 1 : SP)) o.p1item.push_back((uint32_t)c | kind << 16 | (uint32_t)q << 20);
+                const int step = kind == 0u ? 1 : per;
+                for (int q = 0; q < S; q += step)
+                    o.p1item.push_back((uint32_t)c | kind << 16 | (uint32_t)q << 20 | (uint32_t)std::min(step, S - q) << 24);
             }
     }
 
@@ -905,6 +913,17 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         while (wi <= NW) o.bsplit[wi++] = (int32_t)cost.size();
     }
 
+    // ---- gather tables in shared memory?  (one copy per CTA, read with 16-byte shared loads instead of
+    // through L1 / L2 for every batch)
+    if (hints.stage == 1) {
+        const SmemPlan pl = make_smem_plan(ns, o.n_e, (int)((o.achunk.size() / 2 + 1) / 2), (int)(o.a_ent.size() / 4),
+                                           (int)(o.b_ent.size() / 4));
+        const long long bytes = ((long long)S * pl.total + pl.shared_total) * 8;
+        if (bytes > std::min<long long>(228 * 1024 / o.ctas_target - 1024 - 128, hints.smem_bytes))
+            throw Fail{PYJAC_ELIMIT, "the gather tables do not fit the shared memory of this launch shape"};
+        o.stage = true;
+    }
+
     // ---- self-check of what the kernels rely on without bounds checks: every source offset and every
     // output index inside the block's E array, every block a chunk or an item reads inside its table
     {
@@ -951,6 +970,7 @@ ShapeHints hints_from_shape(const pyjac_launch_shape *shape, long long smem_opti
     if (shape) {
         h.S = shape->states_per_cta; h.threads = shape->threads; h.ctas = shape->ctas_per_sm;
         h.cap = shape->list_cap; h.cell_cap = shape->cell_cap; h.rp = shape->rows_per_lane;
+        h.p1_states = shape->p1_states; h.stage = shape->stage_tables;
     }
     return h;
 }

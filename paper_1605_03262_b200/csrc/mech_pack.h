@@ -42,6 +42,7 @@ struct HostPack {
     // launch shape chosen with the tables: S states per CTA iteration, threads per CTA, the CTAs per SM
     // the shared-memory footprint was sized for
     int S = 1, threads = 128, ctas_target = 1;
+    bool stage = false;                   // gather tables staged in shared memory
     // statistics (pyjac_pack_stats)
     long long n_cell_entries = 0, n_cells = 0, n_heavy_cells = 0, n_heavy_pieces = 0, n_a_steps = 0, n_b_steps = 0;
     long long n_plain_chunks = 0;
@@ -58,6 +59,8 @@ struct ShapeHints {
     int cap = 0;        // longest list one lane walks in phase A
     int cell_cap = 0;   // longest Jacobian-cell list gathered in phase B (1..3); longer ones are summed piecewise in phase A
     int rp = 0;         // rows per lane in phase B (1 or 2)
+    int p1_states = 0;  // states per work item of the fast reaction path (0: all S)
+    int stage = 0;      // 1: copy the gather tables of phases A and B to shared memory once per CTA
 };
 
 // The hints of an explicit launch shape (NULL: all zeros = choose); `smem_optin` = the device's opt-in
