@@ -3,6 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
                     [--also 2,3] [--sweep short|full|off] [--no-cpu-baseline] [--no-e2e] [--peaks]
+    python bench.py --ncu-target CFG:KERNEL:N      # the short command the ncu captures of profiles/ wrap
+    python bench.py --ncu-import REPORT --ncu-label WORKLOAD:KERNEL:N    # one row of profiles/r2_ncu_counters.csv
 
 A "step" is one pass of the whole hot path (thermo -> rates -> source term -> Jacobian -> store;
 SURVEY.md section 8(a) rows S0-S10, one kernel launch) over one batch of seeded synthetic states.
@@ -290,6 +292,82 @@ def run_peaks():
                       "hbm_copy_gbs": peak, "hbm_copy_source": src}))
 
 
+def run_ncu_target(spec: str):
+    """CFG:KERNEL:N -- three launches (two warm-up) of one kernel on the first N states of a configuration and
+    nothing else: what `ncu --set full -s 2 -c 1` wraps for the captures under profiles/."""
+    import torch
+    from paper_1605_03262_b200 import build, synth
+    from paper_1605_03262_b200.binding import PyJac
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    cfg, kernel, n = spec.split(":")
+    cfg, n = int(cfg), int(n)
+    m = synth.make_mechanism(cfg)
+    T, P, Y = synth.config_states(cfg, min(n, synth.CONFIGS[cfg].n_states))
+    n = len(T)
+    pj = PyJac(m, device=0)
+    dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
+    ld = m.n_species + 1
+    out = torch.empty((n, ld * ld if kernel == "jacobian" else ld), dtype=torch.float64, device="cuda")
+    fn = {"jacobian": lambda: pj.eval_jacobian(dT, dP, dY, out=out),
+          "dydt": lambda: pj.eval_dydt(dT, dP, dY, out=out),
+          "rates": lambda: pj.eval_rates(dT, dP, dY, want=("wdot",))}[kernel]
+    total, per = time_gpu(pj, torch, dT, dP, dY, out, 1, 2, fn=fn)
+    print(json.dumps({"workload": synth.CONFIGS[cfg].name, "kernel": kernel, "n_states": n, "launch_ms": per[0],
+                      "launch_config": pj.launch_config(n)}))
+
+
+NCU_CSV_FIELDS = ("workload", "kernel", "n_states", "kernel_source_sha16", "duration_us", "dram_bytes_per_state",
+                  "fp64_flop_per_state", "fp64_inst_per_state", "warp_inst_per_state", "lsu_wavefronts_per_state",
+                  "shared_wavefronts_per_state", "lsu_data_pipe_pct", "fp64_pipe_pct", "issue_active_pct",
+                  "registers", "source")
+
+
+def run_ncu_import(report: str, label: str):
+    """Reads one kernel from an `.ncu-rep` (`ncu -i REPORT --page raw --csv`, no GPU needed) and prints the row
+    of profiles/r2_ncu_counters.csv that describes it: per-state DRAM bytes, fp64 operations (DFMA counts two
+    flops), warp instructions and L1TEX LSU data-pipe wavefronts, with the hash of the kernel sources."""
+    import csv
+    import io
+    workload, kernel, n = label.split(":")
+    n = float(n)
+    txt = subprocess.run(["ncu", "-i", report, "--page", "raw", "--csv"], capture_output=True, text=True).stdout
+    rows = list(csv.reader(io.StringIO(txt)))
+    d = dict(zip(rows[0], rows[2]))
+    units = dict(zip(rows[0], rows[1]))
+
+    def g(k):
+        v = float(d[k].replace(",", ""))
+        u = units.get(k, "")
+        return v * {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "msecond": 1e3, "second": 1e6}.get(u, 1.0)
+
+    dur_us = g("gpu__time_duration.sum") * (1e-3 if units.get("gpu__time_duration.sum") == "nsecond" else 1.0)
+    cyc = g("smsp__cycles_elapsed.max") if "smsp__cycles_elapsed.max" in d else g("sm__cycles_elapsed.max")
+    ops = {k: g("smsp__sass_thread_inst_executed_op_%s_pred_on.sum.per_cycle_elapsed" % k) * cyc for k in ("dfma", "dmul", "dadd")}
+    # all LSU data-pipe wavefronts (shared + global + local): the shared count scaled by the ratio of the two
+    # utilisation figures the report carries for the same pipe
+    lsu = g("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum") * \
+        g("l1tex__data_pipe_lsu_wavefronts.sum.pct_of_peak_sustained_elapsed") / \
+        g("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed")
+    row = {"workload": workload, "kernel": kernel, "n_states": int(n), "kernel_source_sha16": kernel_source_sha16(),
+           "duration_us": "%.1f" % dur_us,
+           "dram_bytes_per_state": "%.1f" % ((g("dram__bytes_read.sum") + g("dram__bytes_write.sum")) / n),
+           "fp64_flop_per_state": "%.1f" % ((2 * ops["dfma"] + ops["dmul"] + ops["dadd"]) / n),
+           "fp64_inst_per_state": "%.1f" % ((ops["dfma"] + ops["dmul"] + ops["dadd"]) / n),
+           "warp_inst_per_state": "%.1f" % (g("smsp__inst_executed.sum") / n),
+           "lsu_wavefronts_per_state": "%.1f" % (lsu / n),
+           "shared_wavefronts_per_state": "%.1f" % (g("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum") / n),
+           "lsu_data_pipe_pct": "%.1f" % g("l1tex__data_pipe_lsu_wavefronts.sum.pct_of_peak_sustained_elapsed"),
+           "fp64_pipe_pct": "%.1f" % g("sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active"),
+           "issue_active_pct": "%.1f" % g("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+           "registers": int(g("launch__registers_per_thread")), "source": os.path.basename(report)}
+    w = csv.DictWriter(sys.stdout, fieldnames=NCU_CSV_FIELDS)
+    if os.environ.get("NCU_CSV_HEADER"):
+        w.writeheader()
+    w.writerow(row)
+
+
 def max_over_ranks(ms: float, dist, device: str) -> float:
     """Device-timed milliseconds of the timed region, MAX over the ranks (the only collective of the
     run: states are independent, every rank evaluates its own replica)."""
@@ -320,7 +398,16 @@ def main():
     ap.add_argument("--peaks", action="store_true",
                     help="measure the write-only store stream and the fp64 FMA rate (SURVEY.md 8(d)) and exit")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ncu-target", default=None, help="CFG:KERNEL:N (KERNEL = jacobian | dydt | rates): three launches, for ncu")
+    ap.add_argument("--ncu-import", default=None, help="an .ncu-rep to turn into a row of profiles/r2_ncu_counters.csv")
+    ap.add_argument("--ncu-label", default=None, help="WORKLOAD:KERNEL:N of the imported report")
     args = ap.parse_args()
+    if args.ncu_target:
+        run_ncu_target(args.ncu_target)
+        return
+    if args.ncu_import:
+        run_ncu_import(args.ncu_import, args.ncu_label)
+        return
     if args.impl == "reference":
         run_reference(args)
         return

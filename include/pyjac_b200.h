@@ -193,6 +193,25 @@ int pyjac_eval_jacobian_host(const pyjac_mech *mech, int64_t n, const double *T,
 int pyjac_eval_dydt_host(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
                          const double *Y, int64_t ldy, double *dydt, int64_t chunk_states);
 
+/* First-order forward-difference Jacobian from the source term (the paper's own comparison: "a simple
+ * first-order forward difference adapted from CVODE", Tables 4-5), in
+ * the layout of pyjac_eval_jacobian.  With Phi = (T, Y_1 .. Y_{Nsp-1}), N = N_sp unknowns, f = dPhi/dt:
+ *   w_j = 1 / (rtol |Phi_j| + atol),  D_j = max(sqrt(eps) |Phi_j|, sqrt(eps) / w_j),
+ *   J(:, j) = (f(Phi + D_j e_j) - f(Phi)) / D_j
+ * (CVODE's rule with its step-dependent floor 1000 |h| eps N |f| replaced by sqrt(eps): DESIGN.md C21),
+ * a mass-fraction increment being taken from Y_Nsp (Eq. 2); column N_sp is zero.  rtol > 0, atol >= 0.
+ * All pointers are DEVICE pointers.  `work` is caller-owned scratch of `work_doubles` doubles; the
+ * states are evaluated in chunks of work_doubles / pyjac_fd_workspace_doubles(mech, 1) states
+ * (PYJAC_EINVAL if that is zero): 1 + N_sp source-term evaluations per state, 4 kernel launches
+ * per chunk, asynchronous on `stream`, no allocation. */
+int pyjac_eval_jacobian_fd(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
+                           const double *Y, int64_t ldy, double rtol, double atol, double *jac,
+                           double *work, int64_t work_doubles, void *stream);
+
+/* Doubles of scratch pyjac_eval_jacobian_fd needs to evaluate `chunk_states` states at once
+ * (-1 for an invalid argument). */
+int64_t pyjac_fd_workspace_doubles(const pyjac_mech *mech, int64_t chunk_states);
+
 /* Number of kernel launches this library has enqueued since it was loaded (all handles). */
 int64_t pyjac_kernel_launches(void);
 

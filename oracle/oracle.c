@@ -502,3 +502,52 @@ int orc_eval_jacobian_complex_step(const orc_mech *m, long n, const double *T, c
 {
     return orc_eval_jacobian_impl(m, n, T, P, Y, ldy, jac, 1);
 }
+
+/* ---- first-order forward-difference Jacobian of the oracle's own source term ------------------------
+ * The paper's comparison method ("a simple first-order forward difference adapted from
+ * CVODE"; Tables 4-5).  The paper does not print the increment rule; DESIGN.md reading
+ * C21 is followed step by step: with Phi = (T, Y_1 .. Y_{Ns-1}), N = N_s unknowns, f = dPhi/dt,
+ *   w_j = 1 / (rtol |Phi_j| + atol),  D_j = max(sqrt(eps) |Phi_j|, sqrt(eps) / w_j),
+ *   J(:,j) = (f(Phi + D_j e_j) - f(Phi)) / D_j,
+ * a mass-fraction increment being taken from Y_Ns (Eq. 2).  Layout of orc_eval_jacobian; column N_s zero. */
+int orc_eval_jacobian_fd(const orc_mech *m, long n, const double *T, const double *P, const double *Y,
+                         long ldy, double rtol, double atol, double *jac)
+{
+    int err = 0;
+    const int ns = m->ns, LD = ns + 1, last = ns - 1;
+    const size_t stride = (size_t)LD * LD;
+    const double eps = 2.220446049250313e-16, srur = sqrt(eps);
+#pragma omp parallel
+    {
+        orc_work_d w;
+        double *f0 = (double *)malloc((size_t)LD * sizeof(double));
+        double *Yp = (double *)malloc((size_t)ns * sizeof(double));
+        if (!f0 || !Yp || orc_work_alloc_d(&w, m->ns, m->nr) != 0) {
+#pragma omp atomic write
+            err = -1;
+        } else {
+#pragma omp for schedule(static)
+            for (long s = 0; s < n; ++s) {
+                const double *Ys = Y + s * ldy;
+                double *J = jac + s * stride;
+                memset(J, 0, stride * sizeof(double));
+                orc_source_d(m, T[s], P[s], Ys, &w);
+                for (int r = 0; r < LD; ++r) f0[r] = w.dydt[r];
+                for (int j = 0; j < ns; ++j) {
+                    const double phi = j == 0 ? T[s] : Ys[j - 1];
+                    const double a = srur * fabs(phi), b = srur * (rtol * fabs(phi) + atol);
+                    const double d = a > b ? a : b;
+                    double Tp = T[s];
+                    for (int k = 0; k < ns; ++k) Yp[k] = Ys[k];
+                    if (j == 0) Tp = T[s] + d;
+                    else { Yp[j - 1] = Ys[j - 1] + d; Yp[last] = Yp[last] - d; }
+                    orc_source_d(m, Tp, P[s], Yp, &w);
+                    for (int r = 0; r < LD; ++r) J[r + (size_t)j * LD] = (w.dydt[r] - f0[r]) / d;
+                }
+            }
+            orc_work_free_d(&w);
+        }
+        free(f0); free(Yp);
+    }
+    return err;
+}

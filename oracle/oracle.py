@@ -141,6 +141,20 @@ class Oracle:
         return self._jac(self.lib.orc_eval_jacobian_complex_step, T, P, Y)
 
 
+    def jacobian_fd(self, T, P, Y, rtol: float = 1e-8, atol: float = 1e-15):
+        """First-order forward-difference Jacobian of the oracle's source term with the increments of
+        DESIGN.md reading C21 (the paper's comparison method): [n][(ns+1)^2]."""
+        T, P, Y = self._state(T, P, Y)
+        n = T.shape[0]
+        ld = self.ns + 1
+        jac = np.empty((n, ld * ld))
+        rc = self.lib.orc_eval_jacobian_fd(C.byref(self._s), C.c_long(n), _dp(T), _dp(P), _dp(Y),
+                                           C.c_long(Y.shape[1]), C.c_double(rtol), C.c_double(atol), _dp(jac))
+        if rc != 0:
+            raise MemoryError("oracle allocation failed")
+        return jac
+
+
 def as_matrix(jac_flat, ns):
     """[n][(ns+1)^2] column-major -> [n][row][col]"""
     ld = ns + 1

@@ -47,7 +47,8 @@ class LaunchShape(C.Structure):
 
 EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_sizes",
            "pyjac_eval_rates", "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
-           "pyjac_eval_dydt_host", "pyjac_kernel_launches", "pyjac_jacobian_launch_config", "pyjac_strerror")
+           "pyjac_eval_dydt_host", "pyjac_eval_jacobian_fd", "pyjac_fd_workspace_doubles", "pyjac_kernel_launches",
+           "pyjac_jacobian_launch_config", "pyjac_strerror")
 TOOLS_EXPORTS = ("pyjac_tools_pack_stats", "pyjac_tools_peak_store_stream", "pyjac_tools_peak_dfma")
 
 _lib = None
@@ -74,6 +75,9 @@ def load_library(path: str | None = None):
     lib.pyjac_eval_jacobian.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp]
     lib.pyjac_eval_jacobian_host.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64]
     lib.pyjac_eval_dydt_host.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64]
+    lib.pyjac_eval_jacobian_fd.argtypes = [vp, i64, vp, vp, vp, i64, C.c_double, C.c_double, vp, vp, i64, vp]
+    lib.pyjac_fd_workspace_doubles.argtypes = [vp, i64]
+    lib.pyjac_fd_workspace_doubles.restype = i64
     lib.pyjac_kernel_launches.argtypes = []
     lib.pyjac_kernel_launches.restype = i64
     lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 5
@@ -281,6 +285,27 @@ class PyJac:
         out = self._dev_out(out, n, ld * ld, T)
         _check(self.lib.pyjac_eval_jacobian(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
                                             out.data_ptr(), self._stream()), "pyjac_eval_jacobian")
+        return out
+
+    def fd_workspace_doubles(self, chunk_states: int) -> int:
+        return int(self.lib.pyjac_fd_workspace_doubles(self._h, int(chunk_states)))
+
+    def eval_jacobian_fd(self, T, P, Y, out=None, rtol: float = 1e-8, atol: float = 1e-15, work=None,
+                         chunk_states: int = 4096):
+        """First-order forward-difference Jacobians from the source term (pyjac_eval_jacobian_fd), same layout
+        as eval_jacobian.  `work`: a float64 CUDA tensor of scratch (default: one for `chunk_states` states)."""
+        import torch
+        n, ldy = self._dev_inputs(T, P, Y)
+        ld = self.ns + 1
+        out = self._dev_out(out, n, ld * ld, T)
+        if work is None:
+            work = torch.empty(self.fd_workspace_doubles(max(1, min(int(chunk_states), n))), dtype=torch.float64,
+                               device=T.device)
+        if not work.is_cuda or work.dtype != torch.float64 or not work.is_contiguous() or work.device != T.device:
+            raise ValueError("work must be a contiguous float64 CUDA tensor on the inputs' device")
+        _check(self.lib.pyjac_eval_jacobian_fd(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
+                                               float(rtol), float(atol), out.data_ptr(), work.data_ptr(),
+                                               int(work.numel()), self._stream()), "pyjac_eval_jacobian_fd")
         return out
 
     # ---- host-pointer calls (copies inside; synchronous)

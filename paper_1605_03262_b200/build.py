@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libpyjac_b200.so")
 TOOLS_SO = os.path.join(HERE, "libpyjac_b200_tools.so")          # bench / test helpers, not the product
-HOST_SOURCES = ["api.cu", "mech_pack.cu", "dispatch.cu", "tools.cu"]
+HOST_SOURCES = ["api.cu", "mech_pack.cu", "dispatch.cu", "fd.cu", "tools.cu"]
 # states a CTA interleaves per iteration -- keep in step with csrc/dispatch.cu
 KERNEL_S = [1, 2, 3, 4, 6]
 HEADERS = ["device_mech.h", "kernels.h", "mech_pack.h", os.path.join("..", "..", "include", "pyjac_b200.h"),

@@ -80,6 +80,11 @@ int launch(const pyjac_mech *m, int level, int64_t n, const double *T, const dou
 
 }  // namespace
 
+namespace pyjac {
+void count_launches(int k) { g_launches.fetch_add(k, std::memory_order_relaxed); }
+int mech_device(const pyjac_mech *m) { return m->device; }
+}  // namespace pyjac
+
 extern "C" {
 
 int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)

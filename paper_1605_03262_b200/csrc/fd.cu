@@ -1,0 +1,126 @@
+// fd.cu -- first-order forward-difference Jacobian built on the source-term kernel (Section 5.2:
+// "a simple first-order forward difference adapted from CVODE", the paper's own comparison, Tables 4-5
+// PAPER.md:823-853).  SURVEY.md section 8(f) row f2; the increment rule is DESIGN.md reading C21.
+//
+// Per state, with Phi = (T, Y_1 .. Y_{Ns-1}), N = N_s unknowns and f = dPhi/dt (pyjac_eval_dydt):
+//   w_j    = 1 / (rtol |Phi_j| + atol)                        error weights
+//   D_j    = max(sqrt(eps) |Phi_j|, sigma_0 / w_j)            increment of unknown j, sigma_0 = sqrt(eps)
+//   J(:,j) = (f(Phi + D_j e_j) - f(Phi)) / D_j                 a mass-fraction increment is taken from Y_Ns (Eq. 2)
+// (CVODE's sigma_0 = 1000 |h| eps N |f|_wrms carries the integrator's step h, which a stand-alone evaluation
+// does not have.)
+// Three steps per chunk of states: the source term of the states, one warp per state for the increments
+// and the N perturbed states, the source term of those, and the difference quotient in the layout of
+// pyjac_eval_jacobian (column N_s is zero).
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "kernels.h"
+
+namespace {
+
+constexpr double kSqrtEps = 1.4901161193847656e-08;
+
+// one warp per state: increments inc[s][j] and the perturbed states (state s, unknown j) at row s * ns + j
+__global__ void fd_perturb_kernel(int ns, long long n, const double *__restrict__ T, const double *__restrict__ P,
+                                  const double *__restrict__ Y, long long ldy, double rtol, double atol, double *__restrict__ inc, double *__restrict__ Tp,
+                                  double *__restrict__ Pp, double *__restrict__ Yp)
+{
+    const int lane = threadIdx.x & 31;
+    const long long s = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (s >= n) return;
+    const int last = ns - 1;
+    const double *Ys = Y + s * ldy;
+    const double Ts = T[s], Ps = P[s];
+    for (int j = 0; j < ns; ++j) {
+        const double phi = j == 0 ? Ts : Ys[j - 1];
+        const double d = fmax(kSqrtEps * fabs(phi), kSqrtEps * (rtol * fabs(phi) + atol));
+        const long long row = s * ns + j;
+        if (lane == 0) {
+            inc[row] = d;
+            Tp[row] = j == 0 ? Ts + d : Ts;
+            Pp[row] = Ps;
+        }
+        double *yp = Yp + row * ns;
+        for (int k = lane; k < ns; k += 32) {
+            double y = Ys[k];
+            if (j > 0 && k == j - 1) y += d;
+            if (j > 0 && k == last) y -= d;
+            yp[k] = y;
+        }
+    }
+}
+
+// J[s][r + j ld] = (f1[s ns + j][r] - f0[s][r]) / inc[s][j]; column ns is zero
+__global__ void fd_difference_kernel(int ns, long long n, const double *__restrict__ f0, const double *__restrict__ f1,
+                                     const double *__restrict__ inc, double *__restrict__ jac)
+{
+    const int ld = ns + 1;
+    const long long per = (long long)ld * ld;
+    const long long total = n * per;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+        const long long s = i / per;
+        const int e = (int)(i - s * per), j = e / ld, r = e - j * ld;
+        double v = 0.0;
+        if (j < ns) v = (f1[(s * ns + j) * ld + r] - f0[s * ld + r]) / inc[s * ns + j];
+        __stcs(jac + i, v);
+    }
+}
+
+}  // namespace
+
+extern "C" {
+
+int64_t pyjac_fd_workspace_doubles(const pyjac_mech *m, int64_t chunk_states)
+{
+    int32_t ns = 0;
+    if (pyjac_mech_sizes(m, &ns, nullptr) != PYJAC_OK || chunk_states < 1) return -1;
+    const int64_t ld = ns + 1;
+    // f0, inc, perturbed T and P, perturbed Y, f1
+    return chunk_states * (ld + (int64_t)ns + 2 * (int64_t)ns + (int64_t)ns * ns + (int64_t)ns * ld);
+}
+
+int pyjac_eval_jacobian_fd(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                           int64_t ldy, double rtol, double atol, double *jac, double *work, int64_t work_doubles,
+                           void *stream)
+{
+    int32_t ns = 0;
+    if (pyjac_mech_sizes(m, &ns, nullptr) != PYJAC_OK || n < 0) return PYJAC_EINVAL;
+    if (n == 0) return PYJAC_OK;
+    if (!T || !P || !Y || !jac || !work || ldy < ns || !(rtol > 0.0) || !(atol >= 0.0)) return PYJAC_EINVAL;
+    const int64_t per_state = pyjac_fd_workspace_doubles(m, 1);
+    int64_t chunk = work_doubles / per_state;
+    if (chunk < 1) return PYJAC_EINVAL;
+    if (chunk > n) chunk = n;
+    const int64_t ld = ns + 1;
+    double *f0 = work, *inc = f0 + chunk * ld, *Tp = inc + chunk * ns, *Pp = Tp + chunk * ns,
+           *Yp = Pp + chunk * ns, *f1 = Yp + chunk * ns * ns;
+    cudaStream_t st = (cudaStream_t)stream;
+    int prev = -1;
+    const int device = pyjac::mech_device(m);
+    if (cudaGetDevice(&prev) != cudaSuccess) return PYJAC_ECUDA;
+    if (prev != device && cudaSetDevice(device) != cudaSuccess) return PYJAC_ECUDA;
+    int result = PYJAC_OK;
+    for (int64_t s0 = 0; s0 < n && result == PYJAC_OK; s0 += chunk) {
+        const int64_t c = n - s0 < chunk ? n - s0 : chunk;
+        int rc = pyjac_eval_dydt(m, c, T + s0, P + s0, Y + s0 * ldy, ldy, f0, stream);
+        if (rc != PYJAC_OK) { result = rc; break; }
+        const int warps = 8;
+        fd_perturb_kernel<<<(unsigned)((c + warps - 1) / warps), 32 * warps, 0, st>>>(
+            ns, c, T + s0, P + s0, Y + s0 * ldy, ldy, rtol, atol, inc, Tp, Pp, Yp);
+        if (cudaGetLastError() != cudaSuccess) { result = PYJAC_ECUDA; break; }
+        pyjac::count_launches(1);
+        rc = pyjac_eval_dydt(m, c * ns, Tp, Pp, Yp, ns, f1, stream);
+        if (rc != PYJAC_OK) { result = rc; break; }
+        const long long total = (long long)c * ld * ld;
+        const long long blocks = (total + 255) / 256;
+        fd_difference_kernel<<<(unsigned)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, st>>>(
+            ns, c, f0, f1, inc, jac + s0 * ld * ld);
+        if (cudaGetLastError() != cudaSuccess) { result = PYJAC_ECUDA; break; }
+        pyjac::count_launches(1);
+    }
+    if (prev != device) cudaSetDevice(prev);
+    return result;
+}
+
+}  // extern "C"

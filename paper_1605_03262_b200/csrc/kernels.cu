@@ -22,9 +22,6 @@
 //       finish and store the energy row (Eq. 113).
 // There are no atomics on data: every sum has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
-#ifdef PYJAC_PROF
-#include <cstdio>
-#endif
 
 #include "device_mech.h"
 #include "kernels.h"
@@ -724,7 +721,7 @@ __device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double 
 // 16-byte streaming store of two consecutive Jacobian rows
 __device__ __forceinline__ void st_cs_v2(double *p, double a, double b)
 {
-    asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(p), "d"(a), "d"(b) : "memory");
+    __stcs(reinterpret_cast<double2 *>(p), make_double2(a, b));     // st.global.cs.v2.f64; no compiler barrier
 }
 
 // ---- phase A, one chunk: 32 lanes, 32 >> rshift sums (device_mech.h).  An entry is decoded once and
@@ -1081,18 +1078,8 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
                                       min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
     }
     __syncthreads();
-#ifdef PYJAC_PROF
-    long long tP1 = 0, tP1w = 0, tA = 0, tAw = 0, tB = 0, tBw = 0, t0, t1;
-    int nb_ = 0;
-#define PROF_T(x) x = clock64();
-#define PROF_ACC(acc, a, b_) acc += (b_) - (a);
-#else
-#define PROF_T(x)
-#define PROF_ACC(acc, a, b_)
-#endif
     for (long long b = blockIdx.x; b < nbatch; b += gridDim.x, par ^= 1) {
         const long long state0 = b * S;
-        PROF_T(t0)
         double *P0 = sm + (sp.P0 + par * sp.p0size) * S;
         const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S;
         // ---- P1: reactions
@@ -1116,9 +1103,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
             else if (kind == 2) p1_group<LEVEL, S, true>(m, E, X, sc, etab, s, q, q + nq, out, state0, n);
             else reaction<LEVEL, S>(m, sp, E, X, sc, etab, s, q, out, state0, n);
         }
-        PROF_T(t1) PROF_ACC(tP1w, t0, t1)
         __syncthreads();
-        PROF_T(t1) PROF_ACC(tP1, t0, t1) PROF_T(t0)
         if (tid == 0) ctr[0] = 0;
         // ---- A: sums over the reactions per species / per column, pieces of the long cell lists
         {
@@ -1131,9 +1116,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
                 h = hn;
             }
         }
-        PROF_T(t1) PROF_ACC(tAw, t0, t1)
         __syncthreads();
-        PROF_T(t1) PROF_ACC(tA, t0, t1) PROF_T(t0)
         const int nvalid = (int)min((long long)S, n - state0);
         if (LEVEL == 2) {
             // ---- B: the Jacobian column by column, the energy row
@@ -1166,18 +1149,8 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
                     out.dydt[(state0 + q) * ld + r] = v;
                 }
         }
-        PROF_T(t1) PROF_ACC(tBw, t0, t1)
         __syncthreads();
-        PROF_T(t1) PROF_ACC(tB, t0, t1)
-#ifdef PYJAC_PROF
-        ++nb_;
-#endif
     }
-#ifdef PYJAC_PROF
-    if (blockIdx.x == 0 && lane == 0)
-        printf("warp %2d batches %d  P1 %lld (own %lld)  A %lld (own %lld)  B+P0 %lld (own %lld) cycles per batch\n", warp, nb_,
-               tP1 / nb_, tP1w / nb_, tA / nb_, tAw / nb_, tB / nb_, tBw / nb_);
-#endif
 }
 
 }  // namespace

@@ -22,4 +22,9 @@ cudaError_t launch_eval(int level, int threads, int S, const DeviceMech &m, cons
                         long long n, const double *T, const double *P, const double *Y, long long ldy,
                         const EvalOut &out, cudaStream_t stream);
 
+// adds to the count pyjac_kernel_launches() reports (kernels launched outside api.cu's `launch`)
+void count_launches(int k);
+// the device a handle's tables live on
+int mech_device(const pyjac_mech *m);
+
 }  // namespace pyjac

@@ -101,6 +101,7 @@ def _dydt_term_scale(o, ref, T, P, Y, part):
     return out[:, None]
 
 
+FD_OBSERVED = {}    # config -> largest forward-difference error over its bound (test_fd_jacobian_matches_oracle_fd)
 OBSERVED = {}       # label -> largest errors seen, printed at the end of the module (pytest -s) and written to gpurun_out/
 
 
@@ -184,7 +185,8 @@ def _report_observed():
     try:
         os.makedirs(out, exist_ok=True)
         with open(os.path.join(out, "parity_observed.json"), "w") as f:
-            json.dump(dict(jacobian=OBSERVED, rates=RATES_OBSERVED), f, indent=1, sort_keys=True)
+            json.dump(dict(jacobian=OBSERVED, rates=RATES_OBSERVED, fd_error_over_bound=FD_OBSERVED), f, indent=1,
+                      sort_keys=True)
     except OSError:
         pass
 
@@ -396,6 +398,10 @@ def test_host_buffer_variant_matches_device_variant(torch, PyJac):
     (1, 301, dict(cell_cap=1, list_cap=4)),                    # everything summed in the summing phase, short lane lists
     (1, 301, dict(states_per_cta=2, cell_cap=2, list_cap=30)),
     (1, 301, dict(rows_per_lane=1)),                                                # one row per lane, 8-byte stores
+    (1, 301, dict(p1_states=1)),                                      # one state per reaction work item
+    (1, 301, dict(states_per_cta=6, threads=512, ctas_per_sm=1, p1_states=2)),   # pairs of states, constants in registers
+    (1, 301, dict(states_per_cta=2, threads=512, ctas_per_sm=1, stage_tables=1)),  # gather tables staged in shared memory
+    (0, 1024, dict(stage_tables=1)),
     (0, 1024, dict(states_per_cta=1, threads=64)),
     (2, 65, dict(states_per_cta=2)),
 ])
@@ -409,6 +415,87 @@ def test_launch_shapes(torch, PyJac, cfg, n, shape):
     o = Oracle(m)
     check_jacobian(torch, pj, o, T, P, Y, label="launch_shapes")
     check_rates(torch, pj, o, T[:64], P[:64], Y[:64])
+
+
+# ---------------------------------------------------------------------------------- near-equilibrium states (f4)
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_equilibrium_and_trajectory_states(torch, PyJac, cfg):
+    """States the paper singles out: at chemical equilibrium of every K_c-reversible
+    reaction (element potentials, tests/trajectory.py: R_f = R_r to rounding, so q_i is a cancelled
+    difference), a step of 1e-8 and of 1e-3 off it, and -- for the two smaller mechanisms -- along a
+    linearly implicit Euler march of the source term from a seeded state.  Same tolerances as everywhere:
+    R_f, R_r, c_i element-wise, the production rates against the size of what was summed (C19), the
+    Jacobian per state, row, element and column."""
+    from trajectory import equilibrium_states, march_to_equilibrium
+    m = synth.make_mechanism(cfg)
+    o, pj = Oracle(m), PyJac(m)
+    temps = np.linspace(850.0, 2400.0, 12)
+    parts = [equilibrium_states(m, temps, p_target_atm=p, perturb=d, seed=7)
+             for p, d in ((1.0, 0.0), (20.0, 0.0), (5.0, 1e-8), (5.0, 1e-3))]
+    if cfg <= 1:
+        T0, P0, Y0 = synth.config_states(cfg, 2)
+        for k in range(2):
+            Tt, Pt, Yt, _ = march_to_equilibrium(m, T0[k], P0[k], Y0[k], n_steps=60, growth=2.0)
+            parts.append((Tt, Pt, Yt))
+    T = np.concatenate([p[0] for p in parts]); P = np.concatenate([p[1] for p in parts])
+    Y = np.concatenate([p[2] for p in parts])
+    ref = o.source(T[:24], P[:24], Y[:24])
+    rel = np.abs(ref["rf"] - ref["rr"]) / np.maximum(ref["rf"] + ref["rr"], 1e-300)
+    assert np.median(rel) < 1e-10 or cfg == 0          # the first 24 states really are at equilibrium
+    check_rates(torch, pj, o, T, P, Y, label="cfg%d_equilibrium" % cfg)
+    check_jacobian(torch, pj, o, T, P, Y, label="cfg%d_equilibrium" % cfg)
+
+
+# ---------------------------------------------------------------------------------- forward differences (f2)
+
+@pytest.mark.parametrize("cfg,n,chunk", [(0, 1024, 100), (1, 300, 64), (2, 40, 7), (3, 6, 4)])
+def test_fd_jacobian_matches_oracle_fd(torch, PyJac, cfg, n, chunk):
+    """pyjac_eval_jacobian_fd (the paper's comparison method; C21) against the
+    oracle's forward difference with the same increments.  Both subtract two source terms and divide by
+    D_j = sqrt(eps) max(|Phi_j|, rtol |Phi_j| + atol), so a disagreement of the source terms of t times
+    the size of the terms they sum (RATE_TOL, asserted in check_rates) becomes 2 t (term size) / D_j in
+    column j: that is the element-wise tolerance.  Column N_s is exactly zero; chunks smaller than the
+    batch (ragged last chunk) give bit-identical results to one chunk."""
+    m = synth.make_mechanism(cfg)
+    o, pj = Oracle(m), PyJac(m)
+    ns, ld = m.n_species, m.n_species + 1
+    T, P, Y = synth.config_states(cfg, n)
+    rtol, atol = 1e-8, 1e-12
+    dT, dP, dY = dev(torch, T, P, Y)
+    J = pj.eval_jacobian_fd(dT, dP, dY, rtol=rtol, atol=atol, chunk_states=chunk).cpu().numpy()
+    J1 = pj.eval_jacobian_fd(dT, dP, dY, rtol=rtol, atol=atol, chunk_states=n).cpu().numpy()
+    assert np.array_equal(J, J1)
+    Jr = o.jacobian_fd(T, P, Y, rtol=rtol, atol=atol)
+    A = J.reshape(n, ld, ld).transpose(0, 2, 1)
+    B = Jr.reshape(n, ld, ld).transpose(0, 2, 1)
+    assert np.all(A[:, :, ns] == 0.0)
+    ref = o.source(T, P, Y)
+    phi = np.concatenate([T[:, None], Y[:, :ns - 1]], axis=1)
+    inc = np.sqrt(EPS) * np.maximum(np.abs(phi), rtol * np.abs(phi) + atol)              # [n][ns]
+    term = np.empty((n, ld))
+    term[:, :1] = np.maximum(np.abs(ref["dydt"][:, :1]), _dydt_term_scale(o, ref, T, P, Y, slice(0, 1)))
+    term[:, 1:] = np.maximum(np.abs(ref["dydt"][:, 1:]).max(axis=1, keepdims=True),
+                             _dydt_term_scale(o, ref, T, P, Y, slice(1, None)))
+    bound = 2.0 * RATE_TOL * term[:, :, None] / inc[:, None, :]                          # [n][row][col]
+    err = np.abs(A[:, :, :ns] - B[:, :, :ns])
+    FD_OBSERVED["cfg%d" % cfg] = float((err / bound).max())
+    assert np.all(err <= bound), float((err / bound).max())
+
+
+def test_fd_jacobian_argument_errors(torch, PyJac):
+    m = synth.make_mechanism(0)
+    pj = PyJac(m)
+    T, P, Y = synth.config_states(0, 8)
+    dT, dP, dY = dev(torch, T, P, Y)
+    from paper_1605_03262_b200.binding import PyJacError
+    with pytest.raises(PyJacError):       # scratch for less than one state
+        pj.eval_jacobian_fd(dT, dP, dY, work=torch.empty(8, dtype=torch.float64, device="cuda"))
+    with pytest.raises(PyJacError):
+        pj.eval_jacobian_fd(dT, dP, dY, rtol=0.0)
+    assert pj.fd_workspace_doubles(0) == -1
+    l0 = pj.kernel_launches()
+    pj.eval_jacobian_fd(dT, dP, dY, chunk_states=4)
+    assert pj.kernel_launches() - l0 == 8             # two chunks of four launches
 
 
 @pytest.mark.gpu

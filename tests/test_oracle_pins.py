@@ -567,3 +567,63 @@ def test_oracle_regression_fixture():
             assert np.allclose(src["dydt"][s], dy, rtol=1e-12, atol=1e-12 * np.abs(dy).max())
             assert np.linalg.norm(J[s] - Js) <= 1e-12 * np.linalg.norm(Js)
         i += 1 + 2 * n
+
+
+# ---------------------------------------------------------------- forward-difference Jacobian (f2)
+def test_fd_jacobian_approximates_the_derivative(tiny_mechs):
+    """PAPER.md:817 (the paper's comparison method, Tables 4-5): the oracle's first-order forward
+    difference (reading C21) against the plain definition J = df/dPhi by complex step.  A
+    forward difference with increment D carries a truncation error D f''/2; here the measure is the
+    paper's own (Eq. 132) plus a per-element bound at the row scale, loose enough for a
+    first-order quotient (the paper reports FD errors that prevented its use as the reference,
+    PAPER.md:765-780) and far too tight for a wrong sign, index, transposition or a missed Eq. 2
+    compensation.  Column N_s is exactly zero; a mechanism without reactions gives exactly zero."""
+    for m in tiny_mechs:
+        o = Oracle(m)
+        ns = m.n_species
+        T, P, Y = synth.make_states(ns, 16, 33, t_range=(700.0, 2500.0), p_range_atm=(0.5, 20.0))
+        Jf = as_matrix(o.jacobian_fd(T, P, Y, rtol=1e-8, atol=1e-12), ns)
+        Jc = as_matrix(o.jacobian_complex_step(T, P, Y), ns)
+        for s in range(len(T)):
+            assert np.all(Jf[s][:, -1] == 0.0)
+            assert np.linalg.norm(Jf[s] - Jc[s]) <= 2e-2 * np.linalg.norm(Jc[s])
+            rowmax = np.abs(Jc[s]).max(axis=1, keepdims=True)
+            assert np.all(np.abs(Jf[s] - Jc[s]) <= 0.2 * rowmax + 1e-300)
+    # the Eq. 2 compensation: the mass-fraction columns differentiate along Y_j - Y_Ns.  Without it the
+    # quotient would be the unconstrained partial derivative, which differs at first order
+    m = tiny_mechs[0]
+    o = Oracle(m)
+    ns = m.n_species
+    T, P, Y = synth.make_states(ns, 4, 34)
+    Jf = as_matrix(o.jacobian_fd(T, P, Y, rtol=1e-8, atol=1e-12), ns)
+    for s in range(len(T)):
+        f0 = o.source(T[s:s + 1], P[s:s + 1], Y[s:s + 1])["dydt"][0]
+        j = int(np.argmax(Y[s, :-1]))
+        d = np.sqrt(2.220446049250313e-16) * Y[s, j]
+        Yp = Y[s].copy(); Yp[j] += d                       # no compensation
+        g = (o.source(T[s:s + 1], P[s:s + 1], Yp[None])["dydt"][0] - f0) / d
+        assert np.linalg.norm(g - Jf[s][:, j + 1]) > 1e-3 * np.linalg.norm(Jf[s][:, j + 1])
+    # no reactions: f = 0 identically
+    b = MechanismBuilder(["A", "B"], ["X"], np.array([[1], [1]], dtype=np.int32), np.array([10.0, 20.0]),
+                         np.tile(np.array([3.5, 0, 0, 0, 0, 0, 0.0]), (2, 1)), np.tile(np.array([3.5, 0, 0, 0, 0, 0, 0.0]), (2, 1)),
+                         np.array([1000.0, 1000.0]))
+    m0 = b.build()
+    J0 = Oracle(m0).jacobian_fd(np.array([1200.0]), np.array([101325.0]), np.array([[0.3, 0.7]]))
+    assert np.all(J0 == 0.0)
+
+
+def test_element_potential_composition_is_at_equilibrium():
+    """Eqs. 18-19, 23-27 together, by a construction the oracle does not use: for ANY element potentials
+    lambda the concentrations ln[X_k] = B_k + ln(p_atm/R) + sum_e lambda_e a_ke put every element-balanced
+    reaction with k_r = k_f / K_c at equilibrium, R_f = R_r (tests/trajectory.py builds such states from the
+    species B_k alone).  A wrong sign in B_k, a wrong power of p_atm/R in K_c (Eq. 26) or a wrong
+    stoichiometric exponent in R_f / R_r breaks it for every reaction with sum nu != 0."""
+    from trajectory import equilibrium_states
+    m = synth.make_mechanism(1)
+    o = Oracle(m)
+    T, P, Y = equilibrium_states(m, [900.0, 1400.0, 2300.0], p_target_atm=3.0)
+    src = o.source(T, P, Y)
+    rev = np.asarray(m.rev_type) == REV_FROM_KC
+    rf, rr = src["rf"][:, rev], src["rr"][:, rev]
+    assert rev.sum() > 200
+    assert np.all(np.abs(rf - rr) <= 1e-11 * (rf + rr))
