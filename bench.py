@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
                     [--also 2,3] [--sweep short|full|off] [--no-cpu-baseline] [--no-e2e] [--peaks]
-    python bench.py --ncu-target CFG:KERNEL:N      # the short command the ncu captures of profiles/ wrap
+    python bench.py --ncu-target CFG:KERNEL:N[:SHAPE]      # the short command the ncu captures of profiles/ wrap
     python bench.py --ncu-import REPORT --ncu-label WORKLOAD:KERNEL:N    # one row of profiles/r2_ncu_counters.csv
 
 A "step" is one pass of the whole hot path (thermo -> rates -> source term -> Jacobian -> store;
@@ -293,7 +293,7 @@ def run_peaks():
 
 
 def run_ncu_target(spec: str):
-    """CFG:KERNEL:N -- three launches (two warm-up) of one kernel on the first N states of a configuration and
+    """CFG:KERNEL:N[:SHAPE] -- three launches (two warm-up) of one kernel on the first N states of a configuration and
     nothing else: what `ncu --set full -s 2 -c 1` wraps for the captures under profiles/."""
     import torch
     from paper_1605_03262_b200 import build, synth
@@ -301,16 +301,19 @@ def run_ncu_target(spec: str):
     build.build()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    cfg, kernel, n = spec.split(":")
-    cfg, n = int(cfg), int(n)
+    parts = spec.split(":")
+    cfg, kernel, n = int(parts[0]), parts[1], int(parts[2])
+    # optional fourth field: an explicit launch shape, e.g. states_per_cta=1,threads=128 (pyjac_launch_shape)
+    shape = dict((k, int(v)) for k, v in (kv.split("=") for kv in parts[3].split(","))) if len(parts) > 3 else None
     m = synth.make_mechanism(cfg)
     T, P, Y = synth.config_states(cfg, min(n, synth.CONFIGS[cfg].n_states))
     n = len(T)
-    pj = PyJac(m, device=0)
+    pj = PyJac(m, device=0, shape=shape)
     dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
     ld = m.n_species + 1
-    out = torch.empty((n, ld * ld if kernel == "jacobian" else ld), dtype=torch.float64, device="cuda")
+    out = torch.empty((n, ld * ld if kernel in ("jacobian", "jacobian_fd") else ld), dtype=torch.float64, device="cuda")
     fn = {"jacobian": lambda: pj.eval_jacobian(dT, dP, dY, out=out),
+          "jacobian_fd": lambda: pj.eval_jacobian_fd(dT, dP, dY, out=out, chunk_states=256),
           "dydt": lambda: pj.eval_dydt(dT, dP, dY, out=out),
           "rates": lambda: pj.eval_rates(dT, dP, dY, want=("wdot",))}[kernel]
     total, per = time_gpu(pj, torch, dT, dP, dY, out, 1, 2, fn=fn)

@@ -128,6 +128,7 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
     dm.eWdot = hp.eWdot; dm.eG0 = hp.eG0;
     dm.eS1 = hp.eS1; dm.eA0 = hp.eA0; dm.eS4 = hp.eS4; dm.eZero = hp.eZero; dm.eDump = hp.eDump; dm.eHs = hp.eHs;
     dm.n_e = hp.n_e;
+    dm.n_aent = (int)(hp.a_ent.size() / 4); dm.n_bent = (int)(hp.b_ent.size() / 4); dm.n_achunk = (int)(hp.achunk.size() / 2);
     Uploader up;
     try {
         up.add(&dm.inv_mw, hp.inv_mw); up.add(&dm.mw, hp.mw);

@@ -133,6 +133,7 @@ struct DeviceMech {
     int eDump;                  // a slot nobody reads (stores of empty reaction slots)
     int eHs;                    // partial sums of the long Jacobian-cell lists
     int n_e;                    // size of E
+    int n_aent, n_bent, n_achunk;   // sizes of a_ent, b_ent (16-byte units) and achunk (8-byte units): the checked build
 };
 
 // per-state scalars (region Scal of the shared-memory plan)

@@ -26,6 +26,16 @@
 #include "device_mech.h"
 #include "kernels.h"
 
+// -DPYJAC_CHECKED builds the kernels with a bounds check on every table-driven shared-memory access and
+// every gather-table read (the shipped build relies on the self-check of mech_pack.cu instead); a violation
+// traps, which the next synchronisation reports as a launch failure.  Used by tests/test_gpu_parity.py's
+// checked-build run (profiles/r2_checked_build.md): compute-sanitizer is closed on the measurement pool.
+#ifdef PYJAC_CHECKED
+#define PYJAC_CHECK(cond) do { if (!(cond)) __trap(); } while (0)
+#else
+#define PYJAC_CHECK(cond) do { } while (0)
+#endif
+
 namespace pyjac {
 
 namespace {
@@ -238,6 +248,9 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
         n_eff = m.eff_base[grp + 1] - m.eff_base[grp];
     }
     const int eq = (m.eQ + 3 * s) * S, eh = (m.eH + s) * S;
+    PYJAC_CHECK(x0 <= m.ns * S && x1 <= m.ns * S && x2 <= m.ns * S && x3 <= m.ns * S && x4 <= m.ns * S && x5 <= m.ns * S);
+    PYJAC_CHECK(v0 < m.n_e * S && v1 < m.n_e * S && v2 < m.n_e * S && v3 < m.n_e * S && v4 < m.n_e * S && v5 < m.n_e * S);
+    PYJAC_CHECK(eq + 3 * S <= m.n_e * S && eh + S <= m.n_e * S && q0 >= 0 && q1 <= S);
 
     // NQ states at a time (independent chains: the fp64 pipe sees several of them)
     auto body = [&](auto nq_c, const int q) {
@@ -305,6 +318,7 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
                 for (int k = 0; k < 4; ++k) {
                     const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
                     const int xo = (w[k].x & 0xFFFF) * S + q;
+                    PYJAC_CHECK((int)(w[k].x & 0xFFFF) <= m.ns);
 #pragma unroll
                     for (int u = 0; u < NQ; ++u) Xi[u] = fma(eps, X[xo + u], Xi[u]);
                 }
@@ -375,6 +389,7 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
                     for (int k = 0; k < 4; ++k) {
                         const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
                         const int eo = (w[k].x >> 16) * S + q;
+                        PYJAC_CHECK((int)(w[k].x >> 16) < m.n_e);
 #pragma unroll
                         for (int u = 0; u < NQ; ++u) E[eo + u] = bb[u] * eps;
                     }
@@ -733,6 +748,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
     const uint32_t kind = (ch.y >> 8) & 0xF;
     const int steps = (int)(ch.y & 0xFF), rshift = (int)(ch.y >> 12) & 0xF, width = 1 << rshift;
     const uint4 *ep = a_ent + ch.x + lane;
+    PYJAC_CHECK((int)ch.x + 32 * (2 + ((int)((ch.y >> 8) & 0xF) == (int)kAll3 ? 0 : ((int)(ch.y & 0xFF) + 3) / 4)) <= m.n_aent);
     const uint4 r0 = ep[0];
     const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
     const char *Eb = reinterpret_cast<const char *>(E);
@@ -767,6 +783,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
             auto step = [&](uint32_t w) {
                 const double cf = entry_coef(w);
                 double a[S];
+                PYJAC_CHECK((w & kEntOffMask) + 8u * S <= 8u * S * (uint32_t)m.n_e);
                 ldv<S>(reinterpret_cast<const double *>(Eb + (w & kEntOffMask)), a);
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] = fma(cf, a[q], acc[q]);
@@ -775,6 +792,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
             for (int o = 1; o < width; o <<= 1)
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
+            PYJAC_CHECK(!head || (int)r0.x < m.n_e);
             if (head) {
                 const double cst = __hiloint2double((int)r0.z, (int)r0.y);
 #pragma unroll
@@ -789,6 +807,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
             for (int q = 0; q < S; ++q) acc[q] = 0.0;
             auto step = [&](uint32_t w) {
                 double a[S], b[S];
+                PYJAC_CHECK((int)(w & 0xFFFF) < m.n_e && (int)(w >> 16) < m.n_e);
                 ldv<S>(reinterpret_cast<const double *>(Eb + (w & 0xFFFF) * (S * 8)), a);
                 ldv<S>(reinterpret_cast<const double *>(Eb + (w >> 16) * (S * 8)), b);
 #pragma unroll
@@ -798,6 +817,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
             for (int o = 1; o < width; o <<= 1)
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[q] += __shfl_xor_sync(0xFFFFFFFFu, acc[q], o);
+            PYJAC_CHECK(!head || (int)r0.x < m.n_e);
             if (head) stv<S>(E + r0.x * S, acc);
         }
     } else {
@@ -811,6 +831,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
         if (kind == kSum3) {
             auto step = [&](uint32_t w_) {
                 const double cf = entry_coef(w_);
+                PYJAC_CHECK((w_ & kEntOffMask) + 8u * S * NA <= 8u * S * (uint32_t)m.n_e);
                 const double *src = reinterpret_cast<const double *>(Eb + (w_ & kEntOffMask));
 #pragma unroll
                 for (int w = 0; w < NA; ++w) {
@@ -847,6 +868,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
             }
         } else if (head) {
             const uint32_t k = r0.x;
+            PYJAC_CHECK((int)k < m.ns);
             stv<S>(E + (m.eWdot + k) * S, acc[0]);
             if (LEVEL == 2) {
                 // alpha'_{k+1} of Eq. 112 regrouped and the T column (Eq. 111), both without W_k
@@ -954,6 +976,7 @@ __device__ __forceinline__ void b_run(const DeviceMech &m, const uint4 *b_ent, c
 #pragma unroll
         for (int hh = 0; hh < RP; ++hh) wr[hh] = wrow[rr + hh];
         const uint4 *ep = ebase + (size_t)it * (32 * RP);
+        PYJAC_CHECK(it >= 0 && c1 <= ld && (it + (c1 - c0) + 1) * (32 * RP) <= m.n_bent && slab >= 0 && slab < m.n_slab);
         const double *cc = colc + 4 * c0;
         uint32_t off = (uint32_t)(c0 * ld + r);                  // element (r, c) of the batch's first state
         uint4 wA = ep[0], wB = wA;
@@ -971,6 +994,7 @@ __device__ __forceinline__ void b_run(const DeviceMech &m, const uint4 *b_ent, c
             auto step = [&](uint32_t w, int hh) {
                 const double cf = entry_coef(w);
                 double a[S];
+                PYJAC_CHECK((w & kEntOffMask) + 8u * S <= 8u * S * (uint32_t)m.n_e);
                 ldv<S>(reinterpret_cast<const double *>(Eb + (w & kEntOffMask)), a);
 #pragma unroll
                 for (int q = 0; q < S; ++q) acc[hh * S + q] = fma(cf, a[q], acc[hh * S + q]);
@@ -1096,6 +1120,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
                 continue;
             }
             // item = {group of 32 reactions, path, first state}: most expensive first (device_mech.h `p1item`)
+            PYJAC_CHECK(it - S < m.n_p1item);
             const uint32_t w = m.p1item[it - S];
             const int c = (int)(w & 0xFFFF), kind = (int)(w >> 16) & 0xF, q = (int)(w >> 20) & 0xF, nq = (int)(w >> 24);
             const int s = min(c * 32 + lane, nr - 1);
@@ -1111,6 +1136,7 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
             uint2 h = *hp;
             for (int row = 0; row < arows; ++row) {
                 hp += NW;
+                PYJAC_CHECK((row + 1) * NW + warp < m.n_achunk);
                 const uint2 hn = *hp;                 // the header table is padded by one row
                 a_chunk<LEVEL, S>(m, a_ent, E, sc, h, lane);
                 h = hn;
