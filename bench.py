@@ -64,7 +64,8 @@ def ncu_counters():
                 continue
             out.setdefault(row["workload"], {})[row["kernel"]] = {
                 "dram_bytes_per_state": float(row["dram_bytes_per_state"]),
-                "fp64_flop_per_state": float(row["fp64_flop_per_state"])}
+                "fp64_flop_per_state": float(row["fp64_flop_per_state"]),
+                "lsu_wavefronts_per_state": float(row["lsu_wavefronts_per_state"])}
             src = "profiles/r2_ncu_counters.csv (%s)" % row["source"]
     except Exception:
         return {}, None
@@ -401,6 +402,7 @@ def main():
     ap.add_argument("--peaks", action="store_true",
                     help="measure the write-only store stream and the fp64 FMA rate (SURVEY.md 8(d)) and exit")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-fd", action="store_true", help="skip the finite-difference / analytical time ratio")
     ap.add_argument("--ncu-target", default=None, help="CFG:KERNEL:N (KERNEL = jacobian | dydt | rates): three launches, for ncu")
     ap.add_argument("--ncu-import", default=None, help="an .ncu-rep to turn into a row of profiles/r2_ncu_counters.csv")
     ap.add_argument("--ncu-label", default=None, help="WORKLOAD:KERNEL:N of the imported report")
@@ -473,6 +475,18 @@ def main():
         return {"bound": "alu", "achieved": tf, "peak": fp64_peak(), "unit": "TFLOP/s", "frac": tf / fp64_peak(),
                 "flop_per_state": c["fp64_flop_per_state"], "peak_source": "bench.py --peaks (profiles/r1_machine_peaks.md)"}
 
+    def lsu_of(name, kernel, states, ms, sm_mhz):
+        """the pipe that binds the Jacobian kernel: L1TEX LSU data-pipe wavefronts (shared
+        and global accesses; one per SM and clock at best), counted by ncu per state, over this launch's time"""
+        c = counters.get(name, {}).get(kernel)
+        if not c or not sm_mhz:
+            return None
+        rate = c["lsu_wavefronts_per_state"] * states / (ms * 1e-3) / 1e9
+        peak = 148 * sm_mhz * 1e6 / 1e9
+        return {"bound": "lsu", "achieved": rate, "peak": peak, "unit": "Gwavefront/s", "frac": rate / peak,
+                "wavefronts_per_state": c["lsu_wavefronts_per_state"],
+                "peak_source": "one L1TEX data-pipe wavefront per SM and clock, 148 SMs at the SM clock sampled during the run"}
+
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic_of(c.name, r["per_launch"]), "traffic_source": counters_src,
                 "peak_source": peak_src,
@@ -481,7 +495,8 @@ def main():
                 "algorithmic_bytes_note": "(Ns+2) doubles read + (Ns+1)^2 doubles written per state, the placeholder "
                                           "row and the zero column of the (Ns+1)^2 layout included",
                 "launch_ms": launch_ms, "launch_config": pj.launch_config(r["per_launch"]),
-                "fp64": fp64_of(c.name, "jacobian", r["per_launch"], launch_ms)}
+                "fp64": fp64_of(c.name, "jacobian", r["per_launch"], launch_ms),
+                "lsu": lsu_of(c.name, "jacobian", r["per_launch"], launch_ms, clocks.get("sm_mhz"))}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -530,7 +545,8 @@ def main():
                             "roofline": {"bound": "hbm", "achieved": ab / (lm * 1e-3) / 1e9, "peak": peak,
                                          "unit": "GB/s", "frac": ab / (lm * 1e-3) / 1e9 / peak,
                                          "traffic": traffic_of(cc.name, rr["per_launch"]),
-                                         "fp64": fp64_of(cc.name, "jacobian", rr["per_launch"], lm)},
+                                         "fp64": fp64_of(cc.name, "jacobian", rr["per_launch"], lm),
+                                         "lsu": lsu_of(cc.name, "jacobian", rr["per_launch"], lm, clocks.get("sm_mhz"))},
                             "launch_config": rr["pj"].launch_config(rr["per_launch"])}
             del rr
             torch.cuda.empty_cache()
@@ -538,12 +554,42 @@ def main():
             line["per_config"] = per
         if args.sweep != "off":
             line["sweep_53sp"] = sweep(torch, args, fp64_of)
+        if not args.no_fd:
+            line["fd_vs_analytical"] = fd_ratio(torch)
         if not args.no_cpu_baseline:
             line["cpu_baseline"], _ = time_oracle(cfg, CPU_SAMPLE[cfg], steps=3, warmup=1, single_thread=True)
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def fd_ratio(torch):
+    """The paper's own comparison (Table 5): the first-order forward-difference
+    Jacobian built on the source-term kernel (pyjac_eval_jacobian_fd, 1 + N_sp source-term evaluations per
+    state) against the analytical one, same states, CUDA events, per mechanism.  The paper's GPU ratios
+    (Tesla C2075, one thread per state) are 1.37 - 2.73; context, not a target."""
+    from paper_1605_03262_b200 import synth
+    from paper_1605_03262_b200.binding import PyJac
+    out = {}
+    for cfg, n in ((0, 1024), (1, 8192), (2, 4096), (3, 512)):
+        m = synth.make_mechanism(cfg)
+        T, P, Y = synth.config_states(cfg, n)
+        pj = PyJac(m, device=torch.cuda.current_device())
+        ld = m.n_species + 1
+        dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
+        jac = torch.empty((n, ld * ld), dtype=torch.float64, device="cuda")
+        chunk = max(1, min(n, (1 << 28) // pj.fd_workspace_doubles(1)))           # 2 GiB of scratch at most
+        work = torch.empty(pj.fd_workspace_doubles(chunk), dtype=torch.float64, device="cuda")
+        ta, _ = time_gpu(pj, torch, dT, dP, dY, jac, 5, 3)
+        tf, _ = time_gpu(pj, torch, dT, dP, dY, jac, 3, 3,
+                         fn=lambda: pj.eval_jacobian_fd(dT, dP, dY, out=jac, work=work))
+        out[synth.CONFIGS[cfg].name] = {"n_states": n, "analytical_ms": ta / 5, "fd_ms": tf / 3,
+                                        "fd_over_analytical": (tf / 3) / (ta / 5)}
+        del jac, work
+        torch.cuda.empty_cache()
+    out["paper_gpu_ratio_range"] = [1.37, 2.73]
+    return out
 
 
 def sweep(torch, args, fp64_of):

@@ -180,6 +180,18 @@ int pyjac_eval_dydt(const pyjac_mech *mech, int64_t n, const double *T, const do
 int pyjac_eval_jacobian(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
                         const double *Y, int64_t ldy, double *jac, void *stream);
 
+/* Jacobian-vector product without the matrix: jv[n][N_sp+1] = J v per state, J the matrix of
+ * pyjac_eval_jacobian (rows 0..N_sp, the placeholder row included) and v[n][ldv] one vector per state
+ * with entries 0..N_sp (entry N_sp multiplies the zero column and is not read); ldv >= N_sp+1.  This is
+ * what a matrix-free implicit integrator consumes (the paper's motivation): the
+ * (N_sp+1)^2 doubles per state never go to memory.  The column sum is taken per reaction first,
+ *   (J v)_{k+1} = W_k sum_i nu_ki tau_i,  tau_i = sum_j s'_ij v_j / W_j + (U a_i + v_0 Theta_i) / rho,
+ * with the per-reaction products of Section 4.1, so the cost is
+ * that of the source term, O(N_reac), not O(N_sp^2).  Device pointers, asynchronous on `stream`. */
+int pyjac_eval_jvp(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
+                   const double *Y, int64_t ldy, const double *v, int64_t ldv, double *jv,
+                   void *stream);
+
 /* Host-buffer variants: T, P, Y and the output are HOST pointers (pinned memory makes the copies
  * asynchronous; pageable memory works but serialises them).  The call copies the inputs to the
  * device, runs the same kernels as above in chunks of at most `chunk_states` states (<= 0: a

@@ -47,7 +47,7 @@ class LaunchShape(C.Structure):
 
 EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_sizes",
            "pyjac_eval_rates", "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
-           "pyjac_eval_dydt_host", "pyjac_eval_jacobian_fd", "pyjac_fd_workspace_doubles", "pyjac_kernel_launches",
+           "pyjac_eval_dydt_host", "pyjac_eval_jvp", "pyjac_eval_jacobian_fd", "pyjac_fd_workspace_doubles", "pyjac_kernel_launches",
            "pyjac_jacobian_launch_config", "pyjac_strerror")
 TOOLS_EXPORTS = ("pyjac_tools_pack_stats", "pyjac_tools_peak_store_stream", "pyjac_tools_peak_dfma")
 
@@ -75,6 +75,7 @@ def load_library(path: str | None = None):
     lib.pyjac_eval_jacobian.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp]
     lib.pyjac_eval_jacobian_host.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64]
     lib.pyjac_eval_dydt_host.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64]
+    lib.pyjac_eval_jvp.argtypes = [vp, i64, vp, vp, vp, i64, vp, i64, vp, vp]
     lib.pyjac_eval_jacobian_fd.argtypes = [vp, i64, vp, vp, vp, i64, C.c_double, C.c_double, vp, vp, i64, vp]
     lib.pyjac_fd_workspace_doubles.argtypes = [vp, i64]
     lib.pyjac_fd_workspace_doubles.restype = i64
@@ -285,6 +286,21 @@ class PyJac:
         out = self._dev_out(out, n, ld * ld, T)
         _check(self.lib.pyjac_eval_jacobian(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
                                             out.data_ptr(), self._stream()), "pyjac_eval_jacobian")
+        return out
+
+    def eval_jvp(self, T, P, Y, v, out=None):
+        """[n][Nsp+1] Jacobian-vector products J v, one vector v[n][>= Nsp+1] per state (pyjac_eval_jvp): the
+        matrix is never formed."""
+        import torch
+        n, ldy = self._dev_inputs(T, P, Y)
+        ld = self.ns + 1
+        if (not isinstance(v, torch.Tensor) or not v.is_cuda or v.dtype != torch.float64 or v.dim() != 2
+                or v.shape[0] != n or v.shape[1] < ld or v.stride(1) != 1 or v.device != T.device):
+            raise ValueError("v must be a float64 CUDA tensor [n][>= Nsp+1] with unit inner stride on the inputs' device")
+        out = self._dev_out(out, n, ld, T)
+        ldv = v.stride(0) if n > 1 else max(v.shape[1], ld)
+        _check(self.lib.pyjac_eval_jvp(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy, v.data_ptr(),
+                                       int(ldv), out.data_ptr(), self._stream()), "pyjac_eval_jvp")
         return out
 
     def fd_workspace_doubles(self, chunk_states: int) -> int:

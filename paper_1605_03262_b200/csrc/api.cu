@@ -22,8 +22,8 @@ struct pyjac_mech {
     SmemPlan plan{};
     int threads = 128;
     int S = 1;                  // states per CTA iteration
-    size_t smem[3] = {0, 0, 0}; // dynamic shared memory per level
-    int ctas_per_sm[3] = {1, 1, 1};
+    size_t smem[4] = {0, 0, 0, 0}; // dynamic shared memory per level
+    int ctas_per_sm[4] = {1, 1, 1, 1};
     int n_sm = 1;
     // staging of the *_host calls: two device buffer pairs and two streams, kept between calls.  The handle
     // is otherwise immutable; this part is guarded by `ws_busy` (a caller that finds it taken stages with
@@ -170,7 +170,7 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
             // stays L1 (the gather tables are re-read from L1 / L2 by every CTA iteration)
             int carveout = (int)((100 * ((long long)hp.ctas_target * (long long)(bytes + 1024 + 16)) + 228 * 1024 - 1) / (228 * 1024));
             carveout = carveout > 100 ? 100 : carveout < 0 ? 0 : carveout;
-            for (int level = 0; level < 3 && rc == PYJAC_OK; ++level) {
+            for (int level = 0; level < 4 && rc == PYJAC_OK; ++level) {
                 m->smem[level] = bytes;
                 const void *k = eval_kernel_ptr(level, m->S, hp.stage);
                 // the kernel function is shared by every handle of this shape: its dynamic shared-memory limit
@@ -228,7 +228,7 @@ int pyjac_eval_rates(const pyjac_mech *m, int64_t n, const double *T, const doub
 {
     int rc = check_eval_args(m, n, T, P, Y, ldy);
     if (rc != PYJAC_OK) return rc;
-    EvalOut out{rf, rr, cmod, wdot, nullptr, nullptr};
+    EvalOut out{rf, rr, cmod, wdot, nullptr, nullptr, nullptr, 0, nullptr};
     return launch(m, 0, n, T, P, Y, ldy, out, stream);
 }
 
@@ -238,7 +238,7 @@ int pyjac_eval_dydt(const pyjac_mech *m, int64_t n, const double *T, const doubl
     int rc = check_eval_args(m, n, T, P, Y, ldy);
     if (rc != PYJAC_OK) return rc;
     if (n > 0 && !dydt) return PYJAC_EINVAL;
-    EvalOut out{nullptr, nullptr, nullptr, nullptr, dydt, nullptr};
+    EvalOut out{nullptr, nullptr, nullptr, nullptr, dydt, nullptr, nullptr, 0, nullptr};
     return launch(m, 1, n, T, P, Y, ldy, out, stream);
 }
 
@@ -248,8 +248,18 @@ int pyjac_eval_jacobian(const pyjac_mech *m, int64_t n, const double *T, const d
     int rc = check_eval_args(m, n, T, P, Y, ldy);
     if (rc != PYJAC_OK) return rc;
     if (n > 0 && !jac) return PYJAC_EINVAL;
-    EvalOut out{nullptr, nullptr, nullptr, nullptr, nullptr, jac};
+    EvalOut out{nullptr, nullptr, nullptr, nullptr, nullptr, jac, nullptr, 0, nullptr};
     return launch(m, 2, n, T, P, Y, ldy, out, stream);
+}
+
+int pyjac_eval_jvp(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                   int64_t ldy, const double *v, int64_t ldv, double *jv, void *stream)
+{
+    int rc = check_eval_args(m, n, T, P, Y, ldy);
+    if (rc != PYJAC_OK) return rc;
+    if (n > 0 && (!v || !jv || ldv < m->ns + 1)) return PYJAC_EINVAL;
+    EvalOut out{nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, v, (long long)ldv, jv};
+    return launch(m, 3, n, T, P, Y, ldy, out, stream);
 }
 
 int64_t pyjac_kernel_launches(void) { return g_launches.load(std::memory_order_relaxed); }
@@ -351,7 +361,8 @@ int eval_host(const pyjac_mech *m, int level, int64_t n, const double *T, const 
             e = cudaMemcpy2DAsync(dY, (size_t)ns * sizeof(double), Y + s0 * ldy, (size_t)ldy * sizeof(double),
                                   (size_t)ns * sizeof(double), c, cudaMemcpyHostToDevice, st[b]);
         if (e != cudaSuccess) { rc = PYJAC_ECUDA; break; }
-        EvalOut out{nullptr, nullptr, nullptr, nullptr, level == 1 ? dout[b] : nullptr, level == 2 ? dout[b] : nullptr};
+        EvalOut out{nullptr, nullptr, nullptr, nullptr, level == 1 ? dout[b] : nullptr, level == 2 ? dout[b] : nullptr,
+                    nullptr, 0, nullptr};
         rc = launch(m, level, (int64_t)c, dT, dP, dY, ns, out, st[b]);
         if (rc != PYJAC_OK) break;
         e = cudaMemcpyAsync(outp + (size_t)s0 * out_per, dout[b], c * out_per * sizeof(double),

@@ -138,7 +138,10 @@ struct DeviceMech {
 
 // per-state scalars (region Scal of the shared-memory plan)
 enum {
-    kT = 0, kLnT, kInvT, kP, kLnP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kIcp, kNScal = 12
+    kT = 0, kLnT, kInvT, kP, kLnP, kRho, kIrho, kW, kM, kCpMix, kDcpDT, kIcp,
+    // Jacobian-vector product (level 3): v_0, U / rho and v_0 / rho with U = sum_j d_j v_j, and
+    // C_v = sum_j (c_pj - c_pNs) v_j (the vector's entries for T and the species, Eq. 1)
+    kV0, kUrho, kV0rho, kCv, kNScal = 16
 };
 
 // Shared-memory plan (offsets in doubles PER STATE).  The S states of a CTA iteration are interleaved:
@@ -151,6 +154,7 @@ struct SmemPlan {
     int p0size;
     int oX;                             // within a mixture part: [ns+1] concentrations; slot ns = 1 (empty reaction slots)
     int oCp;                            // [ns] c_pk (mass based)
+    int oVw;                            // [ns+1] level 3: v_j / W_j per species (the last one: -sum_j v_j / W_Ns; slot ns = 0)
     int oScal;                          // [kNScal]
     int total;                          // doubles per state
     int colc;                           // [ld][4], offset in doubles from the end of the state part
@@ -173,6 +177,7 @@ inline SmemPlan make_smem_plan(int ns, int n_e, int n_achunk16 = 0, int n_aent16
         const int base = o;
         p.oX = take(ns + 1) - base;
         p.oCp = take(ns) - base;
+        p.oVw = take(ns + 1) - base;
         p.oScal = take(kNScal) - base;
         p.p0size = o - base;
         o += p.p0size;

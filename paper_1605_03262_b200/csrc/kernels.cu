@@ -198,10 +198,11 @@ __device__ __forceinline__ void special_rate(const DeviceMech &m, int s, int typ
 // replace ln k_f and L, pressure-dependent lanes (third body, falloff, chemically activated) scale the
 // products of the common part by c_i and add the derivative terms of c_i (Eqs. 77-100).
 template <int LEVEL, int S, bool GEN>
-__device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const double *X, const double *sc,
+__device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const double *X, const double *Vw, const double *sc,
                                          const double *etab, int s, int q0, int q1, const EvalOut &out,
                                          long long state0, long long n)
 {
+    constexpr bool DER = LEVEL >= 2;       // the derivative terms: Jacobian (2) and Jacobian-vector product (3)
     const int nr = m.nr;
     const uint4 sl = m.slots[s];
     const uint32_t meta = sl.w;
@@ -290,7 +291,7 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
             const double R = Rf[u] - Rr[u];
             vq0[u] = R; vq1[u] = 0.0; vq2[u] = 0.0; W[u] = 0.0; cm[u] = 1.0;
             vh[u] = kRu * T[u] * fma(T[u], sdB[u], dnu);
-            if (LEVEL == 2) {
+            if (DER) {
                 W[u] = sc[kW * S + q + u];
                 const double iT = invT[u];
                 // Theta_dT,i (Eq. 115) with Eqs. 66, 75; the d_j coefficient of Eq. 119 plus W q_i
@@ -303,6 +304,9 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
                 vs[3][u] = nkr * (c4 * c5); vs[4][u] = nkr * (c3 * c5); vs[5][u] = nkr * p34;           // Eq. 121
             }
         }
+        double sig[NQ];                   // level 3: the efficiency part of sigma_i = sum_j s'_ij v_j / W_j
+#pragma unroll
+        for (int u = 0; u < NQ; ++u) sig[u] = 0.0;
         if (GEN) {
             // ---- pressure modification c_i (Eq. 20) and its derivatives (Eqs. 77-100): q_i = c R,
             // Theta = dc/dT R + c Theta0, a = c a0 + b (rho - W [X]_i), s'_ij = c s0_ij, and b (alpha_ij - 1)
@@ -371,7 +375,7 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
                     dcdT[u] = G * lPrT + cc * fT;
                 }
             }
-            if (LEVEL == 2) {
+            if (DER) {
 #pragma unroll
                 for (int u = 0; u < NQ; ++u) {
                     const double mixW = mixM ? sc[kRho * S + q + u] - W[u] * Xi[u] : -W[u] * Xi[u];
@@ -384,14 +388,21 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
                 for (int e = 0; e < n_eff; e += 128) {
                     uint4 w[4];
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
+                    for (int k = 0; k < 4; ++k)
+                        w[k] = e + 32 * k < n_eff ? ef[e + 32 * k] : make_uint4((uint32_t)m.ns | (uint32_t)m.eDump << 16, 0u, 0u, 0u);
 #pragma unroll
                     for (int k = 0; k < 4; ++k) {
                         const double eps = __hiloint2double((int)w[k].w, (int)w[k].z);
-                        const int eo = (w[k].x >> 16) * S + q;
-                        PYJAC_CHECK((int)(w[k].x >> 16) < m.n_e);
+                        if (LEVEL == 2) {
+                            const int eo = (w[k].x >> 16) * S + q;
+                            PYJAC_CHECK((int)(w[k].x >> 16) < m.n_e);
 #pragma unroll
-                        for (int u = 0; u < NQ; ++u) E[eo + u] = bb[u] * eps;
+                            for (int u = 0; u < NQ; ++u) E[eo + u] = bb[u] * eps;
+                        } else {        // level 3: b (alpha_ij - 1) v_j / W_j into sigma_i
+                            const int xo = (w[k].x & 0xFFFF) * S + q;
+#pragma unroll
+                            for (int u = 0; u < NQ; ++u) sig[u] = fma(bb[u] * eps, Vw[xo + u], sig[u]);
+                        }
                     }
                 }
             }
@@ -411,6 +422,16 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
             }
             E[eq + q + u] = vq0[u];
             if (LEVEL >= 1) E[eh + q + u] = vh[u];
+            if (LEVEL == 3) {
+                // tau_i = sum_j s'_ij v_j / W_j + (U / rho) a_i + (v_0 / rho) Theta_i: the one per-reaction
+                // scalar of the Jacobian-vector product, (J v)_{k+1} = W_k sum_i nu_ki tau_i
+                double t = sig[u];
+                t = fma(vs[0][u], Vw[x0 + q + u], t); t = fma(vs[1][u], Vw[x1 + q + u], t); t = fma(vs[2][u], Vw[x2 + q + u], t);
+                t = fma(vs[3][u], Vw[x3 + q + u], t); t = fma(vs[4][u], Vw[x4 + q + u], t); t = fma(vs[5][u], Vw[x5 + q + u], t);
+                t = fma(sc[kUrho * S + q + u], vq1[u], t);
+                t = fma(sc[kV0rho * S + q + u], vq2[u], t);
+                E[eq + S + q + u] = t;
+            }
             if (LEVEL == 2) {
                 E[eq + S + q + u] = vq1[u];
                 E[eq + 2 * S + q + u] = vq2[u];
@@ -429,7 +450,7 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
 
 // ---- P1, general path: one reaction of any type, one state (q) ----------------------------------------
 template <int LEVEL, int S>
-__device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *E, const double *X,
+__device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp, double *E, const double *X, const double *Vw,
                                          const double *sc, const double *etab, int s, int q, const EvalOut &out,
                                          long long state0, long long n)
 {
@@ -659,30 +680,46 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
                 if (out.cmod) out.cmod[o] = c;
             }
         }
-        if (LEVEL == 2) {
+        if (LEVEL >= 2) {
             // Theta_dT,i of Eqs. 115-117: dc/dT R + c (dR/dT + R/T)
             const double dcdT = pdep ? G * lPrT + c * fT : 0.0;
             const double dRfdT = Rf * (L - (double)snu_f * invT);                 // Eq. 66
             const double dRrdT = Rr * (Lr - (double)snu_r * invT);                // Eqs. 69, 75
-            E[(m.eQ + 3 * s + 2) * S + q] = dcdT * R + c * (dRfdT - dRrdT + R * invT);
+            const double theta = dcdT * R + c * (dRfdT - dRrdT + R * invT);
             // coefficient of d_j (Eqs. 119, 123, 127 regrouped), plus W q_i: the omega_k W d_j term of
             // Eq. 112 summed per reaction
             const double W = sc[kW * S + q];
             const double base = -W * (Rf * (double)snu_f - Rr * (double)snu_r);
             const double mix = (pdep && !meta_single(meta)) ? sc[kRho * S + q] : 0.0;
-            E[(m.eQ + 3 * s + 1) * S + q] = c * base + b * (mix - W * Xi) + W * qi;
+            const double ai = c * base + b * (mix - W * Xi) + W * qi;
             // sparse terms s'_ij = c (k_f S'_j - k_r S''_j) per slot, b (alpha_ij - 1) per efficiency
             const double ckf = c * kf, ckr = -c * kr;
-            E[v0 + q] = ckf * sk0; E[v1 + q] = ckf * sk1; E[v2 + q] = ckf * sk2;
-            E[v3 + q] = ckr * sk3; E[v4 + q] = ckr * sk4; E[v5 + q] = ckr * sk5;
+            if (LEVEL == 2) {
+                E[(m.eQ + 3 * s + 2) * S + q] = theta;
+                E[(m.eQ + 3 * s + 1) * S + q] = ai;
+                E[v0 + q] = ckf * sk0; E[v1 + q] = ckf * sk1; E[v2 + q] = ckf * sk2;
+                E[v3 + q] = ckr * sk3; E[v4 + q] = ckr * sk4; E[v5 + q] = ckr * sk5;
+            }
+            // level 3: tau_i = sum_j s'_ij v_j / W_j + (U / rho) a_i + (v_0 / rho) Theta_i (see p1_group)
+            double tau = fma(sc[kUrho * S + q], ai, sc[kV0rho * S + q] * theta);
+            if (LEVEL == 3) {
+                tau = fma(ckf * sk0, Vw[x0 + q], tau); tau = fma(ckf * sk1, Vw[x1 + q], tau); tau = fma(ckf * sk2, Vw[x2 + q], tau);
+                tau = fma(ckr * sk3, Vw[x3 + q], tau); tau = fma(ckr * sk4, Vw[x4 + q], tau); tau = fma(ckr * sk5, Vw[x5 + q], tau);
+            }
             if (pdep)
                 for (int e = 0; e < n_eff; e += 256) {
                     uint4 w[8];
 #pragma unroll
-                    for (int u = 0; u < 8; ++u) w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.eDump << 16, 0u, 0u, 0u);
+                    for (int u = 0; u < 8; ++u)
+                        w[u] = e + 32 * u < n_eff ? ef[e + 32 * u] : make_uint4((uint32_t)m.ns | (uint32_t)m.eDump << 16, 0u, 0u, 0u);
 #pragma unroll
-                    for (int u = 0; u < 8; ++u) E[(w[u].x >> 16) * S + q] = b * __hiloint2double((int)w[u].w, (int)w[u].z);
+                    for (int u = 0; u < 8; ++u) {
+                        const double be = b * __hiloint2double((int)w[u].w, (int)w[u].z);
+                        if (LEVEL == 2) E[(w[u].x >> 16) * S + q] = be;
+                        else tau = fma(be, Vw[(w[u].x & 0xFFFF) * S + q], tau);
+                    }
                 }
+            if (LEVEL == 3) E[(m.eQ + 3 * s + 1) * S + q] = tau;
         }
     }
 }
@@ -700,10 +737,10 @@ __device__ __forceinline__ int grab(int *ctr, int lane)
 
 // ---- P0: mixture (Eqs. 3-5) and species (Eqs. 5, 9, 12-13, 54-55) of one state, by one warp ----------
 template <int LEVEL, int S>
-__device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double *X, double *Cp, double *sc, int q,
+__device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double *X, double *Cp, double *Vw, double *sc, int q,
                                                     long long st, const double *__restrict__ Tg,
                                                     const double *__restrict__ Pg, const double *__restrict__ Yg,
-                                                    long long ldy, int lane)
+                                                    long long ldy, int lane, const double *__restrict__ vg, long long ldv)
 {
     const int ns = m.ns;
     const double *Ys = Yg + st * ldy;
@@ -722,10 +759,35 @@ __device__ __forceinline__ void mixture_and_species(const DeviceMech &m, double 
             const double cpk = kRu * (a0 + T * (a1 + T * (a2 + T * (a3 + a4 * T)))) * iw;
             Cp[k * S + q] = cpk;
             cp += y * cpk;
-            if (LEVEL == 2) dcp += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
+            if (LEVEL >= 2) dcp += y * (kRu * iw * (a1 + T * (2.0 * a2 + T * (3.0 * a3 + 4.0 * a4 * T))));
         }
     }
     if (LEVEL >= 1) { cp = warp_sum(cp); dcp = warp_sum(dcp); }
+    if (LEVEL == 3) {
+        // the vector of the Jacobian-vector product: v_0 (T), v_{j+1} (Y_j), the last species' entry unused
+        // (Eq. 2).  Vw_j = v_{j+1} / W_j; the last species takes -sum_j v_{j+1} / W_Ns, which folds the
+        // gamma_r term of Eq. 112 into the per-reaction sums
+        const double *vs = vg + st * ldv;
+        const double iwl = m.inv_mw[ns - 1];
+        double U = 0.0, Vs = 0.0, Cv = 0.0;
+        __syncwarp();
+        for (int k = lane; k < ns - 1; k += 32) {
+            const double vk = vs[k + 1], iw = m.inv_mw[k];
+            Vw[k * S + q] = vk * iw;
+            U = fma(iw - iwl, vk, U);
+            Vs += vk;
+            Cv = fma(Cp[k * S + q], vk, Cv);
+        }
+        U = warp_sum(U); Vs = warp_sum(Vs); Cv = warp_sum(Cv);
+        __syncwarp();
+        if (lane == 0) {
+            const double rho_ = rho, v0 = vs[0];
+            Vw[(ns - 1) * S + q] = -Vs * iwl;
+            Vw[ns * S + q] = 0.0;
+            sc[kV0 * S + q] = v0; sc[kUrho * S + q] = U / rho_; sc[kV0rho * S + q] = v0 / rho_;
+            sc[kCv * S + q] = Cv - Cp[(ns - 1) * S + q] * Vs;
+        }
+    }
     if (lane == 0) {
         sc[kT * S + q] = T; sc[kLnT * S + q] = log(T); sc[kInvT * S + q] = 1.0 / T; sc[kP * S + q] = P; sc[kLnP * S + q] = log(P);
         sc[kM * S + q] = M; sc[kW * S + q] = W; sc[kRho * S + q] = rho; sc[kIrho * S + q] = 1.0 / rho;
@@ -822,7 +884,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
         }
     } else {
         // kSum3 / kAll3: three sums at once (one for the rates / source-term kernels)
-        constexpr int NA = LEVEL == 2 ? 3 : 1;
+        constexpr int NA = LEVEL == 2 ? 3 : LEVEL == 3 ? 2 : 1;        // level 3: q_i and tau_i
         double acc[NA][S];
 #pragma unroll
         for (int w = 0; w < NA; ++w)
@@ -865,11 +927,13 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
             if (lane == 0) {
                 stv<S>(E + m.eS1 * S, acc[0]);
                 if (LEVEL == 2) { stv<S>(E + m.eA0 * S, acc[iA]); stv<S>(E + m.eS4 * S, acc[iT]); }
+                if (LEVEL == 3) stv<S>(E + m.eA0 * S, acc[iA]);          // sum_i H_i tau_i
             }
         } else if (head) {
             const uint32_t k = r0.x;
             PYJAC_CHECK((int)k < m.ns);
             stv<S>(E + (m.eWdot + k) * S, acc[0]);
+            if (LEVEL == 3) stv<S>(E + (m.eAlpha + k + 1) * S, acc[iA]);    // sum_i nu_ki tau_i = (J v)_{k+1} / W_k
             if (LEVEL == 2) {
                 // alpha'_{k+1} of Eq. 112 regrouped and the T column (Eq. 111), both without W_k
                 double ir[S], al[S], tc[S];
@@ -1091,21 +1155,21 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
     if (tid == 0) ctr[0] = 0;
     const long long nbatch = (n + S - 1) / S;
     const int n_p1 = m.n_p1item;
-    const int arows = LEVEL == 2 ? m.n_arow : m.n_arow01;
+    const int arows = LEVEL == 2 ? m.n_arow : m.n_arow01;      // levels 0, 1, 3: the per-species sums only
     const int it0 = m.bsplit[warp], it1 = m.bsplit[warp + 1];
     const int nfix = 1 + (ns + 31) / 32;
     const bool aligned16 = (reinterpret_cast<uintptr_t>(out.jac) & 15) == 0;
     int par = 0;
     if ((long long)blockIdx.x < nbatch && warp < S) {
         double *P0 = sm + sp.P0 * S;
-        mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oScal * S, warp,
-                                      min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane);
+        mixture_and_species<LEVEL, S>(m, P0 + sp.oX * S, P0 + sp.oCp * S, P0 + sp.oVw * S, P0 + sp.oScal * S, warp,
+                                      min((long long)blockIdx.x * S + warp, n - 1), Tg, Pg, Yg, ldy, lane, out.v, out.ldv);
     }
     __syncthreads();
     for (long long b = blockIdx.x; b < nbatch; b += gridDim.x, par ^= 1) {
         const long long state0 = b * S;
         double *P0 = sm + (sp.P0 + par * sp.p0size) * S;
-        const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S;
+        const double *X = P0 + sp.oX * S, *sc = P0 + sp.oScal * S, *Vw = P0 + sp.oVw * S;
         // ---- P1: reactions
         // the queue starts with the mixtures of the NEXT batch (into the other mixture part, which nobody reads
         // during this iteration): their input reads from HBM overlap the reactions
@@ -1114,8 +1178,8 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
             if (it < S) {
                 if (more) {
                     double *Pn = sm + (sp.P0 + (par ^ 1) * sp.p0size) * S;
-                    mixture_and_species<LEVEL, S>(m, Pn + sp.oX * S, Pn + sp.oCp * S, Pn + sp.oScal * S, it,
-                                                  min((b + gridDim.x) * S + it, n - 1), Tg, Pg, Yg, ldy, lane);
+                    mixture_and_species<LEVEL, S>(m, Pn + sp.oX * S, Pn + sp.oCp * S, Pn + sp.oVw * S, Pn + sp.oScal * S, it,
+                                                  min((b + gridDim.x) * S + it, n - 1), Tg, Pg, Yg, ldy, lane, out.v, out.ldv);
                 }
                 continue;
             }
@@ -1124,9 +1188,9 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
             const uint32_t w = m.p1item[it - S];
             const int c = (int)(w & 0xFFFF), kind = (int)(w >> 16) & 0xF, q = (int)(w >> 20) & 0xF, nq = (int)(w >> 24);
             const int s = min(c * 32 + lane, nr - 1);
-            if (kind == 1) p1_group<LEVEL, S, false>(m, E, X, sc, etab, s, q, q + nq, out, state0, n);
-            else if (kind == 2) p1_group<LEVEL, S, true>(m, E, X, sc, etab, s, q, q + nq, out, state0, n);
-            else reaction<LEVEL, S>(m, sp, E, X, sc, etab, s, q, out, state0, n);
+            if (kind == 1) p1_group<LEVEL, S, false>(m, E, X, Vw, sc, etab, s, q, q + nq, out, state0, n);
+            else if (kind == 2) p1_group<LEVEL, S, true>(m, E, X, Vw, sc, etab, s, q, q + nq, out, state0, n);
+            else reaction<LEVEL, S>(m, sp, E, X, Vw, sc, etab, s, q, out, state0, n);
         }
         __syncthreads();
         if (tid == 0) ctr[0] = 0;
@@ -1175,6 +1239,39 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
                     out.dydt[(state0 + q) * ld + r] = v;
                 }
         }
+        if (LEVEL == 3) {
+            // ---- Jacobian-vector product without the matrix: (J v)_{k+1} = W_k sum_i nu_ki tau_i (Eq. 112
+            // times v, summed over the columns per reaction first); the energy row (Eq. 113) the same way
+            for (int r = 1 + tid; r < ld; r += NT)
+#pragma unroll
+                for (int q = 0; q < S; ++q)
+                    if (q < nvalid) out.jv[(state0 + q) * ld + r] = wrow[r] * E[(m.eAlpha + r) * S + q];
+            if (warp == NW - 1) {
+                const double *Cp = P0 + sp.oCp * S;
+                double s3[S];       // sum_k c_pk W_k wdot_k
+#pragma unroll
+                for (int q = 0; q < S; ++q) s3[q] = 0.0;
+                for (int k = lane; k < ns; k += 32) {
+                    const double wk = wrow[k + 1];
+#pragma unroll
+                    for (int q = 0; q < S; ++q) s3[q] = fma(Cp[k * S + q] * wk, E[(m.eWdot + k) * S + q], s3[q]);
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+                    for (int q = 0; q < S; ++q) s3[q] += __shfl_xor_sync(0xFFFFFFFFu, s3[q], o);
+                if (lane < S && lane < nvalid) {
+                    const int q = lane;
+                    double sq = s3[0];
+#pragma unroll
+                    for (int u = 1; u < S; ++u) sq = q == u ? s3[u] : sq;
+                    const double icp = sc[kIcp * S + q], irho = sc[kIrho * S + q], S1 = E[m.eS1 * S + q];
+                    out.jv[(state0 + q) * ld] = -icp * E[m.eA0 * S + q]
+                                                - icp * irho * (sq - sc[kDcpDT * S + q] * icp * S1) * sc[kV0 * S + q]
+                                                + irho * S1 * icp * icp * sc[kCv * S + q];
+                }
+            }
+        }
         __syncthreads();
     }
 }
@@ -1194,10 +1291,12 @@ const void *PYJAC_NAME(eval_kernel_ptr_, PYJAC_S)(int level, bool stage)
     if (stage)
         return level == 0 ? (const void *)eval_kernel<0, PYJAC_S, true>
              : level == 1 ? (const void *)eval_kernel<1, PYJAC_S, true>
-                          : (const void *)eval_kernel<2, PYJAC_S, true>;
+             : level == 2 ? (const void *)eval_kernel<2, PYJAC_S, true>
+                          : (const void *)eval_kernel<3, PYJAC_S, true>;
     return level == 0 ? (const void *)eval_kernel<0, PYJAC_S, false>
          : level == 1 ? (const void *)eval_kernel<1, PYJAC_S, false>
-                      : (const void *)eval_kernel<2, PYJAC_S, false>;
+         : level == 2 ? (const void *)eval_kernel<2, PYJAC_S, false>
+                      : (const void *)eval_kernel<3, PYJAC_S, false>;
 }
 
 cudaError_t PYJAC_NAME(launch_eval_, PYJAC_S)(int level, int threads, const DeviceMech &m, const SmemPlan &sp, int grid,
@@ -1208,11 +1307,13 @@ cudaError_t PYJAC_NAME(launch_eval_, PYJAC_S)(int level, int threads, const Devi
     if (sp.staged) {
         if (level == 0) PYJAC_LAUNCH(0, true);
         else if (level == 1) PYJAC_LAUNCH(1, true);
-        else PYJAC_LAUNCH(2, true);
+        else if (level == 2) PYJAC_LAUNCH(2, true);
+        else PYJAC_LAUNCH(3, true);
     } else {
         if (level == 0) PYJAC_LAUNCH(0, false);
         else if (level == 1) PYJAC_LAUNCH(1, false);
-        else PYJAC_LAUNCH(2, false);
+        else if (level == 2) PYJAC_LAUNCH(2, false);
+        else PYJAC_LAUNCH(3, false);
     }
 #undef PYJAC_LAUNCH
     return cudaGetLastError();

@@ -12,9 +12,12 @@ struct EvalOut {
     double *rf, *rr, *cmod, *wdot;   // level 0
     double *dydt;                    // level 1
     double *jac;                     // level 2
+    const double *v;                 // level 3: the vectors [n][ldv] (N_sp + 1 entries used per state)
+    long long ldv;
+    double *jv;                      // level 3: [n][N_sp + 1]
 };
 
-// level: 0 rates, 1 source term, 2 Jacobian.  S: states a CTA interleaves per iteration (1, 2, 3, 4, 6);
+// level: 0 rates, 1 source term, 2 Jacobian, 3 Jacobian-vector product.  S: states a CTA interleaves per iteration (1, 2, 3, 4, 6);
 // threads: a multiple of 32, at least 32 S, up to kMaxThreads.
 const void *eval_kernel_ptr(int level, int S, bool stage);
 size_t eval_smem_bytes(const SmemPlan &sp, int S);

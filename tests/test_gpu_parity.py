@@ -101,6 +101,7 @@ def _dydt_term_scale(o, ref, T, P, Y, part):
     return out[:, None]
 
 
+JVP_OBSERVED = {}   # config -> largest error of (J v)_r over max_c |J_rc| sum_c |v_c|
 FD_OBSERVED = {}    # config -> largest forward-difference error over its bound (test_fd_jacobian_matches_oracle_fd)
 OBSERVED = {}       # label -> largest errors seen, printed at the end of the module (pytest -s) and written to gpurun_out/
 
@@ -170,7 +171,7 @@ def check_jacobian(torch, pj, o, T, P, Y, tol=JAC_TOL, label=None):
 @pytest.fixture(scope="module", autouse=True)
 def _report_observed():
     yield
-    if not OBSERVED and not RATES_OBSERVED:
+    if not OBSERVED and not RATES_OBSERVED and not JVP_OBSERVED and not FD_OBSERVED:
         return
     import json
     import os
@@ -185,7 +186,8 @@ def _report_observed():
     try:
         os.makedirs(out, exist_ok=True)
         with open(os.path.join(out, "parity_observed.json"), "w") as f:
-            json.dump(dict(jacobian=OBSERVED, rates=RATES_OBSERVED, fd_error_over_bound=FD_OBSERVED), f, indent=1,
+            json.dump(dict(jacobian=OBSERVED, rates=RATES_OBSERVED, fd_error_over_bound=FD_OBSERVED,
+                           jvp_error_over_scale=JVP_OBSERVED), f, indent=1,
                       sort_keys=True)
     except OSError:
         pass
@@ -444,6 +446,65 @@ def test_equilibrium_and_trajectory_states(torch, PyJac, cfg):
     assert np.median(rel) < 1e-10 or cfg == 0          # the first 24 states really are at equilibrium
     check_rates(torch, pj, o, T, P, Y, label="cfg%d_equilibrium" % cfg)
     check_jacobian(torch, pj, o, T, P, Y, label="cfg%d_equilibrium" % cfg)
+
+
+# ---------------------------------------------------------------------------------- Jacobian-vector product (f1)
+
+@pytest.mark.parametrize("cfg,n", [(0, 1024), (1, 700), (2, 200), (3, 20)])
+def test_jvp_matches_oracle_jacobian_times_vector(torch, PyJac, cfg, n):
+    """pyjac_eval_jvp (the Jacobian consumed on chip) against the plain
+    definition: the oracle's analytical Jacobian (Eqs. 44-113) times the vector, in numpy.  An element J_rc is
+    a rounded sum of terms of the size of its row's largest entry (the alpha_r d_c part of Eq. 112 is in every
+    column: see `jacobian_errors`), and the product sums those terms per reaction before it sums over the
+    columns, so entry r of J v is judged at max_c |J_rc| * sum_c |v_c|: tolerance JAC_TOL of it, observed
+    maxima recorded.  Vectors: seeded normal entries scaled to the state (T-sized first entry, mass-fraction
+    sized others), a unit vector per state (one column of J), and padded ldv."""
+    m = synth.make_mechanism(cfg)
+    o, pj = Oracle(m), PyJac(m)
+    ns, ld = m.n_species, m.n_species + 1
+    T, P, Y = synth.config_states(cfg, n)
+    rng = np.random.default_rng(77 + cfg)
+    v = np.zeros((n, ld + 3))
+    v[:, 0] = T * 1e-3 * rng.standard_normal(n)
+    v[:, 1:ld] = Y * rng.standard_normal((n, ns))
+    v[:, ld:] = 1e300                                   # padding of ldv: never read
+    unit = np.zeros((n, ld)); unit[np.arange(n), rng.integers(0, ns, n)] = 1.0
+    Jr = o.jacobian(T, P, Y).reshape(n, ld, ld).transpose(0, 2, 1)        # [n][row][col]
+    dT, dP, dY = dev(torch, T, P, Y)
+    worst = 0.0
+    for vec in (v, unit):
+        dv = torch.from_numpy(vec).cuda()
+        got = pj.eval_jvp(dT, dP, dY, dv).cpu().numpy()
+        ref = np.einsum("nrc,nc->nr", Jr, vec[:, :ld])
+        scale = np.abs(Jr).max(axis=2) * np.abs(vec[:, :ns]).sum(axis=1, keepdims=True)
+        err = np.abs(got - ref)
+        worst = max(worst, float((err / np.maximum(scale, 1e-300))[scale > 0].max(initial=0.0)))
+        assert np.all(err <= JAC_TOL * scale + 1e-300), worst
+        assert np.all(got[scale == 0.0] == 0.0)
+    JVP_OBSERVED["cfg%d" % cfg] = worst
+
+
+def test_jvp_tiny_mechanisms_and_arguments(torch, PyJac, tiny_mechs):
+    """Every reaction type (one-state general path included), a single state, n = 0, and the argument checks."""
+    from paper_1605_03262_b200.binding import PyJacError
+    for m in tiny_mechs:
+        o, pj = Oracle(m), PyJac(m)
+        ns, ld = m.n_species, m.n_species + 1
+        T, P, Y = synth.make_states(ns, 130, 9, t_range=(500.0, 2800.0), p_range_atm=(0.05, 80.0))
+        rng = np.random.default_rng(3)
+        v = np.concatenate([(T * rng.standard_normal(len(T)))[:, None], rng.standard_normal((len(T), ns))], axis=1)
+        Jr = o.jacobian(T, P, Y).reshape(len(T), ld, ld).transpose(0, 2, 1)
+        dT, dP, dY = dev(torch, T, P, Y)
+        got = pj.eval_jvp(dT, dP, dY, torch.from_numpy(v).cuda()).cpu().numpy()
+        ref = np.einsum("nrc,nc->nr", Jr, v)
+        scale = np.abs(Jr).max(axis=2) * np.abs(v[:, :ns]).sum(axis=1, keepdims=True)
+        assert np.all(np.abs(got - ref) <= JAC_TOL * scale + 1e-300)
+        one = pj.eval_jvp(dT[:1], dP[:1], dY[:1], torch.from_numpy(v[:1]).cuda()).cpu().numpy()
+        assert np.array_equal(one[0], got[0])
+        assert pj.eval_jvp(dT[:0], dP[:0], dY[:0], torch.from_numpy(v[:0]).cuda()).shape == (0, ld)
+        with pytest.raises(ValueError):
+            pj.eval_jvp(dT, dP, dY, torch.from_numpy(v[:, :ns]).cuda())       # vector too short
+    assert isinstance(PyJacError(-1, "x"), Exception)
 
 
 # ---------------------------------------------------------------------------------- forward differences (f2)
