@@ -344,9 +344,10 @@ def run_ncu_import(report: str, label: str):
     def g(k):
         v = float(d[k].replace(",", ""))
         u = units.get(k, "")
-        return v * {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "msecond": 1e3, "second": 1e6}.get(u, 1.0)
+        return v * {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(u, 1.0)
 
-    dur_us = g("gpu__time_duration.sum") * (1e-3 if units.get("gpu__time_duration.sum") == "nsecond" else 1.0)
+    dur_us = g("gpu__time_duration.sum") * {"ns": 1e-3, "nsecond": 1e-3, "us": 1.0, "usecond": 1.0, "ms": 1e3, "msecond": 1e3,
+                                            "s": 1e6, "second": 1e6}[units["gpu__time_duration.sum"]]
     cyc = g("smsp__cycles_elapsed.max") if "smsp__cycles_elapsed.max" in d else g("sm__cycles_elapsed.max")
     ops = {k: g("smsp__sass_thread_inst_executed_op_%s_pred_on.sum.per_cycle_elapsed" % k) * cyc for k in ("dfma", "dmul", "dadd")}
     # all LSU data-pipe wavefronts (shared + global + local): the shared count scaled by the ratio of the two
@@ -556,6 +557,7 @@ def main():
             line["sweep_53sp"] = sweep(torch, args, fp64_of)
         if not args.no_fd:
             line["fd_vs_analytical"] = fd_ratio(torch)
+            line["jvp_on_chip"] = jvp_rates(torch)
         if not args.no_cpu_baseline:
             line["cpu_baseline"], _ = time_oracle(cfg, CPU_SAMPLE[cfg], steps=3, warmup=1, single_thread=True)
     if rank == 0:
@@ -589,6 +591,28 @@ def fd_ratio(torch):
         del jac, work
         torch.cuda.empty_cache()
     out["paper_gpu_ratio_range"] = [1.37, 2.73]
+    return out
+
+
+def jvp_rates(torch):
+    """the Jacobian consumed on chip.  pyjac_eval_jvp evaluates J v per state without
+    forming J (the (N_sp+1)^2 store that sets the HBM roof disappears); states/s per mechanism, next to the
+    time the full Jacobian takes for the same states."""
+    import numpy as np
+    from paper_1605_03262_b200 import synth
+    from paper_1605_03262_b200.binding import PyJac
+    out = {}
+    for cfg, n in ((1, 100_000), (2, 50_000), (3, 8192)):
+        m = synth.make_mechanism(cfg)
+        T, P, Y = synth.config_states(cfg, n)
+        pj = PyJac(m, device=torch.cuda.current_device())
+        ld = m.n_species + 1
+        dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
+        v = torch.from_numpy(np.random.default_rng(1).standard_normal((n, ld))).cuda()      # host-made: no library kernel
+        jv = torch.empty((n, ld), dtype=torch.float64, device="cuda")
+        t, _ = time_gpu(pj, torch, dT, dP, dY, None, 10, 3, fn=lambda: pj.eval_jvp(dT, dP, dY, v, out=jv))
+        out[synth.CONFIGS[cfg].name] = {"n_states": n, "jvp_ms": t / 10, "jvp_states_per_s": n / (t / 10 * 1e-3),
+                                        "bytes_per_state": (2 * ld + m.n_species + 2) * 8}
     return out
 
 
