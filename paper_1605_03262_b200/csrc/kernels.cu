@@ -1,25 +1,26 @@
 // kernels.cu -- sm_100a kernels for the batched source term and analytical Jacobian.
 //
-// One CTA evaluates NP blocks of S thermochemical states per iteration of a persistent grid-stride loop.
-// The S states of a block are interleaved in shared memory (element i of a region for state q at
-// (R + i) * S + q), so whatever does not depend on the state -- decoding a reaction, a gather entry, a
-// column constant -- is done once per lane and applied to the S states of each of the NP blocks with
-// vector loads.  Per iteration, separated by CTA barriers:
-//   P0  mixture (Eqs. 3-5) and species, warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT
-//       (Eqs. 9-13, 54-55); computed one iteration ahead, at the end of phase B
-//   P1  reactions, lane <-> reaction, groups of 32 from one dynamic queue: k_f, k_r (K_c from the
-//       per-reaction polynomial of device_mech.h `th_data`), R_f, R_r, c_i and the reusable per-reaction
-//       products of Section 4.1 into E: q_i, Theta_dT,i, a_i (the coefficient of d_j),
-//       the sparse terms s'_ij, the enthalpy H_i.  Two states at a time; the common part of every rate
-//       form is branch-free, pressure-dependent lanes add the c_i tail.
+// One CTA evaluates S thermochemical states per iteration of a persistent grid-stride loop.  The S states
+// are interleaved in shared memory (element i of a region for state q at (R + i) * S + q), so whatever does
+// not depend on the state -- decoding a reaction, a gather entry, a column constant -- is done once per lane
+// and applied to the S states.  Per iteration, separated by CTA barriers:
+//   P1  one dynamic queue.  Its first S items are the mixtures of the NEXT batch (Eqs. 3-5, 9-13, 54-55;
+//       warp <-> state: [X_k], c_pk, mixture c_p, d c_p / dT; for the Jacobian-vector product also the
+//       vector), written into the other of two mixture parts.  The others are groups of 32 reactions,
+//       lane <-> reaction: k_f, k_r (K_c from the per-reaction polynomial of device_mech.h `th_data`), R_f,
+//       R_r, c_i and the reusable per-reaction products of Section 4.1 into E: q_i,
+//       Theta_dT,i, a_i (the coefficient of d_j), the sparse terms s'_ij, the enthalpy H_i.  The reaction's
+//       constants are read once per item and stay in registers over its states; the common part of every
+//       rate form is branch-free, pressure-dependent lanes add the c_i tail.
 //   A   fixed-order gathers over E, lane <-> sum (or a share of one): wdot_k (Eq. 14), alpha'_r, gamma'_r
 //       of Eq. 112, the T column (Eq. 111), the column sums of the energy row (Eq. 113), and the long
 //       Jacobian-cell lists piece by piece
-//   B   the Jacobian, column by column, lane <-> two rows: every cell gathers its (at most four) entries
+//   B   the Jacobian, column by column, lane <-> two rows: every cell gathers its (at most three) entries
 //       on top of alpha'_r u_c - gamma'_r v_c, which is Eq. 112 with the per-reaction terms of Eqs.
 //       118-127 regrouped by what they multiply, and is stored at once: a warp
-//       stores 512 contiguous bytes per state and column, nothing is staged.  FIX items of the same phase
-//       finish and store the energy row (Eq. 113).
+//       stores up to 512 contiguous bytes per state and column, nothing is staged.  FIX items of the same
+//       phase finish and store the energy row (Eq. 113).  The rates, source-term and Jacobian-vector-product
+//       kernels (LEVEL 0, 1, 3) write their outputs here instead: they need the per-species sums only.
 // There are no atomics on data: every sum has an order fixed at pyjac_mech_create.
 #include <cuda_runtime.h>
 
