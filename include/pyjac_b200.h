@@ -143,6 +143,8 @@ typedef struct pyjac_launch_shape {
                                constants held in registers (0: all states_per_cta) */
     int32_t stage_tables;   /* 1: copy the gather tables to shared memory once per CTA (PYJAC_ELIMIT if they
                                do not fit this shape); 0: read them through L1 / L2 */
+    int32_t layout;         /* 2: keep the per-reaction terms in allocation order in shared memory; 0 / 1: place
+                               them so that the gathers meet few bank conflicts (same numbers either way) */
 } pyjac_launch_shape;
 
 /* As pyjac_mech_create with an explicit launch shape (tuning and tests; `shape` may be NULL).

@@ -29,7 +29,7 @@ extern "C" {
  *  16..19 summing-phase steps by kind (three sums at once, one sum, products, all reactions)
  *  20, 21 shared-memory wavefronts beyond the minimum that the entry placement leaves, per CTA
  *         iteration (summing phase, streaming phase; the bank model of mech_pack.cu)
- *  22, 23 reserved (0)
+ *  22, 23 bank-group excess of the gather groups before / after the layout search of the per-reaction terms
  * Errors as pyjac_mech_create_shaped (PYJAC_EINVAL, PYJAC_ELIMIT, PYJAC_ENOMEM). */
 int pyjac_tools_pack_stats(const pyjac_mech_desc *host_desc, const pyjac_launch_shape *shape,
                            int64_t *stats);

@@ -42,7 +42,7 @@ class LaunchShape(C.Structure):
     """struct pyjac_launch_shape (0 = let the library choose)"""
     _fields_ = [("states_per_cta", C.c_int32), ("threads", C.c_int32), ("ctas_per_sm", C.c_int32),
                 ("list_cap", C.c_int32), ("cell_cap", C.c_int32), ("rows_per_lane", C.c_int32),
-                ("p1_states", C.c_int32), ("stage_tables", C.c_int32)]
+                ("p1_states", C.c_int32), ("stage_tables", C.c_int32), ("layout", C.c_int32)]
 
 
 EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_sizes",
@@ -161,7 +161,7 @@ PACK_STAT_NAMES = ("e_elements", "cell_entries", "b_steps", "a_steps", "cells", 
                    "smem_bytes_per_cta", "reaction_groups", "states_per_cta", "threads", "reserved10",
                    "ctas_per_sm_target", "heavy_cells", "heavy_pieces", "a_table_bytes", "b_table_bytes",
                    "a_steps_sum3", "a_steps_sum1", "a_steps_prod", "a_steps_all3", "a_conflict_wf", "b_conflict_wf",
-                   "reserved22", "reserved23")
+                   "layout_excess_before", "layout_excess_after")
 
 
 def pack_stats(mech: Mechanism, shape=None) -> dict:

@@ -277,16 +277,22 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     std::vector<std::array<uint32_t, 6>> vslot(nr);
     std::vector<std::vector<uint32_t>> veff(nr);
     uint32_t nv = 0;
+    // v_run[v] = (group, position, lane) of the store instruction that writes V entry v (the layout
+    // optimisation below permutes indices among the lanes of one shared-memory wavefront of such a store)
+    std::vector<std::array<int, 3>> v_run;
     for (int c = 0; c < o.n_rchunk; ++c) {
         const int s0 = 32 * c, s1 = std::min(nr, 32 * c + 32);
         for (int p = 0; p < 6; ++p)
-            for (int s = s0; s < s1; ++s) vslot[s][p] = sl[s].nu[p] ? nv++ : 0xFFFFFFFFu;
+            for (int s = s0; s < s1; ++s) {
+                vslot[s][p] = sl[s].nu[p] ? nv++ : 0xFFFFFFFFu;
+                if (sl[s].nu[p]) v_run.push_back({c, p, s - s0});
+            }
         int maxeff = 0;
         for (int s = s0; s < s1; ++s) maxeff = std::max(maxeff, n_eff_terms(d, order[s]));
         for (int s = s0; s < s1; ++s) veff[s].clear();
         for (int e = 0; e < maxeff; ++e)
             for (int s = s0; s < s1; ++s)
-                if (n_eff_terms(d, order[s]) > e) veff[s].push_back(nv++);
+                if (n_eff_terms(d, order[s]) > e) { veff[s].push_back(nv++); v_run.push_back({c, 6 + e, s - s0}); }
     }
     int next_slot = (int)nv;
     auto take = [&](int n) { int r = next_slot; next_slot += n; return r; };
@@ -682,6 +688,79 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             }
             return cost;
         };
+        // single-stream lists: an exact start.  Within one wavefront group (LP lanes) the entries are the edges of
+        // a bipartite multigraph lanes x bank groups; `steps` colours (= steps) colour it without two edges of
+        // one colour at a vertex iff no bank group is read more often than `steps` times (Koenig) -- then every
+        // step reads LP different bank groups.  Alternating-path edge colouring; an edge whose bank group is
+        // over capacity takes a step that is free at its lane and stays a conflict for the search below.
+        if (nstream == 1) {
+            for (int q = 0; q < nq; ++q) {
+                std::vector<std::array<int, 3>> edges;                 // lane (within the group), bank group, word
+                for (int j = 0; j < LP; ++j)
+                    for (int st = 0; st < steps; ++st) {
+                        const uint32_t w = grid[(size_t)(q * LP + j) * steps + st];
+                        if (w != kPad) edges.push_back({j, (int)(granule(w, 0) % (uint32_t)LP), (int)w});
+                    }
+                std::vector<int> at_lane((size_t)LP * steps, -1), at_res((size_t)LP * steps, -1), colour(edges.size(), -1);
+                for (size_t e = 0; e < edges.size(); ++e) {
+                    const int u = edges[e][0], r = edges[e][1];
+                    int a = -1, b = -1;
+                    for (int c = 0; c < steps && a < 0; ++c) if (at_lane[(size_t)u * steps + c] < 0) a = c;
+                    for (int c = 0; c < steps && b < 0; ++c) if (at_res[(size_t)r * steps + c] < 0) b = c;
+                    REQUIRE(a >= 0, "internal: a lane holds more gather entries than steps");
+                    if (b < 0) { colour[e] = a; at_lane[(size_t)u * steps + a] = (int)e; continue; }   // over capacity
+                    if (at_res[(size_t)r * steps + a] >= 0) {
+                        // flip the a / b alternating path that starts at bank group r with colour a
+                        std::vector<int> path;
+                        int cur_res = r, col = a;
+                        for (;;) {
+                            const int e1 = at_res[(size_t)cur_res * steps + col];
+                            if (e1 < 0) break;
+                            path.push_back(e1);
+                            const int lane1 = edges[e1][0], other = col == a ? b : a;
+                            const int e2 = at_lane[(size_t)lane1 * steps + other];
+                            if (e2 < 0) break;
+                            path.push_back(e2);
+                            cur_res = edges[e2][1];
+                            if (at_res[(size_t)cur_res * steps + other] != e2) break;     // e2 was an over-capacity edge
+                        }
+                        for (int pe : path) {
+                            const int c0 = colour[pe];
+                            if (at_lane[(size_t)edges[pe][0] * steps + c0] == pe) at_lane[(size_t)edges[pe][0] * steps + c0] = -1;
+                            if (at_res[(size_t)edges[pe][1] * steps + c0] == pe) at_res[(size_t)edges[pe][1] * steps + c0] = -1;
+                        }
+                        for (int pe : path) {
+                            const int c1 = colour[pe] == a ? b : a;
+                            colour[pe] = c1;
+                            at_lane[(size_t)edges[pe][0] * steps + c1] = pe;
+                            if (at_res[(size_t)edges[pe][1] * steps + c1] < 0) at_res[(size_t)edges[pe][1] * steps + c1] = pe;
+                        }
+                    }
+                    if (at_lane[(size_t)u * steps + a] >= 0 || at_res[(size_t)r * steps + a] >= 0) {
+                        // the flip could not free colour a here (an over-capacity edge cut the path): any free step
+                        a = -1;
+                        for (int c = 0; c < steps && a < 0; ++c) if (at_lane[(size_t)u * steps + c] < 0) a = c;
+                        colour[e] = a; at_lane[(size_t)u * steps + a] = (int)e;
+                        if (at_res[(size_t)r * steps + a] < 0) at_res[(size_t)r * steps + a] = (int)e;
+                        continue;
+                    }
+                    colour[e] = a;
+                    at_lane[(size_t)u * steps + a] = (int)e;
+                    at_res[(size_t)r * steps + a] = (int)e;
+                }
+                // write the group's lanes back: entry of colour c at step c, the rest pads
+                std::vector<uint32_t> fresh((size_t)LP * steps, kPad);
+                bool ok = true;
+                for (size_t e = 0; e < edges.size(); ++e) {
+                    uint32_t &slot = fresh[(size_t)edges[e][0] * steps + colour[e]];
+                    if (slot != kPad) ok = false;
+                    slot = (uint32_t)edges[e][2];
+                }
+                if (ok)
+                    for (int j = 0; j < LP; ++j)
+                        for (int st = 0; st < steps; ++st) grid[(size_t)(q * LP + j) * steps + st] = fresh[(size_t)j * steps + st];
+            }
+        }
         for (int pass = 0; pass < 6; ++pass) {
             bool improved = false;
             for (int lane = 0; lane < 32; ++lane) {
@@ -818,6 +897,120 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         }
         o.n_arow = (int)(arranged.size() / NW);
         o.n_arow01 = rows01;
+
+        // ---- bank-aware LAYOUT of the s' values.  Where a value sits in E decides its bank; the lanes of one
+        // shared-memory wavefront of a gather (LP lanes) should read LP different bank groups at every step.  The
+        // reaction phase writes the values of one slot position of 32 reactions to consecutive indices, so any
+        // permutation of the indices AMONG the lanes of one of its store wavefronts keeps those stores
+        // conflict-free.  That freedom is used here: a gather group (the LP lanes of a chunk or of a phase-B
+        // cell column, `cap` steps) is conflict-free iff no bank group is read more than `cap` times (the
+        // lane x bank-group multigraph is then cap-edge-colourable, Koenig; `place` below finds the steps), and
+        // pairs of values of one store wavefront trade indices while that lowers the total excess.
+        if (hints.layout != 2 && nv > 0) {
+            const uint32_t unit = (uint32_t)(S * 8 / gsz);
+            auto res_of = [&](uint32_t e) { return (int)((e * unit) % (uint32_t)LP); };
+            struct Grp { int cap; std::array<int, 16> cnt; };
+            std::vector<Grp> groups;
+            std::vector<std::vector<int>> member(nv);                  // V entry -> groups (with multiplicity)
+            auto add_entry = [&](int g, uint32_t e) {
+                if (e < nv) member[e].push_back(g);
+                groups[g].cnt[res_of(e)] += 1;
+            };
+            for (auto &c : arranged) {
+                if (c.kind != kSum1 && c.kind != kProd) continue;
+                const int width = 1 << c.rshift;
+                const int g0 = (int)groups.size();
+                for (int h = 0; h < nq; ++h) groups.push_back(Grp{c.steps, {}});
+                for (size_t i = 0; i < c.t.size(); ++i) {
+                    std::vector<std::pair<uint32_t, int>> ww;
+                    if (c.kind == kProd) ww = c.t[i]->ent; else split(c.t[i]->ent, ww);
+                    for (size_t e = 0; e < ww.size(); ++e) {
+                        const int lane = (int)i * width + (int)(e % width);
+                        add_entry(g0 + lane / LP, c.kind == kProd ? (ww[e].first & 0xFFFF) : ww[e].first);
+                    }
+                }
+            }
+            for (int slab = 0; slab < o.n_slab; ++slab)
+                for (int c = 0; c < ld; ++c)
+                    for (int h = 0; h < rp; ++h) {
+                        int nst = 0;
+                        for (int lane = 0; lane < 32; ++lane) {
+                            const int r = rp * (32 * slab + lane) + h;
+                            if (r < ld) nst = std::max(nst, (int)cell_w[(size_t)r + (size_t)c * ld].size());
+                        }
+                        if (nst == 0) continue;
+                        const int g0 = (int)groups.size();
+                        for (int hh = 0; hh < nq; ++hh) groups.push_back(Grp{nst == 1 ? 1 : 3, {}});
+                        for (int lane = 0; lane < 32; ++lane) {
+                            const int r = rp * (32 * slab + lane) + h;
+                            if (r >= ld) continue;
+                            for (auto &e : cell_w[(size_t)r + (size_t)c * ld]) add_entry(g0 + lane / LP, e.first);
+                        }
+                    }
+            auto excess = [&](int g) {
+                int x = 0;
+                for (int k = 0; k < LP; ++k) x += std::max(0, groups[g].cnt[k] - groups[g].cap);
+                return x;
+            };
+            // store wavefronts: V entries with the same (group, position, lane / LP), consecutive in v_run
+            std::vector<uint32_t> where(nv);                          // where[v] = index v's value now sits at
+            for (uint32_t v = 0; v < nv; ++v) where[v] = v;
+            long long before = 0, after = 0;
+            for (size_t g = 0; g < groups.size(); ++g) before += excess((int)g);
+            for (int sweep = 0; sweep < 12; ++sweep) {
+                bool improved = false;
+                for (uint32_t a0 = 0; a0 < nv;) {
+                    uint32_t a1 = a0 + 1;
+                    while (a1 < nv && v_run[a1][0] == v_run[a0][0] && v_run[a1][1] == v_run[a0][1] &&
+                           v_run[a1][2] / LP == v_run[a0][2] / LP)
+                        ++a1;
+                    for (uint32_t x = a0; x < a1; ++x)
+                        for (uint32_t y = x + 1; y < a1; ++y) {
+                            // values x and y trade places: every group of x moves one count from res(where[x]) to
+                            // res(where[y]) and vice versa
+                            const int rx = res_of(where[x]), ry = res_of(where[y]);
+                            if (rx == ry) continue;
+                            int cost0 = 0, cost1 = 0;
+                            for (int g : member[x]) cost0 += excess(g);
+                            for (int g : member[y]) cost0 += excess(g);
+                            for (int g : member[x]) { groups[g].cnt[rx] -= 1; groups[g].cnt[ry] += 1; }
+                            for (int g : member[y]) { groups[g].cnt[ry] -= 1; groups[g].cnt[rx] += 1; }
+                            for (int g : member[x]) cost1 += excess(g);
+                            for (int g : member[y]) cost1 += excess(g);
+                            if (cost1 < cost0) {
+                                std::swap(where[x], where[y]);
+                                improved = true;
+                            } else {
+                                for (int g : member[x]) { groups[g].cnt[rx] += 1; groups[g].cnt[ry] -= 1; }
+                                for (int g : member[y]) { groups[g].cnt[ry] += 1; groups[g].cnt[rx] -= 1; }
+                            }
+                        }
+                    a0 = a1;
+                }
+                if (!improved) break;
+            }
+            for (size_t g = 0; g < groups.size(); ++g) after += excess((int)g);
+            o.n_layout_excess[0] = before; o.n_layout_excess[1] = after;
+            // apply: every reference to V entry v now names where[v]
+            auto mv = [&](uint32_t e) { return e < nv ? where[e] : e; };
+            for (int sr = 0; sr < nr; ++sr) {
+                for (int w = 0; w < 3; ++w) {
+                    const uint32_t lo = o.vidx[4 * sr + w] & 0xFFFF, hi = o.vidx[4 * sr + w] >> 16;
+                    o.vidx[4 * sr + w] = mv(lo) | mv(hi) << 16;
+                }
+            }
+            for (size_t k = 0; k < o.eff_ent.size(); k += 4) {
+                const uint32_t sp = o.eff_ent[k] & 0xFFFF, vi = o.eff_ent[k] >> 16;
+                o.eff_ent[k] = sp | mv(vi) << 16;
+            }
+            for (auto &t : sums) {
+                if (t.kind == kSum1) for (auto &e : t.ent) e.first = mv(e.first);
+                if (t.kind == kProd) for (auto &e : t.ent) e.first = mv(e.first & 0xFFFF) | (e.first & 0xFFFF0000u);
+            }
+            for (auto &cl : cell_w)
+                for (auto &e : cl) e.first = mv(e.first);
+        }
+
         for (auto &c : arranged) {
             const uint32_t base = (uint32_t)(o.a_ent.size() / 4);       // in uint4 units
             const int width = 1 << c.rshift, per_row = 32 / width;
@@ -970,7 +1163,7 @@ ShapeHints hints_from_shape(const pyjac_launch_shape *shape, long long smem_opti
     if (shape) {
         h.S = shape->states_per_cta; h.threads = shape->threads; h.ctas = shape->ctas_per_sm;
         h.cap = shape->list_cap; h.cell_cap = shape->cell_cap; h.rp = shape->rows_per_lane;
-        h.p1_states = shape->p1_states; h.stage = shape->stage_tables;
+        h.p1_states = shape->p1_states; h.stage = shape->stage_tables; h.layout = shape->layout;
     }
     return h;
 }

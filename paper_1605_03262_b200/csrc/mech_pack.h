@@ -47,6 +47,7 @@ struct HostPack {
     long long n_cell_entries = 0, n_cells = 0, n_heavy_cells = 0, n_heavy_pieces = 0, n_a_steps = 0, n_b_steps = 0;
     long long n_plain_chunks = 0;
     long long n_a_steps_kind[4] = {0, 0, 0, 0};     // phase-A steps by chunk kind
+    long long n_layout_excess[2] = {0, 0};          // bank-group excess of the gather groups before / after the layout search
     long long n_conflict_wf[2] = {0, 0};            // shared-memory wavefronts beyond one per lane group and step that the
                                                     // placement leaves (phase A, phase B; model of mech_pack.cu `place`)
 };
@@ -61,6 +62,7 @@ struct ShapeHints {
     int rp = 0;         // rows per lane in phase B (1 or 2)
     int p1_states = 0;  // states per work item of the fast reaction path (0: all S)
     int stage = 0;      // 1: copy the gather tables of phases A and B to shared memory once per CTA
+    int layout = 0;     // 2: keep the s' values in allocation order (no bank-aware layout of E)
 };
 
 // The hints of an explicit launch shape (NULL: all zeros = choose); `smem_optin` = the device's opt-in

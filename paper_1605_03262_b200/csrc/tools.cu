@@ -48,6 +48,7 @@ int pyjac_tools_pack_stats(const pyjac_mech_desc *d, const pyjac_launch_shape *s
     stats[15] = (int64_t)hp.b_ent.size() * 4;
     for (int k = 0; k < 4; ++k) stats[16 + k] = hp.n_a_steps_kind[k];
     stats[20] = hp.n_conflict_wf[0]; stats[21] = hp.n_conflict_wf[1];
+    stats[22] = hp.n_layout_excess[0]; stats[23] = hp.n_layout_excess[1];
     return PYJAC_OK;
 }
 
