@@ -84,8 +84,9 @@ struct DeviceMech {
                                 // 2 = any rate form with at most three molecules per side, k_r from K_c and one NASA
                                 // breakpoint: the item's states one after the other, the reaction's constants in registers
     const uint4 *slots;         // [nr] {spec0|spec1<<16, spec2|spec3<<16, spec4|spec5<<16, meta}
-    const uint4 *vidx;          // [nr] E indices of the slots' s'_ij: {v0|v1<<16, v2|v3<<16, v4|v5<<16, 0}
-                                //      (empty slots point at the dump slot)
+    const uint4 *vidx;          // [nr] E indices of the slots' s'_ij: {v0|v1<<16, v2|v3<<16, v4|v5<<16, rpos}
+                                //      (empty slots point at the dump slot); rpos = the reaction's position in the
+                                //      regions Q and H (a permutation within its store wavefront, mech_pack.cu)
     const double *lnA, *beta, *Ta;               // [nr] forward Arrhenius (k_inf for falloff forms)
     const int32_t *rxn_orig;    // [nr] caller's reaction index
     const double *rev_lnA, *rev_beta, *rev_Ta;   // [nr] explicit reverse parameters
@@ -122,8 +123,8 @@ struct DeviceMech {
                                 // cell h (padded with the zero slot), steps of the item's cells h: 0 none, 1 one, 2 three}
     const int32_t *bsplit;      // [NW + 1] the items of warp w are [bsplit[w], bsplit[w + 1])
     // ---- regions of E (indices in elements per state)
-    int eQ;                     // [nr][3] {q_i, a_i + W q_i, Theta_dT,i}
-    int eH;                     // [nr] reaction enthalpy H_i
+    int eQ;                     // [nr][3] {q_i, a_i + W q_i, Theta_dT,i} of the reaction at position rpos
+    int eH;                     // [nr] reaction enthalpy H_i, same positions
     int eAlpha, eGamma;         // [ns+1] alpha'_r = A_k / rho, gamma'_r = Gamma_k / W_Ns by Jacobian row r = k + 1
     int eTc;                    // [ns+1] the T column by row: sum_i nu_ki Theta_i / rho (Eq. 111 without W_k)
     int eWdot;                  // [ns]

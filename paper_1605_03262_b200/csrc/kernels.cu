@@ -234,8 +234,8 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
     const double *th = m.th_soa + s;
     const double brk = m.brk_common == m.brk_common ? m.brk_common : th[0];
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
+    const uint4 vi = m.vidx[s];
     if (LEVEL == 2) {
-        const uint4 vi = m.vidx[s];
         v0 = (vi.x & 0xFFFF) * S; v1 = (vi.x >> 16) * S; v2 = (vi.y & 0xFFFF) * S;
         v3 = (vi.y >> 16) * S; v4 = (vi.z & 0xFFFF) * S; v5 = (vi.z >> 16) * S;
     }
@@ -249,7 +249,7 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
         ef = m.eff_ent + m.eff_base[grp] + (s & 31);
         n_eff = m.eff_base[grp + 1] - m.eff_base[grp];
     }
-    const int eq = (m.eQ + 3 * s) * S, eh = (m.eH + s) * S;
+    const int eq = (m.eQ + 3 * (int)vi.w) * S, eh = (m.eH + (int)vi.w) * S;
     PYJAC_CHECK(x0 <= m.ns * S && x1 <= m.ns * S && x2 <= m.ns * S && x3 <= m.ns * S && x4 <= m.ns * S && x5 <= m.ns * S);
     PYJAC_CHECK(v0 < m.n_e * S && v1 < m.n_e * S && v2 < m.n_e * S && v3 < m.n_e * S && v4 < m.n_e * S && v5 < m.n_e * S);
     PYJAC_CHECK(eq + 3 * S <= m.n_e * S && eh + S <= m.n_e * S && q0 >= 0 && q1 <= S);
@@ -477,8 +477,9 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     for (int i = 0; i < 5; ++i) fp[i] = m.fall_par[5 * s_pd + i];
     const double dnu = (double)(snu_r - snu_f);
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
+    const uint4 vi = m.vidx[s];
+    const int rq = (m.eQ + 3 * (int)vi.w) * S, rh = (m.eH + (int)vi.w) * S;     // the reaction's places in Q and H
     if (LEVEL == 2) {
-        const uint4 vi = m.vidx[s];
         v0 = (vi.x & 0xFFFF) * S; v1 = (vi.x >> 16) * S; v2 = (vi.y & 0xFFFF) * S;
         v3 = (vi.y >> 16) * S; v4 = (vi.z & 0xFFFF) * S; v5 = (vi.z >> 16) * S;
     }
@@ -670,8 +671,8 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             }
         }
         const double qi = c * R;
-        E[(m.eQ + 3 * s) * S + q] = qi;
-        if (LEVEL >= 1) E[(m.eH + s) * S + q] = H;
+        E[rq + q] = qi;
+        if (LEVEL >= 1) E[rh + q] = H;
         if (LEVEL == 0) {
             const long long st = state0 + q;
             if (st < n) {
@@ -696,8 +697,8 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
             // sparse terms s'_ij = c (k_f S'_j - k_r S''_j) per slot, b (alpha_ij - 1) per efficiency
             const double ckf = c * kf, ckr = -c * kr;
             if (LEVEL == 2) {
-                E[(m.eQ + 3 * s + 2) * S + q] = theta;
-                E[(m.eQ + 3 * s + 1) * S + q] = ai;
+                E[rq + 2 * S + q] = theta;
+                E[rq + S + q] = ai;
                 E[v0 + q] = ckf * sk0; E[v1 + q] = ckf * sk1; E[v2 + q] = ckf * sk2;
                 E[v3 + q] = ckr * sk3; E[v4 + q] = ckr * sk4; E[v5 + q] = ckr * sk5;
             }
@@ -720,7 +721,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
                         else tau = fma(be, Vw[(w[u].x & 0xFFFF) * S + q], tau);
                     }
                 }
-            if (LEVEL == 3) E[(m.eQ + 3 * s + 1) * S + q] = tau;
+            if (LEVEL == 3) E[rq + S + q] = tau;
         }
     }
 }

@@ -693,7 +693,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         // one colour at a vertex iff no bank group is read more often than `steps` times (Koenig) -- then every
         // step reads LP different bank groups.  Alternating-path edge colouring; an edge whose bank group is
         // over capacity takes a step that is free at its lane and stays a conflict for the search below.
-        if (nstream == 1) {
+        {       // (two streams: the colouring takes the first stream, the search below sees both)
             for (int q = 0; q < nq; ++q) {
                 std::vector<std::array<int, 3>> edges;                 // lane (within the group), bank group, word
                 for (int j = 0; j < LP; ++j)
@@ -898,6 +898,25 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         o.n_arow = (int)(arranged.size() / NW);
         o.n_arow01 = rows01;
 
+        // the partial sums of the long cell lists (region Hs) in the order in which the chunks' lanes produce them:
+        // the 32 results of a chunk go to 32 consecutive elements (their stores meet few bank conflicts)
+        if (hints.layout != 2 && o.n_heavy_pieces > 0) {
+            std::vector<uint32_t> renum((size_t)o.n_heavy_pieces, 0xFFFFFFFFu);
+            uint32_t next = 0;
+            for (auto &c : arranged)
+                if (c.kind == kSum1)
+                    for (Task *t : c.t)
+                        if (t->out >= (uint32_t)eHs && t->out < (uint32_t)(eHs + o.n_heavy_pieces)) {
+                            renum[t->out - (uint32_t)eHs] = next;
+                            t->out = (uint32_t)eHs + next++;
+                        }
+            REQUIRE(next == (uint32_t)o.n_heavy_pieces, "internal: a partial sum of a cell list is in no chunk");
+            for (auto &cl : cell_w)
+                for (auto &e : cl)
+                    if (e.first >= (uint32_t)eHs && e.first < (uint32_t)(eHs + o.n_heavy_pieces))
+                        e.first = (uint32_t)eHs + renum[e.first - (uint32_t)eHs];
+        }
+
         // ---- bank-aware LAYOUT of the s' values.  Where a value sits in E decides its bank; the lanes of one
         // shared-memory wavefront of a gather (LP lanes) should read LP different bank groups at every step.  The
         // reaction phase writes the values of one slot position of 32 reactions to consecutive indices, so any
@@ -1010,6 +1029,74 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             for (auto &cl : cell_w)
                 for (auto &e : cl) e.first = mv(e.first);
         }
+        // The same for the per-reaction blocks {q_i, a_i, Theta_i} (region Q, three elements per reaction) and H_i:
+        // reaction s keeps both at position rpos[s]; positions are traded among the reactions of one store
+        // wavefront (LP lanes of a group of 32) against the gather groups of the per-species sums (they read Q)
+        // and of the energy-row column sums (their second stream reads H).
+        std::vector<uint32_t> rpos(std::max(nr, 1));
+        for (int sr = 0; sr < nr; ++sr) rpos[sr] = (uint32_t)sr;
+        if (hints.layout != 2 && nr > 0) {
+            const uint32_t unit = (uint32_t)(S * 8 / gsz);
+            auto res_t = [&](int type, uint32_t pos) {
+                return (int)(((type == 0 ? (uint32_t)eQ + 3u * pos : (uint32_t)eH + pos) * unit) % (uint32_t)LP);
+            };
+            struct Grp { int cap; std::array<int, 16> cnt; };
+            std::vector<Grp> groups;
+            std::vector<std::vector<std::pair<int, int>>> member(nr);      // reaction -> (group, type)
+            for (auto &c : arranged) {
+                if (c.kind != kSum3 && c.kind != kProd) continue;
+                const int width = 1 << c.rshift, type = c.kind == kSum3 ? 0 : 1;
+                const int g0 = (int)groups.size();
+                for (int h = 0; h < nq; ++h) groups.push_back(Grp{c.steps, {}});
+                for (size_t i = 0; i < c.t.size(); ++i) {
+                    std::vector<std::pair<uint32_t, int>> ww;
+                    if (c.kind == kProd) ww = c.t[i]->ent; else split(c.t[i]->ent, ww);
+                    for (size_t e = 0; e < ww.size(); ++e) {
+                        const int lane = (int)i * width + (int)(e % width);
+                        const int sr = c.kind == kSum3 ? (int)(ww[e].first - (uint32_t)eQ) / 3 : (int)((ww[e].first >> 16) - (uint32_t)eH);
+                        member[sr].push_back({g0 + lane / LP, type});
+                        groups[g0 + lane / LP].cnt[res_t(type, (uint32_t)sr)] += 1;
+                    }
+                }
+            }
+            auto excess = [&](int g) {
+                int x = 0;
+                for (int k = 0; k < LP; ++k) x += std::max(0, groups[g].cnt[k] - groups[g].cap);
+                return x;
+            };
+            auto move = [&](int sr, uint32_t from, uint32_t to) {
+                for (auto &mg : member[sr]) {
+                    groups[mg.first].cnt[res_t(mg.second, from)] -= 1;
+                    groups[mg.first].cnt[res_t(mg.second, to)] += 1;
+                }
+            };
+            for (int sweep = 0; sweep < 12; ++sweep) {
+                bool improved = false;
+                for (int a0 = 0; a0 < nr; a0 += LP) {
+                    const int a1 = std::min(nr, std::min(a0 + LP, (a0 / 32 + 1) * 32));
+                    for (int x = a0; x < a1; ++x)
+                        for (int y = x + 1; y < a1; ++y) {
+                            int cost0 = 0, cost1 = 0;
+                            for (auto &mg : member[x]) cost0 += excess(mg.first);
+                            for (auto &mg : member[y]) cost0 += excess(mg.first);
+                            const uint32_t px = rpos[x], py = rpos[y];
+                            move(x, px, py); move(y, py, px);
+                            for (auto &mg : member[x]) cost1 += excess(mg.first);
+                            for (auto &mg : member[y]) cost1 += excess(mg.first);
+                            if (cost1 < cost0) { std::swap(rpos[x], rpos[y]); improved = true; }
+                            else { move(x, py, px); move(y, px, py); }
+                        }
+                }
+                if (!improved) break;
+            }
+            for (auto &t : sums) {
+                if (t.kind == kSum3)
+                    for (auto &e : t.ent) e.first = (uint32_t)eQ + 3u * rpos[(e.first - (uint32_t)eQ) / 3];
+                if (t.kind == kProd)
+                    for (auto &e : t.ent) e.first = (e.first & 0xFFFF) | ((uint32_t)eH + rpos[(e.first >> 16) - (uint32_t)eH]) << 16;
+            }
+        }
+        for (int sr = 0; sr < nr; ++sr) o.vidx[4 * sr + 3] = rpos[sr];
 
         for (auto &c : arranged) {
             const uint32_t base = (uint32_t)(o.a_ent.size() / 4);       // in uint4 units
