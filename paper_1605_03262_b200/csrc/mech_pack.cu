@@ -624,10 +624,11 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     // ---- work items of P1: the groups that need the one-state path first, then the pressure-dependent
     // groups, then the plain ones, each for every state (pair)
     {
-        // states per fast-path item: all S (the reaction's constants are read once per batch) when several CTAs
-        // share an SM and fill each other's queue tails; one state per item when a single CTA has the SM to
-        // itself (111 species: 6.5 against 8.1 ms per 100,000 states)
-        const int per = hints.p1_states > 0 ? std::min(hints.p1_states, S) : o.ctas_target > 1 ? S : 1;
+        // states per fast-path item: two when the states come in pairs (S even), else one.  Finer items balance the
+        // reaction queue over the warps; with the bank-aware layout in place that is worth more than reading a
+        // reaction's constants once per batch (53 species, S = 3: 2.29 ms with one state per item, 2.32 with two,
+        // 2.44 with three; profiles/r2_shape_sweeps.md)
+        const int per = hints.p1_states > 0 ? std::min(hints.p1_states, S) : (S % 2 == 0 ? 2 : 1);
         for (uint32_t kind : {0u, 2u, 1u})
             for (int c = 0; c < o.n_rchunk; ++c) {
                 if (o.rchunk[c] != kind) continue;
