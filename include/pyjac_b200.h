@@ -140,7 +140,9 @@ typedef struct pyjac_launch_shape {
     int32_t rows_per_lane;  /* 1 or 2 Jacobian rows per lane in the streaming phase (2 needs N_sp odd,
                                i.e. an even leading dimension; 16-byte stores) */
     int32_t p1_states;      /* states one work item of the reaction phase evaluates with the reaction's
-                               constants held in registers (0: all states_per_cta) */
+                               constants held in registers: p + 16 g = p states per item of a group of plain
+                               elementary reactions, g per item of a group with other rate forms (g = 0: p);
+                               0: all states_per_cta for plain groups, one for the others */
     int32_t stage_tables;   /* 1: copy the gather tables to shared memory once per CTA (PYJAC_ELIMIT if they
                                do not fit this shape); 0: read them through L1 / L2 */
     int32_t layout;         /* 2: keep the per-reaction terms in allocation order in shared memory; 0 / 1: place

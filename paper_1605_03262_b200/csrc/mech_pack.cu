@@ -547,7 +547,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     REQUIRE(hints.cell_cap >= 0 && hints.cell_cap <= 3, "cell_cap must be 0 (choose) or 1..3");
     REQUIRE(hints.cap >= 0 && hints.rp >= 0 && hints.rp <= 2 && hints.ctas >= 0 && hints.ctas <= 4 && hints.threads >= 0 && hints.S >= 0,
             "launch shape out of range");
-    REQUIRE(hints.p1_states >= 0 && hints.p1_states <= 15, "p1_states out of range");
+    REQUIRE(hints.p1_states >= 0 && hints.p1_states <= 255, "p1_states out of range");
     const int cell_cap = hints.cell_cap >= 1 ? hints.cell_cap : 3;
     constexpr int kPiece = 8;
     std::vector<std::vector<std::pair<uint32_t, int>>> cell_w((size_t)ld * ld);
@@ -624,15 +624,19 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     // ---- work items of P1: the groups that need the one-state path first, then the pressure-dependent
     // groups, then the plain ones, each for every state (pair)
     {
-        // states per fast-path item: two when the states come in pairs (S even), else one.  Finer items balance the
-        // reaction queue over the warps; with the bank-aware layout in place that is worth more than reading a
-        // reaction's constants once per batch (53 species, S = 3: 2.29 ms with one state per item, 2.32 with two,
-        // 2.44 with three; profiles/r2_shape_sweeps.md)
-        const int per = hints.p1_states > 0 ? std::min(hints.p1_states, S) : (S % 2 == 0 ? 2 : 1);
+        // states per fast-path item.  Plain groups (nine of eleven on 53 species) take all S states in one item:
+        // the reaction's constants are read once per batch and stay in registers.  Groups with pressure-dependent
+        // or PLOG / Chebyshev lanes cost two to three times as much per state and are the long items of the queue:
+        // one state per item, so that the queue balances over the warps.  Measured with the bank-aware layout in
+        // place (profiles/r2_shape_sweeps.md), 53 species S = 3: 2.16 ms against 2.29 (one state per item
+        // everywhere) and 2.44 (three everywhere); 111 species 5.72 against 6.02 ms.
+        // shape.p1_states: 0 = this rule; else states per plain item + 16 * states per general item (0: the same)
+        const int per = hints.p1_states > 0 ? std::max(1, std::min(hints.p1_states % 16, S)) : S;
+        const int per_gen = hints.p1_states >= 16 ? std::min(hints.p1_states / 16, S) : hints.p1_states > 0 ? per : 1;
         for (uint32_t kind : {0u, 2u, 1u})
             for (int c = 0; c < o.n_rchunk; ++c) {
                 if (o.rchunk[c] != kind) continue;
-                const int step = kind == 0u ? 1 : per;
+                const int step = kind == 0u ? 1 : kind == 2u ? per_gen : per;
                 for (int q = 0; q < S; q += step)
                     o.p1item.push_back((uint32_t)c | kind << 16 | (uint32_t)q << 20 | (uint32_t)std::min(step, S - q) << 24);
             }
