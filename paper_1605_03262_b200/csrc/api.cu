@@ -138,7 +138,7 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
         up.add(&dm.lnA, hp.lnA); up.add(&dm.beta, hp.beta); up.add(&dm.Ta, hp.Ta);
         up.add(&dm.rxn_orig, hp.rxn_orig); up.add(&dm.p1item, hp.p1item);
         up.add(&dm.rev_lnA, hp.rev_lnA); up.add(&dm.rev_beta, hp.rev_beta); up.add(&dm.rev_Ta, hp.rev_Ta);
-        up.add(&dm.th_off, hp.th_off); up.add(&dm.th_data, hp.th_data); up.add(&dm.th_soa, hp.th_soa);
+        up.add(&dm.th_off, hp.th_off); up.add(&dm.th_data, hp.th_data); up.add(&dm.th_soa, hp.th_soa); up.add(&dm.th_brk, hp.th_brk);
         up.add(&dm.lo_lnA, hp.lo_lnA); up.add(&dm.lo_beta, hp.lo_beta); up.add(&dm.lo_Ta, hp.lo_Ta);
         up.add(&dm.fall_par, hp.fall_par);
         up.add(&dm.eff_base, hp.eff_base); up.add((const uint32_t **)&dm.eff_ent, hp.eff_ent);

@@ -96,9 +96,10 @@ struct DeviceMech {
                                 // (Eq. 27 summed over the reaction, one set per interval between the t_mid of
                                 // its species; g0 includes (sum nu) ln(p_atm / R) of Eq. 26)
     double brk_common;          // the breakpoint every reaction shares (all n_int <= 2, one t_mid), else NaN
-    const double *th_soa;       // [15][nr] the same for reactions with n_int <= 2, coalesced over reactions:
-                                // row 0 the breakpoint (+inf if n_int = 1), rows 1..7 g of the lower interval,
-                                // rows 8..14 g of the upper one
+    const double *th_soa;       // the same for reactions with n_int <= 2, per group of 32 reactions and interval:
+                                // g_c of reaction s at [(((s >> 5) * 2 + interval) * 7 + c) * 32 + (s & 31)], so that a
+                                // lane reads its seven coefficients at constant offsets from one address (coalesced)
+    const double *th_brk;       // [nr] the breakpoint (+inf if n_int = 1, NaN if n_int > 2)
     const double *lo_lnA, *lo_beta, *lo_Ta;      // [n_pd] k_0
     const double *fall_par;                      // [n_pd][5]; Troe: {a, 1/T***, 1/T*, T**, has T**}; SRI: {a, b, 1/c, d, e}
     const int32_t *eff_base;    // [general groups + 1] first efficiency entry of a group of 32 reactions

@@ -231,8 +231,8 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
         if (type == PYJAC_CHEM_ACTIVATED) { lnA = l0; beta = b0; Ta = t0; }
     }
     // sum_k nu_ki B_k (Eq. 27 over the reaction): both intervals
-    const double *th = m.th_soa + s;
-    const double brk = m.brk_common == m.brk_common ? m.brk_common : th[0];
+    const double *th = m.th_soa + (size_t)(s >> 5) * (2 * 7 * 32) + (s & 31);
+    const double brk = m.brk_common == m.brk_common ? m.brk_common : m.th_brk[s];
     int v0 = 0, v1 = 0, v2 = 0, v3 = 0, v4 = 0, v5 = 0;
     const uint4 vi = m.vidx[s];
     if (LEVEL == 2) {
@@ -272,8 +272,8 @@ __device__ __forceinline__ void p1_group(const DeviceMech &m, double *E, const d
         // sum_k nu_ki B_k and its T derivative (Eq. 74)
 #pragma unroll
         for (int u = 0; u < NQ; ++u) {
-            const double *g = th + (T[u] > brk ? 8 : 1) * nr;
-            const double g0 = g[0], g1 = g[nr], g2 = g[2 * nr], g3 = g[3 * nr], g4 = g[4 * nr], g5 = g[5 * nr], g6 = g[6 * nr];
+            const double *g = th + (T[u] > brk ? 7 * 32 : 0);
+            const double g0 = g[0], g1 = g[32], g2 = g[64], g3 = g[96], g4 = g[128], g5 = g[160], g6 = g[192];
             const double t = T[u];
             sB[u] = fma(g1, lnT[u], g0) + fma(t, fma(t, fma(t, fma(t, g5, g4), g3), g2), g6 * invT[u]);
             sdB[u] = fma(fma(-g6, invT[u], g1), invT[u], g2) + t * fma(t, fma(4.0 * g5, t, 3.0 * g4), 2.0 * g3);
@@ -468,7 +468,7 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
     // every table read of the reaction is issued here, before the first use, so that the reads
     // overlap (one L2 round trip instead of one per parameter group); indices are clamped, the values
     // of reactions that do not use them are ignored
-    const double brk = m.brk_common == m.brk_common ? m.brk_common : m.th_soa[s];   // NaN: more than two intervals, see th_data
+    const double brk = m.brk_common == m.brk_common ? m.brk_common : m.th_brk[s];   // NaN: more than two intervals, see th_data
     const double lnA = m.lnA[s], beta = m.beta[s], Ta = m.Ta[s];
     const int s_pd = min(s, max(m.n_pd, 1) - 1);
     const double lo_lnA = m.lo_lnA[s_pd], lo_beta = m.lo_beta[s_pd], lo_Ta = m.lo_Ta[s_pd];
@@ -565,9 +565,8 @@ __device__ __forceinline__ void reaction(const DeviceMech &m, const SmemPlan &sp
         //      enthalpy H_i = sum_k nu_ki h_k W_k = R T (T d(sum nu B)/dT + sum nu)
         double g0, g1, g2, g3, g4, g5, g6;
         if (brk == brk) {
-            const double *g = m.th_soa + s + (size_t)(T > brk ? 8 : 1) * m.nr;
-            const size_t nrs = (size_t)m.nr;
-            g0 = g[0]; g1 = g[nrs]; g2 = g[2 * nrs]; g3 = g[3 * nrs]; g4 = g[4 * nrs]; g5 = g[5 * nrs]; g6 = g[6 * nrs];
+            const double *g = m.th_soa + (size_t)((s >> 5) * 2 + (T > brk ? 1 : 0)) * (7 * 32) + (s & 31);
+            g0 = g[0]; g1 = g[32]; g2 = g[64]; g3 = g[96]; g4 = g[128]; g5 = g[160]; g6 = g[192];
         } else {
             const double *th = m.th_data + m.th_off[s];
             const int nint = (int)th[0];

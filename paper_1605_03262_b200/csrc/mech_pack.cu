@@ -311,7 +311,9 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     o.vidx.assign((size_t)4 * std::max(nr, 1), 0u);
     o.rxn_orig.resize(nr);
     o.th_off.resize(nr);
-    o.th_soa.assign((size_t)15 * std::max(nr, 1), 0.0);
+    o.th_brk.assign(std::max(nr, 1), 0.0);
+    o.th_soa.assign((size_t)((nr + 31) / 32 + 1) * 2 * 7 * 32, 0.0);
+    auto th_at = [&](int sr, int iv, int c) -> double & { return o.th_soa[((size_t)((sr >> 5) * 2 + iv) * 7 + c) * 32 + (sr & 31)]; };
     o.n_pd = 0; o.n_pk = 0;
     o.pk_ptr.assign(1, 0);
     o.eff_ptr.assign(1, 0);
@@ -371,7 +373,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             o.th_off[s] = (uint32_t)o.th_data.size();
             o.th_data.push_back((double)nint);
             for (double b : brk) o.th_data.push_back(b);
-            o.th_soa[s] = nint == 2 ? brk[0] : nint == 1 ? HUGE_VAL : std::nan("");
+            o.th_brk[s] = nint == 2 ? brk[0] : nint == 1 ? HUGE_VAL : std::nan("");
             for (int iv = 0; iv < nint; ++iv) {
                 // interval iv: brk[iv-1] < T <= brk[iv]; species k is in its low range iff T <= t_mid[k]
                 double da[7] = {0, 0, 0, 0, 0, 0, 0};
@@ -387,8 +389,8 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                 for (int c = 0; c < 7; ++c) o.th_data.push_back(g[c]);
                 if (nint <= 2)
                     for (int c = 0; c < 7; ++c) {
-                        o.th_soa[(size_t)(1 + 7 * iv + c) * nr + s] = g[c];
-                        if (nint == 1) o.th_soa[(size_t)(8 + c) * nr + s] = g[c];
+                        th_at(s, iv, c) = g[c];
+                        if (nint == 1) th_at(s, 1, c) = g[c];
                     }
             }
         }
@@ -451,12 +453,12 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
 
 
     // ---- one breakpoint for all reactions?  (reactions with a single interval carry the same
-    // coefficients in both rows of th_soa, so any breakpoint is right for them)
+    // coefficients for both intervals in th_soa, so any breakpoint is right for them)
     {
         double common = HUGE_VAL;
         bool ok = true;
         for (int sr = 0; sr < nr && ok; ++sr) {
-            const double b = o.th_soa[sr];
+            const double b = o.th_brk[sr];
             if (b != b) ok = false;
             else if (b != HUGE_VAL) {
                 if (common == HUGE_VAL) common = b;

@@ -18,7 +18,7 @@ struct HostPack {
     std::vector<double> lnA, beta, Ta, rev_lnA, rev_beta, rev_Ta;
     std::vector<int32_t> rxn_orig;
     std::vector<uint32_t> th_off;
-    std::vector<double> th_data, th_soa;
+    std::vector<double> th_data, th_soa, th_brk;
     double brk_common = 0.0;              // NaN unless every reaction has at most two intervals and one breakpoint
     std::vector<double> lo_lnA, lo_beta, lo_Ta, fall_par;
     std::vector<int32_t> eff_ptr;
