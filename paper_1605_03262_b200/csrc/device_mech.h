@@ -25,6 +25,7 @@ constexpr double kRu = 8314.46261815324;   // J kmol^-1 K^-1
 constexpr double kPatm = 101325.0;         // Pa
 constexpr int kMaxSide = 3;                // species per reaction side
 constexpr int kMaxThreads = 512;           // threads per CTA the kernels are compiled for
+constexpr int kBPad = 3;                   // items of padding behind the phase-B table (the kernel reads that far ahead)
 
 // meta word of a reaction: bits 0..23 six 4-bit nu (slots 0-2 reactants, 3-5 products; 0 = empty
 // slot), 24..26 rxn_type, 27..28 rev_type, 29..30 falloff_form, 31 third body is a single species.

@@ -1041,7 +1041,7 @@ __device__ __forceinline__ void b_run(const DeviceMech &m, const uint4 *b_ent, c
 #pragma unroll
         for (int hh = 0; hh < RP; ++hh) wr[hh] = wrow[rr + hh];
         const uint4 *ep = ebase + (size_t)it * (32 * RP);
-        PYJAC_CHECK(it >= 0 && c1 <= ld && (it + (c1 - c0) + 1) * (32 * RP) <= m.n_bent && slab >= 0 && slab < m.n_slab);
+        PYJAC_CHECK(it >= 0 && c1 <= ld && (it + (c1 - c0) + kBPad) * (32 * RP) <= m.n_bent && slab >= 0 && slab < m.n_slab);
         const double *cc = colc + 4 * c0;
         // element (r, c) of the batch's first state: a running pointer when there is one state (measured: 360
         // species 2.63 -> 2.40 ms per 4,096 states), a 32-bit offset otherwise (S pointers cost registers: 53
@@ -1049,13 +1049,35 @@ __device__ __forceinline__ void b_run(const DeviceMech &m, const uint4 *b_ent, c
         double *dq0 = J0 + (size_t)(c0 * ld + r);
         uint32_t off = (uint32_t)(c0 * ld + r);
         auto dst_of = [&](int q) { return S == 1 ? dq0 : J0 + (off + (uint32_t)q * j_state); };
-        uint4 wA = ep[0], wB = wA;
-        if (RP == 2) wB = ep[32];
+        // the entries of the next D items are in flight while this one is summed (the table is padded by kBPad
+        // items).  One state per CTA makes an item short against the L2 latency of its table words: three items
+        // ahead there (360 species, 4,096 states: 2.37 ms with one, 2.05 with two); with S > 1 the registers cost
+        // more than the latency (53 species 2.13 -> 2.17 ms with two)
+        constexpr int D = S == 1 ? kBPad : 1;
+        uint4 qA[D + 1], qB[D + 1];
+        uint4 cA = ep[0], cB = cA;                                // D = 1: the current and the next item only
+        if (RP == 2) cB = ep[32];
+        if (D > 1) {
+#pragma unroll
+            for (int k = 0; k <= D; ++k) {
+                qA[k] = ep[(size_t)k * 32 * RP];
+                qB[k] = RP == 2 ? ep[(size_t)k * 32 * RP + 32] : qA[k];
+            }
+            ep += (size_t)D * 32 * RP;
+        }
         for (int c = c0; c < c1; ++c, cc += 4) {
             ep += 32 * RP;
-            const uint4 wAn = ep[0];                              // the table is padded by one item
-            uint4 wBn = wAn;
-            if (RP == 2) wBn = ep[32];
+            uint4 wA = cA, wB = cB;
+            if (D > 1) {
+                wA = qA[0]; wB = qB[0];
+#pragma unroll
+                for (int k = 0; k < D; ++k) { qA[k] = qA[k + 1]; qB[k] = qB[k + 1]; }
+                qA[D] = ep[0];
+                qB[D] = RP == 2 ? ep[32] : qA[D];
+            } else {
+                cA = ep[0];
+                cB = RP == 2 ? ep[32] : cA;
+            }
             const double2 uv = *reinterpret_cast<const double2 *>(cc);
             const double iw = cc[2];
             double acc[RP * S];
@@ -1111,7 +1133,6 @@ __device__ __forceinline__ void b_run(const DeviceMech &m, const uint4 *b_ent, c
                     }
                 }
             }
-            wA = wAn; wB = wBn;
             if (S == 1) dq0 += ld; else off += (uint32_t)ld;
         }
         it += c1 - c0;

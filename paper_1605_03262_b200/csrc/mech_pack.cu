@@ -1159,7 +1159,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
     // step count of the item's cells h: 0 (no lane has an entry), 1 (one step), 2 (three steps).
     {
         const size_t n_item = (size_t)o.n_slab * ld;
-        o.b_ent.assign((n_item + 1) * rp * 128, (uint32_t)(eZero * S * 8));     // one item of padding: read ahead
+        o.b_ent.assign((n_item + kBPad) * rp * 128, (uint32_t)(eZero * S * 8));     // padding items: read ahead
         std::vector<double> cost(n_item, 0.0);
         for (int slab = 0; slab < o.n_slab; ++slab)
             for (int c = 0; c < ld; ++c) {
@@ -1239,7 +1239,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
                 }
             }
         }
-        if (o.b_ent.size() != ((size_t)o.n_slab * ld + 1) * rp * 128) bad("internal: phase B table has the wrong size");
+        if (o.b_ent.size() != ((size_t)o.n_slab * ld + kBPad) * rp * 128) bad("internal: phase B table has the wrong size");
         for (size_t k = 0; k < o.b_ent.size(); ++k) {
             const uint32_t wd = o.b_ent[k];
             if (k % 4 == 3) { if (wd > 2u) bad("internal: a phase-B step count is out of range"); continue; }
