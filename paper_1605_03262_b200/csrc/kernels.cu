@@ -806,13 +806,16 @@ __device__ __forceinline__ void st_cs_v2(double *p, double a, double b)
 // applied to the S states; whole blocks of four steps run without a branch, the chunk's last block by
 // its step count.
 template <int LEVEL, int S>
-__device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent, double *E, const double *sc, const uint2 ch, int lane)
+__device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent, double *E, const double *sc, const uint2 ch, int lane,
+                                        const uint4 r0_pre, const uint4 w0_pre)
 {
+    // one state per CTA (S = 1): the chunk's first two table blocks were fetched while the previous chunk was summed
+    constexpr bool PRE = S == 1;
     const uint32_t kind = (ch.y >> 8) & 0xF;
     const int steps = (int)(ch.y & 0xFF), rshift = (int)(ch.y >> 12) & 0xF, width = 1 << rshift;
     const uint4 *ep = a_ent + ch.x + lane;
     PYJAC_CHECK((int)ch.x + 32 * (2 + ((int)((ch.y >> 8) & 0xF) == (int)kAll3 ? 0 : ((int)(ch.y & 0xFF) + 3) / 4)) <= m.n_aent);
-    const uint4 r0 = ep[0];
+    const uint4 r0 = PRE ? r0_pre : ep[0];
     const bool head = (lane & (width - 1)) == 0 && r0.x != 0xFFFFFFFFu;
     const char *Eb = reinterpret_cast<const char *>(E);
     const int nr = m.nr;
@@ -822,7 +825,7 @@ __device__ __forceinline__ void a_chunk(const DeviceMech &m, const uint4 *a_ent,
 #define PYJAC_WALK(step)                                                   \
     {                                                                      \
         const uint4 *bp = ep + 32;                                         \
-        uint4 w = *bp;                                                     \
+        uint4 w = PRE ? w0_pre : *bp;                                      \
         for (int b = 0; b < nfull; ++b) {                                  \
             bp += 32;                                                      \
             const uint4 wn = *bp; /* one block ahead (the table is padded) */ \
@@ -1226,12 +1229,19 @@ __global__ void __launch_bounds__(kMaxThreads, 1)
         {
             const uint2 *hp = achunk + warp;
             uint2 h = *hp;
+            uint4 r0 = make_uint4(0u, 0u, 0u, 0u), w0 = r0;
+            if (S == 1) { r0 = a_ent[h.x + lane]; w0 = a_ent[h.x + 32 + lane]; }
             for (int row = 0; row < arows; ++row) {
                 hp += NW;
                 PYJAC_CHECK((row + 1) * NW + warp < m.n_achunk);
                 const uint2 hn = *hp;                 // the header table is padded by one row
-                a_chunk<LEVEL, S>(m, a_ent, E, sc, h, lane);
-                h = hn;
+                uint4 r0n = r0, w0n = w0;
+                if (S == 1) {                         // both tables are padded for the reads behind the last chunk
+                    PYJAC_CHECK((int)hn.x + 64 <= m.n_aent);
+                    r0n = a_ent[hn.x + lane]; w0n = a_ent[hn.x + 32 + lane];
+                }
+                a_chunk<LEVEL, S>(m, a_ent, E, sc, h, lane, r0, w0);
+                h = hn; r0 = r0n; w0 = w0n;
             }
         }
         __syncthreads();
