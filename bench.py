@@ -66,7 +66,7 @@ def ncu_counters():
                 "dram_bytes_per_state": float(row["dram_bytes_per_state"]),
                 "fp64_flop_per_state": float(row["fp64_flop_per_state"]),
                 "lsu_wavefronts_per_state": float(row["lsu_wavefronts_per_state"])}
-            src = "profiles/r2_ncu_counters.csv (%s)" % row["source"]
+            src = "profiles/r2_ncu_counters.csv (ncu --set full captures of kernel sources %s, profiles/r2_ncu_counters.md)" % sha
     except Exception:
         return {}, None
     return out, src

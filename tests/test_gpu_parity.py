@@ -293,18 +293,26 @@ def test_empty_and_single_state(torch, PyJac, tiny_mechs):
     check_jacobian(torch, pj, o, T, P, Y)
 
 
-def test_padded_leading_dimension_and_batch_split_bit_identical(torch, PyJac):
-    """ldy > Nsp; results do not depend on n, batch split or stream (header contract; App. D)."""
-    m = synth.make_mechanism(0)
+@pytest.mark.parametrize("cfg,n", [(0, 777), (1, 1999), (2, 1000), (3, 130)])
+def test_padded_leading_dimension_and_batch_split_bit_identical(torch, PyJac, cfg, n):
+    """ldy > Nsp; results do not depend on n, batch split, stream or repetition (header contract; App. D).  A
+    batch split changes which CTA evaluates which state and with which neighbours in its batch, and so the
+    timing of every phase: a race between the phases would show as a difference (compute-sanitizer's racecheck
+    is closed on the pool, profiles/r2_checked_build.md).  All four mechanisms: one and several resident CTAs,
+    S = 1 and 3, one and two rows per lane."""
+    m = synth.make_mechanism(cfg)
     pj = PyJac(m)
-    T, P, Y = synth.config_states(0, 777)
+    T, P, Y = synth.config_states(cfg, n)
     dT, dP, dY = dev(torch, T, P, Y)
     J = pj.eval_jacobian(dT, dP, dY)
-    Ypad = torch.full((777, m.n_species + 5), 7.0, dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        assert torch.equal(pj.eval_jacobian(dT, dP, dY), J)
+    Ypad = torch.full((n, m.n_species + 5), 7.0, dtype=torch.float64, device="cuda")
     Ypad[:, : m.n_species] = dY
     assert torch.equal(pj.eval_jacobian(dT, dP, Ypad), J)
+    cuts = (0, 1, n // 3 + 1, n)
     parts = [pj.eval_jacobian(dT[a:b].contiguous(), dP[a:b].contiguous(), dY[a:b].contiguous())
-             for a, b in ((0, 1), (1, 300), (300, 777))]
+             for a, b in zip(cuts[:-1], cuts[1:])]
     assert torch.equal(torch.cat(parts), J)
     s = torch.cuda.Stream()
     torch.cuda.synchronize()
@@ -635,19 +643,21 @@ def test_binding_rejects_bad_output_tensors(torch, PyJac):
 
 
 @pytest.mark.gpu
-def test_output_pointer_not_16_byte_aligned(torch, PyJac):
-    """An output pointer that is only 8-byte aligned takes the 8-byte store path; same numbers."""
-    m = synth.make_mechanism(0)
+@pytest.mark.parametrize("cfg,n", [(0, 257), (1, 301), (2, 100)])
+def test_output_pointer_not_16_byte_aligned(torch, PyJac, cfg, n):
+    """An output pointer that is only 8-byte aligned takes the 8-byte store path; same numbers (one and two
+    slabs of rows, one and two resident CTAs)."""
+    m = synth.make_mechanism(cfg)
     pj = PyJac(m)
-    T, P, Y = synth.config_states(0, 257)
+    T, P, Y = synth.config_states(cfg, n)
     dT, dP, dY = dev(torch, T, P, Y)
     J = pj.eval_jacobian(dT, dP, dY)
     ld = m.n_species + 1
-    buf = torch.zeros(257 * ld * ld + 1, dtype=torch.float64, device="cuda")
+    buf = torch.zeros(n * ld * ld + 1, dtype=torch.float64, device="cuda")
     view = buf[1:]
     assert view.data_ptr() % 16 == 8
     pj.eval_jacobian(dT, dP, dY, out=view)
-    assert torch.equal(view.reshape(257, ld * ld), J)
+    assert torch.equal(view.reshape(n, ld * ld), J)
     assert float(buf[0]) == 0.0
 
 
