@@ -409,6 +409,11 @@ def test_host_buffer_variant_matches_device_variant(torch, PyJac):
     (1, 301, dict(states_per_cta=2, cell_cap=2, list_cap=30)),
     (1, 301, dict(rows_per_lane=1)),                                                # one row per lane, 8-byte stores
     (1, 301, dict(p1_states=1)),                                      # one state per reaction work item
+    (1, 301, dict(p1_states=3)),                                      # all states in one item, every rate form
+    (1, 301, dict(p1_states=2 + 16 * 2)),                             # two per item, plain and general groups
+    (1, 301, dict(layout=2)),                                         # per-reaction terms in allocation order
+    (2, 65, dict(layout=2, p1_states=3)),
+    (3, 9, dict(layout=2)),
     (1, 301, dict(states_per_cta=6, threads=512, ctas_per_sm=1, p1_states=2)),   # pairs of states, constants in registers
     (1, 301, dict(states_per_cta=2, threads=512, ctas_per_sm=1, stage_tables=1)),  # gather tables staged in shared memory
     (0, 1024, dict(stage_tables=1)),

@@ -151,7 +151,8 @@ def test_binding_refuses_cpu_tensors():
 @pytest.mark.parametrize("shape", [
     None, dict(states_per_cta=1), dict(states_per_cta=2, ctas_per_sm=3, threads=160), dict(states_per_cta=6),
     dict(states_per_cta=4, ctas_per_sm=1), dict(states_per_cta=1, threads=64), dict(list_cap=6), dict(list_cap=64),
-    dict(cell_cap=1), dict(cell_cap=2, rows_per_lane=1),
+    dict(cell_cap=1), dict(cell_cap=2, rows_per_lane=1), dict(layout=2), dict(p1_states=1), dict(p1_states=3 + 16 * 1),
+    dict(states_per_cta=2, threads=512, ctas_per_sm=1, stage_tables=1),
 ])
 def test_pack_self_check_over_launch_shapes(shape):
     """pyjac_tools_pack_stats packs exactly as pyjac_mech_create_shaped does, including the self-check of
@@ -168,6 +169,22 @@ def test_pack_self_check_over_launch_shapes(shape):
         assert st["threads"] % 32 == 0 and st["threads"] >= 32 * st["states_per_cta"]
     for seed in range(4):
         binding.pack_stats(synth.make_tiny_mechanism(seed), shape)
+
+
+def test_layout_search_lowers_the_modelled_bank_conflicts():
+    """mech_pack.cu: the layout search of the per-reaction terms (indices traded within a store wavefront against
+    the gather groups) and the exact edge colouring of the gather steps.  Host-only model (shared-memory wavefronts
+    beyond one per lane group and step): the streaming phase must be nearly conflict-free and the capacity excess of
+    the gather groups must drop by more than half; with layout = 2 (allocation order) the excess is not computed."""
+    for cfg in (1, 2, 3):
+        m = synth.make_mechanism(cfg)
+        on, off = binding.pack_stats(m), binding.pack_stats(m, dict(layout=2))
+        assert on["layout_excess_before"] > 0 and 2 * on["layout_excess_after"] < on["layout_excess_before"]
+        assert off["layout_excess_before"] == 0 and off["layout_excess_after"] == 0
+        assert on["b_conflict_wf"] < off["b_conflict_wf"] and on["a_conflict_wf"] < off["a_conflict_wf"]
+        assert on["b_conflict_wf"] <= 0.02 * on["b_steps"] * 2
+        for k in ("e_elements", "cell_entries", "a_steps", "b_steps", "smem_bytes_per_cta"):
+            assert on[k] == off[k]                      # a permutation: nothing else changes
 
 
 def test_launch_shape_validation():
