@@ -57,6 +57,7 @@ extern "C" {
 #define PYJAC_ENOMEM (-2) /* host or device allocation failed */
 #define PYJAC_ECUDA (-3)  /* CUDA runtime / launch error (no device, wrong architecture, ...) */
 #define PYJAC_ELIMIT (-4) /* mechanism exceeds a table limit of this build (see pyjac_mech_create) */
+#define PYJAC_ESCRATCH (-5) /* batch too large for the built-in scratch array (pyjac_eval_jacobian_fd_static) */
 
 /* rxn_type: which case of Eq. 20 / which rate form applies */
 enum {
@@ -227,6 +228,36 @@ int pyjac_eval_jacobian_fd(const pyjac_mech *mech, int64_t n, const double *T, c
 /* Doubles of scratch pyjac_eval_jacobian_fd needs to evaluate `chunk_states` states at once
  * (-1 for an invalid argument). */
 int64_t pyjac_fd_workspace_doubles(const pyjac_mech *mech, int64_t chunk_states);
+
+/* pyjac_eval_jacobian_fd for callers that cannot allocate device memory and so have no `work` buffer to
+ * pass: a flow solver that gave the whole GPU to its own arena at start-up (any later cudaMalloc fails), an
+ * integrator callback inside a time-step loop where cudaMalloc / cudaFree would stall every stream of the
+ * device through their device-wide synchronisation, a plug-in whose host forbids driver allocations after
+ * initialisation.  Same operation, arguments, layout and numbers (bit for bit) as pyjac_eval_jacobian_fd
+ * (C21); the caller still owns T, P, Y and jac (DEVICE pointers).  The scratch is an
+ * array compiled into the library: 4 Mi doubles = 32 MiB of device memory, which every GPU that loads the
+ * library holds until the process exits whether or not this function is ever called.
+ *   - Limit: all n states of a call must fit the array at once, n <= pyjac_fd_static_max_states(mech)
+ *     (32 MiB / pyjac_fd_workspace_doubles(mech, 1) doubles: 712 states at 53 species, 166 at 111, 16 at 360).
+ *     A larger n, or a mechanism of which not even one state fits, returns PYJAC_ESCRATCH and enqueues
+ *     nothing; loop over sub-batches instead.  Other errors as pyjac_eval_jacobian_fd.
+ *   - The function and everything under it call no cudaMalloc, cudaFree or other allocating routine.
+ *   - The first call on each device looks the array's device address up (cudaGetSymbolAddress, with that
+ *     device made current for the moment); this is host-side set-up, possibly a module load.  Make that
+ *     first call early, before any stream capture is begun on the thread.  Later calls only enqueue the
+ *     four kernels on `stream`.
+ *   - There is ONE array per GPU, shared by every handle, stream and host thread.  Two calls whose kernels
+ *     can overlap on the GPU (different streams without an ordering between them, or two host threads)
+ *     race on it and produce garbage: order them on one stream or with events.  The array keeps whatever
+ *     the last call wrote; this path never reads a scratch word before writing it in the same call, so no
+ *     clearing is needed and stale contents cannot leak into a result. */
+int pyjac_eval_jacobian_fd_static(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
+                                  const double *Y, int64_t ldy, double rtol, double atol, double *jac,
+                                  void *stream);
+
+/* Largest n pyjac_eval_jacobian_fd_static accepts for this mechanism (0 if one state does not fit the
+ * 32 MiB array; -1 for an invalid handle). */
+int64_t pyjac_fd_static_max_states(const pyjac_mech *mech);
 
 /* Number of kernel launches this library has enqueued since it was loaded (all handles). */
 int64_t pyjac_kernel_launches(void);

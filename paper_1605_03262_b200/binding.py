@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpyjac_b200.so")
 TOOLS_LIB_PATH = os.path.join(_HERE, "libpyjac_b200_tools.so")     # include/pyjac_b200_tools.h: bench / test helpers
 
-PYJAC_OK, PYJAC_EINVAL, PYJAC_ENOMEM, PYJAC_ECUDA, PYJAC_ELIMIT = 0, -1, -2, -3, -4
+PYJAC_OK, PYJAC_EINVAL, PYJAC_ENOMEM, PYJAC_ECUDA, PYJAC_ELIMIT, PYJAC_ESCRATCH = 0, -1, -2, -3, -4, -5
 
 _pd = C.POINTER(C.c_double)
 _pi = C.POINTER(C.c_int32)
@@ -47,7 +47,8 @@ class LaunchShape(C.Structure):
 
 EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_sizes",
            "pyjac_eval_rates", "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
-           "pyjac_eval_dydt_host", "pyjac_eval_jvp", "pyjac_eval_jacobian_fd", "pyjac_fd_workspace_doubles", "pyjac_kernel_launches",
+           "pyjac_eval_dydt_host", "pyjac_eval_jvp", "pyjac_eval_jacobian_fd", "pyjac_fd_workspace_doubles",
+           "pyjac_eval_jacobian_fd_static", "pyjac_fd_static_max_states", "pyjac_kernel_launches",
            "pyjac_jacobian_launch_config", "pyjac_strerror")
 TOOLS_EXPORTS = ("pyjac_tools_pack_stats", "pyjac_tools_peak_store_stream", "pyjac_tools_peak_dfma")
 
@@ -79,13 +80,17 @@ def load_library(path: str | None = None):
     lib.pyjac_eval_jacobian_fd.argtypes = [vp, i64, vp, vp, vp, i64, C.c_double, C.c_double, vp, vp, i64, vp]
     lib.pyjac_fd_workspace_doubles.argtypes = [vp, i64]
     lib.pyjac_fd_workspace_doubles.restype = i64
+    lib.pyjac_eval_jacobian_fd_static.argtypes = [vp, i64, vp, vp, vp, i64, C.c_double, C.c_double, vp, vp]
+    lib.pyjac_fd_static_max_states.argtypes = [vp]
+    lib.pyjac_fd_static_max_states.restype = i64
     lib.pyjac_kernel_launches.argtypes = []
     lib.pyjac_kernel_launches.restype = i64
     lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 5
     lib.pyjac_strerror.argtypes = [C.c_int]
     lib.pyjac_strerror.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("pyjac_kernel_launches", "pyjac_strerror"):
+        if name not in ("pyjac_kernel_launches", "pyjac_strerror", "pyjac_fd_workspace_doubles",
+                        "pyjac_fd_static_max_states"):
             getattr(lib, name).restype = C.c_int
     if path is None:
         _lib = lib
@@ -322,6 +327,27 @@ class PyJac:
         _check(self.lib.pyjac_eval_jacobian_fd(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
                                                float(rtol), float(atol), out.data_ptr(), work.data_ptr(),
                                                int(work.numel()), self._stream()), "pyjac_eval_jacobian_fd")
+        return out
+
+    def fd_static_max_states(self) -> int:
+        """Largest batch eval_jacobian_fd_static takes for this mechanism (pyjac_fd_static_max_states)."""
+        return int(self.lib.pyjac_fd_static_max_states(self._h))
+
+    def eval_jacobian_fd_static(self, T, P, Y, out, rtol: float = 1e-8, atol: float = 1e-15):
+        """eval_jacobian_fd for callers that cannot allocate device memory (pyjac_eval_jacobian_fd_static): an
+        application whose own arena already owns the whole GPU, or a callback in a time-step loop that must not
+        trigger cudaMalloc's device-wide synchronisation.  The scratch is a 32 MiB array built into the library, so
+        `out` is required (nothing is allocated here either) and at most fd_static_max_states() states go in one
+        call; more raises PyJacError with code PYJAC_ESCRATCH.  One array per GPU is shared by all calls: keep calls
+        ordered on one stream.  The first call on a device does a one-time address lookup on the host."""
+        n, ldy = self._dev_inputs(T, P, Y)
+        ld = self.ns + 1
+        if out is None:
+            raise ValueError("eval_jacobian_fd_static allocates nothing: pass `out`")
+        out = self._dev_out(out, n, ld * ld, T)
+        _check(self.lib.pyjac_eval_jacobian_fd_static(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
+                                                      float(rtol), float(atol), out.data_ptr(), self._stream()),
+               "pyjac_eval_jacobian_fd_static")
         return out
 
     # ---- host-pointer calls (copies inside; synchronous)

@@ -286,6 +286,9 @@ const char *pyjac_strerror(int code)
         case PYJAC_ENOMEM: return "host or device allocation failed";
         case PYJAC_ECUDA: return "CUDA runtime or launch error";
         case PYJAC_ELIMIT: return "mechanism exceeds a table limit of this build";
+        case PYJAC_ESCRATCH:
+            return "the call needs more scratch than the library's built-in 32 MiB device array holds "
+                   "(pyjac_fd_static_max_states gives the largest batch)";
         default: return "unknown error code";
     }
 }

@@ -14,6 +14,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <mutex>
 
 #include "kernels.h"
 
@@ -121,6 +122,78 @@ int pyjac_eval_jacobian_fd(const pyjac_mech *m, int64_t n, const double *T, cons
     }
     if (prev != device) cudaSetDevice(prev);
     return result;
+}
+
+}  // extern "C"
+
+// ---- forward-difference Jacobian for callers that cannot allocate device memory -------------------------------
+//
+// pyjac_eval_jacobian_fd needs a caller-owned scratch buffer.  Some callers have no way to get one: a reacting-flow
+// solver that handed the whole GPU to its own arena at start-up (a later cudaMalloc simply fails), an integrator
+// callback that runs inside a time-step loop where cudaMalloc / cudaFree would stall every stream of the device
+// through their device-wide synchronisation, or a plug-in whose host application forbids driver allocations after
+// initialisation.  For them the scratch lives in the library image itself: a file-scope __device__ array of
+// kFdStaticDoubles doubles (32 MiB), which every GPU that loads this library holds from module load to process exit.
+//
+// `g_fd_static_scratch` below is two different things.  In device code it is the array.  In host code the name is only
+// a host-side shadow symbol: its host address is NOT device memory, and a kernel handed `g_fd_static_scratch` from
+// the host would fault (or, on a system where the GPU can reach host memory, silently use the wrong bytes).  The
+// host side therefore asks the runtime for the real device address, once per device, with that device current
+// (fd_static_device_ptr), and passes that pointer to the kernels.
+constexpr int64_t kFdStaticDoubles = (int64_t)4 << 20;        // 4 Mi doubles = 32 MiB per GPU
+constexpr int kFdStaticMaxDevices = 64;
+
+static __device__ __align__(256) double g_fd_static_scratch[kFdStaticDoubles];
+
+namespace {
+
+std::mutex g_fd_static_mutex;
+double *g_fd_static_ptr[kFdStaticMaxDevices] = {};           // device address of the array, per device (NULL: not asked yet)
+
+// Device address of g_fd_static_scratch on `device` (NULL on error).  The first call for a device makes that device
+// current, resolves the symbol (which loads this module on the device if it is not loaded yet) and restores the
+// caller's device; later calls return the cached pointer.
+double *fd_static_device_ptr(int device)
+{
+    if (device < 0 || device >= kFdStaticMaxDevices) return nullptr;
+    std::lock_guard<std::mutex> lock(g_fd_static_mutex);
+    if (g_fd_static_ptr[device]) return g_fd_static_ptr[device];
+    int prev = -1;
+    if (cudaGetDevice(&prev) != cudaSuccess) return nullptr;
+    if (prev != device && cudaSetDevice(device) != cudaSuccess) return nullptr;
+    double *ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_fd_static_scratch);
+    if (prev != device) cudaSetDevice(prev);
+    if (e != cudaSuccess || !ptr) return nullptr;
+    g_fd_static_ptr[device] = ptr;
+    return ptr;
+}
+
+}  // namespace
+
+extern "C" {
+
+int64_t pyjac_fd_static_max_states(const pyjac_mech *m)
+{
+    const int64_t per_state = pyjac_fd_workspace_doubles(m, 1);
+    if (per_state < 1) return -1;
+    return kFdStaticDoubles / per_state;
+}
+
+int pyjac_eval_jacobian_fd_static(const pyjac_mech *m, int64_t n, const double *T, const double *P, const double *Y,
+                                  int64_t ldy, double rtol, double atol, double *jac, void *stream)
+{
+    int32_t ns = 0;
+    if (pyjac_mech_sizes(m, &ns, nullptr) != PYJAC_OK || n < 0) return PYJAC_EINVAL;
+    if (n == 0) return PYJAC_OK;
+    // one chunk only: the states of a call must fit the array together, the caller loops over larger batches
+    if (n > pyjac_fd_static_max_states(m)) return PYJAC_ESCRATCH;
+    double *scratch = fd_static_device_ptr(pyjac::mech_device(m));
+    if (!scratch) return PYJAC_ECUDA;
+    // Every scratch word a kernel of this path reads has been written earlier in the same call (f0 and f1 by the
+    // source-term launches, the increments and perturbed states by fd_perturb_kernel), so what the previous call
+    // left in the array is never seen and nothing has to be cleared.
+    return pyjac_eval_jacobian_fd(m, n, T, P, Y, ldy, rtol, atol, jac, scratch, kFdStaticDoubles, stream);
 }
 
 }  // extern "C"
