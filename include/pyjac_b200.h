@@ -132,7 +132,7 @@ int pyjac_mech_create(const pyjac_mech_desc *host_desc, int device, pyjac_mech *
  * reaction products stay in shared memory instead). */
 typedef struct pyjac_launch_shape {
     int32_t states_per_cta; /* 1, 2, 3, 4 or 6 */
-    int32_t threads;        /* per CTA: a multiple of 32, at least 32 * states_per_cta, at most 512 */
+    int32_t threads;        /* per CTA: a multiple of 32, at least 64 and 32 * states_per_cta, at most 512 */
     int32_t ctas_per_sm;    /* resident CTAs the shared-memory footprint is sized for, 1..4 */
     int32_t list_cap;       /* longest list one lane sums in the per-species / per-column phase; longer
                                lists are shared by 2, 4, .. lanes and combined by warp shuffles */
@@ -152,7 +152,9 @@ typedef struct pyjac_launch_shape {
 
 /* As pyjac_mech_create with an explicit launch shape (tuning and tests; `shape` may be NULL).
  * Every shape evaluates the same numbers up to the order of a sum.  PYJAC_EINVAL for a value out
- * of range, PYJAC_ELIMIT if the shape does not fit the shared memory of one SM. */
+ * of range -- explicit values are never adjusted: too few threads for states_per_cta, rows_per_lane = 2
+ * with an even N_sp or a negative field are errors -- PYJAC_ELIMIT if the shape does not fit the shared
+ * memory of one SM. */
 int pyjac_mech_create_shaped(const pyjac_mech_desc *host_desc, int device,
                              const pyjac_launch_shape *shape, pyjac_mech **out);
 
@@ -200,15 +202,22 @@ int pyjac_eval_jvp(const pyjac_mech *mech, int64_t n, const double *T, const dou
 /* Host-buffer variants: T, P, Y and the output are HOST pointers (pinned memory makes the copies
  * asynchronous; pageable memory works but serialises them).  The call copies the inputs to the
  * device, runs the same kernels as above in chunks of at most `chunk_states` states (<= 0: a
- * default sized to the device's free memory), copies the result back with copies of one chunk
- * overlapping the evaluation of the next, and returns after the last byte has arrived.  The two
- * device staging buffers and the two streams are kept with the handle and reused by later calls
- * (grown when a call needs more; freed by pyjac_mech_destroy); a second thread that calls while
- * they are in use gets temporary ones. */
+ * default whose output buffer is at most 512 MiB and a quarter of the device's free memory), copies
+ * the result back with copies of one chunk overlapping the evaluation of the next, and returns after
+ * the last byte has arrived.  The two device staging buffer pairs and the two streams are kept with
+ * the handle and reused by later calls (grown when a call needs more): with the default chunk that is
+ * up to ~1.1 GiB of device memory per handle, held until pyjac_mech_trim or pyjac_mech_destroy.  A
+ * call whose explicit `chunk_states` needs a buffer above 512 MiB, and a second thread that calls
+ * while the kept buffers are in use, stage through temporary buffers freed before the call returns. */
 int pyjac_eval_jacobian_host(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
                              const double *Y, int64_t ldy, double *jac, int64_t chunk_states);
 int pyjac_eval_dydt_host(const pyjac_mech *mech, int64_t n, const double *T, const double *P,
                          const double *Y, int64_t ldy, double *dydt, int64_t chunk_states);
+
+/* Frees the staging buffers the *_host calls left with the handle (no-op returning PYJAC_OK when there
+ * are none or while a *_host call is using them).  The handle stays usable; the next *_host call
+ * allocates again. */
+int pyjac_mech_trim(pyjac_mech *mech);
 
 /* First-order forward-difference Jacobian from the source term (the paper's own comparison: "a simple
  * first-order forward difference adapted from CVODE", Tables 4-5), in
@@ -216,7 +225,9 @@ int pyjac_eval_dydt_host(const pyjac_mech *mech, int64_t n, const double *T, con
  *   w_j = 1 / (rtol |Phi_j| + atol),  D_j = max(sqrt(eps) |Phi_j|, sqrt(eps) / w_j),
  *   J(:, j) = (f(Phi + D_j e_j) - f(Phi)) / D_j
  * (CVODE's rule with its step-dependent floor 1000 |h| eps N |f| replaced by sqrt(eps): DESIGN.md C21),
- * a mass-fraction increment being taken from Y_Nsp (Eq. 2); column N_sp is zero.  rtol > 0, atol >= 0.
+ * a mass-fraction increment being taken from Y_Nsp (Eq. 2); column N_sp is zero.  rtol > 0 and atol > 0
+ * (PYJAC_EINVAL otherwise: with atol = 0 an unknown that is exactly zero, as absent species are, would get
+ * D_j = 0 and a column of 0/0).
  * All pointers are DEVICE pointers.  `work` is caller-owned scratch of `work_doubles` doubles; the
  * states are evaluated in chunks of work_doubles / pyjac_fd_workspace_doubles(mech, 1) states
  * (PYJAC_EINVAL if that is zero): 1 + N_sp source-term evaluations per state, 4 kernel launches

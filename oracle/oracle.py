@@ -143,7 +143,10 @@ class Oracle:
 
     def jacobian_fd(self, T, P, Y, rtol: float = 1e-8, atol: float = 1e-15):
         """First-order forward-difference Jacobian of the oracle's source term with the increments of
-        DESIGN.md reading C21 (the paper's comparison method): [n][(ns+1)^2]."""
+        DESIGN.md reading C21 (the paper's comparison method): [n][(ns+1)^2].  rtol and atol must
+        be positive: with atol = 0 an unknown that is exactly zero gets the increment D_j = 0 (C21)."""
+        if not (rtol > 0.0 and atol > 0.0):
+            raise ValueError("jacobian_fd needs rtol > 0 and atol > 0 (DESIGN.md C21: D_j = 0 for a zero unknown otherwise)")
         T, P, Y = self._state(T, P, Y)
         n = T.shape[0]
         ld = self.ns + 1

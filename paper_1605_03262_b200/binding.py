@@ -45,7 +45,7 @@ class LaunchShape(C.Structure):
                 ("p1_states", C.c_int32), ("stage_tables", C.c_int32), ("layout", C.c_int32)]
 
 
-EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_sizes",
+EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_trim", "pyjac_mech_sizes",
            "pyjac_eval_rates", "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
            "pyjac_eval_dydt_host", "pyjac_eval_jvp", "pyjac_eval_jacobian_fd", "pyjac_fd_workspace_doubles",
            "pyjac_eval_jacobian_fd_static", "pyjac_fd_static_max_states", "pyjac_kernel_launches",
@@ -70,6 +70,7 @@ def load_library(path: str | None = None):
     lib.pyjac_mech_create.argtypes = [C.POINTER(MechDesc), C.c_int, C.POINTER(vp)]
     lib.pyjac_mech_create_shaped.argtypes = [C.POINTER(MechDesc), C.c_int, C.POINTER(LaunchShape), C.POINTER(vp)]
     lib.pyjac_mech_destroy.argtypes = [vp]
+    lib.pyjac_mech_trim.argtypes = [vp]
     lib.pyjac_mech_sizes.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     lib.pyjac_eval_rates.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, vp]
     lib.pyjac_eval_dydt.argtypes = [vp, i64, vp, vp, vp, i64, vp, vp]
@@ -259,15 +260,21 @@ class PyJac:
         return out
 
     # ---- device-pointer calls (enqueue on torch's current stream)
-    def eval_rates(self, T, P, Y, want=("rf", "rr", "cmod", "wdot")):
-        """dict of float64 CUDA tensors rf, rr, cmod [n][Nreac], wdot [n][Nsp] (pyjac_eval_rates)."""
+    def eval_rates(self, T, P, Y, want=("rf", "rr", "cmod", "wdot"), out=None):
+        """dict of float64 CUDA tensors rf, rr, cmod [n][Nreac], wdot [n][Nsp] (pyjac_eval_rates).  `out`: a dict of
+        caller-owned tensors to write in place (its keys are the outputs wanted; nothing is allocated then)."""
         import torch
         n, ldy = self._dev_inputs(T, P, Y)
-        out = {}
-        for name in ("rf", "rr", "cmod", "wdot"):
-            if name in want:
-                out[name] = torch.empty((n, self.ns if name == "wdot" else self.nr),
-                                        dtype=torch.float64, device=T.device)
+        if out is not None:
+            if set(out) - {"rf", "rr", "cmod", "wdot"}:
+                raise ValueError("unknown rate outputs: %s" % sorted(set(out) - {"rf", "rr", "cmod", "wdot"}))
+            out = {k: self._dev_out(v, n, self.ns if k == "wdot" else self.nr, T) for k, v in out.items()}
+        else:
+            out = {}
+            for name in ("rf", "rr", "cmod", "wdot"):
+                if name in want:
+                    out[name] = torch.empty((n, self.ns if name == "wdot" else self.nr),
+                                            dtype=torch.float64, device=T.device)
         ptr = lambda k: C.c_void_p(out[k].data_ptr()) if k in out else None
         _check(self.lib.pyjac_eval_rates(self._h, n, T.data_ptr(), P.data_ptr(), Y.data_ptr(), ldy,
                                          ptr("rf"), ptr("rr"), ptr("cmod"), ptr("wdot"),
@@ -396,6 +403,10 @@ class PyJac:
     def eval_dydt_host(self, T, P, Y, out, chunk_states: int = 0):
         return self._host_call(self.lib.pyjac_eval_dydt_host, "pyjac_eval_dydt_host", T, P, Y, out, self.ns + 1,
                                chunk_states)
+
+    def trim(self):
+        """Frees the device staging buffers the *_host calls keep with the handle (pyjac_mech_trim)."""
+        _check(self.lib.pyjac_mech_trim(self._h), "pyjac_mech_trim")
 
     def launch_config(self, n: int):
         v = [C.c_int32() for _ in range(5)]

@@ -5,7 +5,10 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "device_mech.h"
@@ -37,6 +40,10 @@ struct pyjac_mech {
 namespace {
 
 std::atomic<long long> g_launches{0};
+
+// preferred shared-memory carve-out (percent) set so far per (device, kernel function); see pyjac_mech_create_shaped
+std::mutex g_carveout_mutex;
+std::map<std::pair<int, const void *>, int> g_carveout;
 
 struct Uploader {
     std::vector<unsigned char> host;
@@ -83,6 +90,7 @@ int launch(const pyjac_mech *m, int level, int64_t n, const double *T, const dou
 namespace pyjac {
 void count_launches(int k) { g_launches.fetch_add(k, std::memory_order_relaxed); }
 int mech_device(const pyjac_mech *m) { return m->device; }
+int mech_sm_count(const pyjac_mech *m) { return m->n_sm; }
 }  // namespace pyjac
 
 extern "C" {
@@ -170,9 +178,16 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
             // stays L1 (the gather tables are re-read from L1 / L2 by every CTA iteration)
             int carveout = (int)((100 * ((long long)hp.ctas_target * (long long)(bytes + 1024 + 16)) + 228 * 1024 - 1) / (228 * 1024));
             carveout = carveout > 100 ? 100 : carveout < 0 ? 0 : carveout;
+            // The kernel functions are shared by every handle of this (S, stage): the carve-out of a function is
+            // the LARGEST any handle on this device has asked for so far and is never lowered, so a handle made
+            // later cannot take shared memory (and with it resident CTAs) away from an earlier one whose grid was
+            // sized at its own creation; an earlier handle may at most find more CTAs resident than it counted.
+            std::lock_guard<std::mutex> lock(g_carveout_mutex);
             for (int level = 0; level < 4 && rc == PYJAC_OK; ++level) {
                 m->smem[level] = bytes;
                 const void *k = eval_kernel_ptr(level, m->S, hp.stage);
+                int &set = g_carveout[{device, k}];
+                if (carveout < set) carveout = set;
                 // the kernel function is shared by every handle of this shape: its dynamic shared-memory limit
                 // is raised to what the device allows, once and for all, never to one handle's size
                 cudaFuncAttributes fa{};
@@ -184,6 +199,8 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
                         cudaSuccess ||
                     m->ctas_per_sm[level] < 1)
                     rc = PYJAC_ECUDA;
+                else
+                    set = carveout;
             }
         }
     }
@@ -212,6 +229,24 @@ int pyjac_mech_destroy(pyjac_mech *m)
     }
     if (prev >= 0) cudaSetDevice(prev);
     delete m;
+    return e == cudaSuccess ? PYJAC_OK : PYJAC_ECUDA;
+}
+
+int pyjac_mech_trim(pyjac_mech *m)
+{
+    if (!m) return PYJAC_EINVAL;
+    if (m->ws_busy.test_and_set(std::memory_order_acquire)) return PYJAC_OK;      // a *_host call is using them: keep
+    int prev = -1;
+    cudaGetDevice(&prev);
+    cudaError_t e = cudaSetDevice(m->device);
+    for (int b = 0; b < 2 && e == cudaSuccess; ++b) {
+        if (m->ws_in[b] && cudaFree(m->ws_in[b]) != cudaSuccess) e = cudaErrorUnknown;
+        if (m->ws_out[b] && cudaFree(m->ws_out[b]) != cudaSuccess) e = cudaErrorUnknown;
+        m->ws_in[b] = m->ws_out[b] = nullptr;
+    }
+    m->ws_in_cap = m->ws_out_cap = 0;
+    if (prev >= 0) cudaSetDevice(prev);
+    m->ws_busy.clear(std::memory_order_release);
     return e == cudaSuccess ? PYJAC_OK : PYJAC_ECUDA;
 }
 
@@ -298,6 +333,10 @@ const char *pyjac_strerror(int code)
 // ---- host-buffer variants: chunked, double-buffered H2D -> kernel -> D2H ---------------------------
 namespace {
 
+// largest staging buffer a handle keeps between *_host calls (two input and two output buffers: at most four times this,
+// in practice ~2.1x because the inputs are small), and the size of the default chunk's output buffer
+constexpr size_t kStageCacheBytes = (size_t)512 << 20;
+
 int eval_host(const pyjac_mech *m, int level, int64_t n, const double *T, const double *P, const double *Y,
               int64_t ldy, double *outp, int64_t chunk_states)
 {
@@ -315,7 +354,9 @@ int eval_host(const pyjac_mech *m, int level, int64_t n, const double *T, const 
         if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaSetDevice(prev); return PYJAC_ECUDA; }
         const size_t per_state = (out_per + in_per) * sizeof(double) * 2;   // two buffers
         size_t c = (free_b / 4) / per_state;
-        const size_t want = (size_t)1 << 15;       // copies of ~0.1-1 GB overlap well; more adds nothing
+        // by bytes, not by states: one output buffer of at most kStageCacheBytes (copies of that size already
+        // overlap well; a 360-species Jacobian is 1 MB per state), so that what the handle keeps stays ~1 GiB
+        const size_t want = kStageCacheBytes / ((out_per > in_per ? out_per : in_per) * sizeof(double));
         if (c > want) c = want;
         if (c < 1) c = 1;
         chunk_states = (int64_t)c;
@@ -326,7 +367,10 @@ int eval_host(const pyjac_mech *m, int level, int64_t n, const double *T, const 
     cudaStream_t st[2] = {nullptr, nullptr};
     rc = PYJAC_OK;
     // the handle's staging buffers if nobody else is using them (grown on demand), else temporary ones
-    const bool cached = !m->ws_busy.test_and_set(std::memory_order_acquire);
+    // ... and only if the buffers are small enough to keep: a caller's explicit chunk beyond kStageCacheBytes per
+    // buffer is staged through temporary buffers that are freed before the call returns
+    const bool keepable = C * out_per * sizeof(double) <= kStageCacheBytes && C * in_per * sizeof(double) <= kStageCacheBytes;
+    const bool cached = keepable && !m->ws_busy.test_and_set(std::memory_order_acquire);
     if (cached) {
         for (int b = 0; b < 2 && rc == PYJAC_OK; ++b)
             if (!m->ws_stream[b] && cudaStreamCreateWithFlags(&m->ws_stream[b], cudaStreamNonBlocking) != cudaSuccess)

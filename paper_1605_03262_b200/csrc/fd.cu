@@ -88,7 +88,7 @@ int pyjac_eval_jacobian_fd(const pyjac_mech *m, int64_t n, const double *T, cons
     int32_t ns = 0;
     if (pyjac_mech_sizes(m, &ns, nullptr) != PYJAC_OK || n < 0) return PYJAC_EINVAL;
     if (n == 0) return PYJAC_OK;
-    if (!T || !P || !Y || !jac || !work || ldy < ns || !(rtol > 0.0) || !(atol >= 0.0)) return PYJAC_EINVAL;
+    if (!T || !P || !Y || !jac || !work || ldy < ns || !(rtol > 0.0) || !(atol > 0.0)) return PYJAC_EINVAL;
     const int64_t per_state = pyjac_fd_workspace_doubles(m, 1);
     int64_t chunk = work_doubles / per_state;
     if (chunk < 1) return PYJAC_EINVAL;
@@ -102,6 +102,7 @@ int pyjac_eval_jacobian_fd(const pyjac_mech *m, int64_t n, const double *T, cons
     if (cudaGetDevice(&prev) != cudaSuccess) return PYJAC_ECUDA;
     if (prev != device && cudaSetDevice(device) != cudaSuccess) return PYJAC_ECUDA;
     int result = PYJAC_OK;
+    const long long max_blocks = (long long)pyjac::mech_sm_count(m) * 16;      // grid-stride loop: 16 CTAs of 256 per SM
     for (int64_t s0 = 0; s0 < n && result == PYJAC_OK; s0 += chunk) {
         const int64_t c = n - s0 < chunk ? n - s0 : chunk;
         int rc = pyjac_eval_dydt(m, c, T + s0, P + s0, Y + s0 * ldy, ldy, f0, stream);
@@ -115,7 +116,7 @@ int pyjac_eval_jacobian_fd(const pyjac_mech *m, int64_t n, const double *T, cons
         if (rc != PYJAC_OK) { result = rc; break; }
         const long long total = (long long)c * ld * ld;
         const long long blocks = (total + 255) / 256;
-        fd_difference_kernel<<<(unsigned)(blocks < 148 * 16 ? blocks : 148 * 16), 256, 0, st>>>(
+        fd_difference_kernel<<<(unsigned)(blocks < max_blocks ? blocks : max_blocks), 256, 0, st>>>(
             ns, c, f0, f1, inc, jac + s0 * ld * ld);
         if (cudaGetLastError() != cudaSuccess) { result = PYJAC_ECUDA; break; }
         pyjac::count_launches(1);

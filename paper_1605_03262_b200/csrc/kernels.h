@@ -29,5 +29,7 @@ cudaError_t launch_eval(int level, int threads, int S, const DeviceMech &m, cons
 void count_launches(int k);
 // the device a handle's tables live on
 int mech_device(const pyjac_mech *m);
+// ... and the number of SMs of that device
+int mech_sm_count(const pyjac_mech *m);
 
 }  // namespace pyjac

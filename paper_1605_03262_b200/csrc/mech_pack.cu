@@ -610,6 +610,10 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         // measured on B200 (profiles/r2_shape_sweeps.md): with one state per CTA (the 360-species mechanism)
         // 384 threads beat 512 (1.55 M against 1.40 M states/s): fewer warps share the one-state queue tails
         int threads = hints.threads > 0 ? hints.threads : S == 1 && ctas == 1 ? 384 : (kMaxThreads / ctas) & ~31;
+        // an explicit value outside the contract is an error (a sweep must not record a shape that never ran);
+        // only the library's own choice is raised to the minimum
+        if (hints.threads < 0 || (hints.threads > 0 && (threads < 32 * S || threads < 64)))
+            throw Fail{PYJAC_EINVAL, "threads per CTA must be at least 64 and 32 per interleaved state"};
         if (threads < 32 * S) threads = 32 * S;
         if (threads < 64) threads = 64;
         if (threads > kMaxThreads || threads % 32) throw Fail{PYJAC_EINVAL, "threads per CTA must be a multiple of 32 up to kMaxThreads"};
@@ -618,8 +622,10 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
             throw Fail{PYJAC_ELIMIT, "per-CTA tables exceed the 256 KB offset range of a gather entry"};
     }
     const int S = o.S, NW = o.threads / 32;
+    if (hints.rp == 2 && ld % 2 != 0)
+        throw Fail{PYJAC_EINVAL, "two rows per lane need an odd number of species (even leading dimension)"};
+    if (hints.p1_states < 0) throw Fail{PYJAC_EINVAL, "p1_states must not be negative"};
     o.rp = (hints.rp == 1 || hints.rp == 2) ? hints.rp : (ld % 2 == 0 ? 2 : 1);
-    if (ld % 2 != 0) o.rp = 1;
     const int rp = o.rp;
     o.n_slab = (ld + 32 * rp - 1) / (32 * rp);
 

@@ -231,10 +231,26 @@ def test_config_prefix(torch, PyJac, cfg, n):
 
 
 # ---------------------------------------------------------------------------------- full sizes
-@pytest.mark.parametrize("cfg,chunk,n_sample", [(1, 100_000, 96), (2, 100_000, 32), (3, 8192, 6)])
+def named_states(n, S, grid):
+    """States of a launch of n states worth looking at by name (the kernel is a persistent grid-stride loop over
+    batches of S consecutive states, CTA c taking batches c, c + grid, ..; it rotates two mixture blocks and
+    prefetches the next batch while the current one runs): every state of the first three and last three batches
+    of the first and of the last CTA -- both parities of the rotating blocks, the prologue without a predecessor
+    and the epilogue without a successor -- and the ragged last batch of the launch."""
+    nb = (n + S - 1) // S
+    batches = {nb - 1}
+    for cta in {0, min(grid, nb) - 1}:
+        it = list(range(cta, nb, grid))
+        batches.update(it[:3] + it[-3:])
+    return np.array(sorted({s for b in batches for s in range(b * S, min(n, (b + 1) * S))}))
+
+
+@pytest.mark.parametrize("cfg,chunk,n_sample", [(1, 100_000, 8192), (2, 100_000, 2048), (3, 8192, 64)])
 def test_config_full_size_sampled(torch, PyJac, cfg, chunk, n_sample):
     """BASELINE.json's full state counts in the launch configuration bench.py times (one launch per
-    chunk); sampled states against the oracle, invariants on every state."""
+    chunk); sampled states against the oracle -- the named ones of `named_states` plus uniform draws up to
+    n_sample per launch (8,192 / 2,048 / 4 x 64 states: about a second of oracle time each on the box's cores) --
+    and invariants on every state."""
     m = synth.make_mechanism(cfg)
     o, pj = Oracle(m), PyJac(m)
     T, P, Y = synth.config_states(cfg)
@@ -253,7 +269,12 @@ def test_config_full_size_sampled(torch, PyJac, cfg, chunk, n_sample):
         resid = sp.sum(dim=2).abs().amax(dim=1)
         scale = sp.abs().amax(dim=1).sum(dim=1)
         assert bool((resid <= 1e-12 * scale).all())
-        pick = np.sort(rng.choice(s1 - s0, size=min(n_sample, s1 - s0), replace=False))
+        lc = pj.launch_config(s1 - s0)
+        named = named_states(s1 - s0, lc["states_per_cta"], lc["grid"])
+        assert len(named) <= 13 * lc["states_per_cta"] and named[-1] == s1 - s0 - 1 and named[0] == 0
+        drawn = rng.choice(s1 - s0, size=min(n_sample, s1 - s0), replace=False)
+        pick = np.unique(np.concatenate([named, drawn]))[: max(n_sample, len(named))]
+        pick = np.unique(np.concatenate([named, pick]))
         Jr = o.jacobian(T[s0:s1][pick], P[s0:s1][pick], Y[s0:s1][pick])
         Jg = J.reshape(-1, ld * ld)[torch.from_numpy(pick).cuda()].cpu().numpy()
         assert_jacobian(Jg, Jr, ns, label="cfg%d_full_sampled" % cfg)
@@ -397,6 +418,33 @@ def test_host_buffer_variant_matches_device_variant(torch, PyJac):
     assert pj.kernel_launches() == before + 1
 
 
+def test_host_variant_keeps_a_bounded_footprint_and_trim_returns_it(torch, PyJac):
+    """the staging buffers a *_host call leaves with the handle are capped by bytes (one output buffer
+    of at most 512 MiB, ~1.1 GiB in all), an explicit larger chunk goes through temporary buffers, and
+    pyjac_mech_trim gives the kept ones back.  111 species: 100,352 B per state, 5,349 states per default chunk."""
+    m = synth.make_mechanism(2)
+    pj = PyJac(m)
+    ld = m.n_species + 1
+    n = 6000
+    T, P, Y = synth.config_states(2, n)
+    dT, dP, dY = dev(torch, T, P, Y)
+    J = pj.eval_jacobian(dT, dP, dY).cpu().numpy()
+    torch.cuda.synchronize()
+    out = np.empty((n, ld * ld))
+    free0 = torch.cuda.mem_get_info()[0]
+    pj.eval_jacobian_host(T, P, Y, out)                            # default chunk: two chunks, buffers kept
+    assert np.array_equal(out, J)
+    kept = free0 - torch.cuda.mem_get_info()[0]
+    assert (512 << 20) <= kept <= int(1.2 * (1 << 30)), kept
+    pj.trim()
+    assert free0 - torch.cuda.mem_get_info()[0] < (64 << 20)       # the streams' few KB may stay
+    out[:] = 0.0
+    pj.eval_jacobian_host(T, P, Y, out, chunk_states=n)            # 602 MB per output buffer: above the cap, not kept
+    assert np.array_equal(out, J)
+    assert free0 - torch.cuda.mem_get_info()[0] < (64 << 20)
+    pj.trim()                                                      # nothing to free: still fine
+
+
 # ---------------------------------------------------------------------------------- launch shapes
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg,n,shape", [
@@ -414,6 +462,8 @@ def test_host_buffer_variant_matches_device_variant(torch, PyJac):
     (1, 301, dict(layout=2)),                                         # per-reaction terms in allocation order
     (2, 65, dict(layout=2, p1_states=3)),
     (3, 9, dict(layout=2)),
+    (3, 211, dict(threads=512)),                                      # 360 species, one state per CTA: read-ahead paths over
+                                                                      # two grid-stride iterations and a ragged last one
     (1, 301, dict(states_per_cta=6, threads=512, ctas_per_sm=1, p1_states=2)),   # pairs of states, constants in registers
     (1, 301, dict(states_per_cta=2, threads=512, ctas_per_sm=1, stage_tables=1)),  # gather tables staged in shared memory
     (0, 1024, dict(stage_tables=1)),
@@ -566,6 +616,18 @@ def test_fd_jacobian_argument_errors(torch, PyJac):
         pj.eval_jacobian_fd(dT, dP, dY, work=torch.empty(8, dtype=torch.float64, device="cuda"))
     with pytest.raises(PyJacError):
         pj.eval_jacobian_fd(dT, dP, dY, rtol=0.0)
+    with pytest.raises(PyJacError):       # atol = 0 would give an absent species the increment 0 and a column of 0/0
+        pj.eval_jacobian_fd(dT, dP, dY, atol=0.0)
+    Y0 = Y.copy()
+    Y0[:, -1] += Y0[:, 2]
+    Y0[:, 2] = 0.0                        # an unknown that is exactly zero: finite with the smallest positive atol in use
+    J0 = pj.eval_jacobian_fd(dT, dP, torch.from_numpy(Y0).cuda(), atol=1e-15).cpu().numpy()
+    Jr0 = Oracle(m).jacobian_fd(T, P, Y0, atol=1e-15)
+    assert np.all(np.isfinite(J0)) and np.all(np.isfinite(Jr0))
+    # (the zero unknown's column is a quotient of rounding noise by 1.5e-23 on both sides: only finiteness is
+    # asserted there; the temperature column has a sane increment and must agree)
+    ld = m.n_species + 1
+    assert np.allclose(J0[:, :ld], Jr0[:, :ld], rtol=1e-6, atol=1e-6 * np.abs(Jr0[:, :ld]).max())
     assert pj.fd_workspace_doubles(0) == -1
     l0 = pj.kernel_launches()
     pj.eval_jacobian_fd(dT, dP, dY, chunk_states=4)

@@ -190,10 +190,17 @@ def test_layout_search_lowers_the_modelled_bank_conflicts():
 def test_launch_shape_validation():
     m = synth.make_mechanism(0)
     for bad in (dict(states_per_cta=5), dict(threads=100), dict(threads=1024), dict(ctas_per_sm=9),
-                dict(cell_cap=4), dict(rows_per_lane=3), dict(states_per_cta=-1)):
+                dict(cell_cap=4), dict(rows_per_lane=3), dict(states_per_cta=-1),
+                # explicit values are never adjusted: too few threads for the interleaved states,
+                # fewer than two warps, a negative field
+                dict(states_per_cta=3, threads=64), dict(threads=32), dict(p1_states=-1), dict(threads=-32)):
         with pytest.raises(binding.PyJacError) as e:
             binding.pack_stats(m, bad)
         assert e.value.code == binding.PYJAC_EINVAL
+    with pytest.raises(binding.PyJacError) as e:       # two rows per lane need an even leading dimension: 360 species is even
+        binding.pack_stats(synth.make_mechanism(3), dict(rows_per_lane=2))
+    assert e.value.code == binding.PYJAC_EINVAL
+    assert binding.pack_stats(m, dict(rows_per_lane=2, threads=64, states_per_cta=2))["threads"] == 64
     with pytest.raises(ValueError):
         binding.launch_shape(dict(no_such_field=1))
 

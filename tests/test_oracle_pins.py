@@ -593,6 +593,14 @@ def test_fd_jacobian_approximates_the_derivative(tiny_mechs):
     # quotient would be the unconstrained partial derivative, which differs at first order
     m = tiny_mechs[0]
     o = Oracle(m)
+    # C21: atol = 0 would give an absent species the increment 0 (a column of 0/0): refused; with atol > 0 a
+    # state with a zero mass fraction has a finite forward difference
+    with pytest.raises(ValueError):
+        o.jacobian_fd(*synth.make_states(m.n_species, 2, 1), atol=0.0)
+    Tz, Pz, Yz = synth.make_states(m.n_species, 3, 35)
+    Yz[:, -1] += Yz[:, 0]
+    Yz[:, 0] = 0.0
+    assert np.all(np.isfinite(o.jacobian_fd(Tz, Pz, Yz, atol=1e-15)))
     ns = m.n_species
     T, P, Y = synth.make_states(ns, 4, 34)
     Jf = as_matrix(o.jacobian_fd(T, P, Y, rtol=1e-8, atol=1e-12), ns)
