@@ -4,7 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
                     [--also 2,3] [--sweep short|full|off] [--no-cpu-baseline] [--no-e2e] [--peaks]
     python bench.py --ncu-target CFG:KERNEL:N[:SHAPE]      # the short command the ncu captures of profiles/ wrap
-    python bench.py --ncu-import REPORT --ncu-label WORKLOAD:KERNEL:N    # one row of profiles/r2_ncu_counters.csv
+    python bench.py --ncu-import REPORT --ncu-label WORKLOAD:KERNEL:N    # one row of profiles/r3_ncu_counters.csv
 
 A "step" is one pass of the whole hot path (thermo -> rates -> source term -> Jacobian -> store;
 SURVEY.md section 8(a) rows S0-S10, one kernel launch) over one batch of seeded synthetic states.
@@ -37,7 +37,7 @@ CPU_SAMPLE = {0: 1024, 1: 8192, 2: 2048, 3: 256}
 # Counters of the committed `ncu` captures (profiles/r2_ncu_counters.csv, written from the reports the .md
 # beside it names): DRAM bytes and fp64 flops per state of each kernel.  They describe the kernels whose
 # source hash they carry; with different sources the bench reports null instead of a stale number.
-NCU_COUNTERS = os.path.join(ROOT, "profiles", "r2_ncu_counters.csv")
+NCU_COUNTERS = [os.path.join(ROOT, "profiles", f) for f in ("r3_ncu_counters.csv", "r2_ncu_counters.csv")]
 KERNEL_SOURCES = ("kernels.cu", "mech_pack.cu", "device_mech.h", "api.cu", "dispatch.cu")
 FP64_PEAK_TFLOPS = 33.74        # measured: bench.py --peaks, profiles/r1_machine_peaks.md (8 FMA chains per thread)
 
@@ -58,22 +58,55 @@ def ncu_counters():
     out, src = {}, None
     try:
         sha = kernel_source_sha16()
-        for row in csv.DictReader(open(NCU_COUNTERS)):
-            if row["kernel_source_sha16"] != sha:
-                src = "profiles/r2_ncu_counters.csv describes other kernel sources (%s)" % row["kernel_source_sha16"]
+        for path in NCU_COUNTERS:
+            if not os.path.exists(path) or out:
                 continue
-            out.setdefault(row["workload"], {})[row["kernel"]] = {
-                "dram_bytes_per_state": float(row["dram_bytes_per_state"]),
-                "fp64_flop_per_state": float(row["fp64_flop_per_state"]),
-                "lsu_wavefronts_per_state": float(row["lsu_wavefronts_per_state"])}
-            src = "profiles/r2_ncu_counters.csv (ncu --set full captures of kernel sources %s, profiles/r2_ncu_counters.md)" % sha
+            rel = os.path.relpath(path, ROOT)
+            for row in csv.DictReader(open(path)):
+                if row["kernel_source_sha16"] != sha:
+                    src = src or "%s describes other kernel sources (%s)" % (rel, row["kernel_source_sha16"])
+                    continue
+                out.setdefault(row["workload"], {})[row["kernel"]] = {
+                    "dram_bytes_per_state": float(row["dram_bytes_per_state"]),
+                    "fp64_flop_per_state": float(row["fp64_flop_per_state"]), "n_states": int(row["n_states"]),
+                    "lsu_wavefronts_per_state": float(row["lsu_wavefronts_per_state"])}
+                src = "%s (ncu --set full captures of kernel sources %s, %s)" % (rel, sha, rel[:-4] + ".md")
     except Exception:
         return {}, None
     return out, src
 
 
+_FP64_PEAK = {"tflops": FP64_PEAK_TFLOPS,
+              "source": "round-1 measurement (bench.py --peaks, profiles/r1_machine_peaks.md), not re-measured in this run"}
+
+
 def fp64_peak():
-    return FP64_PEAK_TFLOPS
+    return _FP64_PEAK["tflops"]
+
+
+def measure_fp64_peak(torch):
+    """The fp64 FMA probe of `--peaks` (8 independent chains per thread, 3 warm-up + 10 timed launches, best),
+    run inside this bench run so that the fp64 roofline entries divide by a peak of the same box and clocks."""
+    try:
+        from paper_1605_03262_b200 import binding
+        sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+        out = torch.empty(sms * 4096, dtype=torch.float64, device="cuda")
+        sp = torch.cuda.current_stream().cuda_stream
+        flops = [0]
+        for _ in range(3):
+            flops[0] = binding.peak_dfma(out, 1 << 16, sp)
+        torch.cuda.synchronize()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(11)]
+        ev[0].record()
+        for i in range(10):
+            binding.peak_dfma(out, 1 << 16, sp)
+            ev[i + 1].record()
+        torch.cuda.synchronize()
+        best = min(ev[i].elapsed_time(ev[i + 1]) for i in range(10))
+        _FP64_PEAK["tflops"] = flops[0] / best / 1e9
+        _FP64_PEAK["source"] = "fp64 FMA probe of the tools library, measured in this run (best of 10 launches)"
+    except Exception as e:      # the probe is a helper, not the product: fall back to the recorded figure
+        _FP64_PEAK["source"] += " (probe failed: %s)" % type(e).__name__
 
 
 def measured_peaks():
@@ -262,7 +295,7 @@ def run_peaks():
     torch.cuda.set_device(0)
     sp = torch.cuda.current_stream().cuda_stream
     buf = torch.empty(1 << 29, dtype=torch.float64, device="cuda")          # 4 GiB, far beyond L2
-    out = torch.empty(148 * 4096, dtype=torch.float64, device="cuda")
+    out = torch.empty(torch.cuda.get_device_properties(0).multi_processor_count * 4096, dtype=torch.float64, device="cuda")
 
     def timed(fn):
         for _ in range(3):
@@ -293,6 +326,12 @@ def run_peaks():
                       "hbm_copy_gbs": peak, "hbm_copy_source": src}))
 
 
+def rates_buffers(torch, pj, n):
+    """the four outputs of pyjac_eval_rates (R_f, R_r, c_i [n][N_reac], wdot [n][N_sp]), allocated once"""
+    return {k: torch.empty((n, pj.ns if k == "wdot" else pj.nr), dtype=torch.float64, device="cuda")
+            for k in ("rf", "rr", "cmod", "wdot")}
+
+
 def run_ncu_target(spec: str):
     """CFG:KERNEL:N[:SHAPE] -- three launches (two warm-up) of one kernel on the first N states of a configuration and
     nothing else: what `ncu --set full -s 2 -c 1` wraps for the captures under profiles/."""
@@ -313,10 +352,12 @@ def run_ncu_target(spec: str):
     dT, dP, dY = (torch.from_numpy(a).cuda() for a in (T, P, Y))
     ld = m.n_species + 1
     out = torch.empty((n, ld * ld if kernel in ("jacobian", "jacobian_fd") else ld), dtype=torch.float64, device="cuda")
+    rates_out = rates_buffers(torch, pj, n)
     fn = {"jacobian": lambda: pj.eval_jacobian(dT, dP, dY, out=out),
           "jacobian_fd": lambda: pj.eval_jacobian_fd(dT, dP, dY, out=out, chunk_states=256),
           "dydt": lambda: pj.eval_dydt(dT, dP, dY, out=out),
-          "rates": lambda: pj.eval_rates(dT, dP, dY, want=("wdot",))}[kernel]
+          "rates": lambda: pj.eval_rates(dT, dP, dY, out=rates_out),
+          "rates_wdot": lambda: pj.eval_rates(dT, dP, dY, out={"wdot": rates_out["wdot"]})}[kernel]
     total, per = time_gpu(pj, torch, dT, dP, dY, out, 1, 2, fn=fn)
     print(json.dumps({"workload": synth.CONFIGS[cfg].name, "kernel": kernel, "n_states": n, "launch_ms": per[0],
                       "launch_config": pj.launch_config(n)}))
@@ -404,7 +445,7 @@ def main():
                     help="measure the write-only store stream and the fp64 FMA rate (SURVEY.md 8(d)) and exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fd", action="store_true", help="skip the finite-difference / analytical time ratio")
-    ap.add_argument("--ncu-target", default=None, help="CFG:KERNEL:N (KERNEL = jacobian | dydt | rates): three launches, for ncu")
+    ap.add_argument("--ncu-target", default=None, help="CFG:KERNEL:N (KERNEL = jacobian | jacobian_fd | dydt | rates | rates_wdot): three launches, for ncu")
     ap.add_argument("--ncu-import", default=None, help="an .ncu-rep to turn into a row of profiles/r2_ncu_counters.csv")
     ap.add_argument("--ncu-label", default=None, help="WORKLOAD:KERNEL:N of the imported report")
     args = ap.parse_args()
@@ -461,10 +502,19 @@ def main():
     alg_bytes = algorithmic_bytes(c.n_species, r["per_launch"])
     achieved = alg_bytes / (launch_ms * 1e-3) / 1e9
     counters, counters_src = ncu_counters()
+    n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+    measure_fp64_peak(torch)
 
     def traffic_of(name, states):
+        """EXTRAPOLATED: DRAM bytes per state of the committed ncu capture (taken at fewer states, see
+        `traffic_capture_states`) times the states of this launch; lines still dirty in L2 when the captured kernel
+        ended are not in it, so it can sit a few per cent below the bytes the kernel stores"""
         c = counters.get(name, {}).get("jacobian")
         return None if not c else int(round(c["dram_bytes_per_state"] * states))
+
+    def capture_states(name):
+        c = counters.get(name, {}).get("jacobian")
+        return None if not c else c.get("n_states")
 
     def fp64_of(name, kernel, states, ms):
         """achieved fp64 FLOP/s of one launch from the counted DFMA / DADD / DMUL per state (ncu), against the
@@ -474,7 +524,7 @@ def main():
             return None
         tf = c["fp64_flop_per_state"] * states / (ms * 1e-3) / 1e12
         return {"bound": "alu", "achieved": tf, "peak": fp64_peak(), "unit": "TFLOP/s", "frac": tf / fp64_peak(),
-                "flop_per_state": c["fp64_flop_per_state"], "peak_source": "bench.py --peaks (profiles/r1_machine_peaks.md)"}
+                "flop_per_state": c["fp64_flop_per_state"], "peak_source": _FP64_PEAK["source"]}
 
     def lsu_of(name, kernel, states, ms, sm_mhz):
         """the pipe that binds the Jacobian kernel: L1TEX LSU data-pipe wavefronts (shared
@@ -483,13 +533,18 @@ def main():
         if not c or not sm_mhz:
             return None
         rate = c["lsu_wavefronts_per_state"] * states / (ms * 1e-3) / 1e9
-        peak = 148 * sm_mhz * 1e6 / 1e9
-        return {"bound": "lsu", "achieved": rate, "peak": peak, "unit": "Gwavefront/s", "frac": rate / peak,
+        peak = n_sm * sm_mhz * 1e6 / 1e9
+        return {"bound": "lsu", "diagnostic": True,
+                "note": "a diagnosis, not a roofline: the wavefront count is derived (shared-memory count scaled by the "
+                        "ratio of two utilisation figures of the same ncu report) and the peak is nominal, not measured",
+                "achieved": rate, "peak": peak, "unit": "Gwavefront/s", "frac": rate / peak,
                 "wavefronts_per_state": c["lsu_wavefronts_per_state"],
-                "peak_source": "one L1TEX data-pipe wavefront per SM and clock, 148 SMs at the SM clock sampled during the run"}
+                "peak_source": "one L1TEX data-pipe wavefront per SM and clock, %d SMs at the SM clock sampled during the run" % n_sm}
 
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic_of(c.name, r["per_launch"]), "traffic_source": counters_src,
+                "traffic_kind": "extrapolated from a smaller capture (per-state DRAM bytes x states of this launch)",
+                "traffic_capture_states": capture_states(c.name),
                 "peak_source": peak_src,
                 "kernel": "pyjac::eval_kernel<2 (Jacobian), S = %d states per CTA iteration>" % pj.launch_config(r["per_launch"])["states_per_cta"],
                 "algorithmic_bytes_per_launch": alg_bytes,
@@ -553,6 +608,12 @@ def main():
             torch.cuda.empty_cache()
         if per:
             line["per_config"] = per
+            # north_star names two target configurations: the other one (and the 360-species one) inside the
+            # headline's roofline object, with the same definition of `frac`
+            line["roofline"]["other_configs"] = {
+                k: {"launch_ms": v["launch_ms"], "states_per_launch": v["states_per_launch"],
+                    "achieved": v["roofline"]["achieved"], "frac": v["roofline"]["frac"], "value": v["value"]}
+                for k, v in per.items()}
         if args.sweep != "off":
             line["sweep_53sp"] = sweep(torch, args, fp64_of)
         if not args.no_fd:
@@ -591,6 +652,9 @@ def fd_ratio(torch):
         del jac, work
         torch.cuda.empty_cache()
     out["paper_gpu_ratio_range"] = [1.37, 2.73]
+    out["note"] = ("cost of THIS forward-difference path, not of the method: pyjac_eval_jacobian_fd writes N_sp perturbed "
+                   "copies of every state (N_sp^2 doubles) to HBM, reads them back through 1 + N_sp source-term "
+                   "evaluations and a difference kernel (csrc/fd.cu); not comparable with the paper's ratios")
     return out
 
 
@@ -634,15 +698,20 @@ def sweep(torch, args, fp64_of):
         steps = 10
         tj, _ = time_gpu(pj, torch, dT, dP, dY, out, steps, 3)
         td, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3, fn=lambda: pj.eval_dydt(dT, dP, dY, out=dy))
-        tr, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3,
-                         fn=lambda: pj.eval_rates(dT, dP, dY, want=("wdot",)))
+        ro = rates_buffers(torch, pj, n)
+        # all four outputs (8.2 KB per state for the rate arrays); the wdot-only figure beside it
+        tr, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3, fn=lambda: pj.eval_rates(dT, dP, dY, out=ro))
+        tw, _ = time_gpu(pj, torch, dT, dP, dY, None, steps, 3,
+                         fn=lambda: pj.eval_rates(dT, dP, dY, out={"wdot": ro["wdot"]}))
         name = synth.CONFIGS[1].name
         res.append({"n_states": n, "jacobian_states_per_s": n / (tj / steps * 1e-3),
                     "dydt_states_per_s": n / (td / steps * 1e-3), "rates_states_per_s": n / (tr / steps * 1e-3),
+                    "rates_outputs": "rf, rr, cmod, wdot (%d B per state)" % ((3 * pj.nr + pj.ns) * 8),
+                    "rates_wdot_only_states_per_s": n / (tw / steps * 1e-3),
                     "fp64": {"jacobian": fp64_of(name, "jacobian", n, tj / steps),
                              "dydt": fp64_of(name, "dydt", n, td / steps),
                              "rates": fp64_of(name, "rates", n, tr / steps)}})
-        del out, dy
+        del out, dy, ro
         torch.cuda.empty_cache()
     return res
 
