@@ -318,8 +318,24 @@ def run_peaks():
     def dfma():
         flops[0] = binding.peak_dfma(out, iters, sp)
     fbest, fmean = timed(dfma)
+    # the output path of a tile kernel: per-state tiles filled in shared memory, one bulk copy each (mode 0) or a read-back
+    # through the LSU pipe (mode 1); tile = one state's (N_s+1)^2 matrix of the 53- and 111-species mechanisms
+    tiles = {}
+    for ns, ctas_list in ((53, (1, 2, 4)), (111, (1, 2))):
+        td = (ns + 1) * (ns + 1)
+        nt = min(100_000, buf.numel() // td)
+        for mode in (0, 1):
+            for ctas in ctas_list:
+                tb, tm = timed(lambda: binding.peak_tile_store(buf, nt, td, mode, ctas, sp))
+                tiles["%dsp_%s_%dcta" % (ns, "bulk" if mode == 0 else "lds_stg", ctas)] = {
+                    "tile_bytes": td * 8, "tiles": nt, "ctas_per_sm": ctas, "best_gbs": nt * td * 8 / tb / 1e6,
+                    "mean_gbs": nt * td * 8 / tm / 1e6}
+    # the buffer must hold what the probe wrote: tile t, element i = t + i (checked on the last configuration run)
+    td = 112 * 112
+    chk = buf[: 3 * td].cpu()
+    tiles["last_run_verified"] = bool(chk[0] == 0.0 and chk[td - 1] == td - 1 and chk[td] == 1.0 and chk[3 * td - 1] == 2 + td - 1)
     peak, src = measured_peaks()
-    print(json.dumps({"store_stream": {"bytes": nbytes, "best_gbs": nbytes / best / 1e6, "mean_gbs": nbytes / mean / 1e6,
+    print(json.dumps({"tile_store": tiles, "store_stream": {"bytes": nbytes, "best_gbs": nbytes / best / 1e6, "mean_gbs": nbytes / mean / 1e6,
                                        "instruction": "st.global.cs.v2.f64"},
                       "fp64_fma": {"flops": flops[0], "best_tflops": flops[0] / fbest / 1e9, "mean_tflops": flops[0] / fmean / 1e9,
                                    "chains_per_thread": 8},

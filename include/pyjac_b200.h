@@ -158,6 +158,11 @@ typedef struct pyjac_launch_shape {
 int pyjac_mech_create_shaped(const pyjac_mech_desc *host_desc, int device,
                              const pyjac_launch_shape *shape, pyjac_mech **out);
 
+/* Why the last pyjac_mech_create / pyjac_mech_create_shaped call of THIS host thread failed: a static,
+ * never-NULL sentence naming the rule that was broken ("nu outside 1..3", "PLOG pressures must ascend",
+ * "threads per CTA must be ...", ...); "" after a call that succeeded. */
+const char *pyjac_mech_create_error(void);
+
 /* Frees the device tables.  NULL is a no-op returning PYJAC_OK. */
 int pyjac_mech_destroy(pyjac_mech *mech);
 

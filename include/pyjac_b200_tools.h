@@ -44,6 +44,16 @@ int pyjac_tools_pack_stats(const pyjac_mech_desc *host_desc, const pyjac_launch_
  *     148 * 2048 doubles at least; the thread count used is returned); flops = 2 * 8 * iters *
  *     *n_threads. */
 int pyjac_tools_peak_store_stream(double *buf, int64_t n_doubles, void *stream);
+/*   pyjac_tools_peak_tile_store: the output path of a kernel that assembles each state's Jacobian in
+ *     shared memory first.  n_tiles tiles of tile_doubles doubles (even; 8 tile_doubles a multiple of
+ *     16 bytes) are each written element by element with 8-byte shared-memory stores and then moved
+ *     to buf[t * tile_doubles ..) by mode 0: one cp.async.bulk.global.shared::cta per tile (bulk-copy
+ *     engine, two buffers per CTA so that a copy drains while the next tile is filled), mode 1: a
+ *     read-back with 16-byte shared loads and st.global.cs.v2.f64.  256 threads per CTA,
+ *     ctas_per_sm x SM count CTAs; bytes moved = 8 n_tiles tile_doubles.  PYJAC_ELIMIT if two tiles
+ *     exceed the shared memory of one CTA. */
+int pyjac_tools_peak_tile_store(double *buf, int64_t n_tiles, int32_t tile_doubles, int32_t mode,
+                                int32_t ctas_per_sm, void *stream);
 int pyjac_tools_peak_dfma(double *out, int64_t iters, int64_t *n_threads, void *stream);
 
 #ifdef __cplusplus

@@ -45,12 +45,14 @@ class LaunchShape(C.Structure):
                 ("p1_states", C.c_int32), ("stage_tables", C.c_int32), ("layout", C.c_int32)]
 
 
-EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_destroy", "pyjac_mech_trim", "pyjac_mech_sizes",
+EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_create_error", "pyjac_mech_destroy", "pyjac_mech_trim",
+           "pyjac_mech_sizes",
            "pyjac_eval_rates", "pyjac_eval_dydt", "pyjac_eval_jacobian", "pyjac_eval_jacobian_host",
            "pyjac_eval_dydt_host", "pyjac_eval_jvp", "pyjac_eval_jacobian_fd", "pyjac_fd_workspace_doubles",
            "pyjac_eval_jacobian_fd_static", "pyjac_fd_static_max_states", "pyjac_kernel_launches",
            "pyjac_jacobian_launch_config", "pyjac_strerror")
-TOOLS_EXPORTS = ("pyjac_tools_pack_stats", "pyjac_tools_peak_store_stream", "pyjac_tools_peak_dfma")
+TOOLS_EXPORTS = ("pyjac_tools_pack_stats", "pyjac_tools_peak_store_stream", "pyjac_tools_peak_tile_store",
+                 "pyjac_tools_peak_dfma")
 
 _lib = None
 _tools = None
@@ -89,8 +91,10 @@ def load_library(path: str | None = None):
     lib.pyjac_jacobian_launch_config.argtypes = [vp, i64] + [C.POINTER(i32)] * 5
     lib.pyjac_strerror.argtypes = [C.c_int]
     lib.pyjac_strerror.restype = C.c_char_p
+    lib.pyjac_mech_create_error.argtypes = []
+    lib.pyjac_mech_create_error.restype = C.c_char_p
     for name in EXPORTS:
-        if name not in ("pyjac_kernel_launches", "pyjac_strerror", "pyjac_fd_workspace_doubles",
+        if name not in ("pyjac_kernel_launches", "pyjac_strerror", "pyjac_mech_create_error", "pyjac_fd_workspace_doubles",
                         "pyjac_fd_static_max_states"):
             getattr(lib, name).restype = C.c_int
     if path is None:
@@ -111,6 +115,7 @@ def load_tools(path: str | None = None):
     lib.pyjac_tools_pack_stats.argtypes = [C.POINTER(MechDesc), C.POINTER(LaunchShape), C.POINTER(i64)]
     lib.pyjac_tools_peak_store_stream.argtypes = [vp, i64, vp]
     lib.pyjac_tools_peak_dfma.argtypes = [vp, i64, C.POINTER(i64), vp]
+    lib.pyjac_tools_peak_tile_store.argtypes = [vp, i64, C.c_int32, C.c_int32, C.c_int32, vp]
     for name in TOOLS_EXPORTS:
         getattr(lib, name).restype = C.c_int
     if path is None:
@@ -121,7 +126,11 @@ def load_tools(path: str | None = None):
 class PyJacError(RuntimeError):
     def __init__(self, code, what):
         self.code = code
-        msg = load_library().pyjac_strerror(code).decode()
+        lib = load_library()
+        msg = lib.pyjac_strerror(code).decode()
+        if what.startswith("pyjac_mech_create"):
+            why = lib.pyjac_mech_create_error().decode()
+            msg = msg + (": " + why if why else "")
         super().__init__("%s failed: %s (%d)" % (what, msg, code))
 
 
@@ -184,6 +193,15 @@ def peak_store_stream(buf, stream_ptr):
     """Enqueues one write-only pass over the CUDA float64 tensor `buf` (pyjac_tools_peak_store_stream)."""
     _check(load_tools().pyjac_tools_peak_store_stream(buf.data_ptr(), int(buf.numel()), stream_ptr),
            "pyjac_tools_peak_store_stream")
+
+
+def peak_tile_store(buf, n_tiles, tile_doubles, mode, ctas_per_sm, stream_ptr):
+    """Enqueues the tile-store probe on the CUDA float64 tensor `buf` (pyjac_tools_peak_tile_store): mode 0 one bulk
+    copy per tile, mode 1 shared-memory read-back and streaming stores."""
+    if buf.numel() < int(n_tiles) * int(tile_doubles):
+        raise ValueError("buf is too small for n_tiles tiles")
+    _check(load_tools().pyjac_tools_peak_tile_store(buf.data_ptr(), int(n_tiles), int(tile_doubles), int(mode),
+                                                    int(ctas_per_sm), stream_ptr), "pyjac_tools_peak_tile_store")
 
 
 def peak_dfma(out, iters, stream_ptr):

@@ -41,6 +41,9 @@ namespace {
 
 std::atomic<long long> g_launches{0};
 
+// reason of the last failed pyjac_mech_create* on this thread (static strings only), "" after a success
+thread_local const char *t_last_error = "";
+
 // preferred shared-memory carve-out (percent) set so far per (device, kernel function); see pyjac_mech_create_shaped
 std::mutex g_carveout_mutex;
 std::map<std::pair<int, const void *>, int> g_carveout;
@@ -102,23 +105,25 @@ int pyjac_mech_create(const pyjac_mech_desc *d, int device, pyjac_mech **out)
 
 int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_launch_shape *shape, pyjac_mech **out)
 {
-    if (!out) return PYJAC_EINVAL;
+    t_last_error = "";
+    if (!out) { t_last_error = "the output handle pointer is NULL"; return PYJAC_EINVAL; }
     *out = nullptr;
     // validate and pack first (no CUDA call yet) with the architecture's shared-memory size; the
     // real device's limit is checked below
     HostPack hp;
     const char *why = nullptr;
     int rc = pack_mechanism(d, hp, hints_from_shape(shape, 227 * 1024), &why);
-    if (rc != PYJAC_OK) return rc;
+    if (rc != PYJAC_OK) { t_last_error = why ? why : ""; return rc; }
     int prev = -1;
     cudaDeviceProp prop{};
     if (cudaGetDevice(&prev) != cudaSuccess || cudaSetDevice(device) != cudaSuccess ||
         cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
         cudaGetLastError();
+        t_last_error = "no usable CUDA device with this index";
         return PYJAC_ECUDA;
     }
     pyjac_mech *m = new (std::nothrow) pyjac_mech();
-    if (!m) { cudaSetDevice(prev); return PYJAC_ENOMEM; }
+    if (!m) { cudaSetDevice(prev); t_last_error = "host allocation failed"; return PYJAC_ENOMEM; }
     m->device = device;
     m->ns = hp.ns;
     m->nr = hp.nr;
@@ -157,6 +162,7 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
     } catch (...) {
         delete m;
         cudaSetDevice(prev);
+        t_last_error = "host allocation failed";
         return PYJAC_ENOMEM;
     }
     rc = PYJAC_OK;
@@ -209,6 +215,9 @@ int pyjac_mech_create_shaped(const pyjac_mech_desc *d, int device, const pyjac_l
         cudaGetLastError();
         if (m->blob) cudaFree(m->blob);
         delete m;
+        t_last_error = rc == PYJAC_ELIMIT ? "the per-state tables of this launch shape exceed the device's shared memory per CTA"
+                       : rc == PYJAC_ENOMEM ? "device allocation of the tables failed"
+                                            : "a CUDA call failed while uploading the tables or configuring the kernels";
         return rc;
     }
     *out = m;
@@ -312,6 +321,8 @@ int pyjac_jacobian_launch_config(const pyjac_mech *m, int64_t n, int32_t *thread
     if (grid) *grid = (int32_t)(blocks < cap ? blocks : cap);
     return PYJAC_OK;
 }
+
+const char *pyjac_mech_create_error(void) { return t_last_error; }
 
 const char *pyjac_strerror(int code)
 {

@@ -1,5 +1,5 @@
 // tools.cu -- libpyjac_b200_tools.so: bench / test helpers of include/pyjac_b200_tools.h.  Not on the
-// evaluation path: table statistics (host only) and the two machine-peak probes.
+// evaluation path: table statistics (host only) and the machine-peak probes.
 #include <cuda_runtime.h>
 
 #include "device_mech.h"
@@ -26,6 +26,47 @@ __global__ void __launch_bounds__(256) peak_dfma_kernel(double *out, long long i
         a4 = fma(a4, x, y); a5 = fma(a5, x, y); a6 = fma(a6, x, y); a7 = fma(a7, x, y);
     }
     out[(long long)blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+// Tile probe: what a Jacobian kernel that assembles one state's matrix in shared memory and hands it to the bulk-copy
+// engine would do for its output.  Per tile of `tile_doubles` doubles (one state's (N_s+1)^2 matrix): every element is
+// written once with an 8-byte shared-memory store (MODE 0, 1: one STS.64 per element and lane, as a lane that owns a cell
+// would), then either ONE cp.async.bulk.global.shared::cta of the whole tile issued by one thread (MODE 0: no load / store
+// instruction of the SM touches the bytes again) or a read-back with LDS.128 and 16-byte streaming stores (MODE 1: the
+// round-1 tile kernel's way, twice through the LSU data pipe).  Two tile buffers per CTA: the copy of tile t drains while
+// tile t + 1 is filled.
+template <int MODE>
+__global__ void __launch_bounds__(256) peak_tile_store_kernel(double *out, long long n_tiles, int tile_doubles)
+{
+    extern __shared__ __align__(128) double tile_smem[];
+    int buf = 0;
+    for (long long t = blockIdx.x; t < n_tiles; t += gridDim.x, buf ^= 1) {
+        double *b = tile_smem + (size_t)buf * tile_doubles;
+        if (MODE == 0) {
+            // this buffer went to the copy engine two tiles ago: wait until the engine has read it
+            if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < tile_doubles; i += blockDim.x) b[i] = (double)(t + i);
+        if (MODE == 0) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        double *g = out + t * (long long)tile_doubles;
+        if (MODE == 0) {
+            if (threadIdx.x == 0) {
+                const unsigned src = (unsigned)__cvta_generic_to_shared(b);
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(g), "r"(src),
+                             "r"(tile_doubles * 8)
+                             : "memory");
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+        } else {
+            for (int i = threadIdx.x; i < tile_doubles / 2; i += blockDim.x) {
+                const double2 v = reinterpret_cast<const double2 *>(b)[i];
+                asm volatile("st.global.cs.v2.f64 [%0], {%1, %2};" ::"l"(g + 2 * i), "d"(v.x), "d"(v.y) : "memory");
+            }
+        }
+    }
+    if (MODE == 0 && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 }  // namespace
@@ -60,6 +101,25 @@ int pyjac_tools_peak_store_stream(double *buf, int64_t n_doubles, void *stream)
         cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
         return PYJAC_ECUDA;
     peak_store_kernel<<<n_sm * 8, 256, 0, (cudaStream_t)stream>>>(buf, n_doubles / 2);
+    return cudaGetLastError() == cudaSuccess ? PYJAC_OK : PYJAC_ECUDA;
+}
+
+int pyjac_tools_peak_tile_store(double *buf, int64_t n_tiles, int32_t tile_doubles, int32_t mode, int32_t ctas_per_sm,
+                                void *stream)
+{
+    if (!buf || n_tiles < 1 || tile_doubles < 2 || (tile_doubles & 1) || (reinterpret_cast<uintptr_t>(buf) & 15) ||
+        (mode != 0 && mode != 1) || ctas_per_sm < 1 || ctas_per_sm > 8)
+        return PYJAC_EINVAL;
+    const size_t smem = (size_t)2 * tile_doubles * sizeof(double);
+    int dev = 0, n_sm = 0, optin = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        return PYJAC_ECUDA;
+    if (smem > (size_t)optin) return PYJAC_ELIMIT;
+    auto k = mode == 0 ? peak_tile_store_kernel<0> : peak_tile_store_kernel<1>;
+    if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return PYJAC_ECUDA;
+    k<<<n_sm * ctas_per_sm, 256, smem, (cudaStream_t)stream>>>(buf, n_tiles, tile_doubles);
     return cudaGetLastError() == cudaSuccess ? PYJAC_OK : PYJAC_ECUDA;
 }
 

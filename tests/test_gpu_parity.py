@@ -445,6 +445,25 @@ def test_host_variant_keeps_a_bounded_footprint_and_trim_returns_it(torch, PyJac
     pj.trim()                                                      # nothing to free: still fine
 
 
+def test_tile_store_probe_writes_every_element(torch, PyJac):
+    """Helper library, not the product: the tile-store probe behind profiles/r3_tile_store_probe.md (per-state tiles
+    filled in shared memory, then one cp.async.bulk per tile, or a read-back and streaming stores) must write tile t,
+    element i = t + i for every tile, including counts that are no multiple of the grid and both tile sizes."""
+    from paper_1605_03262_b200 import binding
+    sp = torch.cuda.current_stream().cuda_stream
+    for td, nt in ((54 * 54, 1000), (112 * 112, 301), (14 * 14, 5)):
+        want = (torch.arange(nt, dtype=torch.float64, device="cuda")[:, None]
+                + torch.arange(td, dtype=torch.float64, device="cuda")[None, :])
+        for mode in (0, 1):
+            for ctas in (1, 2):
+                buf = torch.full((nt + 1, td), -1.0, dtype=torch.float64, device="cuda")
+                binding.peak_tile_store(buf, nt, td, mode, ctas, sp)
+                torch.cuda.synchronize()
+                assert torch.equal(buf[:nt], want) and bool((buf[nt] == -1.0).all())
+    with pytest.raises(binding.PyJacError):
+        binding.peak_tile_store(torch.empty(2 * 127 * 127 + 1, dtype=torch.float64, device="cuda")[1:], 2, 127 * 127 - 1, 0, 1, sp)
+
+
 # ---------------------------------------------------------------------------------- launch shapes
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg,n,shape", [

@@ -136,6 +136,7 @@ def test_validation_rejects_bad_descriptions(lib, what):
         i = int(np.where(m.rxn_type == THIRD_BODY)[0][0])
         m.tb_species = m.tb_species.copy(); m.tb_species[i] = m.n_species
     assert _create(lib, m) == binding.PYJAC_EINVAL
+    assert len(lib.pyjac_mech_create_error()) > 8          # the broken rule is named, not just the code
 
 
 def test_binding_refuses_cpu_tensors():
