@@ -348,6 +348,47 @@ def rates_buffers(torch, pj, n):
             for k in ("rf", "rr", "cmod", "wdot")}
 
 
+def run_gather_probe(n_states: int = 100_000):
+    """profiles/r3_gather_probe.md: the timing prototype of unpadded, length-balanced gathers into a per-state tile +
+    one bulk copy per state (tools library, real cell lists of the 53- and 111-species mechanisms, stand-in values),
+    for several shapes; every launch's output is compared with the expected tile."""
+    import numpy as np
+    import torch
+    from paper_1605_03262_b200 import build, binding, synth
+    build.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    sp = torch.cuda.current_stream().cuda_stream
+    res = []
+    for cfg, shapes in ((1, ((3, 512, 1, 1), (2, 512, 1, 2), (2, 256, 2, 1), (1, 256, 2, 2), (1, 128, 4, 1), (1, 256, 3, 1))),
+                        (2, ((1, 512, 1, 1), (1, 256, 1, 1)))):
+        m = synth.make_mechanism(cfg)
+        ld = m.n_species + 1
+        n = min(n_states, (3 << 30) // (ld * ld * 8))
+        out = torch.empty((n, ld * ld), dtype=torch.float64, device="cuda")
+        for S, threads, ctas, nbuf in shapes:
+            out.fill_(-1.0)
+            try:
+                r = binding.gather_probe(m, out, n, S, threads, ctas, nbuf, 10, sp)
+            except binding.PyJacError as e:
+                res.append({"workload": synth.CONFIGS[cfg].name, "S": S, "threads": threads, "ctas_per_sm": ctas, "n_buf": nbuf,
+                            "error": str(e)})
+                continue
+            torch.cuda.synchronize()
+            exp = torch.from_numpy(r.pop("expected")).cuda()
+            err = float(((out - exp[None, :]).abs() / exp.abs().clamp_min(1e-300)).max())
+            alg = algorithmic_bytes(m.n_species, n)
+            res.append({"workload": synth.CONFIGS[cfg].name, "n_states": n, "S": S, "threads": threads, "ctas_per_sm": ctas,
+                        "n_buf": nbuf, **r, "max_rel_err_vs_expected": err,
+                        "states_per_s": n / (r["ms_best"] * 1e-3), "gbs": alg / (r["ms_best"] * 1e-3) / 1e9})
+        del out
+        torch.cuda.empty_cache()
+    peak, src = measured_peaks()
+    print(json.dumps({"gather_probe": res, "hbm_copy_gbs": peak, "hbm_copy_source": src,
+                      "note": "timing prototype (stand-in values, real cell lists); not an evaluation"}))
+
+
 def run_ncu_target(spec: str):
     """CFG:KERNEL:N[:SHAPE] -- three launches (two warm-up) of one kernel on the first N states of a configuration and
     nothing else: what `ncu --set full -s 2 -c 1` wraps for the captures under profiles/."""
@@ -459,6 +500,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--peaks", action="store_true",
                     help="measure the write-only store stream and the fp64 FMA rate (SURVEY.md 8(d)) and exit")
+    ap.add_argument("--gather-probe", action="store_true",
+                    help="run the gather timing prototype of the tools library (profiles/r3_gather_probe.md) and exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fd", action="store_true", help="skip the finite-difference / analytical time ratio")
     ap.add_argument("--ncu-target", default=None, help="CFG:KERNEL:N (KERNEL = jacobian | jacobian_fd | dydt | rates | rates_wdot): three launches, for ncu")
@@ -476,6 +519,9 @@ def main():
         return
     if args.peaks:
         run_peaks()
+        return
+    if args.gather_probe:
+        run_gather_probe()
         return
     args.warmup = max(3, args.warmup)
 

@@ -56,6 +56,24 @@ int pyjac_tools_peak_tile_store(double *buf, int64_t n_tiles, int32_t tile_doubl
                                 int32_t ctas_per_sm, void *stream);
 int pyjac_tools_peak_dfma(double *out, int64_t iters, int64_t *n_threads, void *stream);
 
+/* Gather probe -- a TIMING PROTOTYPE, not an evaluation: the output half of a Jacobian kernel whose
+ * gathers carry no padding, on the REAL contribution lists of the mechanism's Jacobian cells but with
+ * stand-in values for the per-reaction terms they sum.  Per batch of S (1..3) states a CTA writes the
+ * rank-one part of every cell to a per-state tile in shared memory, adds the cells' sparse sums (cells
+ * sorted by list length, 32 cells of nearly equal length per warp chunk, one shared-memory load per
+ * entry and state) and moves each tile to out[state][(N_sp+1)^2] with one cp.async.bulk; n_buf = 2
+ * tile sets overlap the copies with the next batch.  Builds and uploads its tables, runs 2 warm-up and
+ * `reps` timed launches (CUDA events on `stream`), frees the tables.  Outputs: ms_best / ms_mean per
+ * launch; expected_host[(N_sp+1)^2] = the tile every state must hold (the stand-in values do not
+ * depend on the state) for the caller to compare with `out` (DEVICE pointer, n_states tiles);
+ * stats[8] = list entries, entries with chunk padding, chunks, E elements per state, shared memory
+ * per CTA in bytes, non-empty cells, cells, grid.  PYJAC_ELIMIT if the shape does not fit shared
+ * memory; allocates (probe only). */
+int pyjac_tools_gather_probe(const pyjac_mech_desc *host_desc, int32_t S, int32_t threads,
+                             int32_t ctas_per_sm, int32_t n_buf, int64_t n_states, double *out,
+                             double *expected_host, int64_t *stats, int32_t reps, float *ms_best,
+                             float *ms_mean, void *stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -52,7 +52,7 @@ EXPORTS = ("pyjac_mech_create", "pyjac_mech_create_shaped", "pyjac_mech_create_e
            "pyjac_eval_jacobian_fd_static", "pyjac_fd_static_max_states", "pyjac_kernel_launches",
            "pyjac_jacobian_launch_config", "pyjac_strerror")
 TOOLS_EXPORTS = ("pyjac_tools_pack_stats", "pyjac_tools_peak_store_stream", "pyjac_tools_peak_tile_store",
-                 "pyjac_tools_peak_dfma")
+                 "pyjac_tools_peak_dfma", "pyjac_tools_gather_probe")
 
 _lib = None
 _tools = None
@@ -116,6 +116,8 @@ def load_tools(path: str | None = None):
     lib.pyjac_tools_peak_store_stream.argtypes = [vp, i64, vp]
     lib.pyjac_tools_peak_dfma.argtypes = [vp, i64, C.POINTER(i64), vp]
     lib.pyjac_tools_peak_tile_store.argtypes = [vp, i64, C.c_int32, C.c_int32, C.c_int32, vp]
+    lib.pyjac_tools_gather_probe.argtypes = [C.POINTER(MechDesc), C.c_int32, C.c_int32, C.c_int32, C.c_int32, i64, vp,
+                                             _pd, C.POINTER(i64), C.c_int32, C.POINTER(C.c_float), C.POINTER(C.c_float), vp]
     for name in TOOLS_EXPORTS:
         getattr(lib, name).restype = C.c_int
     if path is None:
@@ -202,6 +204,24 @@ def peak_tile_store(buf, n_tiles, tile_doubles, mode, ctas_per_sm, stream_ptr):
         raise ValueError("buf is too small for n_tiles tiles")
     _check(load_tools().pyjac_tools_peak_tile_store(buf.data_ptr(), int(n_tiles), int(tile_doubles), int(mode),
                                                     int(ctas_per_sm), stream_ptr), "pyjac_tools_peak_tile_store")
+
+
+def gather_probe(mech: Mechanism, out, n_states, S, threads, ctas_per_sm, n_buf, reps, stream_ptr) -> dict:
+    """Runs the gather probe of the tools library (pyjac_tools_gather_probe: unpadded, length-balanced gathers into a
+    per-state shared-memory tile + one bulk copy per state; timing prototype on the mechanism's real cell lists) and
+    returns its timings, table statistics and the expected tile."""
+    d, keep = mech_desc(mech)
+    ld = mech.n_species + 1
+    if out.numel() < int(n_states) * ld * ld:
+        raise ValueError("out is too small")
+    expected = np.empty(ld * ld)
+    stats = (C.c_int64 * 8)()
+    best, mean = C.c_float(), C.c_float()
+    _check(load_tools().pyjac_tools_gather_probe(C.byref(d), int(S), int(threads), int(ctas_per_sm), int(n_buf), int(n_states),
+                                                 out.data_ptr(), expected.ctypes.data_as(_pd), stats, int(reps),
+                                                 C.byref(best), C.byref(mean), stream_ptr), "pyjac_tools_gather_probe")
+    names = ("entries", "entries_padded", "chunks", "e_elements", "smem_bytes", "nonempty_cells", "cells", "grid")
+    return dict(ms_best=best.value, ms_mean=mean.value, expected=expected, **dict(zip(names, [int(v) for v in stats])))
 
 
 def peak_dfma(out, iters, stream_ptr):

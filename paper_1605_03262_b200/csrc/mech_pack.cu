@@ -532,6 +532,7 @@ static void pack_impl(const pyjac_mech_desc *d, HostPack &o, const ShapeHints &h
         }
     }
     for (int r = 1; r < ld; ++r) cell[(size_t)r].push_back({(uint32_t)(eTc + r), 1});
+    if (hints.keep_cells == 1) o.raw_cells = cell;
 
     // ---- entries after splitting coefficients beyond +-8 (device_mech.h); E indices, not yet offsets
     auto split = [&](const std::vector<std::pair<uint32_t, int>> &ent, std::vector<std::pair<uint32_t, int>> &w) {

@@ -1,6 +1,7 @@
 // mech_pack.h -- host-side packing of a pyjac_mech_desc into the tables of device_mech.h.
 #pragma once
 #include <cstdint>
+#include <utility>
 #include <vector>
 
 #include "../../include/pyjac_b200.h"
@@ -43,6 +44,9 @@ struct HostPack {
     // the shared-memory footprint was sized for
     int S = 1, threads = 128, ctas_target = 1;
     bool stage = false;                   // gather tables staged in shared memory
+    // only with ShapeHints::keep_cells: per flat cell index r + c * ld the (E index, integer coefficient) pairs summed into
+    // the cell, before any splitting or piecewise summing (the gather probe of tools.cu deals them out its own way)
+    std::vector<std::vector<std::pair<uint32_t, int>>> raw_cells;
     // statistics (pyjac_pack_stats)
     long long n_cell_entries = 0, n_cells = 0, n_heavy_cells = 0, n_heavy_pieces = 0, n_a_steps = 0, n_b_steps = 0;
     long long n_plain_chunks = 0;
@@ -63,6 +67,7 @@ struct ShapeHints {
     int p1_states = 0;  // states per work item of the fast reaction path (0: all S)
     int stage = 0;      // 1: copy the gather tables of phases A and B to shared memory once per CTA
     int layout = 0;     // 2: keep the s' values in allocation order (no bank-aware layout of E)
+    int keep_cells = 0; // 1: also return the raw contribution lists of the Jacobian cells (HostPack::raw_cells; probes only)
 };
 
 // The hints of an explicit launch shape (NULL: all zeros = choose); `smem_optin` = the device's opt-in

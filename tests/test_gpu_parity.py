@@ -464,6 +464,27 @@ def test_tile_store_probe_writes_every_element(torch, PyJac):
         binding.peak_tile_store(torch.empty(2 * 127 * 127 + 1, dtype=torch.float64, device="cuda")[1:], 2, 127 * 127 - 1, 0, 1, sp)
 
 
+def test_gather_probe_sums_the_real_cell_lists(torch, PyJac):
+    """Helper library, not the product: the gather timing prototype behind profiles/r3_gather_probe.md must really sum
+    the mechanism's cell lists (its timing means nothing otherwise): every state's tile equals the tile the host
+    computes from the same lists and stand-in values, for every S, both buffer counts and a ragged last batch."""
+    from paper_1605_03262_b200 import binding
+    sp = torch.cuda.current_stream().cuda_stream
+    for cfg, n in ((0, 1000), (1, 500)):
+        m = synth.make_mechanism(cfg)
+        ld = m.n_species + 1
+        st0 = binding.pack_stats(m)
+        for S, threads, ctas, nbuf in ((1, 128, 2, 2), (2, 256, 1, 2), (3, 512, 1, 1), (3, 96, 1, 2)):
+            out = torch.full((n + 1, ld * ld), -1.0, dtype=torch.float64, device="cuda")
+            r = binding.gather_probe(m, out, n, S, threads, ctas, nbuf, 1, sp)
+            torch.cuda.synchronize()
+            exp = torch.from_numpy(r["expected"]).cuda()
+            assert bool(((out[:n] - exp[None, :]).abs() <= 1e-13 * exp.abs().max()).all())
+            assert bool((out[n] == -1.0).all())
+            assert r["cells"] == ld * ld and r["nonempty_cells"] == st0["cells"] and r["entries"] <= r["entries_padded"]
+            assert r["entries_padded"] <= 1.25 * r["entries"] + 32 * 16          # sorted by length: little padding
+
+
 # ---------------------------------------------------------------------------------- launch shapes
 @pytest.mark.gpu
 @pytest.mark.parametrize("cfg,n,shape", [
