@@ -693,6 +693,45 @@ def test_two_live_handles_share_a_kernel(torch, PyJac):
 
 
 @pytest.mark.gpu
+def test_later_handle_does_not_take_shared_memory_from_an_earlier_one(torch, PyJac):
+    """the preferred shared-memory carve-out is an attribute of the kernel FUNCTION, which every handle
+    of the same S shares.  The 53-species handle needs ~90 % of the SM's memory as shared memory for its two resident
+    CTAs; the 13-species handle created after it would ask for a few per cent.  The library keeps the largest value
+    ever asked for, so the first handle still runs with the CTAs per SM its grid was sized for: same launch time
+    (a drop from two resident CTAs to one costs far more than the 15 % allowed here) and the same bits."""
+    big, small = synth.make_mechanism(1), synth.make_mechanism(0)
+    T, P, Y = synth.config_states(1, 30_000)
+    dT, dP, dY = dev(torch, T, P, Y)
+    pj_big = PyJac(big)
+    out = torch.empty((len(T), (big.n_species + 1) ** 2), dtype=torch.float64, device="cuda")
+
+    def launch_ms():
+        for _ in range(3):
+            pj_big.eval_jacobian(dT, dP, dY, out=out)
+        torch.cuda.synchronize()
+        times = []
+        for _ in range(7):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            pj_big.eval_jacobian(dT, dP, dY, out=out)
+            b.record()
+            torch.cuda.synchronize()
+            times.append(a.elapsed_time(b))
+        return sorted(times)[3]
+
+    before = launch_ms()
+    J0 = out.clone()
+    cfg_before = pj_big.launch_config(len(T))
+    pj_small = PyJac(small)
+    assert pj_small.launch_config(64)["states_per_cta"] == cfg_before["states_per_cta"]      # the same kernel function
+    Ts, Ps, Ys = synth.config_states(0, 256)
+    pj_small.eval_jacobian(*dev(torch, Ts, Ps, Ys))
+    after = launch_ms()
+    assert torch.equal(out, J0)
+    assert after <= 1.15 * before, (before, after)
+
+
+@pytest.mark.gpu
 def test_one_handle_from_two_host_threads(torch, PyJac):
     """Evaluation on a handle is re-entrant (the paper's complaint about TChem): two host
     threads evaluate on the same handle at once, each on its own stream, device-pointer and host-buffer
