@@ -188,6 +188,35 @@ def test_layout_search_lowers_the_modelled_bank_conflicts():
             assert on[k] == off[k]                      # a permutation: nothing else changes
 
 
+def test_gather_probe_tables_cover_every_cell_list():
+    """Helper library, host half of the gather timing prototype (profiles/r3_gather_probe.md): its chunk tables are built
+    before any CUDA call, so without a GPU the call ends with PYJAC_ECUDA but has already reported what it built -- every
+    entry of every non-empty cell list (the same counts pyjac_tools_pack_stats reports), dealt into chunks of 32 cells
+    of nearly equal length (little padding), and a shared-memory size that grows with S and the tile sets."""
+    tools = binding.load_tools()
+    for cfg in (0, 1, 2):
+        m = synth.make_mechanism(cfg)
+        d, keep = binding.mech_desc(m)
+        ld = m.n_species + 1
+        st0 = binding.pack_stats(m)
+        seen = []
+        for S, nbuf in ((1, 1), (3, 2)):
+            exp = np.full(ld * ld, np.nan)
+            stats = (C.c_int64 * 8)()
+            a, b = C.c_float(), C.c_float()
+            rc = tools.pyjac_tools_gather_probe(C.byref(d), S, 256, 1, nbuf, 100, C.c_void_p(16), exp.ctypes.data_as(binding._pd),
+                                                stats, 1, C.byref(a), C.byref(b), None)
+            assert rc in ((binding.PYJAC_OK, binding.PYJAC_ELIMIT) if _has_gpu() else (binding.PYJAC_ECUDA,))
+            entries, padded, chunks, n_e, smem, nonempty, cells, _ = list(stats)
+            assert cells == ld * ld and nonempty == st0["cells"] and entries == st0["cell_entries"] and n_e == st0["e_elements"]
+            assert chunks == (nonempty + 31) // 32 and entries <= padded <= 1.25 * entries + 32 * 16
+            assert smem == (((n_e * S + 15) // 16 * 16) + nbuf * S * cells) * 8
+            assert np.all(np.isfinite(exp))                       # the expected tile was filled for every cell
+            seen.append(exp.copy())
+        assert np.array_equal(seen[0], seen[1])                   # it does not depend on the launch shape
+    assert tools.pyjac_tools_gather_probe(None, 1, 256, 1, 1, 1, None, None, None, 1, None, None, None) == binding.PYJAC_EINVAL
+
+
 def test_launch_shape_validation():
     m = synth.make_mechanism(0)
     for bad in (dict(states_per_cta=5), dict(threads=100), dict(threads=1024), dict(ctas_per_sm=9),
