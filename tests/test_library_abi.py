@@ -200,11 +200,16 @@ def test_gather_probe_tables_cover_every_cell_list():
         ld = m.n_species + 1
         st0 = binding.pack_stats(m)
         seen = []
+        out_ptr, out_keep = C.c_void_p(16), None                  # never dereferenced without a device
+        if _has_gpu():                                            # with one the probe really runs: give it real memory
+            import torch
+            out_keep = torch.empty(100 * ld * ld, dtype=torch.float64, device="cuda")
+            out_ptr = C.c_void_p(out_keep.data_ptr())
         for S, nbuf in ((1, 1), (3, 2)):
             exp = np.full(ld * ld, np.nan)
             stats = (C.c_int64 * 8)()
             a, b = C.c_float(), C.c_float()
-            rc = tools.pyjac_tools_gather_probe(C.byref(d), S, 256, 1, nbuf, 100, C.c_void_p(16), exp.ctypes.data_as(binding._pd),
+            rc = tools.pyjac_tools_gather_probe(C.byref(d), S, 256, 1, nbuf, 100, out_ptr, exp.ctypes.data_as(binding._pd),
                                                 stats, 1, C.byref(a), C.byref(b), None)
             assert rc in ((binding.PYJAC_OK, binding.PYJAC_ELIMIT) if _has_gpu() else (binding.PYJAC_ECUDA,))
             entries, padded, chunks, n_e, smem, nonempty, cells, _ = list(stats)
